@@ -42,8 +42,8 @@ def lib():
         L.orc_delay_index.restype = C.c_int
         L.orc_delay_index.argtypes = [C.c_double, C.c_double, C.c_double]
         L.orc_philox4x32_10.argtypes = [C.POINTER(C.c_uint), C.POINTER(C.c_uint), C.POINTER(C.c_uint)]
-        L.orc_uniform24.restype = C.c_double
-        L.orc_uniform24.argtypes = [C.c_uint]
+        L.orc_uniform23.restype = C.c_double
+        L.orc_uniform23.argtypes = [C.c_uint]
         L.orc_normal.restype = C.c_double
         L.orc_normal.argtypes = [C.c_ulonglong, C.c_longlong, C.c_int, C.c_longlong]
         L.orc_tf.argtypes = [_dp, C.c_int, C.c_double, C.c_double, C.c_double, _dp, _dp]
@@ -98,8 +98,8 @@ def philox4x32_10(ctr, key):
     return tuple(int(x) for x in o)
 
 
-def uniform24(x):
-    return lib().orc_uniform24(x)
+def uniform23(x):
+    return lib().orc_uniform23(x)
 
 
 def normal(seed, sim, region, step):

@@ -180,7 +180,9 @@ inline void philox4x32_10(const uint32_t ctr[4], const uint32_t key[2], uint32_t
   }
   out[0] = c0; out[1] = c1; out[2] = c2; out[3] = c3;
 }
-inline double u24(uint32_t x) { return ((double)(x >> 8) + 0.5) * (1.0 / 16777216.0); }
+// u(x) = ((x >> 9) + 0.5) * 2^-23: (2k+1)/2^24 with k < 2^23 is exact in FP32 and FP64 (A12 as
+// amended in DESIGN.md: 24 bits + 0.5 would need a 25-bit significand).
+inline double u23(uint32_t x) { return ((double)(x >> 9) + 0.5) * (1.0 / 8388608.0); }
 
 // xi_{s,k,n}: counter = (q_lo, q_hi, region, sim), q = n/4; key = (seed_lo, seed_hi)
 double normal_variate(uint64_t seed, int64_t sim, int32_t region, int64_t step) {
@@ -192,8 +194,8 @@ double normal_variate(uint64_t seed, int64_t sim, int32_t region, int64_t step) 
   const double two_pi = 6.2831853071795864769252867665590;
   int w = (int)(step & 3);
   uint32_t xa = w < 2 ? x[0] : x[2], xb = w < 2 ? x[1] : x[3];
-  double r = std::sqrt(-2.0 * std::log(u24(xa)));
-  double th = two_pi * u24(xb);
+  double r = std::sqrt(-2.0 * std::log(u23(xa)));
+  double th = two_pi * u23(xb);
   return (w & 1) ? r * std::sin(th) : r * std::cos(th);
 }
 
@@ -406,7 +408,7 @@ int orc_delay_index(double L_mm, double v, double dt) { return delay_index(L_mm,
 void orc_philox4x32_10(const unsigned* ctr, const unsigned* key, unsigned* out) {
   philox4x32_10(ctr, key, out);
 }
-double orc_uniform24(unsigned x) { return u24(x); }
+double orc_uniform23(unsigned x) { return u23(x); }
 double orc_normal(unsigned long long seed, long long sim, int region, long long step) {
   return normal_variate(seed, sim, region, step);
 }
