@@ -1,0 +1,7 @@
+"""tvbx: B200-native batched TVB-AdEx parameter-sweep integrator (arxiv 2311.13337 hot path).
+
+The product is the C-ABI library `libtvbx.so` (include/tvbx.h; sources in csrc/); this package is
+its thin Python binding.  See DESIGN.md.
+"""
+from .binding import (Connectome, Sweep, TvbxError, build, default_params, lib, sweep_from_config,  # noqa: F401
+                      PARAM_IDS, N_PARAMS, TVBX_F32, TVBX_F64, LIB_PATH, EXPORTS)

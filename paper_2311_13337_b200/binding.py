@@ -1,0 +1,328 @@
+"""Thin Python binding of the C ABI in include/tvbx.h (argument marshalling only).
+
+Every step of the hot path runs in the CUDA kernels of libtvbx.so; PyTorch is used only for device
+buffers and streams.  There is no CPU fallback: importing works without a GPU (so the symbol table
+can be checked), but any compute call fails with TvbxError(TVBX_ECUDA) when no device is present, and
+loading fails loudly when the library has not been built.
+"""
+from __future__ import annotations
+
+import ctypes as C
+import os
+import subprocess
+
+import numpy as np
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+_ROOT = os.path.dirname(_HERE)
+LIB_PATH = os.path.join(_HERE, "libtvbx.so")
+SRC_DIR = os.path.join(_HERE, "csrc")
+NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std=c++17",
+              "-Xcompiler", "-fPIC", "-shared"]
+
+TVBX_OK, TVBX_EINVAL, TVBX_ENOMEM, TVBX_ECUDA, TVBX_ESTATE = 0, -1, -2, -3, -4
+TVBX_F32, TVBX_F64 = 0, 1
+
+# parameter ids (include/tvbx.h enum tvbx_param_id)
+PARAM_IDS = dict(
+    G=0, b_e=1, a_e=2, tau_w_e=3, v=4, wNoise=5, E_L_e=6, E_L_i=7, T=8, c_Fee=9, c_Fei=10, c_Fie=11,
+    c_Fii=12, b_i=13, a_i=14, tau_w_i=15, g_L=16, C_m=17, Q_e=18, tau_e=19, E_e=20, Q_i=21, tau_i=22,
+    E_i=23, N_tot=24, p_conn=25, g_inh=26, tau_OU=27, mu_OU=28, sigma_OU=29, muV0=30, dmuV0=31, sV0=32,
+    dsV0=33, tauVN0=34, dtauVN0=35, eps_nu=36, muV_local=37, kappa=38)
+P_POLY_E, P_POLY_I, N_PARAMS, N_SWEEPABLE = 39, 49, 59, 13
+
+
+class TvbxError(RuntimeError):
+    def __init__(self, code, msg):
+        super().__init__(f"tvbx error {code}: {msg}")
+        self.code = code
+
+
+class ModelParams(C.Structure):
+    _fields_ = [("p", C.c_double * N_PARAMS)]
+
+
+class Axis(C.Structure):
+    _fields_ = [("param_id", C.c_int32), ("n", C.c_int32), ("lo", C.c_double), ("hi", C.c_double),
+                ("values", C.POINTER(C.c_double))]
+
+
+class SweepOpts(C.Structure):
+    _fields_ = [("precision", C.c_int32), ("sims_per_cta", C.c_int32), ("n_sims", C.c_int64),
+                ("sim_ids", C.POINTER(C.c_int64)), ("chunk_samples", C.c_int64),
+                ("threads_per_cta", C.c_int32), ("reserved", C.c_int32)]
+
+
+class RunOpts(C.Structure):
+    _fields_ = [("noise_on", C.c_int32), ("ds", C.c_int32), ("discard_steps", C.c_int64),
+                ("traj", C.c_void_p), ("traj_steps", C.c_int64), ("traj_on_device", C.c_int32),
+                ("reserved", C.c_int32), ("cuda_stream", C.c_void_p)]
+
+
+EXPORTS = [
+    "tvbx_default_params", "tvbx_create_connectome", "tvbx_destroy_connectome", "tvbx_sweep_create",
+    "tvbx_sweep_destroy", "tvbx_sweep_set_initial", "tvbx_run", "tvbx_fc_readout", "tvbx_sweep_size",
+    "tvbx_sweep_param", "tvbx_sweep_ext_id", "tvbx_delay_index", "tvbx_ring_len", "tvbx_steps_done",
+    "tvbx_samples_kept", "tvbx_sweep_state", "tvbx_launch_info", "tvbx_launch_count", "tvbx_last_error",
+    "tvbx_version",
+]
+
+
+def build(force: bool = False, verbose: bool = False) -> str:
+    """Compile csrc/*.cu for sm_100a into libtvbx.so (in-tree).  nvcc cross-compiles without a GPU."""
+    srcs = [os.path.join(SRC_DIR, f) for f in sorted(os.listdir(SRC_DIR))]
+    hdr = os.path.join(_ROOT, "include", "tvbx.h")
+    newest = max(os.path.getmtime(f) for f in srcs + [hdr])
+    if force or not os.path.exists(LIB_PATH) or os.path.getmtime(LIB_PATH) < newest:
+        cmd = ["nvcc", *NVCC_FLAGS, "-o", LIB_PATH, os.path.join(SRC_DIR, "tvbx_api.cu")]
+        if verbose:
+            cmd.insert(1, "-Xptxas=-v")
+        subprocess.check_call(cmd)
+    return LIB_PATH
+
+
+_lib = None
+
+
+def lib():
+    global _lib
+    if _lib is None:
+        if not os.path.exists(LIB_PATH):
+            raise ImportError(f"{LIB_PATH} is missing: run `python -c 'import __graft_entry__ as g; g.build()'` "
+                              "(there is no CPU fallback)")
+        L = C.CDLL(LIB_PATH)
+        vp, i32, i64, dbl = C.c_void_p, C.c_int32, C.c_int64, C.c_double
+        dp, fp = C.POINTER(C.c_double), C.POINTER(C.c_float)
+        sig = {
+            "tvbx_default_params": [C.POINTER(ModelParams)],
+            "tvbx_create_connectome": [i32, dp, dp, C.POINTER(vp)],
+            "tvbx_destroy_connectome": [vp],
+            "tvbx_sweep_create": [vp, C.POINTER(ModelParams), i32, C.POINTER(Axis), C.c_uint64,
+                                  C.POINTER(SweepOpts), C.POINTER(vp)],
+            "tvbx_sweep_destroy": [vp],
+            "tvbx_sweep_set_initial": [vp, dp],
+            "tvbx_run": [vp, i64, dbl, C.POINTER(RunOpts)],
+            "tvbx_fc_readout": [vp, vp, vp, vp, i32, vp],
+            "tvbx_sweep_size": [vp, C.POINTER(i64), C.POINTER(i64), C.POINTER(i32)],
+            "tvbx_sweep_param": [vp, i64, i32, dp],
+            "tvbx_sweep_ext_id": [vp, i64, C.POINTER(i64)],
+            "tvbx_delay_index": [vp, i64, i32, i32, dbl, C.POINTER(i32)],
+            "tvbx_ring_len": [vp, i64, dbl, C.POINTER(i32), C.POINTER(i32)],
+            "tvbx_steps_done": [vp, C.POINTER(i64)],
+            "tvbx_samples_kept": [vp, C.POINTER(i64)],
+            "tvbx_sweep_state": [vp, dp, dp],
+            "tvbx_launch_info": [vp, C.POINTER(i32)],
+            "tvbx_launch_count": [vp, C.POINTER(i64)],
+        }
+        for name, argtypes in sig.items():
+            fn = getattr(L, name)
+            fn.argtypes = argtypes
+            fn.restype = i32
+        L.tvbx_last_error.restype = C.c_char_p
+        L.tvbx_version.restype = i32
+        _lib = L
+    return _lib
+
+
+def _chk(rc):
+    if rc != 0:
+        raise TvbxError(rc, lib().tvbx_last_error().decode())
+
+
+def _dptr(a):
+    return a.ctypes.data_as(C.POINTER(C.c_double))
+
+
+def default_params() -> np.ndarray:
+    m = ModelParams()
+    _chk(lib().tvbx_default_params(C.byref(m)))
+    return np.array(m.p[:], dtype=np.float64)
+
+
+class Connectome:
+    """tvbx_create_connectome / tvbx_destroy_connectome.  W[k, j] = weight of source j into target k."""
+
+    def __init__(self, W, L_mm):
+        W = np.ascontiguousarray(W, dtype=np.float64)
+        L = np.ascontiguousarray(L_mm, dtype=np.float64)
+        assert W.ndim == 2 and W.shape[0] == W.shape[1] and W.shape == L.shape
+        self.n = W.shape[0]
+        self._h = C.c_void_p()
+        _chk(lib().tvbx_create_connectome(self.n, _dptr(W), _dptr(L), C.byref(self._h)))
+
+    def close(self):
+        if getattr(self, "_h", None):
+            lib().tvbx_destroy_connectome(self._h)
+            self._h = None
+
+    __del__ = close
+
+
+class Sweep:
+    """tvbx_sweep_create ... tvbx_sweep_destroy.
+
+    axes: list of dicts {name | param_id, lo, hi, n, values (optional list)} (workloads.config axes).
+    params: optional full default vector (N_PARAMS float64, include/tvbx.h order) or dict of overrides.
+    """
+
+    def __init__(self, conn: Connectome, axes, seed=0, params=None, precision=TVBX_F32, sims_per_cta=0,
+                 sim_ids=None, chunk_samples=0, threads_per_cta=0, init=None):
+        L = lib()
+        self.conn = conn
+        m = ModelParams()
+        _chk(L.tvbx_default_params(C.byref(m)))
+        if params is not None:
+            if isinstance(params, dict):
+                for k, v in params.items():
+                    if k == "poly_e":
+                        m.p[P_POLY_E:P_POLY_E + 10] = list(map(float, v))
+                    elif k == "poly_i":
+                        m.p[P_POLY_I:P_POLY_I + 10] = list(map(float, v))
+                    else:
+                        m.p[PARAM_IDS[k]] = float(v)
+            else:
+                vec = np.asarray(params, dtype=np.float64)
+                assert vec.shape == (N_PARAMS,)
+                for i in range(N_PARAMS):
+                    m.p[i] = float(vec[i])
+        ax = (Axis * max(1, len(axes)))()
+        keep = []
+        for i, a in enumerate(axes):
+            ax[i].param_id = a["param_id"] if "param_id" in a else PARAM_IDS[a["name"]]
+            ax[i].n = int(a["n"]); ax[i].lo = float(a["lo"]); ax[i].hi = float(a["hi"])
+            if a.get("values") is not None:
+                arr = np.ascontiguousarray(a["values"], dtype=np.float64)
+                keep.append(arr)
+                ax[i].values = _dptr(arr)
+        o = SweepOpts()
+        o.precision = precision; o.sims_per_cta = sims_per_cta; o.chunk_samples = chunk_samples
+        o.threads_per_cta = threads_per_cta
+        if sim_ids is not None:
+            ids = np.ascontiguousarray(sim_ids, dtype=np.int64)
+            keep.append(ids)
+            o.n_sims = ids.size
+            o.sim_ids = ids.ctypes.data_as(C.POINTER(C.c_int64))
+        self._h = C.c_void_p()
+        _chk(L.tvbx_sweep_create(conn._h, C.byref(m), len(axes), ax, seed, C.byref(o), C.byref(self._h)))
+        ns, gs, nr = C.c_int64(), C.c_int64(), C.c_int32()
+        _chk(L.tvbx_sweep_size(self._h, C.byref(ns), C.byref(gs), C.byref(nr)))
+        self.n_sims, self.grid_size, self.n_regions = ns.value, gs.value, nr.value
+        self.precision = precision
+        if init is not None:
+            a = np.ascontiguousarray(init, dtype=np.float64)
+            _chk(L.tvbx_sweep_set_initial(self._h, _dptr(a)))
+
+    def close(self):
+        if getattr(self, "_h", None):
+            lib().tvbx_sweep_destroy(self._h)
+            self._h = None
+
+    __del__ = close
+
+    # ---- tvbx_run --------------------------------------------------------------------------------
+    def run(self, steps, dt=0.1, noise_on=False, ds=10, discard_steps=0, traj_steps=0, traj_device=False,
+            stream=None):
+        """Advance all sims.  Returns the trajectory of the first traj_steps steps of this call,
+        [n_sims][traj_steps][7][N] (numpy on host, or a torch CUDA tensor if traj_device), else None."""
+        o = RunOpts()
+        o.noise_on = int(bool(noise_on)); o.ds = int(ds); o.discard_steps = int(discard_steps)
+        o.cuda_stream = _stream_ptr(stream)
+        traj = None
+        if traj_steps > 0:
+            traj_steps = min(int(traj_steps), int(steps))
+            shape = (self.n_sims, traj_steps, 7, self.n_regions)
+            if traj_device:
+                import torch
+                traj = torch.zeros(shape, device="cuda",
+                                   dtype=torch.float64 if self.precision == TVBX_F64 else torch.float32)
+                o.traj = traj.data_ptr(); o.traj_on_device = 1
+            else:
+                traj = np.zeros(shape, dtype=np.float64 if self.precision == TVBX_F64 else np.float32)
+                o.traj = traj.ctypes.data
+            o.traj_steps = traj_steps
+        _chk(lib().tvbx_run(self._h, int(steps), float(dt), C.byref(o)))
+        return traj
+
+    # ---- tvbx_fc_readout -------------------------------------------------------------------------
+    def fc_readout(self, device=False, stream=None, out=None):
+        """-> (fc [S][N][N], mean_e [S][N], mean_i [S][N]) float32; numpy (host) or torch CUDA tensors.
+        `out`: optional preallocated triple of the right kind."""
+        S, N = self.n_sims, self.n_regions
+        if device:
+            import torch
+            fc, me, mi = out if out is not None else (
+                torch.empty((S, N, N), device="cuda", dtype=torch.float32),
+                torch.empty((S, N), device="cuda", dtype=torch.float32),
+                torch.empty((S, N), device="cuda", dtype=torch.float32))
+            _chk(lib().tvbx_fc_readout(self._h, fc.data_ptr(), me.data_ptr(), mi.data_ptr(), 1, _stream_ptr(stream)))
+        else:
+            fc, me, mi = out if out is not None else (
+                np.empty((S, N, N), np.float32), np.empty((S, N), np.float32), np.empty((S, N), np.float32))
+            _chk(lib().tvbx_fc_readout(self._h, fc.ctypes.data, me.ctypes.data, mi.ctypes.data, 0, _stream_ptr(stream)))
+        return fc, me, mi
+
+    # ---- accessors ---------------------------------------------------------------------------------
+    def param(self, sim, name_or_id):
+        pid = name_or_id if isinstance(name_or_id, int) else PARAM_IDS[name_or_id]
+        out = C.c_double()
+        _chk(lib().tvbx_sweep_param(self._h, sim, pid, C.byref(out)))
+        return out.value
+
+    def ext_id(self, sim):
+        out = C.c_int64()
+        _chk(lib().tvbx_sweep_ext_id(self._h, sim, C.byref(out)))
+        return out.value
+
+    def delay_index(self, sim, k, j, dt=0.0):
+        out = C.c_int32()
+        _chk(lib().tvbx_delay_index(self._h, sim, k, j, dt, C.byref(out)))
+        return out.value
+
+    def ring_len(self, sim, dt=0.0):
+        h, hp = C.c_int32(), C.c_int32()
+        _chk(lib().tvbx_ring_len(self._h, sim, dt, C.byref(h), C.byref(hp)))
+        return h.value, hp.value
+
+    def steps_done(self):
+        out = C.c_int64()
+        _chk(lib().tvbx_steps_done(self._h, C.byref(out)))
+        return out.value
+
+    def samples_kept(self):
+        out = C.c_int64()
+        _chk(lib().tvbx_samples_kept(self._h, C.byref(out)))
+        return out.value
+
+    def state(self):
+        """-> (y [S][7][N], ou [S][N]) float64 on host (synchronises)."""
+        y = np.zeros((self.n_sims, 7, self.n_regions)); ou = np.zeros((self.n_sims, self.n_regions))
+        _chk(lib().tvbx_sweep_state(self._h, _dptr(y), _dptr(ou)))
+        return y, ou
+
+    def launch_info(self):
+        a = (C.c_int32 * 8)()
+        _chk(lib().tvbx_launch_info(self._h, a))
+        keys = ("ctas", "threads", "sims_per_cta", "regs", "smem", "passes", "chunk_samples", "local_bytes")
+        return dict(zip(keys, a[:]))
+
+    def launch_count(self):
+        out = C.c_int64()
+        _chk(lib().tvbx_launch_count(self._h, C.byref(out)))
+        return out.value
+
+
+def _stream_ptr(stream):
+    if stream is None:
+        return None
+    if isinstance(stream, int):
+        return stream
+    return stream.cuda_stream      # torch.cuda.Stream
+
+
+def sweep_from_config(cfg: dict, W, L_mm, **kw):
+    """Convenience: (Connectome, Sweep) for a workloads.config() dict."""
+    conn = Connectome(W, L_mm)
+    params = dict(cfg.get("fixed", {}))
+    params.update(kw.pop("params", {}) or {})
+    sw = Sweep(conn, cfg["axes"], seed=kw.pop("seed", cfg["seed"]), params=params, **kw)
+    return conn, sw

@@ -1,0 +1,715 @@
+// tvbx_api.cu -- host side of the C ABI declared in include/tvbx.h: connectome, parameter grid,
+// delay tables, grouping of simulations by speed, device memory, kernel launches.
+// No torch types, no CPU fallback: every compute entry point needs a CUDA device.
+#include "../../include/tvbx.h"
+
+#include <cuda_runtime.h>
+
+#include <algorithm>
+#include <cmath>
+#include <cstdarg>
+#include <cstdio>
+#include <cstdlib>
+#include <cstring>
+#include <map>
+#include <memory>
+#include <new>
+#include <string>
+#include <vector>
+
+#include "tvbx_fc.cuh"
+#include "tvbx_integrate.cuh"
+
+namespace {
+
+thread_local std::string g_err;
+int32_t fail(int32_t code, const char* fmt, ...) {
+  char buf[512];
+  va_list ap;
+  va_start(ap, fmt);
+  vsnprintf(buf, sizeof buf, fmt, ap);
+  va_end(ap);
+  g_err = buf;
+  return code;
+}
+#define CU(call)                                                                              \
+  do {                                                                                        \
+    cudaError_t e_ = (call);                                                                  \
+    if (e_ != cudaSuccess)                                                                    \
+      return fail(e_ == cudaErrorMemoryAllocation ? TVBX_ENOMEM : TVBX_ECUDA, "%s: %s", #call, \
+                  cudaGetErrorString(e_));                                                    \
+  } while (0)
+
+// library defaults
+const double kPolyRS[10] = {-48.9, 5.1, -25.0, 1.4, -0.41, 10.5, -36.0, 7.4, 1.2, 40.7};
+const double kPolyFS[10] = {-51.4, 0.4, -8.3, 0.2, -0.5, 1.4, -14.6, 4.5, 2.8, 15.3};
+
+void default_params(tvbx_model_params* m) {
+  double* p = m->p;
+  for (int i = 0; i < TVBX_N_PARAMS; ++i) p[i] = 0.0;
+  p[TVBX_P_G] = 0.0; p[TVBX_P_B_E] = 0.0; p[TVBX_P_A_E] = 0.0; p[TVBX_P_TAU_W_E] = 500.0;
+  p[TVBX_P_V] = 4.0; p[TVBX_P_WNOISE] = 1e-6; p[TVBX_P_EL_E] = -64.0; p[TVBX_P_EL_I] = -64.0;
+  p[TVBX_P_T] = 20.0;
+  p[TVBX_P_CFEE] = 0.3e-3; p[TVBX_P_CFEI] = 0.0; p[TVBX_P_CFIE] = 0.3e-3; p[TVBX_P_CFII] = 0.0;
+  p[TVBX_P_B_I] = 0.0; p[TVBX_P_A_I] = 0.0; p[TVBX_P_TAU_W_I] = 1.0;
+  p[TVBX_P_GL] = 10.0; p[TVBX_P_CM] = 200.0;
+  p[TVBX_P_QE] = 1.5; p[TVBX_P_TAUE] = 5.0; p[TVBX_P_EE] = 0.0;
+  p[TVBX_P_QI] = 5.0; p[TVBX_P_TAUI] = 5.0; p[TVBX_P_EI] = -80.0;
+  p[TVBX_P_NTOT] = 10000.0; p[TVBX_P_PCONN] = 0.05; p[TVBX_P_GINH] = 0.2;
+  p[TVBX_P_TAU_OU] = 5.0; p[TVBX_P_MU_OU] = 0.0; p[TVBX_P_SIGMA_OU] = 1.0;
+  p[TVBX_P_MUV0] = -60.0; p[TVBX_P_DMUV0] = 10.0; p[TVBX_P_SV0] = 4.0; p[TVBX_P_DSV0] = 6.0;
+  p[TVBX_P_TVN0] = 0.5; p[TVBX_P_DTVN0] = 1.0;
+  p[TVBX_P_EPS_NU] = 1e-6; p[TVBX_P_MUV_LOCAL] = 0.0; p[TVBX_P_KAPPA] = 1e-3;
+  for (int i = 0; i < 10; ++i) { p[TVBX_P_POLY_E + i] = kPolyRS[i]; p[TVBX_P_POLY_I + i] = kPolyFS[i]; }
+}
+
+// A19: equally spaced, closed interval, last value forced to hi
+double axis_value(double lo, double hi, int n, int i) {
+  if (n <= 1) return lo;
+  if (i == n - 1) return hi;
+  const double step = (hi - lo) / (double)(n - 1);
+  return lo + (double)i * step;
+}
+// A13
+int32_t delay_steps(double L_mm, double v, double dt) { return (int32_t)std::nearbyint((L_mm / v) / dt); }
+
+struct HostEdge { int32_t j; double w; double L; };
+
+struct Axis { int32_t id; std::vector<double> vals; };
+
+struct HostTable {      // one per distinct speed
+  double v = 0;
+  int32_t D = 0, dmin = 0, B = 1, Hp = 2;
+  std::vector<int32_t> delays;   // per kept edge, CSR order
+  std::vector<int64_t> sims;     // local sim indices
+};
+struct HostGroup { int32_t table; std::vector<int64_t> lanes; };  // lanes[sl] = local sim or -1
+
+// polymorphic device side (float / double)
+struct DeviceSide {
+  virtual ~DeviceSide() {}
+  virtual int32_t start(double dt) = 0;
+  virtual int32_t run(int64_t steps, const tvbx_run_opts* o) = 0;
+  virtual int32_t readout(float* fc, float* me, float* mi, int on_device, cudaStream_t st) = 0;
+  virtual int32_t state(double* y, double* ou) = 0;
+};
+
+}  // namespace
+
+struct tvbx_connectome {
+  int32_t n;
+  std::vector<double> W, L;
+  std::vector<int32_t> rowptr;       // CSR of the non-zero weights, ascending j
+  std::vector<HostEdge> edges;
+};
+
+struct tvbx_sweep {
+  tvbx_connectome conn;
+  tvbx_model_params defaults;
+  std::vector<Axis> axes;
+  int64_t grid_size = 1, n_sims = 0;
+  std::vector<int64_t> ext_ids;
+  uint64_t seed = 0;
+  int32_t precision = TVBX_F32, spc = 8, threads_req = 0;
+  int64_t chunk_req = 0;
+  double init[7] = {0.001, 0.001, 0, 0, 0, 0, 0};
+  // grouping
+  std::vector<HostTable> tables;
+  std::vector<int32_t> sim_table;    // local sim -> table
+  std::vector<HostGroup> groups;
+  std::vector<std::pair<int32_t, int32_t>> sim_slot;   // local sim -> (group, lane)
+  // run state
+  bool started = false;
+  double dt = 0;
+  int64_t n = 0, cnt = 0, fill = 0, CS = 0, launches = 0;
+  int32_t info[8] = {0, 0, 0, 0, 0, 0, 0, 0};
+  int device = 0;
+  std::unique_ptr<DeviceSide> dev;
+
+  double param(int64_t sim, int32_t id) const {
+    int64_t s = ext_ids[sim];
+    double val = defaults.p[id];
+    for (int a = (int)axes.size() - 1; a >= 0; --a) {
+      const int64_t na = (int64_t)axes[a].vals.size();
+      const int64_t dig = s % na;
+      s /= na;
+      if (axes[a].id == id) val = axes[a].vals[dig];
+    }
+    return val;
+  }
+};
+
+// ====================================================================================================
+//  Device side
+// ====================================================================================================
+namespace {
+
+using namespace tvbx;
+
+template <typename T>
+struct DevBuf {
+  T* p = nullptr;
+  size_t n = 0;
+  ~DevBuf() { if (p) cudaFree(p); }
+  cudaError_t alloc(size_t count) {
+    if (p) { cudaFree(p); p = nullptr; }
+    n = count;
+    return cudaMalloc((void**)&p, std::max<size_t>(count, 1) * sizeof(T));
+  }
+  cudaError_t upload(const std::vector<T>& h) {
+    cudaError_t e = alloc(h.size());
+    if (e != cudaSuccess) return e;
+    return cudaMemcpy(p, h.data(), h.size() * sizeof(T), cudaMemcpyHostToDevice);
+  }
+};
+
+template <typename R>
+__global__ void fill_kernel(R* p, size_t n, R v) {
+  for (size_t i = blockIdx.x * (size_t)blockDim.x + threadIdx.x; i < n; i += (size_t)gridDim.x * blockDim.x) p[i] = v;
+}
+
+template <typename R> struct KernelPick { void (*fn)(const IntegrateParams<R>); int maxt; };
+
+// (SPC, SINGLE) -> kernel instantiation.  MAXT bounds the registers: 544 threads -> <= 120 registers
+// (FP32), 256 threads -> <= 255 (FP64).
+template <typename R> struct MaxT;
+template <> struct MaxT<float> { static constexpr int v = 544; };
+template <> struct MaxT<double> { static constexpr int v = 256; };
+
+template <typename R>
+KernelPick<R> pick_kernel(int spc, bool single) {
+  constexpr int MT = MaxT<R>::v;
+#define TVBX_CASE(S)                                                                         \
+  case S:                                                                                    \
+    return single ? KernelPick<R>{integrate_kernel<R, S, true, MT>, MT}                      \
+                  : KernelPick<R>{integrate_kernel<R, S, false, MT>, MT};
+  switch (spc) {
+    TVBX_CASE(1) TVBX_CASE(2) TVBX_CASE(4) TVBX_CASE(8) TVBX_CASE(16) TVBX_CASE(32)
+    default: return KernelPick<R>{nullptr, 0};
+  }
+#undef TVBX_CASE
+}
+
+template <typename R>
+struct DeviceImpl : DeviceSide {
+  tvbx_sweep* sw;
+  DevBuf<TableDesc> d_tables;
+  DevBuf<GroupDesc> d_groups;
+  DevBuf<Edge<R>> d_edges;
+  DevBuf<int32_t> d_rowptr, d_ext, d_loc;
+  DevBuf<R> d_psim, d_ring, d_state, d_xbar;
+  DevBuf<double> d_sums, d_cmean, d_mean, d_M;
+  IntegrateParams<R> P;
+  KernelPick<R> kp{nullptr, 0};
+  int threads = 0, smem = 0;
+  bool single = true;
+
+  explicit DeviceImpl(tvbx_sweep* s) : sw(s) { std::memset(&P, 0, sizeof P); }
+
+  int32_t start(double dt) override {
+    const tvbx_connectome& c = sw->conn;
+    const int N = c.n, SPC = sw->spc;
+    const int G = (int)sw->groups.size();
+    const double* dp = sw->defaults.p;
+    int ndev = 0;
+    if (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev == 0) return fail(TVBX_ECUDA, "no CUDA device");
+    CU(cudaGetDevice(&sw->device));
+
+    // ---- delay tables per distinct speed (A13) and ring geometry ----
+    std::vector<TableDesc> tds(sw->tables.size());
+    std::vector<Edge<R>> edges;
+    std::vector<int32_t> rowptr;
+    for (size_t t = 0; t < sw->tables.size(); ++t) {
+      HostTable& ht = sw->tables[t];
+      ht.delays.clear();
+      int32_t D = 0, dmin = INT32_MAX;
+      for (const HostEdge& e : c.edges) {
+        const int32_t d = delay_steps(e.L, ht.v, dt);
+        if (d < 0 || d > 1000000) return fail(TVBX_EINVAL, "delay of %d steps out of range (v=%g, dt=%g)", d, ht.v, dt);
+        ht.delays.push_back(d);
+        D = std::max(D, d); dmin = std::min(dmin, d);
+      }
+      if (c.edges.empty()) dmin = 0;
+      ht.D = D; ht.dmin = dmin; ht.B = std::max(1, dmin); ht.Hp = D + ht.B + 1;
+      if ((int64_t)N * ht.Hp >= (int64_t)INT32_MAX / 2) return fail(TVBX_EINVAL, "ring too deep for 32-bit slot indices");
+      tds[t].Hp = ht.Hp; tds[t].B = ht.B; tds[t].n_edges = (int32_t)c.edges.size(); tds[t].pad = 0;
+      tds[t].edge_off = (int64_t)edges.size(); tds[t].rowptr_off = (int64_t)rowptr.size();
+      for (size_t e = 0; e < c.edges.size(); ++e) {
+        Edge<R> ed;
+        std::memset(&ed, 0, sizeof ed);
+        ed.w = (R)c.edges[e].w; ed.jbase = c.edges[e].j * ht.Hp; ed.back = ht.Hp - ht.delays[e];
+        edges.push_back(ed);
+      }
+      rowptr.insert(rowptr.end(), c.rowptr.begin(), c.rowptr.end());
+    }
+    // ---- groups ----
+    std::vector<GroupDesc> gds(G);
+    std::vector<int32_t> ext((size_t)G * SPC), loc((size_t)G * SPC);
+    std::vector<R> psim((size_t)G * NPS * SPC);
+    size_t ring_elems = 0;
+    for (int g = 0; g < G; ++g) {
+      const HostGroup& hg = sw->groups[g];
+      gds[g].table = hg.table; gds[g].pad = 0; gds[g].ring_off = (int64_t)ring_elems;
+      ring_elems += (size_t)N * sw->tables[hg.table].Hp * SPC;
+      for (int sl = 0; sl < SPC; ++sl) {
+        const int64_t s = hg.lanes[sl];
+        const int64_t src = s >= 0 ? s : hg.lanes[0];      // padding lanes replay lane 0, never read back
+        ext[(size_t)g * SPC + sl] = (int32_t)sw->ext_ids[src];
+        loc[(size_t)g * SPC + sl] = s >= 0 ? (int32_t)s : -1;
+        const double tw = sw->param(src, TVBX_P_TAU_W_E);
+        const double vals[NPS] = {sw->param(src, TVBX_P_G), sw->param(src, TVBX_P_WNOISE), sw->param(src, TVBX_P_B_E),
+                                  sw->param(src, TVBX_P_A_E) / tw, 1.0 / tw, sw->param(src, TVBX_P_EL_E),
+                                  sw->param(src, TVBX_P_EL_I), 1.0 / sw->param(src, TVBX_P_T),
+                                  sw->param(src, TVBX_P_CFEE), sw->param(src, TVBX_P_CFEI),
+                                  sw->param(src, TVBX_P_CFIE), sw->param(src, TVBX_P_CFII)};
+        for (int q = 0; q < NPS; ++q) psim[((size_t)g * NPS + q) * SPC + sl] = (R)vals[q];
+      }
+    }
+    // ---- memory budget ----
+    const size_t row = (size_t)N * SPC;
+    size_t free_b = 0, total_b = 0;
+    CU(cudaMemGetInfo(&free_b, &total_b));
+    int64_t CS = sw->chunk_req;
+    if (CS <= 0) {
+      const size_t budget = (size_t)1 << 30;
+      CS = (int64_t)(budget / std::max<size_t>(1, (size_t)G * row * sizeof(R)));
+      CS = std::min<int64_t>(std::max<int64_t>(CS, 16), 4096);
+    }
+    const size_t need = ring_elems * sizeof(R) + (size_t)G * CS * row * sizeof(R) +
+                        (size_t)G * SPC * N * N * sizeof(double) * 2 + (size_t)G * 16 * row * sizeof(double);
+    if (need > free_b)
+      return fail(TVBX_ENOMEM, "sweep needs %.2f GB of device memory (ring %.2f GB), %.2f GB free",
+                  need / 1e9, ring_elems * sizeof(R) / 1e9, free_b / 1e9);
+    sw->CS = CS;
+    CU(d_tables.upload(tds)); CU(d_groups.upload(gds)); CU(d_edges.upload(edges)); CU(d_rowptr.upload(rowptr));
+    CU(d_ext.upload(ext)); CU(d_loc.upload(loc)); CU(d_psim.upload(psim));
+    CU(d_ring.alloc(ring_elems));
+    CU(d_xbar.alloc((size_t)G * CS * row));
+    CU(d_cmean.alloc((size_t)G * row)); CU(d_mean.alloc((size_t)G * row));
+    CU(d_M.alloc((size_t)G * SPC * N * N));
+    CU(cudaMemset(d_M.p, 0, d_M.n * sizeof(double)));
+    CU(cudaMemset(d_mean.p, 0, d_mean.n * sizeof(double)));
+    CU(cudaMemset(d_xbar.p, 0, d_xbar.n * sizeof(R)));
+    // state: [G][10][N][SPC], sums [G][2][N][SPC]
+    std::vector<R> st((size_t)G * (NSV - 2) * row, R(0));
+    for (int g = 0; g < G; ++g)
+      for (int q = 0; q < 7; ++q)
+        for (size_t i = 0; i < row; ++i) st[((size_t)g * (NSV - 2) + q) * row + i] = (R)sw->init[q];
+    CU(d_state.upload(st));
+    CU(d_sums.alloc((size_t)G * 2 * row));
+    CU(cudaMemset(d_sums.p, 0, d_sums.n * sizeof(double)));
+    fill_kernel<R><<<1184, 256>>>(d_ring.p, ring_elems, (R)sw->init[0]);    // A14
+    CU(cudaGetLastError());
+
+    // ---- uniform constants ----
+    TFConst<R>& tf = P.tf;
+    const double Ke = dp[TVBX_P_PCONN] * dp[TVBX_P_NTOT] * (1.0 - dp[TVBX_P_GINH]);
+    const double Ki = dp[TVBX_P_PCONN] * dp[TVBX_P_NTOT] * dp[TVBX_P_GINH];
+    tf.gL = (R)dp[TVBX_P_GL]; tf.Cm = (R)dp[TVBX_P_CM];
+    tf.ae = (R)(dp[TVBX_P_QE] * dp[TVBX_P_TAUE] * Ke); tf.ai = (R)(dp[TVBX_P_QI] * dp[TVBX_P_TAUI] * Ki);
+    tf.aeEe = (R)(dp[TVBX_P_QE] * dp[TVBX_P_TAUE] * Ke * dp[TVBX_P_EE]);
+    tf.aiEi = (R)(dp[TVBX_P_QI] * dp[TVBX_P_TAUI] * Ki * dp[TVBX_P_EI]);
+    tf.Ee = (R)dp[TVBX_P_EE]; tf.Ei = (R)dp[TVBX_P_EI]; tf.Qe = (R)dp[TVBX_P_QE]; tf.Qi = (R)dp[TVBX_P_QI];
+    tf.cAe = (R)(Ke * dp[TVBX_P_TAUE] * dp[TVBX_P_TAUE]); tf.cAi = (R)(Ki * dp[TVBX_P_TAUI] * dp[TVBX_P_TAUI]);
+    tf.Te = (R)dp[TVBX_P_TAUE]; tf.Ti = (R)dp[TVBX_P_TAUI];
+    tf.gL_over_Cm = (R)(dp[TVBX_P_GL] / dp[TVBX_P_CM]);
+    tf.m_s = (R)(1.0 / dp[TVBX_P_DMUV0]); tf.m_o = (R)(-dp[TVBX_P_MUV0] / dp[TVBX_P_DMUV0]);
+    tf.s_s = (R)(1.0 / dp[TVBX_P_DSV0]);  tf.s_o = (R)(-dp[TVBX_P_SV0] / dp[TVBX_P_DSV0]);
+    tf.t_s = (R)(1.0 / dp[TVBX_P_DTVN0]); tf.t_o = (R)(-dp[TVBX_P_TVN0] / dp[TVBX_P_DTVN0]);
+    for (int i = 0; i < 10; ++i) { tf.P[0][i] = (R)dp[TVBX_P_POLY_E + i]; tf.P[1][i] = (R)dp[TVBX_P_POLY_I + i]; }
+    tf.eps = (R)dp[TVBX_P_EPS_NU];
+    tf.same_tau = dp[TVBX_P_TAUE] == dp[TVBX_P_TAUI];
+    P.b_i = (R)dp[TVBX_P_B_I]; P.a_i_over_tau = (R)(dp[TVBX_P_A_I] / dp[TVBX_P_TAU_W_I]);
+    P.inv_tau_w_i = (R)(1.0 / dp[TVBX_P_TAU_W_I]);
+    P.inv_Ne = (R)(1.0 / (dp[TVBX_P_NTOT] * (1.0 - dp[TVBX_P_GINH])));
+    P.inv_Ni = (R)(1.0 / (dp[TVBX_P_NTOT] * dp[TVBX_P_GINH]));
+    P.kappa = (R)dp[TVBX_P_KAPPA];
+    const double rho = std::exp(-dt / dp[TVBX_P_TAU_OU]);
+    P.ou_rho = (R)rho; P.ou_s = (R)(dp[TVBX_P_SIGMA_OU] * std::sqrt(1.0 - rho * rho));
+    P.ou_m = (R)(dp[TVBX_P_MU_OU] * (1.0 - rho));
+    P.dt = (R)dt;
+    P.muV_local = dp[TVBX_P_MUV_LOCAL] != 0.0;
+    P.N = N; P.seed = sw->seed; P.chunk_samples = (int32_t)CS;
+    P.tables = d_tables.p; P.groups = d_groups.p; P.edges = d_edges.p; P.rowptr = d_rowptr.p;
+    P.psim = d_psim.p; P.ext_id = d_ext.p; P.loc_id = d_loc.p; P.ring = d_ring.p; P.state = d_state.p;
+    P.sums = d_sums.p; P.xbar = d_xbar.p;
+
+    // ---- launch geometry ----
+    const int maxt = sw->threads_req > 0 ? std::min(sw->threads_req, MaxT<R>::v) : MaxT<R>::v;
+    const int pairs = N * SPC;
+    if (pairs <= maxt) { single = true; threads = ((pairs + 31) / 32) * 32; if (threads > maxt) threads = pairs; }
+    else {
+      single = false;
+      const int rtmax = std::max(1, maxt / SPC);
+      const int passes = (N + rtmax - 1) / rtmax;
+      const int rt = (N + passes - 1) / passes;
+      threads = rt * SPC;
+    }
+    kp = pick_kernel<R>(SPC, single);
+    if (!kp.fn) return fail(TVBX_EINVAL, "sims_per_cta=%d not supported", SPC);
+    const size_t tbytes = c.edges.size() * sizeof(Edge<R>) + (size_t)(N + 1) * 4;
+    P.smem_table = tbytes <= 160 * 1024;
+    smem = P.smem_table ? (int)((tbytes + 15) / 16 * 16) : 0;
+    CU(cudaFuncSetAttribute((const void*)kp.fn, cudaFuncAttributeMaxDynamicSharedMemorySize, std::max(smem, 1024)));
+    cudaFuncAttributes fa;
+    CU(cudaFuncGetAttributes(&fa, (const void*)kp.fn));
+    const int rt_block = threads / SPC;
+    sw->info[0] = G; sw->info[1] = threads; sw->info[2] = SPC; sw->info[3] = fa.numRegs; sw->info[4] = smem;
+    sw->info[5] = single ? 1 : (N + rt_block - 1) / rt_block; sw->info[6] = (int32_t)CS; sw->info[7] = (int32_t)fa.localSizeBytes;
+    CU(cudaDeviceSynchronize());
+    return TVBX_OK;
+  }
+
+  int32_t accumulate(double* Mbuf, double* meanbuf, int64_t cnt, int n_c, cudaStream_t st) {
+    const int N = sw->conn.n, SPC = sw->spc, G = (int)sw->groups.size();
+    FcParams<R> F;
+    F.xbar = d_xbar.p; F.cmean = d_cmean.p; F.mean = meanbuf; F.M = Mbuf; F.cnt = cnt; F.n_c = n_c;
+    F.CS = (int32_t)sw->CS; F.N = N; F.SPC = SPC; F.G = G;
+    const int row = N * SPC;
+    dim3 g1((row + 127) / 128, G);
+    fc_chunk_mean_kernel<R><<<g1, 128, 0, st>>>(F);
+    const int nt = (N + 31) / 32;
+    dim3 g2(nt, nt, G * SPC);
+    fc_comoment_kernel<R><<<g2, 64, 0, st>>>(F);
+    fc_mean_update_kernel<R><<<g1, 128, 0, st>>>(F);
+    sw->launches += 3;
+    CU(cudaGetLastError());
+    return TVBX_OK;
+  }
+
+  int32_t run(int64_t steps, const tvbx_run_opts* o) override {
+    cudaStream_t st = (cudaStream_t)o->cuda_stream;
+    const int N = sw->conn.n;
+    const int G = (int)sw->groups.size();
+    DevBuf<R> tmp_traj;
+    R* traj = nullptr;
+    const int64_t tsteps = o->traj ? std::min<int64_t>(o->traj_steps, steps) : 0;
+    const size_t traj_elems = (size_t)sw->n_sims * tsteps * 7 * N;
+    if (tsteps > 0) {
+      if (o->traj_on_device) traj = (R*)o->traj;
+      else { CU(tmp_traj.alloc(traj_elems)); traj = tmp_traj.p; }
+    }
+    P.noise_on = o->noise_on != 0; P.ds = o->ds; P.discard_steps = o->discard_steps;
+    P.traj = traj; P.traj_steps = o->traj_steps; P.traj_n0 = sw->n;
+    if (tsteps > 0) P.traj_steps = tsteps;
+    int64_t remaining = steps;
+    const int64_t ds = o->ds;
+    while (remaining > 0) {
+      int64_t take = remaining;
+      int64_t kept = 0;
+      if (ds > 0) {
+        const int64_t cap = sw->CS - sw->fill;                 // samples the chunk can still take
+        const int64_t e1 = std::max((sw->n / ds + 1) * ds, (o->discard_steps / ds + 1) * ds);  // first kept window end > n
+        const int64_t ec = e1 + (cap - 1) * ds;                // window end that fills the chunk
+        take = std::min(remaining, ec - sw->n);
+        const int64_t end = sw->n + take;
+        kept = end >= e1 ? (end - e1) / ds + 1 : 0;
+      }
+      P.n_begin = sw->n; P.n_end = sw->n + take; P.sample_base = (int32_t)sw->fill;
+      kp.fn<<<G, threads, smem, st>>>(P);
+      sw->launches += 1;
+      CU(cudaGetLastError());
+      sw->n += take; remaining -= take; sw->fill += kept;
+      if (ds > 0 && sw->fill == sw->CS) {
+        int32_t rc = accumulate(d_M.p, d_mean.p, sw->cnt, (int)sw->fill, st);
+        if (rc) return rc;
+        sw->cnt += sw->fill; sw->fill = 0;
+      }
+    }
+    if (tsteps > 0 && !o->traj_on_device) {
+      CU(cudaMemcpyAsync(o->traj, traj, traj_elems * sizeof(R), cudaMemcpyDeviceToHost, st));
+      CU(cudaStreamSynchronize(st));
+    }
+    return TVBX_OK;
+  }
+
+  int32_t readout(float* fc, float* me, float* mi, int on_device, cudaStream_t st) override {
+    const int N = sw->conn.n, SPC = sw->spc, G = (int)sw->groups.size();
+    const int64_t total = sw->cnt + sw->fill;
+    if (total < 2) return fail(TVBX_ESTATE, "fewer than 2 samples kept (%lld)", (long long)total);
+    DevBuf<double> tM, tmean;
+    const double* Msrc = d_M.p;
+    if (sw->fill > 0) {     // merge the open chunk into a scratch copy; the accumulators stay untouched
+      CU(tM.alloc(d_M.n)); CU(tmean.alloc(d_mean.n));
+      CU(cudaMemcpyAsync(tM.p, d_M.p, d_M.n * sizeof(double), cudaMemcpyDeviceToDevice, st));
+      CU(cudaMemcpyAsync(tmean.p, d_mean.p, d_mean.n * sizeof(double), cudaMemcpyDeviceToDevice, st));
+      int32_t rc = accumulate(tM.p, tmean.p, sw->cnt, (int)sw->fill, st);
+      if (rc) return rc;
+      Msrc = tM.p;
+    }
+    DevBuf<float> dfc, dme, dmi;
+    ReadoutParams Q;
+    Q.M = Msrc; Q.sums = d_sums.p; Q.loc_id = d_loc.p; Q.cnt = total; Q.N = N; Q.SPC = SPC; Q.G = G;
+    Q.fc = fc; Q.mean_e = me; Q.mean_i = mi;
+    if (!on_device) {
+      if (fc) { CU(dfc.alloc((size_t)sw->n_sims * N * N)); Q.fc = dfc.p; }
+      if (me) { CU(dme.alloc((size_t)sw->n_sims * N)); Q.mean_e = dme.p; }
+      if (mi) { CU(dmi.alloc((size_t)sw->n_sims * N)); Q.mean_i = dmi.p; }
+    }
+    dim3 grid((N * N + 255) / 256, G * SPC);
+    fc_readout_kernel<<<grid, 256, 0, st>>>(Q);
+    sw->launches += 1;
+    CU(cudaGetLastError());
+    if (!on_device) {
+      if (fc) CU(cudaMemcpyAsync(fc, dfc.p, dfc.n * sizeof(float), cudaMemcpyDeviceToHost, st));
+      if (me) CU(cudaMemcpyAsync(me, dme.p, dme.n * sizeof(float), cudaMemcpyDeviceToHost, st));
+      if (mi) CU(cudaMemcpyAsync(mi, dmi.p, dmi.n * sizeof(float), cudaMemcpyDeviceToHost, st));
+      CU(cudaStreamSynchronize(st));
+    } else if (sw->fill > 0) {
+      CU(cudaStreamSynchronize(st));   // scratch copies are freed on return
+    }
+    return TVBX_OK;
+  }
+
+  int32_t state(double* y, double* ou) override {
+    const int N = sw->conn.n, SPC = sw->spc, G = (int)sw->groups.size();
+    const size_t row = (size_t)N * SPC;
+    std::vector<R> h((size_t)G * (NSV - 2) * row);
+    CU(cudaDeviceSynchronize());
+    CU(cudaMemcpy(h.data(), d_state.p, h.size() * sizeof(R), cudaMemcpyDeviceToHost));
+    for (int64_t s = 0; s < sw->n_sims; ++s) {
+      const int g = sw->sim_slot[s].first, sl = sw->sim_slot[s].second;
+      for (int k = 0; k < N; ++k) {
+        for (int q = 0; q < 7; ++q)
+          if (y) y[((size_t)s * 7 + q) * N + k] = (double)h[((size_t)g * (NSV - 2) + q) * row + (size_t)k * SPC + sl];
+        if (ou) ou[(size_t)s * N + k] = (double)h[((size_t)g * (NSV - 2) + 7) * row + (size_t)k * SPC + sl];
+      }
+    }
+    return TVBX_OK;
+  }
+};
+
+}  // namespace
+
+// ====================================================================================================
+//  extern "C" entry points
+// ====================================================================================================
+extern "C" {
+
+const char* tvbx_last_error(void) { return g_err.c_str(); }
+int32_t tvbx_version(void) { return TVBX_VERSION; }
+
+int32_t tvbx_default_params(tvbx_model_params* out) {
+  if (!out) return fail(TVBX_EINVAL, "out is NULL");
+  default_params(out);
+  return TVBX_OK;
+}
+
+int32_t tvbx_create_connectome(int32_t n, const double* W, const double* L_mm, tvbx_connectome** out) {
+  if (!out) return fail(TVBX_EINVAL, "out is NULL");
+  *out = nullptr;
+  if (n < 1 || n > 32767) return fail(TVBX_EINVAL, "n=%d out of range [1, 32767]", n);
+  if (!W || !L_mm) return fail(TVBX_EINVAL, "W or L_mm is NULL");
+  for (int64_t i = 0; i < (int64_t)n * n; ++i) {
+    if (!std::isfinite(W[i]) || W[i] < 0.0) return fail(TVBX_EINVAL, "W[%lld] is negative or not finite", (long long)i);
+    if (!std::isfinite(L_mm[i]) || L_mm[i] < 0.0) return fail(TVBX_EINVAL, "L_mm[%lld] is negative or not finite", (long long)i);
+  }
+  tvbx_connectome* c = new (std::nothrow) tvbx_connectome();
+  if (!c) return fail(TVBX_ENOMEM, "host allocation failed");
+  c->n = n;
+  c->W.assign(W, W + (size_t)n * n);
+  c->L.assign(L_mm, L_mm + (size_t)n * n);
+  c->rowptr.assign(n + 1, 0);
+  for (int k = 0; k < n; ++k) {
+    for (int j = 0; j < n; ++j) {
+      const double w = W[(size_t)k * n + j];
+      if (w != 0.0) c->edges.push_back({j, w, L_mm[(size_t)k * n + j]});
+    }
+    c->rowptr[k + 1] = (int32_t)c->edges.size();
+  }
+  *out = c;
+  return TVBX_OK;
+}
+int32_t tvbx_destroy_connectome(tvbx_connectome* c) { delete c; return TVBX_OK; }
+
+int32_t tvbx_sweep_create(const tvbx_connectome* c, const tvbx_model_params* defaults, int32_t n_axes,
+                          const tvbx_axis* axes, uint64_t seed, const tvbx_sweep_opts* opts, tvbx_sweep** out) {
+  if (!out) return fail(TVBX_EINVAL, "out is NULL");
+  *out = nullptr;
+  if (!c) return fail(TVBX_EINVAL, "connectome is NULL");
+  if (n_axes < 0 || n_axes > 16 || (n_axes > 0 && !axes)) return fail(TVBX_EINVAL, "bad axes");
+  std::unique_ptr<tvbx_sweep> sw(new (std::nothrow) tvbx_sweep());
+  if (!sw) return fail(TVBX_ENOMEM, "host allocation failed");
+  sw->conn = *c;
+  if (defaults) sw->defaults = *defaults; else default_params(&sw->defaults);
+  sw->seed = seed;
+  for (int a = 0; a < n_axes; ++a) {
+    const tvbx_axis& ax = axes[a];
+    if (ax.param_id < 0 || ax.param_id >= TVBX_N_SWEEPABLE) return fail(TVBX_EINVAL, "axis %d: parameter id %d is not sweepable", a, ax.param_id);
+    if (ax.n < 1) return fail(TVBX_EINVAL, "axis %d: n=%d", a, ax.n);
+    for (int b = 0; b < a; ++b) if (axes[b].param_id == ax.param_id) return fail(TVBX_EINVAL, "parameter id %d on two axes", ax.param_id);
+    Axis h; h.id = ax.param_id;
+    for (int i = 0; i < ax.n; ++i) {
+      const double val = ax.values ? ax.values[i] : axis_value(ax.lo, ax.hi, ax.n, i);
+      if (!std::isfinite(val)) return fail(TVBX_EINVAL, "axis %d: value %d not finite", a, i);
+      h.vals.push_back(val);
+    }
+    if (sw->grid_size > (int64_t)2147483647 / ax.n) return fail(TVBX_EINVAL, "grid larger than 2^31-1 simulations");
+    sw->grid_size *= ax.n;
+    sw->axes.push_back(std::move(h));
+  }
+  if (opts && opts->n_sims > 0) {
+    if (!opts->sim_ids) return fail(TVBX_EINVAL, "n_sims > 0 but sim_ids is NULL");
+    for (int64_t i = 0; i < opts->n_sims; ++i) {
+      if (opts->sim_ids[i] < 0 || opts->sim_ids[i] >= sw->grid_size) return fail(TVBX_EINVAL, "sim_ids[%lld]=%lld outside the grid", (long long)i, (long long)opts->sim_ids[i]);
+      sw->ext_ids.push_back(opts->sim_ids[i]);
+    }
+  } else {
+    sw->ext_ids.resize(sw->grid_size);
+    for (int64_t i = 0; i < sw->grid_size; ++i) sw->ext_ids[i] = i;
+  }
+  sw->n_sims = (int64_t)sw->ext_ids.size();
+  sw->precision = opts ? opts->precision : TVBX_F32;
+  if (sw->precision != TVBX_F32 && sw->precision != TVBX_F64) return fail(TVBX_EINVAL, "precision=%d", sw->precision);
+  sw->threads_req = opts ? opts->threads_per_cta : 0;
+  sw->chunk_req = opts ? opts->chunk_samples : 0;
+  // parameter sanity
+  for (int64_t s = 0; s < sw->n_sims; ++s) {
+    if (!(sw->param(s, TVBX_P_V) > 0.0)) return fail(TVBX_EINVAL, "speed v must be > 0 (sim %lld)", (long long)s);
+    if (!(sw->param(s, TVBX_P_T) > 0.0) || !(sw->param(s, TVBX_P_TAU_W_E) > 0.0)) return fail(TVBX_EINVAL, "T and tau_w_e must be > 0 (sim %lld)", (long long)s);
+  }
+  const double* dp = sw->defaults.p;
+  if (!(dp[TVBX_P_TAU_W_I] > 0) || !(dp[TVBX_P_TAU_OU] > 0) || !(dp[TVBX_P_GL] > 0) || !(dp[TVBX_P_CM] > 0) ||
+      !(dp[TVBX_P_DMUV0] != 0) || !(dp[TVBX_P_DSV0] != 0) || !(dp[TVBX_P_DTVN0] != 0) || !(dp[TVBX_P_EPS_NU] > 0) ||
+      !(dp[TVBX_P_GINH] > 0 && dp[TVBX_P_GINH] < 1) || !(dp[TVBX_P_NTOT] > 0) || !(dp[TVBX_P_PCONN] > 0))
+    return fail(TVBX_EINVAL, "uniform model parameters out of range");
+  // sims per CTA
+  int spc = opts ? opts->sims_per_cta : 0;
+  if (const char* e = getenv("TVBX_SPC")) if (spc == 0) spc = atoi(e);
+  if (spc == 0) {
+    spc = sw->precision == TVBX_F64 ? 2 : 8;
+    while (spc > 1 && sw->n_sims / spc < 148) spc /= 2;      // at least one CTA per SM when the sweep allows
+  }
+  if (spc != 1 && spc != 2 && spc != 4 && spc != 8 && spc != 16 && spc != 32) return fail(TVBX_EINVAL, "sims_per_cta=%d", spc);
+  sw->spc = spc;
+  // group the simulations by speed (one delay table per distinct v), then into CTAs of spc lanes
+  std::map<double, int32_t> vmap;
+  sw->sim_table.resize(sw->n_sims);
+  for (int64_t s = 0; s < sw->n_sims; ++s) {
+    const double v = sw->param(s, TVBX_P_V);
+    auto it = vmap.find(v);
+    if (it == vmap.end()) {
+      it = vmap.emplace(v, (int32_t)sw->tables.size()).first;
+      HostTable t; t.v = v; sw->tables.push_back(t);
+    }
+    sw->sim_table[s] = it->second;
+    sw->tables[it->second].sims.push_back(s);
+  }
+  sw->sim_slot.resize(sw->n_sims);
+  for (size_t t = 0; t < sw->tables.size(); ++t) {
+    const std::vector<int64_t>& v = sw->tables[t].sims;
+    for (size_t i = 0; i < v.size(); i += spc) {
+      HostGroup g; g.table = (int32_t)t; g.lanes.assign(spc, -1);
+      for (int sl = 0; sl < spc && i + sl < v.size(); ++sl) {
+        g.lanes[sl] = v[i + sl];
+        sw->sim_slot[v[i + sl]] = {(int32_t)sw->groups.size(), sl};
+      }
+      sw->groups.push_back(std::move(g));
+    }
+  }
+  *out = sw.release();
+  return TVBX_OK;
+}
+
+int32_t tvbx_sweep_destroy(tvbx_sweep* sw) { delete sw; return TVBX_OK; }
+
+int32_t tvbx_sweep_set_initial(tvbx_sweep* sw, const double init[7]) {
+  if (!sw || !init) return fail(TVBX_EINVAL, "NULL argument");
+  if (sw->started) return fail(TVBX_ESTATE, "initial state can only be set before the first tvbx_run");
+  for (int i = 0; i < 7; ++i) { if (!std::isfinite(init[i])) return fail(TVBX_EINVAL, "init[%d] not finite", i); sw->init[i] = init[i]; }
+  return TVBX_OK;
+}
+
+int32_t tvbx_run(tvbx_sweep* sw, int64_t steps, double dt, const tvbx_run_opts* opts) {
+  if (!sw) return fail(TVBX_EINVAL, "sweep is NULL");
+  if (steps < 0) return fail(TVBX_EINVAL, "steps < 0");
+  if (!(dt > 0.0) || !std::isfinite(dt)) return fail(TVBX_EINVAL, "dt must be > 0");
+  tvbx_run_opts o;
+  std::memset(&o, 0, sizeof o);
+  if (opts) o = *opts;
+  if (o.ds < 0 || o.discard_steps < 0 || o.traj_steps < 0) return fail(TVBX_EINVAL, "negative ds / discard_steps / traj_steps");
+  if (!sw->started) {
+    if (sw->precision == TVBX_F64) sw->dev.reset(new (std::nothrow) DeviceImpl<double>(sw));
+    else sw->dev.reset(new (std::nothrow) DeviceImpl<float>(sw));
+    if (!sw->dev) return fail(TVBX_ENOMEM, "host allocation failed");
+    int32_t rc = sw->dev->start(dt);
+    if (rc) { sw->dev.reset(); return rc; }
+    sw->dt = dt; sw->started = true;
+  } else if (dt != sw->dt) {
+    return fail(TVBX_EINVAL, "dt=%g differs from the dt of the first run (%g): the delay tables depend on it", dt, sw->dt);
+  }
+  if (steps == 0) return TVBX_OK;
+  return sw->dev->run(steps, &o);
+}
+
+int32_t tvbx_fc_readout(tvbx_sweep* sw, float* fc, float* mean_e, float* mean_i, int32_t on_device, void* stream) {
+  if (!sw) return fail(TVBX_EINVAL, "sweep is NULL");
+  if (!sw->started) return fail(TVBX_ESTATE, "no run yet");
+  return sw->dev->readout(fc, mean_e, mean_i, on_device, (cudaStream_t)stream);
+}
+
+int32_t tvbx_sweep_size(const tvbx_sweep* sw, int64_t* n_sims, int64_t* grid_size, int32_t* n_regions) {
+  if (!sw) return fail(TVBX_EINVAL, "sweep is NULL");
+  if (n_sims) *n_sims = sw->n_sims;
+  if (grid_size) *grid_size = sw->grid_size;
+  if (n_regions) *n_regions = sw->conn.n;
+  return TVBX_OK;
+}
+int32_t tvbx_sweep_param(const tvbx_sweep* sw, int64_t sim, int32_t id, double* out) {
+  if (!sw || !out) return fail(TVBX_EINVAL, "NULL argument");
+  if (sim < 0 || sim >= sw->n_sims || id < 0 || id >= TVBX_N_PARAMS) return fail(TVBX_EINVAL, "sim or param id out of range");
+  *out = sw->param(sim, id);
+  return TVBX_OK;
+}
+int32_t tvbx_sweep_ext_id(const tvbx_sweep* sw, int64_t sim, int64_t* out) {
+  if (!sw || !out || sim < 0 || sim >= sw->n_sims) return fail(TVBX_EINVAL, "bad argument");
+  *out = sw->ext_ids[sim];
+  return TVBX_OK;
+}
+int32_t tvbx_delay_index(const tvbx_sweep* sw, int64_t sim, int32_t k, int32_t j, double dt, int32_t* out) {
+  if (!sw || !out) return fail(TVBX_EINVAL, "NULL argument");
+  const int n = sw->conn.n;
+  if (sim < 0 || sim >= sw->n_sims || k < 0 || k >= n || j < 0 || j >= n) return fail(TVBX_EINVAL, "index out of range");
+  if (!(dt > 0.0)) { if (!sw->started) return fail(TVBX_ESTATE, "dt unknown before the first run"); dt = sw->dt; }
+  *out = sw->conn.W[(size_t)k * n + j] == 0.0 ? -1 : delay_steps(sw->conn.L[(size_t)k * n + j], sw->param(sim, TVBX_P_V), dt);
+  return TVBX_OK;
+}
+int32_t tvbx_ring_len(const tvbx_sweep* sw, int64_t sim, double dt, int32_t* H, int32_t* H_phys) {
+  if (!sw) return fail(TVBX_EINVAL, "sweep is NULL");
+  if (sim < 0 || sim >= sw->n_sims) return fail(TVBX_EINVAL, "sim out of range");
+  if (!(dt > 0.0)) { if (!sw->started) return fail(TVBX_ESTATE, "dt unknown before the first run"); dt = sw->dt; }
+  const double v = sw->param(sim, TVBX_P_V);
+  int32_t D = 0, dmin = INT32_MAX;
+  for (const HostEdge& e : sw->conn.edges) { const int32_t d = delay_steps(e.L, v, dt); D = std::max(D, d); dmin = std::min(dmin, d); }
+  if (sw->conn.edges.empty()) dmin = 0;
+  if (H) *H = D + 1;
+  if (H_phys) *H_phys = D + std::max(1, dmin) + 1;
+  return TVBX_OK;
+}
+int32_t tvbx_steps_done(const tvbx_sweep* sw, int64_t* n) {
+  if (!sw || !n) return fail(TVBX_EINVAL, "NULL argument");
+  *n = sw->n;
+  return TVBX_OK;
+}
+int32_t tvbx_samples_kept(const tvbx_sweep* sw, int64_t* n) {
+  if (!sw || !n) return fail(TVBX_EINVAL, "NULL argument");
+  *n = sw->cnt + sw->fill;
+  return TVBX_OK;
+}
+int32_t tvbx_sweep_state(tvbx_sweep* sw, double* y, double* ou) {
+  if (!sw) return fail(TVBX_EINVAL, "sweep is NULL");
+  if (!sw->started) return fail(TVBX_ESTATE, "no run yet");
+  return sw->dev->state(y, ou);
+}
+int32_t tvbx_launch_info(const tvbx_sweep* sw, int32_t info[8]) {
+  if (!sw || !info) return fail(TVBX_EINVAL, "NULL argument");
+  for (int i = 0; i < 8; ++i) info[i] = sw->info[i];
+  return TVBX_OK;
+}
+int32_t tvbx_launch_count(const tvbx_sweep* sw, int64_t* n) {
+  if (!sw || !n) return fail(TVBX_EINVAL, "NULL argument");
+  *n = sw->launches;
+  return TVBX_OK;
+}
+
+}  // extern "C"

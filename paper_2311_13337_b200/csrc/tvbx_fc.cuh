@@ -1,0 +1,159 @@
+// tvbx_fc.cuh -- the epilogue kernels: per-chunk mean, centred co-moment (X^T X) merged into the
+// running accumulators in Welford/Chan form (S7), and the Pearson finalisation (S8).
+// DESIGN.md section 6.4; PAPER.md P:113 ("covariance of the resulting time-series for all
+// concurrent simulations"), Eq. (6) P:161.
+//
+// The integrator leaves the kept 1-ms excitatory samples of the current chunk in
+//   xbar[group][sample][region][SPC]            (R = float or double)
+// For every simulation the running statistics are (cnt, mean[N], M[N][N]) in FP64:
+//   M_kl = sum_q (x_qk - mean_k)(x_ql - mean_l).
+// A chunk (n_c samples, chunk mean m_c, centred co-moment M_c computed in R after centring on m_c)
+// is merged with Chan's pairwise update
+//   delta = m_c - mean;  M += M_c + delta_k delta_l * cnt*n_c/(cnt+n_c);  mean += delta*n_c/(cnt+n_c).
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+namespace tvbx {
+
+template <typename R>
+struct FcParams {
+  const R* xbar;        // [G][CS][N][SPC]
+  double* cmean;        // [G][N][SPC]   chunk means (scratch)
+  double* mean;         // [G][N][SPC]   running mean
+  double* M;            // [G][SPC][N][N] running co-moment
+  int64_t cnt;          // samples merged so far (same for all sims)
+  int32_t n_c;          // samples in this chunk
+  int32_t CS, N, SPC, G;
+};
+
+// chunk mean per (group, region, sim lane): one thread each, coalesced over (region, lane)
+template <typename R>
+__global__ void fc_chunk_mean_kernel(FcParams<R> P) {
+  const int g = blockIdx.y;
+  const int idx = blockIdx.x * blockDim.x + threadIdx.x;     // region*SPC + lane
+  const int row = P.N * P.SPC;
+  if (idx >= row) return;
+  const R* x = P.xbar + (size_t)g * P.CS * row + idx;
+  double acc = 0.0;
+  for (int q = 0; q < P.n_c; ++q) acc += (double)x[(size_t)q * row];
+  P.cmean[(size_t)g * row + idx] = acc / (double)P.n_c;
+}
+
+// centred co-moment of one (group, sim lane, 32x32 output tile), merged into M.
+// 64 threads, each a 4x4 register tile; samples are staged through shared memory 32 at a time.
+template <typename R>
+__global__ void __launch_bounds__(64) fc_comoment_kernel(FcParams<R> P) {
+  constexpr int TS = 32, QT = 32;
+  __shared__ R sa[QT][TS + 1];
+  __shared__ R sb[QT][TS + 1];
+  const int g = blockIdx.z / P.SPC, sl = blockIdx.z % P.SPC;
+  const int tk = blockIdx.y, tl = blockIdx.x;
+  if (tl < tk) return;                                        // upper-triangular tiles only
+  const int row = P.N * P.SPC;
+  const R* x = P.xbar + (size_t)g * P.CS * row + sl;
+  const double* cm = P.cmean + (size_t)g * row + sl;
+  const int k0 = tk * TS, l0 = tl * TS;
+  const int ty = threadIdx.x / 8, tx = threadIdx.x % 8;       // 8x8 threads, 4x4 outputs each
+  R acc[4][4];
+#pragma unroll
+  for (int a = 0; a < 4; ++a)
+#pragma unroll
+    for (int b = 0; b < 4; ++b) acc[a][b] = R(0);
+  for (int q0 = 0; q0 < P.n_c; q0 += QT) {
+    for (int i = threadIdx.x; i < QT * TS; i += 64) {
+      const int q = i / TS, c = i % TS;
+      R va = R(0), vb = R(0);
+      if (q0 + q < P.n_c) {
+        if (k0 + c < P.N) va = (R)((double)x[((size_t)(q0 + q) * P.N + k0 + c) * P.SPC] - cm[(size_t)(k0 + c) * P.SPC]);
+        if (l0 + c < P.N) vb = (R)((double)x[((size_t)(q0 + q) * P.N + l0 + c) * P.SPC] - cm[(size_t)(l0 + c) * P.SPC]);
+      }
+      sa[q][c] = va; sb[q][c] = vb;
+    }
+    __syncthreads();
+#pragma unroll 4
+    for (int q = 0; q < QT; ++q) {
+      R a[4], b[4];
+#pragma unroll
+      for (int u = 0; u < 4; ++u) { a[u] = sa[q][ty * 4 + u]; b[u] = sb[q][tx * 4 + u]; }
+#pragma unroll
+      for (int u = 0; u < 4; ++u)
+#pragma unroll
+        for (int w = 0; w < 4; ++w) acc[u][w] += a[u] * b[w];
+    }
+    __syncthreads();
+  }
+  // Chan merge into the FP64 accumulators (both triangles)
+  const double* mean = P.mean + (size_t)g * row + sl;
+  double* M = P.M + ((size_t)g * P.SPC + sl) * P.N * P.N;
+  const double f = P.cnt > 0 ? (double)P.cnt * (double)P.n_c / (double)(P.cnt + P.n_c) : 0.0;
+#pragma unroll
+  for (int u = 0; u < 4; ++u)
+#pragma unroll
+    for (int w = 0; w < 4; ++w) {
+      const int k = k0 + ty * 4 + u, l = l0 + tx * 4 + w;
+      if (k >= P.N || l >= P.N) continue;
+      if (tk == tl && l < k) continue;
+      double v = (double)acc[u][w];
+      if (P.cnt > 0) {
+        const double dk = cm[(size_t)k * P.SPC] - mean[(size_t)k * P.SPC];
+        const double dl = cm[(size_t)l * P.SPC] - mean[(size_t)l * P.SPC];
+        v += dk * dl * f;
+      }
+      M[(size_t)k * P.N + l] += v;
+      if (k != l) M[(size_t)l * P.N + k] += v;
+    }
+}
+
+// running mean update (after every tile of fc_comoment_kernel has read the old mean)
+template <typename R>
+__global__ void fc_mean_update_kernel(FcParams<R> P) {
+  const int g = blockIdx.y;
+  const int idx = blockIdx.x * blockDim.x + threadIdx.x;
+  const int row = P.N * P.SPC;
+  if (idx >= row) return;
+  const size_t o = (size_t)g * row + idx;
+  if (P.cnt == 0) P.mean[o] = P.cmean[o];
+  else P.mean[o] += (P.cmean[o] - P.mean[o]) * ((double)P.n_c / (double)(P.cnt + P.n_c));
+}
+
+struct ReadoutParams {
+  const double* M;       // [G][SPC][N][N]
+  const double* sums;    // [G][2][N][SPC]
+  const int32_t* loc_id; // [G][SPC]
+  float* fc;             // [n_sims][N][N] or null
+  float* mean_e;         // [n_sims][N] or null
+  float* mean_i;
+  int64_t cnt;
+  int32_t N, SPC, G;
+};
+
+// Pearson finalise (Eq. 6; A18) in local-simulation order
+__global__ void fc_readout_kernel(ReadoutParams P) {
+  const int g = blockIdx.y / P.SPC, sl = blockIdx.y % P.SPC;
+  const int loc = P.loc_id[(size_t)g * P.SPC + sl];
+  if (loc < 0) return;
+  const double* M = P.M + ((size_t)g * P.SPC + sl) * P.N * P.N;
+  const int NN = P.N * P.N;
+  for (int i = blockIdx.x * blockDim.x + threadIdx.x; i < NN; i += gridDim.x * blockDim.x) {
+    const int k = i / P.N, l = i % P.N;
+    if (P.fc) {
+      float r;
+      if (k == l) r = 1.0f;
+      else {
+        const double den = M[(size_t)k * P.N + k] * M[(size_t)l * P.N + l];
+        double v = (den > 0.0 && isfinite(den)) ? M[i] / sqrt(den) : 0.0;
+        r = isfinite(v) ? (float)v : 0.0f;
+      }
+      P.fc[(size_t)loc * NN + i] = r;
+    }
+    if (l == 0 && blockIdx.x * blockDim.x + threadIdx.x < NN) {
+      const size_t row = (size_t)P.N * P.SPC;
+      const double* s = P.sums + (size_t)g * 2 * row + (size_t)k * P.SPC + sl;
+      if (P.mean_e) P.mean_e[(size_t)loc * P.N + k] = (float)(s[0] / (double)P.cnt);
+      if (P.mean_i) P.mean_i[(size_t)loc * P.N + k] = (float)(s[row] / (double)P.cnt);
+    }
+  }
+}
+
+}  // namespace tvbx
