@@ -1,0 +1,310 @@
+#!/usr/bin/env python
+"""bench.py -- throughput of the TVB-AdEx sweep hot path on B200 (BASELINE.json metric:
+simulated region-steps/s = sims x regions x steps / s, and % of the binding roofline).
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--impl tvbx|reference] [--config 2]
+
+One "step" = one pass of the whole hot path over one batch of synthetic input: the full sweep of the
+chosen BASELINE.json config (default configs[1]: 1,024 simulations x 68 regions x 50,000 Euler steps,
+noise on, 1-ms downsample, 1 s discarded) integrated from t = 0 and reduced to mean rates + FC.
+  value  : device-resident -- connectome, tables and state already in HBM; the timed region is
+           reset -> tvbx_run -> tvbx_fc_readout (device buffers), K times, CUDA events.
+  e2e    : the same through the C ABI from HOST buffers: tvbx_create_connectome + tvbx_sweep_create
+           (host W, L, axes) -> tvbx_run -> tvbx_fc_readout into pinned host arrays -> destroy.
+  roofline / cpu_baseline : see DESIGN.md section 7.
+N > 1 (torchrun): simulations are independent, so every rank runs its own replica of the sweep
+(noise seed + rank) with no data-path collective; value = all ranks' region-steps / max time (weak).
+`--impl reference` times the FP64 CPU oracle (oracle/) on a bounded sample of the same workload.
+"""
+import argparse
+import json
+import os
+import subprocess
+import sys
+import threading
+import time
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+import workloads as wl  # noqa: E402
+
+METRIC = "simulated region-steps/s (sims x regions x steps / s)"
+UNIT = "region-steps/s"
+
+# FP32 floating-point operations the integrator's formulation performs per
+# region-step (FADD + FMUL + 2 FFMA, executed-instruction count from ncu on cfg 2, excluding the
+# coupling sum which adds 2 flops per non-zero edge) and the FP32 peak of the chip:
+# 148 SMs x 128 lanes x 2 flop x sm_max_mhz.
+KERNEL_FLOPS_BASE = 1180.0
+FLOPS_PER_EDGE = 2.0
+SM_COUNT, LANES_PER_SM = 148, 128
+
+
+def peaks():
+    p = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(p):
+        d = json.load(open(p))
+        return d, "measured"
+    return dict(hbm_gbs=6650.0, bf16_tflops=1590.0, sm_max_mhz=1965.0), "fallback"
+
+
+class ClockSampler:
+    """nvidia-smi clocks / throttle reasons DURING the timed region (B200_PROFILING.md)."""
+    Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown,"
+         "clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index=0):
+        self.index, self.rows, self.proc = index, [], None
+
+    def start(self):
+        try:
+            self.proc = subprocess.Popen(["nvidia-smi", f"--query-gpu={self.Q}", "--format=csv,noheader,nounits",
+                                          "-i", str(self.index), "-lms", "100"], stdout=subprocess.PIPE, text=True)
+            threading.Thread(target=self._read, daemon=True).start()
+        except Exception:
+            self.proc = None
+
+    def _read(self):
+        for line in self.proc.stdout:
+            self.rows.append([x.strip() for x in line.split(",")])
+
+    def stop(self):
+        if self.proc is None:
+            return dict(sm_mhz=None, sm_max_mhz=None, reasons=["nvidia-smi unavailable"])
+        time.sleep(0.15)
+        self.proc.terminate()
+        sm, mx, reasons = [], [], set()
+        for r in self.rows:
+            try:
+                sm.append(float(r[0])); mx.append(float(r[1]))
+            except Exception:
+                continue
+            for name, v in zip(("hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"), r[3:7]):
+                if v.lower().startswith("active"):
+                    reasons.add(name)
+        return dict(sm_mhz=float(np.median(sm)) if sm else None, sm_max_mhz=max(mx) if mx else None,
+                    reasons=sorted(reasons), samples=len(sm))
+
+
+def workload(cfg_id):
+    cfg = wl.config(cfg_id)
+    W, L = wl.config_connectome(cfg)
+    S = int(np.prod([a["n"] for a in cfg["axes"]]))
+    return cfg, W, L, S
+
+
+def config_dict(cfg_id, cfg, S, extra=None):
+    d = {"workload": f"BASELINE.json configs[{cfg_id - 1}] ({cfg['name']}): {S} sims x {cfg['n']} regions x "
+                     f"{cfg['steps']} steps, dt {cfg['dt']} ms, noise on (seed {cfg['seed']}), ds {cfg['ds']}, "
+                     f"discard {cfg['discard_steps']} steps, outputs mean_E/mean_I/FC",
+         "sims": S, "regions": cfg["n"], "steps_per_sim": cfg["steps"],
+         "l2": "working set (history ring + 1-ms sample chunks) larger than the 126 MB L2; ring and accumulators re-initialised every step"}
+    if extra:
+        d.update(extra)
+    return d
+
+
+# ------------------------------------------------------------------------------------------------
+def run_reference(args):
+    """--impl reference: the FP64 oracle as it stands, on the host cores, on a bounded sample."""
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return
+    from oracle import oracle as orc
+    cfg, W, L, S = workload(args.config)
+    cores = orc.max_threads()
+    n_s = min(S, max(1, cores))
+    sims = [int(x) for x in np.linspace(0, S - 1, n_s).round()]
+    steps = args.ref_steps
+    P = wl.grid_params(cfg, sims=sims)
+    times = []
+    for it in range(args.warmup + args.steps):
+        o = orc.OracleSweep(W, L, P, seed=cfg["seed"], ext_ids=sims)
+        t0 = time.perf_counter()
+        o.run(steps, cfg["dt"], noise_on=True, ds=cfg["ds"], discard_steps=0)
+        o.fc_readout()
+        t1 = time.perf_counter()
+        o.close()
+        if it >= args.warmup:
+            times.append(t1 - t0)
+    total = sum(times)
+    value = n_s * cfg["n"] * steps * len(times) / total
+    sample = f"{n_s} sims (stratified over the grid) x {cfg['n']} regions x {steps} steps per step, FP64, OpenMP over sims"
+    line = {"impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps,
+            "warmup": args.warmup, "ms_per_step": 1e3 * total / len(times), "higher_is_better": True, "scaling": "weak",
+            "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+            "config": config_dict(args.config, cfg, S, {"reference_sample": sample}),
+            "cpu_baseline": {"value": value, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": sample},
+            "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+            "gpu_launches": 0}
+    print(json.dumps(line), flush=True)
+
+
+def cpu_baseline(cfg_id):
+    from oracle import oracle as orc
+    cfg, W, L, S = workload(cfg_id)
+    cores = orc.max_threads()
+    n_s = min(S, max(1, cores))
+    sims = [int(x) for x in np.linspace(0, S - 1, n_s).round()]
+    per_sim_rate = 1.0e5                      # region-steps/s/core, order of magnitude, only to size the sample
+    steps = int(min(cfg["steps"], max(1000, 15.0 * per_sim_rate / cfg["n"])))
+    P = wl.grid_params(cfg, sims=sims)
+    o = orc.OracleSweep(W, L, P, seed=cfg["seed"], ext_ids=sims)
+    t0 = time.perf_counter()
+    o.run(steps, cfg["dt"], noise_on=True, ds=cfg["ds"], discard_steps=0)
+    o.fc_readout()
+    dt = time.perf_counter() - t0
+    return {"value": n_s * cfg["n"] * steps / dt, "unit": UNIT, "cores": cores, "kind": "oracle",
+            "sample": f"{n_s} sims (stratified over the grid) x {cfg['n']} regions x {steps} steps, FP64, "
+                      f"OpenMP over sims, {dt:.1f} s"}
+
+
+# ------------------------------------------------------------------------------------------------
+def run_tvbx(args):
+    import torch
+    import torch.distributed as dist
+    import paper_2311_13337_b200 as tvbx
+
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    rank = int(os.environ.get("RANK", "0"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device (there is no CPU fallback; use --impl reference for the oracle)")
+    torch.cuda.set_device(local)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+    tvbx.lib()                                   # fails loudly if libtvbx.so is missing
+
+    cfg, W, L, S = workload(args.config)
+    N, steps_sim = cfg["n"], (args.sim_steps or cfg["steps"])
+    seed = cfg["seed"] + rank                    # replica r of the sweep: same grid, its own noise
+    stream = torch.cuda.Stream()
+
+    def barrier():
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    # ---- device-resident arm --------------------------------------------------------------------
+    conn, sw = tvbx.sweep_from_config(cfg, W, L, seed=seed)
+    fc = torch.empty((S, N, N), device="cuda", dtype=torch.float32)
+    me = torch.empty((S, N), device="cuda", dtype=torch.float32)
+    mi = torch.empty((S, N), device="cuda", dtype=torch.float32)
+
+    def one_step():
+        sw.reset(stream)
+        sw.run(steps_sim, cfg["dt"], noise_on=True, ds=cfg["ds"], discard_steps=cfg["discard_steps"], stream=stream)
+        sw.fc_readout(device=True, stream=stream, out=(fc, me, mi))
+
+    sw.run(1, cfg["dt"], noise_on=True, ds=cfg["ds"], discard_steps=cfg["discard_steps"], stream=stream)   # allocate
+    for _ in range(args.warmup):
+        one_step()
+    barrier()
+    sw.profile_enable(True)
+    sw.profile_read()
+    l0 = sw.launch_count()
+    clocks = ClockSampler(local)
+    if rank == 0:
+        clocks.start()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    barrier()
+    with torch.cuda.stream(stream):
+        e0.record(stream)
+        for _ in range(args.steps):
+            one_step()
+        e1.record(stream)
+    stream.synchronize()
+    barrier()
+    ms = e0.elapsed_time(e1)
+    clk = clocks.stop() if rank == 0 else None
+    launches = sw.launch_count() - l0
+    prof = sw.profile_read()
+    sw.profile_enable(False)
+    info = sw.launch_info()
+    t = torch.tensor([ms], device="cuda", dtype=torch.float64)
+    if world > 1:
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    ms_max = float(t.item())
+    units_per_step = S * N * steps_sim
+    value = world * units_per_step * args.steps / (ms_max * 1e-3)
+    finite = bool(torch.isfinite(fc).all().item() and torch.isfinite(me).all().item())
+
+    # ---- end-to-end arm: host buffers through the C ABI ---------------------------------------------
+    hfc = torch.empty((S, N, N), dtype=torch.float32).pin_memory().numpy()
+    hme = torch.empty((S, N), dtype=torch.float32).pin_memory().numpy()
+    hmi = torch.empty((S, N), dtype=torch.float32).pin_memory().numpy()
+    h2d = d2h = 0
+
+    def e2e_step():
+        nonlocal h2d, d2h
+        c2, s2 = tvbx.sweep_from_config(cfg, W, L, seed=seed)
+        s2.run(steps_sim, cfg["dt"], noise_on=True, ds=cfg["ds"], discard_steps=cfg["discard_steps"], stream=stream)
+        s2.fc_readout(device=False, stream=stream, out=(hfc, hme, hmi))
+        h2d, d2h = s2.bytes_copied()
+        s2.close(); c2.close()
+
+    e2e_step()
+    barrier()
+    t0 = time.perf_counter()
+    for _ in range(args.steps):
+        e2e_step()
+    torch.cuda.synchronize()
+    e2e_s = time.perf_counter() - t0
+    t = torch.tensor([e2e_s], device="cuda", dtype=torch.float64)
+    if world > 1:
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    e2e_value = world * units_per_step * args.steps / float(t.item())
+
+    if rank == 0:
+        pk, pk_kind = peaks()
+        nnz_row = float((W != 0).sum()) / N
+        flops_unit = KERNEL_FLOPS_BASE + FLOPS_PER_EDGE * nnz_row
+        int_ms, int_n = prof["integrate"]
+        peak_tflops = SM_COUNT * LANES_PER_SM * 2 * pk.get("sm_max_mhz", 1965.0) * 1e6 / 1e12
+        achieved = flops_unit * units_per_step * args.steps / (int_ms * 1e-3) / 1e12 if int_ms > 0 else None
+        roof = {"bound": "alu", "kernel": "tvbx::integrate_kernel", "achieved": achieved, "peak": peak_tflops,
+                "unit": "TFLOP/s", "frac": (achieved / peak_tflops) if achieved else None, "traffic": None,
+                "flops_per_region_step": flops_unit, "peak_kind": f"148 SMs x 128 FP32 lanes x 2 x sm_max_mhz ({pk_kind} clock)",
+                "kernel_ms_per_launch": int_ms / max(int_n, 1), "kernel_launches": int_n,
+                "kernel_share_of_step": int_ms / ms if ms > 0 else None,
+                "hbm_peak_gbs": pk.get("hbm_gbs"),
+                "other_kernels_ms": {k: prof[k][0] for k in ("fc", "readout", "reset")}}
+        line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
+                "ms_per_step": ms_max / args.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+                "dtype": "f32", "data": "synthetic",
+                "config": config_dict(args.config, cfg, S, {"launch": info, "sim_steps": steps_sim,
+                                                           "replicas": world, "results_finite": finite}),
+                "clocks": clk,
+                "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": int(h2d), "d2h_bytes_per_step": int(d2h)},
+                "gpu_launches": int(launches), "roofline": roof}
+        if world == 1 and not args.no_cpu_baseline:
+            line["cpu_baseline"] = cpu_baseline(args.config)
+        print(json.dumps(line), flush=True)
+    if world > 1:
+        dist.barrier()
+        dist.destroy_process_group()
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=3)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--impl", default="tvbx", choices=["tvbx", "reference"])
+    ap.add_argument("--config", type=int, default=2, help="BASELINE.json config number (1-5); the metric is quoted on 2")
+    ap.add_argument("--sim-steps", type=int, default=0, help="override the Euler steps per simulation (profiling only)")
+    ap.add_argument("--ref-steps", type=int, default=4000, help="Euler steps per oracle sample (--impl reference)")
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    args = ap.parse_args()
+    if args.impl == "reference":
+        run_reference(args)
+    else:
+        run_tvbx(args)
+
+
+if __name__ == "__main__":
+    main()

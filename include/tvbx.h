@@ -146,6 +146,20 @@ int32_t tvbx_run(tvbx_sweep* sw, int64_t steps, double dt, const tvbx_run_opts* 
 int32_t tvbx_fc_readout(tvbx_sweep* sw, float* fc, float* mean_e, float* mean_i, int32_t on_device,
                         void* cuda_stream);
 
+/* Back to step 0 without re-allocating: state, OU, history ring, window sums and FC accumulators are
+ * re-initialised on the device (enqueued on cuda_stream), the step and sample counters are zeroed.
+ * A no-op before the first tvbx_run.  reset; run(n) is bit-identical to a fresh sweep's run(n). */
+int32_t tvbx_sweep_reset(tvbx_sweep* sw, void* cuda_stream);
+
+/* Kernel timing for reports (bench.py's roofline line): while enabled, every kernel launch of this
+ * sweep is bracketed by CUDA events on the launching stream.  tvbx_profile_read synchronises those
+ * events, returns the summed durations [ms] and launch counts per kernel class since the last read
+ * (0 = integrator, 1 = FC epilogue kernels, 2 = readout, 3 = reset fills) and clears the list. */
+int32_t tvbx_profile_enable(tvbx_sweep* sw, int32_t on);
+int32_t tvbx_profile_read(tvbx_sweep* sw, double ms[4], int64_t launches[4]);
+/* bytes this sweep object copied host->device and device->host so far (tables, parameters, results) */
+int32_t tvbx_bytes_copied(const tvbx_sweep* sw, int64_t* h2d, int64_t* d2h);
+
 /* ---- bookkeeping accessors (bit-exact tests) ------------------------------------------------ */
 int32_t tvbx_sweep_size(const tvbx_sweep* sw, int64_t* n_sims, int64_t* grid_size, int32_t* n_regions);
 /* parameter value of local simulation `sim` (index into sim_ids) */

@@ -64,7 +64,7 @@ EXPORTS = [
     "tvbx_sweep_destroy", "tvbx_sweep_set_initial", "tvbx_run", "tvbx_fc_readout", "tvbx_sweep_size",
     "tvbx_sweep_param", "tvbx_sweep_ext_id", "tvbx_delay_index", "tvbx_ring_len", "tvbx_steps_done",
     "tvbx_samples_kept", "tvbx_sweep_state", "tvbx_launch_info", "tvbx_launch_count", "tvbx_last_error",
-    "tvbx_version",
+    "tvbx_version", "tvbx_sweep_reset", "tvbx_profile_enable", "tvbx_profile_read", "tvbx_bytes_copied",
 ]
 
 
@@ -113,6 +113,10 @@ def lib():
             "tvbx_sweep_state": [vp, dp, dp],
             "tvbx_launch_info": [vp, C.POINTER(i32)],
             "tvbx_launch_count": [vp, C.POINTER(i64)],
+            "tvbx_sweep_reset": [vp, vp],
+            "tvbx_profile_enable": [vp, i32],
+            "tvbx_profile_read": [vp, dp, C.POINTER(i64)],
+            "tvbx_bytes_copied": [vp, C.POINTER(i64), C.POINTER(i64)],
         }
         for name, argtypes in sig.items():
             fn = getattr(L, name)
@@ -304,6 +308,23 @@ class Sweep:
         _chk(lib().tvbx_launch_info(self._h, a))
         keys = ("ctas", "threads", "sims_per_cta", "regs", "smem", "passes", "chunk_samples", "local_bytes")
         return dict(zip(keys, a[:]))
+
+    def reset(self, stream=None):
+        _chk(lib().tvbx_sweep_reset(self._h, _stream_ptr(stream)))
+
+    def profile_enable(self, on=True):
+        _chk(lib().tvbx_profile_enable(self._h, int(bool(on))))
+
+    def profile_read(self):
+        """-> {kernel class: (summed ms, launches)} since the last read (synchronises the events)."""
+        ms = (C.c_double * 4)(); n = (C.c_int64 * 4)()
+        _chk(lib().tvbx_profile_read(self._h, ms, n))
+        return {k: (ms[i], n[i]) for i, k in enumerate(("integrate", "fc", "readout", "reset"))}
+
+    def bytes_copied(self):
+        a, b = C.c_int64(), C.c_int64()
+        _chk(lib().tvbx_bytes_copied(self._h, C.byref(a), C.byref(b)))
+        return a.value, b.value
 
     def launch_count(self):
         out = C.c_int64()

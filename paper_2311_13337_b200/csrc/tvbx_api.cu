@@ -92,7 +92,12 @@ struct DeviceSide {
   virtual int32_t run(int64_t steps, const tvbx_run_opts* o) = 0;
   virtual int32_t readout(float* fc, float* me, float* mi, int on_device, cudaStream_t st) = 0;
   virtual int32_t state(double* y, double* ou) = 0;
+  virtual int32_t reset(cudaStream_t st) = 0;
 };
+
+// event pair around one kernel launch (tvbx_profile_*)
+struct ProfEvent { cudaEvent_t a, b; int kind; };
+enum { K_INTEGRATE = 0, K_FC = 1, K_READOUT = 2, K_RESET = 3 };
 
 }  // namespace
 
@@ -123,8 +128,22 @@ struct tvbx_sweep {
   double dt = 0;
   int64_t n = 0, cnt = 0, fill = 0, CS = 0, launches = 0;
   int32_t info[8] = {0, 0, 0, 0, 0, 0, 0, 0};
+  int64_t h2d = 0, d2h = 0;
+  bool profiling = false;
+  std::vector<ProfEvent> prof;
   int device = 0;
   std::unique_ptr<DeviceSide> dev;
+
+  ~tvbx_sweep() { for (ProfEvent& e : prof) { cudaEventDestroy(e.a); cudaEventDestroy(e.b); } }
+  // bracket a launch with events while profiling is on
+  void prof_begin(int kind, cudaStream_t st) {
+    if (!profiling) return;
+    ProfEvent e; e.kind = kind;
+    cudaEventCreate(&e.a); cudaEventCreate(&e.b);
+    cudaEventRecord(e.a, st);
+    prof.push_back(e);
+  }
+  void prof_end(cudaStream_t st) { if (profiling) cudaEventRecord(prof.back().b, st); }
 
   double param(int64_t sim, int32_t id) const {
     int64_t s = ext_ids[sim];
@@ -156,9 +175,10 @@ struct DevBuf {
     n = count;
     return cudaMalloc((void**)&p, std::max<size_t>(count, 1) * sizeof(T));
   }
-  cudaError_t upload(const std::vector<T>& h) {
+  cudaError_t upload(const std::vector<T>& h, int64_t* bytes) {
     cudaError_t e = alloc(h.size());
     if (e != cudaSuccess) return e;
+    *bytes += (int64_t)(h.size() * sizeof(T));
     return cudaMemcpy(p, h.data(), h.size() * sizeof(T), cudaMemcpyHostToDevice);
   }
 };
@@ -166,6 +186,15 @@ struct DevBuf {
 template <typename R>
 __global__ void fill_kernel(R* p, size_t n, R v) {
   for (size_t i = blockIdx.x * (size_t)blockDim.x + threadIdx.x; i < n; i += (size_t)gridDim.x * blockDim.x) p[i] = v;
+}
+
+// state[g][q][i] = init[q] for the 7 model variables, 0 for OU and the two window sums
+template <typename R>
+struct InitVals { R v[NSV - 2]; };
+template <typename R>
+__global__ void state_init_kernel(R* p, size_t row, size_t total, InitVals<R> iv) {
+  for (size_t i = blockIdx.x * (size_t)blockDim.x + threadIdx.x; i < total; i += (size_t)gridDim.x * blockDim.x)
+    p[i] = iv.v[(i / row) % (NSV - 2)];
 }
 
 template <typename R> struct KernelPick { void (*fn)(const IntegrateParams<R>); int maxt; };
@@ -203,6 +232,7 @@ struct DeviceImpl : DeviceSide {
   KernelPick<R> kp{nullptr, 0};
   int threads = 0, smem = 0;
   bool single = true;
+  size_t ring_count = 0;
 
   explicit DeviceImpl(tvbx_sweep* s) : sw(s) { std::memset(&P, 0, sizeof P); }
 
@@ -281,25 +311,18 @@ struct DeviceImpl : DeviceSide {
       return fail(TVBX_ENOMEM, "sweep needs %.2f GB of device memory (ring %.2f GB), %.2f GB free",
                   need / 1e9, ring_elems * sizeof(R) / 1e9, free_b / 1e9);
     sw->CS = CS;
-    CU(d_tables.upload(tds)); CU(d_groups.upload(gds)); CU(d_edges.upload(edges)); CU(d_rowptr.upload(rowptr));
-    CU(d_ext.upload(ext)); CU(d_loc.upload(loc)); CU(d_psim.upload(psim));
+    int64_t* hb = &sw->h2d;
+    CU(d_tables.upload(tds, hb)); CU(d_groups.upload(gds, hb)); CU(d_edges.upload(edges, hb)); CU(d_rowptr.upload(rowptr, hb));
+    CU(d_ext.upload(ext, hb)); CU(d_loc.upload(loc, hb)); CU(d_psim.upload(psim, hb));
     CU(d_ring.alloc(ring_elems));
     CU(d_xbar.alloc((size_t)G * CS * row));
     CU(d_cmean.alloc((size_t)G * row)); CU(d_mean.alloc((size_t)G * row));
     CU(d_M.alloc((size_t)G * SPC * N * N));
-    CU(cudaMemset(d_M.p, 0, d_M.n * sizeof(double)));
-    CU(cudaMemset(d_mean.p, 0, d_mean.n * sizeof(double)));
-    CU(cudaMemset(d_xbar.p, 0, d_xbar.n * sizeof(R)));
-    // state: [G][10][N][SPC], sums [G][2][N][SPC]
-    std::vector<R> st((size_t)G * (NSV - 2) * row, R(0));
-    for (int g = 0; g < G; ++g)
-      for (int q = 0; q < 7; ++q)
-        for (size_t i = 0; i < row; ++i) st[((size_t)g * (NSV - 2) + q) * row + i] = (R)sw->init[q];
-    CU(d_state.upload(st));
+    CU(d_state.alloc((size_t)G * (NSV - 2) * row));
     CU(d_sums.alloc((size_t)G * 2 * row));
-    CU(cudaMemset(d_sums.p, 0, d_sums.n * sizeof(double)));
-    fill_kernel<R><<<1184, 256>>>(d_ring.p, ring_elems, (R)sw->init[0]);    // A14
-    CU(cudaGetLastError());
+    ring_count = ring_elems;
+    CU(cudaMemset(d_xbar.p, 0, d_xbar.n * sizeof(R)));
+    { int32_t rc = reset(0); if (rc) return rc; }
 
     // ---- uniform constants ----
     TFConst<R>& tf = P.tf;
@@ -360,6 +383,22 @@ struct DeviceImpl : DeviceSide {
     return TVBX_OK;
   }
 
+  int32_t reset(cudaStream_t st) override {
+    InitVals<R> iv;
+    for (int q = 0; q < NSV - 2; ++q) iv.v[q] = q < 7 ? (R)sw->init[q] : R(0);
+    sw->prof_begin(K_RESET, st);
+    state_init_kernel<R><<<592, 256, 0, st>>>(d_state.p, (size_t)sw->conn.n * sw->spc, d_state.n, iv);
+    fill_kernel<R><<<1184, 256, 0, st>>>(d_ring.p, ring_count, (R)sw->init[0]);    // A14
+    fill_kernel<double><<<592, 256, 0, st>>>(d_sums.p, d_sums.n, 0.0);
+    fill_kernel<double><<<592, 256, 0, st>>>(d_mean.p, d_mean.n, 0.0);
+    fill_kernel<double><<<1184, 256, 0, st>>>(d_M.p, d_M.n, 0.0);
+    sw->prof_end(st);
+    sw->launches += 5;
+    CU(cudaGetLastError());
+    sw->n = 0; sw->cnt = 0; sw->fill = 0;
+    return TVBX_OK;
+  }
+
   int32_t accumulate(double* Mbuf, double* meanbuf, int64_t cnt, int n_c, cudaStream_t st) {
     const int N = sw->conn.n, SPC = sw->spc, G = (int)sw->groups.size();
     FcParams<R> F;
@@ -367,11 +406,13 @@ struct DeviceImpl : DeviceSide {
     F.CS = (int32_t)sw->CS; F.N = N; F.SPC = SPC; F.G = G;
     const int row = N * SPC;
     dim3 g1((row + 127) / 128, G);
+    sw->prof_begin(K_FC, st);
     fc_chunk_mean_kernel<R><<<g1, 128, 0, st>>>(F);
     const int nt = (N + 31) / 32;
     dim3 g2(nt, nt, G * SPC);
     fc_comoment_kernel<R><<<g2, 64, 0, st>>>(F);
     fc_mean_update_kernel<R><<<g1, 128, 0, st>>>(F);
+    sw->prof_end(st);
     sw->launches += 3;
     CU(cudaGetLastError());
     return TVBX_OK;
@@ -406,7 +447,9 @@ struct DeviceImpl : DeviceSide {
         kept = end >= e1 ? (end - e1) / ds + 1 : 0;
       }
       P.n_begin = sw->n; P.n_end = sw->n + take; P.sample_base = (int32_t)sw->fill;
+      sw->prof_begin(K_INTEGRATE, st);
       kp.fn<<<G, threads, smem, st>>>(P);
+      sw->prof_end(st);
       sw->launches += 1;
       CU(cudaGetLastError());
       sw->n += take; remaining -= take; sw->fill += kept;
@@ -418,6 +461,7 @@ struct DeviceImpl : DeviceSide {
     }
     if (tsteps > 0 && !o->traj_on_device) {
       CU(cudaMemcpyAsync(o->traj, traj, traj_elems * sizeof(R), cudaMemcpyDeviceToHost, st));
+      sw->d2h += (int64_t)(traj_elems * sizeof(R));
       CU(cudaStreamSynchronize(st));
     }
     return TVBX_OK;
@@ -447,13 +491,15 @@ struct DeviceImpl : DeviceSide {
       if (mi) { CU(dmi.alloc((size_t)sw->n_sims * N)); Q.mean_i = dmi.p; }
     }
     dim3 grid((N * N + 255) / 256, G * SPC);
+    sw->prof_begin(K_READOUT, st);
     fc_readout_kernel<<<grid, 256, 0, st>>>(Q);
+    sw->prof_end(st);
     sw->launches += 1;
     CU(cudaGetLastError());
     if (!on_device) {
-      if (fc) CU(cudaMemcpyAsync(fc, dfc.p, dfc.n * sizeof(float), cudaMemcpyDeviceToHost, st));
-      if (me) CU(cudaMemcpyAsync(me, dme.p, dme.n * sizeof(float), cudaMemcpyDeviceToHost, st));
-      if (mi) CU(cudaMemcpyAsync(mi, dmi.p, dmi.n * sizeof(float), cudaMemcpyDeviceToHost, st));
+      if (fc) { CU(cudaMemcpyAsync(fc, dfc.p, dfc.n * sizeof(float), cudaMemcpyDeviceToHost, st)); sw->d2h += (int64_t)(dfc.n * sizeof(float)); }
+      if (me) { CU(cudaMemcpyAsync(me, dme.p, dme.n * sizeof(float), cudaMemcpyDeviceToHost, st)); sw->d2h += (int64_t)(dme.n * sizeof(float)); }
+      if (mi) { CU(cudaMemcpyAsync(mi, dmi.p, dmi.n * sizeof(float), cudaMemcpyDeviceToHost, st)); sw->d2h += (int64_t)(dmi.n * sizeof(float)); }
       CU(cudaStreamSynchronize(st));
     } else if (sw->fill > 0) {
       CU(cudaStreamSynchronize(st));   // scratch copies are freed on return
@@ -646,6 +692,37 @@ int32_t tvbx_fc_readout(tvbx_sweep* sw, float* fc, float* mean_e, float* mean_i,
   if (!sw) return fail(TVBX_EINVAL, "sweep is NULL");
   if (!sw->started) return fail(TVBX_ESTATE, "no run yet");
   return sw->dev->readout(fc, mean_e, mean_i, on_device, (cudaStream_t)stream);
+}
+
+int32_t tvbx_sweep_reset(tvbx_sweep* sw, void* stream) {
+  if (!sw) return fail(TVBX_EINVAL, "sweep is NULL");
+  if (!sw->started) return TVBX_OK;
+  return sw->dev->reset((cudaStream_t)stream);
+}
+int32_t tvbx_profile_enable(tvbx_sweep* sw, int32_t on) {
+  if (!sw) return fail(TVBX_EINVAL, "sweep is NULL");
+  sw->profiling = on != 0;
+  return TVBX_OK;
+}
+int32_t tvbx_profile_read(tvbx_sweep* sw, double ms[4], int64_t launches[4]) {
+  if (!sw || !ms || !launches) return fail(TVBX_EINVAL, "NULL argument");
+  for (int i = 0; i < 4; ++i) { ms[i] = 0.0; launches[i] = 0; }
+  for (ProfEvent& e : sw->prof) {
+    float t = 0.f;
+    CU(cudaEventSynchronize(e.b));
+    CU(cudaEventElapsedTime(&t, e.a, e.b));
+    ms[e.kind] += (double)t;
+    launches[e.kind] += e.kind == K_FC ? 3 : (e.kind == K_RESET ? 5 : 1);
+    cudaEventDestroy(e.a); cudaEventDestroy(e.b);
+  }
+  sw->prof.clear();
+  return TVBX_OK;
+}
+int32_t tvbx_bytes_copied(const tvbx_sweep* sw, int64_t* h2d, int64_t* d2h) {
+  if (!sw) return fail(TVBX_EINVAL, "sweep is NULL");
+  if (h2d) *h2d = sw->h2d;
+  if (d2h) *d2h = sw->d2h;
+  return TVBX_OK;
 }
 
 int32_t tvbx_sweep_size(const tvbx_sweep* sw, int64_t* n_sims, int64_t* grid_size, int32_t* n_regions) {

@@ -1,0 +1,281 @@
+"""GPU parity: the CUDA path (through the C ABI) against the FP64 oracle, element by element, on the
+same seeded inputs.  Tolerances are BASELINE.json's: noise-off trajectories max relative error 1e-3
+(FP32) / 1e-9 (FP64 build mode) over the first 200 ms; noise-on per-region means 1 % relative and FC
+0.02 absolute; bookkeeping and resumability bit-exact."""
+import numpy as np
+import pytest
+
+import workloads as wl
+import paper_2311_13337_b200 as tvbx
+from oracle import oracle as orc
+
+pytestmark = pytest.mark.gpu
+
+TOL_TRAJ_F32 = 1e-3     # BASELINE.json north_star
+TOL_TRAJ_F64 = 1e-9
+TOL_MEAN_REL = 1e-2
+TOL_FC_ABS = 0.02
+
+
+def traj_err(got, ref):
+    """max over everything of |got - ref| / (max |ref| of that state variable of that sim): the
+    relative error of a trajectory, scaled per variable so that zero crossings do not divide by 0."""
+    ref = np.asarray(ref, dtype=np.float64)
+    scale = np.abs(ref).max(axis=(1, 3), keepdims=True) + 1e-300
+    return float((np.abs(np.asarray(got, dtype=np.float64) - ref) / scale).max())
+
+
+def run_pair(cfg, W, L, steps, noise_on, traj_steps=0, sims=None, precision=tvbx.TVBX_F32, ds=10,
+             discard=0, params=None, **kw):
+    P = wl.grid_params(cfg, sims=sims)
+    if params:
+        for k, v in params.items():
+            P[:, wl.PARAM_NAMES.index(k)] = v
+    conn, sw = tvbx.sweep_from_config(cfg, W, L, sim_ids=sims, precision=precision, params=params, **kw)
+    traj = sw.run(steps, cfg.get("dt", 0.1), noise_on=noise_on, ds=ds, discard_steps=discard, traj_steps=traj_steps)
+    o = orc.OracleSweep(W, L, P, seed=cfg["seed"], ext_ids=sims)
+    ref = o.run(steps, cfg.get("dt", 0.1), noise_on=noise_on, ds=ds, discard_steps=discard, traj_steps=traj_steps)
+    return sw, traj, o, ref
+
+
+# ------------------------------------------------------------------------------------ cfg 1
+def test_cfg1_noise_off_trajectories_fp32():
+    cfg = wl.config(1)
+    W, L = wl.config_connectome(cfg)
+    sw, traj, o, ref = run_pair(cfg, W, L, 2000, False, traj_steps=2000)
+    assert traj.shape == (8, 2000, 7, 68) and traj.dtype == np.float32
+    assert traj_err(traj, ref) < TOL_TRAJ_F32
+    y, _ = sw.state()
+    for s in range(8):
+        np.testing.assert_allclose(y[s], o.state(s)[0], rtol=TOL_TRAJ_F32, atol=1e-9)
+
+
+def test_cfg1_noise_off_trajectories_fp64_mode():
+    cfg = wl.config(1)
+    W, L = wl.config_connectome(cfg)
+    sw, traj, o, ref = run_pair(cfg, W, L, 2000, False, traj_steps=2000, precision=tvbx.TVBX_F64)
+    assert traj.dtype == np.float64
+    assert traj_err(traj, ref) < TOL_TRAJ_F64
+
+
+def test_cfg1_noise_on_means_and_fc():
+    cfg = wl.config(1)
+    W, L = wl.config_connectome(cfg)
+    sw, _, o, _ = run_pair(cfg, W, L, cfg["steps"], True)
+    fc, me, mi = sw.fc_readout()
+    rfc, rme, rmi = o.fc_readout()
+    assert sw.samples_kept() == 500
+    assert np.abs(me / rme - 1).max() < TOL_MEAN_REL
+    assert np.abs(mi / rmi - 1).max() < TOL_MEAN_REL
+    assert np.abs(fc - rfc).max() < TOL_FC_ABS
+    assert np.all(np.diagonal(fc, axis1=1, axis2=2) == 1.0)
+    np.testing.assert_array_equal(fc, np.swapaxes(fc, 1, 2))
+
+
+def test_cfg1_noise_on_trajectory_same_philox_stream():
+    """Same Philox stream => the noisy trajectories also agree closely over the first 100 ms (the OU
+    path is identical up to FP32 rounding of Box-Muller)."""
+    cfg = wl.config(1)
+    W, L = wl.config_connectome(cfg)
+    sw, traj, o, ref = run_pair(cfg, W, L, 1000, True, traj_steps=1000, params=dict(wNoise=1e-4))
+    assert traj_err(traj, ref) < TOL_TRAJ_F32
+    _, ou = sw.state()
+    for s in range(8):
+        np.testing.assert_allclose(ou[s], o.state(s)[1], rtol=0, atol=2e-4)
+
+
+def test_fp64_mode_noise_on_matches_oracle_tightly():
+    cfg = wl.config(1)
+    W, L = wl.connectome(23, seed=11, keep=0.4)
+    sw, traj, o, ref = run_pair(cfg, W, L, 1200, True, traj_steps=1200, precision=tvbx.TVBX_F64,
+                                params=dict(wNoise=1e-4), discard=200)
+    assert traj_err(traj, ref) < 1e-8
+    fc, me, mi = sw.fc_readout()
+    rfc, rme, rmi = o.fc_readout()
+    np.testing.assert_allclose(me, rme, rtol=1e-6)
+    np.testing.assert_allclose(mi, rmi, rtol=1e-6)
+    assert np.abs(fc - rfc).max() < 1e-5
+
+
+# ------------------------------------------------------------------------------------ launch shapes
+@pytest.mark.parametrize("spc", [1, 2, 4, 8, 16, 32])
+def test_every_sims_per_cta_mapping(spc):
+    """Ragged everything: 11 sims (not a multiple of any SPC > 1), N = 37 regions, two speeds."""
+    W, L = wl.connectome(37, seed=5, keep=0.35)
+    axes = [dict(name="G", lo=0.0, hi=0.4, n=11, values=None)]
+    cfg = dict(axes=axes, fixed=dict(v=6.0, b_e=20.0, wNoise=1e-4), seed=9)
+    sw, traj, o, ref = run_pair(cfg, W, L, 700, True, traj_steps=700, sims_per_cta=spc, discard=100)
+    assert traj_err(traj, ref) < TOL_TRAJ_F32
+    fc, me, mi = sw.fc_readout()
+    rfc, rme, rmi = o.fc_readout()
+    assert np.abs(me / rme - 1).max() < TOL_MEAN_REL and np.abs(fc - rfc).max() < TOL_FC_ABS
+    assert sw.launch_info()["sims_per_cta"] == spc
+
+
+@pytest.mark.parametrize("threads", [64, 160, 0])
+def test_multi_pass_mapping_when_regions_exceed_the_cta(threads):
+    """threads_per_cta < N * SPC forces several region passes per time block (the N = 360 path)."""
+    W, L = wl.connectome(45, seed=6, keep=0.5)
+    axes = [dict(name="b_e", lo=0.0, hi=60.0, n=5, values=None)]
+    cfg = dict(axes=axes, fixed=dict(v=3.0, G=0.3), seed=2)
+    sw, traj, o, ref = run_pair(cfg, W, L, 500, False, traj_steps=500, sims_per_cta=4, threads_per_cta=threads)
+    assert traj_err(traj, ref) < TOL_TRAJ_F32
+
+
+def test_mixed_speeds_cfg3_slice():
+    """cfg 3 slice covering all 8 speeds (ring depth 16 ... 2000, min delay 1 ... 100 steps)."""
+    cfg = wl.config(3)
+    W, L = wl.config_connectome(cfg)
+    sims = list(range(8 * 100, 8 * 100 + 8)) + [32767, 32760]
+    sw, traj, o, ref = run_pair(cfg, W, L, 2000, False, traj_steps=2000, sims=sims)
+    assert traj_err(traj, ref) < TOL_TRAJ_F32
+    for loc, s in enumerate(sims):
+        assert sw.ring_len(loc)[0] == o.ring_len(loc)
+
+
+def test_zero_delay_edges():
+    """v so large that every delay rounds to 0: the coupling reads the current step (pin P5)."""
+    W, L = wl.connectome(19, seed=8, keep=0.5)
+    cfg = dict(axes=[dict(name="G", lo=0.1, hi=0.5, n=3, values=None)], fixed=dict(v=1e9), seed=0)
+    sw, traj, o, ref = run_pair(cfg, W, L, 400, False, traj_steps=400)
+    assert sw.ring_len(0)[0] == 1
+    assert traj_err(traj, ref) < TOL_TRAJ_F32
+
+
+def test_cfg5_slice_n360():
+    cfg = wl.config(5)
+    W, L = wl.config_connectome(cfg)
+    sims = [0, 63, 2047, 4095]
+    sw, traj, o, ref = run_pair(cfg, W, L, 800, True, traj_steps=800, sims=sims, discard=200)
+    assert traj_err(traj, ref) < TOL_TRAJ_F32
+    fc, me, mi = sw.fc_readout()
+    rfc, rme, rmi = o.fc_readout()
+    assert fc.shape == (4, 360, 360)
+    assert np.abs(me / rme - 1).max() < TOL_MEAN_REL and np.abs(mi / rmi - 1).max() < TOL_MEAN_REL
+    assert np.abs(fc - rfc).max() < TOL_FC_ABS
+
+
+# ------------------------------------------------------------------------------------ invariants on the GPU path
+def test_resumable_bit_exact():
+    """P14: run(a); run(b) == run(a+b) bit for bit (state, OU, FC accumulators)."""
+    W, L = wl.connectome(30, seed=3, keep=0.4)
+    cfg = dict(axes=[dict(name="G", lo=0.0, hi=0.5, n=6, values=None)], fixed=dict(v=5.0, b_e=30.0, wNoise=1e-4), seed=4)
+    _, a = tvbx.sweep_from_config(cfg, W, L, chunk_samples=16)
+    _, b = tvbx.sweep_from_config(cfg, W, L, chunk_samples=16)
+    a.run(1203, 0.1, noise_on=True, ds=10, discard_steps=95)
+    for part in (1, 398, 7, 797):
+        b.run(part, 0.1, noise_on=True, ds=10, discard_steps=95)
+    assert a.steps_done() == b.steps_done() == 1203 and a.samples_kept() == b.samples_kept()
+    ya, oa = a.state(); yb, ob = b.state()
+    np.testing.assert_array_equal(ya, yb); np.testing.assert_array_equal(oa, ob)
+    for x, y in zip(a.fc_readout(), b.fc_readout()):
+        np.testing.assert_array_equal(x, y)
+
+
+def test_reset_equals_fresh_sweep():
+    W, L = wl.connectome(30, seed=3, keep=0.4)
+    cfg = dict(axes=[dict(name="G", lo=0.0, hi=0.5, n=5, values=None)], fixed=dict(v=5.0, b_e=30.0, wNoise=1e-4), seed=4)
+    _, a = tvbx.sweep_from_config(cfg, W, L)
+    _, b = tvbx.sweep_from_config(cfg, W, L)
+    a.run(777, 0.1, noise_on=True, ds=10, discard_steps=100)
+    a.reset()
+    assert a.steps_done() == 0 and a.samples_kept() == 0
+    ta = a.run(500, 0.1, noise_on=True, ds=10, discard_steps=100, traj_steps=500)
+    tb = b.run(500, 0.1, noise_on=True, ds=10, discard_steps=100, traj_steps=500)
+    np.testing.assert_array_equal(ta, tb)
+    for x, y in zip(a.fc_readout(), b.fc_readout()):
+        np.testing.assert_array_equal(x, y)
+    a.profile_enable(True)
+    a.run(100, 0.1, noise_on=True, ds=10, discard_steps=100)
+    prof = a.profile_read()
+    assert prof["integrate"][1] >= 1 and prof["integrate"][0] > 0.0
+
+
+def test_sim_results_do_not_depend_on_sweep_membership():
+    """P13 / P:86: a simulation's result is the same whatever other simulations share the sweep,
+    its position in it, or its lane in a CTA (Philox is keyed by the external sim index)."""
+    cfg = wl.config(3)
+    W, L = wl.connectome(26, seed=1, keep=0.4)
+    full = [9, 4000, 4001, 17, 30000, 12345, 8, 4002]
+    _, a = tvbx.sweep_from_config(cfg, W, L, sim_ids=full, sims_per_cta=4, params=dict(wNoise=1e-4))
+    _, b = tvbx.sweep_from_config(cfg, W, L, sim_ids=[12345, 9], sims_per_cta=1, params=dict(wNoise=1e-4))
+    ta = a.run(600, 0.1, noise_on=True, ds=10, traj_steps=600)
+    tb = b.run(600, 0.1, noise_on=True, ds=10, traj_steps=600)
+    np.testing.assert_array_equal(ta[5], tb[0])
+    np.testing.assert_array_equal(ta[0], tb[1])
+    fa, fb = a.fc_readout(), b.fc_readout()
+    np.testing.assert_array_equal(fa[1][5], fb[1][0])
+    np.testing.assert_allclose(fa[0][5], fb[0][0], atol=1e-6)
+
+
+def test_uncoupled_regions_reach_the_single_node_fixed_point():
+    """BASELINE invariant 1 on the GPU path: noise off, G = 0 => all regions identical."""
+    cfg = wl.config(1)
+    W, L = wl.config_connectome(cfg)
+    _, sw = tvbx.sweep_from_config(cfg, W, L, sim_ids=[0, 1, 2, 3])
+    traj = sw.run(3000, 0.1, noise_on=False, ds=10, traj_steps=3000)
+    assert np.all(traj == traj[..., :1])
+
+
+def test_device_buffers_and_stream():
+    """Device-pointer outputs on a non-default torch stream give the same numbers as host outputs."""
+    import torch
+    cfg = wl.config(1)
+    W, L = wl.connectome(21, seed=2, keep=0.5)
+    _, a = tvbx.sweep_from_config(cfg, W, L)
+    _, b = tvbx.sweep_from_config(cfg, W, L)
+    ta = a.run(300, 0.1, noise_on=True, ds=10, traj_steps=300)
+    st = torch.cuda.Stream()
+    with torch.cuda.stream(st):
+        tb = b.run(300, 0.1, noise_on=True, ds=10, traj_steps=300, traj_device=True, stream=st)
+        fb = b.fc_readout(device=True, stream=st)
+    st.synchronize()
+    np.testing.assert_array_equal(ta, tb.cpu().numpy())
+    for x, y in zip(a.fc_readout(), fb):
+        np.testing.assert_array_equal(x, y.cpu().numpy())
+
+
+def test_degenerate_fc_is_nan_free():
+    """A18: noise off at the fixed point => zero variance => FC = 0 off the diagonal, 1 on it."""
+    W, L = wl.connectome(12, seed=2, keep=0.5)
+    cfg = dict(axes=[], fixed=dict(G=0.0), seed=0)
+    _, sw = tvbx.sweep_from_config(cfg, W, L, init=(0.0, 0.0, 0, 0, 0, 0, 0), params=dict(T=1e9))
+    sw.run(200, 0.1, noise_on=False, ds=10)
+    fc, me, mi = sw.fc_readout()
+    assert np.isfinite(fc).all() and np.isfinite(me).all()
+    assert np.all(np.diagonal(fc, axis1=1, axis2=2) == 1.0)
+
+
+def test_too_few_samples_is_an_error():
+    W, L = wl.connectome(12, seed=2, keep=0.5)
+    _, sw = tvbx.sweep_from_config(dict(axes=[], fixed={}, seed=0), W, L)
+    sw.run(15, 0.1, ds=10)
+    with pytest.raises(tvbx.TvbxError):
+        sw.fc_readout()
+    with pytest.raises(tvbx.TvbxError):
+        sw.run(5, 0.05)      # dt must not change
+
+
+# ------------------------------------------------------------------------------------ full size, sampled
+def test_cfg2_full_size_sampled_against_oracle():
+    """cfg 2 at full size in the launch configuration bench.py times (1,024 sims, default SPC);
+    the oracle recomputes a stratified sample of simulations one by one (sims are independent).
+    Shortened in time (1 s simulated, 0.2 s discarded) so the CPU side finishes in seconds."""
+    cfg = wl.config(2)
+    W, L = wl.config_connectome(cfg)
+    steps, discard = 10000, 2000
+    conn, sw = tvbx.sweep_from_config(cfg, W, L)
+    sw.run(steps, cfg["dt"], noise_on=True, ds=10, discard_steps=discard)
+    fc, me, mi = sw.fc_readout()
+    assert fc.shape == (1024, 68, 68) and np.isfinite(fc).all()
+    sims = [0, 31, 5 * 32 + 9, 16 * 32 + 16, 1023 - 31, 1023]
+    o = orc.OracleSweep(W, L, wl.grid_params(cfg, sims=sims), seed=cfg["seed"], ext_ids=sims)
+    o.run(steps, cfg["dt"], noise_on=True, ds=10, discard_steps=discard)
+    rfc, rme, rmi = o.fc_readout()
+    assert np.abs(me[sims] / rme - 1).max() < TOL_MEAN_REL
+    assert np.abs(mi[sims] / rmi - 1).max() < TOL_MEAN_REL
+    assert np.abs(fc[sims] - rfc).max() < TOL_FC_ABS
+    # properties that hold for every simulation at any size
+    assert np.all(np.abs(fc) <= 1.0 + 1e-6)
+    np.testing.assert_array_equal(fc, np.swapaxes(fc, 1, 2))
+    assert (me > 0).all() and (me < 0.2).all() and (mi > 0).all() and (mi < 0.2).all()
