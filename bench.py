@@ -150,9 +150,13 @@ def cpu_baseline(cfg_id):
     cores = orc.max_threads()
     n_s = min(S, max(1, cores))
     sims = [int(x) for x in np.linspace(0, S - 1, n_s).round()]
-    per_sim_rate = 1.0e5                      # region-steps/s/core, order of magnitude, only to size the sample
-    steps = int(min(cfg["steps"], max(1000, 15.0 * per_sim_rate / cfg["n"])))
     P = wl.grid_params(cfg, sims=sims)
+    o = orc.OracleSweep(W, L, P, seed=cfg["seed"], ext_ids=sims)      # size the sample: aim at ~15 s
+    t0 = time.perf_counter()
+    o.run(200, cfg["dt"], noise_on=True, ds=cfg["ds"], discard_steps=0)
+    per_step = (time.perf_counter() - t0) / 200
+    o.close()
+    steps = int(min(cfg["steps"], max(1000, 15.0 / per_step)) // cfg["ds"] * cfg["ds"])
     o = orc.OracleSweep(W, L, P, seed=cfg["seed"], ext_ids=sims)
     t0 = time.perf_counter()
     o.run(steps, cfg["dt"], noise_on=True, ds=cfg["ds"], discard_steps=0)
@@ -181,6 +185,8 @@ def run_tvbx(args):
 
     cfg, W, L, S = workload(args.config)
     N, steps_sim = cfg["n"], (args.sim_steps or cfg["steps"])
+    if steps_sim != cfg["steps"]:                # profiling runs only: keep the discard proportionate
+        cfg["discard_steps"] = min(cfg["discard_steps"], (steps_sim // 5) // cfg["ds"] * cfg["ds"])
     seed = cfg["seed"] + rank                    # replica r of the sweep: same grid, its own noise
     stream = torch.cuda.Stream()
 

@@ -84,7 +84,7 @@ enum tvbx_precision { TVBX_F32 = 0, TVBX_F64 = 1 };
 
 typedef struct tvbx_sweep_opts {
   int32_t precision;      /* TVBX_F32 (default) or TVBX_F64 (the 1e-9 parity build mode) */
-  int32_t sims_per_cta;   /* 0 = choose; else 1,2,4,8,16,32: simulations sharing one CTA / one 32*k-byte ring line */
+  int32_t sims_per_cta;   /* 0 = choose; else 1..32: simulations integrated by one CTA (they share a delay table) */
   int64_t n_sims;         /* 0 = the whole grid; else number of entries of sim_ids */
   const int64_t* sim_ids; /* host: external (grid) indices of the simulations this sweep object holds,
                              e.g. one rank's shard; results are returned in this order */

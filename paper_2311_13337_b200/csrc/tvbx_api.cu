@@ -72,6 +72,12 @@ double axis_value(double lo, double hi, int n, int i) {
 }
 // A13
 int32_t delay_steps(double L_mm, double v, double dt) { return (int32_t)std::nearbyint((L_mm / v) / dt); }
+// steps between CTA barriers: at most the minimum delay (step n reads times <= n - d_min), whole
+// gather chunks when there is room for one
+int32_t block_steps(int32_t dmin) {
+  const int32_t b = std::max(1, dmin);
+  return b >= tvbx::GC ? b / tvbx::GC * tvbx::GC : b;
+}
 
 struct HostEdge { int32_t j; double w; double L; };
 
@@ -197,26 +203,18 @@ __global__ void state_init_kernel(R* p, size_t row, size_t total, InitVals<R> iv
     p[i] = iv.v[(i / row) % (NSV - 2)];
 }
 
-template <typename R> struct KernelPick { void (*fn)(const IntegrateParams<R>); int maxt; };
+template <typename R> struct KernelPick { void (*fn)(const IntegrateParams<R>); };
 
-// (SPC, SINGLE) -> kernel instantiation.  MAXT bounds the registers: 544 threads -> <= 120 registers
-// (FP32), 256 threads -> <= 255 (FP64).
+// MAXT bounds the registers per thread: 1024 threads -> 64 registers (FP32), 384 -> 168 (FP64).
 template <typename R> struct MaxT;
-template <> struct MaxT<float> { static constexpr int v = 544; };
-template <> struct MaxT<double> { static constexpr int v = 256; };
+template <> struct MaxT<float> { static constexpr int v = 1024; };
+template <> struct MaxT<double> { static constexpr int v = 384; };
 
 template <typename R>
-KernelPick<R> pick_kernel(int spc, bool single) {
+KernelPick<R> pick_kernel(bool single, bool closed) {
   constexpr int MT = MaxT<R>::v;
-#define TVBX_CASE(S)                                                                         \
-  case S:                                                                                    \
-    return single ? KernelPick<R>{integrate_kernel<R, S, true, MT>, MT}                      \
-                  : KernelPick<R>{integrate_kernel<R, S, false, MT>, MT};
-  switch (spc) {
-    TVBX_CASE(1) TVBX_CASE(2) TVBX_CASE(4) TVBX_CASE(8) TVBX_CASE(16) TVBX_CASE(32)
-    default: return KernelPick<R>{nullptr, 0};
-  }
-#undef TVBX_CASE
+  if (single) return closed ? KernelPick<R>{integrate_kernel<R, true, true, MT>} : KernelPick<R>{integrate_kernel<R, true, false, MT>};
+  return closed ? KernelPick<R>{integrate_kernel<R, false, true, MT>} : KernelPick<R>{integrate_kernel<R, false, false, MT>};
 }
 
 template <typename R>
@@ -229,7 +227,7 @@ struct DeviceImpl : DeviceSide {
   DevBuf<R> d_psim, d_ring, d_state, d_xbar;
   DevBuf<double> d_sums, d_cmean, d_mean, d_M;
   IntegrateParams<R> P;
-  KernelPick<R> kp{nullptr, 0};
+  KernelPick<R> kp{nullptr};
   int threads = 0, smem = 0;
   bool single = true;
   size_t ring_count = 0;
@@ -260,14 +258,16 @@ struct DeviceImpl : DeviceSide {
         D = std::max(D, d); dmin = std::min(dmin, d);
       }
       if (c.edges.empty()) dmin = 0;
-      ht.D = D; ht.dmin = dmin; ht.B = std::max(1, dmin); ht.Hp = D + ht.B + 1;
-      if ((int64_t)N * ht.Hp >= (int64_t)INT32_MAX / 2) return fail(TVBX_EINVAL, "ring too deep for 32-bit slot indices");
-      tds[t].Hp = ht.Hp; tds[t].B = ht.B; tds[t].n_edges = (int32_t)c.edges.size(); tds[t].pad = 0;
+      ht.D = D; ht.dmin = dmin; ht.B = block_steps(dmin); ht.Hp = D + ht.B + 1;
+      const int32_t Hs = ht.Hp + GC - 1;
+      if (Hs > 65535 || N > 65535) return fail(TVBX_EINVAL, "ring of %d slots (or %d regions) exceeds the 16-bit edge packing", Hs, N);
+      tds[t].Hp = ht.Hp; tds[t].Hs = Hs; tds[t].B = ht.B; tds[t].n_edges = (int32_t)c.edges.size();
       tds[t].edge_off = (int64_t)edges.size(); tds[t].rowptr_off = (int64_t)rowptr.size();
       for (size_t e = 0; e < c.edges.size(); ++e) {
         Edge<R> ed;
         std::memset(&ed, 0, sizeof ed);
-        ed.w = (R)c.edges[e].w; ed.jbase = c.edges[e].j * ht.Hp; ed.back = ht.Hp - ht.delays[e];
+        ed.w = (R)c.edges[e].w;
+        ed.jd = (uint32_t)c.edges[e].j | ((uint32_t)(ht.Hp - ht.delays[e]) << 16);
         edges.push_back(ed);
       }
       rowptr.insert(rowptr.end(), c.rowptr.begin(), c.rowptr.end());
@@ -280,7 +280,7 @@ struct DeviceImpl : DeviceSide {
     for (int g = 0; g < G; ++g) {
       const HostGroup& hg = sw->groups[g];
       gds[g].table = hg.table; gds[g].pad = 0; gds[g].ring_off = (int64_t)ring_elems;
-      ring_elems += (size_t)N * sw->tables[hg.table].Hp * SPC;
+      ring_elems += (size_t)N * (sw->tables[hg.table].Hp + GC - 1) * SPC;
       for (int sl = 0; sl < SPC; ++sl) {
         const int64_t s = hg.lanes[sl];
         const int64_t src = s >= 0 ? s : hg.lanes[0];      // padding lanes replay lane 0, never read back
@@ -342,6 +342,21 @@ struct DeviceImpl : DeviceSide {
     for (int i = 0; i < 10; ++i) { tf.P[0][i] = (R)dp[TVBX_P_POLY_E + i]; tf.P[1][i] = (R)dp[TVBX_P_POLY_I + i]; }
     tf.eps = (R)dp[TVBX_P_EPS_NU];
     tf.same_tau = dp[TVBX_P_TAUE] == dp[TVBX_P_TAUI];
+    {   // closed form (tau_e == tau_i); all in FP64, then cast
+      const double tau = dp[TVBX_P_TAUE], gL = dp[TVBX_P_GL], Cm = dp[TVBX_P_CM], Ee = dp[TVBX_P_EE], Ei = dp[TVBX_P_EI];
+      const double ae = dp[TVBX_P_QE] * tau * Ke, ai = dp[TVBX_P_QI] * tau * Ki;
+      const double de = ai * (Ee - Ei), di = ae * (Ei - Ee);
+      const double ke = Ke * tau * tau * dp[TVBX_P_QE] * dp[TVBX_P_QE], ki = Ki * tau * tau * dp[TVBX_P_QI] * dp[TVBX_P_QI];
+      tf.EegL = (R)(Ee * gL); tf.EigL = (R)(Ei * gL); tf.de = (R)de; tf.di = (R)di; tf.ke = (R)ke; tf.ki = (R)ki;
+      tf.cq_e = (R)(2 * ki * di); tf.cq_i = (R)(2 * ke * de); tf.cq_ee = (R)(2 * ki * di * di); tf.cq_ii = (R)(2 * ke * de * de);
+      tf.tau_ae = (R)(tau * ae); tf.tau_ai = (R)(tau * ai); tf.ae2 = (R)(ae * ae); tf.aeai = (R)(ae * ai); tf.ai2 = (R)(ai * ai);
+      // polynomial variables: m = (mu_V - muV0)/dmuV0, s = (sigma_V - sV0)/dsV0,
+      // t = (tau_V g_L/C_m - tvn0)/dtvn0 = (g_L/dtvn0) (r - r0) with tau_V = tau + C_m r
+      const double ms = 1.0 / dp[TVBX_P_DMUV0], ss = 1.0 / dp[TVBX_P_DSV0], ts = gL / dp[TVBX_P_DTVN0];
+      tf.muV0 = (R)dp[TVBX_P_MUV0]; tf.sV0 = (R)dp[TVBX_P_SV0]; tf.r0 = (R)((dp[TVBX_P_TVN0] - tau * gL / Cm) / gL);
+      const double sc[10] = {1.0, ms, ss, ts, ms * ms, ss * ss, ts * ts, ms * ss, ms * ts, ss * ts};
+      for (int i = 0; i < 10; ++i) { tf.C[0][i] = (R)(dp[TVBX_P_POLY_E + i] * sc[i]); tf.C[1][i] = (R)(dp[TVBX_P_POLY_I + i] * sc[i]); }
+    }
     P.b_i = (R)dp[TVBX_P_B_I]; P.a_i_over_tau = (R)(dp[TVBX_P_A_I] / dp[TVBX_P_TAU_W_I]);
     P.inv_tau_w_i = (R)(1.0 / dp[TVBX_P_TAU_W_I]);
     P.inv_Ne = (R)(1.0 / (dp[TVBX_P_NTOT] * (1.0 - dp[TVBX_P_GINH])));
@@ -352,33 +367,28 @@ struct DeviceImpl : DeviceSide {
     P.ou_m = (R)(dp[TVBX_P_MU_OU] * (1.0 - rho));
     P.dt = (R)dt;
     P.muV_local = dp[TVBX_P_MUV_LOCAL] != 0.0;
-    P.N = N; P.seed = sw->seed; P.chunk_samples = (int32_t)CS;
+    P.N = N; P.SPC = SPC; P.seed = sw->seed; P.chunk_samples = (int32_t)CS;
     P.tables = d_tables.p; P.groups = d_groups.p; P.edges = d_edges.p; P.rowptr = d_rowptr.p;
     P.psim = d_psim.p; P.ext_id = d_ext.p; P.loc_id = d_loc.p; P.ring = d_ring.p; P.state = d_state.p;
     P.sums = d_sums.p; P.xbar = d_xbar.p;
 
-    // ---- launch geometry ----
+    // ---- launch geometry: two lanes per (sim, region) ----
     const int maxt = sw->threads_req > 0 ? std::min(sw->threads_req, MaxT<R>::v) : MaxT<R>::v;
-    const int pairs = N * SPC;
-    if (pairs <= maxt) { single = true; threads = ((pairs + 31) / 32) * 32; if (threads > maxt) threads = pairs; }
-    else {
-      single = false;
-      const int rtmax = std::max(1, maxt / SPC);
-      const int passes = (N + rtmax - 1) / rtmax;
-      const int rt = (N + passes - 1) / passes;
-      threads = rt * SPC;
-    }
-    kp = pick_kernel<R>(SPC, single);
-    if (!kp.fn) return fail(TVBX_EINVAL, "sims_per_cta=%d not supported", SPC);
+    const int rt_max = std::max(1, maxt / (2 * SPC));           // regions per pass
+    int rt;
+    if (N <= rt_max) { single = true; rt = N; }
+    else { single = false; const int passes = (N + rt_max - 1) / rt_max; rt = (N + passes - 1) / passes; }
+    threads = 2 * SPC * rt;
+    kp = pick_kernel<R>(single, tf.same_tau != 0);
     const size_t tbytes = c.edges.size() * sizeof(Edge<R>) + (size_t)(N + 1) * 4;
-    P.smem_table = tbytes <= 160 * 1024;
-    smem = P.smem_table ? (int)((tbytes + 15) / 16 * 16) : 0;
+    const size_t base = (size_t)GC * (threads / 2) * sizeof(R) + 20 * sizeof(R) + 16;
+    P.smem_table = base + tbytes <= 200 * 1024;
+    smem = (int)(base + (P.smem_table ? tbytes : 0));
     CU(cudaFuncSetAttribute((const void*)kp.fn, cudaFuncAttributeMaxDynamicSharedMemorySize, std::max(smem, 1024)));
     cudaFuncAttributes fa;
     CU(cudaFuncGetAttributes(&fa, (const void*)kp.fn));
-    const int rt_block = threads / SPC;
     sw->info[0] = G; sw->info[1] = threads; sw->info[2] = SPC; sw->info[3] = fa.numRegs; sw->info[4] = smem;
-    sw->info[5] = single ? 1 : (N + rt_block - 1) / rt_block; sw->info[6] = (int32_t)CS; sw->info[7] = (int32_t)fa.localSizeBytes;
+    sw->info[5] = single ? 1 : (N + rt - 1) / rt; sw->info[6] = (int32_t)CS; sw->info[7] = (int32_t)fa.localSizeBytes;
     CU(cudaDeviceSynchronize());
     return TVBX_OK;
   }
@@ -619,14 +629,27 @@ int32_t tvbx_sweep_create(const tvbx_connectome* c, const tvbx_model_params* def
       !(dp[TVBX_P_DMUV0] != 0) || !(dp[TVBX_P_DSV0] != 0) || !(dp[TVBX_P_DTVN0] != 0) || !(dp[TVBX_P_EPS_NU] > 0) ||
       !(dp[TVBX_P_GINH] > 0 && dp[TVBX_P_GINH] < 1) || !(dp[TVBX_P_NTOT] > 0) || !(dp[TVBX_P_PCONN] > 0))
     return fail(TVBX_EINVAL, "uniform model parameters out of range");
-  // sims per CTA
+  // sims per CTA: any 1 .. floor(max threads / 2N).  Pick the count that minimises the number of
+  // simulations the busiest SM has to integrate (148 SMs, CTAs of a sweep all resident or in waves).
   int spc = opts ? opts->sims_per_cta : 0;
   if (const char* e = getenv("TVBX_SPC")) if (spc == 0) spc = atoi(e);
+  const int maxt_sel = sw->precision == TVBX_F64 ? 384 : 1024;
+  const int spc_max = std::max(1, std::min(32, maxt_sel / (2 * sw->conn.n)));
   if (spc == 0) {
-    spc = sw->precision == TVBX_F64 ? 2 : 8;
-    while (spc > 1 && sw->n_sims / spc < 148) spc /= 2;      // at least one CTA per SM when the sweep allows
+    // simulations per distinct speed decide the CTA count; approximate with one table here
+    std::map<double, int64_t> per_v;
+    for (int64_t s = 0; s < sw->n_sims; ++s) per_v[sw->param(s, TVBX_P_V)]++;
+    int64_t best_cost = INT64_MAX;
+    for (int cand = 1; cand <= spc_max; ++cand) {
+      int64_t ctas = 0;
+      for (auto& kv : per_v) ctas += (kv.second + cand - 1) / cand;
+      const int64_t resident = std::max<int64_t>(1, maxt_sel / (2 * (int64_t)sw->conn.n * cand));
+      const int64_t slots = 148 * resident;
+      const int64_t cost = ctas <= slots ? ((ctas + 147) / 148) * cand : ((ctas + slots - 1) / slots) * resident * cand;
+      if (cost < best_cost || (cost == best_cost && cand > spc)) { best_cost = cost; spc = cand; }
+    }
   }
-  if (spc != 1 && spc != 2 && spc != 4 && spc != 8 && spc != 16 && spc != 32) return fail(TVBX_EINVAL, "sims_per_cta=%d", spc);
+  if (spc < 1 || spc > 32) return fail(TVBX_EINVAL, "sims_per_cta=%d (valid: 1..32)", spc);
   sw->spc = spc;
   // group the simulations by speed (one delay table per distinct v), then into CTAs of spc lanes
   std::map<double, int32_t> vmap;
@@ -760,7 +783,7 @@ int32_t tvbx_ring_len(const tvbx_sweep* sw, int64_t sim, double dt, int32_t* H, 
   for (const HostEdge& e : sw->conn.edges) { const int32_t d = delay_steps(e.L, v, dt); D = std::max(D, d); dmin = std::min(dmin, d); }
   if (sw->conn.edges.empty()) dmin = 0;
   if (H) *H = D + 1;
-  if (H_phys) *H_phys = D + std::max(1, dmin) + 1;
+  if (H_phys) *H_phys = D + block_steps(dmin) + 1;
   return TVBX_OK;
 }
 int32_t tvbx_steps_done(const tvbx_sweep* sw, int64_t* n) {

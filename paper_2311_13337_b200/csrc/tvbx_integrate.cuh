@@ -5,17 +5,26 @@
 //
 // Mapping (B200-first, not the paper's thread-per-simulation kernel):
 //   CTA      = one "group" of SPC simulations that share a delay table (same speed v), all N regions
-//   thread   = (region lane rl, simulation lane sl); sl is the fastest thread index, so a warp holds
-//              32/SPC regions x SPC sims and every ring access of SPC sims is one contiguous line
-//   ring     = ring[group][region][slot][SPC]  (E only, "temporal buffer")
-//   time     = the kernel is persistent over time: it runs B = max(1, min delay) steps between CTA
-//              barriers, because step n only reads E at times <= n - d_min
+//   lane pair= one (simulation, region); the EVEN lane integrates the excitatory population
+//              (E, C_ee, W_e), the ODD lane the inhibitory one (I, C_ii, W_i).  Both run the same
+//              transfer-function code on different constants (no divergence) and exchange E/I, C,
+//              (F - nu) and the C_ei half-sums with five warp shuffles per step.
+//   ring     = ring[group][sim][region][slot]  (E only, "temporal buffer"): TIME is the
+//              fastest index, so the B consecutive steps of a time block read B consecutive floats
+//              per edge.  Rows carry GC-1 mirror slots so that a chunk of GC reads never wraps.
+//   time     = the kernel is persistent over time: it runs B <= min delay steps between CTA
+//              barriers (step n only reads E at times <= n - d_min), and inside a block it
+//              alternates a GATHER phase (coupling sums of the next <= GC steps, pure loads + FMAs,
+//              the edge list split between the two lanes of a pair) with a COMPUTE phase (<= GC
+//              steps of pure register arithmetic).
 #pragma once
 #include <cuda_runtime.h>
 #include <stdint.h>
 #include "tvbx_tf.cuh"
 
 namespace tvbx {
+
+enum { GC = 8 };        // steps per gather chunk (and mirror slots + 1)
 
 // ---- Philox4x32-10 (A12) -------------------------------------------------------------------------
 __device__ __forceinline__ void philox4x32_10(uint32_t c0, uint32_t c1, uint32_t c2, uint32_t c3,
@@ -30,7 +39,7 @@ __device__ __forceinline__ void philox4x32_10(uint32_t c0, uint32_t c1, uint32_t
   out[0] = c0; out[1] = c1; out[2] = c2; out[3] = c3;
 }
 
-// four N(0,1) variates for steps 4q .. 4q+3 of (sim, region): Box-Muller on 23-bit uniforms
+// two N(0,1) variates from two 32-bit words: Box-Muller on 23-bit uniforms (exact in FP32 and FP64)
 template <typename R> __device__ __forceinline__ void box_muller(uint32_t xa, uint32_t xb, R& zc, R& zs);
 template <> __device__ __forceinline__ void box_muller<float>(uint32_t xa, uint32_t xb, float& zc, float& zs) {
   const float u1 = ((float)(xa >> 9) + 0.5f) * (1.0f / 8388608.0f);
@@ -48,6 +57,7 @@ template <> __device__ __forceinline__ void box_muller<double>(uint32_t xa, uint
   sincospi(2.0 * u2, &s, &c);
   zc = r * c; zs = r * s;
 }
+// the four normals of steps 4q .. 4q+3 of (sim, region)
 template <typename R>
 __device__ __forceinline__ void normals4(uint64_t seed, uint32_t sim, uint32_t region, uint64_t q, R xi[4]) {
   uint32_t x[4];
@@ -56,16 +66,19 @@ __device__ __forceinline__ void normals4(uint64_t seed, uint32_t sim, uint32_t r
   box_muller<R>(x[2], x[3], xi[2], xi[3]);
 }
 
+template <typename R> __device__ __forceinline__ R shfl_x1(unsigned mask, R v) { return __shfl_xor_sync(mask, v, 1); }
+
 // ---- device-side descriptors ------------------------------------------------------------------------
-template <typename R> struct Edge { R w; int32_t jbase; int32_t back; };   // jbase = j*Hp, back = Hp - d
-template <> struct __align__(16) Edge<float> { float w; int32_t jbase; int32_t back; int32_t pad; };
-template <> struct __align__(16) Edge<double> { double w; int32_t jbase; int32_t back; };
+// one non-zero weight: w = W_kj, jd = j | (Hp - d_kj) << 16   (ring slots and regions < 65536)
+template <typename R> struct Edge;
+template <> struct __align__(8) Edge<float> { float w; uint32_t jd; };
+template <> struct __align__(16) Edge<double> { double w; uint32_t jd; uint32_t pad; };
 
 struct TableDesc {      // one per distinct speed v
-  int32_t Hp;           // physical ring length D + B + 1
+  int32_t Hp;           // ring period D + B + 1
+  int32_t Hs;           // row stride Hp + GC - 1 (mirror slots)
   int32_t B;            // steps between CTA barriers
   int32_t n_edges;
-  int32_t pad;
   int64_t edge_off;     // first edge in the edge array
   int64_t rowptr_off;   // first entry of this table's row pointer (N+1 ints)
 };
@@ -87,6 +100,7 @@ struct IntegrateParams {
   R dt;
   int32_t muV_local;
   int32_t N;
+  int32_t SPC;                  // simulations per CTA
   int32_t noise_on;
   int32_t ds;                   // 0 = no downsampling
   int64_t n_begin, n_end;       // global step range of this launch
@@ -100,9 +114,9 @@ struct IntegrateParams {
   const Edge<R>* edges;
   const int32_t* rowptr;
   const R* psim;                // [group][NPS][SPC]
-  const int32_t* ext_id;        // [group][SPC]  external sim index (Philox counter), -1 = padding lane
+  const int32_t* ext_id;        // [group][SPC]  external sim index (Philox counter)
   const int32_t* loc_id;        // [group][SPC]  local sim index (row of traj), -1 = padding lane
-  R* ring;                      // [group][N][Hp][SPC]
+  R* ring;                      // [group][SPC][N][Hs]
   R* state;                     // [group][NSV-2][N][SPC]
   double* sums;                 // [group][2][N][SPC]  running sums of kept E / I samples
   R* xbar;                      // [group][CS][N][SPC] kept excitatory samples of the current chunk
@@ -112,72 +126,94 @@ struct IntegrateParams {
   int32_t smem_table;           // edges + rowptr staged in shared memory
 };
 
-template <typename R> struct Local {   // per (sim, region) registers
-  R E, I, Cee, Cei, Cii, We, Wi, ou, winE, winI;
-  double sumE, sumI;
+// per-lane registers: one population of one (sim, region)
+template <typename R> struct Local {
+  R nu;      // E (even lane) or I (odd lane)
+  R Cs;      // C_ee or C_ii
+  R Cei;     // both lanes keep the same copy
+  R W;       // W_e or W_i
+  R ou;      // both lanes keep the same copy
+  R win;     // running window sum of nu
+  double sum;
 };
 
-template <typename R, int SPC>
-__device__ __forceinline__ void load_local(const IntegrateParams<R>& P, int g, int k, int sl, Local<R>& s) {
-  const size_t stride = (size_t)P.N * SPC;
-  const R* p = P.state + (size_t)g * (NSV - 2) * stride + (size_t)k * SPC + sl;
-  s.E = p[0 * stride]; s.I = p[1 * stride]; s.Cee = p[2 * stride]; s.Cei = p[3 * stride];
-  s.Cii = p[4 * stride]; s.We = p[5 * stride]; s.Wi = p[6 * stride]; s.ou = p[7 * stride];
-  s.winE = p[8 * stride]; s.winI = p[9 * stride];
-  const double* q = P.sums + (size_t)g * 2 * stride + (size_t)k * SPC + sl;
-  s.sumE = q[0]; s.sumI = q[stride];
+template <typename R>
+__device__ __forceinline__ void load_local(const IntegrateParams<R>& P, int g, int k, int sl, int pop, Local<R>& s) {
+  const size_t stride = (size_t)P.N * P.SPC;
+  const R* p = P.state + (size_t)g * (NSV - 2) * stride + (size_t)k * P.SPC + sl;
+  s.nu = p[(0 + pop) * stride]; s.Cs = p[(pop ? 4 : 2) * stride]; s.Cei = p[3 * stride];
+  s.W = p[(5 + pop) * stride]; s.ou = p[7 * stride]; s.win = p[(8 + pop) * stride];
+  s.sum = P.sums[(size_t)g * 2 * stride + pop * stride + (size_t)k * P.SPC + sl];
 }
-template <typename R, int SPC>
-__device__ __forceinline__ void store_local(const IntegrateParams<R>& P, int g, int k, int sl, const Local<R>& s) {
-  const size_t stride = (size_t)P.N * SPC;
-  R* p = P.state + (size_t)g * (NSV - 2) * stride + (size_t)k * SPC + sl;
-  p[0 * stride] = s.E; p[1 * stride] = s.I; p[2 * stride] = s.Cee; p[3 * stride] = s.Cei;
-  p[4 * stride] = s.Cii; p[5 * stride] = s.We; p[6 * stride] = s.Wi; p[7 * stride] = s.ou;
-  p[8 * stride] = s.winE; p[9 * stride] = s.winI;
-  double* q = P.sums + (size_t)g * 2 * stride + (size_t)k * SPC + sl;
-  q[0] = s.sumE; q[stride] = s.sumI;
+template <typename R>
+__device__ __forceinline__ void store_local(const IntegrateParams<R>& P, int g, int k, int sl, int pop, const Local<R>& s) {
+  const size_t stride = (size_t)P.N * P.SPC;
+  R* p = P.state + (size_t)g * (NSV - 2) * stride + (size_t)k * P.SPC + sl;
+  p[(0 + pop) * stride] = s.nu; p[(pop ? 4 : 2) * stride] = s.Cs; p[(5 + pop) * stride] = s.W;
+  p[(8 + pop) * stride] = s.win;
+  if (pop == 0) { p[3 * stride] = s.Cei; p[7 * stride] = s.ou; }
+  P.sums[(size_t)g * 2 * stride + pop * stride + (size_t)k * P.SPC + sl] = s.sum;
 }
 
-// SINGLE: every (sim, region) of the group has its own thread (blockDim >= N*SPC): state stays in
-// registers for the whole launch.  Otherwise the CTA makes several passes over the regions inside
+// SINGLE: every (sim, region) of the group has its own lane pair (blockDim >= 2*N*SPC): state stays
+// in registers for the whole launch.  Otherwise the CTA makes several passes over the regions inside
 // each time block and the state round-trips through global memory (L1/L2 resident).
-template <typename R, int SPC, bool SINGLE, int MAXT>
+// CLOSED: tau_e == tau_i -> tf_closed, else tf_jet.
+template <typename R, bool SINGLE, bool CLOSED, int MAXT>
 __global__ void __launch_bounds__(MAXT, 1) integrate_kernel(const __grid_constant__ IntegrateParams<R> P) {
   extern __shared__ __align__(16) unsigned char smem_raw[];
   const int g = blockIdx.x;
-  const int sl = threadIdx.x % SPC;
-  const int rl = threadIdx.x / SPC;
-  const int RT = blockDim.x / SPC;
-  const int N = P.N;
+  const int N = P.N, SPC = P.SPC;
+  const int pop = threadIdx.x & 1;
+  const int pair = threadIdx.x >> 1;
+  const int PT = blockDim.x >> 1;                 // lane pairs per CTA (a multiple of SPC)
+  const int RT = PT / SPC;                        // regions per pass
+  const int rl = pair / SPC, sl = pair - rl * SPC;
   const GroupDesc gd = P.groups[g];
   const TableDesc td = P.tables[gd.table];
-  const int Hp = td.Hp;
+  const int Hp = td.Hp, Hs = td.Hs;
   const Edge<R>* edges = P.edges + td.edge_off;
   const int32_t* rowptr = P.rowptr + td.rowptr_off;
-  if (P.smem_table) {
-    Edge<R>* se = reinterpret_cast<Edge<R>*>(smem_raw);
-    int32_t* sr = reinterpret_cast<int32_t*>(se + td.n_edges);
-    for (int i = threadIdx.x; i < td.n_edges; i += blockDim.x) se[i] = edges[i];
-    for (int i = threadIdx.x; i <= N; i += blockDim.x) sr[i] = rowptr[i];
+  // shared memory: [GC][PT] coupling sums, 2 x 10 polynomial coefficients, then the optional tables
+  R* s_cpl = reinterpret_cast<R*>(smem_raw);
+  R* s_poly = s_cpl + (size_t)GC * PT;
+  {
+    unsigned char* tab = reinterpret_cast<unsigned char*>(s_poly + 20);
+    tab += (16 - (reinterpret_cast<uintptr_t>(tab) & 15)) & 15;
+    if (threadIdx.x < 20)
+      s_poly[threadIdx.x] = CLOSED ? P.tf.C[threadIdx.x / 10][threadIdx.x % 10] : P.tf.P[threadIdx.x / 10][threadIdx.x % 10];
+    if (P.smem_table) {
+      Edge<R>* se = reinterpret_cast<Edge<R>*>(tab);
+      int32_t* sr = reinterpret_cast<int32_t*>(se + td.n_edges);
+      for (int i = threadIdx.x; i < td.n_edges; i += blockDim.x) se[i] = edges[i];
+      for (int i = threadIdx.x; i <= N; i += blockDim.x) sr[i] = rowptr[i];
+      edges = se; rowptr = sr;
+    }
     __syncthreads();
-    edges = se; rowptr = sr;
   }
-  R* ring = P.ring + gd.ring_off + sl;
+  const R* poly = s_poly + 10 * pop;
+  R* ring = P.ring + gd.ring_off + (size_t)sl * N * Hs;     // this simulation's [N][Hs]
 
-  // per-simulation scalars
+  // per-simulation scalars of this lane's population
   const R* ps = P.psim + (size_t)g * NPS * SPC + sl;
-  const R pG = ps[0 * SPC], pWn = ps[1 * SPC], pBe = ps[2 * SPC], pAeT = ps[3 * SPC], pITw = ps[4 * SPC];
-  const R pELe = ps[5 * SPC], pELi = ps[6 * SPC], pIT = ps[7 * SPC];
-  const R cFee = ps[8 * SPC], cFei = ps[9 * SPC], cFie = ps[10 * SPC], cFii = ps[11 * SPC];
-  const R gLELe = P.tf.gL * pELe, gLELi = P.tf.gL * pELi;
+  const R pG = ps[0 * SPC], pWn = ps[1 * SPC], pIT = ps[7 * SPC];
+  const R pB = pop ? P.b_i : ps[2 * SPC];                  // b
+  const R pAT = pop ? P.a_i_over_tau : ps[3 * SPC];        // a / tau_w
+  const R pITw = pop ? P.inv_tau_w_i : ps[4 * SPC];        // 1 / tau_w
+  const R pEL = ps[(5 + pop) * SPC];
+  const R cFe = ps[(pop ? 10 : 8) * SPC], cFi = ps[(pop ? 11 : 9) * SPC];
+  const R gLEL = P.tf.gL * pEL;
+  const R invNp = pop ? P.inv_Ni : P.inv_Ne;
   const int ext = P.ext_id[(size_t)g * SPC + sl];
   const int loc = P.loc_id[(size_t)g * SPC + sl];
   const R dt = P.dt, kap = P.kappa, kap2 = P.kappa * P.kappa;
   const R inv_ds = P.ds > 0 ? R(1) / R(P.ds) : R(0);
+  const bool noise = P.noise_on != 0;
 
   Local<R> st;
-  if (SINGLE && rl < N) load_local<R, SPC>(P, g, rl, sl, st);
-  R xi[4] = {R(0), R(0), R(0), R(0)};   // the four normals of the current Philox call
+  st.nu = st.Cs = st.Cei = st.W = st.ou = st.win = R(0); st.sum = 0.0;
+  if (SINGLE && rl < N) load_local<R>(P, g, rl, sl, pop, st);
+  R xi[4] = {R(0), R(0), R(0), R(0)};   // the four normals of the Philox call this lane owns
 
   int64_t n = P.n_begin;
   int cur = (int)(n % Hp);                       // ring slot of time index n
@@ -188,109 +224,135 @@ __global__ void __launch_bounds__(MAXT, 1) integrate_kernel(const __grid_constan
   while (n < P.n_end) {
     const int nb = (int)min((int64_t)td.B, P.n_end - n);
     int win_left = win_left0, sidx = sidx0;
-    for (int k = rl; k < N; k += RT) {
-      if (!SINGLE) load_local<R, SPC>(P, g, k, sl, st);
+    for (int k0 = 0; k0 < N; k0 += RT) {
+      const int k = k0 + rl;
+      const unsigned mask = __ballot_sync(0xffffffffu, k < N);   // lanes of this warp that work in this pass
+      if (k >= N) continue;
+      if (!SINGLE) load_local<R>(P, g, k, sl, pop, st);
       win_left = win_left0; sidx = sidx0;
       const int e0 = rowptr[k], e1 = rowptr[k + 1];
-      R* myring = ring + (size_t)k * Hp * SPC;
-      if (P.noise_on && (n & 3) && (!SINGLE || n == P.n_begin))   // re-enter a partly used quad
+      R* myring = ring + (size_t)k * Hs;
+      // this lane owns the Philox quads q with (q & 1) == pop; re-enter a partly used quad
+      if (noise && (n & 3) && (int)((n >> 2) & 1) == pop && (!SINGLE || n == P.n_begin))
         normals4<R>(P.seed, (uint32_t)ext, (uint32_t)k, (uint64_t)n >> 2, xi);
       int c = cur;
-      for (int i = 0; i < nb; ++i) {
-        const int64_t nn = n + i;
-        // ---- S1 delayed gather + coupling sum (ascending j, A16) ----
-        R cpl = R(0);
-        for (int e = e0; e < e1; ++e) {
-          const Edge<R> ed = edges[e];
-          int slot = c + ed.back;
-          slot = slot >= Hp ? slot - Hp : slot;
-          cpl = tfma(ed.w, ring[(size_t)(ed.jbase + slot) * SPC], cpl);
-        }
-        // ---- S2 inputs and transfer functions (Eq. 5; A5, A6, A10) ----
-        if (P.noise_on && (nn & 3) == 0) normals4<R>(P.seed, (uint32_t)ext, (uint32_t)k, (uint64_t)nn >> 2, xi);
-        const R eta = P.noise_on ? pWn * st.ou : R(0);
-        const R drive = tfma(pG, cpl, st.E) + eta;
-        R muVe, muVi;
-        Jet<R> Fe, Fi;
+      for (int c0 = 0; c0 < nb; c0 += GC) {
+        const int ch = min(GC, nb - c0);
+        // ================= GATHER: coupling sums of steps n+c0 .. n+c0+ch-1 (S1) =================
         {
-          const R xe = drive + cFee, xi_ = st.I + cFei;
-          const R se = xe > R(0) ? R(1) : R(0), si = xi_ > R(0) ? R(1) : R(0);
-          Fe = transfer_function<R>(P.tf, 0, fmax(xe, R(0)) + P.tf.eps, fmax(xi_, R(0)) + P.tf.eps,
-                                    gLELe - st.We, &muVe);
-          Fe.e *= kap * se; Fe.i *= kap * si;
-          Fe.ee *= kap2 * se; Fe.ei *= kap2 * se * si; Fe.ii *= kap2 * si;
-        }
-        {
-          const R xe = drive + cFie, xi_ = st.I + cFii;
-          const R se = xe > R(0) ? R(1) : R(0), si = xi_ > R(0) ? R(1) : R(0);
-          Fi = transfer_function<R>(P.tf, 1, fmax(xe, R(0)) + P.tf.eps, fmax(xi_, R(0)) + P.tf.eps,
-                                    gLELi - st.Wi, &muVi);
-          Fi.e *= kap * se; Fi.i *= kap * si;
-          Fi.ee *= kap2 * se; Fi.ei *= kap2 * se * si; Fi.ii *= kap2 * si;
-        }
-        if (P.muV_local) {   // A9b alternative: mu_V of the local rates only
-          const R le = fmax(st.E, R(0)) + P.tf.eps, li = fmax(st.I, R(0)) + P.tf.eps;
-          muVe = mu_V_only<R>(P.tf, le, li, gLELe - st.We);
-          muVi = mu_V_only<R>(P.tf, le, li, gLELi - st.Wi);
-        }
-        // ---- S3 Eqs. (1)-(3), forward Euler (A7, A9) ----
-        const R h = R(0.5);
-        const R dFe = Fe.v - st.E, dFi = Fi.v - st.I;
-        const R dE = (dFe + h * st.Cee * Fe.ee + st.Cei * Fe.ei + h * st.Cii * Fe.ii) * pIT;
-        const R dI = (dFi + h * st.Cee * Fi.ee + st.Cei * Fi.ei + h * st.Cii * Fi.ii) * pIT;
-        const R dCee = (Fe.v * (pIT - Fe.v) * P.inv_Ne + dFe * dFe +
-                        R(2) * (st.Cee * Fe.e + st.Cei * Fe.i) - R(2) * st.Cee) * pIT;
-        const R dCii = (Fi.v * (pIT - Fi.v) * P.inv_Ni + dFi * dFi +
-                        R(2) * (st.Cei * Fi.e + st.Cii * Fi.i) - R(2) * st.Cii) * pIT;
-        const R dCei = (dFe * dFi + (st.Cei * Fe.e + st.Cii * Fe.i) + (st.Cee * Fi.e + st.Cei * Fi.i) -
-                        R(2) * st.Cei) * pIT;
-        const R dWe = -st.We * pITw + pBe * st.E + pAeT * (muVe - pELe);
-        const R dWi = -st.Wi * P.inv_tau_w_i + P.b_i * st.I + P.a_i_over_tau * (muVi - pELi);
-        st.E = tfma(dt, dE, st.E);       st.I = tfma(dt, dI, st.I);
-        st.Cee = tfma(dt, dCee, st.Cee); st.Cei = tfma(dt, dCei, st.Cei); st.Cii = tfma(dt, dCii, st.Cii);
-        st.We = tfma(dt, dWe, st.We);    st.Wi = tfma(dt, dWi, st.Wi);
-        // ---- S4 OU (Eq. 4, A11) ----
-        if (P.noise_on) {
-          const int w = (int)(nn & 3);      // select chain keeps xi[] in registers
-          const R x = w == 0 ? xi[0] : (w == 1 ? xi[1] : (w == 2 ? xi[2] : xi[3]));
-          st.ou = tfma(P.ou_rho, st.ou, tfma(P.ou_s, x, P.ou_m));
-        }
-        // ---- S5 ring write: E at time nn+1 ----
-        c = c + 1 == Hp ? 0 : c + 1;
-        myring[(size_t)c * SPC] = st.E;
-        // ---- trajectory (tests / cfg 1) ----
-        if (P.traj && nn - P.traj_n0 < P.traj_steps && loc >= 0) {
-          R* t = P.traj + (((size_t)loc * P.traj_steps + (size_t)(nn - P.traj_n0)) * 7) * N + k;
-          t[0] = st.E; t[N] = st.I; t[2 * N] = st.Cee; t[3 * N] = st.Cei; t[4 * N] = st.Cii;
-          t[5 * N] = st.We; t[6 * N] = st.Wi;
-        }
-        // ---- S6 temporal average (A17) ----
-        st.winE += st.E; st.winI += st.I;
-        if (--win_left == 0) {
-          win_left = P.ds;
-          if (nn + 1 > P.discard_steps) {
-            const R me = st.winE * inv_ds, mi = st.winI * inv_ds;
-            P.xbar[(((size_t)g * P.chunk_samples + sidx) * N + k) * SPC + sl] = me;
-            st.sumE += (double)me; st.sumI += (double)mi;
-            ++sidx;
+          R acc[GC];
+#pragma unroll
+          for (int i = 0; i < GC; ++i) acc[i] = R(0);
+          if (ch == GC) {
+            for (int e = e0 + pop; e < e1; e += 2) {
+              const Edge<R> ed = edges[e];
+              int start = c + (int)(ed.jd >> 16);
+              start = start >= Hp ? start - Hp : start;
+              const R* src = ring + (size_t)(ed.jd & 0xffffu) * Hs + start;
+#pragma unroll
+              for (int i = 0; i < GC; ++i) acc[i] = tfma(ed.w, src[i], acc[i]);
+            }
+          } else {
+            for (int e = e0 + pop; e < e1; e += 2) {
+              const Edge<R> ed = edges[e];
+              int start = c + (int)(ed.jd >> 16);
+              start = start >= Hp ? start - Hp : start;
+              const R* src = ring + (size_t)(ed.jd & 0xffffu) * Hs + start;
+#pragma unroll
+              for (int i = 0; i < GC; ++i)
+                if (i < ch) acc[i] = tfma(ed.w, src[i], acc[i]);
+            }
           }
-          st.winE = R(0); st.winI = R(0);
+#pragma unroll
+          for (int i = 0; i < GC; ++i) {
+            const R tot = acc[i] + shfl_x1(mask, acc[i]);          // a + b == b + a: both lanes get the same bits
+            if (pop == 0) s_cpl[i * PT + pair] = tot;
+          }
+          __syncwarp(mask);
         }
+        // ================= COMPUTE: ch steps in registers (S2-S6) =================
+        for (int i = 0; i < ch; ++i) {
+          const int64_t nn = n + c0 + i;
+          const R cpl = s_cpl[i * PT + pair];
+          // ---- exchange with the partner lane ----
+          const R nu_o = shfl_x1(mask, st.nu), Cs_o = shfl_x1(mask, st.Cs);
+          const R E = pop ? nu_o : st.nu, I = pop ? st.nu : nu_o;
+          const R Cee = pop ? Cs_o : st.Cs, Cii = pop ? st.Cs : Cs_o, Cei = st.Cei;
+          // ---- noise: the owner of quad q = nn/4 provides xi ----
+          if (noise && (nn & 3) == 0 && (int)((nn >> 2) & 1) == pop)
+            normals4<R>(P.seed, (uint32_t)ext, (uint32_t)k, (uint64_t)nn >> 2, xi);
+          R x_n = R(0);
+          if (noise) {
+            const int w = (int)(nn & 3);      // select chain keeps xi[] in registers
+            const R x_own = w == 0 ? xi[0] : (w == 1 ? xi[1] : (w == 2 ? xi[2] : xi[3]));
+            const R x_oth = shfl_x1(mask, x_own);
+            x_n = (int)((nn >> 2) & 1) == pop ? x_own : x_oth;
+          }
+          // ---- S2 inputs and transfer function of this lane's population (Eq. 5; A5, A6, A10) ----
+          const R eta = noise ? pWn * st.ou : R(0);
+          const R drive = tfma(pG, cpl, E) + eta;
+          const R xe = drive + cFe, xi_ = I + cFi;
+          const R se = xe > R(0) ? kap : R(0), si = xi_ > R(0) ? kap : R(0);
+          R muV;
+          Jet<R> F;
+          if (CLOSED) F = tf_closed<R>(P.tf, poly, fmax(xe, R(0)) + P.tf.eps, fmax(xi_, R(0)) + P.tf.eps, gLEL - st.W, &muV);
+          else        F = tf_jet<R>(P.tf, poly, fmax(xe, R(0)) + P.tf.eps, fmax(xi_, R(0)) + P.tf.eps, gLEL - st.W, &muV);
+          F.e *= se; F.i *= si;               // A22 (kappa) and the clamp of A10
+          F.ee *= se * se; F.ei *= se * si; F.ii *= si * si;
+          if (P.muV_local)                    // A9b alternative: mu_V of the local rates only
+            muV = mu_V_only<R>(P.tf, fmax(E, R(0)) + P.tf.eps, fmax(I, R(0)) + P.tf.eps, gLEL - st.W);
+          // ---- S3 Eqs. (1)-(3), forward Euler (A7, A9) ----
+          const R dF = F.v - st.nu;
+          const R dnu = (dF + R(0.5) * Cee * F.ee + Cei * F.ei + R(0.5) * Cii * F.ii) * pIT;
+          // row `pop` of C with grad F (own covariance), the other row (half of the C_ei equation)
+          const R Ca = pop ? Cei : Cee, Cb = pop ? Cii : Cei;
+          const R Co = pop ? Cee : Cei, Cp = pop ? Cei : Cii;
+          const R dCs = (F.v * (pIT - F.v) * invNp + dF * dF + R(2) * (Ca * F.e + Cb * F.i) - R(2) * st.Cs) * pIT;
+          const R h = Co * F.e + Cp * F.i;
+          const R dF_o = shfl_x1(mask, dF), h_o = shfl_x1(mask, h);
+          const R dCei = (dF * dF_o + (h + h_o) - R(2) * Cei) * pIT;
+          const R dW = -st.W * pITw + pB * st.nu + pAT * (muV - pEL);
+          st.nu = tfma(dt, dnu, st.nu);
+          st.Cs = tfma(dt, dCs, st.Cs);
+          st.Cei = tfma(dt, dCei, st.Cei);
+          st.W = tfma(dt, dW, st.W);
+          // ---- S4 OU (Eq. 4, A11) ----
+          if (noise) st.ou = tfma(P.ou_rho, st.ou, tfma(P.ou_s, x_n, P.ou_m));
+          // ---- S5 ring write: E at time nn+1 (mirror the first GC-1 slots behind the period) ----
+          c = c + 1 == Hp ? 0 : c + 1;
+          if (pop == 0) {
+            myring[c] = st.nu;
+            if (c < GC - 1) myring[Hp + c] = st.nu;
+          }
+          // ---- trajectory (tests / cfg 1) ----
+          if (P.traj && nn - P.traj_n0 < P.traj_steps && loc >= 0) {
+            R* t = P.traj + (((size_t)loc * P.traj_steps + (size_t)(nn - P.traj_n0)) * 7) * N + k;
+            if (pop == 0) { t[0] = st.nu; t[2 * N] = st.Cs; t[3 * N] = st.Cei; t[5 * N] = st.W; }
+            else { t[N] = st.nu; t[4 * N] = st.Cs; t[6 * N] = st.W; }
+          }
+          // ---- S6 temporal average (A17) ----
+          st.win += st.nu;
+          if (--win_left == 0) {
+            win_left = P.ds;
+            if (nn + 1 > P.discard_steps) {
+              const R m = st.win * inv_ds;
+              if (pop == 0) P.xbar[(((size_t)g * P.chunk_samples + sidx) * N + k) * SPC + sl] = m;
+              st.sum += (double)m;
+              ++sidx;
+            }
+            st.win = R(0);
+          }
+        }
+        __syncwarp(mask);
       }
-      if (!SINGLE) store_local<R, SPC>(P, g, k, sl, st);
+      if (!SINGLE) store_local<R>(P, g, k, sl, pop, st);
     }
-    if (rl >= N || N <= 0) {   // idle lanes still have to advance the uniform counters
-      win_left = win_left0; sidx = sidx0;
-      for (int i = 0; i < nb; ++i) {
-        if (--win_left == 0) { win_left = P.ds; if (n + i + 1 > P.discard_steps) ++sidx; }
-      }
-    }
-    win_left0 = win_left; sidx0 = sidx;
+    win_left0 = win_left; sidx0 = sidx;      // (lanes that never work never use them)
     n += nb;
     cur += nb; if (cur >= Hp) cur -= Hp;
     __syncthreads();
   }
-  if (SINGLE && rl < N) store_local<R, SPC>(P, g, rl, sl, st);
+  if (SINGLE && rl < N) store_local<R>(P, g, rl, sl, pop, st);
 }
 
 }  // namespace tvbx
