@@ -225,7 +225,8 @@ struct DeviceImpl : DeviceSide {
   DevBuf<Edge<R>> d_edges;
   DevBuf<int32_t> d_rowptr, d_ext, d_loc;
   DevBuf<R> d_psim, d_ring, d_state, d_xbar;
-  DevBuf<double> d_sums, d_cmean, d_mean, d_M;
+  DevBuf<double> d_sums, d_cmean, d_mean, d_M, d_M_scratch, d_mean_scratch;
+  DevBuf<float> d_out_fc, d_out_me, d_out_mi;
   IntegrateParams<R> P;
   KernelPick<R> kp{nullptr};
   int threads = 0, smem = 0;
@@ -261,6 +262,7 @@ struct DeviceImpl : DeviceSide {
       ht.D = D; ht.dmin = dmin; ht.B = block_steps(dmin); ht.Hp = D + ht.B + 1;
       const int32_t Hs = ht.Hp + GC - 1;
       if (Hs > 65535 || N > 65535) return fail(TVBX_EINVAL, "ring of %d slots (or %d regions) exceeds the 16-bit edge packing", Hs, N);
+      if ((double)N * Hs * SPC >= 4294967295.0) return fail(TVBX_EINVAL, "ring of one CTA exceeds 32-bit element offsets");
       tds[t].Hp = ht.Hp; tds[t].Hs = Hs; tds[t].B = ht.B; tds[t].n_edges = (int32_t)c.edges.size();
       tds[t].edge_off = (int64_t)edges.size(); tds[t].rowptr_off = (int64_t)rowptr.size();
       for (size_t e = 0; e < c.edges.size(); ++e) {
@@ -381,7 +383,7 @@ struct DeviceImpl : DeviceSide {
     threads = 2 * SPC * rt;
     kp = pick_kernel<R>(single, tf.same_tau != 0);
     const size_t tbytes = c.edges.size() * sizeof(Edge<R>) + (size_t)(N + 1) * 4;
-    const size_t base = (size_t)GC * (threads / 2) * sizeof(R) + 20 * sizeof(R) + 16;
+    const size_t base = ((size_t)(GC + 8) * (threads / 2) + (size_t)L_NPAR * threads + 20) * sizeof(R) + 16;
     P.smem_table = base + tbytes <= 200 * 1024;
     smem = (int)(base + (P.smem_table ? tbytes : 0));
     CU(cudaFuncSetAttribute((const void*)kp.fn, cudaFuncAttributeMaxDynamicSharedMemorySize, std::max(smem, 1024)));
@@ -481,24 +483,24 @@ struct DeviceImpl : DeviceSide {
     const int N = sw->conn.n, SPC = sw->spc, G = (int)sw->groups.size();
     const int64_t total = sw->cnt + sw->fill;
     if (total < 2) return fail(TVBX_ESTATE, "fewer than 2 samples kept (%lld)", (long long)total);
-    DevBuf<double> tM, tmean;
+    DevBuf<double>& tM = d_M_scratch; DevBuf<double>& tmean = d_mean_scratch;   // allocated once, kept
     const double* Msrc = d_M.p;
     if (sw->fill > 0) {     // merge the open chunk into a scratch copy; the accumulators stay untouched
-      CU(tM.alloc(d_M.n)); CU(tmean.alloc(d_mean.n));
+      if (tM.n != d_M.n) { CU(tM.alloc(d_M.n)); CU(tmean.alloc(d_mean.n)); }
       CU(cudaMemcpyAsync(tM.p, d_M.p, d_M.n * sizeof(double), cudaMemcpyDeviceToDevice, st));
       CU(cudaMemcpyAsync(tmean.p, d_mean.p, d_mean.n * sizeof(double), cudaMemcpyDeviceToDevice, st));
       int32_t rc = accumulate(tM.p, tmean.p, sw->cnt, (int)sw->fill, st);
       if (rc) return rc;
       Msrc = tM.p;
     }
-    DevBuf<float> dfc, dme, dmi;
+    DevBuf<float>& dfc = d_out_fc; DevBuf<float>& dme = d_out_me; DevBuf<float>& dmi = d_out_mi;   // kept between calls
     ReadoutParams Q;
     Q.M = Msrc; Q.sums = d_sums.p; Q.loc_id = d_loc.p; Q.cnt = total; Q.N = N; Q.SPC = SPC; Q.G = G;
     Q.fc = fc; Q.mean_e = me; Q.mean_i = mi;
     if (!on_device) {
-      if (fc) { CU(dfc.alloc((size_t)sw->n_sims * N * N)); Q.fc = dfc.p; }
-      if (me) { CU(dme.alloc((size_t)sw->n_sims * N)); Q.mean_e = dme.p; }
-      if (mi) { CU(dmi.alloc((size_t)sw->n_sims * N)); Q.mean_i = dmi.p; }
+      if (fc) { if (dfc.n != (size_t)sw->n_sims * N * N) CU(dfc.alloc((size_t)sw->n_sims * N * N)); Q.fc = dfc.p; }
+      if (me) { if (dme.n != (size_t)sw->n_sims * N) CU(dme.alloc((size_t)sw->n_sims * N)); Q.mean_e = dme.p; }
+      if (mi) { if (dmi.n != (size_t)sw->n_sims * N) CU(dmi.alloc((size_t)sw->n_sims * N)); Q.mean_i = dmi.p; }
     }
     dim3 grid((N * N + 255) / 256, G * SPC);
     sw->prof_begin(K_READOUT, st);
@@ -511,8 +513,6 @@ struct DeviceImpl : DeviceSide {
       if (me) { CU(cudaMemcpyAsync(me, dme.p, dme.n * sizeof(float), cudaMemcpyDeviceToHost, st)); sw->d2h += (int64_t)(dme.n * sizeof(float)); }
       if (mi) { CU(cudaMemcpyAsync(mi, dmi.p, dmi.n * sizeof(float), cudaMemcpyDeviceToHost, st)); sw->d2h += (int64_t)(dmi.n * sizeof(float)); }
       CU(cudaStreamSynchronize(st));
-    } else if (sw->fill > 0) {
-      CU(cudaStreamSynchronize(st));   // scratch copies are freed on return
     }
     return TVBX_OK;
   }

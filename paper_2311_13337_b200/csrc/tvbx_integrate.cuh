@@ -39,15 +39,18 @@ __device__ __forceinline__ void philox4x32_10(uint32_t c0, uint32_t c1, uint32_t
   out[0] = c0; out[1] = c1; out[2] = c2; out[3] = c3;
 }
 
-// two N(0,1) variates from two 32-bit words: Box-Muller on 23-bit uniforms (exact in FP32 and FP64)
+// two N(0,1) variates from two 32-bit words: Box-Muller on 23-bit uniforms u = (k + 1/2) 2^-23 (exact
+// in FP32 and FP64, A12).  FP32: r = sqrt(-2 ln u1) and sin/cos(2 pi u2) on the SFU (lg2, sqrt, sin, cos
+// approximations, absolute error ~1e-6 on a unit-variance variate); FP64: libm.
 template <typename R> __device__ __forceinline__ void box_muller(uint32_t xa, uint32_t xb, R& zc, R& zs);
 template <> __device__ __forceinline__ void box_muller<float>(uint32_t xa, uint32_t xb, float& zc, float& zs) {
   const float u1 = ((float)(xa >> 9) + 0.5f) * (1.0f / 8388608.0f);
   const float u2 = ((float)(xb >> 9) + 0.5f) * (1.0f / 8388608.0f);
-  const float r = sqrtf(-2.0f * logf(u1));
-  float s, c;
-  sincospif(2.0f * u2, &s, &c);
-  zc = r * c; zs = r * s;
+  float l2, r;
+  asm("lg2.approx.ftz.f32 %0, %1;" : "=f"(l2) : "f"(u1));
+  asm("sqrt.approx.ftz.f32 %0, %1;" : "=f"(r) : "f"(-1.3862943611198906f * l2));     // -2 ln2 log2(u1)
+  const float th = 6.2831853071795865f * u2;
+  zc = r * __cosf(th); zs = r * __sinf(th);
 }
 template <> __device__ __forceinline__ void box_muller<double>(uint32_t xa, uint32_t xb, double& zc, double& zs) {
   const double u1 = ((double)(xa >> 9) + 0.5) * (1.0 / 8388608.0);
@@ -155,6 +158,10 @@ __device__ __forceinline__ void store_local(const IntegrateParams<R>& P, int g, 
   P.sums[(size_t)g * 2 * stride + pop * stride + (size_t)k * P.SPC + sl] = s.sum;
 }
 
+// per-lane constants kept in shared memory (one column per thread; 64 registers per thread do not
+// hold them next to the transfer function's temporaries)
+enum { L_G = 0, L_WN, L_IT, L_B, L_AT, L_ITW, L_ATEL, L_GLEL, L_CFE, L_CFI, L_INVN, L_NPAR };
+
 // SINGLE: every (sim, region) of the group has its own lane pair (blockDim >= 2*N*SPC): state stays
 // in registers for the whole launch.  Otherwise the CTA makes several passes over the regions inside
 // each time block and the state round-trips through global memory (L1/L2 resident).
@@ -164,9 +171,10 @@ __global__ void __launch_bounds__(MAXT, 1) integrate_kernel(const __grid_constan
   extern __shared__ __align__(16) unsigned char smem_raw[];
   const int g = blockIdx.x;
   const int N = P.N, SPC = P.SPC;
+  const int T = blockDim.x;
   const int pop = threadIdx.x & 1;
   const int pair = threadIdx.x >> 1;
-  const int PT = blockDim.x >> 1;                 // lane pairs per CTA (a multiple of SPC)
+  const int PT = T >> 1;                          // lane pairs per CTA (a multiple of SPC)
   const int RT = PT / SPC;                        // regions per pass
   const int rl = pair / SPC, sl = pair - rl * SPC;
   const GroupDesc gd = P.groups[g];
@@ -174,9 +182,12 @@ __global__ void __launch_bounds__(MAXT, 1) integrate_kernel(const __grid_constan
   const int Hp = td.Hp, Hs = td.Hs;
   const Edge<R>* edges = P.edges + td.edge_off;
   const int32_t* rowptr = P.rowptr + td.rowptr_off;
-  // shared memory: [GC][PT] coupling sums, 2 x 10 polynomial coefficients, then the optional tables
-  R* s_cpl = reinterpret_cast<R*>(smem_raw);
-  R* s_poly = s_cpl + (size_t)GC * PT;
+  // shared memory: [GC][PT] coupling sums | [8][PT] normals | [L_NPAR][T] lane constants | 2 x 10
+  // polynomial coefficients | optional edge table + row pointers
+  R* s_cpl = reinterpret_cast<R*>(smem_raw) + pair;
+  R* s_xi = reinterpret_cast<R*>(smem_raw) + (size_t)GC * PT + pair;
+  R* s_par = reinterpret_cast<R*>(smem_raw) + (size_t)(GC + 8) * PT + threadIdx.x;
+  R* s_poly = reinterpret_cast<R*>(smem_raw) + (size_t)(GC + 8) * PT + (size_t)L_NPAR * T;
   {
     unsigned char* tab = reinterpret_cast<unsigned char*>(s_poly + 20);
     tab += (16 - (reinterpret_cast<uintptr_t>(tab) & 15)) & 15;
@@ -185,35 +196,37 @@ __global__ void __launch_bounds__(MAXT, 1) integrate_kernel(const __grid_constan
     if (P.smem_table) {
       Edge<R>* se = reinterpret_cast<Edge<R>*>(tab);
       int32_t* sr = reinterpret_cast<int32_t*>(se + td.n_edges);
-      for (int i = threadIdx.x; i < td.n_edges; i += blockDim.x) se[i] = edges[i];
-      for (int i = threadIdx.x; i <= N; i += blockDim.x) sr[i] = rowptr[i];
+      for (int i = threadIdx.x; i < td.n_edges; i += T) se[i] = edges[i];
+      for (int i = threadIdx.x; i <= N; i += T) sr[i] = rowptr[i];
       edges = se; rowptr = sr;
     }
+    // per-simulation scalars of this lane's population
+    const R* ps = P.psim + (size_t)g * NPS * SPC + sl;
+    const R pEL = ps[(5 + pop) * SPC];
+    const R pAT = pop ? P.a_i_over_tau : ps[3 * SPC];
+    s_par[L_G * T] = ps[0 * SPC]; s_par[L_WN * T] = ps[1 * SPC]; s_par[L_IT * T] = ps[7 * SPC];
+    s_par[L_B * T] = pop ? P.b_i : ps[2 * SPC];                 // b
+    s_par[L_AT * T] = pAT;                                      // a / tau_w
+    s_par[L_ITW * T] = pop ? P.inv_tau_w_i : ps[4 * SPC];       // 1 / tau_w
+    s_par[L_ATEL * T] = pAT * pEL;
+    s_par[L_GLEL * T] = P.tf.gL * pEL;
+    s_par[L_CFE * T] = ps[(pop ? 10 : 8) * SPC]; s_par[L_CFI * T] = ps[(pop ? 11 : 9) * SPC];
+    s_par[L_INVN * T] = pop ? P.inv_Ni : P.inv_Ne;
     __syncthreads();
   }
   const R* poly = s_poly + 10 * pop;
-  R* ring = P.ring + gd.ring_off + (size_t)sl * N * Hs;     // this simulation's [N][Hs]
-
-  // per-simulation scalars of this lane's population
-  const R* ps = P.psim + (size_t)g * NPS * SPC + sl;
-  const R pG = ps[0 * SPC], pWn = ps[1 * SPC], pIT = ps[7 * SPC];
-  const R pB = pop ? P.b_i : ps[2 * SPC];                  // b
-  const R pAT = pop ? P.a_i_over_tau : ps[3 * SPC];        // a / tau_w
-  const R pITw = pop ? P.inv_tau_w_i : ps[4 * SPC];        // 1 / tau_w
-  const R pEL = ps[(5 + pop) * SPC];
-  const R cFe = ps[(pop ? 10 : 8) * SPC], cFi = ps[(pop ? 11 : 9) * SPC];
-  const R gLEL = P.tf.gL * pEL;
-  const R invNp = pop ? P.inv_Ni : P.inv_Ne;
+  // ring[group][region][slot][sim]: this lane's simulation column, as 32-bit element offsets
+  R* const ringg = P.ring + gd.ring_off;
+  const uint32_t uSPC = (uint32_t)SPC, usl = (uint32_t)sl;
   const int ext = P.ext_id[(size_t)g * SPC + sl];
   const int loc = P.loc_id[(size_t)g * SPC + sl];
-  const R dt = P.dt, kap = P.kappa, kap2 = P.kappa * P.kappa;
+  const R dt = P.dt;
   const R inv_ds = P.ds > 0 ? R(1) / R(P.ds) : R(0);
   const bool noise = P.noise_on != 0;
 
   Local<R> st;
   st.nu = st.Cs = st.Cei = st.W = st.ou = st.win = R(0); st.sum = 0.0;
   if (SINGLE && rl < N) load_local<R>(P, g, rl, sl, pop, st);
-  R xi[4] = {R(0), R(0), R(0), R(0)};   // the four normals of the Philox call this lane owns
 
   int64_t n = P.n_begin;
   int cur = (int)(n % Hp);                       // ring slot of time index n
@@ -231,10 +244,16 @@ __global__ void __launch_bounds__(MAXT, 1) integrate_kernel(const __grid_constan
       if (!SINGLE) load_local<R>(P, g, k, sl, pop, st);
       win_left = win_left0; sidx = sidx0;
       const int e0 = rowptr[k], e1 = rowptr[k + 1];
-      R* myring = ring + (size_t)k * Hs;
-      // this lane owns the Philox quads q with (q & 1) == pop; re-enter a partly used quad
-      if (noise && (n & 3) && (int)((n >> 2) & 1) == pop && (!SINGLE || n == P.n_begin))
-        normals4<R>(P.seed, (uint32_t)ext, (uint32_t)k, (uint64_t)n >> 2, xi);
+      const uint32_t myrow = (uint32_t)(k * Hs) * uSPC + usl;
+      // Philox: at every step that is a multiple of 8 the even lane draws the quad of steps 8m..8m+3, the
+      // odd lane that of 8m+4..8m+7 (no divergence); re-enter a partly used octet here
+      if (noise && (n & 7) && (!SINGLE || n == P.n_begin)) {
+        R xi[4];
+        normals4<R>(P.seed, (uint32_t)ext, (uint32_t)k, (((uint64_t)n >> 3) << 1) + pop, xi);
+#pragma unroll
+        for (int q = 0; q < 4; ++q) s_xi[(pop * 4 + q) * PT] = xi[q];
+        __syncwarp(mask);
+      }
       int c = cur;
       for (int c0 = 0; c0 < nb; c0 += GC) {
         const int ch = min(GC, nb - c0);
@@ -248,85 +267,88 @@ __global__ void __launch_bounds__(MAXT, 1) integrate_kernel(const __grid_constan
               const Edge<R> ed = edges[e];
               int start = c + (int)(ed.jd >> 16);
               start = start >= Hp ? start - Hp : start;
-              const R* src = ring + (size_t)(ed.jd & 0xffffu) * Hs + start;
+              const uint32_t o = ((ed.jd & 0xffffu) * (uint32_t)Hs + (uint32_t)start) * uSPC + usl;
 #pragma unroll
-              for (int i = 0; i < GC; ++i) acc[i] = tfma(ed.w, src[i], acc[i]);
+              for (int i = 0; i < GC; ++i) acc[i] = tfma(ed.w, ringg[o + (uint32_t)i * uSPC], acc[i]);
             }
           } else {
             for (int e = e0 + pop; e < e1; e += 2) {
               const Edge<R> ed = edges[e];
               int start = c + (int)(ed.jd >> 16);
               start = start >= Hp ? start - Hp : start;
-              const R* src = ring + (size_t)(ed.jd & 0xffffu) * Hs + start;
+              const uint32_t o = ((ed.jd & 0xffffu) * (uint32_t)Hs + (uint32_t)start) * uSPC + usl;
 #pragma unroll
               for (int i = 0; i < GC; ++i)
-                if (i < ch) acc[i] = tfma(ed.w, src[i], acc[i]);
+                if (i < ch) acc[i] = tfma(ed.w, ringg[o + (uint32_t)i * uSPC], acc[i]);
             }
           }
 #pragma unroll
           for (int i = 0; i < GC; ++i) {
-            const R tot = acc[i] + shfl_x1(mask, acc[i]);          // a + b == b + a: both lanes get the same bits
-            if (pop == 0) s_cpl[i * PT + pair] = tot;
+            const R tot = acc[i] + shfl_x1(mask, acc[i]);    // a + b == b + a: both lanes get the same bits
+            if (pop == 0) s_cpl[i * PT] = tot;
           }
           __syncwarp(mask);
         }
         // ================= COMPUTE: ch steps in registers (S2-S6) =================
+        const int64_t nn0 = n + c0;
+        const bool traj_on = P.traj != nullptr && loc >= 0 && nn0 - P.traj_n0 < P.traj_steps;
         for (int i = 0; i < ch; ++i) {
-          const int64_t nn = n + c0 + i;
-          const R cpl = s_cpl[i * PT + pair];
+          const uint32_t nlo = (uint32_t)nn0 + (uint32_t)i;      // low bits of the step index
+          // ---- noise: new octet of normals ----
+          if (noise && (nlo & 7u) == 0) {
+            R xi[4];
+            __syncwarp(mask);
+            normals4<R>(P.seed, (uint32_t)ext, (uint32_t)k, ((uint64_t)(nn0 + i) >> 2) + pop, xi);
+#pragma unroll
+            for (int q = 0; q < 4; ++q) s_xi[(pop * 4 + q) * PT] = xi[q];
+            __syncwarp(mask);
+          }
+          const R cpl = s_cpl[i * PT];
           // ---- exchange with the partner lane ----
           const R nu_o = shfl_x1(mask, st.nu), Cs_o = shfl_x1(mask, st.Cs);
           const R E = pop ? nu_o : st.nu, I = pop ? st.nu : nu_o;
-          const R Cee = pop ? Cs_o : st.Cs, Cii = pop ? st.Cs : Cs_o, Cei = st.Cei;
-          // ---- noise: the owner of quad q = nn/4 provides xi ----
-          if (noise && (nn & 3) == 0 && (int)((nn >> 2) & 1) == pop)
-            normals4<R>(P.seed, (uint32_t)ext, (uint32_t)k, (uint64_t)nn >> 2, xi);
-          R x_n = R(0);
-          if (noise) {
-            const int w = (int)(nn & 3);      // select chain keeps xi[] in registers
-            const R x_own = w == 0 ? xi[0] : (w == 1 ? xi[1] : (w == 2 ? xi[2] : xi[3]));
-            const R x_oth = shfl_x1(mask, x_own);
-            x_n = (int)((nn >> 2) & 1) == pop ? x_own : x_oth;
-          }
+          const R Cei = st.Cei;
+          const R Ca = pop ? Cei : st.Cs, Cb = pop ? st.Cs : Cei;     // row `pop` of C   (own covariance)
+          const R Co = pop ? Cs_o : Cei, Cp = pop ? Cei : Cs_o;       // the other row    (half of the C_ei equation)
           // ---- S2 inputs and transfer function of this lane's population (Eq. 5; A5, A6, A10) ----
-          const R eta = noise ? pWn * st.ou : R(0);
-          const R drive = tfma(pG, cpl, E) + eta;
-          const R xe = drive + cFe, xi_ = I + cFi;
-          const R se = xe > R(0) ? kap : R(0), si = xi_ > R(0) ? kap : R(0);
+          R drive = tfma(s_par[L_G * T], cpl, E);
+          if (noise) drive = tfma(s_par[L_WN * T], st.ou, drive);
+          const R xe = drive + s_par[L_CFE * T], xi_ = I + s_par[L_CFI * T];
+          const R se = xe > R(0) ? P.kappa : R(0), si = xi_ > R(0) ? P.kappa : R(0);   // A22 and the clamp of A10
+          const R c0w = s_par[L_GLEL * T] - st.W;
           R muV;
           Jet<R> F;
-          if (CLOSED) F = tf_closed<R>(P.tf, poly, fmax(xe, R(0)) + P.tf.eps, fmax(xi_, R(0)) + P.tf.eps, gLEL - st.W, &muV);
-          else        F = tf_jet<R>(P.tf, poly, fmax(xe, R(0)) + P.tf.eps, fmax(xi_, R(0)) + P.tf.eps, gLEL - st.W, &muV);
-          F.e *= se; F.i *= si;               // A22 (kappa) and the clamp of A10
-          F.ee *= se * se; F.ei *= se * si; F.ii *= si * si;
+          if (CLOSED) F = tf_closed<R>(P.tf, poly, fmax(xe, R(0)) + P.tf.eps, fmax(xi_, R(0)) + P.tf.eps, c0w, &muV);
+          else        F = tf_jet<R>(P.tf, poly, fmax(xe, R(0)) + P.tf.eps, fmax(xi_, R(0)) + P.tf.eps, c0w, &muV);
           if (P.muV_local)                    // A9b alternative: mu_V of the local rates only
-            muV = mu_V_only<R>(P.tf, fmax(E, R(0)) + P.tf.eps, fmax(I, R(0)) + P.tf.eps, gLEL - st.W);
+            muV = mu_V_only<R>(P.tf, fmax(E, R(0)) + P.tf.eps, fmax(I, R(0)) + P.tf.eps, c0w);
+          const R Fe = F.e * se, Fi = F.i * si;
           // ---- S3 Eqs. (1)-(3), forward Euler (A7, A9) ----
+          const R pIT = s_par[L_IT * T];
           const R dF = F.v - st.nu;
-          const R dnu = (dF + R(0.5) * Cee * F.ee + Cei * F.ei + R(0.5) * Cii * F.ii) * pIT;
-          // row `pop` of C with grad F (own covariance), the other row (half of the C_ei equation)
-          const R Ca = pop ? Cei : Cee, Cb = pop ? Cii : Cei;
-          const R Co = pop ? Cee : Cei, Cp = pop ? Cei : Cii;
-          const R dCs = (F.v * (pIT - F.v) * invNp + dF * dF + R(2) * (Ca * F.e + Cb * F.i) - R(2) * st.Cs) * pIT;
-          const R h = Co * F.e + Cp * F.i;
+          const R Cee_h = R(0.5) * (pop ? Co : Ca) * se * se, Cei_s = Cei * se * si, Cii_h = R(0.5) * (pop ? Cb : Cp) * si * si;
+          const R dnu = tfma(Cee_h, F.ee, tfma(Cei_s, F.ei, tfma(Cii_h, F.ii, dF))) * pIT;
+          const R dCs = tfma(F.v * (pIT - F.v), s_par[L_INVN * T], tfma(dF, dF, R(2) * (tfma(Ca, Fe, Cb * Fi) - st.Cs))) * pIT;
+          const R h = tfma(Co, Fe, Cp * Fi);
           const R dF_o = shfl_x1(mask, dF), h_o = shfl_x1(mask, h);
-          const R dCei = (dF * dF_o + (h + h_o) - R(2) * Cei) * pIT;
-          const R dW = -st.W * pITw + pB * st.nu + pAT * (muV - pEL);
+          const R dCei = tfma(dF, dF_o, (h + h_o) - R(2) * Cei) * pIT;
+          const R dW = tfma(s_par[L_AT * T], muV, tfma(s_par[L_B * T], st.nu, -tfma(st.W, s_par[L_ITW * T], s_par[L_ATEL * T])));
           st.nu = tfma(dt, dnu, st.nu);
           st.Cs = tfma(dt, dCs, st.Cs);
           st.Cei = tfma(dt, dCei, st.Cei);
           st.W = tfma(dt, dW, st.W);
           // ---- S4 OU (Eq. 4, A11) ----
-          if (noise) st.ou = tfma(P.ou_rho, st.ou, tfma(P.ou_s, x_n, P.ou_m));
+          if (noise) st.ou = tfma(P.ou_rho, st.ou, tfma(P.ou_s, s_xi[(nlo & 7u) * PT], P.ou_m));
           // ---- S5 ring write: E at time nn+1 (mirror the first GC-1 slots behind the period) ----
           c = c + 1 == Hp ? 0 : c + 1;
           if (pop == 0) {
-            myring[c] = st.nu;
-            if (c < GC - 1) myring[Hp + c] = st.nu;
+            const uint32_t o = myrow + (uint32_t)c * uSPC;
+            ringg[o] = st.nu;
+            if (c < GC - 1) ringg[o + (uint32_t)Hp * uSPC] = st.nu;
           }
           // ---- trajectory (tests / cfg 1) ----
-          if (P.traj && nn - P.traj_n0 < P.traj_steps && loc >= 0) {
-            R* t = P.traj + (((size_t)loc * P.traj_steps + (size_t)(nn - P.traj_n0)) * 7) * N + k;
+          if (traj_on && nn0 + i - P.traj_n0 < P.traj_steps) {
+            R* t = P.traj + (((size_t)loc * P.traj_steps + (size_t)(nn0 + i - P.traj_n0)) * 7) * N + k;
             if (pop == 0) { t[0] = st.nu; t[2 * N] = st.Cs; t[3 * N] = st.Cei; t[5 * N] = st.W; }
             else { t[N] = st.nu; t[4 * N] = st.Cs; t[6 * N] = st.W; }
           }
@@ -334,7 +356,7 @@ __global__ void __launch_bounds__(MAXT, 1) integrate_kernel(const __grid_constan
           st.win += st.nu;
           if (--win_left == 0) {
             win_left = P.ds;
-            if (nn + 1 > P.discard_steps) {
+            if (nn0 + i + 1 > P.discard_steps) {
               const R m = st.win * inv_ds;
               if (pop == 0) P.xbar[(((size_t)g * P.chunk_samples + sidx) * N + k) * SPC + sl] = m;
               st.sum += (double)m;

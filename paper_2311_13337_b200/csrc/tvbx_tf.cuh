@@ -69,6 +69,32 @@ template <typename R> __device__ __forceinline__ R t_exp(R x);
 template <> __device__ __forceinline__ float t_exp<float>(float x) { return __expf(x); }
 template <> __device__ __forceinline__ double t_exp<double>(double x) { return exp(x); }
 
+// E0 = erfc(z)/2 and ex = exp(-z^2) together.  FP32: erfc(z) = exp(-z^2) * erfcx(z) with
+// erfcx(a) = t R(t), t = 1/(1 + 0.4 a), a = |z|; R is a degree-8 least-squares fit of erfcx(a)/t on
+// t in (0, 1] (coefficients from csrc/gen_erfcx_coeffs.py; relative error of t R(t) evaluated in
+// FP32 <= 4.7e-7 for all a >= 0), and erfc(-a) = 2 - erfc(a).  FP64: libm.
+template <typename R> __device__ __forceinline__ R half_erfc(R z, R* ex);
+template <> __device__ __forceinline__ float half_erfc<float>(float z, float* ex) {
+  const float e = __expf(-z * z);
+  const float t = t_rcp(tfma(0.4f, fabsf(z), 1.0f));
+  float p = 5.018728834e-02f;
+  p = tfma(p, t, -1.826153469e-01f);
+  p = tfma(p, t, 1.686438582e-01f);
+  p = tfma(p, t, -5.255410161e-03f);
+  p = tfma(p, t, 1.412773411e-01f);
+  p = tfma(p, t, 1.685781716e-01f);
+  p = tfma(p, t, 2.078385839e-01f);
+  p = tfma(p, t, 2.256697733e-01f);
+  p = tfma(p, t, 2.256758607e-01f);
+  const float h = 0.5f * e * t * p;
+  *ex = e;
+  return z >= 0.0f ? h : 1.0f - h;
+}
+template <> __device__ __forceinline__ double half_erfc<double>(double z, double* ex) {
+  *ex = exp(-z * z);
+  return 0.5 * erfc(z);
+}
+
 // mu_V alone (value), for the A9b option
 template <typename R>
 __device__ __forceinline__ R mu_V_only(const TFConst<R>& c, R fe, R fi, R gLEL_mW) {
@@ -150,8 +176,9 @@ __device__ __forceinline__ Jet<R> tf_closed(const TFConst<R>& c, const R* __rest
   const R z_ei = Wz * tfma(u, tfma(Le, Li, -Lei), tfma(-u_e, Li, tfma(-u_i, Le, u_ei)));
   const R z_ii = Wz * tfma(u, tfma(Li, Li, -Lii), tfma(R(-2) * u_i, Li, u_ii));
   // E = erfc(z)/2:  E' = -exp(-z^2)/sqrt(pi),  E'' = -2 z E'
-  const R E0 = R(0.5) * t_erfc(z);
-  const R g0 = R(-0.56418958354775628695) * t_exp(-z * z);
+  R ex;
+  const R E0 = half_erfc<R>(z, &ex);
+  const R g0 = R(-0.56418958354775628695) * ex;
   const R zz = -(z + z);
   const R E_e = g0 * z_e, E_i = g0 * z_i;
   const R E_ee = g0 * tfma(zz * z_e, z_e, z_ee), E_ei = g0 * tfma(zz * z_e, z_i, z_ei), E_ii = g0 * tfma(zz * z_i, z_i, z_ii);
