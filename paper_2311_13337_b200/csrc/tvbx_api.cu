@@ -210,11 +210,28 @@ template <typename R> struct MaxT;
 template <> struct MaxT<float> { static constexpr int v = 1024; };
 template <> struct MaxT<double> { static constexpr int v = 384; };
 
+// compile-time simulations-per-CTA values of the FP32 closed-form kernel (else runtime SPC)
+inline bool spc_is_templated(int spc) { return spc == 1 || spc == 2 || spc == 4 || spc == 7; }
+
 template <typename R>
-KernelPick<R> pick_kernel(bool single, bool closed) {
-  constexpr int MT = MaxT<R>::v;
-  if (single) return closed ? KernelPick<R>{integrate_kernel<R, true, true, MT>} : KernelPick<R>{integrate_kernel<R, true, false, MT>};
-  return closed ? KernelPick<R>{integrate_kernel<R, false, true, MT>} : KernelPick<R>{integrate_kernel<R, false, false, MT>};
+KernelPick<R> pick_kernel(bool single, bool closed, int spc);
+template <>
+KernelPick<double> pick_kernel<double>(bool single, bool closed, int) {
+  constexpr int MT = MaxT<double>::v;
+  if (single) return closed ? KernelPick<double>{integrate_kernel<double, true, true, 0, MT>} : KernelPick<double>{integrate_kernel<double, true, false, 0, MT>};
+  return closed ? KernelPick<double>{integrate_kernel<double, false, true, 0, MT>} : KernelPick<double>{integrate_kernel<double, false, false, 0, MT>};
+}
+template <>
+KernelPick<float> pick_kernel<float>(bool single, bool closed, int spc) {
+  constexpr int MT = MaxT<float>::v;
+  if (!closed) return single ? KernelPick<float>{integrate_kernel<float, true, false, 0, MT>} : KernelPick<float>{integrate_kernel<float, false, false, 0, MT>};
+#define TVBX_CASE(S) case S: return single ? KernelPick<float>{integrate_kernel<float, true, true, S, MT>} : KernelPick<float>{integrate_kernel<float, false, true, S, MT>};
+  switch (spc) {
+    TVBX_CASE(1) TVBX_CASE(2) TVBX_CASE(4) TVBX_CASE(7)
+    default: break;
+  }
+#undef TVBX_CASE
+  return single ? KernelPick<float>{integrate_kernel<float, true, true, 0, MT>} : KernelPick<float>{integrate_kernel<float, false, true, 0, MT>};
 }
 
 template <typename R>
@@ -261,7 +278,6 @@ struct DeviceImpl : DeviceSide {
       if (c.edges.empty()) dmin = 0;
       ht.D = D; ht.dmin = dmin; ht.B = block_steps(dmin); ht.Hp = D + ht.B + 1;
       const int32_t Hs = ht.Hp + GC - 1;
-      if (Hs > 65535 || N > 65535) return fail(TVBX_EINVAL, "ring of %d slots (or %d regions) exceeds the 16-bit edge packing", Hs, N);
       if ((double)N * Hs * SPC >= 4294967295.0) return fail(TVBX_EINVAL, "ring of one CTA exceeds 32-bit element offsets");
       tds[t].Hp = ht.Hp; tds[t].Hs = Hs; tds[t].B = ht.B; tds[t].n_edges = (int32_t)c.edges.size();
       tds[t].edge_off = (int64_t)edges.size(); tds[t].rowptr_off = (int64_t)rowptr.size();
@@ -269,7 +285,8 @@ struct DeviceImpl : DeviceSide {
         Edge<R> ed;
         std::memset(&ed, 0, sizeof ed);
         ed.w = (R)c.edges[e].w;
-        ed.jd = (uint32_t)c.edges[e].j | ((uint32_t)(ht.Hp - ht.delays[e]) << 16);
+        ed.jbase = (uint32_t)c.edges[e].j * (uint32_t)Hs * (uint32_t)SPC;
+        ed.back = (uint32_t)(ht.Hp - ht.delays[e]);
         edges.push_back(ed);
       }
       rowptr.insert(rowptr.end(), c.rowptr.begin(), c.rowptr.end());
@@ -381,9 +398,9 @@ struct DeviceImpl : DeviceSide {
     if (N <= rt_max) { single = true; rt = N; }
     else { single = false; const int passes = (N + rt_max - 1) / rt_max; rt = (N + passes - 1) / passes; }
     threads = 2 * SPC * rt;
-    kp = pick_kernel<R>(single, tf.same_tau != 0);
+    kp = pick_kernel<R>(single, tf.same_tau != 0, SPC);
     const size_t tbytes = c.edges.size() * sizeof(Edge<R>) + (size_t)(N + 1) * 4;
-    const size_t base = ((size_t)(GC + 8) * (threads / 2) + (size_t)L_NPAR * threads + 20) * sizeof(R) + 16;
+    const size_t base = ((size_t)(GC + 10) * (threads / 2) + (size_t)L_NPAR * threads + 20) * sizeof(R) + 16;
     P.smem_table = base + tbytes <= 200 * 1024;
     smem = (int)(base + (P.smem_table ? tbytes : 0));
     CU(cudaFuncSetAttribute((const void*)kp.fn, cudaFuncAttributeMaxDynamicSharedMemorySize, std::max(smem, 1024)));
@@ -646,7 +663,7 @@ int32_t tvbx_sweep_create(const tvbx_connectome* c, const tvbx_model_params* def
       const int64_t resident = std::max<int64_t>(1, maxt_sel / (2 * (int64_t)sw->conn.n * cand));
       const int64_t slots = 148 * resident;
       const int64_t cost = ctas <= slots ? ((ctas + 147) / 148) * cand : ((ctas + slots - 1) / slots) * resident * cand;
-      if (cost < best_cost || (cost == best_cost && cand > spc)) { best_cost = cost; spc = cand; }
+      if (cost < best_cost || (cost == best_cost && (spc_is_templated(cand) || !spc_is_templated(spc)))) { best_cost = cost; spc = cand; }
     }
   }
   if (spc < 1 || spc > 32) return fail(TVBX_EINVAL, "sims_per_cta=%d (valid: 1..32)", spc);

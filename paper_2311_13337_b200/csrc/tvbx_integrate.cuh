@@ -72,10 +72,11 @@ __device__ __forceinline__ void normals4(uint64_t seed, uint32_t sim, uint32_t r
 template <typename R> __device__ __forceinline__ R shfl_x1(unsigned mask, R v) { return __shfl_xor_sync(mask, v, 1); }
 
 // ---- device-side descriptors ------------------------------------------------------------------------
-// one non-zero weight: w = W_kj, jd = j | (Hp - d_kj) << 16   (ring slots and regions < 65536)
+// one non-zero weight: w = W_kj, jbase = j * Hs * SPC (element offset of the source region's ring row),
+// back = Hp - d_kj
 template <typename R> struct Edge;
-template <> struct __align__(8) Edge<float> { float w; uint32_t jd; };
-template <> struct __align__(16) Edge<double> { double w; uint32_t jd; uint32_t pad; };
+template <> struct __align__(16) Edge<float> { float w; uint32_t jbase; uint32_t back; uint32_t pad; };
+template <> struct __align__(16) Edge<double> { double w; uint32_t jbase; uint32_t back; };
 
 struct TableDesc {      // one per distinct speed v
   int32_t Hp;           // ring period D + B + 1
@@ -166,11 +167,13 @@ enum { L_G = 0, L_WN, L_IT, L_B, L_AT, L_ITW, L_ATEL, L_GLEL, L_CFE, L_CFI, L_IN
 // in registers for the whole launch.  Otherwise the CTA makes several passes over the regions inside
 // each time block and the state round-trips through global memory (L1/L2 resident).
 // CLOSED: tau_e == tau_i -> tf_closed, else tf_jet.
-template <typename R, bool SINGLE, bool CLOSED, int MAXT>
+// SPC_T: simulations per CTA as a compile-time constant (0 = take P.SPC): the ring loads of a gather
+// chunk then use immediate offsets.
+template <typename R, bool SINGLE, bool CLOSED, int SPC_T, int MAXT>
 __global__ void __launch_bounds__(MAXT, 1) integrate_kernel(const __grid_constant__ IntegrateParams<R> P) {
   extern __shared__ __align__(16) unsigned char smem_raw[];
   const int g = blockIdx.x;
-  const int N = P.N, SPC = P.SPC;
+  const int N = P.N, SPC = SPC_T > 0 ? SPC_T : P.SPC;
   const int T = blockDim.x;
   const int pop = threadIdx.x & 1;
   const int pair = threadIdx.x >> 1;
@@ -182,12 +185,12 @@ __global__ void __launch_bounds__(MAXT, 1) integrate_kernel(const __grid_constan
   const int Hp = td.Hp, Hs = td.Hs;
   const Edge<R>* edges = P.edges + td.edge_off;
   const int32_t* rowptr = P.rowptr + td.rowptr_off;
-  // shared memory: [GC][PT] coupling sums | [8][PT] normals | [L_NPAR][T] lane constants | 2 x 10
-  // polynomial coefficients | optional edge table + row pointers
-  R* s_cpl = reinterpret_cast<R*>(smem_raw) + pair;
-  R* s_xi = reinterpret_cast<R*>(smem_raw) + (size_t)GC * PT + pair;
-  R* s_par = reinterpret_cast<R*>(smem_raw) + (size_t)(GC + 8) * PT + threadIdx.x;
-  R* s_poly = reinterpret_cast<R*>(smem_raw) + (size_t)(GC + 8) * PT + (size_t)L_NPAR * T;
+  // shared memory: [PT][GC+1] coupling sums | [PT][9] normals | [T][L_NPAR] lane constants (odd row
+  // lengths: conflict-free) | 2 x 10 polynomial coefficients | optional edge table + row pointers
+  R* s_cpl = reinterpret_cast<R*>(smem_raw) + (size_t)pair * (GC + 1);
+  R* s_xi = reinterpret_cast<R*>(smem_raw) + (size_t)PT * (GC + 1) + (size_t)pair * 9;
+  R* s_par = reinterpret_cast<R*>(smem_raw) + (size_t)PT * (GC + 10) + (size_t)threadIdx.x * L_NPAR;
+  R* s_poly = reinterpret_cast<R*>(smem_raw) + (size_t)PT * (GC + 10) + (size_t)L_NPAR * T;
   {
     unsigned char* tab = reinterpret_cast<unsigned char*>(s_poly + 20);
     tab += (16 - (reinterpret_cast<uintptr_t>(tab) & 15)) & 15;
@@ -204,20 +207,20 @@ __global__ void __launch_bounds__(MAXT, 1) integrate_kernel(const __grid_constan
     const R* ps = P.psim + (size_t)g * NPS * SPC + sl;
     const R pEL = ps[(5 + pop) * SPC];
     const R pAT = pop ? P.a_i_over_tau : ps[3 * SPC];
-    s_par[L_G * T] = ps[0 * SPC]; s_par[L_WN * T] = ps[1 * SPC]; s_par[L_IT * T] = ps[7 * SPC];
-    s_par[L_B * T] = pop ? P.b_i : ps[2 * SPC];                 // b
-    s_par[L_AT * T] = pAT;                                      // a / tau_w
-    s_par[L_ITW * T] = pop ? P.inv_tau_w_i : ps[4 * SPC];       // 1 / tau_w
-    s_par[L_ATEL * T] = pAT * pEL;
-    s_par[L_GLEL * T] = P.tf.gL * pEL;
-    s_par[L_CFE * T] = ps[(pop ? 10 : 8) * SPC]; s_par[L_CFI * T] = ps[(pop ? 11 : 9) * SPC];
-    s_par[L_INVN * T] = pop ? P.inv_Ni : P.inv_Ne;
+    s_par[L_G] = ps[0 * SPC]; s_par[L_WN] = ps[1 * SPC]; s_par[L_IT] = ps[7 * SPC];
+    s_par[L_B] = pop ? P.b_i : ps[2 * SPC];                 // b
+    s_par[L_AT] = pAT;                                      // a / tau_w
+    s_par[L_ITW] = pop ? P.inv_tau_w_i : ps[4 * SPC];       // 1 / tau_w
+    s_par[L_ATEL] = pAT * pEL;
+    s_par[L_GLEL] = P.tf.gL * pEL;
+    s_par[L_CFE] = ps[(pop ? 10 : 8) * SPC]; s_par[L_CFI] = ps[(pop ? 11 : 9) * SPC];
+    s_par[L_INVN] = pop ? P.inv_Ni : P.inv_Ne;
     __syncthreads();
   }
   const R* poly = s_poly + 10 * pop;
   // ring[group][region][slot][sim]: this lane's simulation column, as 32-bit element offsets
-  R* const ringg = P.ring + gd.ring_off;
-  const uint32_t uSPC = (uint32_t)SPC, usl = (uint32_t)sl;
+  R* const ringg = P.ring + gd.ring_off + sl;
+  const uint32_t uSPC = (uint32_t)SPC;
   const int ext = P.ext_id[(size_t)g * SPC + sl];
   const int loc = P.loc_id[(size_t)g * SPC + sl];
   const R dt = P.dt;
@@ -244,14 +247,14 @@ __global__ void __launch_bounds__(MAXT, 1) integrate_kernel(const __grid_constan
       if (!SINGLE) load_local<R>(P, g, k, sl, pop, st);
       win_left = win_left0; sidx = sidx0;
       const int e0 = rowptr[k], e1 = rowptr[k + 1];
-      const uint32_t myrow = (uint32_t)(k * Hs) * uSPC + usl;
+      const uint32_t myrow = (uint32_t)(k * Hs) * uSPC;
       // Philox: at every step that is a multiple of 8 the even lane draws the quad of steps 8m..8m+3, the
       // odd lane that of 8m+4..8m+7 (no divergence); re-enter a partly used octet here
       if (noise && (n & 7) && (!SINGLE || n == P.n_begin)) {
         R xi[4];
         normals4<R>(P.seed, (uint32_t)ext, (uint32_t)k, (((uint64_t)n >> 3) << 1) + pop, xi);
 #pragma unroll
-        for (int q = 0; q < 4; ++q) s_xi[(pop * 4 + q) * PT] = xi[q];
+        for (int q = 0; q < 4; ++q) s_xi[pop * 4 + q] = xi[q];
         __syncwarp(mask);
       }
       int c = cur;
@@ -265,27 +268,27 @@ __global__ void __launch_bounds__(MAXT, 1) integrate_kernel(const __grid_constan
           if (ch == GC) {
             for (int e = e0 + pop; e < e1; e += 2) {
               const Edge<R> ed = edges[e];
-              int start = c + (int)(ed.jd >> 16);
+              int start = c + (int)ed.back;
               start = start >= Hp ? start - Hp : start;
-              const uint32_t o = ((ed.jd & 0xffffu) * (uint32_t)Hs + (uint32_t)start) * uSPC + usl;
+              const R* src = ringg + (ed.jbase + (uint32_t)start * uSPC);
 #pragma unroll
-              for (int i = 0; i < GC; ++i) acc[i] = tfma(ed.w, ringg[o + (uint32_t)i * uSPC], acc[i]);
+              for (int i = 0; i < GC; ++i) acc[i] = tfma(ed.w, src[i * SPC], acc[i]);
             }
           } else {
             for (int e = e0 + pop; e < e1; e += 2) {
               const Edge<R> ed = edges[e];
-              int start = c + (int)(ed.jd >> 16);
+              int start = c + (int)ed.back;
               start = start >= Hp ? start - Hp : start;
-              const uint32_t o = ((ed.jd & 0xffffu) * (uint32_t)Hs + (uint32_t)start) * uSPC + usl;
+              const R* src = ringg + (ed.jbase + (uint32_t)start * uSPC);
 #pragma unroll
               for (int i = 0; i < GC; ++i)
-                if (i < ch) acc[i] = tfma(ed.w, ringg[o + (uint32_t)i * uSPC], acc[i]);
+                if (i < ch) acc[i] = tfma(ed.w, src[i * SPC], acc[i]);
             }
           }
 #pragma unroll
           for (int i = 0; i < GC; ++i) {
             const R tot = acc[i] + shfl_x1(mask, acc[i]);    // a + b == b + a: both lanes get the same bits
-            if (pop == 0) s_cpl[i * PT] = tot;
+            if (pop == 0) s_cpl[i] = tot;
           }
           __syncwarp(mask);
         }
@@ -300,10 +303,10 @@ __global__ void __launch_bounds__(MAXT, 1) integrate_kernel(const __grid_constan
             __syncwarp(mask);
             normals4<R>(P.seed, (uint32_t)ext, (uint32_t)k, ((uint64_t)(nn0 + i) >> 2) + pop, xi);
 #pragma unroll
-            for (int q = 0; q < 4; ++q) s_xi[(pop * 4 + q) * PT] = xi[q];
+            for (int q = 0; q < 4; ++q) s_xi[pop * 4 + q] = xi[q];
             __syncwarp(mask);
           }
-          const R cpl = s_cpl[i * PT];
+          const R cpl = s_cpl[i];
           // ---- exchange with the partner lane ----
           const R nu_o = shfl_x1(mask, st.nu), Cs_o = shfl_x1(mask, st.Cs);
           const R E = pop ? nu_o : st.nu, I = pop ? st.nu : nu_o;
@@ -311,11 +314,11 @@ __global__ void __launch_bounds__(MAXT, 1) integrate_kernel(const __grid_constan
           const R Ca = pop ? Cei : st.Cs, Cb = pop ? st.Cs : Cei;     // row `pop` of C   (own covariance)
           const R Co = pop ? Cs_o : Cei, Cp = pop ? Cei : Cs_o;       // the other row    (half of the C_ei equation)
           // ---- S2 inputs and transfer function of this lane's population (Eq. 5; A5, A6, A10) ----
-          R drive = tfma(s_par[L_G * T], cpl, E);
-          if (noise) drive = tfma(s_par[L_WN * T], st.ou, drive);
-          const R xe = drive + s_par[L_CFE * T], xi_ = I + s_par[L_CFI * T];
+          R drive = tfma(s_par[L_G], cpl, E);
+          if (noise) drive = tfma(s_par[L_WN], st.ou, drive);
+          const R xe = drive + s_par[L_CFE], xi_ = I + s_par[L_CFI];
           const R se = xe > R(0) ? P.kappa : R(0), si = xi_ > R(0) ? P.kappa : R(0);   // A22 and the clamp of A10
-          const R c0w = s_par[L_GLEL * T] - st.W;
+          const R c0w = s_par[L_GLEL] - st.W;
           R muV;
           Jet<R> F;
           if (CLOSED) F = tf_closed<R>(P.tf, poly, fmax(xe, R(0)) + P.tf.eps, fmax(xi_, R(0)) + P.tf.eps, c0w, &muV);
@@ -324,21 +327,21 @@ __global__ void __launch_bounds__(MAXT, 1) integrate_kernel(const __grid_constan
             muV = mu_V_only<R>(P.tf, fmax(E, R(0)) + P.tf.eps, fmax(I, R(0)) + P.tf.eps, c0w);
           const R Fe = F.e * se, Fi = F.i * si;
           // ---- S3 Eqs. (1)-(3), forward Euler (A7, A9) ----
-          const R pIT = s_par[L_IT * T];
+          const R pIT = s_par[L_IT];
           const R dF = F.v - st.nu;
           const R Cee_h = R(0.5) * (pop ? Co : Ca) * se * se, Cei_s = Cei * se * si, Cii_h = R(0.5) * (pop ? Cb : Cp) * si * si;
           const R dnu = tfma(Cee_h, F.ee, tfma(Cei_s, F.ei, tfma(Cii_h, F.ii, dF))) * pIT;
-          const R dCs = tfma(F.v * (pIT - F.v), s_par[L_INVN * T], tfma(dF, dF, R(2) * (tfma(Ca, Fe, Cb * Fi) - st.Cs))) * pIT;
+          const R dCs = tfma(F.v * (pIT - F.v), s_par[L_INVN], tfma(dF, dF, R(2) * (tfma(Ca, Fe, Cb * Fi) - st.Cs))) * pIT;
           const R h = tfma(Co, Fe, Cp * Fi);
           const R dF_o = shfl_x1(mask, dF), h_o = shfl_x1(mask, h);
           const R dCei = tfma(dF, dF_o, (h + h_o) - R(2) * Cei) * pIT;
-          const R dW = tfma(s_par[L_AT * T], muV, tfma(s_par[L_B * T], st.nu, -tfma(st.W, s_par[L_ITW * T], s_par[L_ATEL * T])));
+          const R dW = tfma(s_par[L_AT], muV, tfma(s_par[L_B], st.nu, -tfma(st.W, s_par[L_ITW], s_par[L_ATEL])));
           st.nu = tfma(dt, dnu, st.nu);
           st.Cs = tfma(dt, dCs, st.Cs);
           st.Cei = tfma(dt, dCei, st.Cei);
           st.W = tfma(dt, dW, st.W);
           // ---- S4 OU (Eq. 4, A11) ----
-          if (noise) st.ou = tfma(P.ou_rho, st.ou, tfma(P.ou_s, s_xi[(nlo & 7u) * PT], P.ou_m));
+          if (noise) st.ou = tfma(P.ou_rho, st.ou, tfma(P.ou_s, s_xi[nlo & 7u], P.ou_m));
           // ---- S5 ring write: E at time nn+1 (mirror the first GC-1 slots behind the period) ----
           c = c + 1 == Hp ? 0 : c + 1;
           if (pop == 0) {
