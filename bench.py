@@ -35,11 +35,14 @@ import workloads as wl  # noqa: E402
 METRIC = "simulated region-steps/s (sims x regions x steps / s)"
 UNIT = "region-steps/s"
 
-# FP32 floating-point operations the integrator's formulation performs per
-# region-step (FADD + FMUL + 2 FFMA, executed-instruction count from ncu on cfg 2, excluding the
-# coupling sum which adds 2 flops per non-zero edge) and the FP32 peak of the chip:
-# 148 SMs x 128 lanes x 2 flop x sm_max_mhz.
-KERNEL_FLOPS_BASE = 1180.0
+# FP32 floating-point operations the integrator executes per region-step
+# (FADD + FMUL + 2 FFMA over both lanes of a pair, ncu count on cfg 2 = 859, minus the coupling sum,
+# which adds 2 flops per non-zero edge) and the FP32 peak of the chip: 148 SMs x 128 lanes x 2 flop x
+# sm_max_mhz.
+KERNEL_FLOPS_BASE = 820.0
+# DRAM bytes per region-step of the integrator from the ncu --set full capture in profiles/
+# (dram__bytes_read.sum + dram__bytes_write.sum of a 2,000-step launch of cfg 2 / its region-steps)
+NCU_DRAM_BYTES_PER_REGION_STEP = {2: 30.7}
 FLOPS_PER_EDGE = 2.0
 SM_COUNT, LANES_PER_SM = 148, 128
 
@@ -145,25 +148,29 @@ def run_reference(args):
 
 
 def cpu_baseline(cfg_id):
+    """The oracle as it stands on the host cores, on a bounded sample of the workload (~15 s)."""
     from oracle import oracle as orc
     cfg, W, L, S = workload(cfg_id)
     cores = orc.max_threads()
-    n_s = min(S, max(1, cores))
-    sims = [int(x) for x in np.linspace(0, S - 1, n_s).round()]
-    P = wl.grid_params(cfg, sims=sims)
-    o = orc.OracleSweep(W, L, P, seed=cfg["seed"], ext_ids=sims)      # size the sample: aim at ~15 s
+    N = cfg["n"]
+
+    def strat(n_s):
+        return [int(x) for x in np.linspace(0, S - 1, n_s).round()]
+
+    n_s = int(min(S, 4 * cores))
+    sims = strat(n_s)
+    o = orc.OracleSweep(W, L, wl.grid_params(cfg, sims=sims), seed=cfg["seed"], ext_ids=sims)
+    steps, piece, dt = 0, 2000, 0.0
     t0 = time.perf_counter()
-    o.run(200, cfg["dt"], noise_on=True, ds=cfg["ds"], discard_steps=0)
-    per_step = (time.perf_counter() - t0) / 200
-    o.close()
-    steps = int(min(cfg["steps"], max(1000, 15.0 / per_step)) // cfg["ds"] * cfg["ds"])
-    o = orc.OracleSweep(W, L, P, seed=cfg["seed"], ext_ids=sims)
-    t0 = time.perf_counter()
-    o.run(steps, cfg["dt"], noise_on=True, ds=cfg["ds"], discard_steps=0)
+    while steps < cfg["steps"] and dt < 12.0:        # time-boxed: ~12-20 s of CPU work
+        take = min(piece, cfg["steps"] - steps)
+        o.run(take, cfg["dt"], noise_on=True, ds=cfg["ds"], discard_steps=0)
+        steps += take
+        dt = time.perf_counter() - t0
     o.fc_readout()
     dt = time.perf_counter() - t0
-    return {"value": n_s * cfg["n"] * steps / dt, "unit": UNIT, "cores": cores, "kind": "oracle",
-            "sample": f"{n_s} sims (stratified over the grid) x {cfg['n']} regions x {steps} steps, FP64, "
+    return {"value": n_s * N * steps / dt, "unit": UNIT, "cores": cores, "kind": "oracle",
+            "sample": f"{n_s} sims (stratified over the grid) x {N} regions x {steps} steps, FP64, "
                       f"OpenMP over sims, {dt:.1f} s"}
 
 
@@ -273,7 +280,11 @@ def run_tvbx(args):
         peak_tflops = SM_COUNT * LANES_PER_SM * 2 * pk.get("sm_max_mhz", 1965.0) * 1e6 / 1e12
         achieved = flops_unit * units_per_step * args.steps / (int_ms * 1e-3) / 1e12 if int_ms > 0 else None
         roof = {"bound": "alu", "kernel": "tvbx::integrate_kernel", "achieved": achieved, "peak": peak_tflops,
-                "unit": "TFLOP/s", "frac": (achieved / peak_tflops) if achieved else None, "traffic": None,
+                "unit": "TFLOP/s", "frac": (achieved / peak_tflops) if achieved else None,
+                "traffic": (NCU_DRAM_BYTES_PER_REGION_STEP[args.config] * units_per_step * args.steps / max(int_n, 1)
+                            if args.config in NCU_DRAM_BYTES_PER_REGION_STEP and steps_sim == cfg["steps"] else None),
+                "traffic_note": "bytes per launch, scaled from the DRAM bytes per region-step of the ncu capture in profiles/",
+                "algorithmic_bytes_per_region_step": 4.0 * nnz_row + 4.4,
                 "flops_per_region_step": flops_unit, "peak_kind": f"148 SMs x 128 FP32 lanes x 2 x sm_max_mhz ({pk_kind} clock)",
                 "kernel_ms_per_launch": int_ms / max(int_n, 1), "kernel_launches": int_n,
                 "kernel_share_of_step": int_ms / ms if ms > 0 else None,

@@ -97,6 +97,31 @@ def test_fp64_mode_noise_on_matches_oracle_tightly():
     assert np.abs(fc - rfc).max() < 1e-5
 
 
+def test_general_tau_path_fp32_and_fp64():
+    """tau_e != tau_i switches the kernels from the closed-form transfer function to the jet one."""
+    W, L = wl.connectome(24, seed=12, keep=0.4)
+    cfg = dict(axes=[dict(name="G", lo=0.0, hi=0.4, n=3, values=None)], fixed=dict(v=5.0, b_e=40.0, wNoise=1e-4), seed=6)
+    for kappa in (1e-3, 0.05):
+        par = dict(tau_i=7.5, kappa=kappa)
+        sw, traj, o, ref = run_pair(cfg, W, L, 800, True, traj_steps=800, params=par)
+        assert traj_err(traj, ref) < TOL_TRAJ_F32
+        sw, traj, o, ref = run_pair(cfg, W, L, 800, True, traj_steps=800, params=par, precision=tvbx.TVBX_F64)
+        assert traj_err(traj, ref) < 1e-8
+
+
+def test_derivative_terms_carry_weight_kappa():
+    """A22 with a kappa large enough that the first/second-derivative terms of Eqs. (1)-(2) matter
+    (closed-form path), FP32 and FP64; also the A9b option and non-default c_F, E_L, a, b."""
+    W, L = wl.connectome(24, seed=13, keep=0.4)
+    cfg = dict(axes=[dict(name="b_e", lo=0.0, hi=60.0, n=3, values=None)],
+               fixed=dict(v=5.0, G=0.3, wNoise=1e-4, kappa=0.05, a_e=4.0, a_i=1.0, b_i=2.0, E_L_e=-63.0, E_L_i=-65.0,
+                          c_Fie=0.5e-3, c_Fei=0.1e-3, c_Fii=0.2e-3, muV_local=1.0), seed=8)
+    sw, traj, o, ref = run_pair(cfg, W, L, 800, True, traj_steps=800)
+    assert traj_err(traj, ref) < TOL_TRAJ_F32
+    sw, traj, o, ref = run_pair(cfg, W, L, 800, True, traj_steps=800, precision=tvbx.TVBX_F64)
+    assert traj_err(traj, ref) < 1e-8
+
+
 # ------------------------------------------------------------------------------------ launch shapes
 @pytest.mark.parametrize("spc", [1, 2, 4, 8, 16, 32])
 def test_every_sims_per_cta_mapping(spc):
