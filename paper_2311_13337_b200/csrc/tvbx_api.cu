@@ -19,6 +19,7 @@
 
 #include "tvbx_fc.cuh"
 #include "tvbx_integrate.cuh"
+#include "tvbx_integrate2.cuh"
 
 namespace {
 
@@ -78,6 +79,19 @@ int32_t block_steps(int32_t dmin) {
   const int32_t b = std::max(1, dmin);
   return b >= tvbx::GC ? b / tvbx::GC * tvbx::GC : b;
 }
+// Ring geometry of one delay table.  integrate_kernel (general): B steps between CTA barriers, period
+// D + B + 1.  integrate2_kernel (packed FP32): chunks of CH = min(GC, d_min + 1) steps; chunk m reads
+// times <= CH m + CH - 1 - d_min, written by chunks <= m - LAG with LAG = ceil((d_min + 2)/CH) - 1, so a
+// warp may run LAG chunks ahead of the slowest one and the period is D + CH LAG + 1.
+struct RingGeom { int32_t B, CH, LAG, Hp; };
+RingGeom ring_geom(int32_t D, int32_t dmin, bool packed) {
+  RingGeom g;
+  g.B = block_steps(dmin);
+  g.CH = std::min<int32_t>(tvbx::GC, std::max(0, dmin) + 1);
+  g.LAG = std::max(1, std::min<int32_t>(tvbx::LAGMAX, (dmin + 2 + g.CH - 1) / g.CH - 1));
+  g.Hp = packed ? D + g.CH * g.LAG + 1 : D + g.B + 1;
+  return g;
+}
 
 struct HostEdge { int32_t j; double w; double L; };
 
@@ -122,6 +136,7 @@ struct tvbx_sweep {
   std::vector<int64_t> ext_ids;
   uint64_t seed = 0;
   int32_t precision = TVBX_F32, spc = 8, threads_req = 0;
+  bool packed = false;               // FP32 closed-form product kernel (integrate2_kernel)
   int64_t chunk_req = 0;
   double init[7] = {0.001, 0.001, 0, 0, 0, 0, 0};
   // grouping
@@ -234,6 +249,21 @@ KernelPick<float> pick_kernel<float>(bool single, bool closed, int spc) {
   return single ? KernelPick<float>{integrate_kernel<float, true, true, 0, MT>} : KernelPick<float>{integrate_kernel<float, false, true, 0, MT>};
 }
 
+// integrate2_kernel instances: compile-time simulations per CTA 1..7 (N = 68 allows up to 7), else runtime
+typedef void (*Kernel2Fn)(const Integrate2Params);
+inline Kernel2Fn pick_kernel2(int spc) {
+  switch (spc) {
+    case 1: return integrate2_kernel<1>;
+    case 2: return integrate2_kernel<2>;
+    case 3: return integrate2_kernel<3>;
+    case 4: return integrate2_kernel<4>;
+    case 5: return integrate2_kernel<5>;
+    case 6: return integrate2_kernel<6>;
+    case 7: return integrate2_kernel<7>;
+    default: return integrate2_kernel<0>;
+  }
+}
+
 template <typename R>
 struct DeviceImpl : DeviceSide {
   tvbx_sweep* sw;
@@ -246,11 +276,15 @@ struct DeviceImpl : DeviceSide {
   DevBuf<float> d_out_fc, d_out_me, d_out_mi;
   IntegrateParams<R> P;
   KernelPick<R> kp{nullptr};
+  // packed FP32 product kernel (sw->packed)
+  Integrate2Params P2;
+  Kernel2Fn fn2 = nullptr;
+  DevBuf<float2> d_psim2;
   int threads = 0, smem = 0;
   bool single = true;
   size_t ring_count = 0;
 
-  explicit DeviceImpl(tvbx_sweep* s) : sw(s) { std::memset(&P, 0, sizeof P); }
+  explicit DeviceImpl(tvbx_sweep* s) : sw(s) { std::memset(&P, 0, sizeof P); std::memset(&P2, 0, sizeof P2); }
 
   int32_t start(double dt) override {
     const tvbx_connectome& c = sw->conn;
@@ -275,11 +309,13 @@ struct DeviceImpl : DeviceSide {
         ht.delays.push_back(d);
         D = std::max(D, d); dmin = std::min(dmin, d);
       }
-      if (c.edges.empty()) dmin = 0;
-      ht.D = D; ht.dmin = dmin; ht.B = block_steps(dmin); ht.Hp = D + ht.B + 1;
+      if (c.edges.empty()) dmin = GC;
+      const RingGeom rg = ring_geom(D, dmin, sw->packed);
+      ht.D = D; ht.dmin = dmin; ht.B = rg.B; ht.Hp = rg.Hp;
       const int32_t Hs = ht.Hp + GC - 1;
       if ((double)N * Hs * SPC >= 4294967295.0) return fail(TVBX_EINVAL, "ring of one CTA exceeds 32-bit element offsets");
       tds[t].Hp = ht.Hp; tds[t].Hs = Hs; tds[t].B = ht.B; tds[t].n_edges = (int32_t)c.edges.size();
+      tds[t].CH = rg.CH; tds[t].LAG = rg.LAG;
       tds[t].edge_off = (int64_t)edges.size(); tds[t].rowptr_off = (int64_t)rowptr.size();
       for (size_t e = 0; e < c.edges.size(); ++e) {
         Edge<R> ed;
@@ -295,6 +331,7 @@ struct DeviceImpl : DeviceSide {
     std::vector<GroupDesc> gds(G);
     std::vector<int32_t> ext((size_t)G * SPC), loc((size_t)G * SPC);
     std::vector<R> psim((size_t)G * NPS * SPC);
+    std::vector<float2> psim2(sw->packed ? (size_t)G * NP2 * SPC : 0);
     size_t ring_elems = 0;
     for (int g = 0; g < G; ++g) {
       const HostGroup& hg = sw->groups[g];
@@ -312,6 +349,13 @@ struct DeviceImpl : DeviceSide {
                                   sw->param(src, TVBX_P_CFEE), sw->param(src, TVBX_P_CFEI),
                                   sw->param(src, TVBX_P_CFIE), sw->param(src, TVBX_P_CFII)};
         for (int q = 0; q < NPS; ++q) psim[((size_t)g * NPS + q) * SPC + sl] = (R)vals[q];
+        if (sw->packed) {     // the same scalars as (excitatory, inhibitory) pairs
+          const double twi = dp[TVBX_P_TAU_W_I], ati = dp[TVBX_P_A_I] / twi, gL = dp[TVBX_P_GL];
+          const double pr[NP2][2] = {{vals[0], vals[1]}, {vals[7], vals[7]}, {vals[2], dp[TVBX_P_B_I]}, {vals[3], ati},
+                                     {vals[4], 1.0 / twi}, {vals[3] * vals[5], ati * vals[6]}, {gL * vals[5], gL * vals[6]},
+                                     {vals[8], vals[10]}, {vals[9], vals[11]}};
+          for (int q = 0; q < NP2; ++q) psim2[((size_t)g * NP2 + q) * SPC + sl] = make_float2((float)pr[q][0], (float)pr[q][1]);
+        }
       }
     }
     // ---- memory budget ----
@@ -333,6 +377,7 @@ struct DeviceImpl : DeviceSide {
     int64_t* hb = &sw->h2d;
     CU(d_tables.upload(tds, hb)); CU(d_groups.upload(gds, hb)); CU(d_edges.upload(edges, hb)); CU(d_rowptr.upload(rowptr, hb));
     CU(d_ext.upload(ext, hb)); CU(d_loc.upload(loc, hb)); CU(d_psim.upload(psim, hb));
+    if (sw->packed) CU(d_psim2.upload(psim2, hb));
     CU(d_ring.alloc(ring_elems));
     CU(d_xbar.alloc((size_t)G * CS * row));
     CU(d_cmean.alloc((size_t)G * row)); CU(d_mean.alloc((size_t)G * row));
@@ -408,7 +453,42 @@ struct DeviceImpl : DeviceSide {
     CU(cudaFuncGetAttributes(&fa, (const void*)kp.fn));
     sw->info[0] = G; sw->info[1] = threads; sw->info[2] = SPC; sw->info[3] = fa.numRegs; sw->info[4] = smem;
     sw->info[5] = single ? 1 : (N + rt - 1) / rt; sw->info[6] = (int32_t)CS; sw->info[7] = (int32_t)fa.localSizeBytes;
+    if (sw->packed) { int32_t rc = start_packed(tbytes); if (rc) return rc; }
     CU(cudaDeviceSynchronize());
+    return TVBX_OK;
+  }
+
+  // integrate2_kernel: one thread per (sim, region), both populations in packed FP32 pairs
+  int32_t start_packed(size_t tbytes) {
+    const int N = sw->conn.n, SPC = sw->spc;
+    const double* dp = sw->defaults.p;
+    TF2Const& t = P2.tf;
+    const TFConst<R>& f = P.tf;
+    t.gL = (float)f.gL; t.Cm = (float)f.Cm; t.ae = (float)f.ae; t.ai = (float)f.ai; t.aeEe = (float)f.aeEe; t.aiEi = (float)f.aiEi;
+    t.Te = (float)f.Te; t.de = (float)f.de; t.di = (float)f.di; t.ke = (float)f.ke; t.ki = (float)f.ki;
+    t.EegL = (float)f.EegL; t.EigL = (float)f.EigL; t.cq_e = (float)f.cq_e; t.cq_i = (float)f.cq_i;
+    t.cq_ee = (float)f.cq_ee; t.cq_ii = (float)f.cq_ii; t.tau_ae = (float)f.tau_ae; t.tau_ai = (float)f.tau_ai;
+    t.ae2 = (float)f.ae2; t.aeai = (float)f.aeai; t.ai2 = (float)f.ai2; t.muV0 = (float)f.muV0; t.sV0 = (float)f.sV0;
+    t.r0 = (float)f.r0; t.eps = (float)f.eps; t.m2Te = (float)(-2.0 * dp[TVBX_P_TAUE]); t.pad0 = 0.f;
+    for (int i = 0; i < 10; ++i) t.C[i] = make_float2((float)f.C[0][i], (float)f.C[1][i]);
+    t.D4 = make_float2(2.f * t.C[4].x, 2.f * t.C[4].y); t.D5 = make_float2(2.f * t.C[5].x, 2.f * t.C[5].y);
+    t.D6 = make_float2(2.f * t.C[6].x, 2.f * t.C[6].y);
+    P2.kappa = (float)P.kappa; P2.inv_Ne = (float)P.inv_Ne; P2.inv_Ni = (float)P.inv_Ni;
+    P2.ou_rho = (float)P.ou_rho; P2.ou_s = (float)P.ou_s; P2.ou_m = (float)P.ou_m; P2.dt = (float)P.dt;
+    P2.muV_local = P.muV_local; P2.N = N; P2.SPC = SPC; P2.seed = P.seed; P2.chunk_samples = P.chunk_samples;
+    P2.tables = P.tables; P2.groups = P.groups; P2.edges = (const Edge<float>*)P.edges; P2.rowptr = P.rowptr;
+    P2.psim2 = d_psim2.p; P2.ext_id = P.ext_id; P2.loc_id = P.loc_id; P2.ring = (float*)P.ring; P2.state = (float*)P.state;
+    P2.sums = P.sums; P2.xbar = (float*)P.xbar;
+    threads = (N * SPC + 31) / 32 * 32;
+    single = true;
+    fn2 = pick_kernel2(SPC);
+    const size_t base = (size_t)NBAR * 8 + (size_t)(GC + 4) * threads * sizeof(float) + (size_t)NP2 * SPC * sizeof(float2) + 16;
+    P2.smem_table = base + tbytes <= 200 * 1024;
+    smem = (int)(base + (P2.smem_table ? tbytes : 0));
+    CU(cudaFuncSetAttribute((const void*)fn2, cudaFuncAttributeMaxDynamicSharedMemorySize, std::max(smem, 1024)));
+    cudaFuncAttributes fa;
+    CU(cudaFuncGetAttributes(&fa, (const void*)fn2));
+    sw->info[1] = threads; sw->info[3] = fa.numRegs; sw->info[4] = smem; sw->info[5] = 1; sw->info[7] = (int32_t)fa.localSizeBytes;
     return TVBX_OK;
   }
 
@@ -477,7 +557,14 @@ struct DeviceImpl : DeviceSide {
       }
       P.n_begin = sw->n; P.n_end = sw->n + take; P.sample_base = (int32_t)sw->fill;
       sw->prof_begin(K_INTEGRATE, st);
-      kp.fn<<<G, threads, smem, st>>>(P);
+      if (sw->packed) {
+        P2.noise_on = P.noise_on; P2.ds = P.ds; P2.discard_steps = P.discard_steps; P2.traj = (float*)P.traj;
+        P2.traj_steps = P.traj_steps; P2.traj_n0 = P.traj_n0; P2.n_begin = P.n_begin; P2.n_end = P.n_end;
+        P2.sample_base = P.sample_base;
+        fn2<<<G, threads, smem, st>>>(P2);
+      } else {
+        kp.fn<<<G, threads, smem, st>>>(P);
+      }
       sw->prof_end(st);
       sw->launches += 1;
       CU(cudaGetLastError());
@@ -650,8 +737,13 @@ int32_t tvbx_sweep_create(const tvbx_connectome* c, const tvbx_model_params* def
   // simulations the busiest SM has to integrate (148 SMs, CTAs of a sweep all resident or in waves).
   int spc = opts ? opts->sims_per_cta : 0;
   if (const char* e = getenv("TVBX_SPC")) if (spc == 0) spc = atoi(e);
-  const int maxt_sel = sw->precision == TVBX_F64 ? 384 : 1024;
-  const int spc_max = std::max(1, std::min(32, maxt_sel / (2 * sw->conn.n)));
+  // the packed FP32 kernel (one thread per (sim, region), <= 512 threads) serves tau_e == tau_i and
+  // N <= 512; everything else runs the general kernel (two lanes per (sim, region))
+  const bool packed_ok = sw->precision == TVBX_F32 && dp[TVBX_P_TAUE] == dp[TVBX_P_TAUI] && sw->conn.n <= 512 &&
+                         getenv("TVBX_GENERAL_KERNEL") == nullptr;
+  const int lanes_per_node = packed_ok ? 1 : 2;
+  const int maxt_sel = packed_ok ? 512 : (sw->precision == TVBX_F64 ? 384 : 1024);
+  const int spc_max = std::max(1, std::min(32, maxt_sel / (lanes_per_node * sw->conn.n)));
   if (spc == 0) {
     // simulations per distinct speed decide the CTA count; approximate with one table here
     std::map<double, int64_t> per_v;
@@ -660,14 +752,16 @@ int32_t tvbx_sweep_create(const tvbx_connectome* c, const tvbx_model_params* def
     for (int cand = 1; cand <= spc_max; ++cand) {
       int64_t ctas = 0;
       for (auto& kv : per_v) ctas += (kv.second + cand - 1) / cand;
-      const int64_t resident = std::max<int64_t>(1, maxt_sel / (2 * (int64_t)sw->conn.n * cand));
+      const int64_t resident = std::max<int64_t>(1, maxt_sel / (lanes_per_node * (int64_t)sw->conn.n * cand));
       const int64_t slots = 148 * resident;
       const int64_t cost = ctas <= slots ? ((ctas + 147) / 148) * cand : ((ctas + slots - 1) / slots) * resident * cand;
-      if (cost < best_cost || (cost == best_cost && (spc_is_templated(cand) || !spc_is_templated(spc)))) { best_cost = cost; spc = cand; }
+      const bool tc = packed_ok ? cand <= 7 : spc_is_templated(cand), ts = packed_ok ? spc <= 7 : spc_is_templated(spc);
+      if (cost < best_cost || (cost == best_cost && (tc || !ts))) { best_cost = cost; spc = cand; }
     }
   }
   if (spc < 1 || spc > 32) return fail(TVBX_EINVAL, "sims_per_cta=%d (valid: 1..32)", spc);
   sw->spc = spc;
+  sw->packed = packed_ok && sw->conn.n * spc <= 512 && (sw->threads_req == 0 || sw->threads_req >= sw->conn.n * spc);
   // group the simulations by speed (one delay table per distinct v), then into CTAs of spc lanes
   std::map<double, int32_t> vmap;
   sw->sim_table.resize(sw->n_sims);
@@ -798,9 +892,9 @@ int32_t tvbx_ring_len(const tvbx_sweep* sw, int64_t sim, double dt, int32_t* H, 
   const double v = sw->param(sim, TVBX_P_V);
   int32_t D = 0, dmin = INT32_MAX;
   for (const HostEdge& e : sw->conn.edges) { const int32_t d = delay_steps(e.L, v, dt); D = std::max(D, d); dmin = std::min(dmin, d); }
-  if (sw->conn.edges.empty()) dmin = 0;
+  if (sw->conn.edges.empty()) dmin = tvbx::GC;
   if (H) *H = D + 1;
-  if (H_phys) *H_phys = D + block_steps(dmin) + 1;
+  if (H_phys) *H_phys = ring_geom(D, dmin, sw->packed).Hp;
   return TVBX_OK;
 }
 int32_t tvbx_steps_done(const tvbx_sweep* sw, int64_t* n) {

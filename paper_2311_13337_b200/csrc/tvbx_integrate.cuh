@@ -1,4 +1,5 @@
-// tvbx_integrate.cuh -- the integrator kernel: delayed gather + coupling sum (S1), both transfer
+// tvbx_integrate.cuh -- the GENERAL integrator kernel (FP64 build mode, tau_e != tau_i, CTAs that need
+// several region passes); the FP32 product path is tvbx_integrate2.cuh.  Delayed gather + coupling sum (S1), both transfer
 // functions with derivatives (S2), Euler update of the 7 state variables (S3), OU noise from
 // in-kernel Philox4x32-10 (S4), history-ring write (S5), temporal-average downsample (S6) and the
 // per-thread running sums for the mean rates.  DESIGN.md section 6 describes the mapping.
@@ -9,9 +10,9 @@
 //              (E, C_ee, W_e), the ODD lane the inhibitory one (I, C_ii, W_i).  Both run the same
 //              transfer-function code on different constants (no divergence) and exchange E/I, C,
 //              (F - nu) and the C_ei half-sums with five warp shuffles per step.
-//   ring     = ring[group][sim][region][slot]  (E only, "temporal buffer"): TIME is the
-//              fastest index, so the B consecutive steps of a time block read B consecutive floats
-//              per edge.  Rows carry GC-1 mirror slots so that a chunk of GC reads never wraps.
+//   ring     = ring[group][region][slot][sim]  (E only, "temporal buffer"): the SPC simulations
+//              of a group are the fastest index, so the lanes that share a region read one contiguous
+//              run per (edge, step).  Rows carry GC-1 mirror slots so that a chunk of GC reads never wraps.
 //   time     = the kernel is persistent over time: it runs B <= min delay steps between CTA
 //              barriers (step n only reads E at times <= n - d_min), and inside a block it
 //              alternates a GATHER phase (coupling sums of the next <= GC steps, pure loads + FMAs,
@@ -79,10 +80,12 @@ template <> struct __align__(16) Edge<float> { float w; uint32_t jbase; uint32_t
 template <> struct __align__(16) Edge<double> { double w; uint32_t jbase; uint32_t back; };
 
 struct TableDesc {      // one per distinct speed v
-  int32_t Hp;           // ring period D + B + 1
+  int32_t Hp;           // ring period (D + B + 1, or D + CH (LAG + 1) + 1 for the rolling pipeline)
   int32_t Hs;           // row stride Hp + GC - 1 (mirror slots)
-  int32_t B;            // steps between CTA barriers
+  int32_t B;            // steps between CTA barriers (integrate_kernel)
   int32_t n_edges;
+  int32_t CH;           // steps per chunk (integrate2_kernel): min(GC, d_min + 1)
+  int32_t LAG;          // chunks a warp may run ahead of the slowest one (integrate2_kernel)
   int64_t edge_off;     // first edge in the edge array
   int64_t rowptr_off;   // first entry of this table's row pointer (N+1 ints)
 };

@@ -1,0 +1,153 @@
+// tvbx_tf2.cuh -- the closed-form transfer function of tvbx_tf.cuh (tau_e == tau_i) evaluated for BOTH
+// populations at once in packed FP32 pairs: every quantity is a float2 whose .x belongs to the
+// excitatory population and .y to the inhibitory one, and every arithmetic instruction is one of
+// Blackwell's two-wide FP32 operations (FFMA2 / FMUL2 / FADD2, PTX fma/mul/add.rn.f32x2).  The two
+// populations run the same formulas on different constants (Table-1 row, E_L, c_F, W), so one
+// instruction stream serves both and the FP32 work of a region-step takes half the issue slots.
+//
+// Same mathematics as tf_closed (Eq. (5), Table 1 P:68-73,
+// P:84; readings A1, A2, A8): value, first and second partial derivatives with respect to the two
+// input rates (f_e, f_i).
+#pragma once
+#include <cuda_runtime.h>
+
+namespace tvbx {
+
+typedef float2 f2;
+
+__device__ __forceinline__ f2 mk2(float a, float b) { return make_float2(a, b); }
+__device__ __forceinline__ f2 bc2(float a) { return make_float2(a, a); }          // scalar broadcast (free: .F32 operand form)
+__device__ __forceinline__ f2 neg2(f2 a) { return make_float2(-a.x, -a.y); }      // folds into an operand modifier
+__device__ __forceinline__ f2 fma2(f2 a, f2 b, f2 c) { return __ffma2_rn(a, b, c); }
+__device__ __forceinline__ f2 mul2(f2 a, f2 b) { return __fmul2_rn(a, b); }
+__device__ __forceinline__ f2 add2(f2 a, f2 b) { return __fadd2_rn(a, b); }
+__device__ __forceinline__ f2 sub2(f2 a, f2 b) { return __fadd2_rn(a, neg2(b)); }
+__device__ __forceinline__ f2 fms2(f2 a, f2 b, f2 c) { return __ffma2_rn(a, b, neg2(c)); }    // a*b - c
+__device__ __forceinline__ f2 fnma2(f2 a, f2 b, f2 c) { return __ffma2_rn(neg2(a), b, c); }   // c - a*b
+__device__ __forceinline__ f2 scl2(float s, f2 a) { return __fmul2_rn(bc2(s), a); }
+
+__device__ __forceinline__ float sfu_rcp(float x) { float y; asm("rcp.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x)); return y; }
+__device__ __forceinline__ float sfu_sqrt(float x) { float y; asm("sqrt.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x)); return y; }
+__device__ __forceinline__ float sfu_ex2(float x) { float y; asm("ex2.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x)); return y; }
+__device__ __forceinline__ f2 rcp2(f2 a) { return mk2(sfu_rcp(a.x), sfu_rcp(a.y)); }
+__device__ __forceinline__ f2 sqrt2(f2 a) { return mk2(sfu_sqrt(a.x), sfu_sqrt(a.y)); }
+
+// uniform constants of the closed form (scalars are broadcast into both halves by the instruction;
+// the Table-1 rows are true pairs: .x = RS row / excitatory, .y = FS row / inhibitory)
+struct TF2Const {
+  float gL, Cm, ae, ai, aeEe, aiEi, Te, de, di, ke, ki, EegL, EigL, cq_e, cq_i, cq_ee, cq_ii;
+  float tau_ae, tau_ai, ae2, aeai, ai2, muV0, sV0, r0, eps;
+  float m2Te;          // -2 tau
+  float pad0;
+  f2 C[10];            // Table-1 rows rescaled to the centred raw variables (mu_V - muV0, sigma_V - sV0, r - r0)
+  f2 D4, D5, D6;       // 2 C4, 2 C5, 2 C6
+};
+
+struct Jet2 { f2 v, e, i, ee, ei, ii; };
+
+// erfc(z)/2 and exp(-z^2) per half (tvbx_tf.cuh half_erfc<float>: erfc(z) = exp(-z^2) t R(t),
+// t = 1/(1 + 0.4|z|), degree-8 fit from csrc/gen_erfcx_coeffs.py, relative error <= 4.7e-7)
+__device__ __forceinline__ f2 half_erfc2(f2 z, f2* ex) {
+  const f2 zz = mul2(z, z);
+  const f2 e = mk2(sfu_ex2(-1.4426950408889634f * zz.x), sfu_ex2(-1.4426950408889634f * zz.y));
+  const f2 t = mk2(sfu_rcp(__fmaf_rn(0.4f, fabsf(z.x), 1.0f)), sfu_rcp(__fmaf_rn(0.4f, fabsf(z.y), 1.0f)));
+  f2 p = bc2(5.018728834e-02f);
+  p = fma2(p, t, bc2(-1.826153469e-01f));
+  p = fma2(p, t, bc2(1.686438582e-01f));
+  p = fma2(p, t, bc2(-5.255410161e-03f));
+  p = fma2(p, t, bc2(1.412773411e-01f));
+  p = fma2(p, t, bc2(1.685781716e-01f));
+  p = fma2(p, t, bc2(2.078385839e-01f));
+  p = fma2(p, t, bc2(2.256697733e-01f));
+  p = fma2(p, t, bc2(2.256758607e-01f));
+  const f2 h = mul2(mul2(scl2(0.5f, e), t), p);
+  *ex = e;
+  return mk2(z.x >= 0.0f ? h.x : 1.0f - h.x, z.y >= 0.0f ? h.y : 1.0f - h.y);
+}
+
+// F_mu(f_e, f_i, W_mu) for mu = e (.x) and mu = i (.y).  c0 = g_L E_L,mu - W_mu.  *muV_out = mu_V.
+__device__ __forceinline__ Jet2 tf_closed2(const TF2Const& c, f2 fe, f2 fi, f2 c0, f2* muV_out) {
+  const f2 A = fma2(bc2(c.ae), fe, fma2(bc2(c.ai), fi, bc2(c.gL)));
+  const f2 r = rcp2(A);
+  const f2 B = fma2(bc2(c.Te), A, bc2(c.Cm));
+  const f2 iB = rcp2(B);
+  const f2 muV = mul2(fma2(bc2(c.aeEe), fe, fma2(bc2(c.aiEi), fi, c0)), r);
+  const f2 pe = fma2(bc2(c.de), fi, sub2(bc2(c.EegL), c0));
+  const f2 pi = fma2(bc2(c.di), fe, sub2(bc2(c.EigL), c0));
+  const f2 t1 = mul2(scl2(c.ke, pe), pe), t2 = mul2(scl2(c.ki, pi), pi);
+  const f2 Q = fma2(fe, t1, mul2(fi, t2));
+  const f2 Qe = fma2(bc2(c.cq_e), mul2(fi, pi), t1);
+  const f2 Qi = fma2(bc2(c.cq_i), mul2(fe, pe), t2);
+  const f2 Qee = scl2(c.cq_ee, fi), Qii = scl2(c.cq_ii, fe);
+  const f2 Qei = fma2(bc2(c.cq_i), pe, scl2(c.cq_e, pi));
+  const f2 iQ = rcp2(Q);
+  const f2 a1 = scl2(c.ae, r), a2 = scl2(c.ai, r), b1 = scl2(c.tau_ae, iB), b2 = scl2(c.tau_ai, iB);
+  const f2 q1 = mul2(Qe, iQ), q2 = mul2(Qi, iQ);
+  // L = ln sigma_V
+  const f2 Le = scl2(0.5f, sub2(q1, fma2(bc2(3.0f), a1, b1)));
+  const f2 Li = scl2(0.5f, sub2(q2, fma2(bc2(3.0f), a2, b2)));
+  const f2 a1_3 = scl2(3.0f, a1);
+  const f2 Lee = scl2(0.5f, fma2(Qee, iQ, fma2(a1_3, a1, fms2(b1, b1, mul2(q1, q1)))));
+  const f2 Lei = scl2(0.5f, fma2(Qei, iQ, fma2(a1_3, a2, fms2(b1, b2, mul2(q1, q2)))));
+  const f2 Lii = scl2(0.5f, fma2(Qii, iQ, fma2(scl2(3.0f, a2), a2, fms2(b2, b2, mul2(q2, q2)))));
+  const f2 sig = sqrt2(mul2(mul2(scl2(0.5f, mul2(r, r)), mul2(r, Q)), iB));
+  const f2 s_e = mul2(sig, Le), s_i = mul2(sig, Li);
+  const f2 s_ee = mul2(sig, fma2(Le, Le, Lee)), s_ei = mul2(sig, fma2(Le, Li, Lei)), s_ii = mul2(sig, fma2(Li, Li, Lii));
+  // mu_V: mu_e = ae (E_e - mu_V) r, mu_i = ai (E_i - mu_V) r; second derivatives from (mu_V A)_xy = 0
+  const f2 m_e = mul2(a1, mul2(pe, r)), m_i = mul2(a2, mul2(pi, r));
+  const f2 m_ee = mul2(scl2(-2.0f, a1), m_e), m_ei = neg2(fma2(a1, m_i, mul2(a2, m_e))), m_ii = mul2(scl2(-2.0f, a2), m_i);
+  // r = 1/A
+  const f2 r_e = neg2(mul2(a1, r)), r_i = neg2(mul2(a2, r));
+  const f2 r_ee = mul2(scl2(-2.0f, a1), r_e), r_ei = mul2(scl2(-2.0f, a1), r_i), r_ii = mul2(scl2(-2.0f, a2), r_i);
+  // Table-1 polynomial in the centred variables (x, y, w) = (mu_V - muV0, sigma_V - sV0, r - r0)
+  const f2 x = sub2(muV, bc2(c.muV0)), y = sub2(sig, bc2(c.sV0)), w = sub2(r, bc2(c.r0));
+  const f2 C4x = mul2(c.C[4], x), C5y = mul2(c.C[5], y), C6w = mul2(c.C[6], w);
+  const f2 lm = fma2(c.C[7], y, fma2(c.C[8], w, c.C[1])), ls = fma2(c.C[9], w, c.C[2]);
+  const f2 V = fma2(x, add2(lm, C4x), fma2(y, add2(ls, C5y), fma2(w, add2(c.C[3], C6w), c.C[0])));
+  const f2 gm = add2(lm, add2(C4x, C4x));
+  const f2 gs = add2(fma2(c.C[7], x, ls), add2(C5y, C5y));
+  const f2 gt = add2(fma2(c.C[8], x, fma2(c.C[9], y, c.C[3])), add2(C6w, C6w));
+  const f2 hm_e = fma2(c.D4, m_e, fma2(c.C[7], s_e, mul2(c.C[8], r_e))), hs_e = fma2(c.D5, s_e, fma2(c.C[7], m_e, mul2(c.C[9], r_e))),
+           ht_e = fma2(c.D6, r_e, fma2(c.C[8], m_e, mul2(c.C[9], s_e)));
+  const f2 hm_i = fma2(c.D4, m_i, fma2(c.C[7], s_i, mul2(c.C[8], r_i))), hs_i = fma2(c.D5, s_i, fma2(c.C[7], m_i, mul2(c.C[9], r_i))),
+           ht_i = fma2(c.D6, r_i, fma2(c.C[8], m_i, mul2(c.C[9], s_i)));
+  // u = V_thr - mu_V
+  const f2 u = sub2(V, muV);
+  const f2 u_e = sub2(fma2(gm, m_e, fma2(gs, s_e, mul2(gt, r_e))), m_e);
+  const f2 u_i = sub2(fma2(gm, m_i, fma2(gs, s_i, mul2(gt, r_i))), m_i);
+  const f2 u_ee = sub2(fma2(gm, m_ee, fma2(gs, s_ee, fma2(gt, r_ee, fma2(hm_e, m_e, fma2(hs_e, s_e, mul2(ht_e, r_e)))))), m_ee);
+  const f2 u_ei = sub2(fma2(gm, m_ei, fma2(gs, s_ei, fma2(gt, r_ei, fma2(hm_e, m_i, fma2(hs_e, s_i, mul2(ht_e, r_i)))))), m_ei);
+  const f2 u_ii = sub2(fma2(gm, m_ii, fma2(gs, s_ii, fma2(gt, r_ii, fma2(hm_i, m_i, fma2(hs_i, s_i, mul2(ht_i, r_i)))))), m_ii);
+  // z = u / (sqrt2 sigma): with Wz = 1/(sqrt2 sigma), Wz_x = -Wz L_x, Wz_xy = Wz (L_x L_y - L_xy)
+  const f2 Wz = scl2(0.70710678118654752440f, rcp2(sig));
+  const f2 z = mul2(u, Wz);
+  const f2 z_e = mul2(Wz, fnma2(u, Le, u_e)), z_i = mul2(Wz, fnma2(u, Li, u_i));
+  const f2 z_ee = mul2(Wz, fma2(u, fms2(Le, Le, Lee), fma2(scl2(-2.0f, u_e), Le, u_ee)));
+  const f2 z_ei = mul2(Wz, fma2(u, fms2(Le, Li, Lei), fnma2(u_e, Li, fnma2(u_i, Le, u_ei))));
+  const f2 z_ii = mul2(Wz, fma2(u, fms2(Li, Li, Lii), fma2(scl2(-2.0f, u_i), Li, u_ii)));
+  // E = erfc(z)/2:  E' = -exp(-z^2)/sqrt(pi),  E'' = -2 z E'
+  f2 ex;
+  const f2 E0 = half_erfc2(z, &ex);
+  const f2 g0 = scl2(-0.56418958354775628695f, ex);
+  const f2 zz = scl2(-2.0f, z);
+  const f2 E_e = mul2(g0, z_e), E_i = mul2(g0, z_i);
+  const f2 zze = mul2(zz, z_e);
+  const f2 E_ee = mul2(g0, fma2(zze, z_e, z_ee)), E_ei = mul2(g0, fma2(zze, z_i, z_ei)), E_ii = mul2(g0, fma2(mul2(zz, z_i), z_i, z_ii));
+  // 1/(2 tau_V) = A/(2B):  Rv = A/B, dRv/dA = C_m/B^2, d2Rv/dA2 = -2 tau C_m / B^3
+  const f2 Rv = mul2(A, iB);
+  const f2 RA = mul2(scl2(c.Cm, iB), iB);
+  const f2 RAA = mul2(scl2(c.m2Te, RA), iB);
+  const f2 R_e = scl2(c.ae, RA), R_i = scl2(c.ai, RA);
+  Jet2 F;
+  F.v = mul2(E0, Rv);
+  F.e = fma2(E_e, Rv, mul2(E0, R_e));
+  F.i = fma2(E_i, Rv, mul2(E0, R_i));
+  const f2 E0RAA = mul2(E0, RAA);
+  F.ee = fma2(E_ee, Rv, fma2(add2(E_e, E_e), R_e, scl2(c.ae2, E0RAA)));
+  F.ei = fma2(E_ei, Rv, fma2(E_e, R_i, fma2(E_i, R_e, scl2(c.aeai, E0RAA))));
+  F.ii = fma2(E_ii, Rv, fma2(add2(E_i, E_i), R_i, scl2(c.ai2, E0RAA)));
+  *muV_out = muV;
+  return F;
+}
+
+}  // namespace tvbx
