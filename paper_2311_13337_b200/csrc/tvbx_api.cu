@@ -80,14 +80,15 @@ int32_t block_steps(int32_t dmin) {
   return b >= tvbx::GC ? b / tvbx::GC * tvbx::GC : b;
 }
 // Ring geometry of one delay table.  integrate_kernel (general): B steps between CTA barriers, period
-// D + B + 1.  integrate2_kernel (packed FP32): chunks of CH = min(GC, d_min + 1) steps; chunk m reads
-// times <= CH m + CH - 1 - d_min, written by chunks <= m - LAG with LAG = ceil((d_min + 2)/CH) - 1, so a
-// warp may run LAG chunks ahead of the slowest one and the period is D + CH LAG + 1.
+// D + B + 1.  integrate2_kernel (packed FP32): chunks of CH = clamp((d_min + 1)/2, 1, GC) steps; chunk m reads
+// times <= CH m + CH - 1 - d_min, written by chunks <= m - LAG with LAG = ceil((d_min + 2)/CH) - 1 (>= 2 unless
+// d_min = 0; capped at the NST stages of coupling sums), so the gather of chunk m + 1 can precede the compute
+// of chunk m, a warp may run LAG chunks ahead of the slowest one and the period is D + CH LAG + 1.
 struct RingGeom { int32_t B, CH, LAG, Hp; };
 RingGeom ring_geom(int32_t D, int32_t dmin, bool packed) {
   RingGeom g;
   g.B = block_steps(dmin);
-  g.CH = std::min<int32_t>(tvbx::GC, std::max(0, dmin) + 1);
+  g.CH = std::max(1, std::min<int32_t>(tvbx::GC, (std::max(0, dmin) + 1) / 2));
   g.LAG = std::max(1, std::min<int32_t>(tvbx::LAGMAX, (dmin + 2 + g.CH - 1) / g.CH - 1));
   g.Hp = packed ? D + g.CH * g.LAG + 1 : D + g.B + 1;
   return g;
@@ -137,6 +138,7 @@ struct tvbx_sweep {
   uint64_t seed = 0;
   int32_t precision = TVBX_F32, spc = 8, threads_req = 0;
   bool packed = false;               // FP32 closed-form product kernel (integrate2_kernel)
+  int k2_mode = 0;                   // its gather mode (K2_THREAD / K2_WARP / K2_DEDICATED)
   int64_t chunk_req = 0;
   double init[7] = {0.001, 0.001, 0, 0, 0, 0, 0};
   // grouping
@@ -249,19 +251,23 @@ KernelPick<float> pick_kernel<float>(bool single, bool closed, int spc) {
   return single ? KernelPick<float>{integrate_kernel<float, true, true, 0, MT>} : KernelPick<float>{integrate_kernel<float, false, true, 0, MT>};
 }
 
-// integrate2_kernel instances: compile-time simulations per CTA 1..7 (N = 68 allows up to 7), else runtime
+// integrate2_kernel instances: compile-time simulations per CTA 1..8
 typedef void (*Kernel2Fn)(const Integrate2Params);
-inline Kernel2Fn pick_kernel2(int spc) {
+template <int DED>
+inline Kernel2Fn pick_kernel2_spc(int spc) {
   switch (spc) {
-    case 1: return integrate2_kernel<1>;
-    case 2: return integrate2_kernel<2>;
-    case 3: return integrate2_kernel<3>;
-    case 4: return integrate2_kernel<4>;
-    case 5: return integrate2_kernel<5>;
-    case 6: return integrate2_kernel<6>;
-    case 7: return integrate2_kernel<7>;
-    default: return integrate2_kernel<0>;
+    case 1: return integrate2_kernel<1, DED>;
+    case 2: return integrate2_kernel<2, DED>;
+    case 3: return integrate2_kernel<3, DED>;
+    case 4: return integrate2_kernel<4, DED>;
+    case 5: return integrate2_kernel<5, DED>;
+    case 6: return integrate2_kernel<6, DED>;
+    case 7: return integrate2_kernel<7, DED>;
+    default: return integrate2_kernel<8, DED>;
   }
+}
+inline Kernel2Fn pick_kernel2(int spc, int mode) {
+  return mode == K2_DEDICATED ? pick_kernel2_spc<K2_DEDICATED>(spc) : (mode == K2_WARP ? pick_kernel2_spc<K2_WARP>(spc) : (mode == K2_PIPE ? pick_kernel2_spc<K2_PIPE>(spc) : pick_kernel2_spc<K2_THREAD>(spc)));
 }
 
 template <typename R>
@@ -295,6 +301,8 @@ struct DeviceImpl : DeviceSide {
     if (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev == 0) return fail(TVBX_ECUDA, "no CUDA device");
     CU(cudaGetDevice(&sw->device));
 
+    // simulation columns of a ring slot: SPC, or the next power of two for the packed kernel's 8-byte gathers
+    const int RS = sw->packed ? ring_cols(SPC, sw->k2_mode) : SPC;
     // ---- delay tables per distinct speed (A13) and ring geometry ----
     std::vector<TableDesc> tds(sw->tables.size());
     std::vector<Edge<R>> edges;
@@ -313,19 +321,26 @@ struct DeviceImpl : DeviceSide {
       const RingGeom rg = ring_geom(D, dmin, sw->packed);
       ht.D = D; ht.dmin = dmin; ht.B = rg.B; ht.Hp = rg.Hp;
       const int32_t Hs = ht.Hp + GC - 1;
-      if ((double)N * Hs * SPC >= 4294967295.0) return fail(TVBX_EINVAL, "ring of one CTA exceeds 32-bit element offsets");
+      if ((double)N * Hs * RS >= 4294967295.0) return fail(TVBX_EINVAL, "ring of one CTA exceeds 32-bit element offsets");
       tds[t].Hp = ht.Hp; tds[t].Hs = Hs; tds[t].B = ht.B; tds[t].n_edges = (int32_t)c.edges.size();
       tds[t].CH = rg.CH; tds[t].LAG = rg.LAG;
       tds[t].edge_off = (int64_t)edges.size(); tds[t].rowptr_off = (int64_t)rowptr.size();
-      for (size_t e = 0; e < c.edges.size(); ++e) {
-        Edge<R> ed;
-        std::memset(&ed, 0, sizeof ed);
-        ed.w = (R)c.edges[e].w;
-        ed.jbase = (uint32_t)c.edges[e].j * (uint32_t)Hs * (uint32_t)SPC;
-        ed.back = (uint32_t)(ht.Hp - ht.delays[e]);
-        edges.push_back(ed);
+      const int pad_to = 1;      // (rows may be padded with zero-weight copies of their first edge)
+      for (int k = 0; k < N; ++k) {
+        rowptr.push_back((int32_t)(edges.size() - (size_t)tds[t].edge_off));
+        const int r0 = c.rowptr[k], r1 = c.rowptr[k + 1];
+        for (int e = r0; e < r1 || (e - r0) % pad_to != 0; ++e) {
+          const int es = e < r1 ? e : r0;
+          Edge<R> ed;
+          std::memset(&ed, 0, sizeof ed);
+          ed.w = e < r1 ? (R)c.edges[es].w : R(0);
+          ed.jbase = (uint32_t)c.edges[es].j * (uint32_t)Hs * (uint32_t)RS;
+          ed.back = (uint32_t)(ht.Hp - ht.delays[es]);
+          edges.push_back(ed);
+        }
       }
-      rowptr.insert(rowptr.end(), c.rowptr.begin(), c.rowptr.end());
+      rowptr.push_back((int32_t)(edges.size() - (size_t)tds[t].edge_off));
+      tds[t].n_edges = (int32_t)(edges.size() - (size_t)tds[t].edge_off);
     }
     // ---- groups ----
     std::vector<GroupDesc> gds(G);
@@ -336,7 +351,7 @@ struct DeviceImpl : DeviceSide {
     for (int g = 0; g < G; ++g) {
       const HostGroup& hg = sw->groups[g];
       gds[g].table = hg.table; gds[g].pad = 0; gds[g].ring_off = (int64_t)ring_elems;
-      ring_elems += (size_t)N * (sw->tables[hg.table].Hp + GC - 1) * SPC;
+      ring_elems += (size_t)N * (sw->tables[hg.table].Hp + GC - 1) * RS;
       for (int sl = 0; sl < SPC; ++sl) {
         const int64_t s = hg.lanes[sl];
         const int64_t src = s >= 0 ? s : hg.lanes[0];      // padding lanes replay lane 0, never read back
@@ -444,7 +459,7 @@ struct DeviceImpl : DeviceSide {
     else { single = false; const int passes = (N + rt_max - 1) / rt_max; rt = (N + passes - 1) / passes; }
     threads = 2 * SPC * rt;
     kp = pick_kernel<R>(single, tf.same_tau != 0, SPC);
-    const size_t tbytes = c.edges.size() * sizeof(Edge<R>) + (size_t)(N + 1) * 4;
+    const size_t tbytes = (size_t)tds[0].n_edges * sizeof(Edge<R>) + (size_t)(N + 1) * 4;
     const size_t base = ((size_t)(GC + 10) * (threads / 2) + (size_t)L_NPAR * threads + 20) * sizeof(R) + 16;
     P.smem_table = base + tbytes <= 200 * 1024;
     smem = (int)(base + (P.smem_table ? tbytes : 0));
@@ -479,11 +494,22 @@ struct DeviceImpl : DeviceSide {
     P2.tables = P.tables; P2.groups = P.groups; P2.edges = (const Edge<float>*)P.edges; P2.rowptr = P.rowptr;
     P2.psim2 = d_psim2.p; P2.ext_id = P.ext_id; P2.loc_id = P.loc_id; P2.ring = (float*)P.ring; P2.state = (float*)P.state;
     P2.sums = P.sums; P2.xbar = (float*)P.xbar;
-    threads = (N * SPC + 31) / 32 * 32;
+    const int TC = (N * SPC + 31) / 32 * 32;      // consumer threads, then the producer warps (gather + normals)
+    int npw = 0;                                  // dedicated producer warps (K2_DEDICATED)
+    if (sw->k2_mode == K2_DEDICATED) {
+      npw = 4;
+      if (const char* e = getenv("TVBX_NPW")) npw = std::max(1, atoi(e));
+      npw = std::max(1, std::min(npw, (K2_MAXT_DED - TC) / 32));
+    }
+    threads = TC + 32 * npw;
     single = true;
-    fn2 = pick_kernel2(SPC);
-    const size_t base = (size_t)NBAR * 8 + (size_t)(GC + 4) * threads * sizeof(float) + (size_t)NP2 * SPC * sizeof(float2) + 16;
+    const bool priv = sw->k2_mode == K2_THREAD || sw->k2_mode == K2_PIPE;
+    const size_t cpls = priv ? (size_t)TC : (size_t)N * spc_pad(SPC) + 8;
+    const size_t nstg = priv ? 1 : NST;
+    const size_t base = (size_t)(NBAR + NST) * 8 + nstg * GC * (TC + cpls) * sizeof(float) + (size_t)NP2 * SPC * sizeof(float2) + 16;
     P2.smem_table = base + tbytes <= 200 * 1024;
+    if (!P2.smem_table && sw->k2_mode == K2_PIPE) sw->k2_mode = K2_THREAD;   // the pipelined gather reads its row from shared memory
+    fn2 = pick_kernel2(SPC, sw->k2_mode);
     smem = (int)(base + (P2.smem_table ? tbytes : 0));
     CU(cudaFuncSetAttribute((const void*)fn2, cudaFuncAttributeMaxDynamicSharedMemorySize, std::max(smem, 1024)));
     cudaFuncAttributes fa;
@@ -737,13 +763,13 @@ int32_t tvbx_sweep_create(const tvbx_connectome* c, const tvbx_model_params* def
   // simulations the busiest SM has to integrate (148 SMs, CTAs of a sweep all resident or in waves).
   int spc = opts ? opts->sims_per_cta : 0;
   if (const char* e = getenv("TVBX_SPC")) if (spc == 0) spc = atoi(e);
-  // the packed FP32 kernel (one thread per (sim, region), <= 512 threads) serves tau_e == tau_i and
-  // N <= 512; everything else runs the general kernel (two lanes per (sim, region))
-  const bool packed_ok = sw->precision == TVBX_F32 && dp[TVBX_P_TAUE] == dp[TVBX_P_TAUI] && sw->conn.n <= 512 &&
+  // the packed FP32 kernel (one thread per (sim, region), <= 480 of them, plus producer warps) serves
+  // tau_e == tau_i and N <= 480; everything else runs the general kernel (two lanes per (sim, region))
+  const bool packed_ok = sw->precision == TVBX_F32 && dp[TVBX_P_TAUE] == dp[TVBX_P_TAUI] && sw->conn.n <= 480 &&
                          getenv("TVBX_GENERAL_KERNEL") == nullptr;
   const int lanes_per_node = packed_ok ? 1 : 2;
-  const int maxt_sel = packed_ok ? 512 : (sw->precision == TVBX_F64 ? 384 : 1024);
-  const int spc_max = std::max(1, std::min(32, maxt_sel / (lanes_per_node * sw->conn.n)));
+  const int maxt_sel = packed_ok ? 480 : (sw->precision == TVBX_F64 ? 384 : 1024);
+  const int spc_max = std::max(1, std::min(packed_ok ? 8 : 32, maxt_sel / (lanes_per_node * sw->conn.n)));
   if (spc == 0) {
     // simulations per distinct speed decide the CTA count; approximate with one table here
     std::map<double, int64_t> per_v;
@@ -755,13 +781,15 @@ int32_t tvbx_sweep_create(const tvbx_connectome* c, const tvbx_model_params* def
       const int64_t resident = std::max<int64_t>(1, maxt_sel / (lanes_per_node * (int64_t)sw->conn.n * cand));
       const int64_t slots = 148 * resident;
       const int64_t cost = ctas <= slots ? ((ctas + 147) / 148) * cand : ((ctas + slots - 1) / slots) * resident * cand;
-      const bool tc = packed_ok ? cand <= 7 : spc_is_templated(cand), ts = packed_ok ? spc <= 7 : spc_is_templated(spc);
+      const bool tc = packed_ok || spc_is_templated(cand), ts = packed_ok || spc_is_templated(spc);
       if (cost < best_cost || (cost == best_cost && (tc || !ts))) { best_cost = cost; spc = cand; }
     }
   }
   if (spc < 1 || spc > 32) return fail(TVBX_EINVAL, "sims_per_cta=%d (valid: 1..32)", spc);
   sw->spc = spc;
-  sw->packed = packed_ok && sw->conn.n * spc <= 512 && (sw->threads_req == 0 || sw->threads_req >= sw->conn.n * spc);
+  sw->k2_mode = tvbx::K2_PIPE;
+  if (const char* e = getenv("TVBX_K2_MODE")) sw->k2_mode = std::max(0, std::min(3, atoi(e)));
+  sw->packed = packed_ok && spc <= 8 && sw->conn.n * spc <= 480 && (sw->threads_req == 0 || sw->threads_req >= sw->conn.n * spc);
   // group the simulations by speed (one delay table per distinct v), then into CTAs of spc lanes
   std::map<double, int32_t> vmap;
   sw->sim_table.resize(sw->n_sims);

@@ -32,7 +32,9 @@ namespace tvbx {
 
 enum { NP2 = 9 };       // packed per-simulation parameters, see P2_*
 enum { P2_GW = 0, P2_IT, P2_B, P2_AT, P2_ITW, P2_ATEL, P2_GLEL, P2_CFE, P2_CFI };
-enum { NBAR = 8, LAGMAX = NBAR - 1 };
+enum { NBAR = 8, NST = 4, LAGMAX = NST };   // mbarrier ring of the consumers, stages of coupling sums
+enum { K2_MAXT_SELF = 480, K2_MAXT_DED = 608 };   // threads per CTA: every warp produces (128 registers) / + 4 dedicated producer warps (96)
+enum { EB = 16 };       // load rounds a producer warp keeps in flight per region (8-byte loads, 2 registers each)
 
 struct Integrate2Params {
   TF2Const tf;
@@ -88,52 +90,265 @@ __device__ __forceinline__ void mbar_wait(uint64_t* bar, uint32_t parity) {
       : "memory");
 }
 
-// SPC_T: simulations per CTA as a compile-time constant (0 = take P.SPC): the ring loads of a gather
-// chunk then use immediate offsets.
-template <int SPC_T>
-__global__ void __launch_bounds__(512, 1) integrate2_kernel(const __grid_constant__ Integrate2Params P) {
+// Gather of one (simulation, region) node for the chunk whose first step sits in ring slot `cur`:
+// acc[i] = (c_{2i}, c_{2i+1}), c_i = sum over the row's edges of W_kj E_j(n + i - d_kj).
+// EBT edges per iteration: all EBT*GC loads are issued before the first FFMA2 needs one.  Every thread adds its
+// row's edges in ascending order, so the sum does not depend on the other simulations of the CTA.
+template <int RS, int EBT, typename EdgePtr>
+__device__ __forceinline__ void gather_node(EdgePtr edges, int e0, int e1, const float* ringg, int cur, int Hp, int ch,
+                                            f2 acc[GC / 2]) {
+  constexpr int SPC = RS;                         // simulation columns of a ring slot
+  constexpr uint32_t uSPC = (uint32_t)RS;
+#pragma unroll
+  for (int i = 0; i < GC / 2; ++i) acc[i] = mk2(0.0f, 0.0f);
+  if (ch == GC) {
+    int e = e0;
+    for (; e + EBT <= e1; e += EBT) {
+      float w[EBT], v[EBT][GC];
+#pragma unroll
+      for (int b = 0; b < EBT; ++b) {
+        const Edge<float> ed = edges[e + b];
+        int start = cur + (int)ed.back;
+        start = start >= Hp ? start - Hp : start;
+        const float* src = ringg + (ed.jbase + (uint32_t)start * uSPC);
+        w[b] = ed.w;
+#pragma unroll
+        for (int i = 0; i < GC; ++i) v[b][i] = src[i * SPC];
+      }
+#pragma unroll
+      for (int b = 0; b < EBT; ++b)
+#pragma unroll
+        for (int i = 0; i < GC / 2; ++i) acc[i] = fma2(bc2(w[b]), mk2(v[b][2 * i], v[b][2 * i + 1]), acc[i]);
+    }
+    for (; e < e1; ++e) {
+      const Edge<float> ed = edges[e];
+      int start = cur + (int)ed.back;
+      start = start >= Hp ? start - Hp : start;
+      const float* src = ringg + (ed.jbase + (uint32_t)start * uSPC);
+#pragma unroll
+      for (int i = 0; i < GC / 2; ++i) acc[i] = fma2(bc2(ed.w), mk2(src[(2 * i) * SPC], src[(2 * i + 1) * SPC]), acc[i]);
+    }
+  } else {
+    for (int e = e0; e < e1; ++e) {
+      const Edge<float> ed = edges[e];
+      int start = cur + (int)ed.back;
+      start = start >= Hp ? start - Hp : start;
+      const float* src = ringg + (ed.jbase + (uint32_t)start * uSPC);
+#pragma unroll
+      for (int i = 0; i < GC / 2; ++i) {
+        const float v0 = 2 * i < ch ? src[(2 * i) * SPC] : 0.0f;
+        const float v1 = 2 * i + 1 < ch ? src[(2 * i + 1) * SPC] : 0.0f;
+        acc[i] = fma2(bc2(ed.w), mk2(v0, v1), acc[i]);
+      }
+    }
+  }
+}
+
+// Warp-cooperative gather of one region k for a chunk whose first step sits in ring slot `cur`.
+// ring[region][slot][SPCP] keeps the SPCP (power of two >= SPC) simulation columns of a slot together, so the
+// GC slots x SPCP simulations one edge needs are 8*SPCP contiguous floats: LPE = 4*SPCP lanes read them with
+// ONE 8-byte load each (a fully coalesced 32*SPCP-byte run), and a warp covers EPL = 32/LPE edges per load
+// instruction.  Lane l of an edge group holds floats (2l, 2l+1) of the run = (slot, sim pair) for SPCP >= 2,
+// (slot pair) for SPCP = 1, so the weighted sum over the row's edges is one FFMA2 per load (P:82:
+// c_k = sum_j W_kj E_j(t - d_kj)).  EBT loads are in flight per lane.
+// Summation order (the same for every SPCP, so a simulation's result does not depend on how many
+// simulations share its CTA): edge e of the row goes to partial sum (e - e0) mod 8; the 8 partial sums are
+// added as the binary tree ((P0+P1)+(P2+P3))+((P4+P5)+(P6+P7)) -- across the edge groups by xor shuffles
+// (low bits of the class), then inside the lane (high bits).
+template <int SPCP, int EBT, typename EdgePtr>
+__device__ __forceinline__ f2 gather_region(EdgePtr edges, int e0, int e1, const float* ringb, int cur, int Hp, int lane) {
+  constexpr int LPE = 4 * SPCP;                   // lanes per edge
+  constexpr int EPL = 32 / LPE;                   // edges per load instruction
+  constexpr int NA = 8 / EPL;                     // partial sums per lane (= SPCP)
+  static_assert(EBT % NA == 0, "EBT must be a multiple of the partial sums per lane");
+  const int grp = lane / LPE, off = 2 * (lane % LPE);
+  f2 acc[NA];
+#pragma unroll
+  for (int a = 0; a < NA; ++a) acc[a] = mk2(0.0f, 0.0f);
+  for (int e = e0 + grp; e < e1; e += EPL * EBT) {
+    f2 v[EBT];
+    float w[EBT];
+#pragma unroll
+    for (int b = 0; b < EBT; ++b) {
+      const int eb = e + b * EPL;
+      v[b] = mk2(0.0f, 0.0f); w[b] = 0.0f;
+      if (eb < e1) {
+        const Edge<float> ed = edges[eb];
+        int start = cur + (int)ed.back;
+        start = start >= Hp ? start - Hp : start;
+        const float* src = ringb + (ed.jbase + (uint32_t)(start * SPCP + off));
+        if (SPCP >= 2) v[b] = *reinterpret_cast<const f2*>(src);      // 8-byte aligned: every term is even
+        else v[b] = mk2(src[0], src[1]);
+        w[b] = ed.w;
+      }
+    }
+#pragma unroll
+    for (int b = 0; b < EBT; ++b) acc[b % NA] = fma2(bc2(w[b]), v[b], acc[b % NA]);
+  }
+#pragma unroll
+  for (int o = LPE; o < 32; o <<= 1) {
+#pragma unroll
+    for (int a = 0; a < NA; ++a) {
+      acc[a].x += __shfl_xor_sync(0xffffffffu, acc[a].x, o);
+      acc[a].y += __shfl_xor_sync(0xffffffffu, acc[a].y, o);
+    }
+  }
+#pragma unroll
+  for (int st = 1; st < NA; st <<= 1)
+#pragma unroll
+    for (int a = 0; a < NA; a += 2 * st) acc[a] = add2(acc[a], acc[a + st]);
+  return acc[0];
+}
+
+// SPC: simulations per CTA (1..8, compile time); SPCP = the next power of two = simulation columns of a ring slot.
+// blockDim = TC consumer threads (N*SPC rounded up to whole warps) + NPW*32 dedicated producer threads (NPW >= 0).
+__host__ __device__ constexpr int spc_pad(int spc) { return spc <= 1 ? 1 : (spc <= 2 ? 2 : (spc <= 4 ? 4 : 8)); }
+
+// MODE: how the coupling sums are gathered
+//   K2_THREAD     every thread gathers its own node right before it computes the chunk (ring[region][slot][SPC])
+//   K2_WARP       every warp gathers whole regions for the NEXT chunk with coalesced 8-byte loads
+//                 (ring[region][slot][SPCP]), then computes the current one
+//   K2_DEDICATED  the same warp-cooperative gather by dedicated producer warps
+//   K2_PIPE       K2_THREAD software-pipelined: compute step i of chunk m issues the ring loads of edges
+//                 [EPS i, EPS (i+1)) of chunk m + 1 before the transfer function and adds them after it, so the
+//                 L2/HBM latency of the gather hides behind the thread's own arithmetic
+enum { K2_THREAD = 0, K2_WARP = 1, K2_DEDICATED = 2, K2_PIPE = 3 };
+enum { EPS = 3 };        // K2_PIPE: edges of the next chunk gathered per compute step
+__host__ __device__ constexpr int ring_cols(int spc, int mode) { return (mode == K2_THREAD || mode == K2_PIPE) ? spc : spc_pad(spc); }
+
+template <int SPC, int MODE>
+__global__ void __launch_bounds__(MODE == K2_DEDICATED ? K2_MAXT_DED : K2_MAXT_SELF, 1) integrate2_kernel(const __grid_constant__ Integrate2Params P) {
   extern __shared__ __align__(16) unsigned char smem_raw[];
+  constexpr int SPCP = spc_pad(SPC);
+  constexpr int RS = ring_cols(SPC, MODE);        // simulation columns of a ring slot
   const int g = blockIdx.x;
-  const int N = P.N, SPC = SPC_T > 0 ? SPC_T : P.SPC;
-  const int T = blockDim.x, tid = threadIdx.x;
-  const int rl = tid / SPC, sl = tid - rl * SPC;
-  const bool active = rl < N;                     // threads past the last region replay it, stores suppressed
-  const int k = active ? rl : N - 1;
+  const int N = P.N;
+  const int tid = threadIdx.x;
+  const int NODES = N * SPC;
+  const int TC = (NODES + 31) & ~31;              // consumer threads
+  constexpr bool PRIV = MODE == K2_THREAD || MODE == K2_PIPE;   // every thread gathers its own node
+  const int CPLS = PRIV ? TC : N * SPCP + 8;   // row stride of the coupling sums (padded against bank conflicts)
+  const int NPT = MODE == K2_DEDICATED ? (int)blockDim.x - TC : 0;   // dedicated producer threads
+  constexpr int NSTG = PRIV ? 1 : NST;   // stages of coupling sums / normals (private columns need one)
   const GroupDesc gd = P.groups[g];
   const TableDesc td = P.tables[gd.table];
   const int Hp = td.Hp, Hs = td.Hs, CH = td.CH, LAG = td.LAG;
   const Edge<float>* edges = P.edges + td.edge_off;
   const int32_t* rowptr = P.rowptr + td.rowptr_off;
-  // shared memory: NBAR mbarriers | [GC][T] coupling sums | [4][T] normals | [NP2][SPC] packed per-sim
-  // parameters | optional edge table + row pointers
-  uint64_t* bars = reinterpret_cast<uint64_t*>(smem_raw);
-  float* s_cpl = reinterpret_cast<float*>(smem_raw + NBAR * 8) + tid;
-  float* s_xi = reinterpret_cast<float*>(smem_raw + NBAR * 8) + (size_t)GC * T + tid;
-  float2* s_ps = reinterpret_cast<float2*>(reinterpret_cast<float*>(smem_raw + NBAR * 8) + (size_t)(GC + 4) * T);
+  // shared memory: NBAR "done" + NST "full" mbarriers | [NST][GC][CPLS] coupling sums | [NST][GC][TC] normals |
+  // [NP2][SPC] packed per-sim parameters | optional edge table + row pointers
+  uint64_t* bar_done = reinterpret_cast<uint64_t*>(smem_raw);
+  uint64_t* bar_full = bar_done + NBAR;
+  float* const s_cpl0 = reinterpret_cast<float*>(smem_raw + (NBAR + NST) * 8);
+  float* const s_xi0 = s_cpl0 + (size_t)NSTG * GC * CPLS;
+  float2* s_ps = reinterpret_cast<float2*>(s_xi0 + (size_t)NSTG * GC * TC);
+  Edge<float>* s_edges;
+  int32_t* s_rowptr;
+  // producing warps: the dedicated ones if the launch has any, else every warp (gather for chunk m + 1, then
+  // compute chunk m)
+  const int NW_P = NPT > 0 ? NPT >> 5 : TC >> 5;
+  const int ptid = NPT > 0 ? tid - TC : tid;      // index among the producing threads (< 0: pure consumer)
   {
-    if (tid < NBAR) mbar_init(bars + tid, (uint32_t)(T >> 5));
-    for (int i = tid; i < NP2 * SPC; i += T) s_ps[i] = P.psim2[(size_t)g * NP2 * SPC + i];
+    if (tid < NBAR) mbar_init(bar_done + tid, (uint32_t)(TC >> 5));
+    else if (tid < NBAR + NST) mbar_init(bar_full + (tid - NBAR), (uint32_t)NW_P);
+    for (int i = tid; i < NP2 * SPC; i += blockDim.x) s_ps[i] = P.psim2[(size_t)g * NP2 * SPC + i];
+    unsigned char* tab = reinterpret_cast<unsigned char*>(s_ps + NP2 * SPC);
+    tab += (16 - (reinterpret_cast<uintptr_t>(tab) & 15)) & 15;
+    s_edges = reinterpret_cast<Edge<float>*>(tab);
+    s_rowptr = reinterpret_cast<int32_t*>(s_edges + td.n_edges);
     if (P.smem_table) {
-      unsigned char* tab = reinterpret_cast<unsigned char*>(s_ps + NP2 * SPC);
-      tab += (16 - (reinterpret_cast<uintptr_t>(tab) & 15)) & 15;
-      Edge<float>* se = reinterpret_cast<Edge<float>*>(tab);
-      int32_t* sr = reinterpret_cast<int32_t*>(se + td.n_edges);
-      for (int i = tid; i < td.n_edges; i += T) se[i] = edges[i];
-      for (int i = tid; i <= N; i += T) sr[i] = rowptr[i];
-      edges = se; rowptr = sr;
+      for (int i = tid; i < td.n_edges; i += blockDim.x) s_edges[i] = edges[i];
+      for (int i = tid; i <= N; i += blockDim.x) s_rowptr[i] = rowptr[i];
     }
     __syncthreads();
   }
+  const bool noise = P.noise_on != 0;
+
+  // ---- produce chunk m (first step n0, ring slot cur0): S1 coupling sums + S4 normals into stage m mod NST ----
+  auto produce = [&](uint32_t m, int64_t n0, int cur0) {
+    const int ch = (int)min((int64_t)CH, P.n_end - n0);
+    // the ring writes of chunk m - LAG (all warps) must be visible before this chunk's gather; LAG <= NST, so
+    // the stage written below has also been read by everybody
+    if (m >= (uint32_t)LAG) { const uint32_t w = m - (uint32_t)LAG; mbar_wait(bar_done + (w & (NBAR - 1)), (w / NBAR) & 1u); }
+    float* const cpl = s_cpl0 + (size_t)(m & (NSTG - 1)) * GC * CPLS;
+    float* const sxi = s_xi0 + (size_t)(m & (NSTG - 1)) * GC * TC;
+    const int lane = tid & 31;
+    if (PRIV) {                                   // S1 + S4 for this thread's own node, private columns of the stage
+      const int nd = tid < NODES ? tid : NODES - 1;
+      const int rl = nd / SPC, sl = nd - rl * SPC;
+      f2 acc[GC / 2];
+      if (P.smem_table) gather_node<RS, 4>(s_edges, s_rowptr[rl], s_rowptr[rl + 1], P.ring + gd.ring_off + sl, cur0, Hp, ch, acc);
+      else gather_node<RS, 4>(edges, rowptr[rl], rowptr[rl + 1], P.ring + gd.ring_off + sl, cur0, Hp, ch, acc);
+#pragma unroll
+      for (int i = 0; i < GC / 2; ++i) { cpl[(2 * i) * CPLS + tid] = acc[i].x; cpl[(2 * i + 1) * CPLS + tid] = acc[i].y; }
+      if (noise) {
+        const uint32_t ext = (uint32_t)P.ext_id[(size_t)g * SPC + sl];
+        float xi[4] = {0.f, 0.f, 0.f, 0.f};
+        for (int i = 0; i < ch; ++i) {
+          const uint64_t nn = (uint64_t)(n0 + i);
+          if (i == 0 || (nn & 3) == 0) normals4<float>(P.seed, ext, (uint32_t)rl, nn >> 2, xi);
+          const uint32_t q = (uint32_t)nn & 3u;
+          sxi[i * TC + tid] = q == 0 ? xi[0] : (q == 1 ? xi[1] : (q == 2 ? xi[2] : xi[3]));
+        }
+      }
+      return;
+    }
+    for (int k = ptid >> 5; k < N; k += NW_P) {   // S1: one region per warp at a time
+      f2 acc;
+      if (P.smem_table) acc = gather_region<SPCP, EB>(s_edges, s_rowptr[k], s_rowptr[k + 1], P.ring + gd.ring_off, cur0, Hp, lane);
+      else acc = gather_region<SPCP, EB>(edges, rowptr[k], rowptr[k + 1], P.ring + gd.ring_off, cur0, Hp, lane);
+      const int f = 2 * lane;                     // float index in the [GC][SPCP] run of this region
+      if (f < GC * SPCP) {
+        if (SPCP >= 2) *reinterpret_cast<f2*>(cpl + (f / SPCP) * CPLS + k * SPCP + (f % SPCP)) = acc;
+        else { cpl[f * CPLS + k] = acc.x; cpl[(f + 1) * CPLS + k] = acc.y; }
+      }
+    }
+    if (noise) {                                  // S4: Philox (A12): one call per (sim, region) per 4 steps
+      for (int node = ptid; node < NODES; node += NW_P * 32) {
+        const int rl = node / SPC, sl = node - rl * SPC;
+        const uint32_t ext = (uint32_t)P.ext_id[(size_t)g * SPC + sl];
+        float xi[4] = {0.f, 0.f, 0.f, 0.f};
+        for (int i = 0; i < ch; ++i) {
+          const uint64_t nn = (uint64_t)(n0 + i);
+          if (i == 0 || (nn & 3) == 0) normals4<float>(P.seed, ext, (uint32_t)rl, nn >> 2, xi);
+          const uint32_t q = (uint32_t)nn & 3u;
+          sxi[i * TC + node] = q == 0 ? xi[0] : (q == 1 ? xi[1] : (q == 2 ? xi[2] : xi[3]));
+        }
+      }
+    }
+    __syncwarp();
+    if (lane == 0) mbar_arrive(bar_full + (m & (NST - 1)));
+  };
+
+  if (tid >= TC) {
+    // ============================ dedicated PRODUCER warps ============================
+    int64_t n = P.n_begin;
+    int cur = (int)(n % Hp);
+    for (uint32_t m = 0; n < P.n_end; ++m) {
+      produce(m, n, cur);
+      const int ch = (int)min((int64_t)CH, P.n_end - n);
+      n += ch;
+      cur += ch; if (cur >= Hp) cur -= Hp;
+    }
+    return;
+  }
+  // without dedicated producers every warp produces: one chunk ahead of its compute when the delays allow
+  // it (LAG >= 2), else just before it
+  const bool self = MODE != K2_DEDICATED;
+  const int LA = ((MODE == K2_WARP || MODE == K2_PIPE) && LAG >= 2) ? 1 : 0;
+  if (self && LA && P.n_begin < P.n_end) produce(0, P.n_begin, (int)(P.n_begin % Hp));   // chunk 0 has no predecessor to hide behind
+
+  // ============================ CONSUMER warps: S2, S3, S5, S6 ============================
+  const bool active = tid < NODES;                // lanes past the last node replay it, stores suppressed
+  const int node = active ? tid : NODES - 1;
+  const int k = node / SPC, sl = node - k * SPC;
   s_ps += sl;
   float* const ringg = P.ring + gd.ring_off + sl;
-  const uint32_t uSPC = (uint32_t)SPC;
+  const uint32_t uSPC = (uint32_t)RS;
   const uint32_t myrow = (uint32_t)(k * Hs) * uSPC;
-  const int e0 = rowptr[k], e1 = rowptr[k + 1];
-  const int ext = P.ext_id[(size_t)g * SPC + sl];
   const int loc = P.loc_id[(size_t)g * SPC + sl];
   const float dt = P.dt;
   const float inv_ds = P.ds > 0 ? 1.0f / (float)P.ds : 0.0f;
-  const bool noise = P.noise_on != 0;
   const f2 invN = mk2(P.inv_Ne, P.inv_Ni);
 
   // ---- state of this (sim, region) in registers: nu = (E, I), Cs = (C_ee, C_ii), W = (W_e, W_i) ----
@@ -148,66 +363,46 @@ __global__ void __launch_bounds__(512, 1) integrate2_kernel(const __grid_constan
   sumE = sump[0]; sumI = sump[stride];
 
   int64_t n = P.n_begin;
-  int cur = (int)(n % Hp);                        // ring slot of time index n
+  int c = (int)(n % Hp);                          // ring slot of time index n
   int win_left = P.ds > 0 ? P.ds - (int)(n % P.ds) : 0x7fffffff;   // steps left in the current window
   int sidx = P.sample_base;
-  // Philox (A12): one call per (sim, region) per 4 steps gives the quad of normals of steps 4q..4q+3;
-  // re-enter a partly used quad at the start of a launch
-  if (noise && (n & 3)) {
-    float xi[4];
-    normals4<float>(P.seed, (uint32_t)ext, (uint32_t)k, (uint64_t)n >> 2, xi);
-#pragma unroll
-    for (int q = 0; q < 4; ++q) s_xi[q * T] = xi[q];
-  }
+  const int pe0 = MODE == K2_PIPE ? s_rowptr[k] : 0, pe1 = MODE == K2_PIPE ? s_rowptr[k + 1] : 0;   // this node's row (K2_PIPE)
 
   for (uint32_t m = 0; n < P.n_end; ++m) {
     const int ch = (int)min((int64_t)CH, P.n_end - n);
-    // the ring writes of chunk m - LAG (all warps) must be visible before this chunk's gather
-    if (m >= (uint32_t)LAG) { const uint32_t w = m - (uint32_t)LAG; mbar_wait(bars + (w & (NBAR - 1)), (w / NBAR) & 1u); }
-    // ================= GATHER: coupling sums of steps n .. n+ch-1 (S1) =================
-    {
-      f2 acc[GC / 2];
-#pragma unroll
-      for (int i = 0; i < GC / 2; ++i) acc[i] = mk2(0.0f, 0.0f);
-      if (ch == GC) {
-        for (int e = e0; e < e1; ++e) {
-          const Edge<float> ed = edges[e];
-          int start = cur + (int)ed.back;
-          start = start >= Hp ? start - Hp : start;
-          const float* src = ringg + (ed.jbase + (uint32_t)start * uSPC);
-#pragma unroll
-          for (int i = 0; i < GC / 2; ++i) acc[i] = fma2(bc2(ed.w), mk2(src[(2 * i) * SPC], src[(2 * i + 1) * SPC]), acc[i]);
-        }
-      } else {
-        for (int e = e0; e < e1; ++e) {
-          const Edge<float> ed = edges[e];
-          int start = cur + (int)ed.back;
-          start = start >= Hp ? start - Hp : start;
-          const float* src = ringg + (ed.jbase + (uint32_t)start * uSPC);
-#pragma unroll
-          for (int i = 0; i < GC / 2; ++i) {
-            const float v0 = 2 * i < ch ? src[(2 * i) * SPC] : 0.0f;
-            const float v1 = 2 * i + 1 < ch ? src[(2 * i + 1) * SPC] : 0.0f;
-            acc[i] = fma2(bc2(ed.w), mk2(v0, v1), acc[i]);
-          }
-        }
-      }
-#pragma unroll
-      for (int i = 0; i < GC / 2; ++i) { s_cpl[(2 * i) * T] = acc[i].x; s_cpl[(2 * i + 1) * T] = acc[i].y; }
+    const bool has_next = n + ch < P.n_end;
+    const int cur1 = c + ch >= Hp ? c + ch - Hp : c + ch;          // ring slot of the next chunk's first step
+    if (self) {
+      if (!LA) produce(m, n, c);
+      else if (MODE == K2_WARP && has_next) produce(m + 1, n + ch, cur1);
     }
-    // ================= COMPUTE: ch steps in registers (S2-S6) =================
+    const bool pipe = MODE == K2_PIPE && LA && has_next;
+    if (pipe && m + 1 >= (uint32_t)LAG) { const uint32_t w = m + 1 - (uint32_t)LAG; mbar_wait(bar_done + (w & (NBAR - 1)), (w / NBAR) & 1u); }
+    f2 pacc[GC / 2];
+#pragma unroll
+    for (int j = 0; j < GC / 2; ++j) pacc[j] = mk2(0.0f, 0.0f);
+    if (!PRIV) mbar_wait(bar_full + (m & (NST - 1)), (m / NST) & 1u);   // coupling sums and normals of chunk m are in
+    const float* const cplp = s_cpl0 + (size_t)(m & (NSTG - 1)) * GC * CPLS + (PRIV ? tid : k * SPCP + sl);
+    const float* const xip = s_xi0 + (size_t)(m & (NSTG - 1)) * GC * TC + (PRIV ? tid : node);
     const bool traj_on = P.traj != nullptr && loc >= 0 && active && n - P.traj_n0 < P.traj_steps;
-    int c = cur;
     for (int i = 0; i < ch; ++i) {
       const int64_t nn = n + i;
-      const uint32_t nlo = (uint32_t)nn;
-      if (noise && (nlo & 3u) == 0) {             // new quad of normals
-        float xi[4];
-        normals4<float>(P.seed, (uint32_t)ext, (uint32_t)k, (uint64_t)nn >> 2, xi);
+      const float cpl = cplp[i * CPLS];
+      // K2_PIPE: ring loads of edges [EPS i, EPS (i + 1)) of this row for the NEXT chunk, consumed below
+      float pv[EPS][GC];
+      if (MODE == K2_PIPE) {
 #pragma unroll
-        for (int q = 0; q < 4; ++q) s_xi[q * T] = xi[q];
+        for (int b = 0; b < EPS; ++b) {
+          const int e = pe0 + EPS * i + b;
+          const bool on = pipe && e < pe1;
+          const Edge<float> ed = s_edges[on ? e : pe0];
+          int start = cur1 + (int)ed.back;
+          start = start >= Hp ? start - Hp : start;
+          const float* src = ringg + (ed.jbase + (uint32_t)start * uSPC);
+#pragma unroll
+          for (int j = 0; j < GC; ++j) pv[b][j] = on ? src[j * RS] : 0.0f;
+        }
       }
-      const float cpl = s_cpl[i * T];
       // ---- S2 inputs (Eq. 5; A5, A6, A10) ----
       const f2 gw = s_ps[P2_GW * SPC];
       float drive = __fmaf_rn(gw.x, cpl, nu.x);
@@ -247,7 +442,16 @@ __global__ void __launch_bounds__(512, 1) integrate2_kernel(const __grid_constan
       Cei = __fmaf_rn(dt, dCei, Cei);
       W = fma2(bc2(dt), dW, W);
       // ---- S4 OU (Eq. 4, A11) ----
-      if (noise) ou = __fmaf_rn(P.ou_rho, ou, __fmaf_rn(P.ou_s, s_xi[(nlo & 3u) * T], P.ou_m));
+      if (noise) ou = __fmaf_rn(P.ou_rho, ou, __fmaf_rn(P.ou_s, xip[i * TC], P.ou_m));
+      if (MODE == K2_PIPE) {
+#pragma unroll
+        for (int b = 0; b < EPS; ++b) {
+          const int e = pe0 + EPS * i + b;
+          const float w = (pipe && e < pe1) ? s_edges[e].w : 0.0f;
+#pragma unroll
+          for (int j = 0; j < GC / 2; ++j) pacc[j] = fma2(bc2(w), mk2(pv[b][2 * j], pv[b][2 * j + 1]), pacc[j]);
+        }
+      }
       // ---- S5 ring write: E at time nn+1 (mirror the first GC-1 slots behind the period) ----
       c = c + 1 == Hp ? 0 : c + 1;
       if (active) {
@@ -273,11 +477,34 @@ __global__ void __launch_bounds__(512, 1) integrate2_kernel(const __grid_constan
         win = mk2(0.0f, 0.0f);
       }
     }
-    // chunk m is written: publish it
+    if (pipe) {       // the row's remaining edges, then the next chunk's sums and normals replace this chunk's
+      for (int e = pe0 + EPS * ch; e < pe1; ++e) {
+        const Edge<float> ed = s_edges[e];
+        int start = cur1 + (int)ed.back;
+        start = start >= Hp ? start - Hp : start;
+        const float* src = ringg + (ed.jbase + (uint32_t)start * uSPC);
+#pragma unroll
+        for (int j = 0; j < GC / 2; ++j) pacc[j] = fma2(bc2(ed.w), mk2(src[(2 * j) * RS], src[(2 * j + 1) * RS]), pacc[j]);
+      }
+      float* const cw = s_cpl0 + tid;
+#pragma unroll
+      for (int j = 0; j < GC / 2; ++j) { cw[(2 * j) * CPLS] = pacc[j].x; cw[(2 * j + 1) * CPLS] = pacc[j].y; }
+      if (noise) {
+        const uint32_t ext = (uint32_t)P.ext_id[(size_t)g * SPC + sl];
+        const int ch1 = (int)min((int64_t)CH, P.n_end - (n + ch));
+        float xi[4] = {0.f, 0.f, 0.f, 0.f};
+        for (int i = 0; i < ch1; ++i) {
+          const uint64_t nn = (uint64_t)(n + ch + i);
+          if (i == 0 || (nn & 3) == 0) normals4<float>(P.seed, ext, (uint32_t)k, nn >> 2, xi);
+          const uint32_t q = (uint32_t)nn & 3u;
+          s_xi0[i * TC + tid] = q == 0 ? xi[0] : (q == 1 ? xi[1] : (q == 2 ? xi[2] : xi[3]));
+        }
+      }
+    }
+    // chunk m is written (and its stage of coupling sums read): publish it
     __syncwarp();
-    if ((tid & 31) == 0) mbar_arrive(bars + (m & (NBAR - 1)));
+    if ((tid & 31) == 0) mbar_arrive(bar_done + (m & (NBAR - 1)));
     n += ch;
-    cur += ch; if (cur >= Hp) cur -= Hp;
   }
   if (active) {
     sp[0] = nu.x; sp[stride] = nu.y; sp[2 * stride] = Cs.x; sp[3 * stride] = Cei; sp[4 * stride] = Cs.y;
