@@ -82,7 +82,7 @@ int32_t block_steps(int32_t dmin) {
 // Ring geometry of one delay table.  integrate_kernel (general): B steps between CTA barriers, period
 // D + B + 1.  integrate2_kernel (packed FP32): chunks of CH = clamp((d_min + 1)/2, 1, GC) steps; chunk m reads
 // times <= CH m + CH - 1 - d_min, written by chunks <= m - LAG with LAG = ceil((d_min + 2)/CH) - 1 (>= 2 unless
-// d_min = 0; capped at the NST stages of coupling sums), so the gather of chunk m + 1 can precede the compute
+// d_min = 0; capped at LAGMAX), so the gather of chunk m + 1 can precede the compute
 // of chunk m, a warp may run LAG chunks ahead of the slowest one and the period is D + CH LAG + 1.
 struct RingGeom { int32_t B, CH, LAG, Hp; };
 RingGeom ring_geom(int32_t D, int32_t dmin, bool packed) {
@@ -138,7 +138,6 @@ struct tvbx_sweep {
   uint64_t seed = 0;
   int32_t precision = TVBX_F32, spc = 8, threads_req = 0;
   bool packed = false;               // FP32 closed-form product kernel (integrate2_kernel)
-  int k2_mode = 0;                   // its gather mode (K2_THREAD / K2_WARP / K2_DEDICATED)
   int64_t chunk_req = 0;
   double init[7] = {0.001, 0.001, 0, 0, 0, 0, 0};
   // grouping
@@ -251,24 +250,22 @@ KernelPick<float> pick_kernel<float>(bool single, bool closed, int spc) {
   return single ? KernelPick<float>{integrate_kernel<float, true, true, 0, MT>} : KernelPick<float>{integrate_kernel<float, false, true, 0, MT>};
 }
 
-// integrate2_kernel instances: compile-time simulations per CTA 1..8
+// integrate2_kernel instances: compile-time simulations per CTA 1..8, delay table in shared memory or not
 typedef void (*Kernel2Fn)(const Integrate2Params);
-template <int DED>
+template <bool SMEMTAB>
 inline Kernel2Fn pick_kernel2_spc(int spc) {
   switch (spc) {
-    case 1: return integrate2_kernel<1, DED>;
-    case 2: return integrate2_kernel<2, DED>;
-    case 3: return integrate2_kernel<3, DED>;
-    case 4: return integrate2_kernel<4, DED>;
-    case 5: return integrate2_kernel<5, DED>;
-    case 6: return integrate2_kernel<6, DED>;
-    case 7: return integrate2_kernel<7, DED>;
-    default: return integrate2_kernel<8, DED>;
+    case 1: return integrate2_kernel<1, SMEMTAB>;
+    case 2: return integrate2_kernel<2, SMEMTAB>;
+    case 3: return integrate2_kernel<3, SMEMTAB>;
+    case 4: return integrate2_kernel<4, SMEMTAB>;
+    case 5: return integrate2_kernel<5, SMEMTAB>;
+    case 6: return integrate2_kernel<6, SMEMTAB>;
+    case 7: return integrate2_kernel<7, SMEMTAB>;
+    default: return integrate2_kernel<8, SMEMTAB>;
   }
 }
-inline Kernel2Fn pick_kernel2(int spc, int mode) {
-  return mode == K2_DEDICATED ? pick_kernel2_spc<K2_DEDICATED>(spc) : (mode == K2_WARP ? pick_kernel2_spc<K2_WARP>(spc) : (mode == K2_PIPE ? pick_kernel2_spc<K2_PIPE>(spc) : pick_kernel2_spc<K2_THREAD>(spc)));
-}
+inline Kernel2Fn pick_kernel2(int spc, bool smemtab) { return smemtab ? pick_kernel2_spc<true>(spc) : pick_kernel2_spc<false>(spc); }
 
 template <typename R>
 struct DeviceImpl : DeviceSide {
@@ -301,8 +298,7 @@ struct DeviceImpl : DeviceSide {
     if (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev == 0) return fail(TVBX_ECUDA, "no CUDA device");
     CU(cudaGetDevice(&sw->device));
 
-    // simulation columns of a ring slot: SPC, or the next power of two for the packed kernel's 8-byte gathers
-    const int RS = sw->packed ? ring_cols(SPC, sw->k2_mode) : SPC;
+    const int RS = SPC;      // simulation columns of a ring slot
     // ---- delay tables per distinct speed (A13) and ring geometry ----
     std::vector<TableDesc> tds(sw->tables.size());
     std::vector<Edge<R>> edges;
@@ -494,22 +490,11 @@ struct DeviceImpl : DeviceSide {
     P2.tables = P.tables; P2.groups = P.groups; P2.edges = (const Edge<float>*)P.edges; P2.rowptr = P.rowptr;
     P2.psim2 = d_psim2.p; P2.ext_id = P.ext_id; P2.loc_id = P.loc_id; P2.ring = (float*)P.ring; P2.state = (float*)P.state;
     P2.sums = P.sums; P2.xbar = (float*)P.xbar;
-    const int TC = (N * SPC + 31) / 32 * 32;      // consumer threads, then the producer warps (gather + normals)
-    int npw = 0;                                  // dedicated producer warps (K2_DEDICATED)
-    if (sw->k2_mode == K2_DEDICATED) {
-      npw = 4;
-      if (const char* e = getenv("TVBX_NPW")) npw = std::max(1, atoi(e));
-      npw = std::max(1, std::min(npw, (K2_MAXT_DED - TC) / 32));
-    }
-    threads = TC + 32 * npw;
+    threads = (N * SPC + 31) / 32 * 32;
     single = true;
-    const bool priv = sw->k2_mode == K2_THREAD || sw->k2_mode == K2_PIPE;
-    const size_t cpls = priv ? (size_t)TC : (size_t)N * spc_pad(SPC) + 8;
-    const size_t nstg = priv ? 1 : NST;
-    const size_t base = (size_t)(NBAR + NST) * 8 + nstg * GC * (TC + cpls) * sizeof(float) + (size_t)NP2 * SPC * sizeof(float2) + 16;
+    const size_t base = (size_t)NBAR * 8 + (size_t)2 * GC * threads * sizeof(float) + (size_t)NP2 * SPC * sizeof(float2) + 16;
     P2.smem_table = base + tbytes <= 200 * 1024;
-    if (!P2.smem_table && sw->k2_mode == K2_PIPE) sw->k2_mode = K2_THREAD;   // the pipelined gather reads its row from shared memory
-    fn2 = pick_kernel2(SPC, sw->k2_mode);
+    fn2 = pick_kernel2(SPC, P2.smem_table != 0);
     smem = (int)(base + (P2.smem_table ? tbytes : 0));
     CU(cudaFuncSetAttribute((const void*)fn2, cudaFuncAttributeMaxDynamicSharedMemorySize, std::max(smem, 1024)));
     cudaFuncAttributes fa;
@@ -763,7 +748,7 @@ int32_t tvbx_sweep_create(const tvbx_connectome* c, const tvbx_model_params* def
   // simulations the busiest SM has to integrate (148 SMs, CTAs of a sweep all resident or in waves).
   int spc = opts ? opts->sims_per_cta : 0;
   if (const char* e = getenv("TVBX_SPC")) if (spc == 0) spc = atoi(e);
-  // the packed FP32 kernel (one thread per (sim, region), <= 480 of them, plus producer warps) serves
+  // the packed FP32 kernel (one thread per (sim, region), <= 480 of them, <= 8 simulations per CTA) serves
   // tau_e == tau_i and N <= 480; everything else runs the general kernel (two lanes per (sim, region))
   const bool packed_ok = sw->precision == TVBX_F32 && dp[TVBX_P_TAUE] == dp[TVBX_P_TAUI] && sw->conn.n <= 480 &&
                          getenv("TVBX_GENERAL_KERNEL") == nullptr;
@@ -787,8 +772,6 @@ int32_t tvbx_sweep_create(const tvbx_connectome* c, const tvbx_model_params* def
   }
   if (spc < 1 || spc > 32) return fail(TVBX_EINVAL, "sims_per_cta=%d (valid: 1..32)", spc);
   sw->spc = spc;
-  sw->k2_mode = tvbx::K2_PIPE;
-  if (const char* e = getenv("TVBX_K2_MODE")) sw->k2_mode = std::max(0, std::min(3, atoi(e)));
   sw->packed = packed_ok && spc <= 8 && sw->conn.n * spc <= 480 && (sw->threads_req == 0 || sw->threads_req >= sw->conn.n * spc);
   // group the simulations by speed (one delay table per distinct v), then into CTAs of spc lanes
   std::map<double, int32_t> vmap;
