@@ -219,6 +219,8 @@ __global__ void state_init_kernel(R* p, size_t row, size_t total, InitVals<R> iv
     p[i] = iv.v[(i / row) % (NSV - 2)];
 }
 
+inline void set_pad(Edge<float>& e, uint32_t v) { e.pad = v; }
+inline void set_pad(Edge<double>&, uint32_t) {}
 template <typename R> struct KernelPick { void (*fn)(const IntegrateParams<R>); };
 
 // MAXT bounds the registers per thread: 1024 threads -> 64 registers (FP32), 384 -> 168 (FP64).
@@ -332,10 +334,18 @@ struct DeviceImpl : DeviceSide {
           ed.w = e < r1 ? (R)c.edges[es].w : R(0);
           ed.jbase = (uint32_t)c.edges[es].j * (uint32_t)Hs * (uint32_t)RS;
           ed.back = (uint32_t)(ht.Hp - ht.delays[es]);
+          set_pad(ed, ed.jbase + ed.back * (uint32_t)RS);
           edges.push_back(ed);
         }
       }
       rowptr.push_back((int32_t)(edges.size() - (size_t)tds[t].edge_off));
+      if (edges.size() == (size_t)tds[t].edge_off) {      // a table is never empty: one zero-weight entry that no row owns
+        Edge<R> ed;
+        std::memset(&ed, 0, sizeof ed);
+        ed.back = 1;
+        set_pad(ed, (uint32_t)RS);
+        edges.push_back(ed);
+      }
       tds[t].n_edges = (int32_t)(edges.size() - (size_t)tds[t].edge_off);
     }
     // ---- groups ----

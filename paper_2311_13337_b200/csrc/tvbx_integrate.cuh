@@ -76,7 +76,7 @@ template <typename R> __device__ __forceinline__ R shfl_x1(unsigned mask, R v) {
 // one non-zero weight: w = W_kj, jbase = j * Hs * SPC (element offset of the source region's ring row),
 // back = Hp - d_kj
 template <typename R> struct Edge;
-template <> struct __align__(16) Edge<float> { float w; uint32_t jbase; uint32_t back; uint32_t pad; };
+template <> struct __align__(16) Edge<float> { float w; uint32_t jbase; uint32_t back; uint32_t pad; };   // pad = jbase + back * (ring columns)
 template <> struct __align__(16) Edge<double> { double w; uint32_t jbase; uint32_t back; };
 
 struct TableDesc {      // one per distinct speed v

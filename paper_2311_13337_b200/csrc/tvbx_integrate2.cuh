@@ -102,14 +102,16 @@ __device__ __forceinline__ void mbar_wait(uint64_t* bar, uint32_t parity) {
 // clamped to e_last, rows are GC-1 mirror slots longer than the period) whose weight gather_add sets to zero.
 // The caller adds them with gather_add -- later, when it wants the latency hidden.
 template <int RS, int EBT, typename EdgePtr>
-__device__ __forceinline__ void gather_issue(EdgePtr edges, int e, int e_last, const float* ring_cta, uint32_t sl, int cur,
-                                             int Hp, float v[EBT][GC]) {
+__device__ __forceinline__ void gather_issue(EdgePtr edges, int e, int e_last, const float* ringg, int cur, int Hp,
+                                             float v[EBT][GC]) {
+  // slot of the first read = (cur + back) mod Hp with back = Hp - d in [0, Hp]: wraps iff back >= Hp - cur.
+  // The table stores pad = jbase + back * RS, so the element offset is pad + cur * RS - (wrap ? Hp * RS : 0).
+  const uint32_t thr = (uint32_t)(Hp - cur), curRS = (uint32_t)cur * (uint32_t)RS, wrapRS = (uint32_t)Hp * (uint32_t)RS;
 #pragma unroll
   for (int b = 0; b < EBT; ++b) {
     const Edge<float> ed = edges[min(e + b, e_last)];
-    int start = cur + (int)ed.back;
-    start = start >= Hp ? start - Hp : start;
-    const float* src = ring_cta + (uint32_t)(ed.jbase + (uint32_t)start * (uint32_t)RS + sl);
+    const uint32_t off = ed.pad + curRS - (ed.back >= thr ? wrapRS : 0u);
+    const float* src = ringg + off;
 #pragma unroll
     for (int j = 0; j < GC; ++j) v[b][j] = src[j * RS];
   }
@@ -165,9 +167,8 @@ __global__ void __launch_bounds__(K2_MAXT, 1) integrate2_kernel(const __grid_con
   const int node = active ? tid : NODES - 1;
   const int k = node / SPC, sl = node - k * SPC;
   s_ps += sl;
-  float* const ring_cta = P.ring + gd.ring_off;   // this group's ring; the thread's simulation column is + sl
-  float* const ringg = ring_cta + sl;
-  const int e_last = max(td.n_edges - 1, 0);
+  float* const ringg = P.ring + gd.ring_off + sl;   // this group's ring, the thread's simulation column
+  const int e_last = td.n_edges - 1;
   const uint32_t myrow = (uint32_t)(k * Hs) * (uint32_t)RS;
   const int loc = P.loc_id[(size_t)g * SPC + sl];
   const uint32_t ext = (uint32_t)P.ext_id[(size_t)g * SPC + sl];
@@ -199,8 +200,8 @@ __global__ void __launch_bounds__(K2_MAXT, 1) integrate2_kernel(const __grid_con
     for (int j = 0; j < GC / 2; ++j) acc[j] = mk2(0.0f, 0.0f);
     for (int e = pe0; e < pe1; e += 4) {
       float v[4][GC];
-      if (SMEMTAB) { gather_issue<RS, 4>(s_edges, e, e_last, ring_cta, (uint32_t)sl, cur0, Hp, v); gather_add<4>(s_edges, e, pe1, true, v, acc); }
-      else { gather_issue<RS, 4>(g_edges, e, e_last, ring_cta, (uint32_t)sl, cur0, Hp, v); gather_add<4>(g_edges, e, pe1, true, v, acc); }
+      if (SMEMTAB) { gather_issue<RS, 4>(s_edges, e, e_last, ringg, cur0, Hp, v); gather_add<4>(s_edges, e, pe1, true, v, acc); }
+      else { gather_issue<RS, 4>(g_edges, e, e_last, ringg, cur0, Hp, v); gather_add<4>(g_edges, e, pe1, true, v, acc); }
     }
 #pragma unroll
     for (int j = 0; j < GC / 2; ++j) { s_cpl[(2 * j) * T] = acc[j].x; s_cpl[(2 * j + 1) * T] = acc[j].y; }
@@ -233,7 +234,7 @@ __global__ void __launch_bounds__(K2_MAXT, 1) integrate2_kernel(const __grid_con
       if (noise) normals_now(n, ch);
     }
     // the ring writes of chunk m + 1 - LAG (all warps) must be visible before the loads for chunk m + 1
-    const bool pipe = LA && has_next && td.n_edges > 0;
+    const bool pipe = LA && has_next;
     if (pipe && m + 1 >= (uint32_t)LAG) { const uint32_t w = m + 1 - (uint32_t)LAG; mbar_wait(bar_done + (w & (NBAR - 1)), (w / NBAR) & 1u); }
     f2 pacc[GC / 2];                              // coupling sums of chunk m + 1 in the making
 #pragma unroll
@@ -244,15 +245,8 @@ __global__ void __launch_bounds__(K2_MAXT, 1) integrate2_kernel(const __grid_con
       const float cpl = s_cpl[i * T];
       // ---- S1 for the next chunk: issue the loads of edges [EPS i, EPS (i + 1)) now, add them below ----
       float pv[EPS][GC];
-      if (td.n_edges > 0) {                       // (uniform)
-        if (SMEMTAB) gather_issue<RS, EPS>(s_edges, pe0 + EPS * i, e_last, ring_cta, (uint32_t)sl, cur1, Hp, pv);
-        else gather_issue<RS, EPS>(g_edges, pe0 + EPS * i, e_last, ring_cta, (uint32_t)sl, cur1, Hp, pv);
-      } else {
-#pragma unroll
-        for (int b = 0; b < EPS; ++b)
-#pragma unroll
-          for (int j = 0; j < GC; ++j) pv[b][j] = 0.0f;
-      }
+      if (SMEMTAB) gather_issue<RS, EPS>(s_edges, pe0 + EPS * i, e_last, ringg, cur1, Hp, pv);   // (a table has >= 1 entry)
+      else gather_issue<RS, EPS>(g_edges, pe0 + EPS * i, e_last, ringg, cur1, Hp, pv);
       // ---- S2 inputs (Eq. 5; A5, A6, A10) ----
       const f2 gw = s_ps[P2_GW * SPC];
       float drive = __fmaf_rn(gw.x, cpl, nu.x);
@@ -324,8 +318,8 @@ __global__ void __launch_bounds__(K2_MAXT, 1) integrate2_kernel(const __grid_con
     if (pipe) {       // the row's remaining edges (long rows, short chunks), then chunk m + 1 replaces chunk m
       for (int e = pe0 + EPS * ch; e < pe1; e += 4) {
         float v[4][GC];
-        if (SMEMTAB) { gather_issue<RS, 4>(s_edges, e, e_last, ring_cta, (uint32_t)sl, cur1, Hp, v); gather_add<4>(s_edges, e, pe1, true, v, pacc); }
-        else { gather_issue<RS, 4>(g_edges, e, e_last, ring_cta, (uint32_t)sl, cur1, Hp, v); gather_add<4>(g_edges, e, pe1, true, v, pacc); }
+        if (SMEMTAB) { gather_issue<RS, 4>(s_edges, e, e_last, ringg, cur1, Hp, v); gather_add<4>(s_edges, e, pe1, true, v, pacc); }
+        else { gather_issue<RS, 4>(g_edges, e, e_last, ringg, cur1, Hp, v); gather_add<4>(g_edges, e, pe1, true, v, pacc); }
       }
 #pragma unroll
       for (int j = 0; j < GC / 2; ++j) { s_cpl[(2 * j) * T] = pacc[j].x; s_cpl[(2 * j + 1) * T] = pacc[j].y; }
