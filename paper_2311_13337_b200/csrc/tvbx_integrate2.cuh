@@ -39,7 +39,7 @@ enum { NP2 = 9 };       // packed per-simulation parameters, see P2_*
 enum { P2_GW = 0, P2_IT, P2_B, P2_AT, P2_ITW, P2_ATEL, P2_GLEL, P2_CFE, P2_CFI };
 enum { NBAR = 8, LAGMAX = 4 };   // mbarrier ring; chunks a warp may run ahead
 enum { K2_MAXT = 480 };          // threads per CTA: 65536 / 480 -> 128 registers per thread (rounded down from 136)
-enum { EPS = 4 };                // edges of the next chunk gathered per compute step (rows up to EPS * GC = 32 edges
+enum { EPS = 3 };                // edges of the next chunk gathered per compute step (rows up to EPS * GC = 24 edges
                                  // are fully pipelined; longer rows finish in a batched tail loop)
 
 struct Integrate2Params {
