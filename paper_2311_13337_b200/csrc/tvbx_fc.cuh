@@ -143,7 +143,7 @@ __global__ void fc_readout_kernel(ReadoutParams P) {
       else {
         const double den = M[(size_t)k * P.N + k] * M[(size_t)l * P.N + l];
         double v = (den > 0.0 && isfinite(den)) ? M[i] / sqrt(den) : 0.0;
-        r = isfinite(v) ? (float)v : 0.0f;
+        r = isfinite(v) ? (float)fmin(1.0, fmax(-1.0, v)) : 0.0f;   // |rho| <= 1 (Cauchy-Schwarz); FP32 chunk co-moments can round past it
       }
       P.fc[(size_t)loc * NN + i] = r;
     }

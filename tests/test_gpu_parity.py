@@ -304,3 +304,50 @@ def test_cfg2_full_size_sampled_against_oracle():
     assert np.all(np.abs(fc) <= 1.0 + 1e-6)
     np.testing.assert_array_equal(fc, np.swapaxes(fc, 1, 2))
     assert (me > 0).all() and (me < 0.2).all() and (mi > 0).all() and (mi < 0.2).all()
+
+
+def _sampled_parity(cfg_id, steps, discard, sims, **kw):
+    """Full-size sweep of BASELINE.json configs[cfg_id - 1] in the default launch configuration (the one
+    bench.py times), shortened in time; the oracle recomputes the listed simulations one by one."""
+    cfg = wl.config(cfg_id)
+    W, L = wl.config_connectome(cfg)
+    conn, sw = tvbx.sweep_from_config(cfg, W, L, **kw)
+    sw.run(steps, cfg["dt"], noise_on=True, ds=cfg["ds"], discard_steps=discard)
+    fc, me, mi = sw.fc_readout()
+    o = orc.OracleSweep(W, L, wl.grid_params(cfg, sims=sims), seed=cfg["seed"], ext_ids=sims)
+    o.run(steps, cfg["dt"], noise_on=True, ds=cfg["ds"], discard_steps=discard)
+    rfc, rme, rmi = o.fc_readout()
+    assert np.isfinite(fc).all() and np.isfinite(me).all() and np.isfinite(mi).all()
+    assert np.abs(me[sims] / rme - 1).max() < TOL_MEAN_REL
+    assert np.abs(mi[sims] / rmi - 1).max() < TOL_MEAN_REL
+    assert np.abs(fc[sims] - rfc).max() < TOL_FC_ABS
+    # properties that hold for every simulation at any size
+    assert np.all(np.abs(fc) <= 1.0 + 1e-6)
+    np.testing.assert_array_equal(fc, np.swapaxes(fc, 1, 2))
+    assert np.all(np.diagonal(fc, axis1=1, axis2=2) == 1.0)
+    assert (me > 0).all() and (me < 0.2).all() and (mi > 0).all() and (mi < 0.2).all()
+    return sw, o
+
+
+def test_cfg3_full_size_sampled_against_oracle():
+    """cfg 3 at full size (32,768 sims, 8 speeds = 8 delay tables, ring depth 16 ... 2,000 slots, chunk
+    length 1 ... 8 steps); samples cover every speed and the corners of the (b_e, a_e, G) grid."""
+    sims = [0, 1, 2, 3, 4, 5, 6, 7, 8 * 137 + 3, 8 * 2222 + 6, 32767 - 7, 32767]
+    sw, o = _sampled_parity(3, 3000, 1000, sims)
+    assert sw.n_sims == 32768
+    for loc in (0, 3, 7):
+        assert sw.ring_len(loc)[0] == o.ring_len(loc)
+
+
+def test_cfg5_full_size_sampled_against_oracle():
+    """cfg 5 at full size (4,096 sims x 360 regions, ~180 edges per row, delay table read through L1/L2)."""
+    sw, o = _sampled_parity(5, 1500, 500, [0, 63, 64 * 31 + 17, 4095])
+    assert sw.n_sims == 4096 and sw.n_regions == 360
+
+
+def test_cfg4_streaming_fc_drift_against_oracle():
+    """cfg 4 (256 sims, tau_w_e = 500 ms): the FC is accumulated in Welford/Chan form over 1-ms samples,
+    chunk after chunk (here 20 s simulated = 19,000 kept samples = 5 chunk merges); the first and the
+    last simulation of the grid are checked for drift against the oracle's two-pass FC."""
+    sw, o = _sampled_parity(4, 200000, 10000, [0, 255])
+    assert sw.samples_kept() == 19000 and sw.launch_info()["chunk_samples"] < 19000
