@@ -536,9 +536,9 @@ struct DeviceImpl : DeviceSide {
     F.xbar = d_xbar.p; F.cmean = d_cmean.p; F.mean = meanbuf; F.M = Mbuf; F.cnt = cnt; F.n_c = n_c;
     F.CS = (int32_t)sw->CS; F.N = N; F.SPC = SPC; F.G = G;
     const int row = N * SPC;
-    dim3 g1((row + 127) / 128, G);
+    dim3 g1((row + 127) / 128, G), g0((row + 31) / 32, G);
     sw->prof_begin(K_FC, st);
-    fc_chunk_mean_kernel<R><<<g1, 128, 0, st>>>(F);
+    fc_chunk_mean_kernel<R><<<g0, 1024, 0, st>>>(F);
     const int nt = (N + 31) / 32;
     dim3 g2(nt, nt, G * SPC);
     fc_comoment_kernel<R><<<g2, 64, 0, st>>>(F);

@@ -27,17 +27,28 @@ struct FcParams {
   int32_t CS, N, SPC, G;
 };
 
-// chunk mean per (group, region, sim lane): one thread each, coalesced over (region, lane)
+// chunk mean per (group, region, sim lane): a block of 32 columns x 32 sample slices (coalesced 128-byte rows),
+// the slices folded in shared memory in a fixed order (deterministic)
 template <typename R>
-__global__ void fc_chunk_mean_kernel(FcParams<R> P) {
+__global__ void __launch_bounds__(1024) fc_chunk_mean_kernel(FcParams<R> P) {
+  __shared__ double part[32][33];
   const int g = blockIdx.y;
-  const int idx = blockIdx.x * blockDim.x + threadIdx.x;     // region*SPC + lane
+  const int cx = threadIdx.x & 31, sy = threadIdx.x >> 5;
+  const int idx = blockIdx.x * 32 + cx;                      // region*SPC + lane
   const int row = P.N * P.SPC;
-  if (idx >= row) return;
-  const R* x = P.xbar + (size_t)g * P.CS * row + idx;
   double acc = 0.0;
-  for (int q = 0; q < P.n_c; ++q) acc += (double)x[(size_t)q * row];
-  P.cmean[(size_t)g * row + idx] = acc / (double)P.n_c;
+  if (idx < row) {
+    const R* x = P.xbar + (size_t)g * P.CS * row + idx;
+    for (int q = sy; q < P.n_c; q += 32) acc += (double)x[(size_t)q * row];
+  }
+  part[sy][cx] = acc;
+  __syncthreads();
+  if (sy == 0 && idx < row) {
+    double tot = 0.0;
+#pragma unroll
+    for (int j = 0; j < 32; ++j) tot += part[j][cx];
+    P.cmean[(size_t)g * row + idx] = tot / (double)P.n_c;
+  }
 }
 
 // centred co-moment of one (group, sim lane, 32x32 output tile), merged into M.

@@ -316,10 +316,10 @@ __global__ void __launch_bounds__(K2_MAXT, 1) integrate2_kernel(const __grid_con
       }
     }
     if (pipe) {       // the row's remaining edges (long rows, short chunks), then chunk m + 1 replaces chunk m
-      for (int e = pe0 + EPS * ch; e < pe1; e += 4) {
-        float v[4][GC];
-        if (SMEMTAB) { gather_issue<RS, 4>(s_edges, e, e_last, ringg, cur1, Hp, v); gather_add<4>(s_edges, e, pe1, true, v, pacc); }
-        else { gather_issue<RS, 4>(g_edges, e, e_last, ringg, cur1, Hp, v); gather_add<4>(g_edges, e, pe1, true, v, pacc); }
+      for (int e = pe0 + EPS * ch; e < pe1; e += 8) {              // one round of 8 edges: the registers of the transfer function are free here
+        float v[8][GC];
+        if (SMEMTAB) { gather_issue<RS, 8>(s_edges, e, e_last, ringg, cur1, Hp, v); gather_add<8>(s_edges, e, pe1, true, v, pacc); }
+        else { gather_issue<RS, 8>(g_edges, e, e_last, ringg, cur1, Hp, v); gather_add<8>(g_edges, e, pe1, true, v, pacc); }
       }
 #pragma unroll
       for (int j = 0; j < GC / 2; ++j) { s_cpl[(2 * j) * T] = pacc[j].x; s_cpl[(2 * j + 1) * T] = pacc[j].y; }
