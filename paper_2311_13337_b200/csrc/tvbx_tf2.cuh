@@ -101,23 +101,24 @@ __device__ __forceinline__ Jet2 tf_closed2(const TF2Const& c, f2 fe, f2 fi, f2 c
   const f2 r_ee = mul2(scl2(-2.0f, a1), r_e), r_ei = mul2(scl2(-2.0f, a1), r_i), r_ii = mul2(scl2(-2.0f, a2), r_i);
   // Table-1 polynomial in the centred variables (x, y, w) = (mu_V - muV0, sigma_V - sV0, r - r0)
   const f2 x = sub2(muV, bc2(c.muV0)), y = sub2(sig, bc2(c.sV0)), w = sub2(r, bc2(c.r0));
-  const f2 C4x = mul2(c.C[4], x), C5y = mul2(c.C[5], y), C6w = mul2(c.C[6], w);
-  const f2 lm = fma2(c.C[7], y, fma2(c.C[8], w, c.C[1])), ls = fma2(c.C[9], w, c.C[2]);
-  const f2 V = fma2(x, add2(lm, C4x), fma2(y, add2(ls, C5y), fma2(w, add2(c.C[3], C6w), c.C[0])));
-  const f2 gm = add2(lm, add2(C4x, C4x));
-  const f2 gs = add2(fma2(c.C[7], x, ls), add2(C5y, C5y));
-  const f2 gt = add2(fma2(c.C[8], x, fma2(c.C[9], y, c.C[3])), add2(C6w, C6w));
+  // gradient first; the value then follows from Euler's identity for a quadratic form:
+  // V - C0 = lin + quad and x gm + y gs + w gt = lin + 2 quad  =>  V = C0 + (x (gm + C1) + y (gs + C2) + w (gt + C3)) / 2
+  const f2 gm = fma2(c.D4, x, fma2(c.C[7], y, fma2(c.C[8], w, c.C[1])));
+  const f2 gs = fma2(c.D5, y, fma2(c.C[7], x, fma2(c.C[9], w, c.C[2])));
+  const f2 gt = fma2(c.D6, w, fma2(c.C[8], x, fma2(c.C[9], y, c.C[3])));
+  const f2 V = fma2(bc2(0.5f), fma2(x, add2(gm, c.C[1]), fma2(y, add2(gs, c.C[2]), mul2(w, add2(gt, c.C[3])))), c.C[0]);
   const f2 hm_e = fma2(c.D4, m_e, fma2(c.C[7], s_e, mul2(c.C[8], r_e))), hs_e = fma2(c.D5, s_e, fma2(c.C[7], m_e, mul2(c.C[9], r_e))),
            ht_e = fma2(c.D6, r_e, fma2(c.C[8], m_e, mul2(c.C[9], s_e)));
   const f2 hm_i = fma2(c.D4, m_i, fma2(c.C[7], s_i, mul2(c.C[8], r_i))), hs_i = fma2(c.D5, s_i, fma2(c.C[7], m_i, mul2(c.C[9], r_i))),
            ht_i = fma2(c.D6, r_i, fma2(c.C[8], m_i, mul2(c.C[9], s_i)));
   // u = V_thr - mu_V
   const f2 u = sub2(V, muV);
-  const f2 u_e = sub2(fma2(gm, m_e, fma2(gs, s_e, mul2(gt, r_e))), m_e);
-  const f2 u_i = sub2(fma2(gm, m_i, fma2(gs, s_i, mul2(gt, r_i))), m_i);
-  const f2 u_ee = sub2(fma2(gm, m_ee, fma2(gs, s_ee, fma2(gt, r_ee, fma2(hm_e, m_e, fma2(hs_e, s_e, mul2(ht_e, r_e)))))), m_ee);
-  const f2 u_ei = sub2(fma2(gm, m_ei, fma2(gs, s_ei, fma2(gt, r_ei, fma2(hm_e, m_i, fma2(hs_e, s_i, mul2(ht_e, r_i)))))), m_ei);
-  const f2 u_ii = sub2(fma2(gm, m_ii, fma2(gs, s_ii, fma2(gt, r_ii, fma2(hm_i, m_i, fma2(hs_i, s_i, mul2(ht_i, r_i)))))), m_ii);
+  const f2 gm1 = sub2(gm, bc2(1.0f));             // d(V_thr - mu_V)/d mu_V
+  const f2 u_e = fma2(gm1, m_e, fma2(gs, s_e, mul2(gt, r_e)));
+  const f2 u_i = fma2(gm1, m_i, fma2(gs, s_i, mul2(gt, r_i)));
+  const f2 u_ee = fma2(gm1, m_ee, fma2(gs, s_ee, fma2(gt, r_ee, fma2(hm_e, m_e, fma2(hs_e, s_e, mul2(ht_e, r_e))))));
+  const f2 u_ei = fma2(gm1, m_ei, fma2(gs, s_ei, fma2(gt, r_ei, fma2(hm_e, m_i, fma2(hs_e, s_i, mul2(ht_e, r_i))))));
+  const f2 u_ii = fma2(gm1, m_ii, fma2(gs, s_ii, fma2(gt, r_ii, fma2(hm_i, m_i, fma2(hs_i, s_i, mul2(ht_i, r_i))))));
   // z = u / (sqrt2 sigma): with Wz = 1/(sqrt2 sigma), Wz_x = -Wz L_x, Wz_xy = Wz (L_x L_y - L_xy)
   const f2 Wz = scl2(0.70710678118654752440f, rcp2(sig));
   const f2 z = mul2(u, Wz);
