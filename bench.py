@@ -35,14 +35,15 @@ import workloads as wl  # noqa: E402
 METRIC = "simulated region-steps/s (sims x regions x steps / s)"
 UNIT = "region-steps/s"
 
-# FP32 floating-point operations the integrator executes per region-step
-# (FADD + FMUL + 2 FFMA over both lanes of a pair, ncu count on cfg 2 = 859, minus the coupling sum,
-# which adds 2 flops per non-zero edge) and the FP32 peak of the chip: 148 SMs x 128 lanes x 2 flop x
-# sm_max_mhz.
-KERNEL_FLOPS_BASE = 820.0
+# FP32 floating-point operations the integrator needs per region-step = the operation
+# count of its closed-form transfer function + Euler update + noise as executed by integrate2_kernel
+# (ncu source page of the cfg-2 capture in profiles/: per (sim, region) step 115 FFMA2 x 4 + 111 FMUL2 x 2 +
+# 23 FADD2 x 2 + 8 FFMA x 2 + 10 FMUL/FADD + 3 for Box-Muller = 757), plus 2 flops per non-zero edge of the
+# coupling sum; and the FP32 peak of the chip: 148 SMs x 128 lanes x 2 flop x sm_max_mhz.
+KERNEL_FLOPS_BASE = 757.0
 # DRAM bytes per region-step of the integrator from the ncu --set full capture in profiles/
 # (dram__bytes_read.sum + dram__bytes_write.sum of a 2,000-step launch of cfg 2 / its region-steps)
-NCU_DRAM_BYTES_PER_REGION_STEP = {2: 30.7}
+NCU_DRAM_BYTES_PER_REGION_STEP = {2: 25.4}
 FLOPS_PER_EDGE = 2.0
 SM_COUNT, LANES_PER_SM = 148, 128
 
@@ -279,7 +280,7 @@ def run_tvbx(args):
         int_ms, int_n = prof["integrate"]
         peak_tflops = SM_COUNT * LANES_PER_SM * 2 * pk.get("sm_max_mhz", 1965.0) * 1e6 / 1e12
         achieved = flops_unit * units_per_step * args.steps / (int_ms * 1e-3) / 1e12 if int_ms > 0 else None
-        roof = {"bound": "alu", "kernel": "tvbx::integrate_kernel", "achieved": achieved, "peak": peak_tflops,
+        roof = {"bound": "alu", "kernel": sw.kernel_name(), "achieved": achieved, "peak": peak_tflops,
                 "unit": "TFLOP/s", "frac": (achieved / peak_tflops) if achieved else None,
                 "traffic": (NCU_DRAM_BYTES_PER_REGION_STEP[args.config] * units_per_step * args.steps / max(int_n, 1)
                             if args.config in NCU_DRAM_BYTES_PER_REGION_STEP and steps_sim == cfg["steps"] else None),

@@ -84,12 +84,14 @@ enum tvbx_precision { TVBX_F32 = 0, TVBX_F64 = 1 };
 
 typedef struct tvbx_sweep_opts {
   int32_t precision;      /* TVBX_F32 (default) or TVBX_F64 (the 1e-9 parity build mode) */
-  int32_t sims_per_cta;   /* 0 = choose; else 1..32: simulations integrated by one CTA (they share a delay table) */
+  int32_t sims_per_cta;   /* 0 = choose; else 1..32: simulations integrated by one CTA (they share a delay table);
+                             more than 8, or N * sims_per_cta > 480, selects the general kernel */
   int64_t n_sims;         /* 0 = the whole grid; else number of entries of sim_ids */
   const int64_t* sim_ids; /* host: external (grid) indices of the simulations this sweep object holds,
                              e.g. one rank's shard; results are returned in this order */
   int64_t chunk_samples;  /* 0 = choose; downsampled samples buffered between FC reductions */
-  int32_t threads_per_cta;/* 0 = choose (as many region lanes as registers allow, <= 1024) */
+  int32_t threads_per_cta;/* 0 = choose; a value below the lanes one pass over the regions needs selects the general
+                             kernel with several region passes per time block */
   int32_t reserved;
 } tvbx_sweep_opts;
 
@@ -168,8 +170,8 @@ int32_t tvbx_sweep_ext_id(const tvbx_sweep* sw, int64_t sim, int64_t* out);
 /* d_kj = nearbyint((L_kj / v) / dt) in FP64, round-half-to-even (A13); -1 if W_kj == 0.
  * Valid after the first tvbx_run (needs dt), or pass dt > 0 explicitly. */
 int32_t tvbx_delay_index(const tvbx_sweep* sw, int64_t sim, int32_t k, int32_t j, double dt, int32_t* out);
-/* logical ring length H = D + 1 and the physical one the kernel uses (D + B + 1, B = steps between
- * CTA barriers = max(1, min delay)). */
+/* logical ring length H = D + 1 and the physical one the kernel uses: H plus the steps the fastest warp of a
+ * CTA may be ahead of the slowest (at most the minimum delay + 1). */
 int32_t tvbx_ring_len(const tvbx_sweep* sw, int64_t sim, double dt, int32_t* H, int32_t* H_phys);
 int32_t tvbx_steps_done(const tvbx_sweep* sw, int64_t* n);
 int32_t tvbx_samples_kept(const tvbx_sweep* sw, int64_t* n);
@@ -178,6 +180,10 @@ int32_t tvbx_sweep_state(tvbx_sweep* sw, double* y, double* ou);
 /* launch geometry chosen for the integrator (for reports): CTAs, threads per CTA, sims per CTA,
  * registers per thread, dynamic shared memory bytes, region passes per time block */
 int32_t tvbx_launch_info(const tvbx_sweep* sw, int32_t info[8]);
+/* name of the integrator kernel this sweep runs (for reports): "tvbx::integrate2_kernel" = the packed FP32
+ * product kernel (tau_e == tau_i, N * sims_per_cta <= 480, sims_per_cta <= 8), "tvbx::integrate_kernel" = the
+ * general one (FP64 build mode, tau_e != tau_i, larger CTAs).  Copies at most n bytes including the NUL. */
+int32_t tvbx_kernel_name(const tvbx_sweep* sw, char* buf, int32_t n);
 /* number of kernel launches enqueued by this sweep object so far */
 int32_t tvbx_launch_count(const tvbx_sweep* sw, int64_t* n);
 

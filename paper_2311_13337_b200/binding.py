@@ -63,7 +63,7 @@ EXPORTS = [
     "tvbx_default_params", "tvbx_create_connectome", "tvbx_destroy_connectome", "tvbx_sweep_create",
     "tvbx_sweep_destroy", "tvbx_sweep_set_initial", "tvbx_run", "tvbx_fc_readout", "tvbx_sweep_size",
     "tvbx_sweep_param", "tvbx_sweep_ext_id", "tvbx_delay_index", "tvbx_ring_len", "tvbx_steps_done",
-    "tvbx_samples_kept", "tvbx_sweep_state", "tvbx_launch_info", "tvbx_launch_count", "tvbx_last_error",
+    "tvbx_samples_kept", "tvbx_sweep_state", "tvbx_launch_info", "tvbx_launch_count", "tvbx_kernel_name", "tvbx_last_error",
     "tvbx_version", "tvbx_sweep_reset", "tvbx_profile_enable", "tvbx_profile_read", "tvbx_bytes_copied",
 ]
 
@@ -113,6 +113,7 @@ def lib():
             "tvbx_sweep_state": [vp, dp, dp],
             "tvbx_launch_info": [vp, C.POINTER(i32)],
             "tvbx_launch_count": [vp, C.POINTER(i64)],
+            "tvbx_kernel_name": [vp, C.c_char_p, i32],
             "tvbx_sweep_reset": [vp, vp],
             "tvbx_profile_enable": [vp, i32],
             "tvbx_profile_read": [vp, dp, C.POINTER(i64)],
@@ -325,6 +326,11 @@ class Sweep:
         a, b = C.c_int64(), C.c_int64()
         _chk(lib().tvbx_bytes_copied(self._h, C.byref(a), C.byref(b)))
         return a.value, b.value
+
+    def kernel_name(self):
+        buf = C.create_string_buffer(64)
+        _chk(lib().tvbx_kernel_name(self._h, buf, 64))
+        return buf.value.decode()
 
     def launch_count(self):
         out = C.c_int64()

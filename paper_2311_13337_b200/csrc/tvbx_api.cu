@@ -942,6 +942,11 @@ int32_t tvbx_launch_info(const tvbx_sweep* sw, int32_t info[8]) {
   for (int i = 0; i < 8; ++i) info[i] = sw->info[i];
   return TVBX_OK;
 }
+int32_t tvbx_kernel_name(const tvbx_sweep* sw, char* buf, int32_t n) {
+  if (!sw || !buf || n < 1) return fail(TVBX_EINVAL, "bad argument");
+  snprintf(buf, (size_t)n, "%s", sw->packed ? "tvbx::integrate2_kernel" : "tvbx::integrate_kernel");
+  return TVBX_OK;
+}
 int32_t tvbx_launch_count(const tvbx_sweep* sw, int64_t* n) {
   if (!sw || !n) return fail(TVBX_EINVAL, "NULL argument");
   *n = sw->launches;
