@@ -252,22 +252,27 @@ KernelPick<float> pick_kernel<float>(bool single, bool closed, int spc) {
   return single ? KernelPick<float>{integrate_kernel<float, true, true, 0, MT>} : KernelPick<float>{integrate_kernel<float, false, true, 0, MT>};
 }
 
-// integrate2_kernel instances: compile-time simulations per CTA 1..8, delay table in shared memory or not
+// integrate2_kernel instances: compile-time simulations per CTA 1..8; delay table in shared memory with 2, 4 or
+// 8 ring slots loaded per edge, or read through L1/L2 (8 slots)
 typedef void (*Kernel2Fn)(const Integrate2Params);
-template <bool SMEMTAB>
+template <bool SMEMTAB, int GCE>
 inline Kernel2Fn pick_kernel2_spc(int spc) {
   switch (spc) {
-    case 1: return integrate2_kernel<1, SMEMTAB>;
-    case 2: return integrate2_kernel<2, SMEMTAB>;
-    case 3: return integrate2_kernel<3, SMEMTAB>;
-    case 4: return integrate2_kernel<4, SMEMTAB>;
-    case 5: return integrate2_kernel<5, SMEMTAB>;
-    case 6: return integrate2_kernel<6, SMEMTAB>;
-    case 7: return integrate2_kernel<7, SMEMTAB>;
-    default: return integrate2_kernel<8, SMEMTAB>;
+    case 1: return integrate2_kernel<1, SMEMTAB, GCE>;
+    case 2: return integrate2_kernel<2, SMEMTAB, GCE>;
+    case 3: return integrate2_kernel<3, SMEMTAB, GCE>;
+    case 4: return integrate2_kernel<4, SMEMTAB, GCE>;
+    case 5: return integrate2_kernel<5, SMEMTAB, GCE>;
+    case 6: return integrate2_kernel<6, SMEMTAB, GCE>;
+    case 7: return integrate2_kernel<7, SMEMTAB, GCE>;
+    default: return integrate2_kernel<8, SMEMTAB, GCE>;
   }
 }
-inline Kernel2Fn pick_kernel2(int spc, bool smemtab) { return smemtab ? pick_kernel2_spc<true>(spc) : pick_kernel2_spc<false>(spc); }
+inline Kernel2Fn pick_kernel2(int spc, bool smemtab, int gce) {
+  if (!smemtab) return pick_kernel2_spc<false, 8>(spc);
+  return gce == 2 ? pick_kernel2_spc<true, 2>(spc) : (gce == 4 ? pick_kernel2_spc<true, 4>(spc) : pick_kernel2_spc<true, 8>(spc));
+}
+struct Launch2 { int g0, count; Kernel2Fn fn; };   // consecutive groups whose tables share the slots-per-edge class
 
 template <typename R>
 struct DeviceImpl : DeviceSide {
@@ -283,7 +288,7 @@ struct DeviceImpl : DeviceSide {
   KernelPick<R> kp{nullptr};
   // packed FP32 product kernel (sw->packed)
   Integrate2Params P2;
-  Kernel2Fn fn2 = nullptr;
+  std::vector<Launch2> launches2;
   DevBuf<float2> d_psim2;
   int threads = 0, smem = 0;
   bool single = true;
@@ -505,11 +510,23 @@ struct DeviceImpl : DeviceSide {
     single = true;
     const size_t base = (size_t)NBAR * 8 + (size_t)2 * GC * threads * sizeof(float) + (size_t)NP2 * SPC * sizeof(float2) + 16;
     P2.smem_table = base + tbytes <= 200 * 1024;
-    fn2 = pick_kernel2(SPC, P2.smem_table != 0);
     smem = (int)(base + (P2.smem_table ? tbytes : 0));
-    CU(cudaFuncSetAttribute((const void*)fn2, cudaFuncAttributeMaxDynamicSharedMemorySize, std::max(smem, 1024)));
+    // one launch per run of groups whose chunk length falls in the same class (cfg 3: v <= 8 / 16 / >= 32 m/s)
+    launches2.clear();
     cudaFuncAttributes fa;
-    CU(cudaFuncGetAttributes(&fa, (const void*)fn2));
+    std::memset(&fa, 0, sizeof fa);
+    for (int g = 0; g < (int)sw->groups.size(); ++g) {
+      const HostTable& ht = sw->tables[sw->groups[g].table];
+      const int ch = ring_geom(ht.D, ht.dmin, true).CH;
+      const int gce = !P2.smem_table ? 8 : (ch <= 2 ? 2 : (ch <= 4 ? 4 : 8));
+      Kernel2Fn fn = pick_kernel2(SPC, P2.smem_table != 0, gce);
+      if (!launches2.empty() && launches2.back().fn == fn) { launches2.back().count++; continue; }
+      launches2.push_back({g, 1, fn});
+      CU(cudaFuncSetAttribute((const void*)fn, cudaFuncAttributeMaxDynamicSharedMemorySize, std::max(smem, 1024)));
+      cudaFuncAttributes f1;
+      CU(cudaFuncGetAttributes(&f1, (const void*)fn));
+      if (f1.numRegs >= fa.numRegs) fa = f1;
+    }
     sw->info[1] = threads; sw->info[3] = fa.numRegs; sw->info[4] = smem; sw->info[5] = 1; sw->info[7] = (int32_t)fa.localSizeBytes;
     return TVBX_OK;
   }
@@ -583,7 +600,11 @@ struct DeviceImpl : DeviceSide {
         P2.noise_on = P.noise_on; P2.ds = P.ds; P2.discard_steps = P.discard_steps; P2.traj = (float*)P.traj;
         P2.traj_steps = P.traj_steps; P2.traj_n0 = P.traj_n0; P2.n_begin = P.n_begin; P2.n_end = P.n_end;
         P2.sample_base = P.sample_base;
-        fn2<<<G, threads, smem, st>>>(P2);
+        for (const Launch2& l : launches2) {
+          P2.group0 = l.g0;
+          l.fn<<<l.count, threads, smem, st>>>(P2);
+        }
+        sw->launches += (int64_t)launches2.size() - 1;
       } else {
         kp.fn<<<G, threads, smem, st>>>(P);
       }

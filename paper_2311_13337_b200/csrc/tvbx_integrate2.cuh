@@ -20,13 +20,13 @@
 //             (release) on barrier m mod 8 when it has written chunk m and waits (acquire) for phase
 //             m + 1 - LAG before it touches the ring for chunk m + 1, so it may run ahead of the slowest
 //             warp and nobody idles at a block boundary.
-//   gather  = software-pipelined into the compute loop: step i of chunk m issues the ring loads of edges
-//             [EPS i, EPS (i+1)) of the thread's row for chunk m + 1 BEFORE the transfer function and
+//   gather  = software-pipelined into the compute loop: step i of chunk m issues the ring loads of the next
+//             PVN / GCE edges of the thread's row for chunk m + 1 (GCE slots each) BEFORE the transfer function and
 //             adds them (FFMA2 on slot pairs) AFTER it, so the L2/HBM latency of the gather hides behind
 //             the thread's own ~500 instructions of arithmetic; a CTA has only ~4 warps per scheduler
 //             (the sweep's parallelism is sims x regions), too few to hide it by switching warps.
-//             The sums of chunk m + 1 and its Philox normals replace those of chunk m in the thread's
-//             private shared-memory columns when chunk m is done.
+//             The sums of chunk m + 1 replace those of chunk m in the thread's private shared-memory column
+//             when chunk m is done.
 #pragma once
 #include <cuda_runtime.h>
 #include <stdint.h>
@@ -39,8 +39,9 @@ enum { NP2 = 9 };       // packed per-simulation parameters, see P2_*
 enum { P2_GW = 0, P2_IT, P2_B, P2_AT, P2_ITW, P2_ATEL, P2_GLEL, P2_CFE, P2_CFI };
 enum { NBAR = 8, LAGMAX = 4 };   // mbarrier ring; chunks a warp may run ahead
 enum { K2_MAXT = 480 };          // threads per CTA: 65536 / 480 -> 128 registers per thread (rounded down from 136)
-enum { EPS = 3 };                // edges of the next chunk gathered per compute step (rows up to EPS * GC = 24 edges
-                                 // are fully pipelined; longer rows finish in a batched tail loop)
+enum { PVN = 24 };               // ring values of the next chunk a thread keeps in flight across one compute step:
+                                 // PVN / GCE edges x the first GCE = 8, 4 or 2 slots (GCE >= the chunk length).  Rows up to
+                                 // (PVN / GCE) * CH edges are fully pipelined; longer rows finish in rounds of 8 edges
 
 struct Integrate2Params {
   TF2Const tf;
@@ -72,6 +73,7 @@ struct Integrate2Params {
   int64_t traj_steps;
   int64_t traj_n0;
   int32_t smem_table;             // edge table + row pointers staged in shared memory (else read through L1/L2)
+  int32_t group0;                 // first group of this launch (groups of one launch share GCE)
 };
 
 __device__ __forceinline__ uint32_t smem_u32(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
@@ -96,14 +98,14 @@ __device__ __forceinline__ void mbar_wait(uint64_t* bar, uint32_t parity) {
       : "memory");
 }
 
-// One batch of EBT edges [e, e + EBT) of a row for the chunk whose first step sits in ring slot `cur`: issue
-// all EBT * GC ring loads and return the values in v[][].  The loads are unconditional: a batch may run past the
-// row (or past the CH slots a short chunk uses) -- it then reads other valid ring entries (the table index is
-// clamped to e_last, rows are GC-1 mirror slots longer than the period) whose weight gather_add sets to zero.
-// The caller adds them with gather_add -- later, when it wants the latency hidden.
-template <int RS, int EBT, typename EdgePtr>
-__device__ __forceinline__ void gather_issue(EdgePtr edges, int e, int e_last, const float* ringg, int cur, int Hp,
-                                             float v[EBT][GC]) {
+// One batch of EBT edges [e, e + EBT) of a row for the chunk whose first step sits in ring slot `cur`: issue the
+// ring loads of the first GCE slots of every edge (GCE = 2, 4 or 8 >= the chunk length) and return the values in
+// v[EBT * GCE].  The loads are unconditional: a batch may run past the row (or past the CH slots a short chunk
+// uses) -- it then reads other valid ring entries (the table index is clamped to e_last, rows are GC-1 mirror
+// slots longer than the period) whose weight gather_add sets to zero.  The caller adds them with gather_add --
+// later, when it wants the latency hidden.
+template <int RS, int EBT, int GCE, typename EdgePtr>
+__device__ __forceinline__ void gather_issue(EdgePtr edges, int e, int e_last, const float* ringg, int cur, int Hp, float* v) {
   // slot of the first read = (cur + back) mod Hp with back = Hp - d in [0, Hp]: wraps iff back >= Hp - cur.
   // The table stores pad = jbase + back * RS, so the element offset is pad + cur * RS - (wrap ? Hp * RS : 0).
   const uint32_t thr = (uint32_t)(Hp - cur), curRS = (uint32_t)cur * (uint32_t)RS, wrapRS = (uint32_t)Hp * (uint32_t)RS;
@@ -113,28 +115,39 @@ __device__ __forceinline__ void gather_issue(EdgePtr edges, int e, int e_last, c
     const uint32_t off = ed.pad + curRS - (ed.back >= thr ? wrapRS : 0u);
     const float* src = ringg + off;
 #pragma unroll
-    for (int j = 0; j < GC; ++j) v[b][j] = src[j * RS];
+    for (int j = 0; j < GCE; ++j) v[b * GCE + j] = src[j * RS];
   }
 }
-// acc[j] += w * (E(slot 2j), E(slot 2j+1)): the row's edges are added in ascending order into each slot, so a
-// simulation's coupling sum does not depend on which other simulations share its CTA
-template <int EBT, typename EdgePtr>
-__device__ __forceinline__ void gather_add(EdgePtr edges, int e, int e1, bool enable, const float v[EBT][GC], f2 acc[GC / 2]) {
+// acc[j] += w * (E(slot 2j), E(slot 2j+1)), j < GCE/2: the row's edges are added in ascending order into each
+// slot, so a simulation's coupling sum does not depend on which other simulations share its CTA
+template <int EBT, int GCE, typename EdgePtr>
+__device__ __forceinline__ void gather_add(EdgePtr edges, int e, int e1, bool enable, const float* v, f2 acc[GC / 2]) {
 #pragma unroll
   for (int b = 0; b < EBT; ++b) {
     const float w = (enable && e + b < e1) ? edges[e + b].w : 0.0f;
 #pragma unroll
-    for (int j = 0; j < GC / 2; ++j) acc[j] = fma2(bc2(w), mk2(v[b][2 * j], v[b][2 * j + 1]), acc[j]);
+    for (int j = 0; j < GCE / 2; ++j) acc[j] = fma2(bc2(w), mk2(v[b * GCE + 2 * j], v[b * GCE + 2 * j + 1]), acc[j]);
+  }
+}
+// the edges [e, e1) of a row in unpipelined rounds of 8 edges
+template <int RS, int GCE, typename EdgePtr>
+__device__ __forceinline__ void gather_rounds(EdgePtr edges, int e, int e1, int e_last, const float* ringg, int cur, int Hp,
+                                              f2 acc[GC / 2]) {
+  for (; e < e1; e += 8) {
+    float v[8 * GCE];
+    gather_issue<RS, 8, GCE>(edges, e, e_last, ringg, cur, Hp, v);
+    gather_add<8, GCE>(edges, e, e1, true, v, acc);
   }
 }
 
-// SPC: simulations per CTA (1..8); SMEMTAB: the delay table of the group's speed is staged in shared memory.
+// SPC: simulations per CTA (1..8); SMEMTAB: the delay table of the group's speed is staged in shared memory;
+// GCE: ring slots loaded per edge = 2, 4 or 8 >= the chunk length CH of the launched groups (P.group0 ...).
 // blockDim = N*SPC rounded up to whole warps (<= K2_MAXT); lanes past the last node replay it, stores suppressed.
-template <int SPC, bool SMEMTAB>
+template <int SPC, bool SMEMTAB, int GCE>
 __global__ void __launch_bounds__(K2_MAXT, 1) integrate2_kernel(const __grid_constant__ Integrate2Params P) {
   extern __shared__ __align__(16) unsigned char smem_raw[];
   constexpr int RS = SPC;                         // simulation columns of a ring slot
-  const int g = blockIdx.x;
+  const int g = blockIdx.x + P.group0;
   const int N = P.N;
   const int tid = threadIdx.x, T = blockDim.x;
   const int NODES = N * SPC;
@@ -145,7 +158,8 @@ __global__ void __launch_bounds__(K2_MAXT, 1) integrate2_kernel(const __grid_con
   // [NP2][SPC] packed per-sim parameters | edge table + row pointers (SMEMTAB)
   uint64_t* bar_done = reinterpret_cast<uint64_t*>(smem_raw);
   float* const s_cpl = reinterpret_cast<float*>(smem_raw + NBAR * 8) + tid;
-  float* const s_xi = s_cpl + (size_t)GC * T;
+  float* const s_xi = s_cpl + (size_t)GC * T;     // GCE == 8: the normals of the chunk's steps; GCE < 8: rows 0..3 = the current Philox quad
+  float* const s_quad = s_xi;
   float2* s_ps = reinterpret_cast<float2*>(reinterpret_cast<float*>(smem_raw + NBAR * 8) + (size_t)2 * GC * T);
   unsigned char* tab = reinterpret_cast<unsigned char*>(s_ps + NP2 * SPC);
   tab += (16 - (reinterpret_cast<uintptr_t>(tab) & 15)) & 15;
@@ -194,20 +208,21 @@ __global__ void __launch_bounds__(K2_MAXT, 1) integrate2_kernel(const __grid_con
   int sidx = P.sample_base;
 
   // S1, not pipelined: coupling sums of the chunk that starts at ring slot cur0 into this thread's column
+  auto gather_from = [&](int e, int cur0, f2 acc[GC / 2]) {
+    if (SMEMTAB) gather_rounds<RS, GCE>(s_edges, e, pe1, e_last, ringg, cur0, Hp, acc);
+    else gather_rounds<RS, GCE>(g_edges, e, pe1, e_last, ringg, cur0, Hp, acc);
+  };
   auto gather_now = [&](int cur0) {
     f2 acc[GC / 2];
 #pragma unroll
     for (int j = 0; j < GC / 2; ++j) acc[j] = mk2(0.0f, 0.0f);
-    for (int e = pe0; e < pe1; e += 4) {
-      float v[4][GC];
-      if (SMEMTAB) { gather_issue<RS, 4>(s_edges, e, e_last, ringg, cur0, Hp, v); gather_add<4>(s_edges, e, pe1, true, v, acc); }
-      else { gather_issue<RS, 4>(g_edges, e, e_last, ringg, cur0, Hp, v); gather_add<4>(g_edges, e, pe1, true, v, acc); }
-    }
+    gather_from(pe0, cur0, acc);
 #pragma unroll
     for (int j = 0; j < GC / 2; ++j) { s_cpl[(2 * j) * T] = acc[j].x; s_cpl[(2 * j + 1) * T] = acc[j].y; }
   };
-  // S4: normals of the ch0 steps from n0 on into this thread's column.  Philox (A12): one call per (sim, region)
-  // per 4 steps gives the normals of steps 4q .. 4q+3
+  // S4: Philox (A12): one call per (sim, region) per 4 steps gives the normals of steps 4q .. 4q+3.
+  // Long chunks (GCE == 8): the normals of a whole chunk are drawn next to its gather, into s_xi.
+  // Short chunks (GCE < 8, small minimum delay): the quad lives in s_quad and is redrawn every 4th step.
   auto normals_now = [&](int64_t n0, int ch0) {
     float xi[4] = {0.f, 0.f, 0.f, 0.f};
     for (int i = 0; i < ch0; ++i) {
@@ -217,11 +232,17 @@ __global__ void __launch_bounds__(K2_MAXT, 1) integrate2_kernel(const __grid_con
       s_xi[i * T] = q == 0 ? xi[0] : (q == 1 ? xi[1] : (q == 2 ? xi[2] : xi[3]));
     }
   };
+  if (GCE < 8 && noise && (P.n_begin & 3)) {      // re-enter a partly used quad at the start of a launch
+    float xi[4];
+    normals4<float>(P.seed, ext, (uint32_t)k, (uint64_t)P.n_begin >> 2, xi);
+#pragma unroll
+    for (int q = 0; q < 4; ++q) s_quad[q * T] = xi[q];
+  }
   // the gather of chunk m + 1 can overlap the compute of chunk m only if it does not need chunk m itself
   const bool LA = LAG >= 2;
   if (LA && n < P.n_end) {                        // chunk 0 of the launch has no predecessor to hide behind
     gather_now(c);
-    if (noise) normals_now(n, (int)min((int64_t)CH, P.n_end - n));
+    if (GCE == 8 && noise) normals_now(n, (int)min((int64_t)CH, P.n_end - n));
   }
 
   for (uint32_t m = 0; n < P.n_end; ++m) {
@@ -231,7 +252,7 @@ __global__ void __launch_bounds__(K2_MAXT, 1) integrate2_kernel(const __grid_con
     if (!LA) {                                    // zero minimum delay: gather right before the chunk
       if (m >= (uint32_t)LAG) { const uint32_t w = m - (uint32_t)LAG; mbar_wait(bar_done + (w & (NBAR - 1)), (w / NBAR) & 1u); }
       gather_now(c);
-      if (noise) normals_now(n, ch);
+      if (GCE == 8 && noise) normals_now(n, ch);
     }
     // the ring writes of chunk m + 1 - LAG (all warps) must be visible before the loads for chunk m + 1
     const bool pipe = LA && has_next;
@@ -243,10 +264,10 @@ __global__ void __launch_bounds__(K2_MAXT, 1) integrate2_kernel(const __grid_con
     for (int i = 0; i < ch; ++i) {
       const int64_t nn = n + i;
       const float cpl = s_cpl[i * T];
-      // ---- S1 for the next chunk: issue the loads of edges [EPS i, EPS (i + 1)) now, add them below ----
-      float pv[EPS][GC];
-      if (SMEMTAB) gather_issue<RS, EPS>(s_edges, pe0 + EPS * i, e_last, ringg, cur1, Hp, pv);   // (a table has >= 1 entry)
-      else gather_issue<RS, EPS>(g_edges, pe0 + EPS * i, e_last, ringg, cur1, Hp, pv);
+      // ---- S1 for the next chunk: issue the loads of the next PVN / GCE edges now, add them below ----
+      float pv[PVN];
+      if (SMEMTAB) gather_issue<RS, PVN / GCE, GCE>(s_edges, pe0 + (PVN / GCE) * i, e_last, ringg, cur1, Hp, pv);   // (a table has >= 1 entry)
+      else gather_issue<RS, PVN / GCE, GCE>(g_edges, pe0 + (PVN / GCE) * i, e_last, ringg, cur1, Hp, pv);
       // ---- S2 inputs (Eq. 5; A5, A6, A10) ----
       const f2 gw = s_ps[P2_GW * SPC];
       float drive = __fmaf_rn(gw.x, cpl, nu.x);
@@ -286,10 +307,20 @@ __global__ void __launch_bounds__(K2_MAXT, 1) integrate2_kernel(const __grid_con
       Cei = __fmaf_rn(dt, dCei, Cei);
       W = fma2(bc2(dt), dW, W);
       // ---- S4 OU (Eq. 4, A11) ----
-      if (noise) ou = __fmaf_rn(P.ou_rho, ou, __fmaf_rn(P.ou_s, s_xi[i * T], P.ou_m));
+      if (GCE == 8) {
+        if (noise) ou = __fmaf_rn(P.ou_rho, ou, __fmaf_rn(P.ou_s, s_xi[i * T], P.ou_m));
+      } else if (noise) {
+        if (((uint32_t)nn & 3u) == 0) {           // a new quad of normals
+          float xi[4];
+          normals4<float>(P.seed, ext, (uint32_t)k, (uint64_t)nn >> 2, xi);
+#pragma unroll
+          for (int q = 0; q < 4; ++q) s_quad[q * T] = xi[q];
+        }
+        ou = __fmaf_rn(P.ou_rho, ou, __fmaf_rn(P.ou_s, s_quad[((uint32_t)nn & 3u) * T], P.ou_m));
+      }
       // ---- S1 for the next chunk: the loads issued above have had the whole step to arrive ----
-      if (SMEMTAB) gather_add<EPS>(s_edges, pe0 + EPS * i, pe1, pipe, pv, pacc);
-      else gather_add<EPS>(g_edges, pe0 + EPS * i, pe1, pipe, pv, pacc);
+      if (SMEMTAB) gather_add<PVN / GCE, GCE>(s_edges, pe0 + (PVN / GCE) * i, pe1, pipe, pv, pacc);
+      else gather_add<PVN / GCE, GCE>(g_edges, pe0 + (PVN / GCE) * i, pe1, pipe, pv, pacc);
       // ---- S5 ring write: E at time nn+1 (mirror the first GC-1 slots behind the period) ----
       c = c + 1 == Hp ? 0 : c + 1;
       if (active) {
@@ -316,14 +347,10 @@ __global__ void __launch_bounds__(K2_MAXT, 1) integrate2_kernel(const __grid_con
       }
     }
     if (pipe) {       // the row's remaining edges (long rows, short chunks), then chunk m + 1 replaces chunk m
-      for (int e = pe0 + EPS * ch; e < pe1; e += 8) {              // one round of 8 edges: the registers of the transfer function are free here
-        float v[8][GC];
-        if (SMEMTAB) { gather_issue<RS, 8>(s_edges, e, e_last, ringg, cur1, Hp, v); gather_add<8>(s_edges, e, pe1, true, v, pacc); }
-        else { gather_issue<RS, 8>(g_edges, e, e_last, ringg, cur1, Hp, v); gather_add<8>(g_edges, e, pe1, true, v, pacc); }
-      }
+      gather_from(pe0 + (PVN / GCE) * ch, cur1, pacc);   // (the registers of the transfer function are free here)
+      if (GCE == 8 && noise) normals_now(n + ch, (int)min((int64_t)CH, P.n_end - (n + ch)));
 #pragma unroll
       for (int j = 0; j < GC / 2; ++j) { s_cpl[(2 * j) * T] = pacc[j].x; s_cpl[(2 * j + 1) * T] = pacc[j].y; }
-      if (noise) normals_now(n + ch, (int)min((int64_t)CH, P.n_end - (n + ch)));
     }
     // chunk m is written: publish it
     __syncwarp();
