@@ -92,7 +92,9 @@ typedef struct tvbx_sweep_opts {
   int64_t chunk_samples;  /* 0 = choose; downsampled samples buffered between FC reductions */
   int32_t threads_per_cta;/* 0 = choose; a value below the lanes one pass over the regions needs selects the general
                              kernel with several region passes per time block */
-  int32_t reserved;
+  int32_t ctas_per_group; /* 0 = choose; else 1..8: CTAs (one thread-block cluster) that share the regions of a group of
+                             sims_per_cta simulations -- lets N = 360 run 8 simulations per group (6 CTAs x 60 regions);
+                             packed FP32 kernel only */
 } tvbx_sweep_opts;
 
 typedef struct tvbx_run_opts {
@@ -178,8 +180,9 @@ int32_t tvbx_samples_kept(const tvbx_sweep* sw, int64_t* n);
 /* current state, [n_sims][7][N] + OU [n_sims][N], as double, to HOST buffers (synchronises) */
 int32_t tvbx_sweep_state(tvbx_sweep* sw, double* y, double* ou);
 /* launch geometry chosen for the integrator (for reports): CTAs, threads per CTA, sims per CTA,
- * registers per thread, dynamic shared memory bytes, region passes per time block */
-int32_t tvbx_launch_info(const tvbx_sweep* sw, int32_t info[8]);
+ * registers per thread, dynamic shared memory bytes, region passes per time block, samples per FC chunk,
+ * local-memory bytes per thread, CTAs per group (thread-block cluster size) */
+int32_t tvbx_launch_info(const tvbx_sweep* sw, int32_t info[9]);
 /* name of the integrator kernel this sweep runs (for reports): "tvbx::integrate2_kernel" = the packed FP32
  * product kernel (tau_e == tau_i, N * sims_per_cta <= 480, sims_per_cta <= 8), "tvbx::integrate_kernel" = the
  * general one (FP64 build mode, tau_e != tau_i, larger CTAs).  Copies at most n bytes including the NUL. */

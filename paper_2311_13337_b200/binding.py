@@ -50,7 +50,7 @@ class Axis(C.Structure):
 class SweepOpts(C.Structure):
     _fields_ = [("precision", C.c_int32), ("sims_per_cta", C.c_int32), ("n_sims", C.c_int64),
                 ("sim_ids", C.POINTER(C.c_int64)), ("chunk_samples", C.c_int64),
-                ("threads_per_cta", C.c_int32), ("reserved", C.c_int32)]
+                ("threads_per_cta", C.c_int32), ("ctas_per_group", C.c_int32)]
 
 
 class RunOpts(C.Structure):
@@ -171,7 +171,7 @@ class Sweep:
     """
 
     def __init__(self, conn: Connectome, axes, seed=0, params=None, precision=TVBX_F32, sims_per_cta=0,
-                 sim_ids=None, chunk_samples=0, threads_per_cta=0, init=None):
+                 sim_ids=None, chunk_samples=0, threads_per_cta=0, init=None, ctas_per_group=0):
         L = lib()
         self.conn = conn
         m = ModelParams()
@@ -201,7 +201,7 @@ class Sweep:
                 ax[i].values = _dptr(arr)
         o = SweepOpts()
         o.precision = precision; o.sims_per_cta = sims_per_cta; o.chunk_samples = chunk_samples
-        o.threads_per_cta = threads_per_cta
+        o.threads_per_cta = threads_per_cta; o.ctas_per_group = ctas_per_group
         if sim_ids is not None:
             ids = np.ascontiguousarray(sim_ids, dtype=np.int64)
             keep.append(ids)
@@ -305,9 +305,9 @@ class Sweep:
         return y, ou
 
     def launch_info(self):
-        a = (C.c_int32 * 8)()
+        a = (C.c_int32 * 9)()
         _chk(lib().tvbx_launch_info(self._h, a))
-        keys = ("ctas", "threads", "sims_per_cta", "regs", "smem", "passes", "chunk_samples", "local_bytes")
+        keys = ("ctas", "threads", "sims_per_cta", "regs", "smem", "passes", "chunk_samples", "local_bytes", "ctas_per_group")
         return dict(zip(keys, a[:]))
 
     def reset(self, stream=None):

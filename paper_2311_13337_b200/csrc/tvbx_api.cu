@@ -137,6 +137,7 @@ struct tvbx_sweep {
   std::vector<int64_t> ext_ids;
   uint64_t seed = 0;
   int32_t precision = TVBX_F32, spc = 8, threads_req = 0;
+  int32_t clu = 1;        // CTAs (one thread-block cluster) per group: the regions are split over them
   bool packed = false;               // FP32 closed-form product kernel (integrate2_kernel)
   int64_t chunk_req = 0;
   double init[7] = {0.001, 0.001, 0, 0, 0, 0, 0};
@@ -149,7 +150,7 @@ struct tvbx_sweep {
   bool started = false;
   double dt = 0;
   int64_t n = 0, cnt = 0, fill = 0, CS = 0, launches = 0;
-  int32_t info[8] = {0, 0, 0, 0, 0, 0, 0, 0};
+  int32_t info[9] = {0, 0, 0, 0, 0, 0, 0, 0, 1};
   int64_t h2d = 0, d2h = 0;
   bool profiling = false;
   std::vector<ProfEvent> prof;
@@ -255,20 +256,22 @@ KernelPick<float> pick_kernel<float>(bool single, bool closed, int spc) {
 // integrate2_kernel instances: compile-time simulations per CTA 1..8; delay table in shared memory with 2, 4 or
 // 8 ring slots loaded per edge, or read through L1/L2 (8 slots)
 typedef void (*Kernel2Fn)(const Integrate2Params);
-template <bool SMEMTAB, int GCE>
+template <bool SMEMTAB, int GCE, bool CLU = false>
 inline Kernel2Fn pick_kernel2_spc(int spc) {
   switch (spc) {
-    case 1: return integrate2_kernel<1, SMEMTAB, GCE>;
-    case 2: return integrate2_kernel<2, SMEMTAB, GCE>;
-    case 3: return integrate2_kernel<3, SMEMTAB, GCE>;
-    case 4: return integrate2_kernel<4, SMEMTAB, GCE>;
-    case 5: return integrate2_kernel<5, SMEMTAB, GCE>;
-    case 6: return integrate2_kernel<6, SMEMTAB, GCE>;
-    case 7: return integrate2_kernel<7, SMEMTAB, GCE>;
-    default: return integrate2_kernel<8, SMEMTAB, GCE>;
+    case 1: return integrate2_kernel<1, SMEMTAB, GCE, CLU>;
+    case 2: return integrate2_kernel<2, SMEMTAB, GCE, CLU>;
+    case 3: return integrate2_kernel<3, SMEMTAB, GCE, CLU>;
+    case 4: return integrate2_kernel<4, SMEMTAB, GCE, CLU>;
+    case 5: return integrate2_kernel<5, SMEMTAB, GCE, CLU>;
+    case 6: return integrate2_kernel<6, SMEMTAB, GCE, CLU>;
+    case 7: return integrate2_kernel<7, SMEMTAB, GCE, CLU>;
+    default: return integrate2_kernel<8, SMEMTAB, GCE, CLU>;
   }
 }
-inline Kernel2Fn pick_kernel2(int spc, bool smemtab, int gce) {
+// cluster form (several CTAs per group): table through L1/L2, 8 slots per edge
+inline Kernel2Fn pick_kernel2(int spc, bool smemtab, int gce, bool clu) {
+  if (clu) return pick_kernel2_spc<false, 8, true>(spc);
   if (!smemtab) return pick_kernel2_spc<false, 8>(spc);
   return gce == 2 ? pick_kernel2_spc<true, 2>(spc) : (gce == 4 ? pick_kernel2_spc<true, 4>(spc) : pick_kernel2_spc<true, 8>(spc));
 }
@@ -506,10 +509,11 @@ struct DeviceImpl : DeviceSide {
     P2.tables = P.tables; P2.groups = P.groups; P2.edges = (const Edge<float>*)P.edges; P2.rowptr = P.rowptr;
     P2.psim2 = d_psim2.p; P2.ext_id = P.ext_id; P2.loc_id = P.loc_id; P2.ring = (float*)P.ring; P2.state = (float*)P.state;
     P2.sums = P.sums; P2.xbar = (float*)P.xbar;
-    threads = (N * SPC + 31) / 32 * 32;
+    const int CLU = sw->clu, NL = (N + CLU - 1) / CLU;      // regions per CTA
+    threads = (NL * SPC + 31) / 32 * 32;
     single = true;
     const size_t base = (size_t)NBAR * 8 + (size_t)2 * GC * threads * sizeof(float) + (size_t)NP2 * SPC * sizeof(float2) + 16;
-    P2.smem_table = base + tbytes <= 200 * 1024;
+    P2.smem_table = CLU == 1 && base + tbytes <= 200 * 1024;
     smem = (int)(base + (P2.smem_table ? tbytes : 0));
     // one launch per run of groups whose chunk length falls in the same class (cfg 3: v <= 8 / 16 / >= 32 m/s)
     launches2.clear();
@@ -519,7 +523,7 @@ struct DeviceImpl : DeviceSide {
       const HostTable& ht = sw->tables[sw->groups[g].table];
       const int ch = ring_geom(ht.D, ht.dmin, true).CH;
       const int gce = !P2.smem_table ? 8 : (ch <= 2 ? 2 : (ch <= 4 ? 4 : 8));
-      Kernel2Fn fn = pick_kernel2(SPC, P2.smem_table != 0, gce);
+      Kernel2Fn fn = pick_kernel2(SPC, P2.smem_table != 0, gce, CLU > 1);
       if (!launches2.empty() && launches2.back().fn == fn) { launches2.back().count++; continue; }
       launches2.push_back({g, 1, fn});
       CU(cudaFuncSetAttribute((const void*)fn, cudaFuncAttributeMaxDynamicSharedMemorySize, std::max(smem, 1024)));
@@ -527,7 +531,9 @@ struct DeviceImpl : DeviceSide {
       CU(cudaFuncGetAttributes(&f1, (const void*)fn));
       if (f1.numRegs >= fa.numRegs) fa = f1;
     }
+    sw->info[0] = (int32_t)sw->groups.size() * CLU;
     sw->info[1] = threads; sw->info[3] = fa.numRegs; sw->info[4] = smem; sw->info[5] = 1; sw->info[7] = (int32_t)fa.localSizeBytes;
+    sw->info[8] = CLU;
     return TVBX_OK;
   }
 
@@ -602,7 +608,16 @@ struct DeviceImpl : DeviceSide {
         P2.sample_base = P.sample_base;
         for (const Launch2& l : launches2) {
           P2.group0 = l.g0;
-          l.fn<<<l.count, threads, smem, st>>>(P2);
+          if (sw->clu == 1) { l.fn<<<l.count, threads, smem, st>>>(P2); continue; }
+          cudaLaunchConfig_t lc;
+          std::memset(&lc, 0, sizeof lc);
+          lc.gridDim = dim3((unsigned)(l.count * sw->clu)); lc.blockDim = dim3((unsigned)threads);
+          lc.dynamicSmemBytes = (size_t)smem; lc.stream = st;
+          cudaLaunchAttribute at;
+          at.id = cudaLaunchAttributeClusterDimension;
+          at.val.clusterDim.x = (unsigned)sw->clu; at.val.clusterDim.y = 1; at.val.clusterDim.z = 1;
+          lc.attrs = &at; lc.numAttrs = 1;
+          CU(cudaLaunchKernelEx(&lc, l.fn, P2));
         }
         sw->launches += (int64_t)launches2.size() - 1;
       } else {
@@ -787,6 +802,40 @@ int32_t tvbx_sweep_create(const tvbx_connectome* c, const tvbx_model_params* def
   const int lanes_per_node = packed_ok ? 1 : 2;
   const int maxt_sel = packed_ok ? 480 : (sw->precision == TVBX_F64 ? 384 : 1024);
   const int spc_max = std::max(1, std::min(packed_ok ? 8 : 32, maxt_sel / (lanes_per_node * sw->conn.n)));
+  // CTAs per group (thread-block cluster): the packed kernel can split the regions of a group over up to 8 CTAs.
+  // Chosen when one CTA of <= 480 threads would hold fewer than 4 simulations (N > 120; cfg 5: N = 360 ->
+  // 6 CTAs x 60 regions x 8 simulations): lanes that share a region then read whole sectors of the ring.
+  int clu = opts ? opts->ctas_per_group : 0;
+  if (const char* e = getenv("TVBX_CLUSTER")) if (clu == 0) clu = atoi(e);
+  if (clu < 0 || clu > 8) return fail(TVBX_EINVAL, "ctas_per_group=%d (valid: 0..8)", clu);
+  if (clu > 1 && (!packed_ok || sw->threads_req != 0))
+    return fail(TVBX_EINVAL, "ctas_per_group > 1 needs the packed FP32 kernel (tau_e == tau_i, N <= 480, no threads_per_cta)");
+  auto clu_valid = [&](int c, int sp) {          // every CTA owns >= 1 region and fits 480 threads
+    const int nl = (sw->conn.n + c - 1) / c;
+    return (c - 1) * nl < sw->conn.n && nl * sp <= 480;
+  };
+  if (clu == 0 && spc == 0 && packed_ok && sw->threads_req == 0 && spc_max < 4) {
+    std::map<double, int64_t> per_v;
+    for (int64_t s = 0; s < sw->n_sims; ++s) per_v[sw->param(s, TVBX_P_V)]++;
+    int64_t most = 1;
+    for (auto& kv : per_v) most = std::max(most, kv.second);
+    int want = 8;
+    while (want > 1 && want / 2 >= most) want /= 2;       // no more lanes than the largest speed class can fill
+    int best_thr = -1;
+    for (int c = 1; c <= 8; ++c) {
+      if (!clu_valid(c, want)) continue;
+      const int thr = ((sw->conn.n + c - 1) / c) * want;
+      if (thr > best_thr) { best_thr = thr; clu = c; }
+    }
+    if (best_thr > 0) spc = want; else clu = 0;
+  }
+  if (clu == 0) clu = 1;
+  if (clu > 1) {
+    if (spc == 0) { spc = 8; while (spc > 1 && !clu_valid(clu, spc)) --spc; }
+    if (spc > 8 || !clu_valid(clu, spc))
+      return fail(TVBX_EINVAL, "ctas_per_group=%d with sims_per_cta=%d does not fit (N=%d, <= 480 threads per CTA, no empty CTA)", clu, spc, sw->conn.n);
+  }
+  sw->clu = clu;
   if (spc == 0) {
     // simulations per distinct speed decide the CTA count; approximate with one table here
     std::map<double, int64_t> per_v;
@@ -807,7 +856,7 @@ int32_t tvbx_sweep_create(const tvbx_connectome* c, const tvbx_model_params* def
   }
   if (spc < 1 || spc > 32) return fail(TVBX_EINVAL, "sims_per_cta=%d (valid: 1..32)", spc);
   sw->spc = spc;
-  sw->packed = packed_ok && spc <= 8 && sw->conn.n * spc <= 480 && (sw->threads_req == 0 || sw->threads_req >= sw->conn.n * spc);
+  sw->packed = packed_ok && spc <= 8 && ((sw->conn.n + clu - 1) / clu) * spc <= 480 && (sw->threads_req == 0 || sw->threads_req >= sw->conn.n * spc);
   // group the simulations by speed (one delay table per distinct v), then into CTAs of spc lanes
   std::map<double, int32_t> vmap;
   sw->sim_table.resize(sw->n_sims);
@@ -958,9 +1007,9 @@ int32_t tvbx_sweep_state(tvbx_sweep* sw, double* y, double* ou) {
   if (!sw->started) return fail(TVBX_ESTATE, "no run yet");
   return sw->dev->state(y, ou);
 }
-int32_t tvbx_launch_info(const tvbx_sweep* sw, int32_t info[8]) {
+int32_t tvbx_launch_info(const tvbx_sweep* sw, int32_t info[9]) {
   if (!sw || !info) return fail(TVBX_EINVAL, "NULL argument");
-  for (int i = 0; i < 8; ++i) info[i] = sw->info[i];
+  for (int i = 0; i < 9; ++i) info[i] = sw->info[i];
   return TVBX_OK;
 }
 int32_t tvbx_kernel_name(const tvbx_sweep* sw, char* buf, int32_t n) {

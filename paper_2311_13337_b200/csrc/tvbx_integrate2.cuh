@@ -98,13 +98,46 @@ __device__ __forceinline__ void mbar_wait(uint64_t* bar, uint32_t parity) {
       : "memory");
 }
 
+// ---- thread-block cluster forms (CLU): the regions of a group are split over the CTAs of a cluster; the ring
+// lives in global memory, only the chunk hand-over crosses CTAs: a warp arrives (release.cluster) on the barrier
+// of EVERY CTA of its cluster through distributed shared memory and waits (acquire.cluster) on its own CTA's.
+__device__ __forceinline__ uint32_t cluster_ctarank() { uint32_t r; asm volatile("mov.u32 %0, %%cluster_ctarank;" : "=r"(r)); return r; }
+__device__ __forceinline__ uint32_t cluster_nctarank() { uint32_t r; asm volatile("mov.u32 %0, %%cluster_nctarank;" : "=r"(r)); return r; }
+__device__ __forceinline__ void cluster_sync_all() {
+  asm volatile("barrier.cluster.arrive.release.aligned;\n\tbarrier.cluster.wait.acquire.aligned;" ::: "memory");
+}
+__device__ __forceinline__ void mbar_arrive_cluster(uint64_t* bar, uint32_t nrank) {
+  const uint32_t local = smem_u32(bar);
+  for (uint32_t r = 0; r < nrank; ++r) {
+    uint32_t remote;
+    asm volatile("mapa.shared::cluster.u32 %0, %1, %2;" : "=r"(remote) : "r"(local), "r"(r));
+    asm volatile("mbarrier.arrive.release.cluster.shared::cluster.b64 _, [%0];" ::"r"(remote) : "memory");
+  }
+}
+__device__ __forceinline__ void mbar_wait_cluster(uint64_t* bar, uint32_t parity) {
+  asm volatile(
+      "{\n"
+      ".reg .pred p;\n"
+      "WAITC_%=:\n"
+      "mbarrier.try_wait.parity.acquire.cluster.shared::cta.b64 p, [%0], %1;\n"
+      "@p bra DONEC_%=;\n"
+      "bra WAITC_%=;\n"
+      "DONEC_%=:\n"
+      "}\n" ::"r"(smem_u32(bar)), "r"(parity)
+      : "memory");
+}
+// ring load: CG = through L2 only (cluster form: the line may have been written by another SM since this SM's L1
+// last saw it, and with 8 simulations per slot every 32-byte sector is consumed by one instruction anyway)
+template <bool CG>
+__device__ __forceinline__ float ring_ld(const float* p) { return CG ? __ldcg(p) : *p; }
+
 // One batch of EBT edges [e, e + EBT) of a row for the chunk whose first step sits in ring slot `cur`: issue the
 // ring loads of the first GCE slots of every edge (GCE = 2, 4 or 8 >= the chunk length) and return the values in
 // v[EBT * GCE].  The loads are unconditional: a batch may run past the row (or past the CH slots a short chunk
 // uses) -- it then reads other valid ring entries (the table index is clamped to e_last, rows are GC-1 mirror
 // slots longer than the period) whose weight gather_add sets to zero.  The caller adds them with gather_add --
 // later, when it wants the latency hidden.
-template <int RS, int EBT, int GCE, typename EdgePtr>
+template <int RS, int EBT, int GCE, bool CG, typename EdgePtr>
 __device__ __forceinline__ void gather_issue(EdgePtr edges, int e, int e_last, const float* ringg, int cur, int Hp, float* v) {
   // slot of the first read = (cur + back) mod Hp with back = Hp - d in [0, Hp]: wraps iff back >= Hp - cur.
   // The table stores pad = jbase + back * RS, so the element offset is pad + cur * RS - (wrap ? Hp * RS : 0).
@@ -115,7 +148,7 @@ __device__ __forceinline__ void gather_issue(EdgePtr edges, int e, int e_last, c
     const uint32_t off = ed.pad + curRS - (ed.back >= thr ? wrapRS : 0u);
     const float* src = ringg + off;
 #pragma unroll
-    for (int j = 0; j < GCE; ++j) v[b * GCE + j] = src[j * RS];
+    for (int j = 0; j < GCE; ++j) v[b * GCE + j] = ring_ld<CG>(src + j * RS);
   }
 }
 // acc[j] += w * (E(slot 2j), E(slot 2j+1)), j < GCE/2: the row's edges are added in ascending order into each
@@ -130,27 +163,34 @@ __device__ __forceinline__ void gather_add(EdgePtr edges, int e, int e1, bool en
   }
 }
 // the edges [e, e1) of a row in unpipelined rounds of 8 edges
-template <int RS, int GCE, typename EdgePtr>
+template <int RS, int GCE, bool CG, typename EdgePtr>
 __device__ __forceinline__ void gather_rounds(EdgePtr edges, int e, int e1, int e_last, const float* ringg, int cur, int Hp,
                                               f2 acc[GC / 2]) {
   for (; e < e1; e += 8) {
     float v[8 * GCE];
-    gather_issue<RS, 8, GCE>(edges, e, e_last, ringg, cur, Hp, v);
+    gather_issue<RS, 8, GCE, CG>(edges, e, e_last, ringg, cur, Hp, v);
     gather_add<8, GCE>(edges, e, e1, true, v, acc);
   }
 }
 
 // SPC: simulations per CTA (1..8); SMEMTAB: the delay table of the group's speed is staged in shared memory;
 // GCE: ring slots loaded per edge = 2, 4 or 8 >= the chunk length CH of the launched groups (P.group0 ...).
-// blockDim = N*SPC rounded up to whole warps (<= K2_MAXT); lanes past the last node replay it, stores suppressed.
-template <int SPC, bool SMEMTAB, int GCE>
+// CLU: the group is integrated by a thread-block cluster; CTA r of the cluster owns the regions [r*NL, (r+1)*NL), NL =
+// ceil(N / cluster size) (N = 360: 6 CTAs x 60 regions x 8 simulations -- lanes that share a region then read whole
+// 32-byte sectors of the ring, which a single CTA of <= 480 threads cannot offer at N = 360).
+// blockDim = (regions of the CTA)*SPC rounded up to whole warps (<= K2_MAXT); lanes past the last node replay it,
+// stores suppressed.
+template <int SPC, bool SMEMTAB, int GCE, bool CLU>
 __global__ void __launch_bounds__(K2_MAXT, 1) integrate2_kernel(const __grid_constant__ Integrate2Params P) {
   extern __shared__ __align__(16) unsigned char smem_raw[];
   constexpr int RS = SPC;                         // simulation columns of a ring slot
-  const int g = blockIdx.x + P.group0;
+  const uint32_t nrank = CLU ? cluster_nctarank() : 1u, crank = CLU ? cluster_ctarank() : 0u;
+  const int g = (CLU ? (int)(blockIdx.x / nrank) : (int)blockIdx.x) + P.group0;
   const int N = P.N;
   const int tid = threadIdx.x, T = blockDim.x;
-  const int NODES = N * SPC;
+  const int NL = CLU ? (N + (int)nrank - 1) / (int)nrank : N;      // regions per CTA
+  const int k0 = CLU ? (int)crank * NL : 0;
+  const int NODES = min(NL, N - k0) * SPC;        // (the host picks a cluster size that leaves no CTA empty)
   const GroupDesc gd = P.groups[g];
   const TableDesc td = P.tables[gd.table];
   const int Hp = td.Hp, Hs = td.Hs, CH = td.CH, LAG = td.LAG;
@@ -168,18 +208,18 @@ __global__ void __launch_bounds__(K2_MAXT, 1) integrate2_kernel(const __grid_con
   const Edge<float>* const g_edges = P.edges + td.edge_off;
   const int32_t* const g_rowptr = P.rowptr + td.rowptr_off;
   {
-    if (tid < NBAR) mbar_init(bar_done + tid, (uint32_t)(T >> 5));
+    if (tid < NBAR) mbar_init(bar_done + tid, (uint32_t)(T >> 5) * nrank);
     for (int i = tid; i < NP2 * SPC; i += T) s_ps[i] = P.psim2[(size_t)g * NP2 * SPC + i];
     if (SMEMTAB) {
       for (int i = tid; i < td.n_edges; i += T) s_edges[i] = g_edges[i];
       for (int i = tid; i <= N; i += T) s_rowptr[i] = g_rowptr[i];
     }
-    __syncthreads();
+    if (CLU) cluster_sync_all(); else __syncthreads();      // (remote arrivals need the peers' barriers initialised)
   }
   const bool noise = P.noise_on != 0;
   const bool active = tid < NODES;
   const int node = active ? tid : NODES - 1;
-  const int k = node / SPC, sl = node - k * SPC;
+  const int kl = node / SPC, sl = node - kl * SPC, k = k0 + kl;
   s_ps += sl;
   float* const ringg = P.ring + gd.ring_off + sl;   // this group's ring, the thread's simulation column
   const int e_last = td.n_edges - 1;
@@ -209,8 +249,8 @@ __global__ void __launch_bounds__(K2_MAXT, 1) integrate2_kernel(const __grid_con
 
   // S1, not pipelined: coupling sums of the chunk that starts at ring slot cur0 into this thread's column
   auto gather_from = [&](int e, int cur0, f2 acc[GC / 2]) {
-    if (SMEMTAB) gather_rounds<RS, GCE>(s_edges, e, pe1, e_last, ringg, cur0, Hp, acc);
-    else gather_rounds<RS, GCE>(g_edges, e, pe1, e_last, ringg, cur0, Hp, acc);
+    if (SMEMTAB) gather_rounds<RS, GCE, CLU>(s_edges, e, pe1, e_last, ringg, cur0, Hp, acc);
+    else gather_rounds<RS, GCE, CLU>(g_edges, e, pe1, e_last, ringg, cur0, Hp, acc);
   };
   auto gather_now = [&](int cur0) {
     f2 acc[GC / 2];
@@ -245,18 +285,22 @@ __global__ void __launch_bounds__(K2_MAXT, 1) integrate2_kernel(const __grid_con
     if (GCE == 8 && noise) normals_now(n, (int)min((int64_t)CH, P.n_end - n));
   }
 
+  auto wait_chunk = [&](uint32_t w) {              // all warps of the group have written chunk w
+    if (CLU) mbar_wait_cluster(bar_done + (w & (NBAR - 1)), (w / NBAR) & 1u);
+    else mbar_wait(bar_done + (w & (NBAR - 1)), (w / NBAR) & 1u);
+  };
   for (uint32_t m = 0; n < P.n_end; ++m) {
     const int ch = (int)min((int64_t)CH, P.n_end - n);
     const bool has_next = n + ch < P.n_end;
     const int cur1 = c + ch >= Hp ? c + ch - Hp : c + ch;          // ring slot of the next chunk's first step
     if (!LA) {                                    // zero minimum delay: gather right before the chunk
-      if (m >= (uint32_t)LAG) { const uint32_t w = m - (uint32_t)LAG; mbar_wait(bar_done + (w & (NBAR - 1)), (w / NBAR) & 1u); }
+      if (m >= (uint32_t)LAG) { const uint32_t w = m - (uint32_t)LAG; wait_chunk(w); }
       gather_now(c);
       if (GCE == 8 && noise) normals_now(n, ch);
     }
     // the ring writes of chunk m + 1 - LAG (all warps) must be visible before the loads for chunk m + 1
     const bool pipe = LA && has_next;
-    if (pipe && m + 1 >= (uint32_t)LAG) { const uint32_t w = m + 1 - (uint32_t)LAG; mbar_wait(bar_done + (w & (NBAR - 1)), (w / NBAR) & 1u); }
+    if (pipe && m + 1 >= (uint32_t)LAG) { const uint32_t w = m + 1 - (uint32_t)LAG; wait_chunk(w); }
     f2 pacc[GC / 2];                              // coupling sums of chunk m + 1 in the making
 #pragma unroll
     for (int j = 0; j < GC / 2; ++j) pacc[j] = mk2(0.0f, 0.0f);
@@ -266,8 +310,8 @@ __global__ void __launch_bounds__(K2_MAXT, 1) integrate2_kernel(const __grid_con
       const float cpl = s_cpl[i * T];
       // ---- S1 for the next chunk: issue the loads of the next PVN / GCE edges now, add them below ----
       float pv[PVN];
-      if (SMEMTAB) gather_issue<RS, PVN / GCE, GCE>(s_edges, pe0 + (PVN / GCE) * i, e_last, ringg, cur1, Hp, pv);   // (a table has >= 1 entry)
-      else gather_issue<RS, PVN / GCE, GCE>(g_edges, pe0 + (PVN / GCE) * i, e_last, ringg, cur1, Hp, pv);
+      if (SMEMTAB) gather_issue<RS, PVN / GCE, GCE, CLU>(s_edges, pe0 + (PVN / GCE) * i, e_last, ringg, cur1, Hp, pv);   // (a table has >= 1 entry)
+      else gather_issue<RS, PVN / GCE, GCE, CLU>(g_edges, pe0 + (PVN / GCE) * i, e_last, ringg, cur1, Hp, pv);
       // ---- S2 inputs (Eq. 5; A5, A6, A10) ----
       const f2 gw = s_ps[P2_GW * SPC];
       float drive = __fmaf_rn(gw.x, cpl, nu.x);
@@ -354,9 +398,13 @@ __global__ void __launch_bounds__(K2_MAXT, 1) integrate2_kernel(const __grid_con
     }
     // chunk m is written: publish it
     __syncwarp();
-    if ((tid & 31) == 0) mbar_arrive(bar_done + (m & (NBAR - 1)));
+    if ((tid & 31) == 0) {
+      if (CLU) mbar_arrive_cluster(bar_done + (m & (NBAR - 1)), nrank);
+      else mbar_arrive(bar_done + (m & (NBAR - 1)));
+    }
     n += ch;
   }
+  if (CLU) cluster_sync_all();                    // no CTA leaves while a peer may still arrive on its barriers
   if (active) {
     sp[0] = nu.x; sp[stride] = nu.y; sp[2 * stride] = Cs.x; sp[3 * stride] = Cei; sp[4 * stride] = Cs.y;
     sp[5 * stride] = W.x; sp[6 * stride] = W.y; sp[7 * stride] = ou; sp[8 * stride] = win.x; sp[9 * stride] = win.y;

@@ -147,6 +147,36 @@ def test_multi_pass_mapping_when_regions_exceed_the_cta(threads):
     assert traj_err(traj, ref) < TOL_TRAJ_F32
 
 
+@pytest.mark.parametrize("clu,spc", [(2, 4), (3, 8), (8, 3), (5, 1)])
+def test_cluster_mapping_regions_split_over_ctas(clu, spc):
+    """ctas_per_group > 1: the regions of a group are split over the CTAs of a thread-block cluster (the
+    N = 360 mapping), chunk hand-over through cluster-scope mbarriers.  Ragged: 37 regions over 2, 3, 5, 8
+    CTAs, 12 sims in two speed classes (long and short chunks), sims per group not dividing the class."""
+    W, L = wl.connectome(37, seed=5, keep=0.35)
+    axes = [dict(name="G", lo=0.0, hi=0.4, n=6, values=None), dict(name="v", lo=0, hi=0, n=2, values=[3.0, 40.0])]
+    cfg = dict(axes=axes, fixed=dict(b_e=20.0, wNoise=1e-4), seed=9)
+    sw, traj, o, ref = run_pair(cfg, W, L, 700, True, traj_steps=700, sims_per_cta=spc, ctas_per_group=clu, discard=100)
+    info = sw.launch_info()
+    assert info["ctas_per_group"] == clu and info["sims_per_cta"] == spc and sw.kernel_name() == "tvbx::integrate2_kernel"
+    assert traj_err(traj, ref) < TOL_TRAJ_F32
+    fc, me, mi = sw.fc_readout()
+    rfc, rme, rmi = o.fc_readout()
+    assert np.abs(me / rme - 1).max() < TOL_MEAN_REL and np.abs(fc - rfc).max() < TOL_FC_ABS
+
+
+def test_cluster_mapping_is_bitwise_the_single_cta_mapping():
+    """The cluster only changes which CTA owns a region: same per-node arithmetic, same edge order -> the
+    trajectories equal those of the one-CTA mapping bit for bit."""
+    W, L = wl.connectome(37, seed=5, keep=0.35)
+    cfg = dict(axes=[dict(name="G", lo=0.0, hi=0.4, n=5, values=None)], fixed=dict(v=5.0, wNoise=1e-4), seed=4)
+    _, a = tvbx.sweep_from_config(cfg, W, L, sims_per_cta=4, ctas_per_group=1)
+    _, b = tvbx.sweep_from_config(cfg, W, L, sims_per_cta=4, ctas_per_group=4)
+    ta = a.run(900, 0.1, noise_on=True, ds=10, traj_steps=900)
+    tb = b.run(900, 0.1, noise_on=True, ds=10, traj_steps=900)
+    np.testing.assert_array_equal(ta, tb)
+    np.testing.assert_array_equal(a.fc_readout()[0], b.fc_readout()[0])
+
+
 def test_mixed_speeds_cfg3_slice():
     """cfg 3 slice covering all 8 speeds (ring depth 16 ... 2000, min delay 1 ... 100 steps)."""
     cfg = wl.config(3)
