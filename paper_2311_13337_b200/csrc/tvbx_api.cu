@@ -84,13 +84,17 @@ int32_t block_steps(int32_t dmin) {
 // times <= CH m + CH - 1 - d_min, written by chunks <= m - LAG with LAG = ceil((d_min + 2)/CH) - 1 (>= 2 unless
 // d_min = 0; capped at LAGMAX), so the gather of chunk m + 1 can precede the compute
 // of chunk m, a warp may run LAG chunks ahead of the slowest one and the period is D + CH LAG + 1.
-struct RingGeom { int32_t B, CH, LAG, Hp; };
-RingGeom ring_geom(int32_t D, int32_t dmin, bool packed) {
+// vec_ok: the sweep runs the cluster form whose full-length chunks (CH == GC) use the quad ring layout and the
+// vector gather (tvbx_integrate2.cuh, gather_class_vec): the period is then a multiple of 4.
+struct RingGeom { int32_t B, CH, LAG, Hp, vec; };
+RingGeom ring_geom(int32_t D, int32_t dmin, bool packed, bool vec_ok = false) {
   RingGeom g;
   g.B = block_steps(dmin);
   g.CH = std::max(1, std::min<int32_t>(tvbx::GC, (std::max(0, dmin) + 1) / 2));
   g.LAG = std::max(1, std::min<int32_t>(tvbx::LAGMAX, (dmin + 2 + g.CH - 1) / g.CH - 1));
   g.Hp = packed ? D + g.CH * g.LAG + 1 : D + g.B + 1;
+  g.vec = packed && vec_ok && g.CH == tvbx::GC;
+  if (g.vec) g.Hp = (g.Hp + 3) / 4 * 4;
   return g;
 }
 
@@ -100,7 +104,7 @@ struct Axis { int32_t id; std::vector<double> vals; };
 
 struct HostTable {      // one per distinct speed
   double v = 0;
-  int32_t D = 0, dmin = 0, B = 1, Hp = 2;
+  int32_t D = 0, dmin = 0, B = 1, Hp = 2, vec = 0;
   std::vector<int32_t> delays;   // per kept edge, CSR order
   std::vector<int64_t> sims;     // local sim indices
 };
@@ -138,6 +142,7 @@ struct tvbx_sweep {
   uint64_t seed = 0;
   int32_t precision = TVBX_F32, spc = 8, threads_req = 0;
   int32_t clu = 1;        // CTAs (one thread-block cluster) per group: the regions are split over them
+  bool vec_ok = false;    // cluster form with 4 or 8 simulations per group: vector gather where the chunk length allows
   bool packed = false;               // FP32 closed-form product kernel (integrate2_kernel)
   int64_t chunk_req = 0;
   double init[7] = {0.001, 0.001, 0, 0, 0, 0, 0};
@@ -269,8 +274,9 @@ inline Kernel2Fn pick_kernel2_spc(int spc) {
     default: return integrate2_kernel<8, SMEMTAB, GCE, CLU>;
   }
 }
-// cluster form (several CTAs per group): table through L1/L2, 8 slots per edge
-inline Kernel2Fn pick_kernel2(int spc, bool smemtab, int gce, bool clu) {
+// cluster form (several CTAs per group): table through L1/L2, 8 slots per edge; vec: quad ring layout + vector gather
+inline Kernel2Fn pick_kernel2(int spc, bool smemtab, int gce, bool clu, bool vec) {
+  if (clu && vec) return spc == 8 ? integrate2_kernel<8, false, 8, true, true> : integrate2_kernel<4, false, 8, true, true>;
   if (clu) return pick_kernel2_spc<false, 8, true>(spc);
   if (!smemtab) return pick_kernel2_spc<false, 8>(spc);
   return gce == 2 ? pick_kernel2_spc<true, 2>(spc) : (gce == 4 ? pick_kernel2_spc<true, 4>(spc) : pick_kernel2_spc<true, 8>(spc));
@@ -283,7 +289,7 @@ struct DeviceImpl : DeviceSide {
   DevBuf<TableDesc> d_tables;
   DevBuf<GroupDesc> d_groups;
   DevBuf<Edge<R>> d_edges;
-  DevBuf<int32_t> d_rowptr, d_ext, d_loc;
+  DevBuf<int32_t> d_rowptr, d_seg, d_ext, d_loc;
   DevBuf<R> d_psim, d_ring, d_state, d_xbar;
   DevBuf<double> d_sums, d_cmean, d_mean, d_M, d_M_scratch, d_mean_scratch;
   DevBuf<float> d_out_fc, d_out_me, d_out_mi;
@@ -312,7 +318,7 @@ struct DeviceImpl : DeviceSide {
     // ---- delay tables per distinct speed (A13) and ring geometry ----
     std::vector<TableDesc> tds(sw->tables.size());
     std::vector<Edge<R>> edges;
-    std::vector<int32_t> rowptr;
+    std::vector<int32_t> rowptr, seg;
     for (size_t t = 0; t < sw->tables.size(); ++t) {
       HostTable& ht = sw->tables[t];
       ht.delays.clear();
@@ -324,17 +330,35 @@ struct DeviceImpl : DeviceSide {
         D = std::max(D, d); dmin = std::min(dmin, d);
       }
       if (c.edges.empty()) dmin = GC;
-      const RingGeom rg = ring_geom(D, dmin, sw->packed);
-      ht.D = D; ht.dmin = dmin; ht.B = rg.B; ht.Hp = rg.Hp;
-      const int32_t Hs = ht.Hp + GC - 1;
+      const RingGeom rg = ring_geom(D, dmin, sw->packed, sw->vec_ok);
+      ht.D = D; ht.dmin = dmin; ht.B = rg.B; ht.Hp = rg.Hp; ht.vec = rg.vec;
+      const int32_t Hs = ht.Hp + (rg.vec ? GC : GC - 1);
       if ((double)N * Hs * RS >= 4294967295.0) return fail(TVBX_EINVAL, "ring of one CTA exceeds 32-bit element offsets");
       tds[t].Hp = ht.Hp; tds[t].Hs = Hs; tds[t].B = ht.B; tds[t].n_edges = (int32_t)c.edges.size();
       tds[t].CH = rg.CH; tds[t].LAG = rg.LAG;
       tds[t].edge_off = (int64_t)edges.size(); tds[t].rowptr_off = (int64_t)rowptr.size();
+      tds[t].vec = rg.vec; tds[t].seg_off = (int64_t)seg.size();
       const int pad_to = 1;      // (rows may be padded with zero-weight copies of their first edge)
       for (int k = 0; k < N; ++k) {
         rowptr.push_back((int32_t)(edges.size() - (size_t)tds[t].edge_off));
         const int r0 = c.rowptr[k], r1 = c.rowptr[k + 1];
+        if (rg.vec) {      // quad layout: the row sorted by window alignment class a = (Hp - d) mod 4, ascending j inside
+          for (int a = 0; a < 4; ++a) {
+            for (int e = r0; e < r1; ++e) {
+              const uint32_t back = (uint32_t)(ht.Hp - ht.delays[e]);
+              if ((int)(back & 3u) != a) continue;
+              Edge<R> ed;
+              std::memset(&ed, 0, sizeof ed);
+              ed.w = (R)c.edges[e].w;
+              ed.jbase = (uint32_t)c.edges[e].j * (uint32_t)Hs * (uint32_t)RS;
+              ed.back = back;
+              set_pad(ed, ed.jbase + (back & ~3u) * (uint32_t)RS);
+              edges.push_back(ed);
+            }
+            seg.push_back((int32_t)(edges.size() - (size_t)tds[t].edge_off));
+          }
+          continue;
+        }
         for (int e = r0; e < r1 || (e - r0) % pad_to != 0; ++e) {
           const int es = e < r1 ? e : r0;
           Edge<R> ed;
@@ -365,7 +389,8 @@ struct DeviceImpl : DeviceSide {
     for (int g = 0; g < G; ++g) {
       const HostGroup& hg = sw->groups[g];
       gds[g].table = hg.table; gds[g].pad = 0; gds[g].ring_off = (int64_t)ring_elems;
-      ring_elems += (size_t)N * (sw->tables[hg.table].Hp + GC - 1) * RS;
+      ring_elems += (size_t)N * (sw->tables[hg.table].Hp + (sw->tables[hg.table].vec ? GC : GC - 1)) * RS;
+      ring_elems = (ring_elems + 31) / 32 * 32;      // every group's ring starts on a 128-byte line
       for (int sl = 0; sl < SPC; ++sl) {
         const int64_t s = hg.lanes[sl];
         const int64_t src = s >= 0 ? s : hg.lanes[0];      // padding lanes replay lane 0, never read back
@@ -406,6 +431,8 @@ struct DeviceImpl : DeviceSide {
     sw->CS = CS;
     int64_t* hb = &sw->h2d;
     CU(d_tables.upload(tds, hb)); CU(d_groups.upload(gds, hb)); CU(d_edges.upload(edges, hb)); CU(d_rowptr.upload(rowptr, hb));
+    if (seg.empty()) seg.assign(4, 0);
+    CU(d_seg.upload(seg, hb));
     CU(d_ext.upload(ext, hb)); CU(d_loc.upload(loc, hb)); CU(d_psim.upload(psim, hb));
     if (sw->packed) CU(d_psim2.upload(psim2, hb));
     CU(d_ring.alloc(ring_elems));
@@ -506,7 +533,7 @@ struct DeviceImpl : DeviceSide {
     P2.kappa = (float)P.kappa; P2.inv_Ne = (float)P.inv_Ne; P2.inv_Ni = (float)P.inv_Ni;
     P2.ou_rho = (float)P.ou_rho; P2.ou_s = (float)P.ou_s; P2.ou_m = (float)P.ou_m; P2.dt = (float)P.dt;
     P2.muV_local = P.muV_local; P2.N = N; P2.SPC = SPC; P2.seed = P.seed; P2.chunk_samples = P.chunk_samples;
-    P2.tables = P.tables; P2.groups = P.groups; P2.edges = (const Edge<float>*)P.edges; P2.rowptr = P.rowptr;
+    P2.tables = P.tables; P2.groups = P.groups; P2.edges = (const Edge<float>*)P.edges; P2.rowptr = P.rowptr; P2.seg = d_seg.p;
     P2.psim2 = d_psim2.p; P2.ext_id = P.ext_id; P2.loc_id = P.loc_id; P2.ring = (float*)P.ring; P2.state = (float*)P.state;
     P2.sums = P.sums; P2.xbar = (float*)P.xbar;
     const int CLU = sw->clu, NL = (N + CLU - 1) / CLU;      // regions per CTA
@@ -523,7 +550,7 @@ struct DeviceImpl : DeviceSide {
       const HostTable& ht = sw->tables[sw->groups[g].table];
       const int ch = ring_geom(ht.D, ht.dmin, true).CH;
       const int gce = !P2.smem_table ? 8 : (ch <= 2 ? 2 : (ch <= 4 ? 4 : 8));
-      Kernel2Fn fn = pick_kernel2(SPC, P2.smem_table != 0, gce, CLU > 1);
+      Kernel2Fn fn = pick_kernel2(SPC, P2.smem_table != 0, gce, CLU > 1, ht.vec != 0);
       if (!launches2.empty() && launches2.back().fn == fn) { launches2.back().count++; continue; }
       launches2.push_back({g, 1, fn});
       CU(cudaFuncSetAttribute((const void*)fn, cudaFuncAttributeMaxDynamicSharedMemorySize, std::max(smem, 1024)));
@@ -857,6 +884,7 @@ int32_t tvbx_sweep_create(const tvbx_connectome* c, const tvbx_model_params* def
   if (spc < 1 || spc > 32) return fail(TVBX_EINVAL, "sims_per_cta=%d (valid: 1..32)", spc);
   sw->spc = spc;
   sw->packed = packed_ok && spc <= 8 && ((sw->conn.n + clu - 1) / clu) * spc <= 480 && (sw->threads_req == 0 || sw->threads_req >= sw->conn.n * spc);
+  sw->vec_ok = sw->packed && clu > 1 && (spc == 8 || spc == 4) && getenv("TVBX_NO_VEC") == nullptr;
   // group the simulations by speed (one delay table per distinct v), then into CTAs of spc lanes
   std::map<double, int32_t> vmap;
   sw->sim_table.resize(sw->n_sims);
@@ -989,7 +1017,7 @@ int32_t tvbx_ring_len(const tvbx_sweep* sw, int64_t sim, double dt, int32_t* H, 
   for (const HostEdge& e : sw->conn.edges) { const int32_t d = delay_steps(e.L, v, dt); D = std::max(D, d); dmin = std::min(dmin, d); }
   if (sw->conn.edges.empty()) dmin = tvbx::GC;
   if (H) *H = D + 1;
-  if (H_phys) *H_phys = ring_geom(D, dmin, sw->packed).Hp;
+  if (H_phys) *H_phys = ring_geom(D, dmin, sw->packed, sw->vec_ok).Hp;
   return TVBX_OK;
 }
 int32_t tvbx_steps_done(const tvbx_sweep* sw, int64_t* n) {

@@ -88,6 +88,9 @@ struct TableDesc {      // one per distinct speed v
   int32_t LAG;          // chunks a warp may run ahead of the slowest one (integrate2_kernel)
   int64_t edge_off;     // first edge in the edge array
   int64_t rowptr_off;   // first entry of this table's row pointer (N+1 ints)
+  int64_t seg_off;      // VEC tables (integrate2_kernel, quad ring layout): first entry of the [N][4] class ends
+  int32_t vec;          // 1: quad ring layout, rows sorted by window alignment class
+  int32_t pad0;
 };
 struct GroupDesc {      // one per CTA
   int32_t table;

@@ -62,6 +62,7 @@ struct Integrate2Params {
   const GroupDesc* groups;
   const Edge<float>* edges;
   const int32_t* rowptr;
+  const int32_t* seg;             // VEC tables: [N][4] end of the row's edges of alignment class 0..3 (TableDesc::seg_off)
   const float2* psim2;            // [group][NP2][SPC]
   const int32_t* ext_id;          // [group][SPC]  external sim index (Philox counter)
   const int32_t* loc_id;          // [group][SPC]  local sim index (row of traj), -1 = padding lane
@@ -173,6 +174,48 @@ __device__ __forceinline__ void gather_rounds(EdgePtr edges, int e, int e1, int 
   }
 }
 
+// ---- vector form of the gather (VEC: cluster kernels whose chunk length is GC = 8) ---------------------------
+// Ring layout ring[group][region][slot / 4][sim][slot % 4] (Hp a multiple of 4, 8 mirror slots): the four
+// consecutive time slots of a quad sit in one 16-byte word per simulation, so a thread fetches its 8-slot window
+// with three aligned LDG.128 (12 slots) and the 8 lanes that share a region fetch whole 128-byte lines -- one L2
+// request per line instead of one per sector (the scalar cluster form is bound by the L1->XBAR request rate:
+// l1tex__m_l1tex2xbar_req_cycles_active 65 %).  Chunks start at multiples of GC, so the alignment of an edge's
+// window inside its first quad, a = (Hp - d) mod 4, never changes: the host sorts every row by a, the products
+// of a class are accumulated UNSHIFTED over the 12 fetched slots and folded once per class,
+// cpl[j] += acc[a + j] -- no per-edge select.  Per slot the association is: classes 0..3 in order, inside a class
+// the row's edges in ascending j (gather_head_vec reproduces it for the unaligned first chunk of a launch).
+enum { VR = 5 };                 // edges per round of the vector gather (VR x 12 values in registers)
+template <int RS, int A>
+__device__ __forceinline__ void gather_class_vec(const Edge<float>* edges, int e, int e1, int e_last, const float* ringv,
+                                                 uint32_t curRS, uint32_t thr, uint32_t wrapRS, float cpl[GC]) {
+  f2 acc[6];
+#pragma unroll
+  for (int i = 0; i < 6; ++i) acc[i] = mk2(0.0f, 0.0f);
+  for (; e < e1; e += VR) {
+    float4 q[VR][3];
+    float w[VR];
+#pragma unroll
+    for (int b = 0; b < VR; ++b) {
+      const Edge<float> ed = edges[min(e + b, e_last)];
+      const uint32_t off = ed.pad + curRS - (ed.back >= thr ? wrapRS : 0u);
+      const float4* src = reinterpret_cast<const float4*>(ringv + off);
+      q[b][0] = __ldcg(src); q[b][1] = __ldcg(src + RS); q[b][2] = __ldcg(src + 2 * RS);
+      w[b] = e + b < e1 ? ed.w : 0.0f;
+    }
+#pragma unroll
+    for (int b = 0; b < VR; ++b) {
+#pragma unroll
+      for (int i = 0; i < 3; ++i) {
+        acc[2 * i] = fma2(bc2(w[b]), mk2(q[b][i].x, q[b][i].y), acc[2 * i]);
+        acc[2 * i + 1] = fma2(bc2(w[b]), mk2(q[b][i].z, q[b][i].w), acc[2 * i + 1]);
+      }
+    }
+  }
+  const float a12[12] = {acc[0].x, acc[0].y, acc[1].x, acc[1].y, acc[2].x, acc[2].y, acc[3].x, acc[3].y, acc[4].x, acc[4].y, acc[5].x, acc[5].y};
+#pragma unroll
+  for (int j = 0; j < GC; ++j) cpl[j] += a12[A + j];
+}
+
 // SPC: simulations per CTA (1..8); SMEMTAB: the delay table of the group's speed is staged in shared memory;
 // GCE: ring slots loaded per edge = 2, 4 or 8 >= the chunk length CH of the launched groups (P.group0 ...).
 // CLU: the group is integrated by a thread-block cluster; CTA r of the cluster owns the regions [r*NL, (r+1)*NL), NL =
@@ -180,7 +223,8 @@ __device__ __forceinline__ void gather_rounds(EdgePtr edges, int e, int e1, int 
 // 32-byte sectors of the ring, which a single CTA of <= 480 threads cannot offer at N = 360).
 // blockDim = (regions of the CTA)*SPC rounded up to whole warps (<= K2_MAXT); lanes past the last node replay it,
 // stores suppressed.
-template <int SPC, bool SMEMTAB, int GCE, bool CLU>
+// VEC (with CLU, GCE == 8): quad ring layout and vector gather, see gather_class_vec.
+template <int SPC, bool SMEMTAB, int GCE, bool CLU, bool VEC = false>
 __global__ void __launch_bounds__(K2_MAXT, 1) integrate2_kernel(const __grid_constant__ Integrate2Params P) {
   extern __shared__ __align__(16) unsigned char smem_raw[];
   constexpr int RS = SPC;                         // simulation columns of a ring slot
@@ -221,7 +265,7 @@ __global__ void __launch_bounds__(K2_MAXT, 1) integrate2_kernel(const __grid_con
   const int node = active ? tid : NODES - 1;
   const int kl = node / SPC, sl = node - kl * SPC, k = k0 + kl;
   s_ps += sl;
-  float* const ringg = P.ring + gd.ring_off + sl;   // this group's ring, the thread's simulation column
+  float* const ringg = P.ring + gd.ring_off + (VEC ? 4 * sl : sl);   // this group's ring, the thread's simulation column
   const int e_last = td.n_edges - 1;
   const uint32_t myrow = (uint32_t)(k * Hs) * (uint32_t)RS;
   const int loc = P.loc_id[(size_t)g * SPC + sl];
@@ -252,13 +296,58 @@ __global__ void __launch_bounds__(K2_MAXT, 1) integrate2_kernel(const __grid_con
     if (SMEMTAB) gather_rounds<RS, GCE, CLU>(s_edges, e, pe1, e_last, ringg, cur0, Hp, acc);
     else gather_rounds<RS, GCE, CLU>(g_edges, e, pe1, e_last, ringg, cur0, Hp, acc);
   };
+  // VEC: the row's alignment classes; one class after the other, all edges of the row, for the chunk at slot cur0
+  int4 segk = make_int4(0, 0, 0, 0);
+  if (VEC) segk = *reinterpret_cast<const int4*>(P.seg + td.seg_off + 4 * k);
+  auto gather_vec = [&](int cur0) {                // cur0 a multiple of 4
+    float cpl[GC];
+#pragma unroll
+    for (int j = 0; j < GC; ++j) cpl[j] = 0.0f;
+    const uint32_t thr = (uint32_t)(Hp - cur0), curRS = (uint32_t)cur0 * (uint32_t)RS, wrapRS = (uint32_t)Hp * (uint32_t)RS;
+    gather_class_vec<RS, 0>(g_edges, pe0, segk.x, e_last, ringg, curRS, thr, wrapRS, cpl);
+    gather_class_vec<RS, 1>(g_edges, segk.x, segk.y, e_last, ringg, curRS, thr, wrapRS, cpl);
+    gather_class_vec<RS, 2>(g_edges, segk.y, segk.z, e_last, ringg, curRS, thr, wrapRS, cpl);
+    gather_class_vec<RS, 3>(g_edges, segk.z, segk.w, e_last, ringg, curRS, thr, wrapRS, cpl);
+#pragma unroll
+    for (int j = 0; j < GC; ++j) s_cpl[j * T] = cpl[j];
+  };
+  auto gather_head_vec = [&](int cur0) {           // any alignment (first chunk of a launch): scalar loads, same association
+    float cpl[GC];
+#pragma unroll
+    for (int j = 0; j < GC; ++j) cpl[j] = 0.0f;
+    const int ends[4] = {segk.x, segk.y, segk.z, segk.w};
+    int e = pe0;
+    for (int a = 0; a < 4; ++a) {
+      float acc8[GC];
+#pragma unroll
+      for (int j = 0; j < GC; ++j) acc8[j] = 0.0f;
+      for (; e < ends[a]; ++e) {
+        const Edge<float> ed = g_edges[e];
+        uint32_t s0 = (uint32_t)cur0 + ed.back;
+        if (s0 >= (uint32_t)Hp) s0 -= (uint32_t)Hp;
+#pragma unroll
+        for (int j = 0; j < GC; ++j) {
+          const uint32_t sj = s0 + (uint32_t)j;
+          acc8[j] = __fmaf_rn(ed.w, __ldcg(ringg + ed.jbase + (sj & ~3u) * (uint32_t)RS + (sj & 3u)), acc8[j]);
+        }
+      }
+#pragma unroll
+      for (int j = 0; j < GC; ++j) cpl[j] += acc8[j];
+    }
+#pragma unroll
+    for (int j = 0; j < GC; ++j) s_cpl[j * T] = cpl[j];
+  };
   auto gather_now = [&](int cur0) {
-    f2 acc[GC / 2];
+    if (VEC) {
+      gather_head_vec(cur0);
+    } else {
+      f2 acc[GC / 2];
 #pragma unroll
-    for (int j = 0; j < GC / 2; ++j) acc[j] = mk2(0.0f, 0.0f);
-    gather_from(pe0, cur0, acc);
+      for (int j = 0; j < GC / 2; ++j) acc[j] = mk2(0.0f, 0.0f);
+      gather_from(pe0, cur0, acc);
 #pragma unroll
-    for (int j = 0; j < GC / 2; ++j) { s_cpl[(2 * j) * T] = acc[j].x; s_cpl[(2 * j + 1) * T] = acc[j].y; }
+      for (int j = 0; j < GC / 2; ++j) { s_cpl[(2 * j) * T] = acc[j].x; s_cpl[(2 * j + 1) * T] = acc[j].y; }
+    }
   };
   // S4: Philox (A12): one call per (sim, region) per 4 steps gives the normals of steps 4q .. 4q+3.
   // Long chunks (GCE == 8): the normals of a whole chunk are drawn next to its gather, into s_xi.
@@ -282,7 +371,7 @@ __global__ void __launch_bounds__(K2_MAXT, 1) integrate2_kernel(const __grid_con
   const bool LA = LAG >= 2;
   if (LA && n < P.n_end) {                        // chunk 0 of the launch has no predecessor to hide behind
     gather_now(c);
-    if (GCE == 8 && noise) normals_now(n, (int)min((int64_t)CH, P.n_end - n));
+    if (GCE == 8 && noise) normals_now(n, (int)min((int64_t)(VEC ? CH - (int)(n % CH) : CH), P.n_end - n));
   }
 
   auto wait_chunk = [&](uint32_t w) {              // all warps of the group have written chunk w
@@ -290,7 +379,8 @@ __global__ void __launch_bounds__(K2_MAXT, 1) integrate2_kernel(const __grid_con
     else mbar_wait(bar_done + (w & (NBAR - 1)), (w / NBAR) & 1u);
   };
   for (uint32_t m = 0; n < P.n_end; ++m) {
-    const int ch = (int)min((int64_t)CH, P.n_end - n);
+    // (VEC: a short first chunk brings the chunk starts to multiples of CH = GC, where every window alignment is fixed)
+    const int ch = (int)min((int64_t)(VEC ? CH - (int)(n % CH) : CH), P.n_end - n);
     const bool has_next = n + ch < P.n_end;
     const int cur1 = c + ch >= Hp ? c + ch - Hp : c + ch;          // ring slot of the next chunk's first step
     if (!LA) {                                    // zero minimum delay: gather right before the chunk
@@ -310,7 +400,8 @@ __global__ void __launch_bounds__(K2_MAXT, 1) integrate2_kernel(const __grid_con
       const float cpl = s_cpl[i * T];
       // ---- S1 for the next chunk: issue the loads of the next PVN / GCE edges now, add them below ----
       float pv[PVN];
-      if (SMEMTAB) gather_issue<RS, PVN / GCE, GCE, CLU>(s_edges, pe0 + (PVN / GCE) * i, e_last, ringg, cur1, Hp, pv);   // (a table has >= 1 entry)
+      if (VEC) {}
+      else if (SMEMTAB) gather_issue<RS, PVN / GCE, GCE, CLU>(s_edges, pe0 + (PVN / GCE) * i, e_last, ringg, cur1, Hp, pv);   // (a table has >= 1 entry)
       else gather_issue<RS, PVN / GCE, GCE, CLU>(g_edges, pe0 + (PVN / GCE) * i, e_last, ringg, cur1, Hp, pv);
       // ---- S2 inputs (Eq. 5; A5, A6, A10) ----
       const f2 gw = s_ps[P2_GW * SPC];
@@ -363,14 +454,15 @@ __global__ void __launch_bounds__(K2_MAXT, 1) integrate2_kernel(const __grid_con
         ou = __fmaf_rn(P.ou_rho, ou, __fmaf_rn(P.ou_s, s_quad[((uint32_t)nn & 3u) * T], P.ou_m));
       }
       // ---- S1 for the next chunk: the loads issued above have had the whole step to arrive ----
-      if (SMEMTAB) gather_add<PVN / GCE, GCE>(s_edges, pe0 + (PVN / GCE) * i, pe1, pipe, pv, pacc);
+      if (VEC) {}
+      else if (SMEMTAB) gather_add<PVN / GCE, GCE>(s_edges, pe0 + (PVN / GCE) * i, pe1, pipe, pv, pacc);
       else gather_add<PVN / GCE, GCE>(g_edges, pe0 + (PVN / GCE) * i, pe1, pipe, pv, pacc);
       // ---- S5 ring write: E at time nn+1 (mirror the first GC-1 slots behind the period) ----
       c = c + 1 == Hp ? 0 : c + 1;
       if (active) {
-        const uint32_t o = myrow + (uint32_t)c * (uint32_t)RS;
+        const uint32_t o = VEC ? myrow + ((uint32_t)c & ~3u) * (uint32_t)RS + ((uint32_t)c & 3u) : myrow + (uint32_t)c * (uint32_t)RS;
         ringg[o] = nu.x;
-        if (c < GC - 1) ringg[o + (uint32_t)Hp * (uint32_t)RS] = nu.x;
+        if (c < (VEC ? GC : GC - 1)) ringg[o + (uint32_t)Hp * (uint32_t)RS] = nu.x;
       }
       // ---- trajectory (tests / cfg 1) ----
       if (traj_on && nn - P.traj_n0 < P.traj_steps) {
@@ -390,7 +482,10 @@ __global__ void __launch_bounds__(K2_MAXT, 1) integrate2_kernel(const __grid_con
         win = mk2(0.0f, 0.0f);
       }
     }
-    if (pipe) {       // the row's remaining edges (long rows, short chunks), then chunk m + 1 replaces chunk m
+    if (pipe && VEC) {      // the whole row for chunk m + 1 with vector loads
+      gather_vec(cur1);
+      if (noise) normals_now(n + ch, (int)min((int64_t)CH, P.n_end - (n + ch)));
+    } else if (pipe) {      // the row's remaining edges (long rows, short chunks), then chunk m + 1 replaces chunk m
       gather_from(pe0 + (PVN / GCE) * ch, cur1, pacc);   // (the registers of the transfer function are free here)
       if (GCE == 8 && noise) normals_now(n + ch, (int)min((int64_t)CH, P.n_end - (n + ch)));
 #pragma unroll

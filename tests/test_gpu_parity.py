@@ -165,10 +165,10 @@ def test_cluster_mapping_regions_split_over_ctas(clu, spc):
 
 
 def test_cluster_mapping_is_bitwise_the_single_cta_mapping():
-    """The cluster only changes which CTA owns a region: same per-node arithmetic, same edge order -> the
-    trajectories equal those of the one-CTA mapping bit for bit."""
+    """The cluster (scalar gather: short chunks at v = 40 m/s) only changes which CTA owns a region: same
+    per-node arithmetic, same edge order -> the trajectories equal those of the one-CTA mapping bit for bit."""
     W, L = wl.connectome(37, seed=5, keep=0.35)
-    cfg = dict(axes=[dict(name="G", lo=0.0, hi=0.4, n=5, values=None)], fixed=dict(v=5.0, wNoise=1e-4), seed=4)
+    cfg = dict(axes=[dict(name="G", lo=0.0, hi=0.4, n=5, values=None)], fixed=dict(v=40.0, wNoise=1e-4), seed=4)
     _, a = tvbx.sweep_from_config(cfg, W, L, sims_per_cta=4, ctas_per_group=1)
     _, b = tvbx.sweep_from_config(cfg, W, L, sims_per_cta=4, ctas_per_group=4)
     ta = a.run(900, 0.1, noise_on=True, ds=10, traj_steps=900)
@@ -211,12 +211,15 @@ def test_cfg5_slice_n360():
 
 
 # ------------------------------------------------------------------------------------ invariants on the GPU path
-def test_resumable_bit_exact():
-    """P14: run(a); run(b) == run(a+b) bit for bit (state, OU, FC accumulators)."""
+@pytest.mark.parametrize("kw", [dict(), dict(sims_per_cta=4, ctas_per_group=3)], ids=["one_cta", "cluster_vector_gather"])
+def test_resumable_bit_exact(kw):
+    """P14: run(a); run(b) == run(a+b) bit for bit (state, OU, FC accumulators).  In the cluster form with
+    the vector gather every launch starts with a short unaligned chunk gathered by scalar loads: it has to
+    reproduce the association of the vector path exactly."""
     W, L = wl.connectome(30, seed=3, keep=0.4)
     cfg = dict(axes=[dict(name="G", lo=0.0, hi=0.5, n=6, values=None)], fixed=dict(v=5.0, b_e=30.0, wNoise=1e-4), seed=4)
-    _, a = tvbx.sweep_from_config(cfg, W, L, chunk_samples=16)
-    _, b = tvbx.sweep_from_config(cfg, W, L, chunk_samples=16)
+    _, a = tvbx.sweep_from_config(cfg, W, L, chunk_samples=16, **kw)
+    _, b = tvbx.sweep_from_config(cfg, W, L, chunk_samples=16, **kw)
     a.run(1203, 0.1, noise_on=True, ds=10, discard_steps=95)
     for part in (1, 398, 7, 797):
         b.run(part, 0.1, noise_on=True, ds=10, discard_steps=95)
