@@ -276,6 +276,7 @@ inline Kernel2Fn pick_kernel2_spc(int spc) {
 }
 // cluster form (several CTAs per group): table through L1/L2, 8 slots per edge; vec: quad ring layout + vector gather
 inline Kernel2Fn pick_kernel2(int spc, bool smemtab, int gce, bool clu, bool vec) {
+  if (clu && vec && smemtab) return spc == 8 ? integrate2_kernel<8, true, 8, true, true> : integrate2_kernel<4, true, 8, true, true>;
   if (clu && vec) return spc == 8 ? integrate2_kernel<8, false, 8, true, true> : integrate2_kernel<4, false, 8, true, true>;
   if (clu) return pick_kernel2_spc<false, 8, true>(spc);
   if (!smemtab) return pick_kernel2_spc<false, 8>(spc);
@@ -301,7 +302,7 @@ struct DeviceImpl : DeviceSide {
   DevBuf<float2> d_psim2;
   int threads = 0, smem = 0;
   bool single = true;
-  size_t ring_count = 0;
+  size_t ring_count = 0, max_slice_edges = 0;
 
   explicit DeviceImpl(tvbx_sweep* s) : sw(s) { std::memset(&P, 0, sizeof P); std::memset(&P2, 0, sizeof P2); }
 
@@ -319,6 +320,7 @@ struct DeviceImpl : DeviceSide {
     std::vector<TableDesc> tds(sw->tables.size());
     std::vector<Edge<R>> edges;
     std::vector<int32_t> rowptr, seg;
+    max_slice_edges = 0;
     for (size_t t = 0; t < sw->tables.size(); ++t) {
       HostTable& ht = sw->tables[t];
       ht.delays.clear();
@@ -344,6 +346,7 @@ struct DeviceImpl : DeviceSide {
         const int r0 = c.rowptr[k], r1 = c.rowptr[k + 1];
         if (rg.vec) {      // quad layout: the row sorted by window alignment class a = (Hp - d) mod 4, ascending j inside
           for (int a = 0; a < 4; ++a) {
+            int n_class = 0;
             for (int e = r0; e < r1; ++e) {
               const uint32_t back = (uint32_t)(ht.Hp - ht.delays[e]);
               if ((int)(back & 3u) != a) continue;
@@ -353,6 +356,12 @@ struct DeviceImpl : DeviceSide {
               ed.jbase = (uint32_t)c.edges[e].j * (uint32_t)Hs * (uint32_t)RS;
               ed.back = back;
               set_pad(ed, ed.jbase + (back & ~3u) * (uint32_t)RS);
+              edges.push_back(ed);
+              ++n_class;
+            }
+            for (; n_class % VR != 0; ++n_class) {      // whole rounds: zero-weight copies of the class's last edge
+              Edge<R> ed = edges.back();
+              ed.w = R(0);
               edges.push_back(ed);
             }
             seg.push_back((int32_t)(edges.size() - (size_t)tds[t].edge_off));
@@ -371,14 +380,20 @@ struct DeviceImpl : DeviceSide {
         }
       }
       rowptr.push_back((int32_t)(edges.size() - (size_t)tds[t].edge_off));
-      if (edges.size() == (size_t)tds[t].edge_off) {      // a table is never empty: one zero-weight entry that no row owns
+      {      // a table (and any run of its rows) is never empty: one zero-weight entry at the end that no row owns
         Edge<R> ed;
         std::memset(&ed, 0, sizeof ed);
-        ed.back = 1;
-        set_pad(ed, (uint32_t)RS);
+        ed.back = rg.vec ? 4u : 1u;
+        set_pad(ed, ed.back * (uint32_t)RS);
         edges.push_back(ed);
       }
       tds[t].n_edges = (int32_t)(edges.size() - (size_t)tds[t].edge_off);
+      {      // cluster form: the largest run of rows one CTA stages in shared memory
+        const int NLc = (N + sw->clu - 1) / sw->clu;
+        const int32_t* rp = rowptr.data() + tds[t].rowptr_off;
+        for (int r = 0; r * NLc < N; ++r)
+          max_slice_edges = std::max<size_t>(max_slice_edges, (size_t)(rp[std::min(N, (r + 1) * NLc)] - rp[r * NLc] + 1));
+      }
     }
     // ---- groups ----
     std::vector<GroupDesc> gds(G);
@@ -540,8 +555,16 @@ struct DeviceImpl : DeviceSide {
     threads = (NL * SPC + 31) / 32 * 32;
     single = true;
     const size_t base = (size_t)NBAR * 8 + (size_t)2 * GC * threads * sizeof(float) + (size_t)NP2 * SPC * sizeof(float2) + 16;
-    P2.smem_table = CLU == 1 && base + tbytes <= 200 * 1024;
-    smem = (int)(base + (P2.smem_table ? tbytes : 0));
+    // cluster form: the vector-gather kernels stage the rows of the CTA's regions as 8-byte entries; the scalar
+    // cluster kernels read the table through L1/L2
+    const size_t slice_bytes = max_slice_edges * sizeof(Edge8);
+    // (at most ~half of the SM's 256 KB: the L1 is the landing space of the ring loads in flight -- 15 warps x 15
+    // LDG.128 = 115 KB; measured at N = 360: 212 KB of shared memory halves the throughput)
+    bool clu_tab = CLU > 1 && base + slice_bytes <= (size_t)136 * 1024;
+    for (const HostTable& ht : sw->tables)      // field widths of Edge8
+      if (ht.vec && ((int64_t)N * ((ht.Hp + GC) / 4) >= (1 << 20) || ht.Hp / 4 >= (1 << 12))) clu_tab = false;
+    P2.smem_table = CLU == 1 ? base + tbytes <= 200 * 1024 : clu_tab;
+    smem = (int)(base + (CLU == 1 ? (P2.smem_table ? tbytes : 0) : (clu_tab ? slice_bytes : 0)));
     // one launch per run of groups whose chunk length falls in the same class (cfg 3: v <= 8 / 16 / >= 32 m/s)
     launches2.clear();
     cudaFuncAttributes fa;

@@ -107,22 +107,30 @@ __device__ __forceinline__ uint32_t cluster_nctarank() { uint32_t r; asm volatil
 __device__ __forceinline__ void cluster_sync_all() {
   asm volatile("barrier.cluster.arrive.release.aligned;\n\tbarrier.cluster.wait.acquire.aligned;" ::: "memory");
 }
+// one release fence, then a relaxed arrive per CTA of the cluster (fence + relaxed write = release pattern)
 __device__ __forceinline__ void mbar_arrive_cluster(uint64_t* bar, uint32_t nrank) {
   const uint32_t local = smem_u32(bar);
+  asm volatile("fence.acq_rel.cluster;" ::: "memory");
   for (uint32_t r = 0; r < nrank; ++r) {
     uint32_t remote;
     asm volatile("mapa.shared::cluster.u32 %0, %1, %2;" : "=r"(remote) : "r"(local), "r"(r));
-    asm volatile("mbarrier.arrive.release.cluster.shared::cluster.b64 _, [%0];" ::"r"(remote) : "memory");
+    asm volatile("mbarrier.arrive.relaxed.cluster.shared::cluster.b64 _, [%0];" ::"r"(remote) : "memory");
   }
 }
+// spin relaxed, then observe the completed phase once with acquire semantics (the acquire form invalidates the
+// L1 -- CCTL.IVALL -- on every poll)
 __device__ __forceinline__ void mbar_wait_cluster(uint64_t* bar, uint32_t parity) {
   asm volatile(
       "{\n"
       ".reg .pred p;\n"
       "WAITC_%=:\n"
+      "mbarrier.try_wait.parity.relaxed.cluster.shared::cta.b64 p, [%0], %1;\n"
+      "@p bra ACQC_%=;\n"
+      "bra WAITC_%=;\n"
+      "ACQC_%=:\n"
       "mbarrier.try_wait.parity.acquire.cluster.shared::cta.b64 p, [%0], %1;\n"
       "@p bra DONEC_%=;\n"
-      "bra WAITC_%=;\n"
+      "bra ACQC_%=;\n"
       "DONEC_%=:\n"
       "}\n" ::"r"(smem_u32(bar)), "r"(parity)
       : "memory");
@@ -184,36 +192,76 @@ __device__ __forceinline__ void gather_rounds(EdgePtr edges, int e, int e1, int 
 // of a class are accumulated UNSHIFTED over the 12 fetched slots and folded once per class,
 // cpl[j] += acc[a + j] -- no per-edge select.  Per slot the association is: classes 0..3 in order, inside a class
 // the row's edges in ascending j (gather_head_vec reproduces it for the unaligned first chunk of a launch).
+// The host pads every class of a row to a multiple of VR entries with zero-weight copies of its last edge, so a
+// round needs neither an index clamp nor a weight mask.  Class 0 windows are quad-aligned: two quads suffice.
 enum { VR = 5 };                 // edges per round of the vector gather (VR x 12 values in registers)
-template <int RS, int A>
-__device__ __forceinline__ void gather_class_vec(const Edge<float>* edges, int e, int e1, int e_last, const float* ringv,
+template <int RS, int A, typename EdgePtr>
+__device__ __forceinline__ void gather_class_vec(EdgePtr edges, int e, int e1, const float* ringv,
                                                  uint32_t curRS, uint32_t thr, uint32_t wrapRS, float cpl[GC]) {
-  f2 acc[6];
+  constexpr int NQ = A == 0 ? 2 : 3;
+  f2 acc[2 * NQ];
 #pragma unroll
-  for (int i = 0; i < 6; ++i) acc[i] = mk2(0.0f, 0.0f);
+  for (int i = 0; i < 2 * NQ; ++i) acc[i] = mk2(0.0f, 0.0f);
+  const uint32_t curW = curRS - wrapRS;
   for (; e < e1; e += VR) {
-    float4 q[VR][3];
+    float4 q[VR][NQ];
     float w[VR];
 #pragma unroll
     for (int b = 0; b < VR; ++b) {
-      const Edge<float> ed = edges[min(e + b, e_last)];
-      const uint32_t off = ed.pad + curRS - (ed.back >= thr ? wrapRS : 0u);
+      const Edge<float> ed = edges[e + b];
+      const uint32_t off = ed.pad + (ed.back >= thr ? curW : curRS);
       const float4* src = reinterpret_cast<const float4*>(ringv + off);
-      q[b][0] = __ldcg(src); q[b][1] = __ldcg(src + RS); q[b][2] = __ldcg(src + 2 * RS);
-      w[b] = e + b < e1 ? ed.w : 0.0f;
+#pragma unroll
+      for (int i = 0; i < NQ; ++i) q[b][i] = __ldcg(src + i * RS);
+      w[b] = ed.w;
     }
 #pragma unroll
     for (int b = 0; b < VR; ++b) {
 #pragma unroll
-      for (int i = 0; i < 3; ++i) {
+      for (int i = 0; i < NQ; ++i) {
         acc[2 * i] = fma2(bc2(w[b]), mk2(q[b][i].x, q[b][i].y), acc[2 * i]);
         acc[2 * i + 1] = fma2(bc2(w[b]), mk2(q[b][i].z, q[b][i].w), acc[2 * i + 1]);
       }
     }
   }
-  const float a12[12] = {acc[0].x, acc[0].y, acc[1].x, acc[1].y, acc[2].x, acc[2].y, acc[3].x, acc[3].y, acc[4].x, acc[4].y, acc[5].x, acc[5].y};
 #pragma unroll
-  for (int j = 0; j < GC; ++j) cpl[j] += a12[A + j];
+  for (int j = 0; j < GC; ++j) { const int i = A + j; cpl[j] += (i & 1) ? acc[i >> 1].y : acc[i >> 1].x; }
+}
+
+// The same with the 8-byte entries the vector kernels stage in shared memory (Edge8: w and, in one word, the
+// quad-slot index Q = j * Hs/4 + (Hp - d)/4 in the low 20 bits and (Hp - d)/4 in the high 12): half the shared
+// memory of the 16-byte entries, which leaves the L1 the room it needs as landing space for the loads in flight.
+struct __align__(8) Edge8 { float w; uint32_t qb; };
+template <int RS, int A>
+__device__ __forceinline__ void gather_class_vec8(const Edge8* edges, int e, int e1, const float4* ring4,
+                                                  uint32_t cur4, uint32_t thr4, uint32_t curW4, float cpl[GC]) {
+  constexpr int NQ = A == 0 ? 2 : 3;
+  f2 acc[2 * NQ];
+#pragma unroll
+  for (int i = 0; i < 2 * NQ; ++i) acc[i] = mk2(0.0f, 0.0f);
+  for (; e < e1; e += VR) {
+    float4 q[VR][NQ];
+    float w[VR];
+#pragma unroll
+    for (int b = 0; b < VR; ++b) {
+      const Edge8 ed = edges[e + b];
+      const uint32_t idx = (ed.qb & 0xFFFFFu) + ((ed.qb >> 20) >= thr4 ? curW4 : cur4);
+      const float4* src = ring4 + (size_t)idx * RS;
+#pragma unroll
+      for (int i = 0; i < NQ; ++i) q[b][i] = __ldcg(src + i * RS);
+      w[b] = ed.w;
+    }
+#pragma unroll
+    for (int b = 0; b < VR; ++b) {
+#pragma unroll
+      for (int i = 0; i < NQ; ++i) {
+        acc[2 * i] = fma2(bc2(w[b]), mk2(q[b][i].x, q[b][i].y), acc[2 * i]);
+        acc[2 * i + 1] = fma2(bc2(w[b]), mk2(q[b][i].z, q[b][i].w), acc[2 * i + 1]);
+      }
+    }
+  }
+#pragma unroll
+  for (int j = 0; j < GC; ++j) { const int i = A + j; cpl[j] += (i & 1) ? acc[i >> 1].y : acc[i >> 1].x; }
 }
 
 // SPC: simulations per CTA (1..8); SMEMTAB: the delay table of the group's speed is staged in shared memory;
@@ -247,16 +295,31 @@ __global__ void __launch_bounds__(K2_MAXT, 1) integrate2_kernel(const __grid_con
   float2* s_ps = reinterpret_cast<float2*>(reinterpret_cast<float*>(smem_raw + NBAR * 8) + (size_t)2 * GC * T);
   unsigned char* tab = reinterpret_cast<unsigned char*>(s_ps + NP2 * SPC);
   tab += (16 - (reinterpret_cast<uintptr_t>(tab) & 15)) & 15;
-  Edge<float>* const s_edges = reinterpret_cast<Edge<float>*>(tab);
-  int32_t* const s_rowptr = reinterpret_cast<int32_t*>(s_edges + td.n_edges);
-  const Edge<float>* const g_edges = P.edges + td.edge_off;
+  // the CTA's part of the delay table: all of it, or (CLU) the rows of its regions; edge indices below are relative
+  // to rp0.  (Every table ends with one zero-weight entry that no row owns: a part is never empty.)
   const int32_t* const g_rowptr = P.rowptr + td.rowptr_off;
+  const int rp0 = CLU ? g_rowptr[k0] : 0;
+  const int n_stage = CLU ? g_rowptr[min(k0 + NL, N)] - rp0 + 1 : td.n_edges;
+  Edge<float>* const s_edges = reinterpret_cast<Edge<float>*>(tab);
+  Edge8* const s_edges8 = reinterpret_cast<Edge8*>(tab);           // (VEC: 8-byte entries instead)
+  int32_t* const s_rowptr = reinterpret_cast<int32_t*>(s_edges + n_stage);
+  const Edge<float>* const g_edges = P.edges + td.edge_off + rp0;
   {
     if (tid < NBAR) mbar_init(bar_done + tid, (uint32_t)(T >> 5) * nrank);
     for (int i = tid; i < NP2 * SPC; i += T) s_ps[i] = P.psim2[(size_t)g * NP2 * SPC + i];
     if (SMEMTAB) {
-      for (int i = tid; i < td.n_edges; i += T) s_edges[i] = g_edges[i];
-      for (int i = tid; i <= N; i += T) s_rowptr[i] = g_rowptr[i];
+      if (VEC) {
+        const uint32_t qdiv = 4u * (uint32_t)RS;
+        for (int i = tid; i < n_stage; i += T) {
+          const Edge<float> ed = g_edges[i];
+          Edge8 e8;
+          e8.w = ed.w; e8.qb = (ed.pad / qdiv) | ((ed.back >> 2) << 20);
+          s_edges8[i] = e8;
+        }
+      } else {
+        for (int i = tid; i < n_stage; i += T) s_edges[i] = g_edges[i];
+      }
+      if (!CLU) for (int i = tid; i <= N; i += T) s_rowptr[i] = g_rowptr[i];
     }
     if (CLU) cluster_sync_all(); else __syncthreads();      // (remote arrivals need the peers' barriers initialised)
   }
@@ -266,14 +329,14 @@ __global__ void __launch_bounds__(K2_MAXT, 1) integrate2_kernel(const __grid_con
   const int kl = node / SPC, sl = node - kl * SPC, k = k0 + kl;
   s_ps += sl;
   float* const ringg = P.ring + gd.ring_off + (VEC ? 4 * sl : sl);   // this group's ring, the thread's simulation column
-  const int e_last = td.n_edges - 1;
+  const int e_last = n_stage - 1;
   const uint32_t myrow = (uint32_t)(k * Hs) * (uint32_t)RS;
   const int loc = P.loc_id[(size_t)g * SPC + sl];
   const uint32_t ext = (uint32_t)P.ext_id[(size_t)g * SPC + sl];
   const float dt = P.dt;
   const float inv_ds = P.ds > 0 ? 1.0f / (float)P.ds : 0.0f;
   const f2 invN = mk2(P.inv_Ne, P.inv_Ni);
-  const int pe0 = SMEMTAB ? s_rowptr[k] : g_rowptr[k], pe1 = SMEMTAB ? s_rowptr[k + 1] : g_rowptr[k + 1];   // this node's row
+  const int pe0 = (SMEMTAB && !CLU ? s_rowptr[k] : g_rowptr[k]) - rp0, pe1 = (SMEMTAB && !CLU ? s_rowptr[k + 1] : g_rowptr[k + 1]) - rp0;   // this node's row
 
   // ---- state of this (sim, region) in registers: nu = (E, I), Cs = (C_ee, C_ii), W = (W_e, W_i) ----
   f2 nu, Cs, W, win;
@@ -298,16 +361,28 @@ __global__ void __launch_bounds__(K2_MAXT, 1) integrate2_kernel(const __grid_con
   };
   // VEC: the row's alignment classes; one class after the other, all edges of the row, for the chunk at slot cur0
   int4 segk = make_int4(0, 0, 0, 0);
-  if (VEC) segk = *reinterpret_cast<const int4*>(P.seg + td.seg_off + 4 * k);
+  if (VEC) {
+    segk = *reinterpret_cast<const int4*>(P.seg + td.seg_off + 4 * k);
+    segk.x -= rp0; segk.y -= rp0; segk.z -= rp0; segk.w -= rp0;
+  }
   auto gather_vec = [&](int cur0) {                // cur0 a multiple of 4
     float cpl[GC];
 #pragma unroll
     for (int j = 0; j < GC; ++j) cpl[j] = 0.0f;
     const uint32_t thr = (uint32_t)(Hp - cur0), curRS = (uint32_t)cur0 * (uint32_t)RS, wrapRS = (uint32_t)Hp * (uint32_t)RS;
-    gather_class_vec<RS, 0>(g_edges, pe0, segk.x, e_last, ringg, curRS, thr, wrapRS, cpl);
-    gather_class_vec<RS, 1>(g_edges, segk.x, segk.y, e_last, ringg, curRS, thr, wrapRS, cpl);
-    gather_class_vec<RS, 2>(g_edges, segk.y, segk.z, e_last, ringg, curRS, thr, wrapRS, cpl);
-    gather_class_vec<RS, 3>(g_edges, segk.z, segk.w, e_last, ringg, curRS, thr, wrapRS, cpl);
+    if (SMEMTAB) {
+      const float4* const ring4 = reinterpret_cast<const float4*>(ringg);
+      const uint32_t cur4 = (uint32_t)cur0 >> 2, thr4 = thr >> 2, curW4 = cur4 - ((uint32_t)Hp >> 2);
+      gather_class_vec8<RS, 0>(s_edges8, pe0, segk.x, ring4, cur4, thr4, curW4, cpl);
+      gather_class_vec8<RS, 1>(s_edges8, segk.x, segk.y, ring4, cur4, thr4, curW4, cpl);
+      gather_class_vec8<RS, 2>(s_edges8, segk.y, segk.z, ring4, cur4, thr4, curW4, cpl);
+      gather_class_vec8<RS, 3>(s_edges8, segk.z, segk.w, ring4, cur4, thr4, curW4, cpl);
+    } else {
+      gather_class_vec<RS, 0>(g_edges, pe0, segk.x, ringg, curRS, thr, wrapRS, cpl);
+      gather_class_vec<RS, 1>(g_edges, segk.x, segk.y, ringg, curRS, thr, wrapRS, cpl);
+      gather_class_vec<RS, 2>(g_edges, segk.y, segk.z, ringg, curRS, thr, wrapRS, cpl);
+      gather_class_vec<RS, 3>(g_edges, segk.z, segk.w, ringg, curRS, thr, wrapRS, cpl);
+    }
 #pragma unroll
     for (int j = 0; j < GC; ++j) s_cpl[j * T] = cpl[j];
   };
