@@ -97,7 +97,9 @@ def test_delay_indices_and_ring_lengths_bit_exact(i):
         H, Hp = sw.ring_len(s, dt)
         D, dmin = ref_kept.max(), ref_kept[ref_kept >= 0].min()
         assert H == D + 1
-        assert H + 1 <= Hp <= H + dmin + 1  # the kernel's ring also holds the steps the fastest warp may be ahead (<= min delay + 1)
+        # the kernel's ring also holds the steps the fastest warp may be ahead (<= min delay + 1); the cluster
+        # form's quad ring layout rounds the period up to a multiple of 4
+        assert H + 1 <= Hp <= H + dmin + 1 + 3
 
 
 def test_half_to_even_rounding():
