@@ -95,7 +95,14 @@ typedef struct tvbx_sweep_opts {
   int32_t ctas_per_group; /* 0 = choose; else 1..8: CTAs (one thread-block cluster) that share the regions of a group of
                              sims_per_cta simulations -- lets N = 360 run 8 simulations per group (6 CTAs x 60 regions);
                              packed FP32 kernel only */
+  int32_t fc_mode;        /* co-moment X^T X of the FC epilogue (S7 / S7'): TVBX_FC_AUTO = tensor cores
+                             (tcgen05 kind::tf32, samples centred in FP32 before rounding to TF32, FP32 accumulate,
+                             FP64 merge) for FP32 sweeps with N <= 512, else FP32/FP64 register tiles;
+                             TVBX_FC_FP32 = register tiles always; TVBX_FC_TF32 = tensor cores or TVBX_EINVAL */
+  int32_t reserved;
 } tvbx_sweep_opts;
+
+enum tvbx_fc_mode { TVBX_FC_AUTO = 0, TVBX_FC_FP32 = 1, TVBX_FC_TF32 = 2 };
 
 typedef struct tvbx_run_opts {
   int32_t noise_on;       /* 0: deterministic, OU neither used nor advanced; 1: Philox OU noise (A11, A12) */
@@ -187,6 +194,9 @@ int32_t tvbx_launch_info(const tvbx_sweep* sw, int32_t info[9]);
  * product kernel (tau_e == tau_i, N * sims_per_cta <= 480, sims_per_cta <= 8), "tvbx::integrate_kernel" = the
  * general one (FP64 build mode, tau_e != tau_i, larger CTAs).  Copies at most n bytes including the NUL. */
 int32_t tvbx_kernel_name(const tvbx_sweep* sw, char* buf, int32_t n);
+/* Which kernel forms the co-moment X^T X of the FC epilogue: "tvbx::fc_xtx_tc_kernel" (tcgen05 kind::tf32, S7') or
+ * "tvbx::fc_comoment_kernel" (FP32/FP64 register tiles, S7); see tvbx_sweep_opts.fc_mode. */
+int32_t tvbx_fc_kernel_name(const tvbx_sweep* sw, char* buf, int32_t n);
 /* number of kernel launches enqueued by this sweep object so far */
 int32_t tvbx_launch_count(const tvbx_sweep* sw, int64_t* n);
 

@@ -4,4 +4,4 @@ The product is the C-ABI library `libtvbx.so` (include/tvbx.h; sources in csrc/)
 its thin Python binding.  See DESIGN.md.
 """
 from .binding import (Connectome, Sweep, TvbxError, build, default_params, lib, sweep_from_config,  # noqa: F401
-                      PARAM_IDS, N_PARAMS, TVBX_F32, TVBX_F64, LIB_PATH, EXPORTS)
+                      PARAM_IDS, N_PARAMS, TVBX_F32, TVBX_F64, TVBX_FC_AUTO, TVBX_FC_FP32, TVBX_FC_TF32, LIB_PATH, EXPORTS)

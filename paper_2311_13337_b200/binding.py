@@ -22,6 +22,7 @@ NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", 
 
 TVBX_OK, TVBX_EINVAL, TVBX_ENOMEM, TVBX_ECUDA, TVBX_ESTATE = 0, -1, -2, -3, -4
 TVBX_F32, TVBX_F64 = 0, 1
+TVBX_FC_AUTO, TVBX_FC_FP32, TVBX_FC_TF32 = 0, 1, 2   # tvbx_sweep_opts.fc_mode
 
 # parameter ids (include/tvbx.h enum tvbx_param_id)
 PARAM_IDS = dict(
@@ -50,7 +51,8 @@ class Axis(C.Structure):
 class SweepOpts(C.Structure):
     _fields_ = [("precision", C.c_int32), ("sims_per_cta", C.c_int32), ("n_sims", C.c_int64),
                 ("sim_ids", C.POINTER(C.c_int64)), ("chunk_samples", C.c_int64),
-                ("threads_per_cta", C.c_int32), ("ctas_per_group", C.c_int32)]
+                ("threads_per_cta", C.c_int32), ("ctas_per_group", C.c_int32),
+                ("fc_mode", C.c_int32), ("reserved", C.c_int32)]
 
 
 class RunOpts(C.Structure):
@@ -63,7 +65,7 @@ EXPORTS = [
     "tvbx_default_params", "tvbx_create_connectome", "tvbx_destroy_connectome", "tvbx_sweep_create",
     "tvbx_sweep_destroy", "tvbx_sweep_set_initial", "tvbx_run", "tvbx_fc_readout", "tvbx_sweep_size",
     "tvbx_sweep_param", "tvbx_sweep_ext_id", "tvbx_delay_index", "tvbx_ring_len", "tvbx_steps_done",
-    "tvbx_samples_kept", "tvbx_sweep_state", "tvbx_launch_info", "tvbx_launch_count", "tvbx_kernel_name", "tvbx_last_error",
+    "tvbx_samples_kept", "tvbx_sweep_state", "tvbx_launch_info", "tvbx_launch_count", "tvbx_kernel_name", "tvbx_fc_kernel_name", "tvbx_last_error",
     "tvbx_version", "tvbx_sweep_reset", "tvbx_profile_enable", "tvbx_profile_read", "tvbx_bytes_copied",
 ]
 
@@ -114,6 +116,7 @@ def lib():
             "tvbx_launch_info": [vp, C.POINTER(i32)],
             "tvbx_launch_count": [vp, C.POINTER(i64)],
             "tvbx_kernel_name": [vp, C.c_char_p, i32],
+            "tvbx_fc_kernel_name": [vp, C.c_char_p, i32],
             "tvbx_sweep_reset": [vp, vp],
             "tvbx_profile_enable": [vp, i32],
             "tvbx_profile_read": [vp, dp, C.POINTER(i64)],
@@ -171,7 +174,7 @@ class Sweep:
     """
 
     def __init__(self, conn: Connectome, axes, seed=0, params=None, precision=TVBX_F32, sims_per_cta=0,
-                 sim_ids=None, chunk_samples=0, threads_per_cta=0, init=None, ctas_per_group=0):
+                 sim_ids=None, chunk_samples=0, threads_per_cta=0, init=None, ctas_per_group=0, fc_mode=0):
         L = lib()
         self.conn = conn
         m = ModelParams()
@@ -201,7 +204,7 @@ class Sweep:
                 ax[i].values = _dptr(arr)
         o = SweepOpts()
         o.precision = precision; o.sims_per_cta = sims_per_cta; o.chunk_samples = chunk_samples
-        o.threads_per_cta = threads_per_cta; o.ctas_per_group = ctas_per_group
+        o.threads_per_cta = threads_per_cta; o.ctas_per_group = ctas_per_group; o.fc_mode = fc_mode
         if sim_ids is not None:
             ids = np.ascontiguousarray(sim_ids, dtype=np.int64)
             keep.append(ids)
@@ -330,6 +333,11 @@ class Sweep:
     def kernel_name(self):
         buf = C.create_string_buffer(64)
         _chk(lib().tvbx_kernel_name(self._h, buf, 64))
+        return buf.value.decode()
+
+    def fc_kernel_name(self):
+        buf = C.create_string_buffer(64)
+        _chk(lib().tvbx_fc_kernel_name(self._h, buf, 64))
         return buf.value.decode()
 
     def launch_count(self):

@@ -15,9 +15,11 @@
 #include <memory>
 #include <new>
 #include <string>
+#include <type_traits>
 #include <vector>
 
 #include "tvbx_fc.cuh"
+#include "tvbx_fc_tc.cuh"
 #include "tvbx_integrate.cuh"
 #include "tvbx_integrate2.cuh"
 
@@ -145,6 +147,7 @@ struct tvbx_sweep {
   bool vec_ok = false;    // cluster form with 4 or 8 simulations per group: vector gather where the chunk length allows
   bool packed = false;               // FP32 closed-form product kernel (integrate2_kernel)
   int64_t chunk_req = 0;
+  bool fc_tc = false;                // FC co-moment on the tensor cores (tvbx_fc_tc.cuh)
   double init[7] = {0.001, 0.001, 0, 0, 0, 0, 0};
   // grouping
   std::vector<HostTable> tables;
@@ -292,6 +295,8 @@ struct DeviceImpl : DeviceSide {
   DevBuf<Edge<R>> d_edges;
   DevBuf<int32_t> d_rowptr, d_seg, d_ext, d_loc;
   DevBuf<R> d_psim, d_ring, d_state, d_xbar;
+  DevBuf<float> d_xc;                 // centred TF32 samples of the chunk, K-major (fc_tc)
+  int64_t Kp = 0;
   DevBuf<double> d_sums, d_cmean, d_mean, d_M, d_M_scratch, d_mean_scratch;
   DevBuf<float> d_out_fc, d_out_me, d_out_mi;
   IntegrateParams<R> P;
@@ -438,7 +443,8 @@ struct DeviceImpl : DeviceSide {
       CS = (int64_t)(budget / std::max<size_t>(1, (size_t)G * row * sizeof(R)));
       CS = std::min<int64_t>(std::max<int64_t>(CS, 16), 4096);
     }
-    const size_t need = ring_elems * sizeof(R) + (size_t)G * CS * row * sizeof(R) +
+    Kp = (CS + tvbx::TC_BK - 1) / tvbx::TC_BK * tvbx::TC_BK;
+    const size_t need = ring_elems * sizeof(R) + (size_t)G * CS * row * sizeof(R) + (sw->fc_tc ? (size_t)G * Kp * row * sizeof(float) : 0) +
                         (size_t)G * SPC * N * N * sizeof(double) * 2 + (size_t)G * 16 * row * sizeof(double);
     if (need > free_b)
       return fail(TVBX_ENOMEM, "sweep needs %.2f GB of device memory (ring %.2f GB), %.2f GB free",
@@ -452,6 +458,7 @@ struct DeviceImpl : DeviceSide {
     if (sw->packed) CU(d_psim2.upload(psim2, hb));
     CU(d_ring.alloc(ring_elems));
     CU(d_xbar.alloc((size_t)G * CS * row));
+    if (sw->fc_tc) CU(d_xc.alloc((size_t)G * Kp * row));
     CU(d_cmean.alloc((size_t)G * row)); CU(d_mean.alloc((size_t)G * row));
     CU(d_M.alloc((size_t)G * SPC * N * N));
     CU(d_state.alloc((size_t)G * (NSV - 2) * row));
@@ -603,6 +610,31 @@ struct DeviceImpl : DeviceSide {
     return TVBX_OK;
   }
 
+  // S7': centre + pack to K-major TF32, then the batched X^T X on tcgen05 with the FP64 Chan merge as epilogue
+  int32_t comoment_tc(const FcParams<R>& F, cudaStream_t st) {
+    if constexpr (std::is_same<R, float>::value) {
+      FcTcParams T;
+      T.xbar = F.xbar; T.xc = d_xc.p; T.cmean = F.cmean; T.mean = F.mean; T.M = F.M; T.cnt = F.cnt;
+      T.n_c = F.n_c; T.CS = F.CS; T.Kp = (int32_t)Kp; T.N = F.N; T.SPC = F.SPC; T.G = F.G;
+      T.Rt = (F.N + 127) / 128 * 128; T.Np = (F.N + 15) / 16 * 16;
+      T.tmem_cols = 32;
+      while (T.tmem_cols < T.Np) T.tmem_cols *= 2;
+      const size_t smem_tc = tc_smem_bytes(T.Rt, T.Np);
+      if (!tc_attr_set) {
+        CU(cudaFuncSetAttribute(fc_xtx_tc_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_tc));
+        tc_attr_set = true;
+      }
+      dim3 gp((F.N * F.SPC + 31) / 32, (F.n_c + 31) / 32, F.G);
+      fc_pack_tf32_kernel<<<gp, dim3(32, 8), 0, st>>>(T);
+      dim3 gx(T.Rt / 128, F.G * F.SPC);
+      fc_xtx_tc_kernel<<<gx, TC_THREADS, smem_tc, st>>>(T);
+      return TVBX_OK;
+    } else {
+      return fail(TVBX_EINVAL, "tensor-core FC needs an FP32 sweep");
+    }
+  }
+  bool tc_attr_set = false;
+
   int32_t accumulate(double* Mbuf, double* meanbuf, int64_t cnt, int n_c, cudaStream_t st) {
     const int N = sw->conn.n, SPC = sw->spc, G = (int)sw->groups.size();
     FcParams<R> F;
@@ -612,12 +644,17 @@ struct DeviceImpl : DeviceSide {
     dim3 g1((row + 127) / 128, G), g0((row + 31) / 32, G);
     sw->prof_begin(K_FC, st);
     fc_chunk_mean_kernel<R><<<g0, 1024, 0, st>>>(F);
-    const int nt = (N + 31) / 32;
-    dim3 g2(nt, nt, G * SPC);
-    fc_comoment_kernel<R><<<g2, 64, 0, st>>>(F);
+    if (sw->fc_tc) {
+      int32_t rc = comoment_tc(F, st);
+      if (rc) return rc;
+    } else {
+      const int nt = (N + 31) / 32;
+      dim3 g2(nt, nt, G * SPC);
+      fc_comoment_kernel<R><<<g2, 64, 0, st>>>(F);
+    }
     fc_mean_update_kernel<R><<<g1, 128, 0, st>>>(F);
     sw->prof_end(st);
-    sw->launches += 3;
+    sw->launches += sw->fc_tc ? 4 : 3;
     CU(cudaGetLastError());
     return TVBX_OK;
   }
@@ -831,6 +868,14 @@ int32_t tvbx_sweep_create(const tvbx_connectome* c, const tvbx_model_params* def
   if (sw->precision != TVBX_F32 && sw->precision != TVBX_F64) return fail(TVBX_EINVAL, "precision=%d", sw->precision);
   sw->threads_req = opts ? opts->threads_per_cta : 0;
   sw->chunk_req = opts ? opts->chunk_samples : 0;
+  {
+    int fcm = opts ? opts->fc_mode : TVBX_FC_AUTO;
+    if (const char* e = getenv("TVBX_FC_MODE")) if (fcm == TVBX_FC_AUTO) fcm = atoi(e);
+    const bool tc_ok = sw->precision == TVBX_F32 && sw->conn.n <= tvbx::TC_MAXN;
+    if (fcm < TVBX_FC_AUTO || fcm > TVBX_FC_TF32) return fail(TVBX_EINVAL, "fc_mode=%d", fcm);
+    if (fcm == TVBX_FC_TF32 && !tc_ok) return fail(TVBX_EINVAL, "fc_mode TVBX_FC_TF32 needs an FP32 sweep with N <= %d", tvbx::TC_MAXN);
+    sw->fc_tc = tc_ok && fcm != TVBX_FC_FP32;
+  }
   // parameter sanity
   for (int64_t s = 0; s < sw->n_sims; ++s) {
     if (!(sw->param(s, TVBX_P_V) > 0.0)) return fail(TVBX_EINVAL, "speed v must be > 0 (sim %lld)", (long long)s);
@@ -1066,6 +1111,11 @@ int32_t tvbx_launch_info(const tvbx_sweep* sw, int32_t info[9]) {
 int32_t tvbx_kernel_name(const tvbx_sweep* sw, char* buf, int32_t n) {
   if (!sw || !buf || n < 1) return fail(TVBX_EINVAL, "bad argument");
   snprintf(buf, (size_t)n, "%s", sw->packed ? "tvbx::integrate2_kernel" : "tvbx::integrate_kernel");
+  return TVBX_OK;
+}
+int32_t tvbx_fc_kernel_name(const tvbx_sweep* sw, char* buf, int32_t n) {
+  if (!sw || !buf || n < 1) return fail(TVBX_EINVAL, "bad argument");
+  snprintf(buf, (size_t)n, "%s", sw->fc_tc ? "tvbx::fc_xtx_tc_kernel" : "tvbx::fc_comoment_kernel");
   return TVBX_OK;
 }
 int32_t tvbx_launch_count(const tvbx_sweep* sw, int64_t* n) {

@@ -384,3 +384,58 @@ def test_cfg4_streaming_fc_drift_against_oracle():
     last simulation of the grid are checked for drift against the oracle's two-pass FC."""
     sw, o = _sampled_parity(4, 200000, 10000, [0, 255])
     assert sw.samples_kept() == 19000 and sw.launch_info()["chunk_samples"] < 19000
+
+
+# ------------------------------------------------------------------------------------ S7': FC on the tensor cores
+# TF32 keeps 11 significant bits: each centred sample carries a relative rounding error <= 2^-11, each product
+# <= 2^-10, so |dM_kl| <= 2^-10 sum_q |x_qk x_ql| <= 2^-10 sqrt(M_kk M_ll) (Cauchy-Schwarz) and the Pearson entry
+# moves by at most ~2^-10 from the products plus ~2^-10 |FC| from the two variances: 2e-3 in the worst case,
+# far inside the 0.02 of the north star (DESIGN.md section 6.4).
+TOL_FC_TF32_VS_FP32 = 2e-3
+
+
+@pytest.mark.parametrize("N,spc,clu,chunk,steps", [
+    (68, 0, 0, 0, 3000),       # cfg-1 connectome, one chunk, one 128-row block, n_c = 280 (not a multiple of 32)
+    (23, 3, 1, 37, 2400),      # odd N (scalar FP64 merge), several ragged chunks: Chan merge term
+    (130, 2, 1, 64, 1500),     # two row blocks, the second with 2 live rows
+    (360, 4, 3, 50, 1200),     # cfg-5 size: three row blocks, N extent split 256 + 112, cluster integrator
+], ids=["n68", "n23_odd", "n130", "n360"])
+def test_fc_tensor_core_path_matches_fp32_tiles_and_oracle(N, spc, clu, chunk, steps):
+    if N == 68:
+        cfg = wl.config(1); W, L = wl.config_connectome(cfg); sims = None
+    elif N == 360:
+        cfg = wl.config(5); W, L = wl.config_connectome(cfg); sims = [5, 1000, 2047, 4095, 77]
+    else:
+        W, L = wl.connectome(N, seed=N, keep=0.4); sims = None
+        cfg = dict(axes=[dict(name="G", lo=0.0, hi=0.4, n=5, values=None)], fixed=dict(v=4.0, b_e=20.0, wNoise=1e-4), seed=9)
+    kw = dict(sims_per_cta=spc, ctas_per_group=clu, chunk_samples=chunk, sim_ids=sims)
+    out = {}
+    for mode in (tvbx.TVBX_FC_TF32, tvbx.TVBX_FC_FP32):
+        _, sw = tvbx.sweep_from_config(cfg, W, L, fc_mode=mode, **kw)
+        sw.run(steps, 0.1, noise_on=True, ds=10, discard_steps=200)
+        out[mode] = sw.fc_readout()
+        assert sw.fc_kernel_name() == ("tvbx::fc_xtx_tc_kernel" if mode == tvbx.TVBX_FC_TF32 else "tvbx::fc_comoment_kernel")
+    fc_t, me_t, mi_t = out[tvbx.TVBX_FC_TF32]
+    fc_f, me_f, mi_f = out[tvbx.TVBX_FC_FP32]
+    np.testing.assert_array_equal(me_t, me_f); np.testing.assert_array_equal(mi_t, mi_f)   # same integrator
+    assert np.isfinite(fc_t).all()
+    assert np.abs(fc_t - fc_f).max() < TOL_FC_TF32_VS_FP32
+    np.testing.assert_array_equal(fc_t, np.swapaxes(fc_t, 1, 2))
+    assert np.all(np.diagonal(fc_t, axis1=1, axis2=2) == 1.0)
+    o = orc.OracleSweep(W, L, wl.grid_params(cfg, sims=sims), seed=cfg["seed"], ext_ids=sims)
+    o.run(steps, 0.1, noise_on=True, ds=10, discard_steps=200)
+    rfc, rme, rmi = o.fc_readout()
+    assert np.abs(fc_t - rfc).max() < TOL_FC_ABS
+    # readout is repeatable (the open chunk is merged into a scratch copy)
+    np.testing.assert_array_equal(sw.fc_readout()[0], fc_f)
+
+
+def test_fc_mode_default_and_errors():
+    W, L = wl.connectome(20, seed=7, keep=0.4)
+    cfg = dict(axes=[], fixed=dict(v=4.0), seed=1)
+    _, sw = tvbx.sweep_from_config(cfg, W, L)
+    assert sw.fc_kernel_name() == "tvbx::fc_xtx_tc_kernel"            # FP32 sweep, N <= 512: tensor cores
+    _, sw64 = tvbx.sweep_from_config(cfg, W, L, precision=tvbx.TVBX_F64)
+    assert sw64.fc_kernel_name() == "tvbx::fc_comoment_kernel"        # FP64 build mode keeps FP64 tiles
+    with pytest.raises(tvbx.TvbxError):
+        tvbx.sweep_from_config(cfg, W, L, precision=tvbx.TVBX_F64, fc_mode=tvbx.TVBX_FC_TF32)
