@@ -253,13 +253,21 @@ def run_tvbx(args):
     hmi = torch.empty((S, N), dtype=torch.float32).pin_memory().numpy()
     h2d = d2h = 0
 
+    e2e_phases = []
+
     def e2e_step():
         nonlocal h2d, d2h
+        ta = time.perf_counter()
         c2, s2 = tvbx.sweep_from_config(cfg, W, L, seed=seed)
+        tb = time.perf_counter()
         s2.run(steps_sim, cfg["dt"], noise_on=True, ds=cfg["ds"], discard_steps=cfg["discard_steps"], stream=stream)
+        tc = time.perf_counter()
         s2.fc_readout(device=False, stream=stream, out=(hfc, hme, hmi))
+        td = time.perf_counter()
         h2d, d2h = s2.bytes_copied()
         s2.close(); c2.close()
+        te = time.perf_counter()
+        e2e_phases.append([round(1e3 * x, 2) for x in (tb - ta, tc - tb, td - tc, te - td)])
 
     e2e_step()
     barrier()
@@ -297,7 +305,8 @@ def run_tvbx(args):
                 "config": config_dict(args.config, cfg, S, {"launch": info, "sim_steps": steps_sim,
                                                            "replicas": world, "results_finite": finite}),
                 "clocks": clk,
-                "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": int(h2d), "d2h_bytes_per_step": int(d2h)},
+                "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": int(h2d), "d2h_bytes_per_step": int(d2h),
+                        "phases_ms": {"order": ["create", "run_enqueue", "readout_sync", "destroy"], "steps": e2e_phases[1:]}},
                 "gpu_launches": int(launches), "roofline": roof}
         if world == 1 and not args.no_cpu_baseline:
             line["cpu_baseline"] = cpu_baseline(args.config)

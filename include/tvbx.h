@@ -202,6 +202,11 @@ int32_t tvbx_launch_count(const tvbx_sweep* sw, int64_t* n);
 
 const char* tvbx_last_error(void);
 int32_t tvbx_version(void);
+/* Device buffers of destroyed sweeps are cached inside the library (per device, exact size; capacity
+ * TVBX_POOL_BYTES, default a quarter of the device memory, 0 disables) and reused by the next sweep of the same
+ * shape, so create / run / destroy cycles do not pay cudaMalloc / cudaFree each time.  This call returns every
+ * cached buffer to the driver; *bytes_freed (may be NULL) receives the amount. */
+int32_t tvbx_trim_memory(int64_t* bytes_freed);
 
 #ifdef __cplusplus
 }

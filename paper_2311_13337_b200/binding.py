@@ -66,7 +66,7 @@ EXPORTS = [
     "tvbx_sweep_destroy", "tvbx_sweep_set_initial", "tvbx_run", "tvbx_fc_readout", "tvbx_sweep_size",
     "tvbx_sweep_param", "tvbx_sweep_ext_id", "tvbx_delay_index", "tvbx_ring_len", "tvbx_steps_done",
     "tvbx_samples_kept", "tvbx_sweep_state", "tvbx_launch_info", "tvbx_launch_count", "tvbx_kernel_name", "tvbx_fc_kernel_name", "tvbx_last_error",
-    "tvbx_version", "tvbx_sweep_reset", "tvbx_profile_enable", "tvbx_profile_read", "tvbx_bytes_copied",
+    "tvbx_version", "tvbx_trim_memory", "tvbx_sweep_reset", "tvbx_profile_enable", "tvbx_profile_read", "tvbx_bytes_copied",
 ]
 
 
@@ -118,6 +118,7 @@ def lib():
             "tvbx_kernel_name": [vp, C.c_char_p, i32],
             "tvbx_fc_kernel_name": [vp, C.c_char_p, i32],
             "tvbx_sweep_reset": [vp, vp],
+            "tvbx_trim_memory": [C.POINTER(i64)],
             "tvbx_profile_enable": [vp, i32],
             "tvbx_profile_read": [vp, dp, C.POINTER(i64)],
             "tvbx_bytes_copied": [vp, C.POINTER(i64), C.POINTER(i64)],
@@ -352,6 +353,13 @@ def _stream_ptr(stream):
     if isinstance(stream, int):
         return stream
     return stream.cuda_stream      # torch.cuda.Stream
+
+
+def trim_memory() -> int:
+    """tvbx_trim_memory: return the library's cached device buffers to the driver; bytes freed."""
+    out = C.c_int64()
+    _chk(lib().tvbx_trim_memory(C.byref(out)))
+    return out.value
 
 
 def sweep_from_config(cfg: dict, W, L_mm, **kw):

@@ -13,6 +13,7 @@
 #include <cstring>
 #include <map>
 #include <memory>
+#include <mutex>
 #include <new>
 #include <string>
 #include <type_traits>
@@ -196,15 +197,65 @@ namespace {
 
 using namespace tvbx;
 
+// Device-memory pool: buffers of destroyed sweeps are kept (per device, exact size) and handed to the next sweep
+// that asks for the same size, so a create / run / destroy cycle of equal sweeps pays cudaMalloc / cudaFree
+// once.  Capacity TVBX_POOL_BYTES (default: a quarter of the device memory; 0 disables); tvbx_trim_memory()
+// returns everything to the driver; a failed cudaMalloc trims and retries.
+struct DevPool {
+  std::mutex mu;
+  std::multimap<std::pair<int, size_t>, void*> free_;
+  size_t cached = 0;
+  long long cap = -1;
+  size_t capacity() {
+    if (cap < 0) {
+      if (const char* e = getenv("TVBX_POOL_BYTES")) cap = atoll(e);
+      else { size_t f = 0, t = 0; cap = cudaMemGetInfo(&f, &t) == cudaSuccess ? (long long)(t / 4) : 0; }
+    }
+    return (size_t)cap;
+  }
+  size_t trim_locked() {
+    size_t freed = cached;
+    for (auto& kv : free_) cudaFree(kv.second);
+    free_.clear(); cached = 0;
+    return freed;
+  }
+  size_t trim() { std::lock_guard<std::mutex> g(mu); return trim_locked(); }
+  cudaError_t get(void** p, size_t bytes) {
+    int dev = 0; cudaGetDevice(&dev);
+    std::lock_guard<std::mutex> g(mu);
+    auto it = free_.find({dev, bytes});
+    if (it != free_.end()) { *p = it->second; cached -= bytes; free_.erase(it); return cudaSuccess; }
+    cudaError_t e = cudaMalloc(p, bytes);
+    if (e != cudaSuccess && cached > 0) { cudaGetLastError(); trim_locked(); e = cudaMalloc(p, bytes); }
+    return e;
+  }
+  // the caller has made sure no kernel still uses p
+  void put(void* p, size_t bytes) {
+    int dev = 0; cudaGetDevice(&dev);
+    std::lock_guard<std::mutex> g(mu);
+    if (cached + bytes > capacity()) { cudaFree(p); return; }
+    free_.insert({{dev, bytes}, p}); cached += bytes;
+  }
+  size_t cached_bytes() { std::lock_guard<std::mutex> g(mu); return cached; }
+};
+DevPool& dev_pool() { static DevPool* P = new DevPool; return *P; }   // never destroyed: no cudaFree at process exit
+
 template <typename T>
 struct DevBuf {
   T* p = nullptr;
-  size_t n = 0;
-  ~DevBuf() { if (p) cudaFree(p); }
+  size_t n = 0, bytes = 0;
+  void release() {
+    if (!p) return;
+    cudaDeviceSynchronize();            // what cudaFree did implicitly: nothing in flight may still use p
+    dev_pool().put(p, bytes);
+    p = nullptr;
+  }
+  ~DevBuf() { release(); }
   cudaError_t alloc(size_t count) {
-    if (p) { cudaFree(p); p = nullptr; }
+    release();
     n = count;
-    return cudaMalloc((void**)&p, std::max<size_t>(count, 1) * sizeof(T));
+    bytes = (std::max<size_t>(count, 1) * sizeof(T) + 511) / 512 * 512;
+    return dev_pool().get((void**)&p, bytes);
   }
   cudaError_t upload(const std::vector<T>& h, int64_t* bytes) {
     cudaError_t e = alloc(h.size());
@@ -436,6 +487,7 @@ struct DeviceImpl : DeviceSide {
     const size_t row = (size_t)N * SPC;
     size_t free_b = 0, total_b = 0;
     CU(cudaMemGetInfo(&free_b, &total_b));
+    free_b += dev_pool().cached_bytes();           // pooled buffers are reusable (or trimmed on demand)
     int64_t CS = sw->chunk_req;
     if (CS <= 0) {
       // sample chunk: up to 1/16 of the free device memory, at most 8 GiB (fewer, longer integrator launches)
@@ -793,6 +845,11 @@ extern "C" {
 
 const char* tvbx_last_error(void) { return g_err.c_str(); }
 int32_t tvbx_version(void) { return TVBX_VERSION; }
+int32_t tvbx_trim_memory(int64_t* bytes_freed) {
+  const size_t f = dev_pool().trim();
+  if (bytes_freed) *bytes_freed = (int64_t)f;
+  return TVBX_OK;
+}
 
 int32_t tvbx_default_params(tvbx_model_params* out) {
   if (!out) return fail(TVBX_EINVAL, "out is NULL");
