@@ -676,7 +676,7 @@ struct DeviceImpl : DeviceSide {
         CU(cudaFuncSetAttribute(fc_xtx_tc_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_tc));
         tc_attr_set = true;
       }
-      dim3 gp((F.N * F.SPC + 31) / 32, (F.n_c + 31) / 32, F.G);
+      dim3 gp((F.N * F.SPC + 31) / 32, (F.n_c + PACK_Q - 1) / PACK_Q, F.G);
       fc_pack_tf32_kernel<<<gp, dim3(32, 8), 0, st>>>(T);
       dim3 gx(T.Rt / 128, F.G * F.SPC);
       fc_xtx_tc_kernel<<<gx, TC_THREADS, smem_tc, st>>>(T);

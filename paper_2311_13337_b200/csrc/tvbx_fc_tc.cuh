@@ -49,23 +49,29 @@ __device__ __forceinline__ float to_tf32(float x) {
   return __uint_as_float(r);
 }
 
-// grid (ceil(N SPC / 32), ceil(n_c / 32), G), block (32, 8)
+// grid (ceil(N SPC / 32), ceil(n_c / PACK_Q), G), block (32, 8): a 32-column x PACK_Q-sample tile per block, all
+// its loads in flight before the first store (16 per thread), 512-byte runs on the way out
+constexpr int PACK_Q = 128;
 __global__ void __launch_bounds__(256) fc_pack_tf32_kernel(FcTcParams P) {
-  __shared__ float tile[32][33];
+  __shared__ float tile[PACK_Q][33];
   const int g = blockIdx.z;
   const int row = P.N * P.SPC;
-  const int idx0 = blockIdx.x * 32, q0 = blockIdx.y * 32;
+  const int idx0 = blockIdx.x * 32, q0 = blockIdx.y * PACK_Q;
   const int tx = threadIdx.x, ty = threadIdx.y;
   {
     const int idx = idx0 + tx;
     const double cm = idx < row ? P.cmean[(size_t)g * row + idx] : 0.0;
     const float* x = P.xbar + (size_t)g * P.CS * row + idx;
+    float v[PACK_Q / 8];
 #pragma unroll
-    for (int i = 0; i < 4; ++i) {
+    for (int i = 0; i < PACK_Q / 8; ++i) {
       const int q = q0 + ty + 8 * i;
-      float v = 0.0f;
-      if (idx < row && q < P.n_c) v = to_tf32((float)((double)x[(size_t)q * row] - cm));
-      tile[ty + 8 * i][tx] = v;
+      v[i] = (idx < row && q < P.n_c) ? x[(size_t)q * row] : 0.0f;
+    }
+#pragma unroll
+    for (int i = 0; i < PACK_Q / 8; ++i) {
+      const int q = q0 + ty + 8 * i;
+      tile[ty + 8 * i][tx] = (idx < row && q < P.n_c) ? to_tf32((float)((double)v[i] - cm)) : 0.0f;
     }
   }
   __syncthreads();
@@ -74,7 +80,10 @@ __global__ void __launch_bounds__(256) fc_pack_tf32_kernel(FcTcParams P) {
     const int c = ty + 8 * i, idx = idx0 + c;
     if (idx >= row) continue;
     const int k = idx / P.SPC, s = idx % P.SPC;
-    P.xc[(((size_t)g * P.SPC + s) * P.N + k) * P.Kp + q0 + tx] = tile[tx][c];
+    float* dst = P.xc + (((size_t)g * P.SPC + s) * P.N + k) * P.Kp + q0;
+#pragma unroll
+    for (int t = 0; t < PACK_Q / 32; ++t)
+      if (q0 + 32 * t < P.Kp) dst[32 * t + tx] = tile[32 * t + tx][c];
   }
 }
 
@@ -121,11 +130,14 @@ __device__ __forceinline__ void mma_tf32(uint32_t d_tmem, uint64_t adesc, uint64
 __device__ __forceinline__ void mma_commit(uint32_t bar) {
   asm volatile("tcgen05.commit.cta_group::1.mbarrier::arrive::one.shared::cluster.b64 [%0];" ::"r"(bar) : "memory");
 }
-__device__ __forceinline__ void tmem_ld16(uint32_t taddr, uint32_t (&v)[16]) {
+__device__ __forceinline__ void tmem_ld32(uint32_t taddr, uint32_t (&v)[32]) {
   asm volatile(
-      "tcgen05.ld.sync.aligned.32x32b.x16.b32 {%0, %1, %2, %3, %4, %5, %6, %7, %8, %9, %10, %11, %12, %13, %14, %15}, [%16];"
+      "tcgen05.ld.sync.aligned.32x32b.x32.b32 {%0, %1, %2, %3, %4, %5, %6, %7, %8, %9, %10, %11, %12, %13, %14, %15, "
+      "%16, %17, %18, %19, %20, %21, %22, %23, %24, %25, %26, %27, %28, %29, %30, %31}, [%32];"
       : "=r"(v[0]), "=r"(v[1]), "=r"(v[2]), "=r"(v[3]), "=r"(v[4]), "=r"(v[5]), "=r"(v[6]), "=r"(v[7]), "=r"(v[8]),
-        "=r"(v[9]), "=r"(v[10]), "=r"(v[11]), "=r"(v[12]), "=r"(v[13]), "=r"(v[14]), "=r"(v[15])
+        "=r"(v[9]), "=r"(v[10]), "=r"(v[11]), "=r"(v[12]), "=r"(v[13]), "=r"(v[14]), "=r"(v[15]), "=r"(v[16]),
+        "=r"(v[17]), "=r"(v[18]), "=r"(v[19]), "=r"(v[20]), "=r"(v[21]), "=r"(v[22]), "=r"(v[23]), "=r"(v[24]),
+        "=r"(v[25]), "=r"(v[26]), "=r"(v[27]), "=r"(v[28]), "=r"(v[29]), "=r"(v[30]), "=r"(v[31])
       : "r"(taddr) : "memory");
   asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory");
 }
@@ -226,40 +238,43 @@ __global__ void __launch_bounds__(TC_THREADS) fc_xtx_tc_kernel(FcTcParams P) {
   tc::mbar_wait(bar0 + 8 * ((nkb - 1) % TC_STAGES), (uint32_t)(((nkb - 1) / TC_STAGES) & 1));
   tc::tc_fence_after();
 
-  // ---- epilogue: thread = output row (TMEM lane), 16 columns per tcgen05.ld; Chan merge in FP64 ----
+  // ---- epilogue: TMEM -> registers (thread = output row, 32 columns per tcgen05.ld) -> a 32 x 32 transpose
+  // through the (now free) stage memory -> lanes = 32 consecutive columns of one row, so every read-modify-write
+  // of the FP64 accumulator is one contiguous 256-byte run per warp instruction; Chan merge in FP64 ----
   {
     const int lq = warp & 3, ch = warp >> 2;
-    const int k = mb * 128 + lq * 32 + lane;
-    const int ng = P.Np / 16, gh = (ng + 1) / 2;
+    const int r0 = mb * 128 + lq * 32;                // first output row of this warp
+    const int ng = (P.Np + 31) / 32, gh = (ng + 1) / 2;
     const int gbeg = ch == 0 ? 0 : gh, gend = ch == 0 ? gh : ng;
-    if (mb * 128 + lq * 32 < N) {                     // warp-uniform: some row of this warp exists
+    if (r0 < N) {                                     // warp-uniform: some row of this warp exists
+      float* tile = reinterpret_cast<float*>(smem) + warp * (32 * 33);
       const double f = P.cnt > 0 ? (double)P.cnt * (double)P.n_c / (double)(P.cnt + P.n_c) : 0.0;
-      const double dk = k < N ? delta[k] : 0.0;     // (dk dl) f: the same bits for (k, l) and (l, k)
-      double* Mrow = P.M + (size_t)gs * N * N + (size_t)(k < N ? k : 0) * N;
-      const bool vec2 = (N & 1) == 0;
+      double* Mbase = P.M + (size_t)gs * N * N;
+      const int nrow = min(32, N - r0);
       for (int cg = gbeg; cg < gend; ++cg) {
-        uint32_t v[16];
-        tc::tmem_ld16(tmem + ((uint32_t)(lq * 32) << 16) + (uint32_t)(cg * 16), v);
-        if (k >= N) continue;
-        const int l0 = cg * 16;
-        if (vec2) {
+        uint32_t v[32];
+        tc::tmem_ld32(tmem + ((uint32_t)(lq * 32) << 16) + (uint32_t)(cg * 32), v);
 #pragma unroll
-          for (int j = 0; j < 16; j += 2) {
-            const int l = l0 + j;
-            if (l >= N) break;
-            double2* p = reinterpret_cast<double2*>(Mrow + l);
-            double2 m = *p;
-            m.x += (double)__uint_as_float(v[j]) + (dk * delta[l]) * f;
-            m.y += (double)__uint_as_float(v[j + 1]) + (dk * delta[l + 1]) * f;
-            *p = m;
-          }
-        } else {
+        for (int j = 0; j < 32; ++j) tile[lane * 33 + j] = __uint_as_float(v[j]);
+        __syncwarp();
+        const int l = cg * 32 + lane;
+        if (l < N) {
+          const double dl = delta[l];
+          double* Mcol = Mbase + (size_t)r0 * N + l;
+          for (int rb = 0; rb < nrow; rb += 8) {       // 8 independent loads in flight, then 8 stores
+            double m[8];
 #pragma unroll
-          for (int j = 0; j < 16; ++j) {
-            const int l = l0 + j;
-            if (l < N) Mrow[l] += (double)__uint_as_float(v[j]) + (dk * delta[l]) * f;
+            for (int u = 0; u < 8; ++u)
+              if (rb + u < nrow) m[u] = __ldcs(Mcol + (size_t)(rb + u) * N);
+#pragma unroll
+            for (int u = 0; u < 8; ++u) {
+              const int r = rb + u;
+              // (dk dl) f: the same bits for (k, l) and (l, k), so M and FC stay symmetric
+              if (r < nrow) __stcs(Mcol + (size_t)r * N, m[u] + ((double)tile[r * 33 + lane] + (delta[r0 + r] * dl) * f));
+            }
           }
         }
+        __syncwarp();
       }
     }
   }
