@@ -247,6 +247,25 @@ def run_tvbx(args):
     value = world * units_per_step * args.steps / (ms_max * 1e-3)
     finite = bool(torch.isfinite(fc).all().item() and torch.isfinite(me).all().item())
 
+    # ---- f3 (not part of the step): FCSC / mean FC per simulation from the resident accumulators ----
+    sw.fc_scores(device=True, stream=stream)
+    stream.synchronize()
+    sw.profile_enable(True)
+    sw.profile_read()
+    s0, s1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    per_call = []
+    for _ in range(5):
+        s0.record(stream)
+        sw.fc_scores(device=True, stream=stream)
+        s1.record(stream)
+        stream.synchronize()
+        per_call.append(s0.elapsed_time(s1))
+    scores_ms = sorted(per_call)[len(per_call) // 2]
+    sprof = sw.profile_read()
+    sw.profile_enable(False)
+    scores_kernel_ms = sprof["readout"][0] / max(sprof["readout"][1], 1)      # fc_scores_kernel alone
+    scores_bytes = S * N * N * 8.0          # the FP64 co-moments, read once
+
     # ---- end-to-end arm: host buffers through the C ABI ---------------------------------------------
     hfc = torch.empty((S, N, N), dtype=torch.float32).pin_memory().numpy()
     hme = torch.empty((S, N), dtype=torch.float32).pin_memory().numpy()
@@ -307,7 +326,14 @@ def run_tvbx(args):
                 "clocks": clk,
                 "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": int(h2d), "d2h_bytes_per_step": int(d2h),
                         "phases_ms": {"order": ["create", "run_enqueue", "readout_sync", "destroy"], "steps": e2e_phases[1:]}},
-                "gpu_launches": int(launches), "roofline": roof}
+                "gpu_launches": int(launches), "roofline": roof,
+                "fc_scores": {"ms": scores_ms, "kernel_ms": scores_kernel_ms,
+                              "kernel_achieved_gbs": scores_bytes / (scores_kernel_ms * 1e-3) / 1e9 if scores_kernel_ms > 0 else None,
+                              "kernel_frac_hbm": (scores_bytes / (scores_kernel_ms * 1e-3) / 1e9 / pk.get("hbm_gbs", 6650.0)
+                                                  if scores_kernel_ms > 0 else None),
+                              "note": "tvbx_fc_scores (FCSC + mean FC per simulation, P:113), outside the timed step; ms includes "
+                                      "merging the open sample chunk (S7) into a scratch copy, kernel_ms is fc_scores_kernel alone; "
+                                      "algorithmic bytes = the FP64 co-moments S*N*N*8, read once"}}
         if world == 1 and not args.no_cpu_baseline:
             line["cpu_baseline"] = cpu_baseline(args.config)
         print(json.dumps(line), flush=True)

@@ -157,6 +157,19 @@ int32_t tvbx_run(tvbx_sweep* sw, int64_t steps, double dt, const tvbx_run_opts* 
 int32_t tvbx_fc_readout(tvbx_sweep* sw, float* fc, float* mean_e, float* mean_i, int32_t on_device,
                         void* cuda_stream);
 
+/* FC scores per simulation (Eq. (6), Tab. 2; A23), over the
+ * N(N-1)/2 region pairs k < l of the Pearson matrix tvbx_fc_readout would return (formed in FP64 from the
+ * accumulators, open chunk included, accumulators untouched):
+ *   fcsc[s]    = Pearson(FC_kl, W_kl)      structure-function correlation with the connectome weights (SC)
+ *   fitness[s] = Pearson(FC_kl, ref_kl)    against an externally obtained reference FC; ref_fc = HOST, row-major
+ *                                          N x N doubles (only k < l is read), copied before the call returns
+ *   mean_fc[s] = mean(FC_kl)
+ * Any output may be NULL; outputs are n_sims floats in this sweep's simulation order, host or device
+ * (on_device).  Zero variance gives 0.  TVBX_ESTATE with fewer than 2 kept samples, TVBX_EINVAL if fitness is
+ * asked for without ref_fc or ref_fc holds a non-finite value. */
+int32_t tvbx_fc_scores(tvbx_sweep* sw, const double* ref_fc, float* fcsc, float* fitness, float* mean_fc,
+                       int32_t on_device, void* stream);
+
 /* Back to step 0 without re-allocating: state, OU, history ring, window sums and FC accumulators are
  * re-initialised on the device (enqueued on cuda_stream), the step and sample counters are zeroed.
  * A no-op before the first tvbx_run.  reset; run(n) is bit-identical to a fresh sweep's run(n). */

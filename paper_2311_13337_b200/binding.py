@@ -63,7 +63,7 @@ class RunOpts(C.Structure):
 
 EXPORTS = [
     "tvbx_default_params", "tvbx_create_connectome", "tvbx_destroy_connectome", "tvbx_sweep_create",
-    "tvbx_sweep_destroy", "tvbx_sweep_set_initial", "tvbx_run", "tvbx_fc_readout", "tvbx_sweep_size",
+    "tvbx_sweep_destroy", "tvbx_sweep_set_initial", "tvbx_run", "tvbx_fc_readout", "tvbx_fc_scores", "tvbx_sweep_size",
     "tvbx_sweep_param", "tvbx_sweep_ext_id", "tvbx_delay_index", "tvbx_ring_len", "tvbx_steps_done",
     "tvbx_samples_kept", "tvbx_sweep_state", "tvbx_launch_info", "tvbx_launch_count", "tvbx_kernel_name", "tvbx_fc_kernel_name", "tvbx_last_error",
     "tvbx_version", "tvbx_trim_memory", "tvbx_sweep_reset", "tvbx_profile_enable", "tvbx_profile_read", "tvbx_bytes_copied",
@@ -105,6 +105,7 @@ def lib():
             "tvbx_sweep_set_initial": [vp, dp],
             "tvbx_run": [vp, i64, dbl, C.POINTER(RunOpts)],
             "tvbx_fc_readout": [vp, vp, vp, vp, i32, vp],
+            "tvbx_fc_scores": [vp, vp, vp, vp, vp, i32, vp],
             "tvbx_sweep_size": [vp, C.POINTER(i64), C.POINTER(i64), C.POINTER(i32)],
             "tvbx_sweep_param": [vp, i64, i32, dp],
             "tvbx_sweep_ext_id": [vp, i64, C.POINTER(i64)],
@@ -330,6 +331,24 @@ class Sweep:
         a, b = C.c_int64(), C.c_int64()
         _chk(lib().tvbx_bytes_copied(self._h, C.byref(a), C.byref(b)))
         return a.value, b.value
+
+    def fc_scores(self, ref_fc=None, device=False, stream=None):
+        """tvbx_fc_scores -> dict(fcsc [S], mean_fc [S], fitness [S] if ref_fc is given) float32; numpy or torch CUDA."""
+        S = self.n_sims
+        ref = None if ref_fc is None else np.ascontiguousarray(ref_fc, dtype=np.float64)
+        if ref is not None:
+            assert ref.shape == (self.n_regions, self.n_regions)
+        names = ["fcsc", "fitness", "mean_fc"] if ref is not None else ["fcsc", "mean_fc"]
+        if device:
+            import torch
+            out = {k: torch.empty((S,), device="cuda", dtype=torch.float32) for k in names}
+            ptr = {k: v.data_ptr() for k, v in out.items()}
+        else:
+            out = {k: np.empty((S,), np.float32) for k in names}
+            ptr = {k: v.ctypes.data for k, v in out.items()}
+        _chk(lib().tvbx_fc_scores(self._h, None if ref is None else ref.ctypes.data, ptr["fcsc"], ptr.get("fitness"),
+                                  ptr["mean_fc"], 1 if device else 0, _stream_ptr(stream)))
+        return out
 
     def kernel_name(self):
         buf = C.create_string_buffer(64)

@@ -119,6 +119,7 @@ struct DeviceSide {
   virtual int32_t start(double dt) = 0;
   virtual int32_t run(int64_t steps, const tvbx_run_opts* o) = 0;
   virtual int32_t readout(float* fc, float* me, float* mi, int on_device, cudaStream_t st) = 0;
+  virtual int32_t scores(const double* ref, float* fcsc, float* fitness, float* mean_fc, int on_device, cudaStream_t st) = 0;
   virtual int32_t state(double* y, double* ou) = 0;
   virtual int32_t reset(cudaStream_t st) = 0;
 };
@@ -780,20 +781,74 @@ struct DeviceImpl : DeviceSide {
     return TVBX_OK;
   }
 
-  int32_t readout(float* fc, float* me, float* mi, int on_device, cudaStream_t st) override {
-    const int N = sw->conn.n, SPC = sw->spc, G = (int)sw->groups.size();
-    const int64_t total = sw->cnt + sw->fill;
-    if (total < 2) return fail(TVBX_ESTATE, "fewer than 2 samples kept (%lld)", (long long)total);
+  // co-moments including the open chunk: merged into a scratch copy, the accumulators stay untouched
+  int32_t merged_M(const double** Msrc, cudaStream_t st) {
     DevBuf<double>& tM = d_M_scratch; DevBuf<double>& tmean = d_mean_scratch;   // allocated once, kept
-    const double* Msrc = d_M.p;
-    if (sw->fill > 0) {     // merge the open chunk into a scratch copy; the accumulators stay untouched
+    *Msrc = d_M.p;
+    if (sw->fill > 0) {
       if (tM.n != d_M.n) { CU(tM.alloc(d_M.n)); CU(tmean.alloc(d_mean.n)); }
       CU(cudaMemcpyAsync(tM.p, d_M.p, d_M.n * sizeof(double), cudaMemcpyDeviceToDevice, st));
       CU(cudaMemcpyAsync(tmean.p, d_mean.p, d_mean.n * sizeof(double), cudaMemcpyDeviceToDevice, st));
       int32_t rc = accumulate(tM.p, tmean.p, sw->cnt, (int)sw->fill, st);
       if (rc) return rc;
-      Msrc = tM.p;
+      *Msrc = tM.p;
     }
+    return TVBX_OK;
+  }
+
+  // f3: FCSC, fitness against a reference FC, mean FC per simulation (fc_scores_kernel)
+  DevBuf<double> d_sc, d_ref;
+  DevBuf<float> d_out_sc[3];
+  int32_t scores(const double* ref, float* fcsc, float* fitness, float* mean_fc, int on_device, cudaStream_t st) override {
+    const int N = sw->conn.n, SPC = sw->spc, G = (int)sw->groups.size();
+    const int64_t total = sw->cnt + sw->fill;
+    if (total < 2) return fail(TVBX_ESTATE, "fewer than 2 samples kept (%lld)", (long long)total);
+    const double* Msrc = nullptr;
+    { int32_t rc = merged_M(&Msrc, st); if (rc) return rc; }
+    const size_t nn = (size_t)N * N;
+    if (d_sc.n != nn) {
+      CU(d_sc.alloc(nn));
+      CU(cudaMemcpyAsync(d_sc.p, sw->conn.W.data(), nn * sizeof(double), cudaMemcpyHostToDevice, st));
+      sw->h2d += (int64_t)(nn * sizeof(double));
+    }
+    if (ref) {
+      if (d_ref.n != nn) CU(d_ref.alloc(nn));
+      CU(cudaMemcpyAsync(d_ref.p, ref, nn * sizeof(double), cudaMemcpyHostToDevice, st));
+      sw->h2d += (int64_t)(nn * sizeof(double));
+    }
+    ScoreParams Q;
+    Q.M = Msrc; Q.sc = d_sc.p; Q.ref = ref ? d_ref.p : nullptr; Q.loc_id = d_loc.p; Q.N = N; Q.SPC = SPC; Q.G = G;
+    float* outs[3] = {fcsc, fitness, mean_fc};
+    float* devs[3] = {fcsc, fitness, mean_fc};
+    if (!on_device)
+      for (int i = 0; i < 3; ++i)
+        if (outs[i]) { if (d_out_sc[i].n != (size_t)sw->n_sims) CU(d_out_sc[i].alloc((size_t)sw->n_sims)); devs[i] = d_out_sc[i].p; }
+    Q.fcsc = devs[0]; Q.fitness = devs[1]; Q.mean_fc = devs[2];
+    sw->prof_begin(K_READOUT, st);
+    Q.diag_in_smem = N <= 4096;
+    fc_scores_kernel<<<G * SPC, 256, Q.diag_in_smem ? (size_t)N * sizeof(double) : 0, st>>>(Q);
+    sw->prof_end(st);
+    sw->launches += 1;
+    CU(cudaGetLastError());
+    if (!on_device) {
+      for (int i = 0; i < 3; ++i)
+        if (outs[i]) {
+          CU(cudaMemcpyAsync(outs[i], devs[i], (size_t)sw->n_sims * sizeof(float), cudaMemcpyDeviceToHost, st));
+          sw->d2h += (int64_t)((size_t)sw->n_sims * sizeof(float));
+        }
+      CU(cudaStreamSynchronize(st));
+    } else if (ref) {
+      CU(cudaStreamSynchronize(st));     // the host copy of ref must not be reused before the upload is done
+    }
+    return TVBX_OK;
+  }
+
+  int32_t readout(float* fc, float* me, float* mi, int on_device, cudaStream_t st) override {
+    const int N = sw->conn.n, SPC = sw->spc, G = (int)sw->groups.size();
+    const int64_t total = sw->cnt + sw->fill;
+    if (total < 2) return fail(TVBX_ESTATE, "fewer than 2 samples kept (%lld)", (long long)total);
+    const double* Msrc = nullptr;
+    { int32_t rc = merged_M(&Msrc, st); if (rc) return rc; }
     DevBuf<float>& dfc = d_out_fc; DevBuf<float>& dme = d_out_me; DevBuf<float>& dmi = d_out_mi;   // kept between calls
     ReadoutParams Q;
     Q.M = Msrc; Q.sums = d_sums.p; Q.loc_id = d_loc.p; Q.cnt = total; Q.N = N; Q.SPC = SPC; Q.G = G;
@@ -1070,6 +1125,16 @@ int32_t tvbx_run(tvbx_sweep* sw, int64_t steps, double dt, const tvbx_run_opts* 
   return sw->dev->run(steps, &o);
 }
 
+int32_t tvbx_fc_scores(tvbx_sweep* sw, const double* ref_fc, float* fcsc, float* fitness, float* mean_fc,
+                       int32_t on_device, void* stream) {
+  if (!sw) return fail(TVBX_EINVAL, "sweep is NULL");
+  if (!sw->started) return fail(TVBX_ESTATE, "no run yet");
+  if (fitness && !ref_fc) return fail(TVBX_EINVAL, "fitness needs a reference FC");
+  if (ref_fc)
+    for (size_t i = 0; i < (size_t)sw->conn.n * sw->conn.n; ++i)
+      if (!std::isfinite(ref_fc[i])) return fail(TVBX_EINVAL, "reference FC entry %zu is not finite", i);
+  return sw->dev->scores(ref_fc, fcsc, fitness, mean_fc, on_device, (cudaStream_t)stream);
+}
 int32_t tvbx_fc_readout(tvbx_sweep* sw, float* fc, float* mean_e, float* mean_i, int32_t on_device, void* stream) {
   if (!sw) return fail(TVBX_EINVAL, "sweep is NULL");
   if (!sw->started) return fail(TVBX_ESTATE, "no run yet");

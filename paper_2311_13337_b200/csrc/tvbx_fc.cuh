@@ -167,4 +167,71 @@ __global__ void fc_readout_kernel(ReadoutParams P) {
   }
 }
 
+// ---- FC scores ("FCSC, the correlation with the structure connectivity
+// (SC) ... determined with the Pearson correlation", "comparison to an externally obtained reference FC matrix by
+// correlating it to the computed FC", fitness P:159 with Eq. (6), mean_FC Tab. 2) ----
+// Per simulation, over the N(N-1)/2 region pairs k < l (reading A23: both matrices are symmetric, the diagonal is
+// trivial: FC_kk = 1, W_kk = 0):  fcsc = Pearson(FC_kl, SC_kl), fitness = Pearson(FC_kl, REF_kl),
+// mean_fc = mean(FC_kl).  FC_kl is formed in FP64 from the co-moments exactly as fc_readout_kernel does (before the
+// rounding to float); sums in FP64, folded in a fixed order (deterministic).  Zero variance -> 0 (A18).
+struct ScoreParams {
+  const double* M;       // [G][SPC][N][N]
+  const double* sc;      // [N][N] structural connectivity (the connectome weights), device
+  const double* ref;     // [N][N] reference FC, device, or null
+  const int32_t* loc_id; // [G][SPC]
+  float* fcsc;           // [n_sims] or null
+  float* fitness;        // [n_sims] or null
+  float* mean_fc;        // [n_sims] or null
+  int32_t N, SPC, G;
+  int32_t diag_in_smem;  // the launch carries N doubles of dynamic shared memory
+};
+
+// one CTA of 256 threads per (group, lane); sums: x, xx, a, aa, xa, b, bb, xb  (x = FC, a = SC, b = REF)
+__global__ void __launch_bounds__(256) fc_scores_kernel(ScoreParams P) {
+  __shared__ double part[8][256];
+  const int g = blockIdx.x / P.SPC, sl = blockIdx.x % P.SPC;
+  const int loc = P.loc_id[(size_t)g * P.SPC + sl];
+  if (loc < 0) return;
+  const int N = P.N;
+  const double* M = P.M + ((size_t)g * P.SPC + sl) * N * N;
+  // the diagonal (variances) staged in shared memory when it fits: the strided M_ll lookups stay on chip
+  extern __shared__ double diag[];
+  const bool staged = P.diag_in_smem != 0;
+  if (staged) {
+    for (int k = threadIdx.x; k < N; k += 256) diag[k] = M[(size_t)k * N + k];
+    __syncthreads();
+  }
+  double acc[8] = {0, 0, 0, 0, 0, 0, 0, 0};
+  for (int i = threadIdx.x; i < N * N; i += 256) {
+    const int k = i / N, l = i % N;
+    if (l <= k) continue;
+    const double den = staged ? diag[k] * diag[l] : M[(size_t)k * N + k] * M[(size_t)l * N + l];
+    double x = (den > 0.0 && isfinite(den)) ? M[i] / sqrt(den) : 0.0;
+    x = isfinite(x) ? fmin(1.0, fmax(-1.0, x)) : 0.0;
+    const double a = P.sc[i], b = P.ref ? P.ref[i] : 0.0;
+    acc[0] += x; acc[1] += x * x; acc[2] += a; acc[3] += a * a; acc[4] += x * a; acc[5] += b; acc[6] += b * b; acc[7] += x * b;
+  }
+#pragma unroll
+  for (int q = 0; q < 8; ++q) part[q][threadIdx.x] = acc[q];
+  __syncthreads();
+  for (int w = 128; w > 0; w >>= 1) {
+    if (threadIdx.x < w)
+#pragma unroll
+      for (int q = 0; q < 8; ++q) part[q][threadIdx.x] += part[q][threadIdx.x + w];
+    __syncthreads();
+  }
+  if (threadIdx.x == 0) {
+    const double n = 0.5 * (double)N * (double)(N - 1);
+    const double sx = part[0][0], vx = part[1][0] - sx * sx / n;
+    auto pearson = [&](double sy, double syy, double sxy) {
+      const double vy = syy - sy * sy / n, c = sxy - sx * sy / n, den = vx * vy;
+      const double r = (n > 1.0 && den > 0.0 && isfinite(den)) ? c / sqrt(den) : 0.0;
+      return (float)fmin(1.0, fmax(-1.0, r));
+    };
+    if (P.fcsc) P.fcsc[loc] = pearson(part[2][0], part[3][0], part[4][0]);
+    if (P.fitness) P.fitness[loc] = P.ref ? pearson(part[5][0], part[6][0], part[7][0]) : 0.0f;
+    if (P.mean_fc) P.mean_fc[loc] = n > 0.0 ? (float)(sx / n) : 0.0f;
+  }
+}
+
 }  // namespace tvbx

@@ -439,3 +439,59 @@ def test_fc_mode_default_and_errors():
     assert sw64.fc_kernel_name() == "tvbx::fc_comoment_kernel"        # FP64 build mode keeps FP64 tiles
     with pytest.raises(tvbx.TvbxError):
         tvbx.sweep_from_config(cfg, W, L, precision=tvbx.TVBX_F64, fc_mode=tvbx.TVBX_FC_TF32)
+
+
+# ------------------------------------------------------------------------------------ f3: FC scores
+# Tolerance: the scores are Pearson coefficients / means of FC entries; an FC entry may differ from the oracle's by
+# TOL_FC_ABS (noise-on runs, FP32 integrator), and a perturbation of that size on entries whose spread is O(0.1-1)
+# moves a correlation by the same order at most -- the same absolute 0.02 is used; observed differences ~1e-4.
+@pytest.mark.parametrize("N,kw", [(68, dict()), (23, dict(sims_per_cta=3, chunk_samples=37)),
+                                  (360, dict(sims_per_cta=4, ctas_per_group=3))], ids=["n68", "n23", "n360"])
+def test_fc_scores_match_the_oracle(N, kw):
+    from oracle import fc_scores as ofs
+    if N == 68:
+        cfg = wl.config(1); W, L = wl.config_connectome(cfg); sims = None
+    elif N == 360:
+        cfg = wl.config(5); W, L = wl.config_connectome(cfg); sims = [5, 2047, 4095]
+    else:
+        W, L = wl.connectome(N, seed=N, keep=0.4); sims = None
+        cfg = dict(axes=[dict(name="G", lo=0.0, hi=0.4, n=5, values=None)], fixed=dict(v=4.0, b_e=20.0, wNoise=1e-4), seed=9)
+    steps = 2400 if N != 360 else 1200
+    _, sw = tvbx.sweep_from_config(cfg, W, L, sim_ids=sims, **kw)
+    sw.run(steps, 0.1, noise_on=True, ds=10, discard_steps=200)
+    o = orc.OracleSweep(W, L, wl.grid_params(cfg, sims=sims), seed=cfg["seed"], ext_ids=sims)
+    o.run(steps, 0.1, noise_on=True, ds=10, discard_steps=200)
+    rfc = o.fc_readout()[0]
+    ref = rfc[0] + 0.05 * np.random.default_rng(0).standard_normal(rfc[0].shape)     # an "external" FC
+    ref = 0.5 * (ref + ref.T)
+    want = ofs.fc_scores(rfc, W, ref)
+    got = sw.fc_scores(ref_fc=ref)
+    for k in ("fcsc", "fitness", "mean_fc"):
+        assert got[k].shape == (sw.n_sims,) and np.isfinite(got[k]).all()
+        assert np.abs(got[k] - np.asarray(want[k])).max() < TOL_FC_ABS, k
+    # the same numbers from the FC matrix the library returns (rounded to float32: with G = 0 the entries spread by
+    # only ~1e-2, so 6e-8 of rounding shows up as ~1e-5 in a correlation) through the oracle's definition
+    own = ofs.fc_scores(sw.fc_readout()[0].astype(np.float64), W, ref)
+    for k in ("fcsc", "fitness", "mean_fc"):
+        np.testing.assert_allclose(got[k], own[k], atol=5e-5)
+    # device outputs, no reference; repeatable; accumulators untouched
+    import torch
+    dev = sw.fc_scores(device=True)
+    torch.cuda.synchronize()
+    assert set(dev) == {"fcsc", "mean_fc"}
+    np.testing.assert_array_equal(dev["fcsc"].cpu().numpy(), got["fcsc"])
+    np.testing.assert_array_equal(sw.fc_scores(ref_fc=ref)["fitness"], got["fitness"])
+
+
+def test_fc_scores_errors_and_degenerate():
+    W, L = wl.connectome(12, seed=1, keep=0.5)
+    cfg = dict(axes=[], fixed=dict(v=4.0), seed=1)
+    _, sw = tvbx.sweep_from_config(cfg, W, L)
+    with pytest.raises(tvbx.TvbxError):
+        sw.fc_scores()                                   # no run yet
+    sw.run(300, 0.1, noise_on=False, ds=10)              # noise off, identical start: series are smooth, FC defined
+    bad = np.full((12, 12), np.nan)
+    with pytest.raises(tvbx.TvbxError):
+        sw.fc_scores(ref_fc=bad)
+    const = sw.fc_scores(ref_fc=np.full((12, 12), 0.5))
+    assert const["fitness"][0] == 0.0                    # zero-variance reference -> 0 (A18 / A23)
