@@ -316,28 +316,29 @@ KernelPick<float> pick_kernel<float>(bool single, bool closed, int spc) {
 // integrate2_kernel instances: compile-time simulations per CTA 1..8; delay table in shared memory with 2, 4 or
 // 8 ring slots loaded per edge, or read through L1/L2 (8 slots)
 typedef void (*Kernel2Fn)(const Integrate2Params);
-template <bool SMEMTAB, int GCE, bool CLU = false>
+template <bool SMEMTAB, int GCE, bool CLU = false, bool SRING = false>
 inline Kernel2Fn pick_kernel2_spc(int spc) {
   switch (spc) {
-    case 1: return integrate2_kernel<1, SMEMTAB, GCE, CLU>;
-    case 2: return integrate2_kernel<2, SMEMTAB, GCE, CLU>;
-    case 3: return integrate2_kernel<3, SMEMTAB, GCE, CLU>;
-    case 4: return integrate2_kernel<4, SMEMTAB, GCE, CLU>;
-    case 5: return integrate2_kernel<5, SMEMTAB, GCE, CLU>;
-    case 6: return integrate2_kernel<6, SMEMTAB, GCE, CLU>;
-    case 7: return integrate2_kernel<7, SMEMTAB, GCE, CLU>;
-    default: return integrate2_kernel<8, SMEMTAB, GCE, CLU>;
+    case 1: return integrate2_kernel<1, SMEMTAB, GCE, CLU, false, SRING>;
+    case 2: return integrate2_kernel<2, SMEMTAB, GCE, CLU, false, SRING>;
+    case 3: return integrate2_kernel<3, SMEMTAB, GCE, CLU, false, SRING>;
+    case 4: return integrate2_kernel<4, SMEMTAB, GCE, CLU, false, SRING>;
+    case 5: return integrate2_kernel<5, SMEMTAB, GCE, CLU, false, SRING>;
+    case 6: return integrate2_kernel<6, SMEMTAB, GCE, CLU, false, SRING>;
+    case 7: return integrate2_kernel<7, SMEMTAB, GCE, CLU, false, SRING>;
+    default: return integrate2_kernel<8, SMEMTAB, GCE, CLU, false, SRING>;
   }
 }
 // cluster form (several CTAs per group): table through L1/L2, 8 slots per edge; vec: quad ring layout + vector gather
-inline Kernel2Fn pick_kernel2(int spc, bool smemtab, int gce, bool clu, bool vec) {
+inline Kernel2Fn pick_kernel2(int spc, bool smemtab, int gce, bool clu, bool vec, bool sring = false) {
+  if (sring) return gce == 2 ? pick_kernel2_spc<true, 2, false, true>(spc) : pick_kernel2_spc<true, 4, false, true>(spc);
   if (clu && vec && smemtab) return spc == 8 ? integrate2_kernel<8, true, 8, true, true> : integrate2_kernel<4, true, 8, true, true>;
   if (clu && vec) return spc == 8 ? integrate2_kernel<8, false, 8, true, true> : integrate2_kernel<4, false, 8, true, true>;
   if (clu) return pick_kernel2_spc<false, 8, true>(spc);
   if (!smemtab) return pick_kernel2_spc<false, 8>(spc);
   return gce == 2 ? pick_kernel2_spc<true, 2>(spc) : (gce == 4 ? pick_kernel2_spc<true, 4>(spc) : pick_kernel2_spc<true, 8>(spc));
 }
-struct Launch2 { int g0, count; Kernel2Fn fn; };   // consecutive groups whose tables share the slots-per-edge class
+struct Launch2 { int g0, count; Kernel2Fn fn; int smem; };   // consecutive groups whose tables share the slots-per-edge class
 
 template <typename R>
 struct DeviceImpl : DeviceSide {
@@ -627,16 +628,33 @@ struct DeviceImpl : DeviceSide {
     smem = (int)(base + (CLU == 1 ? (P2.smem_table ? tbytes : 0) : (clu_tab ? slice_bytes : 0)));
     // one launch per run of groups whose chunk length falls in the same class (cfg 3: v <= 8 / 16 / >= 32 m/s)
     launches2.clear();
+    // (process-wide and only ever raised: another live sweep may launch the same instance with more shared memory)
+    static std::map<const void*, int> fn_smem;
+    static std::mutex fn_mu;
+    std::lock_guard<std::mutex> fn_lock(fn_mu);
     cudaFuncAttributes fa;
     std::memset(&fa, 0, sizeof fa);
     for (int g = 0; g < (int)sw->groups.size(); ++g) {
       const HostTable& ht = sw->tables[sw->groups[g].table];
       const int ch = ring_geom(ht.D, ht.dmin, true).CH;
       const int gce = !P2.smem_table ? 8 : (ch <= 2 ? 2 : (ch <= 4 ? 4 : 8));
-      Kernel2Fn fn = pick_kernel2(SPC, P2.smem_table != 0, gce, CLU > 1, ht.vec != 0);
-      if (!launches2.empty() && launches2.back().fn == fn) { launches2.back().count++; continue; }
-      launches2.push_back({g, 1, fn});
-      CU(cudaFuncSetAttribute((const void*)fn, cudaFuncAttributeMaxDynamicSharedMemorySize, std::max(smem, 1024)));
+      // short delays: the group's ring ([N][Hp + GC - 1][SPC] floats) in shared memory next to the table
+      const size_t ring_b = (size_t)N * (ht.Hp + GC - 1) * SPC * sizeof(float) + 16;
+      const bool sring = CLU == 1 && P2.smem_table && gce < 8 && smem + ring_b <= (size_t)200 * 1024 &&
+                         getenv("TVBX_NO_SRING") == nullptr;
+      const int lsmem = smem + (sring ? (int)ring_b : 0);
+      Kernel2Fn fn = pick_kernel2(SPC, P2.smem_table != 0, gce, CLU > 1, ht.vec != 0, sring);
+      int& fmax = fn_smem[(const void*)fn];        // the attribute is per function: keep it at the largest request
+      if (lsmem > fmax) {
+        fmax = lsmem;
+        CU(cudaFuncSetAttribute((const void*)fn, cudaFuncAttributeMaxDynamicSharedMemorySize, std::max(lsmem, 1024)));
+      }
+      if (!launches2.empty() && launches2.back().fn == fn) {
+        launches2.back().count++;
+        launches2.back().smem = std::max(launches2.back().smem, lsmem);
+        continue;
+      }
+      launches2.push_back({g, 1, fn, lsmem});
       cudaFuncAttributes f1;
       CU(cudaFuncGetAttributes(&f1, (const void*)fn));
       if (f1.numRegs >= fa.numRegs) fa = f1;
@@ -748,7 +766,7 @@ struct DeviceImpl : DeviceSide {
         P2.sample_base = P.sample_base;
         for (const Launch2& l : launches2) {
           P2.group0 = l.g0;
-          if (sw->clu == 1) { l.fn<<<l.count, threads, smem, st>>>(P2); continue; }
+          if (sw->clu == 1) { l.fn<<<l.count, threads, l.smem, st>>>(P2); continue; }
           cudaLaunchConfig_t lc;
           std::memset(&lc, 0, sizeof lc);
           lc.gridDim = dim3((unsigned)(l.count * sw->clu)); lc.blockDim = dim3((unsigned)threads);

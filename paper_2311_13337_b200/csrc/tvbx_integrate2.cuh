@@ -272,7 +272,11 @@ __device__ __forceinline__ void gather_class_vec8(const Edge8* edges, int e, int
 // blockDim = (regions of the CTA)*SPC rounded up to whole warps (<= K2_MAXT); lanes past the last node replay it,
 // stores suppressed.
 // VEC (with CLU, GCE == 8): quad ring layout and vector gather, see gather_class_vec.
-template <int SPC, bool SMEMTAB, int GCE, bool CLU, bool VEC = false>
+// SRING (short delays: the group's whole ring fits next to the table): the ring lives in SHARED memory for the
+// launch -- copied in at the start, back at the end (resumable) -- so the per-chunk gathers that a short minimum
+// delay leaves unpipelined (rows longer than PVN / GCE edges, every step when CH = 1) cost a shared-memory
+// round trip instead of an L2 one (cfg 3, v >= 32 m/s).
+template <int SPC, bool SMEMTAB, int GCE, bool CLU, bool VEC = false, bool SRING = false>
 __global__ void __launch_bounds__(K2_MAXT, 1) integrate2_kernel(const __grid_constant__ Integrate2Params P) {
   extern __shared__ __align__(16) unsigned char smem_raw[];
   constexpr int RS = SPC;                         // simulation columns of a ring slot
@@ -304,6 +308,12 @@ __global__ void __launch_bounds__(K2_MAXT, 1) integrate2_kernel(const __grid_con
   Edge8* const s_edges8 = reinterpret_cast<Edge8*>(tab);           // (VEC: 8-byte entries instead)
   int32_t* const s_rowptr = reinterpret_cast<int32_t*>(s_edges + n_stage);
   const Edge<float>* const g_edges = P.edges + td.edge_off + rp0;
+  float* s_ring = nullptr;                                          // SRING: [N][Hs][SPC] behind the row pointers
+  if (SRING) {
+    uintptr_t a = reinterpret_cast<uintptr_t>(s_rowptr + N + 1);
+    a = (a + 15) & ~(uintptr_t)15;
+    s_ring = reinterpret_cast<float*>(a);
+  }
   {
     if (tid < NBAR) mbar_init(bar_done + tid, (uint32_t)(T >> 5) * nrank);
     for (int i = tid; i < NP2 * SPC; i += T) s_ps[i] = P.psim2[(size_t)g * NP2 * SPC + i];
@@ -321,6 +331,11 @@ __global__ void __launch_bounds__(K2_MAXT, 1) integrate2_kernel(const __grid_con
       }
       if (!CLU) for (int i = tid; i <= N; i += T) s_rowptr[i] = g_rowptr[i];
     }
+    if (SRING) {
+      const float* gr = P.ring + gd.ring_off;
+      const int nr = N * Hs * RS;
+      for (int i = tid; i < nr; i += T) s_ring[i] = gr[i];
+    }
     if (CLU) cluster_sync_all(); else __syncthreads();      // (remote arrivals need the peers' barriers initialised)
   }
   const bool noise = P.noise_on != 0;
@@ -328,7 +343,7 @@ __global__ void __launch_bounds__(K2_MAXT, 1) integrate2_kernel(const __grid_con
   const int node = active ? tid : NODES - 1;
   const int kl = node / SPC, sl = node - kl * SPC, k = k0 + kl;
   s_ps += sl;
-  float* const ringg = P.ring + gd.ring_off + (VEC ? 4 * sl : sl);   // this group's ring, the thread's simulation column
+  float* const ringg = (SRING ? s_ring : P.ring + gd.ring_off) + (VEC ? 4 * sl : sl);   // this group's ring, the thread's simulation column
   const int e_last = n_stage - 1;
   const uint32_t myrow = (uint32_t)(k * Hs) * (uint32_t)RS;
   const int loc = P.loc_id[(size_t)g * SPC + sl];
@@ -575,6 +590,12 @@ __global__ void __launch_bounds__(K2_MAXT, 1) integrate2_kernel(const __grid_con
     n += ch;
   }
   if (CLU) cluster_sync_all();                    // no CTA leaves while a peer may still arrive on its barriers
+  if (SRING) {                                    // the ring goes back to global memory for the next launch
+    __syncthreads();
+    float* gr = P.ring + gd.ring_off;
+    const int nr = N * Hs * RS;
+    for (int i = tid; i < nr; i += T) gr[i] = s_ring[i];
+  }
   if (active) {
     sp[0] = nu.x; sp[stride] = nu.y; sp[2 * stride] = Cs.x; sp[3 * stride] = Cei; sp[4 * stride] = Cs.y;
     sp[5 * stride] = W.x; sp[6 * stride] = W.y; sp[7 * stride] = ou; sp[8 * stride] = win.x; sp[9 * stride] = win.y;
