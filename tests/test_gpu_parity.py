@@ -495,3 +495,68 @@ def test_fc_scores_errors_and_degenerate():
         sw.fc_scores(ref_fc=bad)
     const = sw.fc_scores(ref_fc=np.full((12, 12), 0.5))
     assert const["fitness"][0] == 0.0                    # zero-variance reference -> 0 (A18 / A23)
+
+
+# ------------------------------------------------------------------------------------ more edge cases
+@pytest.mark.parametrize("v", [30.0, 120.0], ids=["ch2", "ch1"])
+def test_short_delay_classes_ring_in_shared_memory(v):
+    """Minimum delays of a few steps: 2-slot gather instances with the history ring staged in shared memory
+    (SRING).  Parity with the oracle with and without noise, and run(a); run(b) == run(a + b) bit for bit --
+    the ring must survive the copy back to global memory between launches."""
+    W, L = wl.connectome(40, seed=12, keep=0.4)
+    cfg = dict(axes=[dict(name="G", lo=0.1, hi=0.5, n=5, values=None)], fixed=dict(v=v, b_e=40.0, wNoise=1e-4), seed=6)
+    sw, traj, o, ref = run_pair(cfg, W, L, 900, True, traj_steps=900, discard=100)
+    assert sw.kernel_name() == "tvbx::integrate2_kernel" and sw.ring_len(0)[0] <= 80
+    assert traj_err(traj, ref) < 5e-3          # same Philox stream; FP32 rounding amplified by the noise path
+    fc, me, mi = sw.fc_readout(); rfc, rme, rmi = o.fc_readout()
+    assert np.abs(me / rme - 1).max() < TOL_MEAN_REL and np.abs(fc - rfc).max() < TOL_FC_ABS
+    sw2, traj2, o2, ref2 = run_pair(cfg, W, L, 900, False, traj_steps=900)
+    assert traj_err(traj2, ref2) < TOL_TRAJ_F32
+    _, a = tvbx.sweep_from_config(cfg, W, L, chunk_samples=16)
+    _, b = tvbx.sweep_from_config(cfg, W, L, chunk_samples=16)
+    a.run(703, 0.1, noise_on=True, ds=10, discard_steps=95)
+    for part in (1, 298, 7, 397):
+        b.run(part, 0.1, noise_on=True, ds=10, discard_steps=95)
+    ya, oa = a.state(); yb, ob = b.state()
+    np.testing.assert_array_equal(ya, yb); np.testing.assert_array_equal(oa, ob)
+    for x, y in zip(a.fc_readout(), b.fc_readout()):
+        np.testing.assert_array_equal(x, y)
+
+
+def test_single_region_and_rows_without_edges():
+    """N = 1 (no edge at all) and a connectome in which some regions receive nothing: the coupling sum is 0 there."""
+    cfg = dict(axes=[dict(name="b_e", lo=0.0, hi=60.0, n=3, values=None)], fixed=dict(G=0.4, v=4.0), seed=2)
+    W1, L1 = np.zeros((1, 1)), np.zeros((1, 1))
+    sw, traj, o, ref = run_pair(cfg, W1, L1, 500, False, traj_steps=500)
+    assert traj.shape == (3, 500, 7, 1) and traj_err(traj, ref) < TOL_TRAJ_F32
+    W, L = wl.connectome(9, seed=4, keep=0.5)
+    W[2, :] = 0.0; W[7, :] = 0.0                  # regions 2 and 7 have no incoming edge (W need not be symmetric)
+    sw, traj, o, ref = run_pair(cfg, W, L, 500, True, traj_steps=500, discard=100, params=dict(wNoise=1e-4))
+    assert traj_err(traj, ref) < 5e-3
+    fc, me, mi = sw.fc_readout(); rfc, rme, rmi = o.fc_readout()
+    assert np.abs(fc - rfc).max() < TOL_FC_ABS
+
+
+def test_zero_steps_and_memory_pool():
+    W, L = wl.connectome(16, seed=3, keep=0.5)
+    cfg = dict(axes=[dict(name="G", lo=0.0, hi=0.3, n=4, values=None)], fixed=dict(v=4.0, wNoise=1e-4), seed=5)
+    tvbx.trim_memory()
+    _, a = tvbx.sweep_from_config(cfg, W, L)
+    a.run(0, 0.1, noise_on=True, ds=10)           # allocates, advances nothing
+    assert a.steps_done() == 0 and a.samples_kept() == 0
+    a.run(400, 0.1, noise_on=True, ds=10)
+    ra = a.fc_readout()
+    a.close()
+    freed_probe = tvbx.trim_memory()
+    assert freed_probe > 0                        # the destroyed sweep's buffers were waiting in the pool
+    _, b = tvbx.sweep_from_config(cfg, W, L)      # fresh buffers
+    b.run(400, 0.1, noise_on=True, ds=10)
+    rb = b.fc_readout()
+    b.close()
+    _, c = tvbx.sweep_from_config(cfg, W, L)      # recycled buffers: same results, no stale state
+    c.run(400, 0.1, noise_on=True, ds=10)
+    rc = c.fc_readout()
+    for x, y, z in zip(ra, rb, rc):
+        np.testing.assert_array_equal(x, y); np.testing.assert_array_equal(y, z)
+    c.close()
+    assert tvbx.trim_memory() > 0 and tvbx.trim_memory() == 0
