@@ -45,6 +45,13 @@ KERNEL_FLOPS_BASE = 757.0
 # (dram__bytes_read.sum + dram__bytes_write.sum of a 2,000-step launch of cfg 2 / its region-steps)
 NCU_DRAM_BYTES_PER_REGION_STEP = {2: 25.4}
 FLOPS_PER_EDGE = 2.0
+# the same capture's pipe counters (profiles/r1_integrate2_kernel_cfg2_ncu.txt): what the north star asks to be judged
+# "as measured by ncu" -- reported beside the algorithmic fraction, never instead of it
+NCU_CFG2 = {"source": "profiles/r1_integrate2_kernel_cfg2_ncu.txt",
+            "sm__pipe_fma_cycles_active.avg.pct_of_peak_sustained_active": 61.1,
+            "smsp__issue_active.avg.pct_of_peak_sustained_active": 62.0,
+            "sm__throughput.avg.pct_of_peak_sustained_elapsed": 63.9,
+            "lts__t_sector_hit_rate.pct": 70.0, "gpu__dram_throughput.avg.pct_of_peak_sustained_elapsed": 11.5}
 SM_COUNT, LANES_PER_SM = 148, 128
 
 
@@ -318,6 +325,8 @@ def run_tvbx(args):
                 "kernel_share_of_step": int_ms / ms if ms > 0 else None,
                 "hbm_peak_gbs": pk.get("hbm_gbs"),
                 "other_kernels_ms": {k: prof[k][0] for k in ("fc", "readout", "reset")}}
+        if args.config == 2:
+            roof["ncu"] = NCU_CFG2
         line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
                 "ms_per_step": ms_max / args.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
                 "dtype": "f32", "data": "synthetic",
