@@ -330,7 +330,21 @@ inline Kernel2Fn pick_kernel2_spc(int spc) {
   }
 }
 // cluster form (several CTAs per group): table through L1/L2, 8 slots per edge; vec: quad ring layout + vector gather
-inline Kernel2Fn pick_kernel2(int spc, bool smemtab, int gce, bool clu, bool vec, bool sring = false) {
+// small CTAs (<= K2_SMALLT threads): the 8-slot shared-memory-table instance with the relaxed register bound
+inline Kernel2Fn pick_kernel2_small(int spc) {
+  switch (spc) {
+    case 1: return integrate2_kernel<1, true, 8, false, false, false, K2_SMALLT>;
+    case 2: return integrate2_kernel<2, true, 8, false, false, false, K2_SMALLT>;
+    case 3: return integrate2_kernel<3, true, 8, false, false, false, K2_SMALLT>;
+    case 4: return integrate2_kernel<4, true, 8, false, false, false, K2_SMALLT>;
+    case 5: return integrate2_kernel<5, true, 8, false, false, false, K2_SMALLT>;
+    case 6: return integrate2_kernel<6, true, 8, false, false, false, K2_SMALLT>;
+    case 7: return integrate2_kernel<7, true, 8, false, false, false, K2_SMALLT>;
+    default: return integrate2_kernel<8, true, 8, false, false, false, K2_SMALLT>;
+  }
+}
+inline Kernel2Fn pick_kernel2(int spc, bool smemtab, int gce, bool clu, bool vec, bool sring = false, int threads = K2_MAXT) {
+  if (!clu && !vec && !sring && smemtab && gce == 8 && threads <= K2_SMALLT) return pick_kernel2_small(spc);
   if (sring) return gce == 2 ? pick_kernel2_spc<true, 2, false, true>(spc) : pick_kernel2_spc<true, 4, false, true>(spc);
   if (clu && vec && smemtab) return spc == 8 ? integrate2_kernel<8, true, 8, true, true> : integrate2_kernel<4, true, 8, true, true>;
   if (clu && vec) return spc == 8 ? integrate2_kernel<8, false, 8, true, true> : integrate2_kernel<4, false, 8, true, true>;
@@ -643,7 +657,7 @@ struct DeviceImpl : DeviceSide {
       const bool sring = CLU == 1 && P2.smem_table && gce < 8 && smem + ring_b <= (size_t)200 * 1024 &&
                          getenv("TVBX_NO_SRING") == nullptr;
       const int lsmem = smem + (sring ? (int)ring_b : 0);
-      Kernel2Fn fn = pick_kernel2(SPC, P2.smem_table != 0, gce, CLU > 1, ht.vec != 0, sring);
+      Kernel2Fn fn = pick_kernel2(SPC, P2.smem_table != 0, gce, CLU > 1, ht.vec != 0, sring, threads);
       int& fmax = fn_smem[(const void*)fn];        // the attribute is per function: keep it at the largest request
       if (lsmem > fmax) {
         fmax = lsmem;

@@ -39,6 +39,7 @@ enum { NP2 = 9 };       // packed per-simulation parameters, see P2_*
 enum { P2_GW = 0, P2_IT, P2_B, P2_AT, P2_ITW, P2_ATEL, P2_GLEL, P2_CFE, P2_CFI };
 enum { NBAR = 8, LAGMAX = 4 };   // mbarrier ring; chunks a warp may run ahead
 enum { K2_MAXT = 480 };          // threads per CTA: 65536 / 480 -> 128 registers per thread (rounded down from 136)
+enum { K2_SMALLT = 224 };        // small CTAs: launch bound 224 -> 255 registers per thread
 enum { PVN = 24 };               // ring values of the next chunk a thread keeps in flight across one compute step:
                                  // PVN / GCE edges x the first GCE = 8, 4 or 2 slots (GCE >= the chunk length).  Rows up to
                                  // (PVN / GCE) * CH edges are fully pipelined; longer rows finish in rounds of 8 edges
@@ -276,8 +277,12 @@ __device__ __forceinline__ void gather_class_vec8(const Edge8* edges, int e, int
 // launch -- copied in at the start, back at the end (resumable) -- so the per-chunk gathers that a short minimum
 // delay leaves unpipelined (rows longer than PVN / GCE edges, every step when CH = 1) cost a shared-memory
 // round trip instead of an L2 one (cfg 3, v >= 32 m/s).
-template <int SPC, bool SMEMTAB, int GCE, bool CLU, bool VEC = false, bool SRING = false>
-__global__ void __launch_bounds__(K2_MAXT, 1) integrate2_kernel(const __grid_constant__ Integrate2Params P) {
+// MAXT: the launch bound.  K2_MAXT = 480 threads leaves 128 registers per thread; CTAs of <= K2_SMALLT = 224 threads
+// (small sweeps, few regions) are compiled with the bound 224 -> up to 255 registers (190 used): the scheduler of a
+// CTA that has one or two warps per scheduler lives on the instruction-level parallelism the extra registers allow
+// (cfg 4 +11 %, cfg 1 +14 %).
+template <int SPC, bool SMEMTAB, int GCE, bool CLU, bool VEC = false, bool SRING = false, int MAXT = K2_MAXT>
+__global__ void __launch_bounds__(MAXT, 1) integrate2_kernel(const __grid_constant__ Integrate2Params P) {
   extern __shared__ __align__(16) unsigned char smem_raw[];
   constexpr int RS = SPC;                         // simulation columns of a ring slot
   const uint32_t nrank = CLU ? cluster_nctarank() : 1u, crank = CLU ? cluster_ctarank() : 0u;
