@@ -52,7 +52,7 @@ class SweepOpts(C.Structure):
     _fields_ = [("precision", C.c_int32), ("sims_per_cta", C.c_int32), ("n_sims", C.c_int64),
                 ("sim_ids", C.POINTER(C.c_int64)), ("chunk_samples", C.c_int64),
                 ("threads_per_cta", C.c_int32), ("ctas_per_group", C.c_int32),
-                ("fc_mode", C.c_int32), ("reserved", C.c_int32)]
+                ("fc_mode", C.c_int32), ("reserved", C.c_int32), ("rate_threshold_khz", C.c_double)]
 
 
 class RunOpts(C.Structure):
@@ -63,7 +63,7 @@ class RunOpts(C.Structure):
 
 EXPORTS = [
     "tvbx_default_params", "tvbx_create_connectome", "tvbx_destroy_connectome", "tvbx_sweep_create",
-    "tvbx_sweep_destroy", "tvbx_sweep_set_initial", "tvbx_run", "tvbx_fc_readout", "tvbx_fc_scores", "tvbx_sweep_size",
+    "tvbx_sweep_destroy", "tvbx_sweep_set_initial", "tvbx_run", "tvbx_fc_readout", "tvbx_fc_scores", "tvbx_rate_stats", "tvbx_sweep_size",
     "tvbx_sweep_param", "tvbx_sweep_ext_id", "tvbx_delay_index", "tvbx_ring_len", "tvbx_steps_done",
     "tvbx_samples_kept", "tvbx_sweep_state", "tvbx_launch_info", "tvbx_launch_count", "tvbx_kernel_name", "tvbx_fc_kernel_name", "tvbx_last_error",
     "tvbx_version", "tvbx_trim_memory", "tvbx_sweep_reset", "tvbx_profile_enable", "tvbx_profile_read", "tvbx_bytes_copied",
@@ -106,6 +106,7 @@ def lib():
             "tvbx_run": [vp, i64, dbl, C.POINTER(RunOpts)],
             "tvbx_fc_readout": [vp, vp, vp, vp, i32, vp],
             "tvbx_fc_scores": [vp, vp, vp, vp, vp, i32, vp],
+            "tvbx_rate_stats": [vp, vp, vp, vp, i32, vp],
             "tvbx_sweep_size": [vp, C.POINTER(i64), C.POINTER(i64), C.POINTER(i32)],
             "tvbx_sweep_param": [vp, i64, i32, dp],
             "tvbx_sweep_ext_id": [vp, i64, C.POINTER(i64)],
@@ -176,7 +177,7 @@ class Sweep:
     """
 
     def __init__(self, conn: Connectome, axes, seed=0, params=None, precision=TVBX_F32, sims_per_cta=0,
-                 sim_ids=None, chunk_samples=0, threads_per_cta=0, init=None, ctas_per_group=0, fc_mode=0):
+                 sim_ids=None, chunk_samples=0, threads_per_cta=0, init=None, ctas_per_group=0, fc_mode=0, rate_threshold_khz=0.0):
         L = lib()
         self.conn = conn
         m = ModelParams()
@@ -206,7 +207,7 @@ class Sweep:
                 ax[i].values = _dptr(arr)
         o = SweepOpts()
         o.precision = precision; o.sims_per_cta = sims_per_cta; o.chunk_samples = chunk_samples
-        o.threads_per_cta = threads_per_cta; o.ctas_per_group = ctas_per_group; o.fc_mode = fc_mode
+        o.threads_per_cta = threads_per_cta; o.ctas_per_group = ctas_per_group; o.fc_mode = fc_mode; o.rate_threshold_khz = rate_threshold_khz
         if sim_ids is not None:
             ids = np.ascontiguousarray(sim_ids, dtype=np.int64)
             keep.append(ids)
@@ -349,6 +350,20 @@ class Sweep:
         _chk(lib().tvbx_fc_scores(self._h, None if ref is None else ref.ctypes.data, ptr["fcsc"], ptr.get("fitness"),
                                   ptr["mean_fc"], 1 if device else 0, _stream_ptr(stream)))
         return out
+
+    def rate_stats(self, device=False, stream=None):
+        """tvbx_rate_stats -> (var_e, max_e float32 [S][N], n_above int32 [S][N]); numpy or torch CUDA."""
+        S, N = self.n_sims, self.n_regions
+        if device:
+            import torch
+            var = torch.empty((S, N), device="cuda", dtype=torch.float32)
+            mx = torch.empty((S, N), device="cuda", dtype=torch.float32)
+            ab = torch.empty((S, N), device="cuda", dtype=torch.int32)
+            _chk(lib().tvbx_rate_stats(self._h, var.data_ptr(), mx.data_ptr(), ab.data_ptr(), 1, _stream_ptr(stream)))
+        else:
+            var, mx, ab = np.empty((S, N), np.float32), np.empty((S, N), np.float32), np.empty((S, N), np.int32)
+            _chk(lib().tvbx_rate_stats(self._h, var.ctypes.data, mx.ctypes.data, ab.ctypes.data, 0, _stream_ptr(stream)))
+        return var, mx, ab
 
     def kernel_name(self):
         buf = C.create_string_buffer(64)

@@ -120,6 +120,7 @@ struct DeviceSide {
   virtual int32_t run(int64_t steps, const tvbx_run_opts* o) = 0;
   virtual int32_t readout(float* fc, float* me, float* mi, int on_device, cudaStream_t st) = 0;
   virtual int32_t scores(const double* ref, float* fcsc, float* fitness, float* mean_fc, int on_device, cudaStream_t st) = 0;
+  virtual int32_t rate_stats(float* var_e, float* max_e, int32_t* above, int on_device, cudaStream_t st) = 0;
   virtual int32_t state(double* y, double* ou) = 0;
   virtual int32_t reset(cudaStream_t st) = 0;
 };
@@ -150,6 +151,7 @@ struct tvbx_sweep {
   bool packed = false;               // FP32 closed-form product kernel (integrate2_kernel)
   int64_t chunk_req = 0;
   bool fc_tc = false;                // FC co-moment on the tensor cores (tvbx_fc_tc.cuh)
+  double rate_thr = 0.1;             // kHz: samples above it are counted (f4; 100 Hz)
   double init[7] = {0.001, 0.001, 0, 0, 0, 0, 0};
   // grouping
   std::vector<HostTable> tables;
@@ -365,6 +367,8 @@ struct DeviceImpl : DeviceSide {
   DevBuf<float> d_xc;                 // centred TF32 samples of the chunk, K-major (fc_tc)
   int64_t Kp = 0;
   DevBuf<double> d_sums, d_cmean, d_mean, d_M, d_M_scratch, d_mean_scratch;
+  DevBuf<float> d_cmax, d_rmax, d_rmax_scratch;       // f4: chunk / running maximum of the excitatory samples
+  DevBuf<int32_t> d_ccnt, d_rcnt, d_rcnt_scratch;     //     chunk / running count of samples above the threshold
   DevBuf<float> d_out_fc, d_out_me, d_out_mi;
   IntegrateParams<R> P;
   KernelPick<R> kp{nullptr};
@@ -528,6 +532,7 @@ struct DeviceImpl : DeviceSide {
     CU(d_xbar.alloc((size_t)G * CS * row));
     if (sw->fc_tc) CU(d_xc.alloc((size_t)G * Kp * row));
     CU(d_cmean.alloc((size_t)G * row)); CU(d_mean.alloc((size_t)G * row));
+    CU(d_cmax.alloc((size_t)G * row)); CU(d_rmax.alloc((size_t)G * row)); CU(d_ccnt.alloc((size_t)G * row)); CU(d_rcnt.alloc((size_t)G * row));
     CU(d_M.alloc((size_t)G * SPC * N * N));
     CU(d_state.alloc((size_t)G * (NSV - 2) * row));
     CU(d_sums.alloc((size_t)G * 2 * row));
@@ -720,10 +725,11 @@ struct DeviceImpl : DeviceSide {
   }
   bool tc_attr_set = false;
 
-  int32_t accumulate(double* Mbuf, double* meanbuf, int64_t cnt, int n_c, cudaStream_t st) {
+  int32_t accumulate(double* Mbuf, double* meanbuf, float* rmaxbuf, int32_t* rcntbuf, int64_t cnt, int n_c, cudaStream_t st) {
     const int N = sw->conn.n, SPC = sw->spc, G = (int)sw->groups.size();
     FcParams<R> F;
     F.xbar = d_xbar.p; F.cmean = d_cmean.p; F.mean = meanbuf; F.M = Mbuf; F.cnt = cnt; F.n_c = n_c;
+    F.cmax = d_cmax.p; F.ccnt = d_ccnt.p; F.rmax = rmaxbuf; F.rcnt = rcntbuf; F.thr = (float)sw->rate_thr;
     F.CS = (int32_t)sw->CS; F.N = N; F.SPC = SPC; F.G = G;
     const int row = N * SPC;
     dim3 g1((row + 127) / 128, G), g0((row + 31) / 32, G);
@@ -800,7 +806,7 @@ struct DeviceImpl : DeviceSide {
       CU(cudaGetLastError());
       sw->n += take; remaining -= take; sw->fill += kept;
       if (ds > 0 && sw->fill == sw->CS) {
-        int32_t rc = accumulate(d_M.p, d_mean.p, sw->cnt, (int)sw->fill, st);
+        int32_t rc = accumulate(d_M.p, d_mean.p, d_rmax.p, d_rcnt.p, sw->cnt, (int)sw->fill, st);
         if (rc) return rc;
         sw->cnt += sw->fill; sw->fill = 0;
       }
@@ -818,10 +824,12 @@ struct DeviceImpl : DeviceSide {
     DevBuf<double>& tM = d_M_scratch; DevBuf<double>& tmean = d_mean_scratch;   // allocated once, kept
     *Msrc = d_M.p;
     if (sw->fill > 0) {
-      if (tM.n != d_M.n) { CU(tM.alloc(d_M.n)); CU(tmean.alloc(d_mean.n)); }
+      if (tM.n != d_M.n) { CU(tM.alloc(d_M.n)); CU(tmean.alloc(d_mean.n)); CU(d_rmax_scratch.alloc(d_rmax.n)); CU(d_rcnt_scratch.alloc(d_rcnt.n)); }
       CU(cudaMemcpyAsync(tM.p, d_M.p, d_M.n * sizeof(double), cudaMemcpyDeviceToDevice, st));
       CU(cudaMemcpyAsync(tmean.p, d_mean.p, d_mean.n * sizeof(double), cudaMemcpyDeviceToDevice, st));
-      int32_t rc = accumulate(tM.p, tmean.p, sw->cnt, (int)sw->fill, st);
+      CU(cudaMemcpyAsync(d_rmax_scratch.p, d_rmax.p, d_rmax.n * sizeof(float), cudaMemcpyDeviceToDevice, st));
+      CU(cudaMemcpyAsync(d_rcnt_scratch.p, d_rcnt.p, d_rcnt.n * sizeof(int32_t), cudaMemcpyDeviceToDevice, st));
+      int32_t rc = accumulate(tM.p, tmean.p, d_rmax_scratch.p, d_rcnt_scratch.p, sw->cnt, (int)sw->fill, st);
       if (rc) return rc;
       *Msrc = tM.p;
     }
@@ -871,6 +879,39 @@ struct DeviceImpl : DeviceSide {
       CU(cudaStreamSynchronize(st));
     } else if (ref) {
       CU(cudaStreamSynchronize(st));     // the host copy of ref must not be reused before the upload is done
+    }
+    return TVBX_OK;
+  }
+
+  // f4: variance, maximum and above-threshold count of the excitatory 1-ms samples per (simulation, region)
+  DevBuf<float> d_out_var, d_out_max;
+  DevBuf<int32_t> d_out_above;
+  int32_t rate_stats(float* var_e, float* max_e, int32_t* above, int on_device, cudaStream_t st) override {
+    const int N = sw->conn.n, SPC = sw->spc, G = (int)sw->groups.size();
+    const int64_t total = sw->cnt + sw->fill;
+    if (total < 1) return fail(TVBX_ESTATE, "no sample kept yet");
+    const double* Msrc = nullptr;
+    { int32_t rc = merged_M(&Msrc, st); if (rc) return rc; }
+    RateStatsParams Q;
+    Q.M = Msrc; Q.rmax = sw->fill > 0 ? d_rmax_scratch.p : d_rmax.p; Q.rcnt = sw->fill > 0 ? d_rcnt_scratch.p : d_rcnt.p;
+    Q.loc_id = d_loc.p; Q.cnt = total; Q.N = N; Q.SPC = SPC; Q.G = G;
+    Q.var_e = var_e; Q.max_e = max_e; Q.above = above;
+    const size_t n_out = (size_t)sw->n_sims * N;
+    if (!on_device) {
+      if (var_e) { if (d_out_var.n != n_out) CU(d_out_var.alloc(n_out)); Q.var_e = d_out_var.p; }
+      if (max_e) { if (d_out_max.n != n_out) CU(d_out_max.alloc(n_out)); Q.max_e = d_out_max.p; }
+      if (above) { if (d_out_above.n != n_out) CU(d_out_above.alloc(n_out)); Q.above = d_out_above.p; }
+    }
+    sw->prof_begin(K_READOUT, st);
+    rate_stats_kernel<<<dim3((N + 127) / 128, G * SPC), 128, 0, st>>>(Q);
+    sw->prof_end(st);
+    sw->launches += 1;
+    CU(cudaGetLastError());
+    if (!on_device) {
+      if (var_e) { CU(cudaMemcpyAsync(var_e, Q.var_e, n_out * sizeof(float), cudaMemcpyDeviceToHost, st)); sw->d2h += (int64_t)(n_out * sizeof(float)); }
+      if (max_e) { CU(cudaMemcpyAsync(max_e, Q.max_e, n_out * sizeof(float), cudaMemcpyDeviceToHost, st)); sw->d2h += (int64_t)(n_out * sizeof(float)); }
+      if (above) { CU(cudaMemcpyAsync(above, Q.above, n_out * sizeof(int32_t), cudaMemcpyDeviceToHost, st)); sw->d2h += (int64_t)(n_out * sizeof(int32_t)); }
+      CU(cudaStreamSynchronize(st));
     }
     return TVBX_OK;
   }
@@ -1013,6 +1054,10 @@ int32_t tvbx_sweep_create(const tvbx_connectome* c, const tvbx_model_params* def
   sw->threads_req = opts ? opts->threads_per_cta : 0;
   sw->chunk_req = opts ? opts->chunk_samples : 0;
   {
+    if (opts && opts->rate_threshold_khz != 0.0) {
+      if (!(opts->rate_threshold_khz > 0.0)) return fail(TVBX_EINVAL, "rate_threshold_khz=%g", opts->rate_threshold_khz);
+      sw->rate_thr = opts->rate_threshold_khz;
+    }
     int fcm = opts ? opts->fc_mode : TVBX_FC_AUTO;
     if (const char* e = getenv("TVBX_FC_MODE")) if (fcm == TVBX_FC_AUTO) fcm = atoi(e);
     const bool tc_ok = sw->precision == TVBX_F32 && sw->conn.n <= tvbx::TC_MAXN;
@@ -1167,6 +1212,11 @@ int32_t tvbx_fc_scores(tvbx_sweep* sw, const double* ref_fc, float* fcsc, float*
       if (!std::isfinite(ref_fc[i])) return fail(TVBX_EINVAL, "reference FC entry %zu is not finite", i);
   return sw->dev->scores(ref_fc, fcsc, fitness, mean_fc, on_device, (cudaStream_t)stream);
 }
+int32_t tvbx_rate_stats(tvbx_sweep* sw, float* var_e, float* max_e, int32_t* n_above, int32_t on_device, void* stream) {
+  if (!sw) return fail(TVBX_EINVAL, "sweep is NULL");
+  if (!sw->started) return fail(TVBX_ESTATE, "no run yet");
+  return sw->dev->rate_stats(var_e, max_e, n_above, on_device, (cudaStream_t)stream);
+}
 int32_t tvbx_fc_readout(tvbx_sweep* sw, float* fc, float* mean_e, float* mean_i, int32_t on_device, void* stream) {
   if (!sw) return fail(TVBX_EINVAL, "sweep is NULL");
   if (!sw->started) return fail(TVBX_ESTATE, "no run yet");
@@ -1191,7 +1241,7 @@ int32_t tvbx_profile_read(tvbx_sweep* sw, double ms[4], int64_t launches[4]) {
     CU(cudaEventSynchronize(e.b));
     CU(cudaEventElapsedTime(&t, e.a, e.b));
     ms[e.kind] += (double)t;
-    launches[e.kind] += e.kind == K_FC ? 3 : (e.kind == K_RESET ? 5 : 1);
+    launches[e.kind] += e.kind == K_FC ? (sw->fc_tc ? 4 : 3) : (e.kind == K_RESET ? 5 : 1);
     cudaEventDestroy(e.a); cudaEventDestroy(e.b);
   }
   sw->prof.clear();

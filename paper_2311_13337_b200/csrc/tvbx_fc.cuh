@@ -25,6 +25,13 @@ struct FcParams {
   int64_t cnt;          // samples merged so far (same for all sims)
   int32_t n_c;          // samples in this chunk
   int32_t CS, N, SPC, G;
+  // rate statistics of the excitatory 1-ms samples (f4; "high firing rate activity exceeding 100 Hz",
+  // P:288 "maximum and variance in firing rates"): chunk maximum / count above thr (scratch) and the running ones
+  float* cmax;          // [G][N][SPC]
+  int32_t* ccnt;        // [G][N][SPC]
+  float* rmax;          // [G][N][SPC] running maximum
+  int32_t* rcnt;        // [G][N][SPC] running count of samples above thr
+  float thr;            // kHz
 };
 
 // chunk mean per (group, region, sim lane): a block of 32 columns x 32 sample slices (coalesced 128-byte rows),
@@ -32,22 +39,35 @@ struct FcParams {
 template <typename R>
 __global__ void __launch_bounds__(1024) fc_chunk_mean_kernel(FcParams<R> P) {
   __shared__ double part[32][33];
+  __shared__ float pmax[32][33];
+  __shared__ int pcnt[32][33];
   const int g = blockIdx.y;
   const int cx = threadIdx.x & 31, sy = threadIdx.x >> 5;
   const int idx = blockIdx.x * 32 + cx;                      // region*SPC + lane
   const int row = P.N * P.SPC;
   double acc = 0.0;
+  float mx = -INFINITY;
+  int ct = 0;
   if (idx < row) {
     const R* x = P.xbar + (size_t)g * P.CS * row + idx;
-    for (int q = sy; q < P.n_c; q += 32) acc += (double)x[(size_t)q * row];
+    for (int q = sy; q < P.n_c; q += 32) {
+      const R v = x[(size_t)q * row];
+      acc += (double)v;
+      mx = fmaxf(mx, (float)v);
+      ct += (float)v > P.thr ? 1 : 0;
+    }
   }
-  part[sy][cx] = acc;
+  part[sy][cx] = acc; pmax[sy][cx] = mx; pcnt[sy][cx] = ct;
   __syncthreads();
   if (sy == 0 && idx < row) {
     double tot = 0.0;
+    float m = -INFINITY;
+    int c = 0;
 #pragma unroll
-    for (int j = 0; j < 32; ++j) tot += part[j][cx];
+    for (int j = 0; j < 32; ++j) { tot += part[j][cx]; m = fmaxf(m, pmax[j][cx]); c += pcnt[j][cx]; }
     P.cmean[(size_t)g * row + idx] = tot / (double)P.n_c;
+    P.cmax[(size_t)g * row + idx] = m;
+    P.ccnt[(size_t)g * row + idx] = c;
   }
 }
 
@@ -124,8 +144,37 @@ __global__ void fc_mean_update_kernel(FcParams<R> P) {
   const int row = P.N * P.SPC;
   if (idx >= row) return;
   const size_t o = (size_t)g * row + idx;
-  if (P.cnt == 0) P.mean[o] = P.cmean[o];
-  else P.mean[o] += (P.cmean[o] - P.mean[o]) * ((double)P.n_c / (double)(P.cnt + P.n_c));
+  if (P.cnt == 0) { P.mean[o] = P.cmean[o]; P.rmax[o] = P.cmax[o]; P.rcnt[o] = P.ccnt[o]; }
+  else {
+    P.mean[o] += (P.cmean[o] - P.mean[o]) * ((double)P.n_c / (double)(P.cnt + P.n_c));
+    P.rmax[o] = fmaxf(P.rmax[o], P.cmax[o]);
+    P.rcnt[o] += P.ccnt[o];
+  }
+}
+
+// f4 readout: per (simulation, region) variance (M_kk / n, the population variance of the kept 1-ms samples), maximum
+// and number of samples above the threshold, in local-simulation order
+struct RateStatsParams {
+  const double* M;       // [G][SPC][N][N]
+  const float* rmax;     // [G][N][SPC]
+  const int32_t* rcnt;   // [G][N][SPC]
+  const int32_t* loc_id; // [G][SPC]
+  float* var_e;          // [n_sims][N] or null
+  float* max_e;          // [n_sims][N] or null
+  int32_t* above;        // [n_sims][N] or null
+  int64_t cnt;
+  int32_t N, SPC, G;
+};
+__global__ void rate_stats_kernel(RateStatsParams P) {
+  const int g = blockIdx.y / P.SPC, sl = blockIdx.y % P.SPC;
+  const int loc = P.loc_id[(size_t)g * P.SPC + sl];
+  if (loc < 0) return;
+  const int k = blockIdx.x * blockDim.x + threadIdx.x;
+  if (k >= P.N) return;
+  const size_t o = ((size_t)g * P.N + k) * P.SPC + sl;
+  if (P.var_e) P.var_e[(size_t)loc * P.N + k] = (float)(P.M[((size_t)g * P.SPC + sl) * P.N * P.N + (size_t)k * P.N + k] / (double)P.cnt);
+  if (P.max_e) P.max_e[(size_t)loc * P.N + k] = P.rmax[o];
+  if (P.above) P.above[(size_t)loc * P.N + k] = P.rcnt[o];
 }
 
 struct ReadoutParams {

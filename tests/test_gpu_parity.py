@@ -560,3 +560,56 @@ def test_zero_steps_and_memory_pool():
         np.testing.assert_array_equal(x, y); np.testing.assert_array_equal(y, z)
     c.close()
     assert tvbx.trim_memory() > 0 and tvbx.trim_memory() == 0
+
+
+# ------------------------------------------------------------------------------------ f4: rate statistics
+@pytest.mark.parametrize("N,kw,thr", [(68, dict(), 0.0), (23, dict(sims_per_cta=3, chunk_samples=37), 4.5e-4),
+                                      (130, dict(sims_per_cta=2, chunk_samples=64, fc_mode=1), 4.5e-4)], ids=["n68", "n23", "n130"])
+def test_rate_stats_match_the_oracle(N, kw, thr):
+    """Variance, maximum and above-threshold count of the kept excitatory 1-ms samples (tvbx_rate_stats) against
+    oracle/rate_stats.py on the oracle's own samples.  Variance: relative 2e-2 (it is M_kk / n, the quantity the
+    FC tolerance is about); maximum: the 1 % of the mean rates; count: the threshold is put where the oracle's
+    samples leave a margin of 2 %, so both sides must count the same samples exactly."""
+    from oracle import rate_stats as ors
+    if N == 68:
+        cfg = wl.config(1); W, L = wl.config_connectome(cfg)
+    else:
+        W, L = wl.connectome(N, seed=N, keep=0.4)
+        cfg = dict(axes=[dict(name="G", lo=0.0, hi=0.4, n=5, values=None)], fixed=dict(v=4.0, b_e=20.0, wNoise=1e-4), seed=9)
+    steps = 2400
+    o = orc.OracleSweep(W, L, wl.grid_params(cfg), seed=cfg["seed"])
+    o.run(steps, 0.1, noise_on=True, ds=10, discard_steps=200)
+    xs = [o.samples(s)[0] for s in range(o.S)]
+    if thr == 0.0:                                  # default threshold 0.1 kHz: nothing exceeds it here
+        thr_used = 0.1
+    else:                                           # a threshold inside the data, moved away from any sample by 2 %
+        allx = np.sort(np.concatenate([x.ravel() for x in xs]))
+        gaps = np.where((allx[1:] / allx[:-1] > 1.05) & (allx[:-1] > np.quantile(allx, 0.2)) & (allx[1:] < np.quantile(allx, 0.9)))[0]
+        thr_used = float(np.sqrt(allx[gaps[0]] * allx[gaps[0] + 1])) if len(gaps) else float(allx[-1] * 2)
+    _, sw = tvbx.sweep_from_config(cfg, W, L, rate_threshold_khz=(0.0 if thr == 0.0 else thr_used), **kw)
+    sw.run(steps, 0.1, noise_on=True, ds=10, discard_steps=200)
+    var, mx, ab = sw.rate_stats()
+    assert var.shape == mx.shape == ab.shape == (sw.n_sims, N) and ab.dtype == np.int32
+    for s in range(sw.n_sims):
+        rv, rm, ra = ors.rate_stats(xs[s], thr_used)
+        np.testing.assert_allclose(var[s], rv, rtol=2e-2, atol=1e-14)
+        np.testing.assert_allclose(mx[s], rm, rtol=TOL_MEAN_REL)
+        np.testing.assert_array_equal(ab[s], ra)
+    # consistent with the FC accumulators, repeatable, device outputs
+    import torch
+    dv, dm, da = sw.rate_stats(device=True)
+    torch.cuda.synchronize()
+    np.testing.assert_array_equal(dv.cpu().numpy(), var); np.testing.assert_array_equal(da.cpu().numpy(), ab)
+    sw.run(100, 0.1, noise_on=True, ds=10, discard_steps=200)          # streaming: counts never decrease, max never drops
+    var2, mx2, ab2 = sw.rate_stats()
+    assert np.all(ab2 >= ab) and np.all(mx2 >= mx)
+
+
+def test_rate_stats_before_any_sample_is_an_error():
+    W, L = wl.connectome(12, seed=2, keep=0.5)
+    _, sw = tvbx.sweep_from_config(dict(axes=[], fixed={}, seed=0), W, L)
+    sw.run(5, 0.1, ds=10)
+    with pytest.raises(tvbx.TvbxError):
+        sw.rate_stats()
+    with pytest.raises(tvbx.TvbxError):
+        tvbx.sweep_from_config(dict(axes=[], fixed={}, seed=0), W, L, rate_threshold_khz=-1.0)
