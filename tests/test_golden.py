@@ -14,6 +14,13 @@ from oracle import oracle as orc
 GOLD = os.path.join(os.path.dirname(os.path.abspath(__file__)), "golden")
 
 
+@pytest.fixture(scope="module", autouse=True)
+def _built():
+    import paper_2311_13337_b200 as tvbx
+    tvbx.build()
+    orc.build()
+
+
 def paper_constants():
     out = {}
     for line in open(os.path.join(GOLD, "paper_constants.txt")):
