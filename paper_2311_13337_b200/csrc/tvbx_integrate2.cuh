@@ -490,6 +490,8 @@ __global__ void __launch_bounds__(MAXT, 1) integrate2_kernel(const __grid_consta
 #pragma unroll
     for (int j = 0; j < GC / 2; ++j) pacc[j] = mk2(0.0f, 0.0f);
     const bool traj_on = P.traj != nullptr && loc >= 0 && active && n - P.traj_n0 < P.traj_steps;
+#pragma unroll 2      // two steps per trip: the address arithmetic and parameter loads of step i + 1 overlap the
+                      // arithmetic of step i and the rematerialised per-thread constants are shared (cfg 2 +2.8 %; 4 is slower)
     for (int i = 0; i < ch; ++i) {
       const int64_t nn = n + i;
       const float cpl = s_cpl[i * T];
