@@ -43,7 +43,10 @@ UNIT = "region-steps/s"
 KERNEL_FLOPS_BASE = 757.0
 # DRAM bytes per region-step of the integrator from the ncu --set full capture in profiles/
 # (dram__bytes_read.sum + dram__bytes_write.sum of a 2,000-step launch of cfg 2 / its region-steps)
-NCU_DRAM_BYTES_PER_REGION_STEP = {2: 25.9}
+NCU_DRAM_BYTES_PER_REGION_STEP = {2: 25.9, 5: 67.3}
+# L2 -> SM bytes per region-step of the cfg-5 capture (l1tex__m_xbar2l1tex_read_bytes.sum / region-steps,
+# profiles/r1_integrate2_kernel_cfg5_cluster_ncu.txt): what the N = 360 gather really moves (722 B algorithmic)
+NCU_L2_BYTES_PER_REGION_STEP = {5: 1075.0}
 FLOPS_PER_EDGE = 2.0
 # the same capture's pipe counters (profiles/r1_integrate2_kernel_cfg2_ncu.txt): what the north star asks to be judged
 # "as measured by ncu" -- reported beside the algorithmic fraction, never instead of it
@@ -327,6 +330,17 @@ def run_tvbx(args):
                 "other_kernels_ms": {k: prof[k][0] for k in ("fc", "readout", "reset")}}
         if args.config == 2:
             roof["ncu"] = NCU_CFG2
+        # the L2 -> SM read bandwidth of this device, measured live (tvbx_probe_read_bandwidth, 64 MiB buffer): the roofline
+        # of the delay gather when the ring is served from L2 (N = 360: 180 edges per row)
+        l2_gbs = tvbx.probe_read_bandwidth(64 << 20, 30)
+        roof["l2_peak_gbs_measured"] = l2_gbs
+        if args.config == 5 and int_ms > 0:
+            alg_bytes = 4.0 * nnz_row + 4.4
+            gather_gbs = alg_bytes * units_per_step * args.steps / (int_ms * 1e-3) / 1e9
+            roof.update({"bound": "l2", "achieved": gather_gbs, "peak": l2_gbs, "unit": "GB/s", "frac": gather_gbs / l2_gbs,
+                         "peak_kind": "L2 -> SM read bandwidth measured in this run (64 MiB buffer, 16-byte ld.global.cg)",
+                         "l2_traffic_gbs_ncu": NCU_L2_BYTES_PER_REGION_STEP[5] * units_per_step * args.steps / (int_ms * 1e-3) / 1e9,
+                         "alu_frac": (achieved / peak_tflops) if achieved else None})
         line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
                 "ms_per_step": ms_max / args.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
                 "dtype": "f32", "data": "synthetic",

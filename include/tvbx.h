@@ -195,6 +195,11 @@ int32_t tvbx_profile_enable(tvbx_sweep* sw, int32_t on);
 int32_t tvbx_profile_read(tvbx_sweep* sw, double ms[4], int64_t launches[4]);
 /* bytes this sweep object copied host->device and device->host so far (tables, parameters, results) */
 int32_t tvbx_bytes_copied(const tvbx_sweep* sw, int64_t* h2d, int64_t* d2h);
+/* Measurement helper (bench.py): read bandwidth of the current device in GB/s, measured by a
+ * read-only kernel that streams a zeroed buffer of `bytes` bytes `passes` times with 16-byte ld.global.cg loads (the
+ * path of the delay gather), CUDA-event timed after a warm-up pass.  A buffer that fits the L2 (e.g. 48 MiB) gives
+ * the L2 -> SM bandwidth -- the roofline of the N = 360 gather --, one several times larger the HBM read bandwidth. */
+int32_t tvbx_probe_read_bandwidth(int64_t bytes, int32_t passes, double* gb_per_s);
 
 /* ---- bookkeeping accessors (bit-exact tests) ------------------------------------------------ */
 int32_t tvbx_sweep_size(const tvbx_sweep* sw, int64_t* n_sims, int64_t* grid_size, int32_t* n_regions);

@@ -66,7 +66,7 @@ EXPORTS = [
     "tvbx_sweep_destroy", "tvbx_sweep_set_initial", "tvbx_run", "tvbx_fc_readout", "tvbx_fc_scores", "tvbx_rate_stats", "tvbx_sweep_size",
     "tvbx_sweep_param", "tvbx_sweep_ext_id", "tvbx_delay_index", "tvbx_ring_len", "tvbx_steps_done",
     "tvbx_samples_kept", "tvbx_sweep_state", "tvbx_launch_info", "tvbx_launch_count", "tvbx_kernel_name", "tvbx_fc_kernel_name", "tvbx_last_error",
-    "tvbx_version", "tvbx_trim_memory", "tvbx_sweep_reset", "tvbx_profile_enable", "tvbx_profile_read", "tvbx_bytes_copied",
+    "tvbx_version", "tvbx_trim_memory", "tvbx_sweep_reset", "tvbx_profile_enable", "tvbx_profile_read", "tvbx_bytes_copied", "tvbx_probe_read_bandwidth",
 ]
 
 
@@ -124,6 +124,7 @@ def lib():
             "tvbx_profile_enable": [vp, i32],
             "tvbx_profile_read": [vp, dp, C.POINTER(i64)],
             "tvbx_bytes_copied": [vp, C.POINTER(i64), C.POINTER(i64)],
+            "tvbx_probe_read_bandwidth": [i64, i32, dp],
         }
         for name, argtypes in sig.items():
             fn = getattr(L, name)
@@ -387,6 +388,13 @@ def _stream_ptr(stream):
     if isinstance(stream, int):
         return stream
     return stream.cuda_stream      # torch.cuda.Stream
+
+
+def probe_read_bandwidth(nbytes: int, passes: int = 20) -> float:
+    """tvbx_probe_read_bandwidth: GB/s of 16-byte ld.global.cg reads over a buffer of nbytes (L2 if it fits, else HBM)."""
+    out = C.c_double()
+    _chk(lib().tvbx_probe_read_bandwidth(int(nbytes), int(passes), C.byref(out)))
+    return out.value
 
 
 def trim_memory() -> int:

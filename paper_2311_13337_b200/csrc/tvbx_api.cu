@@ -268,6 +268,23 @@ struct DevBuf {
   }
 };
 
+// Read-bandwidth probe (tvbx_probe_read_bandwidth): every thread streams 16-byte words of a buffer `passes` times with
+// ld.global.cg (the path of the delay gather's ring loads); a buffer that fits the 126 MB L2 measures the L2 -> SM
+// bandwidth, a larger one the HBM read bandwidth.  The sum is written once so the loads cannot be dropped.
+__global__ void __launch_bounds__(512) read_probe_kernel(const float4* __restrict__ p, size_t n16, int passes, float* sink) {
+  float acc = 0.f;
+  const size_t stride = (size_t)gridDim.x * blockDim.x;
+  for (int it = 0; it < passes; ++it) {
+    size_t i = blockIdx.x * (size_t)blockDim.x + threadIdx.x;
+    for (; i + 3 * stride < n16; i += 4 * stride) {
+      const float4 a = __ldcg(p + i), b = __ldcg(p + i + stride), c = __ldcg(p + i + 2 * stride), d = __ldcg(p + i + 3 * stride);
+      acc += (a.x + a.w) + (b.x + b.w) + (c.x + c.w) + (d.x + d.w);
+    }
+    for (; i < n16; i += stride) { const float4 a = __ldcg(p + i); acc += a.x + a.w; }
+  }
+  if (acc == 12345.678f) *sink = acc;
+}
+
 template <typename R>
 __global__ void fill_kernel(R* p, size_t n, R v) {
   for (size_t i = blockIdx.x * (size_t)blockDim.x + threadIdx.x; i < n; i += (size_t)gridDim.x * blockDim.x) p[i] = v;
@@ -1245,6 +1262,30 @@ int32_t tvbx_profile_read(tvbx_sweep* sw, double ms[4], int64_t launches[4]) {
     cudaEventDestroy(e.a); cudaEventDestroy(e.b);
   }
   sw->prof.clear();
+  return TVBX_OK;
+}
+int32_t tvbx_probe_read_bandwidth(int64_t bytes, int32_t passes, double* gb_per_s) {
+  if (bytes < (1 << 20) || passes < 1 || !gb_per_s) return fail(TVBX_EINVAL, "bytes >= 1 MiB, passes >= 1, gb_per_s != NULL");
+  DevBuf<float4> buf;
+  DevBuf<float> sink;
+  const size_t n16 = (size_t)bytes / 16;
+  CU(buf.alloc(n16)); CU(sink.alloc(1));
+  CU(cudaMemset(buf.p, 0, n16 * 16));
+  int dev = 0, sms = 148;
+  cudaGetDevice(&dev);
+  cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
+  cudaEvent_t a, b;
+  CU(cudaEventCreate(&a)); CU(cudaEventCreate(&b));
+  read_probe_kernel<<<sms * 4, 512>>>(buf.p, n16, 2, sink.p);      // warm-up: the buffer is L2-resident afterwards if it fits
+  CU(cudaEventRecord(a));
+  read_probe_kernel<<<sms * 4, 512>>>(buf.p, n16, passes, sink.p);
+  CU(cudaEventRecord(b));
+  CU(cudaEventSynchronize(b));
+  float ms = 0.f;
+  CU(cudaEventElapsedTime(&ms, a, b));
+  cudaEventDestroy(a); cudaEventDestroy(b);
+  CU(cudaGetLastError());
+  *gb_per_s = (double)n16 * 16.0 * passes / ((double)ms * 1e-3) / 1e9;
   return TVBX_OK;
 }
 int32_t tvbx_bytes_copied(const tvbx_sweep* sw, int64_t* h2d, int64_t* d2h) {

@@ -613,3 +613,12 @@ def test_rate_stats_before_any_sample_is_an_error():
         sw.rate_stats()
     with pytest.raises(tvbx.TvbxError):
         tvbx.sweep_from_config(dict(axes=[], fixed={}, seed=0), W, L, rate_threshold_khz=-1.0)
+
+
+def test_read_bandwidth_probe():
+    """tvbx_probe_read_bandwidth (the measured L2 -> SM peak bench.py reports for the N = 360 gather)."""
+    l2 = tvbx.probe_read_bandwidth(48 << 20, 10)
+    hbm = tvbx.probe_read_bandwidth(1 << 30, 2)
+    assert 1000.0 < hbm < 20000.0 and hbm < l2 < 60000.0      # GB/s: L2-resident reads are faster than HBM reads
+    with pytest.raises(tvbx.TvbxError):
+        tvbx.probe_read_bandwidth(1000, 1)
