@@ -622,3 +622,18 @@ def test_read_bandwidth_probe():
     assert 1000.0 < hbm < 20000.0 and hbm < l2 < 60000.0      # GB/s: L2-resident reads are faster than HBM reads
     with pytest.raises(tvbx.TvbxError):
         tvbx.probe_read_bandwidth(1000, 1)
+
+
+def test_more_regions_than_tmem_columns_falls_back_to_register_tiles():
+    """N > 512: the general integrator (several passes over the regions) and the FP32 register-tile X^T X (the tcgen05
+    kernel holds one output row block in <= 512 TMEM columns); fc_mode = TVBX_FC_TF32 is refused."""
+    N = 520
+    W, L = wl.connectome(N, seed=21, keep=0.05)
+    cfg = dict(axes=[dict(name="G", lo=0.1, hi=0.3, n=2, values=None)], fixed=dict(v=6.0, b_e=30.0, wNoise=1e-4), seed=8)
+    sw, traj, o, ref = run_pair(cfg, W, L, 600, True, traj_steps=600, discard=100)
+    assert sw.kernel_name() == "tvbx::integrate_kernel" and sw.fc_kernel_name() == "tvbx::fc_comoment_kernel"
+    assert traj_err(traj, ref) < 5e-3
+    fc, me, mi = sw.fc_readout(); rfc, rme, rmi = o.fc_readout()
+    assert np.abs(me / rme - 1).max() < TOL_MEAN_REL and np.abs(fc - rfc).max() < TOL_FC_ABS
+    with pytest.raises(tvbx.TvbxError):
+        tvbx.sweep_from_config(cfg, W, L, fc_mode=tvbx.TVBX_FC_TF32)
