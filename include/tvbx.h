@@ -26,7 +26,7 @@
 extern "C" {
 #endif
 
-#define TVBX_VERSION 100 /* 0.1.0 */
+#define TVBX_VERSION 110 /* 0.1.10: + tvbx_fc_scores, tvbx_rate_stats, tvbx_fc_kernel_name, tvbx_trim_memory, tvbx_probe_read_bandwidth */
 
 enum tvbx_status {
   TVBX_OK = 0,

@@ -15,8 +15,10 @@
 //                         4-stage ring in the canonical no-swizzle K-major core-matrix layout, one elected
 //                         thread issues tcgen05.mma (M = 128, N <= 256 per instruction, K = 8 per instruction),
 //                         tcgen05.commit on a per-stage mbarrier frees the stage; the epilogue reads TMEM with
-//                         tcgen05.ld (thread = output row) and adds M_c + delta_k delta_l cnt n_c/(cnt + n_c)
-//                         into the FP64 accumulator rows it owns (coalesced per row, no mirrored writes).
+//                         tcgen05.ld (thread = output row, 32 columns), transposes 32 x 32 blocks through the free
+//                         stage memory and adds M_c + (delta_k delta_l) cnt n_c/(cnt + n_c) into the FP64
+//                         accumulator rows the CTA owns -- one contiguous 256-byte run per warp instruction, every
+//                         element written by exactly one thread (no mirrored or atomic writes).
 #pragma once
 #include <cuda_runtime.h>
 #include <stdint.h>
