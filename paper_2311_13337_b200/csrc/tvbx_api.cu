@@ -948,9 +948,10 @@ struct DeviceImpl : DeviceSide {
       if (me) { if (dme.n != (size_t)sw->n_sims * N) CU(dme.alloc((size_t)sw->n_sims * N)); Q.mean_e = dme.p; }
       if (mi) { if (dmi.n != (size_t)sw->n_sims * N) CU(dmi.alloc((size_t)sw->n_sims * N)); Q.mean_i = dmi.p; }
     }
-    dim3 grid((N * N + 255) / 256, G * SPC);
+    dim3 grid((N + RO_ROWS - 1) / RO_ROWS, G * SPC);
+    Q.diag_in_smem = N <= 4096;
     sw->prof_begin(K_READOUT, st);
-    fc_readout_kernel<<<grid, 256, 0, st>>>(Q);
+    fc_readout_kernel<<<grid, 256, Q.diag_in_smem ? (size_t)N * sizeof(double) : 0, st>>>(Q);
     sw->prof_end(st);
     sw->launches += 1;
     CU(cudaGetLastError());

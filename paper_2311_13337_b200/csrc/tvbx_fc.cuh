@@ -186,32 +186,46 @@ struct ReadoutParams {
   float* mean_i;
   int64_t cnt;
   int32_t N, SPC, G;
+  int32_t diag_in_smem;  // the launch carries N doubles of dynamic shared memory
 };
 
-// Pearson finalise (Eq. 6; A18) in local-simulation order
-__global__ void fc_readout_kernel(ReadoutParams P) {
+// Pearson finalise (Eq. 6; A18) in local-simulation order.  grid (ceil(N / RO_ROWS), G * SPC), 256 threads: a
+// block stages the simulation's N variances in shared memory (the strided M_ll lookups stay on chip) and writes RO_ROWS
+// rows of the matrix; block row 0 also writes the mean rates.
+constexpr int RO_ROWS = 8;
+__global__ void __launch_bounds__(256) fc_readout_kernel(ReadoutParams P) {
+  extern __shared__ double rdiag[];
   const int g = blockIdx.y / P.SPC, sl = blockIdx.y % P.SPC;
   const int loc = P.loc_id[(size_t)g * P.SPC + sl];
   if (loc < 0) return;
-  const double* M = P.M + ((size_t)g * P.SPC + sl) * P.N * P.N;
-  const int NN = P.N * P.N;
-  for (int i = blockIdx.x * blockDim.x + threadIdx.x; i < NN; i += gridDim.x * blockDim.x) {
-    const int k = i / P.N, l = i % P.N;
-    if (P.fc) {
+  const int N = P.N;
+  const double* M = P.M + ((size_t)g * P.SPC + sl) * N * N;
+  const bool staged = P.diag_in_smem != 0;
+  if (P.fc && staged) {
+    for (int k = threadIdx.x; k < N; k += 256) rdiag[k] = M[(size_t)k * N + k];
+    __syncthreads();
+  }
+  const int k0 = blockIdx.x * RO_ROWS;
+  const int nrow = min(RO_ROWS, N - k0);
+  if (P.fc) {
+    for (int i = threadIdx.x; i < nrow * N; i += 256) {
+      const int k = k0 + i / N, l = i % N;
       float r;
       if (k == l) r = 1.0f;
       else {
-        const double den = M[(size_t)k * P.N + k] * M[(size_t)l * P.N + l];
-        double v = (den > 0.0 && isfinite(den)) ? M[i] / sqrt(den) : 0.0;
+        const double den = staged ? rdiag[k] * rdiag[l] : M[(size_t)k * N + k] * M[(size_t)l * N + l];
+        double v = (den > 0.0 && isfinite(den)) ? M[(size_t)k * N + l] / sqrt(den) : 0.0;
         r = isfinite(v) ? (float)fmin(1.0, fmax(-1.0, v)) : 0.0f;   // |rho| <= 1 (Cauchy-Schwarz); FP32 chunk co-moments can round past it
       }
-      P.fc[(size_t)loc * NN + i] = r;
+      P.fc[(size_t)loc * N * N + (size_t)k * N + l] = r;
     }
-    if (l == 0 && blockIdx.x * blockDim.x + threadIdx.x < NN) {
-      const size_t row = (size_t)P.N * P.SPC;
+  }
+  if (blockIdx.x == 0) {
+    const size_t row = (size_t)N * P.SPC;
+    for (int k = threadIdx.x; k < N; k += 256) {
       const double* s = P.sums + (size_t)g * 2 * row + (size_t)k * P.SPC + sl;
-      if (P.mean_e) P.mean_e[(size_t)loc * P.N + k] = (float)(s[0] / (double)P.cnt);
-      if (P.mean_i) P.mean_i[(size_t)loc * P.N + k] = (float)(s[row] / (double)P.cnt);
+      if (P.mean_e) P.mean_e[(size_t)loc * N + k] = (float)(s[0] / (double)P.cnt);
+      if (P.mean_i) P.mean_i[(size_t)loc * N + k] = (float)(s[row] / (double)P.cnt);
     }
   }
 }
