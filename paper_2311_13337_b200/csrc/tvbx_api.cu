@@ -448,7 +448,7 @@ struct DeviceImpl : DeviceSide {
               ed.w = (R)c.edges[e].w;
               ed.jbase = (uint32_t)c.edges[e].j * (uint32_t)Hs * (uint32_t)RS;
               ed.back = back;
-              set_pad(ed, ed.jbase + (back & ~3u) * (uint32_t)RS);
+              set_pad(ed, ed.jbase + (back & ~(tvbx::VW - 1u)) * (uint32_t)RS);
               edges.push_back(ed);
               ++n_class;
             }
@@ -659,7 +659,7 @@ struct DeviceImpl : DeviceSide {
     // LDG.128 = 115 KB; measured at N = 360: 212 KB of shared memory halves the throughput)
     bool clu_tab = CLU > 1 && base + slice_bytes <= (size_t)136 * 1024;
     for (const HostTable& ht : sw->tables)      // field widths of Edge8
-      if (ht.vec && ((int64_t)N * ((ht.Hp + GC) / 4) >= (1 << 20) || ht.Hp / 4 >= (1 << 12))) clu_tab = false;
+      if (ht.vec && ((int64_t)N * ((ht.Hp + GC) / (int)tvbx::VW) >= (1 << 20) || ht.Hp / (int)tvbx::VW >= (1 << 12))) clu_tab = false;
     P2.smem_table = CLU == 1 ? base + tbytes <= 200 * 1024 : clu_tab;
     smem = (int)(base + (CLU == 1 ? (P2.smem_table ? tbytes : 0) : (clu_tab ? slice_bytes : 0)));
     // one launch per run of groups whose chunk length falls in the same class (cfg 3: v <= 8 / 16 / >= 32 m/s)

@@ -196,22 +196,49 @@ __device__ __forceinline__ void gather_rounds(EdgePtr edges, int e, int e1, int 
 // The host pads every class of a row to a multiple of VR entries with zero-weight copies of its last edge, so a
 // round needs neither an index clamp nor a weight mask.  Class 0 windows are quad-aligned: two quads suffice.
 enum { VR = 5 };                 // edges per round of the vector gather (VR x 12 values in registers)
+// Slots per ring word of the vector layout: 4 (quads, LDG.128: 2 or 3 loads per edge-chunk, 44 B fetched on average for the
+// 32 B used) or 2 (pairs, LDG.64: 4 or 5 loads, 36 B).  The N = 360 gather is bound by the L2 -> SM bandwidth, so the
+// bytes count; see DESIGN.md section 7.
+#ifndef TVBX_VEC_W
+#define TVBX_VEC_W 4
+#endif
+constexpr uint32_t VW = TVBX_VEC_W;                 // slots per word
+constexpr uint32_t VWS = TVBX_VEC_W == 4 ? 2 : 1;   // log2
+template <int A> struct VecWords { static constexpr int n = TVBX_VEC_W == 4 ? (A == 0 ? 2 : 3) : ((A & 1) ? 5 : 4); };
+struct VecLd {
+#if TVBX_VEC_W == 4
+  typedef float4 word;
+#else
+  typedef float2 word;
+#endif
+};
+// acc += w * (the VW slots of word q): acc holds f2 pairs of consecutive slots
+__device__ __forceinline__ void vec_fma(f2* acc, int i, float w, const VecLd::word& q) {
+#if TVBX_VEC_W == 4
+  acc[2 * i] = fma2(bc2(w), mk2(q.x, q.y), acc[2 * i]);
+  acc[2 * i + 1] = fma2(bc2(w), mk2(q.z, q.w), acc[2 * i + 1]);
+#else
+  acc[i] = fma2(bc2(w), mk2(q.x, q.y), acc[i]);
+#endif
+}
 template <int RS, int A, typename EdgePtr>
 __device__ __forceinline__ void gather_class_vec(EdgePtr edges, int e, int e1, const float* ringv,
                                                  uint32_t curRS, uint32_t thr, uint32_t wrapRS, float cpl[GC]) {
-  constexpr int NQ = A == 0 ? 2 : 3;
-  f2 acc[2 * NQ];
+  constexpr int NQ = VecWords<A>::n;                      // words fetched per edge
+  constexpr int NA = NQ * (int)VW / 2;                    // f2 accumulators (pairs of consecutive slots)
+  constexpr int A0 = A & ((int)VW - 1);                   // offset of the window inside its first word
+  f2 acc[NA];
 #pragma unroll
-  for (int i = 0; i < 2 * NQ; ++i) acc[i] = mk2(0.0f, 0.0f);
+  for (int i = 0; i < NA; ++i) acc[i] = mk2(0.0f, 0.0f);
   const uint32_t curW = curRS - wrapRS;
   for (; e < e1; e += VR) {
-    float4 q[VR][NQ];
+    VecLd::word q[VR][NQ];
     float w[VR];
 #pragma unroll
     for (int b = 0; b < VR; ++b) {
       const Edge<float> ed = edges[e + b];
       const uint32_t off = ed.pad + (ed.back >= thr ? curW : curRS);
-      const float4* src = reinterpret_cast<const float4*>(ringv + off);
+      const VecLd::word* src = reinterpret_cast<const VecLd::word*>(ringv + off);
 #pragma unroll
       for (int i = 0; i < NQ; ++i) q[b][i] = __ldcg(src + i * RS);
       w[b] = ed.w;
@@ -219,35 +246,34 @@ __device__ __forceinline__ void gather_class_vec(EdgePtr edges, int e, int e1, c
 #pragma unroll
     for (int b = 0; b < VR; ++b) {
 #pragma unroll
-      for (int i = 0; i < NQ; ++i) {
-        acc[2 * i] = fma2(bc2(w[b]), mk2(q[b][i].x, q[b][i].y), acc[2 * i]);
-        acc[2 * i + 1] = fma2(bc2(w[b]), mk2(q[b][i].z, q[b][i].w), acc[2 * i + 1]);
-      }
+      for (int i = 0; i < NQ; ++i) vec_fma(acc, i, w[b], q[b][i]);
     }
   }
 #pragma unroll
-  for (int j = 0; j < GC; ++j) { const int i = A + j; cpl[j] += (i & 1) ? acc[i >> 1].y : acc[i >> 1].x; }
+  for (int j = 0; j < GC; ++j) { const int i = A0 + j; cpl[j] += (i & 1) ? acc[i >> 1].y : acc[i >> 1].x; }
 }
 
 // The same with the 8-byte entries the vector kernels stage in shared memory (Edge8: w and, in one word, the
-// quad-slot index Q = j * Hs/4 + (Hp - d)/4 in the low 20 bits and (Hp - d)/4 in the high 12): half the shared
+// word index Q = j * Hs/VW + (Hp - d)/VW in the low 20 bits and (Hp - d)/VW in the high 12): half the shared
 // memory of the 16-byte entries, which leaves the L1 the room it needs as landing space for the loads in flight.
 struct __align__(8) Edge8 { float w; uint32_t qb; };
 template <int RS, int A>
-__device__ __forceinline__ void gather_class_vec8(const Edge8* edges, int e, int e1, const float4* ring4,
+__device__ __forceinline__ void gather_class_vec8(const Edge8* edges, int e, int e1, const VecLd::word* ringw,
                                                   uint32_t cur4, uint32_t thr4, uint32_t curW4, float cpl[GC]) {
-  constexpr int NQ = A == 0 ? 2 : 3;
-  f2 acc[2 * NQ];
+  constexpr int NQ = VecWords<A>::n;
+  constexpr int NA = NQ * (int)VW / 2;
+  constexpr int A0 = A & ((int)VW - 1);
+  f2 acc[NA];
 #pragma unroll
-  for (int i = 0; i < 2 * NQ; ++i) acc[i] = mk2(0.0f, 0.0f);
+  for (int i = 0; i < NA; ++i) acc[i] = mk2(0.0f, 0.0f);
   for (; e < e1; e += VR) {
-    float4 q[VR][NQ];
+    VecLd::word q[VR][NQ];
     float w[VR];
 #pragma unroll
     for (int b = 0; b < VR; ++b) {
       const Edge8 ed = edges[e + b];
       const uint32_t idx = (ed.qb & 0xFFFFFu) + ((ed.qb >> 20) >= thr4 ? curW4 : cur4);
-      const float4* src = ring4 + (size_t)idx * RS;
+      const VecLd::word* src = ringw + (size_t)idx * RS;
 #pragma unroll
       for (int i = 0; i < NQ; ++i) q[b][i] = __ldcg(src + i * RS);
       w[b] = ed.w;
@@ -255,14 +281,11 @@ __device__ __forceinline__ void gather_class_vec8(const Edge8* edges, int e, int
 #pragma unroll
     for (int b = 0; b < VR; ++b) {
 #pragma unroll
-      for (int i = 0; i < NQ; ++i) {
-        acc[2 * i] = fma2(bc2(w[b]), mk2(q[b][i].x, q[b][i].y), acc[2 * i]);
-        acc[2 * i + 1] = fma2(bc2(w[b]), mk2(q[b][i].z, q[b][i].w), acc[2 * i + 1]);
-      }
+      for (int i = 0; i < NQ; ++i) vec_fma(acc, i, w[b], q[b][i]);
     }
   }
 #pragma unroll
-  for (int j = 0; j < GC; ++j) { const int i = A + j; cpl[j] += (i & 1) ? acc[i >> 1].y : acc[i >> 1].x; }
+  for (int j = 0; j < GC; ++j) { const int i = A0 + j; cpl[j] += (i & 1) ? acc[i >> 1].y : acc[i >> 1].x; }
 }
 
 // SPC: simulations per CTA (1..8); SMEMTAB: the delay table of the group's speed is staged in shared memory;
@@ -324,11 +347,11 @@ __global__ void __launch_bounds__(MAXT, 1) integrate2_kernel(const __grid_consta
     for (int i = tid; i < NP2 * SPC; i += T) s_ps[i] = P.psim2[(size_t)g * NP2 * SPC + i];
     if (SMEMTAB) {
       if (VEC) {
-        const uint32_t qdiv = 4u * (uint32_t)RS;
+        const uint32_t qdiv = VW * (uint32_t)RS;
         for (int i = tid; i < n_stage; i += T) {
           const Edge<float> ed = g_edges[i];
           Edge8 e8;
-          e8.w = ed.w; e8.qb = (ed.pad / qdiv) | ((ed.back >> 2) << 20);
+          e8.w = ed.w; e8.qb = (ed.pad / qdiv) | ((ed.back >> VWS) << 20);
           s_edges8[i] = e8;
         }
       } else {
@@ -348,7 +371,7 @@ __global__ void __launch_bounds__(MAXT, 1) integrate2_kernel(const __grid_consta
   const int node = active ? tid : NODES - 1;
   const int kl = node / SPC, sl = node - kl * SPC, k = k0 + kl;
   s_ps += sl;
-  float* const ringg = (SRING ? s_ring : P.ring + gd.ring_off) + (VEC ? 4 * sl : sl);   // this group's ring, the thread's simulation column
+  float* const ringg = (SRING ? s_ring : P.ring + gd.ring_off) + (VEC ? (int)VW * sl : sl);   // this group's ring, the thread's simulation column
   const int e_last = n_stage - 1;
   const uint32_t myrow = (uint32_t)(k * Hs) * (uint32_t)RS;
   const int loc = P.loc_id[(size_t)g * SPC + sl];
@@ -391,8 +414,8 @@ __global__ void __launch_bounds__(MAXT, 1) integrate2_kernel(const __grid_consta
     for (int j = 0; j < GC; ++j) cpl[j] = 0.0f;
     const uint32_t thr = (uint32_t)(Hp - cur0), curRS = (uint32_t)cur0 * (uint32_t)RS, wrapRS = (uint32_t)Hp * (uint32_t)RS;
     if (SMEMTAB) {
-      const float4* const ring4 = reinterpret_cast<const float4*>(ringg);
-      const uint32_t cur4 = (uint32_t)cur0 >> 2, thr4 = thr >> 2, curW4 = cur4 - ((uint32_t)Hp >> 2);
+      const VecLd::word* const ring4 = reinterpret_cast<const VecLd::word*>(ringg);
+      const uint32_t cur4 = (uint32_t)cur0 >> VWS, thr4 = thr >> VWS, curW4 = cur4 - ((uint32_t)Hp >> VWS);
       gather_class_vec8<RS, 0>(s_edges8, pe0, segk.x, ring4, cur4, thr4, curW4, cpl);
       gather_class_vec8<RS, 1>(s_edges8, segk.x, segk.y, ring4, cur4, thr4, curW4, cpl);
       gather_class_vec8<RS, 2>(s_edges8, segk.y, segk.z, ring4, cur4, thr4, curW4, cpl);
@@ -423,7 +446,7 @@ __global__ void __launch_bounds__(MAXT, 1) integrate2_kernel(const __grid_consta
 #pragma unroll
         for (int j = 0; j < GC; ++j) {
           const uint32_t sj = s0 + (uint32_t)j;
-          acc8[j] = __fmaf_rn(ed.w, __ldcg(ringg + ed.jbase + (sj & ~3u) * (uint32_t)RS + (sj & 3u)), acc8[j]);
+          acc8[j] = __fmaf_rn(ed.w, __ldcg(ringg + ed.jbase + (sj & ~(VW - 1u)) * (uint32_t)RS + (sj & (VW - 1u))), acc8[j]);
         }
       }
 #pragma unroll
@@ -557,7 +580,7 @@ __global__ void __launch_bounds__(MAXT, 1) integrate2_kernel(const __grid_consta
       // ---- S5 ring write: E at time nn+1 (mirror the first GC-1 slots behind the period) ----
       c = c + 1 == Hp ? 0 : c + 1;
       if (active) {
-        const uint32_t o = VEC ? myrow + ((uint32_t)c & ~3u) * (uint32_t)RS + ((uint32_t)c & 3u) : myrow + (uint32_t)c * (uint32_t)RS;
+        const uint32_t o = VEC ? myrow + ((uint32_t)c & ~(VW - 1u)) * (uint32_t)RS + ((uint32_t)c & (VW - 1u)) : myrow + (uint32_t)c * (uint32_t)RS;
         ringg[o] = nu.x;
         if (c < (VEC ? GC : GC - 1)) ringg[o + (uint32_t)Hp * (uint32_t)RS] = nu.x;
       }
