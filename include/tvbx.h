@@ -99,7 +99,10 @@ typedef struct tvbx_sweep_opts {
                              (tcgen05 kind::tf32, samples centred in FP32 before rounding to TF32, FP32 accumulate,
                              FP64 merge) for FP32 sweeps with N <= 512, else FP32/FP64 register tiles;
                              TVBX_FC_FP32 = register tiles always; TVBX_FC_TF32 = tensor cores or TVBX_EINVAL */
-  int32_t reserved;
+  int32_t rate_stats_inhibitory; /* 1: also keep the inhibitory 1-ms samples of the chunk (as much memory again as the
+                                    sample chunk) so that tvbx_rate_stats can return var_i, max_i, n_above_i.  Selects
+                                    the general integrator ("tvbx::integrate_kernel", about 0.65 x the throughput of
+                                    the packed one, which is kept free of the extra store) */
   double rate_threshold_khz; /* tvbx_rate_stats counts the 1-ms excitatory samples above this rate; 0 = 0.1 kHz
                                 ("high firing rate activity exceeding 100 Hz") */
 } tvbx_sweep_opts;
@@ -172,15 +175,18 @@ int32_t tvbx_fc_readout(tvbx_sweep* sw, float* fc, float* mean_e, float* mean_i,
 int32_t tvbx_fc_scores(tvbx_sweep* sw, const double* ref_fc, float* fcsc, float* fitness, float* mean_fc,
                        int32_t on_device, void* stream);
 
-/* Rate statistics of the excitatory population per (simulation, region) over the kept 1-ms samples (the series the
- * FC is computed from; "the maximum and variance in firing rates", P:235 / P:282 activity "exceeding
- * 100 Hz" as the mark of the paroxysmal fixed point; A24):
- *   var_e[s][k]   = population variance (1/n) sum (x - mean)^2   [kHz^2]
- *   max_e[s][k]   = maximum                                      [kHz]
+/* Rate statistics per (simulation, region) over the kept 1-ms samples (the series the FC is computed from; PAPER.md
+ * P:288 "the maximum and variance in firing rates for both excitatory and inhibitory populations", P:235 / P:282
+ * activity "exceeding 100 Hz" as the mark of the paroxysmal fixed point; A24), for the excitatory (_e) and,
+ * if the sweep was created with rate_stats_inhibitory, the inhibitory (_i) population:
+ *   var[s][k]     = population variance (1/n) sum (x - mean)^2   [kHz^2]
+ *   max[s][k]     = maximum                                      [kHz]
  *   n_above[s][k] = number of samples > rate_threshold_khz (a region "visits" the paroxysmal state iff > 0)
  * Outputs n_sims x N, host or device (on_device), any may be NULL; the open chunk is included and the
- * accumulators stay untouched.  TVBX_ESTATE before the first kept sample. */
-int32_t tvbx_rate_stats(tvbx_sweep* sw, float* var_e, float* max_e, int32_t* n_above, int32_t on_device, void* stream);
+ * accumulators stay untouched.  TVBX_ESTATE before the first kept sample; TVBX_EINVAL if an _i output is asked for
+ * without rate_stats_inhibitory. */
+int32_t tvbx_rate_stats(tvbx_sweep* sw, float* var_e, float* max_e, int32_t* n_above_e, float* var_i, float* max_i,
+                        int32_t* n_above_i, int32_t on_device, void* stream);
 
 /* Back to step 0 without re-allocating: state, OU, history ring, window sums and FC accumulators are
  * re-initialised on the device (enqueued on cuda_stream), the step and sample counters are zeroed.

@@ -52,7 +52,7 @@ class SweepOpts(C.Structure):
     _fields_ = [("precision", C.c_int32), ("sims_per_cta", C.c_int32), ("n_sims", C.c_int64),
                 ("sim_ids", C.POINTER(C.c_int64)), ("chunk_samples", C.c_int64),
                 ("threads_per_cta", C.c_int32), ("ctas_per_group", C.c_int32),
-                ("fc_mode", C.c_int32), ("reserved", C.c_int32), ("rate_threshold_khz", C.c_double)]
+                ("fc_mode", C.c_int32), ("rate_stats_inhibitory", C.c_int32), ("rate_threshold_khz", C.c_double)]
 
 
 class RunOpts(C.Structure):
@@ -106,7 +106,7 @@ def lib():
             "tvbx_run": [vp, i64, dbl, C.POINTER(RunOpts)],
             "tvbx_fc_readout": [vp, vp, vp, vp, i32, vp],
             "tvbx_fc_scores": [vp, vp, vp, vp, vp, i32, vp],
-            "tvbx_rate_stats": [vp, vp, vp, vp, i32, vp],
+            "tvbx_rate_stats": [vp, vp, vp, vp, vp, vp, vp, i32, vp],
             "tvbx_sweep_size": [vp, C.POINTER(i64), C.POINTER(i64), C.POINTER(i32)],
             "tvbx_sweep_param": [vp, i64, i32, dp],
             "tvbx_sweep_ext_id": [vp, i64, C.POINTER(i64)],
@@ -178,7 +178,7 @@ class Sweep:
     """
 
     def __init__(self, conn: Connectome, axes, seed=0, params=None, precision=TVBX_F32, sims_per_cta=0,
-                 sim_ids=None, chunk_samples=0, threads_per_cta=0, init=None, ctas_per_group=0, fc_mode=0, rate_threshold_khz=0.0):
+                 sim_ids=None, chunk_samples=0, threads_per_cta=0, init=None, ctas_per_group=0, fc_mode=0, rate_threshold_khz=0.0, rate_stats_inhibitory=False):
         L = lib()
         self.conn = conn
         m = ModelParams()
@@ -208,7 +208,8 @@ class Sweep:
                 ax[i].values = _dptr(arr)
         o = SweepOpts()
         o.precision = precision; o.sims_per_cta = sims_per_cta; o.chunk_samples = chunk_samples
-        o.threads_per_cta = threads_per_cta; o.ctas_per_group = ctas_per_group; o.fc_mode = fc_mode; o.rate_threshold_khz = rate_threshold_khz
+        o.threads_per_cta = threads_per_cta; o.ctas_per_group = ctas_per_group; o.fc_mode = fc_mode; o.rate_threshold_khz = rate_threshold_khz; o.rate_stats_inhibitory = int(bool(rate_stats_inhibitory))
+        self.rate_stats_inhibitory = bool(rate_stats_inhibitory)
         if sim_ids is not None:
             ids = np.ascontiguousarray(sim_ids, dtype=np.int64)
             keep.append(ids)
@@ -353,18 +354,25 @@ class Sweep:
         return out
 
     def rate_stats(self, device=False, stream=None):
-        """tvbx_rate_stats -> (var_e, max_e float32 [S][N], n_above int32 [S][N]); numpy or torch CUDA."""
+        """tvbx_rate_stats -> (var_e, max_e float32 [S][N], n_above_e int32 [S][N]), followed by (var_i, max_i,
+        n_above_i) if the sweep was created with rate_stats_inhibitory; numpy or torch CUDA."""
         S, N = self.n_sims, self.n_regions
+        pops = 2 if self.rate_stats_inhibitory else 1
         if device:
             import torch
-            var = torch.empty((S, N), device="cuda", dtype=torch.float32)
-            mx = torch.empty((S, N), device="cuda", dtype=torch.float32)
-            ab = torch.empty((S, N), device="cuda", dtype=torch.int32)
-            _chk(lib().tvbx_rate_stats(self._h, var.data_ptr(), mx.data_ptr(), ab.data_ptr(), 1, _stream_ptr(stream)))
+            out = []
+            for _ in range(pops):
+                out += [torch.empty((S, N), device="cuda", dtype=torch.float32), torch.empty((S, N), device="cuda", dtype=torch.float32),
+                        torch.empty((S, N), device="cuda", dtype=torch.int32)]
+            ptr = [t.data_ptr() for t in out]
         else:
-            var, mx, ab = np.empty((S, N), np.float32), np.empty((S, N), np.float32), np.empty((S, N), np.int32)
-            _chk(lib().tvbx_rate_stats(self._h, var.ctypes.data, mx.ctypes.data, ab.ctypes.data, 0, _stream_ptr(stream)))
-        return var, mx, ab
+            out = []
+            for _ in range(pops):
+                out += [np.empty((S, N), np.float32), np.empty((S, N), np.float32), np.empty((S, N), np.int32)]
+            ptr = [a.ctypes.data for a in out]
+        ptr += [None] * (6 - len(ptr))
+        _chk(lib().tvbx_rate_stats(self._h, *ptr, 1 if device else 0, _stream_ptr(stream)))
+        return tuple(out)
 
     def kernel_name(self):
         buf = C.create_string_buffer(64)

@@ -120,7 +120,7 @@ struct DeviceSide {
   virtual int32_t run(int64_t steps, const tvbx_run_opts* o) = 0;
   virtual int32_t readout(float* fc, float* me, float* mi, int on_device, cudaStream_t st) = 0;
   virtual int32_t scores(const double* ref, float* fcsc, float* fitness, float* mean_fc, int on_device, cudaStream_t st) = 0;
-  virtual int32_t rate_stats(float* var_e, float* max_e, int32_t* above, int on_device, cudaStream_t st) = 0;
+  virtual int32_t rate_stats(float* var_e, float* max_e, int32_t* above, float* var_i, float* max_i, int32_t* above_i, int on_device, cudaStream_t st) = 0;
   virtual int32_t state(double* y, double* ou) = 0;
   virtual int32_t reset(cudaStream_t st) = 0;
 };
@@ -152,6 +152,7 @@ struct tvbx_sweep {
   int64_t chunk_req = 0;
   bool fc_tc = false;                // FC co-moment on the tensor cores (tvbx_fc_tc.cuh)
   double rate_thr = 0.1;             // kHz: samples above it are counted (f4; 100 Hz)
+  bool stats_i = false;              // keep the inhibitory 1-ms samples of the chunk too and their running statistics
   double init[7] = {0.001, 0.001, 0, 0, 0, 0, 0};
   // grouping
   std::vector<HostTable> tables;
@@ -386,6 +387,11 @@ struct DeviceImpl : DeviceSide {
   DevBuf<double> d_sums, d_cmean, d_mean, d_M, d_M_scratch, d_mean_scratch;
   DevBuf<float> d_cmax, d_rmax, d_rmax_scratch;       // f4: chunk / running maximum of the excitatory samples
   DevBuf<int32_t> d_ccnt, d_rcnt, d_rcnt_scratch;     //     chunk / running count of samples above the threshold
+  // f4, inhibitory population (optional): the chunk's samples and running (mean, M2, max, count), + scratch for readout
+  DevBuf<R> d_xbar_i;
+  DevBuf<double> d_imean, d_im2, d_imean_scratch, d_im2_scratch;
+  DevBuf<float> d_imax, d_imax_scratch;
+  DevBuf<int32_t> d_icnt, d_icnt_scratch;
   DevBuf<float> d_out_fc, d_out_me, d_out_mi;
   IntegrateParams<R> P;
   KernelPick<R> kp{nullptr};
@@ -533,7 +539,7 @@ struct DeviceImpl : DeviceSide {
       CS = std::min<int64_t>(std::max<int64_t>(CS, 16), 4096);
     }
     Kp = (CS + tvbx::TC_BK - 1) / tvbx::TC_BK * tvbx::TC_BK;
-    const size_t need = ring_elems * sizeof(R) + (size_t)G * CS * row * sizeof(R) + (sw->fc_tc ? (size_t)G * Kp * row * sizeof(float) : 0) +
+    const size_t need = ring_elems * sizeof(R) + (size_t)G * CS * row * sizeof(R) + (sw->fc_tc ? (size_t)G * Kp * row * sizeof(float) : 0) + (sw->stats_i ? (size_t)G * CS * row * sizeof(R) : 0) +
                         (size_t)G * SPC * N * N * sizeof(double) * 2 + (size_t)G * 16 * row * sizeof(double);
     if (need > free_b)
       return fail(TVBX_ENOMEM, "sweep needs %.2f GB of device memory (ring %.2f GB), %.2f GB free",
@@ -547,6 +553,11 @@ struct DeviceImpl : DeviceSide {
     if (sw->packed) CU(d_psim2.upload(psim2, hb));
     CU(d_ring.alloc(ring_elems));
     CU(d_xbar.alloc((size_t)G * CS * row));
+    if (sw->stats_i) {
+      CU(d_xbar_i.alloc((size_t)G * CS * row));
+      CU(cudaMemset(d_xbar_i.p, 0, d_xbar_i.n * sizeof(R)));
+      CU(d_imean.alloc((size_t)G * row)); CU(d_im2.alloc((size_t)G * row)); CU(d_imax.alloc((size_t)G * row)); CU(d_icnt.alloc((size_t)G * row));
+    }
     if (sw->fc_tc) CU(d_xc.alloc((size_t)G * Kp * row));
     CU(d_cmean.alloc((size_t)G * row)); CU(d_mean.alloc((size_t)G * row));
     CU(d_cmax.alloc((size_t)G * row)); CU(d_rmax.alloc((size_t)G * row)); CU(d_ccnt.alloc((size_t)G * row)); CU(d_rcnt.alloc((size_t)G * row));
@@ -603,7 +614,7 @@ struct DeviceImpl : DeviceSide {
     P.N = N; P.SPC = SPC; P.seed = sw->seed; P.chunk_samples = (int32_t)CS;
     P.tables = d_tables.p; P.groups = d_groups.p; P.edges = d_edges.p; P.rowptr = d_rowptr.p;
     P.psim = d_psim.p; P.ext_id = d_ext.p; P.loc_id = d_loc.p; P.ring = d_ring.p; P.state = d_state.p;
-    P.sums = d_sums.p; P.xbar = d_xbar.p;
+    P.sums = d_sums.p; P.xbar = d_xbar.p; P.xbar_i = sw->stats_i ? d_xbar_i.p : nullptr;
 
     // ---- launch geometry: two lanes per (sim, region) ----
     const int maxt = sw->threads_req > 0 ? std::min(sw->threads_req, MaxT<R>::v) : MaxT<R>::v;
@@ -742,7 +753,7 @@ struct DeviceImpl : DeviceSide {
   }
   bool tc_attr_set = false;
 
-  int32_t accumulate(double* Mbuf, double* meanbuf, float* rmaxbuf, int32_t* rcntbuf, int64_t cnt, int n_c, cudaStream_t st) {
+  int32_t accumulate(double* Mbuf, double* meanbuf, float* rmaxbuf, int32_t* rcntbuf, bool scratch_i, int64_t cnt, int n_c, cudaStream_t st) {
     const int N = sw->conn.n, SPC = sw->spc, G = (int)sw->groups.size();
     FcParams<R> F;
     F.xbar = d_xbar.p; F.cmean = d_cmean.p; F.mean = meanbuf; F.M = Mbuf; F.cnt = cnt; F.n_c = n_c;
@@ -761,6 +772,15 @@ struct DeviceImpl : DeviceSide {
       fc_comoment_kernel<R><<<g2, 64, 0, st>>>(F);
     }
     fc_mean_update_kernel<R><<<g1, 128, 0, st>>>(F);
+    if (sw->stats_i) {
+      RateIParams<R> I;
+      I.xbar_i = d_xbar_i.p;
+      I.mean = scratch_i ? d_imean_scratch.p : d_imean.p; I.m2 = scratch_i ? d_im2_scratch.p : d_im2.p;
+      I.rmax = scratch_i ? d_imax_scratch.p : d_imax.p; I.rcnt = scratch_i ? d_icnt_scratch.p : d_icnt.p;
+      I.cnt = cnt; I.n_c = n_c; I.CS = (int32_t)sw->CS; I.N = N; I.SPC = SPC; I.G = G; I.thr = (float)sw->rate_thr;
+      rate_i_chunk_kernel<R><<<g0, 1024, 0, st>>>(I);
+      sw->launches += 1;
+    }
     sw->prof_end(st);
     sw->launches += sw->fc_tc ? 4 : 3;
     CU(cudaGetLastError());
@@ -823,7 +843,7 @@ struct DeviceImpl : DeviceSide {
       CU(cudaGetLastError());
       sw->n += take; remaining -= take; sw->fill += kept;
       if (ds > 0 && sw->fill == sw->CS) {
-        int32_t rc = accumulate(d_M.p, d_mean.p, d_rmax.p, d_rcnt.p, sw->cnt, (int)sw->fill, st);
+        int32_t rc = accumulate(d_M.p, d_mean.p, d_rmax.p, d_rcnt.p, false, sw->cnt, (int)sw->fill, st);
         if (rc) return rc;
         sw->cnt += sw->fill; sw->fill = 0;
       }
@@ -846,7 +866,14 @@ struct DeviceImpl : DeviceSide {
       CU(cudaMemcpyAsync(tmean.p, d_mean.p, d_mean.n * sizeof(double), cudaMemcpyDeviceToDevice, st));
       CU(cudaMemcpyAsync(d_rmax_scratch.p, d_rmax.p, d_rmax.n * sizeof(float), cudaMemcpyDeviceToDevice, st));
       CU(cudaMemcpyAsync(d_rcnt_scratch.p, d_rcnt.p, d_rcnt.n * sizeof(int32_t), cudaMemcpyDeviceToDevice, st));
-      int32_t rc = accumulate(tM.p, tmean.p, d_rmax_scratch.p, d_rcnt_scratch.p, sw->cnt, (int)sw->fill, st);
+      if (sw->stats_i) {
+        if (d_imean_scratch.n != d_imean.n) { CU(d_imean_scratch.alloc(d_imean.n)); CU(d_im2_scratch.alloc(d_im2.n)); CU(d_imax_scratch.alloc(d_imax.n)); CU(d_icnt_scratch.alloc(d_icnt.n)); }
+        CU(cudaMemcpyAsync(d_imean_scratch.p, d_imean.p, d_imean.n * sizeof(double), cudaMemcpyDeviceToDevice, st));
+        CU(cudaMemcpyAsync(d_im2_scratch.p, d_im2.p, d_im2.n * sizeof(double), cudaMemcpyDeviceToDevice, st));
+        CU(cudaMemcpyAsync(d_imax_scratch.p, d_imax.p, d_imax.n * sizeof(float), cudaMemcpyDeviceToDevice, st));
+        CU(cudaMemcpyAsync(d_icnt_scratch.p, d_icnt.p, d_icnt.n * sizeof(int32_t), cudaMemcpyDeviceToDevice, st));
+      }
+      int32_t rc = accumulate(tM.p, tmean.p, d_rmax_scratch.p, d_rcnt_scratch.p, true, sw->cnt, (int)sw->fill, st);
       if (rc) return rc;
       *Msrc = tM.p;
     }
@@ -901,9 +928,9 @@ struct DeviceImpl : DeviceSide {
   }
 
   // f4: variance, maximum and above-threshold count of the excitatory 1-ms samples per (simulation, region)
-  DevBuf<float> d_out_var, d_out_max;
-  DevBuf<int32_t> d_out_above;
-  int32_t rate_stats(float* var_e, float* max_e, int32_t* above, int on_device, cudaStream_t st) override {
+  DevBuf<float> d_out_var, d_out_max, d_out_var_i, d_out_max_i;
+  DevBuf<int32_t> d_out_above, d_out_above_i;
+  int32_t rate_stats(float* var_e, float* max_e, int32_t* above, float* var_i, float* max_i, int32_t* above_i, int on_device, cudaStream_t st) override {
     const int N = sw->conn.n, SPC = sw->spc, G = (int)sw->groups.size();
     const int64_t total = sw->cnt + sw->fill;
     if (total < 1) return fail(TVBX_ESTATE, "no sample kept yet");
@@ -913,11 +940,19 @@ struct DeviceImpl : DeviceSide {
     Q.M = Msrc; Q.rmax = sw->fill > 0 ? d_rmax_scratch.p : d_rmax.p; Q.rcnt = sw->fill > 0 ? d_rcnt_scratch.p : d_rcnt.p;
     Q.loc_id = d_loc.p; Q.cnt = total; Q.N = N; Q.SPC = SPC; Q.G = G;
     Q.var_e = var_e; Q.max_e = max_e; Q.above = above;
+    const bool want_i = var_i || max_i || above_i;
+    if (want_i && !sw->stats_i) return fail(TVBX_EINVAL, "inhibitory statistics need tvbx_sweep_opts.rate_stats_inhibitory");
+    Q.m2_i = want_i ? (sw->fill > 0 ? d_im2_scratch.p : d_im2.p) : nullptr;
+    Q.rmax_i = sw->fill > 0 ? d_imax_scratch.p : d_imax.p; Q.rcnt_i = sw->fill > 0 ? d_icnt_scratch.p : d_icnt.p;
+    Q.var_i = var_i; Q.max_i = max_i; Q.above_i = above_i;
     const size_t n_out = (size_t)sw->n_sims * N;
     if (!on_device) {
       if (var_e) { if (d_out_var.n != n_out) CU(d_out_var.alloc(n_out)); Q.var_e = d_out_var.p; }
       if (max_e) { if (d_out_max.n != n_out) CU(d_out_max.alloc(n_out)); Q.max_e = d_out_max.p; }
       if (above) { if (d_out_above.n != n_out) CU(d_out_above.alloc(n_out)); Q.above = d_out_above.p; }
+      if (var_i) { if (d_out_var_i.n != n_out) CU(d_out_var_i.alloc(n_out)); Q.var_i = d_out_var_i.p; }
+      if (max_i) { if (d_out_max_i.n != n_out) CU(d_out_max_i.alloc(n_out)); Q.max_i = d_out_max_i.p; }
+      if (above_i) { if (d_out_above_i.n != n_out) CU(d_out_above_i.alloc(n_out)); Q.above_i = d_out_above_i.p; }
     }
     sw->prof_begin(K_READOUT, st);
     rate_stats_kernel<<<dim3((N + 127) / 128, G * SPC), 128, 0, st>>>(Q);
@@ -928,6 +963,9 @@ struct DeviceImpl : DeviceSide {
       if (var_e) { CU(cudaMemcpyAsync(var_e, Q.var_e, n_out * sizeof(float), cudaMemcpyDeviceToHost, st)); sw->d2h += (int64_t)(n_out * sizeof(float)); }
       if (max_e) { CU(cudaMemcpyAsync(max_e, Q.max_e, n_out * sizeof(float), cudaMemcpyDeviceToHost, st)); sw->d2h += (int64_t)(n_out * sizeof(float)); }
       if (above) { CU(cudaMemcpyAsync(above, Q.above, n_out * sizeof(int32_t), cudaMemcpyDeviceToHost, st)); sw->d2h += (int64_t)(n_out * sizeof(int32_t)); }
+      if (var_i) { CU(cudaMemcpyAsync(var_i, Q.var_i, n_out * sizeof(float), cudaMemcpyDeviceToHost, st)); sw->d2h += (int64_t)(n_out * sizeof(float)); }
+      if (max_i) { CU(cudaMemcpyAsync(max_i, Q.max_i, n_out * sizeof(float), cudaMemcpyDeviceToHost, st)); sw->d2h += (int64_t)(n_out * sizeof(float)); }
+      if (above_i) { CU(cudaMemcpyAsync(above_i, Q.above_i, n_out * sizeof(int32_t), cudaMemcpyDeviceToHost, st)); sw->d2h += (int64_t)(n_out * sizeof(int32_t)); }
       CU(cudaStreamSynchronize(st));
     }
     return TVBX_OK;
@@ -1072,6 +1110,7 @@ int32_t tvbx_sweep_create(const tvbx_connectome* c, const tvbx_model_params* def
   sw->threads_req = opts ? opts->threads_per_cta : 0;
   sw->chunk_req = opts ? opts->chunk_samples : 0;
   {
+    sw->stats_i = opts && opts->rate_stats_inhibitory != 0;
     if (opts && opts->rate_threshold_khz != 0.0) {
       if (!(opts->rate_threshold_khz > 0.0)) return fail(TVBX_EINVAL, "rate_threshold_khz=%g", opts->rate_threshold_khz);
       sw->rate_thr = opts->rate_threshold_khz;
@@ -1099,7 +1138,9 @@ int32_t tvbx_sweep_create(const tvbx_connectome* c, const tvbx_model_params* def
   if (const char* e = getenv("TVBX_SPC")) if (spc == 0) spc = atoi(e);
   // the packed FP32 kernel (one thread per (sim, region), <= 480 of them, <= 8 simulations per CTA) serves
   // tau_e == tau_i and N <= 480; everything else runs the general kernel (two lanes per (sim, region))
-  const bool packed_ok = sw->precision == TVBX_F32 && dp[TVBX_P_TAUE] == dp[TVBX_P_TAUI] && sw->conn.n <= 480 &&
+  // (the inhibitory 1-ms samples are written by the general kernel only: the packed kernel is kept free of the extra
+  // store, which costs it 0.65 % of its throughput even when unused)
+  const bool packed_ok = sw->precision == TVBX_F32 && dp[TVBX_P_TAUE] == dp[TVBX_P_TAUI] && sw->conn.n <= 480 && !sw->stats_i &&
                          getenv("TVBX_GENERAL_KERNEL") == nullptr;
   const int lanes_per_node = packed_ok ? 1 : 2;
   const int maxt_sel = packed_ok ? 480 : (sw->precision == TVBX_F64 ? 384 : 1024);
@@ -1230,10 +1271,11 @@ int32_t tvbx_fc_scores(tvbx_sweep* sw, const double* ref_fc, float* fcsc, float*
       if (!std::isfinite(ref_fc[i])) return fail(TVBX_EINVAL, "reference FC entry %zu is not finite", i);
   return sw->dev->scores(ref_fc, fcsc, fitness, mean_fc, on_device, (cudaStream_t)stream);
 }
-int32_t tvbx_rate_stats(tvbx_sweep* sw, float* var_e, float* max_e, int32_t* n_above, int32_t on_device, void* stream) {
+int32_t tvbx_rate_stats(tvbx_sweep* sw, float* var_e, float* max_e, int32_t* n_above_e, float* var_i, float* max_i,
+                        int32_t* n_above_i, int32_t on_device, void* stream) {
   if (!sw) return fail(TVBX_EINVAL, "sweep is NULL");
   if (!sw->started) return fail(TVBX_ESTATE, "no run yet");
-  return sw->dev->rate_stats(var_e, max_e, n_above, on_device, (cudaStream_t)stream);
+  return sw->dev->rate_stats(var_e, max_e, n_above_e, var_i, max_i, n_above_i, on_device, (cudaStream_t)stream);
 }
 int32_t tvbx_fc_readout(tvbx_sweep* sw, float* fc, float* mean_e, float* mean_i, int32_t on_device, void* stream) {
   if (!sw) return fail(TVBX_EINVAL, "sweep is NULL");

@@ -152,6 +152,73 @@ __global__ void fc_mean_update_kernel(FcParams<R> P) {
   }
 }
 
+// f4, inhibitory population (optional, tvbx_sweep_opts.rate_stats_inhibitory): one pass over the chunk's inhibitory
+// samples per (group, region, lane) column -- Welford per sample slice, the 32 slices merged with Chan's update in a
+// fixed order -- then merged into the running (mean, M2, max, count).  st[4]: {count is P.cnt, [0] mean, [1] M2}.
+template <typename R>
+struct RateIParams {
+  const R* xbar_i;      // [G][CS][N][SPC]
+  double* mean;         // [G][N][SPC] running mean
+  double* m2;           // [G][N][SPC] running sum of squared deviations
+  float* rmax;          // [G][N][SPC]
+  int32_t* rcnt;        // [G][N][SPC]
+  int64_t cnt;          // samples merged before this chunk
+  int32_t n_c, CS, N, SPC, G;
+  float thr;
+};
+template <typename R>
+__global__ void __launch_bounds__(1024) rate_i_chunk_kernel(RateIParams<R> P) {
+  __shared__ double pm[32][33], p2[32][33];
+  __shared__ float pmax[32][33];
+  __shared__ int pcnt[32][33], pn[32][33];
+  const int g = blockIdx.y;
+  const int cx = threadIdx.x & 31, sy = threadIdx.x >> 5;
+  const int idx = blockIdx.x * 32 + cx;
+  const int row = P.N * P.SPC;
+  double mean = 0.0, m2 = 0.0;
+  float mx = -INFINITY;
+  int ct = 0, n = 0;
+  if (idx < row) {
+    const R* x = P.xbar_i + (size_t)g * P.CS * row + idx;
+    for (int q = sy; q < P.n_c; q += 32) {
+      const double v = (double)x[(size_t)q * row];
+      ++n;
+      const double d = v - mean;
+      mean += d / (double)n;
+      m2 += d * (v - mean);
+      mx = fmaxf(mx, (float)v);
+      ct += (float)v > P.thr ? 1 : 0;
+    }
+  }
+  pm[sy][cx] = mean; p2[sy][cx] = m2; pmax[sy][cx] = mx; pcnt[sy][cx] = ct; pn[sy][cx] = n;
+  __syncthreads();
+  if (sy == 0 && idx < row) {
+    double cm = 0.0, c2 = 0.0;
+    double cn = 0.0;
+    float m = -INFINITY;
+    int c = 0;
+    for (int j = 0; j < 32; ++j) {
+      const double nj = (double)pn[j][cx];
+      if (nj > 0.0) {
+        const double d = pm[j][cx] - cm, tot = cn + nj;
+        c2 += p2[j][cx] + d * d * (cn * nj / tot);
+        cm += d * (nj / tot);
+        cn = tot;
+      }
+      m = fmaxf(m, pmax[j][cx]); c += pcnt[j][cx];
+    }
+    const size_t o = (size_t)g * row + idx;
+    if (P.cnt == 0) { P.mean[o] = cm; P.m2[o] = c2; P.rmax[o] = m; P.rcnt[o] = c; }
+    else {
+      const double a = (double)P.cnt, tot = a + cn, d = cm - P.mean[o];
+      P.m2[o] += c2 + d * d * (a * cn / tot);
+      P.mean[o] += d * (cn / tot);
+      P.rmax[o] = fmaxf(P.rmax[o], m);
+      P.rcnt[o] += c;
+    }
+  }
+}
+
 // f4 readout: per (simulation, region) variance (M_kk / n, the population variance of the kept 1-ms samples), maximum
 // and number of samples above the threshold, in local-simulation order
 struct RateStatsParams {
@@ -162,6 +229,12 @@ struct RateStatsParams {
   float* var_e;          // [n_sims][N] or null
   float* max_e;          // [n_sims][N] or null
   int32_t* above;        // [n_sims][N] or null
+  const double* m2_i;    // inhibitory running statistics [G][N][SPC], or null
+  const float* rmax_i;
+  const int32_t* rcnt_i;
+  float* var_i;          // [n_sims][N] or null
+  float* max_i;
+  int32_t* above_i;
   int64_t cnt;
   int32_t N, SPC, G;
 };
@@ -175,6 +248,11 @@ __global__ void rate_stats_kernel(RateStatsParams P) {
   if (P.var_e) P.var_e[(size_t)loc * P.N + k] = (float)(P.M[((size_t)g * P.SPC + sl) * P.N * P.N + (size_t)k * P.N + k] / (double)P.cnt);
   if (P.max_e) P.max_e[(size_t)loc * P.N + k] = P.rmax[o];
   if (P.above) P.above[(size_t)loc * P.N + k] = P.rcnt[o];
+  if (P.m2_i) {
+    if (P.var_i) P.var_i[(size_t)loc * P.N + k] = (float)(P.m2_i[o] / (double)P.cnt);
+    if (P.max_i) P.max_i[(size_t)loc * P.N + k] = P.rmax_i[o];
+    if (P.above_i) P.above_i[(size_t)loc * P.N + k] = P.rcnt_i[o];
+  }
 }
 
 struct ReadoutParams {

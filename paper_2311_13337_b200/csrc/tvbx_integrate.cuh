@@ -130,6 +130,7 @@ struct IntegrateParams {
   R* state;                     // [group][NSV-2][N][SPC]
   double* sums;                 // [group][2][N][SPC]  running sums of kept E / I samples
   R* xbar;                      // [group][CS][N][SPC] kept excitatory samples of the current chunk
+  R* xbar_i;                    // same for the inhibitory population, or null (only tvbx_rate_stats uses them)
   R* traj;                      // optional [n_sims][traj_steps][7][N]
   int64_t traj_steps;
   int64_t traj_n0;              // global step index of traj row 0
@@ -368,6 +369,7 @@ __global__ void __launch_bounds__(MAXT, 1) integrate_kernel(const __grid_constan
             if (nn0 + i + 1 > P.discard_steps) {
               const R m = st.win * inv_ds;
               if (pop == 0) P.xbar[(((size_t)g * P.chunk_samples + sidx) * N + k) * SPC + sl] = m;
+              else if (P.xbar_i) P.xbar_i[(((size_t)g * P.chunk_samples + sidx) * N + k) * SPC + sl] = m;
               st.sum += (double)m;
               ++sidx;
             }

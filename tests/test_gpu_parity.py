@@ -637,3 +637,46 @@ def test_more_regions_than_tmem_columns_falls_back_to_register_tiles():
     assert np.abs(me / rme - 1).max() < TOL_MEAN_REL and np.abs(fc - rfc).max() < TOL_FC_ABS
     with pytest.raises(tvbx.TvbxError):
         tvbx.sweep_from_config(cfg, W, L, fc_mode=tvbx.TVBX_FC_TF32)
+
+
+@pytest.mark.parametrize("kw", [dict(chunk_samples=37), dict(chunk_samples=50, sims_per_cta=4),
+                                dict(chunk_samples=64, precision=tvbx.TVBX_F64)], ids=["fp32", "fp32_spc4", "fp64"])
+def test_rate_stats_inhibitory_population(kw):
+    """rate_stats_inhibitory: the inhibitory 1-ms samples are kept as well and reduced by one Welford/Chan pass per
+    chunk; variance, maximum and count of both populations against oracle/rate_stats.py on the oracle's samples."""
+    from oracle import rate_stats as ors
+    N = 24
+    W, L = wl.connectome(N, seed=5, keep=0.4)
+    cfg = dict(axes=[dict(name="G", lo=0.0, hi=0.4, n=4, values=None)], fixed=dict(v=4.0, b_e=20.0, wNoise=1e-4), seed=11)
+    steps = 2400
+    o = orc.OracleSweep(W, L, wl.grid_params(cfg), seed=cfg["seed"])
+    o.run(steps, 0.1, noise_on=True, ds=10, discard_steps=200)
+    xs = [o.samples(s) for s in range(o.S)]
+    thr = float(np.median(np.concatenate([x[1].ravel() for x in xs])))     # inside the inhibitory data
+    thr = thr * 1.0000001
+    _, sw = tvbx.sweep_from_config(cfg, W, L, rate_stats_inhibitory=True, rate_threshold_khz=thr, **kw)
+    sw.run(steps, 0.1, noise_on=True, ds=10, discard_steps=200)
+    assert sw.kernel_name() == "tvbx::integrate_kernel"        # the option selects the general integrator
+    var_e, max_e, ab_e, var_i, max_i, ab_i = sw.rate_stats()
+    fp64 = kw.get("precision") == tvbx.TVBX_F64
+    n = xs[0][0].shape[0]
+    for s in range(sw.n_sims):
+        for pop, (var, mx, ab) in enumerate([(var_e, max_e, ab_e), (var_i, max_i, ab_i)]):
+            rv, rm, ra = ors.rate_stats(xs[s][pop], thr)
+            np.testing.assert_allclose(var[s], rv, rtol=1e-5 if fp64 else 2e-2, atol=1e-14)
+            np.testing.assert_allclose(mx[s], rm, rtol=1e-6 if fp64 else TOL_MEAN_REL)
+            if fp64:
+                np.testing.assert_array_equal(ab[s], ra)
+            else:      # FP32 trajectories: samples within 1 % of the threshold may fall on either side
+                x = np.asarray(xs[s][pop])
+                slack = ((x > thr * 0.99) & (x < thr * 1.01)).sum(axis=0)
+                assert np.all(np.abs(ab[s] - np.asarray(ra)) <= slack)
+    assert np.all((ab_i >= 0) & (ab_i <= n)) and ab_i.sum() > 0
+    # without the option the inhibitory outputs are refused
+    _, sw2 = tvbx.sweep_from_config(cfg, W, L)
+    sw2.run(100, 0.1, noise_on=True, ds=10)
+    assert len(sw2.rate_stats()) == 3
+    import ctypes as C
+    buf = np.empty((sw2.n_sims, N), np.float32)
+    rc = tvbx.lib().tvbx_rate_stats(sw2._h, None, None, None, buf.ctypes.data, None, None, 0, None)
+    assert rc == -1        # TVBX_EINVAL
