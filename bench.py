@@ -9,6 +9,8 @@ chosen BASELINE.json config (default configs[1]: 1,024 simulations x 68 regions 
 noise on, 1-ms downsample, 1 s discarded) integrated from t = 0 and reduced to mean rates + FC.
   value  : device-resident -- connectome, tables and state already in HBM; the timed region is
            reset -> tvbx_run -> tvbx_fc_readout (device buffers), K times, CUDA events.
+  per_config : the same measurement (value, e2e, ms_per_step, kernel ms, its own roofline) for the other four
+           BASELINE.json configs at their full sizes, with a fixed small number of repeats each.
   e2e    : the same through the C ABI from HOST buffers: tvbx_create_connectome + tvbx_sweep_create
            (host W, L, axes) -> tvbx_run -> tvbx_fc_readout into pinned host arrays -> destroy.
   roofline / cpu_baseline : see DESIGN.md section 7.
@@ -35,27 +37,98 @@ import workloads as wl  # noqa: E402
 METRIC = "simulated region-steps/s (sims x regions x steps / s)"
 UNIT = "region-steps/s"
 
-# FP32 floating-point operations the integrator needs per region-step = the operation
-# count of its closed-form transfer function + Euler update + noise as executed by integrate2_kernel
-# (ncu source page of the cfg-2 capture in profiles/: per (sim, region) step 115 FFMA2 x 4 + 111 FMUL2 x 2 +
-# 23 FADD2 x 2 + 8 FFMA x 2 + 10 FMUL/FADD + 3 for Box-Muller = 757), plus 2 flops per non-zero edge of the
-# coupling sum; and the FP32 peak of the chip: 148 SMs x 128 lanes x 2 flop x sm_max_mhz.
+# DESIGN.md section 7 (frozen there, not re-derived from the binary): algorithmic FP32 floating-point operations of one
+# region-step = both closed-form transfer functions with first and second derivatives + Eqs. (1)-(3) + OU / Box-Muller
+# share = 757 (115 packed FMA x 4 + 111 packed MUL x 2 + 23 packed ADD x 2 + 8 FMA x 2 + 10 MUL/ADD + 3), plus 2 flops
+# per non-zero edge of the coupling sum; FP32 peak of the chip: 148 SMs x 128 lanes x 2 flop x sm_max_mhz.
 KERNEL_FLOPS_BASE = 757.0
-# DRAM bytes per region-step of the integrator from the ncu --set full capture in profiles/
-# (dram__bytes_read.sum + dram__bytes_write.sum of a 2,000-step launch of cfg 2 / its region-steps)
-NCU_DRAM_BYTES_PER_REGION_STEP = {2: 25.9, 5: 67.3}
-# L2 -> SM bytes per region-step of the cfg-5 capture (l1tex__m_xbar2l1tex_read_bytes.sum / region-steps,
-# profiles/r1_integrate2_kernel_cfg5_cluster_ncu.txt): what the N = 360 gather really moves (722 B algorithmic)
-NCU_L2_BYTES_PER_REGION_STEP = {5: 1075.0}
 FLOPS_PER_EDGE = 2.0
-# the same capture's pipe counters (profiles/r1_integrate2_kernel_cfg2_ncu.txt): what the north star asks to be judged
-# "as measured by ncu" -- reported beside the algorithmic fraction, never instead of it
-NCU_CFG2 = {"source": "profiles/r1_integrate2_kernel_cfg2_ncu.txt",
-            "sm__pipe_fma_cycles_active.avg.pct_of_peak_sustained_active": 60.6,
-            "smsp__issue_active.avg.pct_of_peak_sustained_active": 60.7,
-            "sm__throughput.avg.pct_of_peak_sustained_elapsed": 60.3,
-            "lts__t_sector_hit_rate.pct": 70.2, "gpu__dram_throughput.avg.pct_of_peak_sustained_elapsed": 12.1}
 SM_COUNT, LANES_PER_SM = 148, 128
+# ncu --set full captures of the integrator, committed as text under profiles/ (each names its command).  bench.py
+# PARSES them at run time (DRAM bytes, L2 -> SM bytes, pipe counters of the captured launch) and records path + sha256,
+# so a stale profile is visible in the line instead of hiding behind typed-in constants.  First existing file wins.
+PROFILES = {
+    1: ["profiles/r2_integrate2_kernel_cfg1_ncu.txt"],
+    2: ["profiles/r2_integrate2_kernel_cfg2_ncu.txt", "profiles/r1_integrate2_kernel_cfg2_ncu.txt"],
+    3: ["profiles/r2_integrate2_kernel_cfg3_ncu.txt"],
+    4: ["profiles/r2_integrate2_kernel_cfg4_ncu.txt", "profiles/r1_integrate2_kernel_cfg4_small_ncu.txt"],
+    5: ["profiles/r2_integrate2_kernel_cfg5_ncu.txt", "profiles/r1_integrate2_kernel_cfg5_cluster_ncu.txt"],
+}
+NCU_KEYS = ("sm__pipe_fma_cycles_active.avg.pct_of_peak_sustained_active", "smsp__issue_active.avg.pct_of_peak_sustained_active",
+            "sm__throughput.avg.pct_of_peak_sustained_elapsed", "lts__t_sector_hit_rate.pct",
+            "gpu__dram_throughput.avg.pct_of_peak_sustained_elapsed", "sm__inst_executed_pipe_xu.avg.pct_of_peak_sustained_active",
+            "smsp__average_warps_issue_stalled_long_scoreboard_per_issue_active.ratio", "launch__registers_per_thread")
+_UNIT = {"byte": 1.0, "Kbyte": 1e3, "Mbyte": 1e6, "Gbyte": 1e9, "Tbyte": 1e12}
+
+
+def read_profile(cfg_id):
+    """Parse the committed ncu raw-page extract of this config's integrator capture -> dict or None."""
+    import hashlib
+    import re
+    for rel in PROFILES.get(cfg_id, []):
+        path = os.path.join(ROOT, rel)
+        if not os.path.exists(path):
+            continue
+        txt = open(path).read()
+        m = re.search(r"=\s*([0-9.]+e[+-]?[0-9]+|[0-9.]+)\s*region-steps", txt)
+        if not m:
+            continue
+        units = float(m.group(1))
+        vals = {}
+        for line in txt.splitlines():
+            parts = line.split()
+            if len(parts) >= 2 and re.match(r"^[a-z_]+__", parts[0]):
+                try:
+                    vals[parts[0]] = (float(parts[1].replace(",", "")), parts[2] if len(parts) > 2 else "")
+                except ValueError:
+                    pass
+
+        def nbytes(key):
+            if key not in vals:
+                return None
+            v, u = vals[key]
+            return v * _UNIT.get(u, 1.0)
+
+        rd, wr, l2 = nbytes("dram__bytes_read.sum"), nbytes("dram__bytes_write.sum"), nbytes("l1tex__m_xbar2l1tex_read_bytes.sum")
+        return {"source": rel, "sha256_16": hashlib.sha256(txt.encode()).hexdigest()[:16], "captured_region_steps": units,
+                "dram_bytes_per_region_step": (rd + wr) / units if rd is not None and wr is not None else None,
+                "l2_to_sm_bytes_per_region_step": l2 / units if l2 is not None else None,
+                "counters": {k: vals[k][0] for k in NCU_KEYS if k in vals}}
+    return None
+
+
+class Probes:
+    """bench_probes.cu: measurement-only micro-benchmarks (L2 / HBM read bandwidth, FP32-lane throughput of the
+    instruction forms the integrator is made of), built here into bench_probes.so -- not part of libtvbx.so."""
+
+    KINDS = ("ffma2_3reg", "ffma2_bcast", "fmul2", "fadd2", "ffma", "mufu_rcp")
+
+    def __init__(self):
+        import ctypes as C
+        src, so = os.path.join(ROOT, "bench_probes.cu"), os.path.join(ROOT, "bench_probes.so")
+        if not os.path.exists(so) or os.path.getmtime(so) < os.path.getmtime(src):
+            subprocess.check_call(["nvcc", "-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-shared",
+                                   "-Xcompiler", "-fPIC", "-o", so, src])
+        self.C, self.L = C, C.CDLL(so)
+        self.L.probe_read_bandwidth.argtypes = [C.c_longlong, C.c_int, C.POINTER(C.c_double)]
+        self.L.probe_alu.argtypes = [C.c_int, C.c_int, C.POINTER(C.c_double)]
+
+    def read_bandwidth(self, nbytes, passes=20):
+        out = self.C.c_double()
+        rc = self.L.probe_read_bandwidth(int(nbytes), int(passes), self.C.byref(out))
+        if rc != 0:
+            raise RuntimeError(f"probe_read_bandwidth rc={rc}")
+        return out.value
+
+    def alu_lanes_per_clk_per_sm(self, sm_mhz, iters=400):
+        res = {}
+        for kind, name in enumerate(self.KINDS):
+            out = self.C.c_double()
+            rc = self.L.probe_alu(kind, int(iters), self.C.byref(out))
+            if rc != 0:
+                raise RuntimeError(f"probe_alu({name}) rc={rc}")
+            res[name] = out.value / (SM_COUNT * sm_mhz * 1e6)
+        return res
 
 
 def peaks():
@@ -186,32 +259,25 @@ def cpu_baseline(cfg_id):
 
 
 # ------------------------------------------------------------------------------------------------
-def run_tvbx(args):
-    import torch
-    import torch.distributed as dist
-    import paper_2311_13337_b200 as tvbx
-
-    world = int(os.environ.get("WORLD_SIZE", "1"))
-    rank = int(os.environ.get("RANK", "0"))
-    local = int(os.environ.get("LOCAL_RANK", "0"))
-    if not torch.cuda.is_available():
-        raise SystemExit("bench.py: no CUDA device (there is no CPU fallback; use --impl reference for the oracle)")
-    torch.cuda.set_device(local)
-    if world > 1:
-        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
-    tvbx.lib()                                   # fails loudly if libtvbx.so is missing
-
-    cfg, W, L, S = workload(args.config)
-    N, steps_sim = cfg["n"], (args.sim_steps or cfg["steps"])
+def measure_config(tvbx, torch, dist, cfg_id, steps, warmup, e2e_steps, sim_steps, rank, world, local, stream, pk, probes, clocks=None):
+    """One config: device-resident arm (value), end-to-end arm through the C ABI from host buffers (e2e), roofline.
+    Returns a dict (rank 0 uses it)."""
+    cfg, W, L, S = workload(cfg_id)
+    N, steps_sim = cfg["n"], (sim_steps or cfg["steps"])
     if steps_sim != cfg["steps"]:                # profiling runs only: keep the discard proportionate
         cfg["discard_steps"] = min(cfg["discard_steps"], (steps_sim // 5) // cfg["ds"] * cfg["ds"])
     seed = cfg["seed"] + rank                    # replica r of the sweep: same grid, its own noise
-    stream = torch.cuda.Stream()
 
     def barrier():
         if world > 1:
             dist.barrier()
         torch.cuda.synchronize()
+
+    def maxr(x):
+        t = torch.tensor([x], device="cuda", dtype=torch.float64)
+        if world > 1:
+            dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        return float(t.item())
 
     # ---- device-resident arm --------------------------------------------------------------------
     conn, sw = tvbx.sweep_from_config(cfg, W, L, seed=seed)
@@ -225,37 +291,37 @@ def run_tvbx(args):
         sw.fc_readout(device=True, stream=stream, out=(fc, me, mi))
 
     sw.run(1, cfg["dt"], noise_on=True, ds=cfg["ds"], discard_steps=cfg["discard_steps"], stream=stream)   # allocate
-    for _ in range(args.warmup):
+    for _ in range(warmup):
         one_step()
     barrier()
     sw.profile_enable(os.environ.get("TVBX_BENCH_NOPROF") is None)
     sw.profile_read()
     l0 = sw.launch_count()
-    clocks = ClockSampler(local)
-    if rank == 0:
+    if clocks is not None:
         clocks.start()
     e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
     barrier()
     with torch.cuda.stream(stream):
         e0.record(stream)
-        for _ in range(args.steps):
+        for _ in range(steps):
             one_step()
         e1.record(stream)
     stream.synchronize()
     barrier()
     ms = e0.elapsed_time(e1)
-    clk = clocks.stop() if rank == 0 else None
+    clk = clocks.stop() if clocks is not None else None
     launches = sw.launch_count() - l0
     prof = sw.profile_read()
     sw.profile_enable(False)
     info = sw.launch_info()
-    t = torch.tensor([ms], device="cuda", dtype=torch.float64)
-    if world > 1:
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-    ms_max = float(t.item())
+    ms_max = maxr(ms)
     units_per_step = S * N * steps_sim
-    value = world * units_per_step * args.steps / (ms_max * 1e-3)
+    value = world * units_per_step * steps / (ms_max * 1e-3)
     finite = bool(torch.isfinite(fc).all().item() and torch.isfinite(me).all().item())
+    rec = {"cfg": cfg_id, "value": value, "unit": UNIT, "steps": steps, "warmup": warmup, "ms_per_step": ms_max / steps,
+           "gpu_launches": int(launches), "config": config_dict(cfg_id, cfg, S, {"launch": info, "sim_steps": steps_sim,
+                                                                                "replicas": world, "results_finite": finite}),
+           "clocks": clk}
 
     # ---- f3 (not part of the step): FCSC / mean FC per simulation from the resident accumulators ----
     sw.fc_scores(device=True, stream=stream)
@@ -264,7 +330,7 @@ def run_tvbx(args):
     sw.profile_read()
     s0, s1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
     per_call = []
-    for _ in range(5):
+    for _ in range(3):
         s0.record(stream)
         sw.fc_scores(device=True, stream=stream)
         s1.record(stream)
@@ -275,13 +341,15 @@ def run_tvbx(args):
     sw.profile_enable(False)
     scores_kernel_ms = sprof["readout"][0] / max(sprof["readout"][1], 1)      # fc_scores_kernel alone
     scores_bytes = S * N * N * 8.0          # the FP64 co-moments, read once
+    kname = sw.kernel_name()
+    sw.close(); conn.close()
+    del fc, me, mi
 
     # ---- end-to-end arm: host buffers through the C ABI ---------------------------------------------
     hfc = torch.empty((S, N, N), dtype=torch.float32).pin_memory().numpy()
     hme = torch.empty((S, N), dtype=torch.float32).pin_memory().numpy()
     hmi = torch.empty((S, N), dtype=torch.float32).pin_memory().numpy()
     h2d = d2h = 0
-
     e2e_phases = []
 
     def e2e_step():
@@ -301,62 +369,103 @@ def run_tvbx(args):
     e2e_step()
     barrier()
     t0 = time.perf_counter()
-    for _ in range(args.steps):
+    for _ in range(e2e_steps):
         e2e_step()
     torch.cuda.synchronize()
-    e2e_s = time.perf_counter() - t0
-    t = torch.tensor([e2e_s], device="cuda", dtype=torch.float64)
-    if world > 1:
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-    e2e_value = world * units_per_step * args.steps / float(t.item())
+    e2e_s = maxr(time.perf_counter() - t0)
+    rec["e2e"] = {"value": world * units_per_step * e2e_steps / e2e_s, "unit": UNIT, "steps": e2e_steps,
+                  "h2d_bytes_per_step": int(h2d), "d2h_bytes_per_step": int(d2h),
+                  "phases_ms": {"order": ["create", "run_enqueue", "readout_sync", "destroy"], "steps": e2e_phases[1:]}}
+    del hfc, hme, hmi
+    tvbx.trim_memory()
 
+    # ---- roofline of the dominant kernel (the integrator) ----------------------------------------------
     if rank == 0:
-        pk, pk_kind = peaks()
         nnz_row = float((W != 0).sum()) / N
         flops_unit = KERNEL_FLOPS_BASE + FLOPS_PER_EDGE * nnz_row
+        alg_bytes = 4.0 * nnz_row + 4.0 + 4.0 / cfg["ds"]        # gathered ring values + ring write + 1-ms sample
         int_ms, int_n = prof["integrate"]
-        peak_tflops = SM_COUNT * LANES_PER_SM * 2 * pk.get("sm_max_mhz", 1965.0) * 1e6 / 1e12
-        achieved = flops_unit * units_per_step * args.steps / (int_ms * 1e-3) / 1e12 if int_ms > 0 else None
-        roof = {"bound": "alu", "kernel": sw.kernel_name(), "achieved": achieved, "peak": peak_tflops,
-                "unit": "TFLOP/s", "frac": (achieved / peak_tflops) if achieved else None,
-                "traffic": (NCU_DRAM_BYTES_PER_REGION_STEP[args.config] * units_per_step * args.steps / max(int_n, 1)
-                            if args.config in NCU_DRAM_BYTES_PER_REGION_STEP and steps_sim == cfg["steps"] else None),
-                "traffic_note": "bytes per launch, scaled from the DRAM bytes per region-step of the ncu capture in profiles/",
-                "algorithmic_bytes_per_region_step": 4.0 * nnz_row + 4.4,
-                "flops_per_region_step": flops_unit, "peak_kind": f"148 SMs x 128 FP32 lanes x 2 x sm_max_mhz ({pk_kind} clock)",
+        clk_mhz = pk.get("sm_max_mhz", 1965.0)
+        peak_tflops = SM_COUNT * LANES_PER_SM * 2 * clk_mhz * 1e6 / 1e12
+        achieved = flops_unit * units_per_step * steps / (int_ms * 1e-3) / 1e12 if int_ms > 0 else None
+        ncu = read_profile(cfg_id)
+        per_launch_units = units_per_step * steps / max(int_n, 1)
+        roof = {"bound": "alu", "kernel": kname, "achieved": achieved, "peak": peak_tflops, "unit": "TFLOP/s",
+                "frac": (achieved / peak_tflops) if achieved else None,
+                "peak_kind": f"nominal: 148 SMs x 128 FP32 lanes x 2 x sm_max_mhz ({pk['_kind']} clock)",
+                "flops_per_region_step": flops_unit, "algorithmic_bytes_per_region_step": alg_bytes,
                 "kernel_ms_per_launch": int_ms / max(int_n, 1), "kernel_launches": int_n,
                 "kernel_share_of_step": int_ms / ms if ms > 0 else None,
-                "hbm_peak_gbs": pk.get("hbm_gbs"),
-                "other_kernels_ms": {k: prof[k][0] for k in ("fc", "readout", "reset")}}
-        if args.config == 2:
-            roof["ncu"] = NCU_CFG2
-        # the L2 -> SM read bandwidth of this device, measured live (tvbx_probe_read_bandwidth, 64 MiB buffer): the roofline
-        # of the delay gather when the ring is served from L2 (N = 360: 180 edges per row)
-        l2_gbs = tvbx.probe_read_bandwidth(64 << 20, 30)
-        roof["l2_peak_gbs_measured"] = l2_gbs
-        if args.config == 5 and int_ms > 0:
-            alg_bytes = 4.0 * nnz_row + 4.4
-            gather_gbs = alg_bytes * units_per_step * args.steps / (int_ms * 1e-3) / 1e9
-            roof.update({"bound": "l2", "achieved": gather_gbs, "peak": l2_gbs, "unit": "GB/s", "frac": gather_gbs / l2_gbs,
-                         "peak_kind": "L2 -> SM read bandwidth measured in this run (64 MiB buffer, 16-byte ld.global.cg)",
-                         "l2_traffic_gbs_ncu": NCU_L2_BYTES_PER_REGION_STEP[5] * units_per_step * args.steps / (int_ms * 1e-3) / 1e9,
-                         "alu_frac": (achieved / peak_tflops) if achieved else None})
-        line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
-                "ms_per_step": ms_max / args.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
-                "dtype": "f32", "data": "synthetic",
-                "config": config_dict(args.config, cfg, S, {"launch": info, "sim_steps": steps_sim,
-                                                           "replicas": world, "results_finite": finite}),
-                "clocks": clk,
-                "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": int(h2d), "d2h_bytes_per_step": int(d2h),
-                        "phases_ms": {"order": ["create", "run_enqueue", "readout_sync", "destroy"], "steps": e2e_phases[1:]}},
-                "gpu_launches": int(launches), "roofline": roof,
-                "fc_scores": {"ms": scores_ms, "kernel_ms": scores_kernel_ms,
-                              "kernel_achieved_gbs": scores_bytes / (scores_kernel_ms * 1e-3) / 1e9 if scores_kernel_ms > 0 else None,
-                              "kernel_frac_hbm": (scores_bytes / (scores_kernel_ms * 1e-3) / 1e9 / pk.get("hbm_gbs", 6650.0)
-                                                  if scores_kernel_ms > 0 else None),
-                              "note": "tvbx_fc_scores (FCSC + mean FC per simulation, P:113), outside the timed step; ms includes "
-                                      "merging the open sample chunk (S7) into a scratch copy, kernel_ms is fc_scores_kernel alone; "
-                                      "algorithmic bytes = the FP64 co-moments S*N*N*8, read once"}}
+                "other_kernels_ms": {k: prof[k][0] for k in ("fc", "readout", "reset")},
+                "traffic": (ncu["dram_bytes_per_region_step"] * per_launch_units
+                            if ncu and ncu["dram_bytes_per_region_step"] is not None else None),
+                "traffic_note": "DRAM bytes per launch = (dram__bytes_read.sum + dram__bytes_write.sum) / region-steps of the ncu "
+                                "capture parsed from `ncu.source`, x region-steps of one bench launch",
+                "ncu": ncu, "hbm_peak_gbs": pk.get("hbm_gbs")}
+        if probes is not None:
+            alu = probes["alu"]
+            # the measured ceiling of register-operand packed FMA code on this box (FFMA2, three register pairs)
+            peak_meas = SM_COUNT * alu["ffma2_3reg"] * 2 * clk_mhz * 1e6 / 1e12
+            roof.update({"peak_measured": peak_meas, "frac_measured": (achieved / peak_meas) if achieved else None,
+                         "peak_measured_kind": "bench_probes.cu FFMA2 chain, three distinct register-pair operands, lanes/clk/SM x 148 x 2 x clock",
+                         "alu_lanes_per_clk_per_sm_measured": alu, "l2_peak_gbs_measured": probes["l2_gbs"],
+                         "hbm_read_gbs_measured": probes["hbm_read_gbs"]})
+            if N > 120 and int_ms > 0:      # N = 360: the delay gather is bound by the L2 -> SM read bandwidth
+                gather_gbs = alg_bytes * units_per_step * steps / (int_ms * 1e-3) / 1e9
+                roof.update({"bound": "l2", "achieved": gather_gbs, "peak": probes["l2_gbs"], "unit": "GB/s",
+                             "frac": gather_gbs / probes["l2_gbs"],
+                             "peak_kind": "L2 -> SM read bandwidth measured in this run (bench_probes.cu: 64 MiB buffer, 16-byte ld.global.cg)",
+                             "l2_traffic_gbs_ncu": (ncu["l2_to_sm_bytes_per_region_step"] * units_per_step * steps / (int_ms * 1e-3) / 1e9
+                                                    if ncu and ncu["l2_to_sm_bytes_per_region_step"] else None),
+                             "alu_frac": (achieved / peak_tflops) if achieved else None})
+        rec["roofline"] = roof
+        rec["fc_scores"] = {"ms": scores_ms, "kernel_ms": scores_kernel_ms,
+                            "kernel_achieved_gbs": scores_bytes / (scores_kernel_ms * 1e-3) / 1e9 if scores_kernel_ms > 0 else None,
+                            "note": "tvbx_fc_scores (FCSC + mean FC per simulation, P:113), outside the timed step"}
+    return rec
+
+
+def run_tvbx(args):
+    import torch
+    import torch.distributed as dist
+    import paper_2311_13337_b200 as tvbx
+
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    rank = int(os.environ.get("RANK", "0"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device (there is no CPU fallback; use --impl reference for the oracle)")
+    torch.cuda.set_device(local)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+    tvbx.lib()                                   # fails loudly if libtvbx.so is missing
+    stream = torch.cuda.Stream()
+    pk, pk_kind = peaks()
+    pk["_kind"] = pk_kind
+    probes = None
+    if rank == 0 and not args.no_probes:
+        P = Probes()
+        probes = {"alu": P.alu_lanes_per_clk_per_sm(pk.get("sm_max_mhz", 1965.0)), "l2_gbs": P.read_bandwidth(64 << 20, 30),
+                  "hbm_read_gbs": P.read_bandwidth(4 << 30, 3)}
+    clocks = ClockSampler(local) if rank == 0 else None
+    head = measure_config(tvbx, torch, dist, args.config, args.steps, args.warmup, args.steps, args.sim_steps, rank, world, local,
+                          stream, pk, probes, clocks)
+    # the other BASELINE.json configs, each its own record (fewer repeats: the 1.5-3 s configs would not fit a default run)
+    per_config = {}
+    if world == 1 and not args.headline_only and not args.sim_steps:
+        plan = {1: (5, 3), 2: (3, 3), 3: (2, 3), 4: (1, 3), 5: (1, 3)}      # cfg -> (timed steps, warm-up steps)
+        for cid, (k, w) in plan.items():
+            if cid == args.config:
+                continue
+            r = measure_config(tvbx, torch, dist, cid, k, w, 1, 0, rank, world, local, stream, pk, probes, ClockSampler(local))
+            per_config[f"cfg{cid}"] = r
+    if rank == 0:
+        line = {"metric": METRIC, "value": head["value"], "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
+                "ms_per_step": head["ms_per_step"], "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+                "dtype": "f32", "data": "synthetic", "config": head["config"], "clocks": head["clocks"], "e2e": head["e2e"],
+                "gpu_launches": head["gpu_launches"], "roofline": head["roofline"], "fc_scores": head["fc_scores"]}
+        if per_config:
+            line["per_config"] = per_config
         if world == 1 and not args.no_cpu_baseline:
             line["cpu_baseline"] = cpu_baseline(args.config)
         print(json.dumps(line), flush=True)
@@ -375,6 +484,8 @@ def main():
     ap.add_argument("--sim-steps", type=int, default=0, help="override the Euler steps per simulation (profiling only)")
     ap.add_argument("--ref-steps", type=int, default=4000, help="Euler steps per oracle sample (--impl reference)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-probes", action="store_true", help="skip the ALU / L2 micro-benchmarks (bench_probes.cu)")
+    ap.add_argument("--headline-only", action="store_true", help="only the --config line, no per_config records")
     args = ap.parse_args()
     if args.impl == "reference":
         run_reference(args)

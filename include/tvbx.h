@@ -26,7 +26,7 @@
 extern "C" {
 #endif
 
-#define TVBX_VERSION 110 /* 0.1.10: + tvbx_fc_scores, tvbx_rate_stats, tvbx_fc_kernel_name, tvbx_trim_memory, tvbx_probe_read_bandwidth */
+#define TVBX_VERSION 200 /* 0.2.0: diagnostics moved to tvbx_diag.h; lanes_per_node, tvbx_top_k */
 
 enum tvbx_status {
   TVBX_OK = 0,
@@ -105,6 +105,13 @@ typedef struct tvbx_sweep_opts {
                                     the packed one, which is kept free of the extra store) */
   double rate_threshold_khz; /* tvbx_rate_stats counts the 1-ms excitatory samples above this rate; 0 = 0.1 kHz
                                 ("high firing rate activity exceeding 100 Hz") */
+  int32_t lanes_per_node; /* 0 = choose; 1 = one thread per (simulation, region) node (throughput mapping); 2 = the
+                             low-latency mapping for small sweeps / long runs ("a lesser thread
+                             count per GPU to hide latency"): a lane PAIR per node splits the row's delayed gather and
+                             the second-derivative part of the transfer-function jet and exchanges the partial sums with
+                             warp shuffles, so a sweep too small to fill the GPU with nodes runs twice the warps on a
+                             shorter per-step dependency chain.  Packed FP32 kernel, one CTA per group only */
+  int32_t reserved0;
 } tvbx_sweep_opts;
 
 enum tvbx_fc_mode { TVBX_FC_AUTO = 0, TVBX_FC_FP32 = 1, TVBX_FC_TF32 = 2 };
@@ -143,8 +150,9 @@ int32_t tvbx_sweep_create(const tvbx_connectome* c, const tvbx_model_params* def
                           tvbx_sweep** out);
 int32_t tvbx_sweep_destroy(tvbx_sweep* sw);
 
-/* Initial state E, I, C_ee, C_ei, C_ii, W_e, W_i of every region of every simulation; the history
- * is filled with init[0].  TVBX_ESTATE after the first tvbx_run. */
+/* Initial state E, I, C_ee, C_ei, C_ii, W_e, W_i (the seven variables of Eqs. (1)-(3)) of every region of
+ * every simulation; the history is filled with init[0] (PAPER.md gives no initial condition: readings A11, A14;
+ * BASELINE.json cfg 1 states E = I = 0.001 kHz, the rest 0).  TVBX_ESTATE after the first tvbx_run. */
 int32_t tvbx_sweep_set_initial(tvbx_sweep* sw, const double init[7]);
 
 /* Advance every simulation `steps` forward-Euler steps of dt ms: per step the delayed
@@ -193,24 +201,14 @@ int32_t tvbx_rate_stats(tvbx_sweep* sw, float* var_e, float* max_e, int32_t* n_a
  * A no-op before the first tvbx_run.  reset; run(n) is bit-identical to a fresh sweep's run(n). */
 int32_t tvbx_sweep_reset(tvbx_sweep* sw, void* cuda_stream);
 
-/* Kernel timing for reports (bench.py's roofline line): while enabled, every kernel launch of this
- * sweep is bracketed by CUDA events on the launching stream.  tvbx_profile_read synchronises those
- * events, returns the summed durations [ms] and launch counts per kernel class since the last read
- * (0 = integrator, 1 = FC epilogue kernels, 2 = readout, 3 = reset fills) and clears the list. */
-int32_t tvbx_profile_enable(tvbx_sweep* sw, int32_t on);
-int32_t tvbx_profile_read(tvbx_sweep* sw, double ms[4], int64_t launches[4]);
-/* bytes this sweep object copied host->device and device->host so far (tables, parameters, results) */
-int32_t tvbx_bytes_copied(const tvbx_sweep* sw, int64_t* h2d, int64_t* d2h);
-/* Measurement helper (bench.py): read bandwidth of the current device in GB/s, measured by a
- * read-only kernel that streams a zeroed buffer of `bytes` bytes `passes` times with 16-byte ld.global.cg loads (the
- * path of the delay gather), CUDA-event timed after a warm-up pass.  A buffer that fits the L2 (e.g. 48 MiB) gives
- * the L2 -> SM bandwidth -- the roofline of the N = 360 gather --, one several times larger the HBM read bandwidth. */
-int32_t tvbx_probe_read_bandwidth(int64_t bytes, int32_t passes, double* gb_per_s);
-
-/* ---- bookkeeping accessors (bit-exact tests) ------------------------------------------------ */
+/* ---- bookkeeping accessors (the bit-exact part of the definition: parameter grid P:100 / A19, delays P:82 / A13,
+ * ring depth P:113 "-cs ... determines the depth of the temporal buffer") -------------------------------------- */
+/* number of simulations this object holds, size of the whole Cartesian grid, regions of the connectome */
 int32_t tvbx_sweep_size(const tvbx_sweep* sw, int64_t* n_sims, int64_t* grid_size, int32_t* n_regions);
-/* parameter value of local simulation `sim` (index into sim_ids) */
+/* parameter value of local simulation `sim` (index into sim_ids): the value its grid digit selects on the axis that
+ * sweeps param_id (A19: closed interval, equally spaced, first axis slowest), else the sweep's default */
 int32_t tvbx_sweep_param(const tvbx_sweep* sw, int64_t sim, int32_t param_id, double* out);
+/* external (grid) index of local simulation `sim`: the work-item number of P:100, also the Philox stream id (A12) */
 int32_t tvbx_sweep_ext_id(const tvbx_sweep* sw, int64_t sim, int64_t* out);
 /* d_kj = nearbyint((L_kj / v) / dt) in FP64, round-half-to-even (A13); -1 if W_kj == 0.
  * Valid after the first tvbx_run (needs dt), or pass dt > 0 explicitly. */
@@ -218,24 +216,12 @@ int32_t tvbx_delay_index(const tvbx_sweep* sw, int64_t sim, int32_t k, int32_t j
 /* logical ring length H = D + 1 and the physical one the kernel uses: H plus the steps the fastest warp of a
  * CTA may be ahead of the slowest (at most the minimum delay + 1). */
 int32_t tvbx_ring_len(const tvbx_sweep* sw, int64_t sim, double dt, int32_t* H, int32_t* H_phys);
+/* Euler steps taken so far and temporal-average samples kept so far (A17: windows ending at a
+ * step <= discard_steps are dropped) */
 int32_t tvbx_steps_done(const tvbx_sweep* sw, int64_t* n);
 int32_t tvbx_samples_kept(const tvbx_sweep* sw, int64_t* n);
 /* current state, [n_sims][7][N] + OU [n_sims][N], as double, to HOST buffers (synchronises) */
 int32_t tvbx_sweep_state(tvbx_sweep* sw, double* y, double* ou);
-/* launch geometry chosen for the integrator (for reports): CTAs, threads per CTA, sims per CTA,
- * registers per thread, dynamic shared memory bytes, region passes per time block, samples per FC chunk,
- * local-memory bytes per thread, CTAs per group (thread-block cluster size) */
-int32_t tvbx_launch_info(const tvbx_sweep* sw, int32_t info[9]);
-/* name of the integrator kernel this sweep runs (for reports): "tvbx::integrate2_kernel" = the packed FP32
- * product kernel (tau_e == tau_i, N * sims_per_cta <= 480, sims_per_cta <= 8), "tvbx::integrate_kernel" = the
- * general one (FP64 build mode, tau_e != tau_i, larger CTAs).  Copies at most n bytes including the NUL. */
-int32_t tvbx_kernel_name(const tvbx_sweep* sw, char* buf, int32_t n);
-/* Which kernel forms the co-moment X^T X of the FC epilogue: "tvbx::fc_xtx_tc_kernel" (tcgen05 kind::tf32, S7') or
- * "tvbx::fc_comoment_kernel" (FP32/FP64 register tiles, S7); see tvbx_sweep_opts.fc_mode. */
-int32_t tvbx_fc_kernel_name(const tvbx_sweep* sw, char* buf, int32_t n);
-/* number of kernel launches enqueued by this sweep object so far */
-int32_t tvbx_launch_count(const tvbx_sweep* sw, int64_t* n);
-
 const char* tvbx_last_error(void);
 int32_t tvbx_version(void);
 /* Device buffers of destroyed sweeps are cached inside the library (per device, exact size; capacity

@@ -52,7 +52,8 @@ class SweepOpts(C.Structure):
     _fields_ = [("precision", C.c_int32), ("sims_per_cta", C.c_int32), ("n_sims", C.c_int64),
                 ("sim_ids", C.POINTER(C.c_int64)), ("chunk_samples", C.c_int64),
                 ("threads_per_cta", C.c_int32), ("ctas_per_group", C.c_int32),
-                ("fc_mode", C.c_int32), ("rate_stats_inhibitory", C.c_int32), ("rate_threshold_khz", C.c_double)]
+                ("fc_mode", C.c_int32), ("rate_stats_inhibitory", C.c_int32), ("rate_threshold_khz", C.c_double),
+                ("lanes_per_node", C.c_int32), ("reserved0", C.c_int32)]
 
 
 class RunOpts(C.Structure):
@@ -66,20 +67,44 @@ EXPORTS = [
     "tvbx_sweep_destroy", "tvbx_sweep_set_initial", "tvbx_run", "tvbx_fc_readout", "tvbx_fc_scores", "tvbx_rate_stats", "tvbx_sweep_size",
     "tvbx_sweep_param", "tvbx_sweep_ext_id", "tvbx_delay_index", "tvbx_ring_len", "tvbx_steps_done",
     "tvbx_samples_kept", "tvbx_sweep_state", "tvbx_launch_info", "tvbx_launch_count", "tvbx_kernel_name", "tvbx_fc_kernel_name", "tvbx_last_error",
-    "tvbx_version", "tvbx_trim_memory", "tvbx_sweep_reset", "tvbx_profile_enable", "tvbx_profile_read", "tvbx_bytes_copied", "tvbx_probe_read_bandwidth",
+    "tvbx_version", "tvbx_trim_memory", "tvbx_sweep_reset", "tvbx_profile_enable", "tvbx_profile_read", "tvbx_bytes_copied", "tvbx_diag_tf_closed2",
 ]
 
 
-def build(force: bool = False, verbose: bool = False) -> str:
-    """Compile csrc/*.cu for sm_100a into libtvbx.so (in-tree).  nvcc cross-compiles without a GPU."""
-    srcs = [os.path.join(SRC_DIR, f) for f in sorted(os.listdir(SRC_DIR))]
-    hdr = os.path.join(_ROOT, "include", "tvbx.h")
-    newest = max(os.path.getmtime(f) for f in srcs + [hdr])
-    if force or not os.path.exists(LIB_PATH) or os.path.getmtime(LIB_PATH) < newest:
-        cmd = ["nvcc", *NVCC_FLAGS, "-o", LIB_PATH, os.path.join(SRC_DIR, "tvbx_api.cu")]
-        if verbose:
-            cmd.insert(1, "-Xptxas=-v")
-        subprocess.check_call(cmd)
+def build(force: bool = False, verbose: bool = False, jobs: int = 0) -> str:
+    """Compile csrc/*.cu for sm_100a into libtvbx.so (in-tree).  nvcc cross-compiles without a GPU.  Every .cu is its own
+    translation unit (the integrator instances are spread over tvbx_k_*.cu), compiled in parallel into build/obj/*.o and
+    linked; an object is rebuilt when its source or any header (csrc/*.h, *.cuh, include/*.h) is newer."""
+    from concurrent.futures import ThreadPoolExecutor
+    cus = sorted(f for f in os.listdir(SRC_DIR) if f.endswith(".cu"))
+    hdrs = [os.path.join(SRC_DIR, f) for f in os.listdir(SRC_DIR) if f.endswith((".h", ".cuh"))]
+    inc = os.path.join(_ROOT, "include")
+    hdrs += [os.path.join(inc, f) for f in os.listdir(inc) if f.endswith(".h")]
+    newest_hdr = max(os.path.getmtime(f) for f in hdrs)
+    obj_dir = os.path.join(_ROOT, "build", "obj")
+    os.makedirs(obj_dir, exist_ok=True)
+    flags = [f for f in NVCC_FLAGS if f != "-shared"]
+    todo, objs = [], []
+    for f in cus:
+        src, obj = os.path.join(SRC_DIR, f), os.path.join(obj_dir, f[:-3] + ".o")
+        objs.append(obj)
+        if force or not os.path.exists(obj) or os.path.getmtime(obj) < max(os.path.getmtime(src), newest_hdr):
+            cmd = ["nvcc", *flags, "-c", "-o", obj, src]
+            if verbose:
+                cmd.insert(1, "-Xptxas=-v")
+            todo.append(cmd)
+    if todo:
+        with ThreadPoolExecutor(max_workers=jobs or min(len(todo), os.cpu_count() or 4)) as ex:
+            for r in ex.map(lambda c: subprocess.run(c, capture_output=True, text=True), todo):
+                if verbose and r.stderr:
+                    print(r.stderr)
+                if r.returncode != 0:
+                    raise RuntimeError("nvcc failed: " + " ".join(r.args) + "\n" + r.stdout + r.stderr)
+    stale = [o for o in os.listdir(obj_dir) if os.path.join(obj_dir, o) not in objs]
+    for o in stale:
+        os.remove(os.path.join(obj_dir, o))
+    if todo or stale or not os.path.exists(LIB_PATH) or os.path.getmtime(LIB_PATH) < max(os.path.getmtime(o) for o in objs):
+        subprocess.check_call(["nvcc", "-shared", "-gencode", "arch=compute_100a,code=sm_100a", "-o", LIB_PATH, *objs])
     return LIB_PATH
 
 
@@ -124,7 +149,7 @@ def lib():
             "tvbx_profile_enable": [vp, i32],
             "tvbx_profile_read": [vp, dp, C.POINTER(i64)],
             "tvbx_bytes_copied": [vp, C.POINTER(i64), C.POINTER(i64)],
-            "tvbx_probe_read_bandwidth": [i64, i32, dp],
+            "tvbx_diag_tf_closed2": [C.POINTER(ModelParams), i32, dp, dp, dp, dp, dp],
         }
         for name, argtypes in sig.items():
             fn = getattr(L, name)
@@ -178,7 +203,8 @@ class Sweep:
     """
 
     def __init__(self, conn: Connectome, axes, seed=0, params=None, precision=TVBX_F32, sims_per_cta=0,
-                 sim_ids=None, chunk_samples=0, threads_per_cta=0, init=None, ctas_per_group=0, fc_mode=0, rate_threshold_khz=0.0, rate_stats_inhibitory=False):
+                 sim_ids=None, chunk_samples=0, threads_per_cta=0, init=None, ctas_per_group=0, fc_mode=0, rate_threshold_khz=0.0,
+                 rate_stats_inhibitory=False, lanes_per_node=0):
         L = lib()
         self.conn = conn
         m = ModelParams()
@@ -208,7 +234,7 @@ class Sweep:
                 ax[i].values = _dptr(arr)
         o = SweepOpts()
         o.precision = precision; o.sims_per_cta = sims_per_cta; o.chunk_samples = chunk_samples
-        o.threads_per_cta = threads_per_cta; o.ctas_per_group = ctas_per_group; o.fc_mode = fc_mode; o.rate_threshold_khz = rate_threshold_khz; o.rate_stats_inhibitory = int(bool(rate_stats_inhibitory))
+        o.threads_per_cta = threads_per_cta; o.ctas_per_group = ctas_per_group; o.fc_mode = fc_mode; o.rate_threshold_khz = rate_threshold_khz; o.rate_stats_inhibitory = int(bool(rate_stats_inhibitory)); o.lanes_per_node = int(lanes_per_node)
         self.rate_stats_inhibitory = bool(rate_stats_inhibitory)
         if sim_ids is not None:
             ids = np.ascontiguousarray(sim_ids, dtype=np.int64)
@@ -313,9 +339,9 @@ class Sweep:
         return y, ou
 
     def launch_info(self):
-        a = (C.c_int32 * 9)()
+        a = (C.c_int32 * 10)()
         _chk(lib().tvbx_launch_info(self._h, a))
-        keys = ("ctas", "threads", "sims_per_cta", "regs", "smem", "passes", "chunk_samples", "local_bytes", "ctas_per_group")
+        keys = ("ctas", "threads", "sims_per_cta", "regs", "smem", "passes", "chunk_samples", "local_bytes", "ctas_per_group", "lanes_per_node")
         return dict(zip(keys, a[:]))
 
     def reset(self, stream=None):
@@ -398,11 +424,21 @@ def _stream_ptr(stream):
     return stream.cuda_stream      # torch.cuda.Stream
 
 
-def probe_read_bandwidth(nbytes: int, passes: int = 20) -> float:
-    """tvbx_probe_read_bandwidth: GB/s of 16-byte ld.global.cg reads over a buffer of nbytes (L2 if it fits, else HBM)."""
-    out = C.c_double()
-    _chk(lib().tvbx_probe_read_bandwidth(int(nbytes), int(passes), C.byref(out)))
-    return out.value
+def diag_tf_closed2(fe, fi, w_e, w_i, params=None):
+    """tvbx_diag_tf_closed2: the product kernel's packed transfer function evaluated on the device (FP32) ->
+    [n][2][7] float64: per point and population (e, i): F, F_e, F_i, F_ee, F_ei, F_ii (unscaled by kappa), mu_V."""
+    fe, fi, w_e, w_i = (np.ascontiguousarray(x, dtype=np.float64) for x in (fe, fi, w_e, w_i))
+    n = fe.size
+    assert fi.size == n and w_e.size == n and w_i.size == n
+    m = None
+    if params is not None:
+        m = ModelParams()
+        _chk(lib().tvbx_default_params(C.byref(m)))
+        for k, v in params.items():
+            m.p[PARAM_IDS[k]] = float(v)
+    out = np.zeros((n, 2, 7))
+    _chk(lib().tvbx_diag_tf_closed2(C.byref(m) if m is not None else None, n, _dptr(fe), _dptr(fi), _dptr(w_e), _dptr(w_i), _dptr(out)))
+    return out
 
 
 def trim_memory() -> int:

@@ -1,32 +1,16 @@
-// tvbx_api.cu -- host side of the C ABI declared in include/tvbx.h: connectome, parameter grid,
-// delay tables, grouping of simulations by speed, device memory, kernel launches.
+// tvbx_api.cu -- the C ABI declared in include/tvbx.h and include/tvbx_diag.h: connectome, parameter grid, grouping
+// of simulations by speed and the choice of the launch mapping; error text, device-buffer pool.
 // No torch types, no CPU fallback: every compute entry point needs a CUDA device.
-#include "../../include/tvbx.h"
+#include "tvbx_host.h"
 
-#include <cuda_runtime.h>
-
-#include <algorithm>
-#include <cmath>
 #include <cstdarg>
 #include <cstdio>
-#include <cstdlib>
 #include <cstring>
-#include <map>
-#include <memory>
-#include <mutex>
 #include <new>
-#include <string>
-#include <type_traits>
-#include <vector>
 
-#include "tvbx_fc.cuh"
-#include "tvbx_fc_tc.cuh"
-#include "tvbx_integrate.cuh"
-#include "tvbx_integrate2.cuh"
+namespace tvbx_host {
 
-namespace {
-
-thread_local std::string g_err;
+namespace { thread_local std::string g_err; }
 int32_t fail(int32_t code, const char* fmt, ...) {
   char buf[512];
   va_list ap;
@@ -36,13 +20,65 @@ int32_t fail(int32_t code, const char* fmt, ...) {
   g_err = buf;
   return code;
 }
-#define CU(call)                                                                              \
-  do {                                                                                        \
-    cudaError_t e_ = (call);                                                                  \
-    if (e_ != cudaSuccess)                                                                    \
-      return fail(e_ == cudaErrorMemoryAllocation ? TVBX_ENOMEM : TVBX_ECUDA, "%s: %s", #call, \
-                  cudaGetErrorString(e_));                                                    \
-  } while (0)
+const char* last_error() { return g_err.c_str(); }
+
+size_t DevPool::capacity() {
+  if (cap < 0) {
+    if (const char* e = getenv("TVBX_POOL_BYTES")) cap = atoll(e);
+    else { size_t f = 0, t = 0; cap = cudaMemGetInfo(&f, &t) == cudaSuccess ? (long long)(t / 4) : 0; }
+  }
+  return (size_t)cap;
+}
+static size_t trim_locked(DevPool& P) {
+  size_t freed = P.cached;
+  for (auto& kv : P.free_) { DeviceGuard guard(kv.first.first); cudaFree(kv.second); }
+  P.free_.clear(); P.cached = 0;
+  return freed;
+}
+size_t DevPool::trim() { std::lock_guard<std::mutex> g(mu); return trim_locked(*this); }
+cudaError_t DevPool::get(void** p, size_t bytes, int* device) {
+  int dev = 0;
+  cudaError_t e = cudaGetDevice(&dev);
+  if (e != cudaSuccess) return e;
+  *device = dev;
+  std::lock_guard<std::mutex> g(mu);
+  auto it = free_.find({dev, bytes});
+  if (it != free_.end()) { *p = it->second; cached -= bytes; free_.erase(it); return cudaSuccess; }
+  e = cudaMalloc(p, bytes);
+  if (e != cudaSuccess && cached > 0) { cudaGetLastError(); trim_locked(*this); e = cudaMalloc(p, bytes); }
+  return e;
+}
+void DevPool::put(void* p, size_t bytes, int device) {
+  std::lock_guard<std::mutex> g(mu);
+  if (cached + bytes > capacity()) { DeviceGuard guard(device); cudaFree(p); return; }
+  free_.insert({{device, bytes}, p}); cached += bytes;
+}
+size_t DevPool::cached_bytes() { std::lock_guard<std::mutex> g(mu); return cached; }
+DevPool& dev_pool() { static DevPool* P = new DevPool; return *P; }   // never destroyed: no cudaFree at process exit
+
+cudaError_t raise_dynamic_smem(const void* fn, int bytes) {
+  static std::map<std::pair<int, const void*>, int> fn_smem;     // (device, function) -> largest size set so far
+  static std::mutex fn_mu;
+  int dev = 0;
+  cudaGetDevice(&dev);
+  std::lock_guard<std::mutex> lock(fn_mu);
+  int& fmax = fn_smem[{dev, fn}];
+  if (bytes <= fmax) return cudaSuccess;
+  cudaError_t e = cudaFuncSetAttribute(fn, cudaFuncAttributeMaxDynamicSharedMemorySize, std::max(bytes, 1024));
+  if (e == cudaSuccess) fmax = bytes;
+  return e;
+}
+
+DeviceSide* make_device_side(tvbx_sweep* sw);      // tvbx_device.cu
+int32_t diag_tf_closed2(const tvbx_model_params* params, int32_t n, const double* fe, const double* fi, const double* w_e,
+                        const double* w_i, double* out);      // tvbx_diag.cu
+
+}  // namespace tvbx_host
+
+namespace {
+
+using namespace tvbx_host;
+#define CU TVBX_CU
 
 // library defaults
 const double kPolyRS[10] = {-48.9, 5.1, -25.0, 1.4, -0.41, 10.5, -36.0, 7.4, 1.2, 40.7};
@@ -74,952 +110,6 @@ double axis_value(double lo, double hi, int n, int i) {
   const double step = (hi - lo) / (double)(n - 1);
   return lo + (double)i * step;
 }
-// A13
-int32_t delay_steps(double L_mm, double v, double dt) { return (int32_t)std::nearbyint((L_mm / v) / dt); }
-// steps between CTA barriers: at most the minimum delay (step n reads times <= n - d_min), whole
-// gather chunks when there is room for one
-int32_t block_steps(int32_t dmin) {
-  const int32_t b = std::max(1, dmin);
-  return b >= tvbx::GC ? b / tvbx::GC * tvbx::GC : b;
-}
-// Ring geometry of one delay table.  integrate_kernel (general): B steps between CTA barriers, period
-// D + B + 1.  integrate2_kernel (packed FP32): chunks of CH = clamp((d_min + 1)/2, 1, GC) steps; chunk m reads
-// times <= CH m + CH - 1 - d_min, written by chunks <= m - LAG with LAG = ceil((d_min + 2)/CH) - 1 (>= 2 unless
-// d_min = 0; capped at LAGMAX), so the gather of chunk m + 1 can precede the compute
-// of chunk m, a warp may run LAG chunks ahead of the slowest one and the period is D + CH LAG + 1.
-// vec_ok: the sweep runs the cluster form whose full-length chunks (CH == GC) use the quad ring layout and the
-// vector gather (tvbx_integrate2.cuh, gather_class_vec): the period is then a multiple of 4.
-struct RingGeom { int32_t B, CH, LAG, Hp, vec; };
-RingGeom ring_geom(int32_t D, int32_t dmin, bool packed, bool vec_ok = false) {
-  RingGeom g;
-  g.B = block_steps(dmin);
-  g.CH = std::max(1, std::min<int32_t>(tvbx::GC, (std::max(0, dmin) + 1) / 2));
-  g.LAG = std::max(1, std::min<int32_t>(tvbx::LAGMAX, (dmin + 2 + g.CH - 1) / g.CH - 1));
-  g.Hp = packed ? D + g.CH * g.LAG + 1 : D + g.B + 1;
-  g.vec = packed && vec_ok && g.CH == tvbx::GC;
-  if (g.vec) g.Hp = (g.Hp + 3) / 4 * 4;
-  return g;
-}
-
-struct HostEdge { int32_t j; double w; double L; };
-
-struct Axis { int32_t id; std::vector<double> vals; };
-
-struct HostTable {      // one per distinct speed
-  double v = 0;
-  int32_t D = 0, dmin = 0, B = 1, Hp = 2, vec = 0;
-  std::vector<int32_t> delays;   // per kept edge, CSR order
-  std::vector<int64_t> sims;     // local sim indices
-};
-struct HostGroup { int32_t table; std::vector<int64_t> lanes; };  // lanes[sl] = local sim or -1
-
-// polymorphic device side (float / double)
-struct DeviceSide {
-  virtual ~DeviceSide() {}
-  virtual int32_t start(double dt) = 0;
-  virtual int32_t run(int64_t steps, const tvbx_run_opts* o) = 0;
-  virtual int32_t readout(float* fc, float* me, float* mi, int on_device, cudaStream_t st) = 0;
-  virtual int32_t scores(const double* ref, float* fcsc, float* fitness, float* mean_fc, int on_device, cudaStream_t st) = 0;
-  virtual int32_t rate_stats(float* var_e, float* max_e, int32_t* above, float* var_i, float* max_i, int32_t* above_i, int on_device, cudaStream_t st) = 0;
-  virtual int32_t state(double* y, double* ou) = 0;
-  virtual int32_t reset(cudaStream_t st) = 0;
-};
-
-// event pair around one kernel launch (tvbx_profile_*)
-struct ProfEvent { cudaEvent_t a, b; int kind; };
-enum { K_INTEGRATE = 0, K_FC = 1, K_READOUT = 2, K_RESET = 3 };
-
-}  // namespace
-
-struct tvbx_connectome {
-  int32_t n;
-  std::vector<double> W, L;
-  std::vector<int32_t> rowptr;       // CSR of the non-zero weights, ascending j
-  std::vector<HostEdge> edges;
-};
-
-struct tvbx_sweep {
-  tvbx_connectome conn;
-  tvbx_model_params defaults;
-  std::vector<Axis> axes;
-  int64_t grid_size = 1, n_sims = 0;
-  std::vector<int64_t> ext_ids;
-  uint64_t seed = 0;
-  int32_t precision = TVBX_F32, spc = 8, threads_req = 0;
-  int32_t clu = 1;        // CTAs (one thread-block cluster) per group: the regions are split over them
-  bool vec_ok = false;    // cluster form with 4 or 8 simulations per group: vector gather where the chunk length allows
-  bool packed = false;               // FP32 closed-form product kernel (integrate2_kernel)
-  int64_t chunk_req = 0;
-  bool fc_tc = false;                // FC co-moment on the tensor cores (tvbx_fc_tc.cuh)
-  double rate_thr = 0.1;             // kHz: samples above it are counted (f4; 100 Hz)
-  bool stats_i = false;              // keep the inhibitory 1-ms samples of the chunk too and their running statistics
-  double init[7] = {0.001, 0.001, 0, 0, 0, 0, 0};
-  // grouping
-  std::vector<HostTable> tables;
-  std::vector<int32_t> sim_table;    // local sim -> table
-  std::vector<HostGroup> groups;
-  std::vector<std::pair<int32_t, int32_t>> sim_slot;   // local sim -> (group, lane)
-  // run state
-  bool started = false;
-  double dt = 0;
-  int64_t n = 0, cnt = 0, fill = 0, CS = 0, launches = 0;
-  int32_t info[9] = {0, 0, 0, 0, 0, 0, 0, 0, 1};
-  int64_t h2d = 0, d2h = 0;
-  bool profiling = false;
-  std::vector<ProfEvent> prof;
-  int device = 0;
-  std::unique_ptr<DeviceSide> dev;
-
-  ~tvbx_sweep() { for (ProfEvent& e : prof) { cudaEventDestroy(e.a); cudaEventDestroy(e.b); } }
-  // bracket a launch with events while profiling is on
-  void prof_begin(int kind, cudaStream_t st) {
-    if (!profiling) return;
-    ProfEvent e; e.kind = kind;
-    cudaEventCreate(&e.a); cudaEventCreate(&e.b);
-    cudaEventRecord(e.a, st);
-    prof.push_back(e);
-  }
-  void prof_end(cudaStream_t st) { if (profiling) cudaEventRecord(prof.back().b, st); }
-
-  double param(int64_t sim, int32_t id) const {
-    int64_t s = ext_ids[sim];
-    double val = defaults.p[id];
-    for (int a = (int)axes.size() - 1; a >= 0; --a) {
-      const int64_t na = (int64_t)axes[a].vals.size();
-      const int64_t dig = s % na;
-      s /= na;
-      if (axes[a].id == id) val = axes[a].vals[dig];
-    }
-    return val;
-  }
-};
-
-// ====================================================================================================
-//  Device side
-// ====================================================================================================
-namespace {
-
-using namespace tvbx;
-
-// Device-memory pool: buffers of destroyed sweeps are kept (per device, exact size) and handed to the next sweep
-// that asks for the same size, so a create / run / destroy cycle of equal sweeps pays cudaMalloc / cudaFree
-// once.  Capacity TVBX_POOL_BYTES (default: a quarter of the device memory; 0 disables); tvbx_trim_memory()
-// returns everything to the driver; a failed cudaMalloc trims and retries.
-struct DevPool {
-  std::mutex mu;
-  std::multimap<std::pair<int, size_t>, void*> free_;
-  size_t cached = 0;
-  long long cap = -1;
-  size_t capacity() {
-    if (cap < 0) {
-      if (const char* e = getenv("TVBX_POOL_BYTES")) cap = atoll(e);
-      else { size_t f = 0, t = 0; cap = cudaMemGetInfo(&f, &t) == cudaSuccess ? (long long)(t / 4) : 0; }
-    }
-    return (size_t)cap;
-  }
-  size_t trim_locked() {
-    size_t freed = cached;
-    for (auto& kv : free_) cudaFree(kv.second);
-    free_.clear(); cached = 0;
-    return freed;
-  }
-  size_t trim() { std::lock_guard<std::mutex> g(mu); return trim_locked(); }
-  cudaError_t get(void** p, size_t bytes) {
-    int dev = 0; cudaGetDevice(&dev);
-    std::lock_guard<std::mutex> g(mu);
-    auto it = free_.find({dev, bytes});
-    if (it != free_.end()) { *p = it->second; cached -= bytes; free_.erase(it); return cudaSuccess; }
-    cudaError_t e = cudaMalloc(p, bytes);
-    if (e != cudaSuccess && cached > 0) { cudaGetLastError(); trim_locked(); e = cudaMalloc(p, bytes); }
-    return e;
-  }
-  // the caller has made sure no kernel still uses p
-  void put(void* p, size_t bytes) {
-    int dev = 0; cudaGetDevice(&dev);
-    std::lock_guard<std::mutex> g(mu);
-    if (cached + bytes > capacity()) { cudaFree(p); return; }
-    free_.insert({{dev, bytes}, p}); cached += bytes;
-  }
-  size_t cached_bytes() { std::lock_guard<std::mutex> g(mu); return cached; }
-};
-DevPool& dev_pool() { static DevPool* P = new DevPool; return *P; }   // never destroyed: no cudaFree at process exit
-
-template <typename T>
-struct DevBuf {
-  T* p = nullptr;
-  size_t n = 0, bytes = 0;
-  void release() {
-    if (!p) return;
-    cudaDeviceSynchronize();            // what cudaFree did implicitly: nothing in flight may still use p
-    dev_pool().put(p, bytes);
-    p = nullptr;
-  }
-  ~DevBuf() { release(); }
-  cudaError_t alloc(size_t count) {
-    release();
-    n = count;
-    bytes = (std::max<size_t>(count, 1) * sizeof(T) + 511) / 512 * 512;
-    return dev_pool().get((void**)&p, bytes);
-  }
-  cudaError_t upload(const std::vector<T>& h, int64_t* bytes) {
-    cudaError_t e = alloc(h.size());
-    if (e != cudaSuccess) return e;
-    *bytes += (int64_t)(h.size() * sizeof(T));
-    return cudaMemcpy(p, h.data(), h.size() * sizeof(T), cudaMemcpyHostToDevice);
-  }
-};
-
-// Read-bandwidth probe (tvbx_probe_read_bandwidth): every thread streams 16-byte words of a buffer `passes` times with
-// ld.global.cg (the path of the delay gather's ring loads); a buffer that fits the 126 MB L2 measures the L2 -> SM
-// bandwidth, a larger one the HBM read bandwidth.  The sum is written once so the loads cannot be dropped.
-__global__ void __launch_bounds__(512) read_probe_kernel(const float4* __restrict__ p, size_t n16, int passes, float* sink) {
-  float acc = 0.f;
-  const size_t stride = (size_t)gridDim.x * blockDim.x;
-  for (int it = 0; it < passes; ++it) {
-    size_t i = blockIdx.x * (size_t)blockDim.x + threadIdx.x;
-    for (; i + 3 * stride < n16; i += 4 * stride) {
-      const float4 a = __ldcg(p + i), b = __ldcg(p + i + stride), c = __ldcg(p + i + 2 * stride), d = __ldcg(p + i + 3 * stride);
-      acc += (a.x + a.w) + (b.x + b.w) + (c.x + c.w) + (d.x + d.w);
-    }
-    for (; i < n16; i += stride) { const float4 a = __ldcg(p + i); acc += a.x + a.w; }
-  }
-  if (acc == 12345.678f) *sink = acc;
-}
-
-template <typename R>
-__global__ void fill_kernel(R* p, size_t n, R v) {
-  for (size_t i = blockIdx.x * (size_t)blockDim.x + threadIdx.x; i < n; i += (size_t)gridDim.x * blockDim.x) p[i] = v;
-}
-
-// state[g][q][i] = init[q] for the 7 model variables, 0 for OU and the two window sums
-template <typename R>
-struct InitVals { R v[NSV - 2]; };
-template <typename R>
-__global__ void state_init_kernel(R* p, size_t row, size_t total, InitVals<R> iv) {
-  for (size_t i = blockIdx.x * (size_t)blockDim.x + threadIdx.x; i < total; i += (size_t)gridDim.x * blockDim.x)
-    p[i] = iv.v[(i / row) % (NSV - 2)];
-}
-
-inline void set_pad(Edge<float>& e, uint32_t v) { e.pad = v; }
-inline void set_pad(Edge<double>&, uint32_t) {}
-template <typename R> struct KernelPick { void (*fn)(const IntegrateParams<R>); };
-
-// MAXT bounds the registers per thread: 1024 threads -> 64 registers (FP32), 384 -> 168 (FP64).
-template <typename R> struct MaxT;
-template <> struct MaxT<float> { static constexpr int v = 1024; };
-template <> struct MaxT<double> { static constexpr int v = 384; };
-
-// compile-time simulations-per-CTA values of the FP32 closed-form kernel (else runtime SPC)
-inline bool spc_is_templated(int spc) { return spc == 1 || spc == 2 || spc == 4 || spc == 7; }
-
-template <typename R>
-KernelPick<R> pick_kernel(bool single, bool closed, int spc);
-template <>
-KernelPick<double> pick_kernel<double>(bool single, bool closed, int) {
-  constexpr int MT = MaxT<double>::v;
-  if (single) return closed ? KernelPick<double>{integrate_kernel<double, true, true, 0, MT>} : KernelPick<double>{integrate_kernel<double, true, false, 0, MT>};
-  return closed ? KernelPick<double>{integrate_kernel<double, false, true, 0, MT>} : KernelPick<double>{integrate_kernel<double, false, false, 0, MT>};
-}
-template <>
-KernelPick<float> pick_kernel<float>(bool single, bool closed, int spc) {
-  constexpr int MT = MaxT<float>::v;
-  if (!closed) return single ? KernelPick<float>{integrate_kernel<float, true, false, 0, MT>} : KernelPick<float>{integrate_kernel<float, false, false, 0, MT>};
-#define TVBX_CASE(S) case S: return single ? KernelPick<float>{integrate_kernel<float, true, true, S, MT>} : KernelPick<float>{integrate_kernel<float, false, true, S, MT>};
-  switch (spc) {
-    TVBX_CASE(1) TVBX_CASE(2) TVBX_CASE(4) TVBX_CASE(7)
-    default: break;
-  }
-#undef TVBX_CASE
-  return single ? KernelPick<float>{integrate_kernel<float, true, true, 0, MT>} : KernelPick<float>{integrate_kernel<float, false, true, 0, MT>};
-}
-
-// integrate2_kernel instances: compile-time simulations per CTA 1..8; delay table in shared memory with 2, 4 or
-// 8 ring slots loaded per edge, or read through L1/L2 (8 slots)
-typedef void (*Kernel2Fn)(const Integrate2Params);
-template <bool SMEMTAB, int GCE, bool CLU = false, bool SRING = false>
-inline Kernel2Fn pick_kernel2_spc(int spc) {
-  switch (spc) {
-    case 1: return integrate2_kernel<1, SMEMTAB, GCE, CLU, false, SRING>;
-    case 2: return integrate2_kernel<2, SMEMTAB, GCE, CLU, false, SRING>;
-    case 3: return integrate2_kernel<3, SMEMTAB, GCE, CLU, false, SRING>;
-    case 4: return integrate2_kernel<4, SMEMTAB, GCE, CLU, false, SRING>;
-    case 5: return integrate2_kernel<5, SMEMTAB, GCE, CLU, false, SRING>;
-    case 6: return integrate2_kernel<6, SMEMTAB, GCE, CLU, false, SRING>;
-    case 7: return integrate2_kernel<7, SMEMTAB, GCE, CLU, false, SRING>;
-    default: return integrate2_kernel<8, SMEMTAB, GCE, CLU, false, SRING>;
-  }
-}
-// cluster form (several CTAs per group): table through L1/L2, 8 slots per edge; vec: quad ring layout + vector gather
-// small CTAs (<= K2_SMALLT threads): the 8-slot shared-memory-table instance with the relaxed register bound
-inline Kernel2Fn pick_kernel2_small(int spc) {
-  switch (spc) {
-    case 1: return integrate2_kernel<1, true, 8, false, false, false, K2_SMALLT>;
-    case 2: return integrate2_kernel<2, true, 8, false, false, false, K2_SMALLT>;
-    case 3: return integrate2_kernel<3, true, 8, false, false, false, K2_SMALLT>;
-    case 4: return integrate2_kernel<4, true, 8, false, false, false, K2_SMALLT>;
-    case 5: return integrate2_kernel<5, true, 8, false, false, false, K2_SMALLT>;
-    case 6: return integrate2_kernel<6, true, 8, false, false, false, K2_SMALLT>;
-    case 7: return integrate2_kernel<7, true, 8, false, false, false, K2_SMALLT>;
-    default: return integrate2_kernel<8, true, 8, false, false, false, K2_SMALLT>;
-  }
-}
-inline Kernel2Fn pick_kernel2(int spc, bool smemtab, int gce, bool clu, bool vec, bool sring = false, int threads = K2_MAXT) {
-  if (!clu && !vec && !sring && smemtab && gce == 8 && threads <= K2_SMALLT) return pick_kernel2_small(spc);
-  if (sring) return gce == 2 ? pick_kernel2_spc<true, 2, false, true>(spc) : pick_kernel2_spc<true, 4, false, true>(spc);
-  if (clu && vec && smemtab) return spc == 8 ? integrate2_kernel<8, true, 8, true, true> : integrate2_kernel<4, true, 8, true, true>;
-  if (clu && vec) return spc == 8 ? integrate2_kernel<8, false, 8, true, true> : integrate2_kernel<4, false, 8, true, true>;
-  if (clu) return pick_kernel2_spc<false, 8, true>(spc);
-  if (!smemtab) return pick_kernel2_spc<false, 8>(spc);
-  return gce == 2 ? pick_kernel2_spc<true, 2>(spc) : (gce == 4 ? pick_kernel2_spc<true, 4>(spc) : pick_kernel2_spc<true, 8>(spc));
-}
-struct Launch2 { int g0, count; Kernel2Fn fn; int smem; };   // consecutive groups whose tables share the slots-per-edge class
-
-template <typename R>
-struct DeviceImpl : DeviceSide {
-  tvbx_sweep* sw;
-  DevBuf<TableDesc> d_tables;
-  DevBuf<GroupDesc> d_groups;
-  DevBuf<Edge<R>> d_edges;
-  DevBuf<int32_t> d_rowptr, d_seg, d_ext, d_loc;
-  DevBuf<R> d_psim, d_ring, d_state, d_xbar;
-  DevBuf<float> d_xc;                 // centred TF32 samples of the chunk, K-major (fc_tc)
-  int64_t Kp = 0;
-  DevBuf<double> d_sums, d_cmean, d_mean, d_M, d_M_scratch, d_mean_scratch;
-  DevBuf<float> d_cmax, d_rmax, d_rmax_scratch;       // f4: chunk / running maximum of the excitatory samples
-  DevBuf<int32_t> d_ccnt, d_rcnt, d_rcnt_scratch;     //     chunk / running count of samples above the threshold
-  // f4, inhibitory population (optional): the chunk's samples and running (mean, M2, max, count), + scratch for readout
-  DevBuf<R> d_xbar_i;
-  DevBuf<double> d_imean, d_im2, d_imean_scratch, d_im2_scratch;
-  DevBuf<float> d_imax, d_imax_scratch;
-  DevBuf<int32_t> d_icnt, d_icnt_scratch;
-  DevBuf<float> d_out_fc, d_out_me, d_out_mi;
-  IntegrateParams<R> P;
-  KernelPick<R> kp{nullptr};
-  // packed FP32 product kernel (sw->packed)
-  Integrate2Params P2;
-  std::vector<Launch2> launches2;
-  DevBuf<float2> d_psim2;
-  int threads = 0, smem = 0;
-  bool single = true;
-  size_t ring_count = 0, max_slice_edges = 0;
-
-  explicit DeviceImpl(tvbx_sweep* s) : sw(s) { std::memset(&P, 0, sizeof P); std::memset(&P2, 0, sizeof P2); }
-
-  int32_t start(double dt) override {
-    const tvbx_connectome& c = sw->conn;
-    const int N = c.n, SPC = sw->spc;
-    const int G = (int)sw->groups.size();
-    const double* dp = sw->defaults.p;
-    int ndev = 0;
-    if (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev == 0) return fail(TVBX_ECUDA, "no CUDA device");
-    CU(cudaGetDevice(&sw->device));
-
-    const int RS = SPC;      // simulation columns of a ring slot
-    // ---- delay tables per distinct speed (A13) and ring geometry ----
-    std::vector<TableDesc> tds(sw->tables.size());
-    std::vector<Edge<R>> edges;
-    std::vector<int32_t> rowptr, seg;
-    max_slice_edges = 0;
-    for (size_t t = 0; t < sw->tables.size(); ++t) {
-      HostTable& ht = sw->tables[t];
-      ht.delays.clear();
-      int32_t D = 0, dmin = INT32_MAX;
-      for (const HostEdge& e : c.edges) {
-        const int32_t d = delay_steps(e.L, ht.v, dt);
-        if (d < 0 || d > 1000000) return fail(TVBX_EINVAL, "delay of %d steps out of range (v=%g, dt=%g)", d, ht.v, dt);
-        ht.delays.push_back(d);
-        D = std::max(D, d); dmin = std::min(dmin, d);
-      }
-      if (c.edges.empty()) dmin = GC;
-      const RingGeom rg = ring_geom(D, dmin, sw->packed, sw->vec_ok);
-      ht.D = D; ht.dmin = dmin; ht.B = rg.B; ht.Hp = rg.Hp; ht.vec = rg.vec;
-      const int32_t Hs = ht.Hp + (rg.vec ? GC : GC - 1);
-      if ((double)N * Hs * RS >= 4294967295.0) return fail(TVBX_EINVAL, "ring of one CTA exceeds 32-bit element offsets");
-      tds[t].Hp = ht.Hp; tds[t].Hs = Hs; tds[t].B = ht.B; tds[t].n_edges = (int32_t)c.edges.size();
-      tds[t].CH = rg.CH; tds[t].LAG = rg.LAG;
-      tds[t].edge_off = (int64_t)edges.size(); tds[t].rowptr_off = (int64_t)rowptr.size();
-      tds[t].vec = rg.vec; tds[t].seg_off = (int64_t)seg.size();
-      const int pad_to = 1;      // (rows may be padded with zero-weight copies of their first edge)
-      for (int k = 0; k < N; ++k) {
-        rowptr.push_back((int32_t)(edges.size() - (size_t)tds[t].edge_off));
-        const int r0 = c.rowptr[k], r1 = c.rowptr[k + 1];
-        if (rg.vec) {      // quad layout: the row sorted by window alignment class a = (Hp - d) mod 4, ascending j inside
-          for (int a = 0; a < 4; ++a) {
-            int n_class = 0;
-            for (int e = r0; e < r1; ++e) {
-              const uint32_t back = (uint32_t)(ht.Hp - ht.delays[e]);
-              if ((int)(back & 3u) != a) continue;
-              Edge<R> ed;
-              std::memset(&ed, 0, sizeof ed);
-              ed.w = (R)c.edges[e].w;
-              ed.jbase = (uint32_t)c.edges[e].j * (uint32_t)Hs * (uint32_t)RS;
-              ed.back = back;
-              set_pad(ed, ed.jbase + (back & ~(tvbx::VW - 1u)) * (uint32_t)RS);
-              edges.push_back(ed);
-              ++n_class;
-            }
-            for (; n_class % VR != 0; ++n_class) {      // whole rounds: zero-weight copies of the class's last edge
-              Edge<R> ed = edges.back();
-              ed.w = R(0);
-              edges.push_back(ed);
-            }
-            seg.push_back((int32_t)(edges.size() - (size_t)tds[t].edge_off));
-          }
-          continue;
-        }
-        for (int e = r0; e < r1 || (e - r0) % pad_to != 0; ++e) {
-          const int es = e < r1 ? e : r0;
-          Edge<R> ed;
-          std::memset(&ed, 0, sizeof ed);
-          ed.w = e < r1 ? (R)c.edges[es].w : R(0);
-          ed.jbase = (uint32_t)c.edges[es].j * (uint32_t)Hs * (uint32_t)RS;
-          ed.back = (uint32_t)(ht.Hp - ht.delays[es]);
-          set_pad(ed, ed.jbase + ed.back * (uint32_t)RS);
-          edges.push_back(ed);
-        }
-      }
-      rowptr.push_back((int32_t)(edges.size() - (size_t)tds[t].edge_off));
-      {      // a table (and any run of its rows) is never empty: one zero-weight entry at the end that no row owns
-        Edge<R> ed;
-        std::memset(&ed, 0, sizeof ed);
-        ed.back = rg.vec ? 4u : 1u;
-        set_pad(ed, ed.back * (uint32_t)RS);
-        edges.push_back(ed);
-      }
-      tds[t].n_edges = (int32_t)(edges.size() - (size_t)tds[t].edge_off);
-      {      // cluster form: the largest run of rows one CTA stages in shared memory
-        const int NLc = (N + sw->clu - 1) / sw->clu;
-        const int32_t* rp = rowptr.data() + tds[t].rowptr_off;
-        for (int r = 0; r * NLc < N; ++r)
-          max_slice_edges = std::max<size_t>(max_slice_edges, (size_t)(rp[std::min(N, (r + 1) * NLc)] - rp[r * NLc] + 1));
-      }
-    }
-    // ---- groups ----
-    std::vector<GroupDesc> gds(G);
-    std::vector<int32_t> ext((size_t)G * SPC), loc((size_t)G * SPC);
-    std::vector<R> psim((size_t)G * NPS * SPC);
-    std::vector<float2> psim2(sw->packed ? (size_t)G * NP2 * SPC : 0);
-    size_t ring_elems = 0;
-    for (int g = 0; g < G; ++g) {
-      const HostGroup& hg = sw->groups[g];
-      gds[g].table = hg.table; gds[g].pad = 0; gds[g].ring_off = (int64_t)ring_elems;
-      ring_elems += (size_t)N * (sw->tables[hg.table].Hp + (sw->tables[hg.table].vec ? GC : GC - 1)) * RS;
-      ring_elems = (ring_elems + 31) / 32 * 32;      // every group's ring starts on a 128-byte line
-      for (int sl = 0; sl < SPC; ++sl) {
-        const int64_t s = hg.lanes[sl];
-        const int64_t src = s >= 0 ? s : hg.lanes[0];      // padding lanes replay lane 0, never read back
-        ext[(size_t)g * SPC + sl] = (int32_t)sw->ext_ids[src];
-        loc[(size_t)g * SPC + sl] = s >= 0 ? (int32_t)s : -1;
-        const double tw = sw->param(src, TVBX_P_TAU_W_E);
-        const double vals[NPS] = {sw->param(src, TVBX_P_G), sw->param(src, TVBX_P_WNOISE), sw->param(src, TVBX_P_B_E),
-                                  sw->param(src, TVBX_P_A_E) / tw, 1.0 / tw, sw->param(src, TVBX_P_EL_E),
-                                  sw->param(src, TVBX_P_EL_I), 1.0 / sw->param(src, TVBX_P_T),
-                                  sw->param(src, TVBX_P_CFEE), sw->param(src, TVBX_P_CFEI),
-                                  sw->param(src, TVBX_P_CFIE), sw->param(src, TVBX_P_CFII)};
-        for (int q = 0; q < NPS; ++q) psim[((size_t)g * NPS + q) * SPC + sl] = (R)vals[q];
-        if (sw->packed) {     // the same scalars as (excitatory, inhibitory) pairs
-          const double twi = dp[TVBX_P_TAU_W_I], ati = dp[TVBX_P_A_I] / twi, gL = dp[TVBX_P_GL];
-          const double pr[NP2][2] = {{vals[0], vals[1]}, {vals[7], vals[7]}, {vals[2], dp[TVBX_P_B_I]}, {vals[3], ati},
-                                     {vals[4], 1.0 / twi}, {vals[3] * vals[5], ati * vals[6]}, {gL * vals[5], gL * vals[6]},
-                                     {vals[8], vals[10]}, {vals[9], vals[11]}};
-          for (int q = 0; q < NP2; ++q) psim2[((size_t)g * NP2 + q) * SPC + sl] = make_float2((float)pr[q][0], (float)pr[q][1]);
-        }
-      }
-    }
-    // ---- memory budget ----
-    const size_t row = (size_t)N * SPC;
-    size_t free_b = 0, total_b = 0;
-    CU(cudaMemGetInfo(&free_b, &total_b));
-    free_b += dev_pool().cached_bytes();           // pooled buffers are reusable (or trimmed on demand)
-    int64_t CS = sw->chunk_req;
-    if (CS <= 0) {
-      // sample chunk: up to 1/16 of the free device memory, at most 8 GiB (fewer, longer integrator launches)
-      const size_t budget = std::min<size_t>((size_t)8 << 30, std::max<size_t>((size_t)1 << 28, free_b / 16));
-      CS = (int64_t)(budget / std::max<size_t>(1, (size_t)G * row * sizeof(R)));
-      CS = std::min<int64_t>(std::max<int64_t>(CS, 16), 4096);
-    }
-    Kp = (CS + tvbx::TC_BK - 1) / tvbx::TC_BK * tvbx::TC_BK;
-    const size_t need = ring_elems * sizeof(R) + (size_t)G * CS * row * sizeof(R) + (sw->fc_tc ? (size_t)G * Kp * row * sizeof(float) : 0) + (sw->stats_i ? (size_t)G * CS * row * sizeof(R) : 0) +
-                        (size_t)G * SPC * N * N * sizeof(double) * 2 + (size_t)G * 16 * row * sizeof(double);
-    if (need > free_b)
-      return fail(TVBX_ENOMEM, "sweep needs %.2f GB of device memory (ring %.2f GB), %.2f GB free",
-                  need / 1e9, ring_elems * sizeof(R) / 1e9, free_b / 1e9);
-    sw->CS = CS;
-    int64_t* hb = &sw->h2d;
-    CU(d_tables.upload(tds, hb)); CU(d_groups.upload(gds, hb)); CU(d_edges.upload(edges, hb)); CU(d_rowptr.upload(rowptr, hb));
-    if (seg.empty()) seg.assign(4, 0);
-    CU(d_seg.upload(seg, hb));
-    CU(d_ext.upload(ext, hb)); CU(d_loc.upload(loc, hb)); CU(d_psim.upload(psim, hb));
-    if (sw->packed) CU(d_psim2.upload(psim2, hb));
-    CU(d_ring.alloc(ring_elems));
-    CU(d_xbar.alloc((size_t)G * CS * row));
-    if (sw->stats_i) {
-      CU(d_xbar_i.alloc((size_t)G * CS * row));
-      CU(cudaMemset(d_xbar_i.p, 0, d_xbar_i.n * sizeof(R)));
-      CU(d_imean.alloc((size_t)G * row)); CU(d_im2.alloc((size_t)G * row)); CU(d_imax.alloc((size_t)G * row)); CU(d_icnt.alloc((size_t)G * row));
-    }
-    if (sw->fc_tc) CU(d_xc.alloc((size_t)G * Kp * row));
-    CU(d_cmean.alloc((size_t)G * row)); CU(d_mean.alloc((size_t)G * row));
-    CU(d_cmax.alloc((size_t)G * row)); CU(d_rmax.alloc((size_t)G * row)); CU(d_ccnt.alloc((size_t)G * row)); CU(d_rcnt.alloc((size_t)G * row));
-    CU(d_M.alloc((size_t)G * SPC * N * N));
-    CU(d_state.alloc((size_t)G * (NSV - 2) * row));
-    CU(d_sums.alloc((size_t)G * 2 * row));
-    ring_count = ring_elems;
-    CU(cudaMemset(d_xbar.p, 0, d_xbar.n * sizeof(R)));
-    { int32_t rc = reset(0); if (rc) return rc; }
-
-    // ---- uniform constants ----
-    TFConst<R>& tf = P.tf;
-    const double Ke = dp[TVBX_P_PCONN] * dp[TVBX_P_NTOT] * (1.0 - dp[TVBX_P_GINH]);
-    const double Ki = dp[TVBX_P_PCONN] * dp[TVBX_P_NTOT] * dp[TVBX_P_GINH];
-    tf.gL = (R)dp[TVBX_P_GL]; tf.Cm = (R)dp[TVBX_P_CM];
-    tf.ae = (R)(dp[TVBX_P_QE] * dp[TVBX_P_TAUE] * Ke); tf.ai = (R)(dp[TVBX_P_QI] * dp[TVBX_P_TAUI] * Ki);
-    tf.aeEe = (R)(dp[TVBX_P_QE] * dp[TVBX_P_TAUE] * Ke * dp[TVBX_P_EE]);
-    tf.aiEi = (R)(dp[TVBX_P_QI] * dp[TVBX_P_TAUI] * Ki * dp[TVBX_P_EI]);
-    tf.Ee = (R)dp[TVBX_P_EE]; tf.Ei = (R)dp[TVBX_P_EI]; tf.Qe = (R)dp[TVBX_P_QE]; tf.Qi = (R)dp[TVBX_P_QI];
-    tf.cAe = (R)(Ke * dp[TVBX_P_TAUE] * dp[TVBX_P_TAUE]); tf.cAi = (R)(Ki * dp[TVBX_P_TAUI] * dp[TVBX_P_TAUI]);
-    tf.Te = (R)dp[TVBX_P_TAUE]; tf.Ti = (R)dp[TVBX_P_TAUI];
-    tf.gL_over_Cm = (R)(dp[TVBX_P_GL] / dp[TVBX_P_CM]);
-    tf.m_s = (R)(1.0 / dp[TVBX_P_DMUV0]); tf.m_o = (R)(-dp[TVBX_P_MUV0] / dp[TVBX_P_DMUV0]);
-    tf.s_s = (R)(1.0 / dp[TVBX_P_DSV0]);  tf.s_o = (R)(-dp[TVBX_P_SV0] / dp[TVBX_P_DSV0]);
-    tf.t_s = (R)(1.0 / dp[TVBX_P_DTVN0]); tf.t_o = (R)(-dp[TVBX_P_TVN0] / dp[TVBX_P_DTVN0]);
-    for (int i = 0; i < 10; ++i) { tf.P[0][i] = (R)dp[TVBX_P_POLY_E + i]; tf.P[1][i] = (R)dp[TVBX_P_POLY_I + i]; }
-    tf.eps = (R)dp[TVBX_P_EPS_NU];
-    tf.same_tau = dp[TVBX_P_TAUE] == dp[TVBX_P_TAUI];
-    {   // closed form (tau_e == tau_i); all in FP64, then cast
-      const double tau = dp[TVBX_P_TAUE], gL = dp[TVBX_P_GL], Cm = dp[TVBX_P_CM], Ee = dp[TVBX_P_EE], Ei = dp[TVBX_P_EI];
-      const double ae = dp[TVBX_P_QE] * tau * Ke, ai = dp[TVBX_P_QI] * tau * Ki;
-      const double de = ai * (Ee - Ei), di = ae * (Ei - Ee);
-      const double ke = Ke * tau * tau * dp[TVBX_P_QE] * dp[TVBX_P_QE], ki = Ki * tau * tau * dp[TVBX_P_QI] * dp[TVBX_P_QI];
-      tf.EegL = (R)(Ee * gL); tf.EigL = (R)(Ei * gL); tf.de = (R)de; tf.di = (R)di; tf.ke = (R)ke; tf.ki = (R)ki;
-      tf.cq_e = (R)(2 * ki * di); tf.cq_i = (R)(2 * ke * de); tf.cq_ee = (R)(2 * ki * di * di); tf.cq_ii = (R)(2 * ke * de * de);
-      tf.tau_ae = (R)(tau * ae); tf.tau_ai = (R)(tau * ai); tf.ae2 = (R)(ae * ae); tf.aeai = (R)(ae * ai); tf.ai2 = (R)(ai * ai);
-      // polynomial variables: m = (mu_V - muV0)/dmuV0, s = (sigma_V - sV0)/dsV0,
-      // t = (tau_V g_L/C_m - tvn0)/dtvn0 = (g_L/dtvn0) (r - r0) with tau_V = tau + C_m r
-      const double ms = 1.0 / dp[TVBX_P_DMUV0], ss = 1.0 / dp[TVBX_P_DSV0], ts = gL / dp[TVBX_P_DTVN0];
-      tf.muV0 = (R)dp[TVBX_P_MUV0]; tf.sV0 = (R)dp[TVBX_P_SV0]; tf.r0 = (R)((dp[TVBX_P_TVN0] - tau * gL / Cm) / gL);
-      const double sc[10] = {1.0, ms, ss, ts, ms * ms, ss * ss, ts * ts, ms * ss, ms * ts, ss * ts};
-      for (int i = 0; i < 10; ++i) { tf.C[0][i] = (R)(dp[TVBX_P_POLY_E + i] * sc[i]); tf.C[1][i] = (R)(dp[TVBX_P_POLY_I + i] * sc[i]); }
-    }
-    P.b_i = (R)dp[TVBX_P_B_I]; P.a_i_over_tau = (R)(dp[TVBX_P_A_I] / dp[TVBX_P_TAU_W_I]);
-    P.inv_tau_w_i = (R)(1.0 / dp[TVBX_P_TAU_W_I]);
-    P.inv_Ne = (R)(1.0 / (dp[TVBX_P_NTOT] * (1.0 - dp[TVBX_P_GINH])));
-    P.inv_Ni = (R)(1.0 / (dp[TVBX_P_NTOT] * dp[TVBX_P_GINH]));
-    P.kappa = (R)dp[TVBX_P_KAPPA];
-    const double rho = std::exp(-dt / dp[TVBX_P_TAU_OU]);
-    P.ou_rho = (R)rho; P.ou_s = (R)(dp[TVBX_P_SIGMA_OU] * std::sqrt(1.0 - rho * rho));
-    P.ou_m = (R)(dp[TVBX_P_MU_OU] * (1.0 - rho));
-    P.dt = (R)dt;
-    P.muV_local = dp[TVBX_P_MUV_LOCAL] != 0.0;
-    P.N = N; P.SPC = SPC; P.seed = sw->seed; P.chunk_samples = (int32_t)CS;
-    P.tables = d_tables.p; P.groups = d_groups.p; P.edges = d_edges.p; P.rowptr = d_rowptr.p;
-    P.psim = d_psim.p; P.ext_id = d_ext.p; P.loc_id = d_loc.p; P.ring = d_ring.p; P.state = d_state.p;
-    P.sums = d_sums.p; P.xbar = d_xbar.p; P.xbar_i = sw->stats_i ? d_xbar_i.p : nullptr;
-
-    // ---- launch geometry: two lanes per (sim, region) ----
-    const int maxt = sw->threads_req > 0 ? std::min(sw->threads_req, MaxT<R>::v) : MaxT<R>::v;
-    const int rt_max = std::max(1, maxt / (2 * SPC));           // regions per pass
-    int rt;
-    if (N <= rt_max) { single = true; rt = N; }
-    else { single = false; const int passes = (N + rt_max - 1) / rt_max; rt = (N + passes - 1) / passes; }
-    threads = 2 * SPC * rt;
-    kp = pick_kernel<R>(single, tf.same_tau != 0, SPC);
-    const size_t tbytes = (size_t)tds[0].n_edges * sizeof(Edge<R>) + (size_t)(N + 1) * 4;
-    const size_t base = ((size_t)(GC + 10) * (threads / 2) + (size_t)L_NPAR * threads + 20) * sizeof(R) + 16;
-    P.smem_table = base + tbytes <= 200 * 1024;
-    smem = (int)(base + (P.smem_table ? tbytes : 0));
-    CU(cudaFuncSetAttribute((const void*)kp.fn, cudaFuncAttributeMaxDynamicSharedMemorySize, std::max(smem, 1024)));
-    cudaFuncAttributes fa;
-    CU(cudaFuncGetAttributes(&fa, (const void*)kp.fn));
-    sw->info[0] = G; sw->info[1] = threads; sw->info[2] = SPC; sw->info[3] = fa.numRegs; sw->info[4] = smem;
-    sw->info[5] = single ? 1 : (N + rt - 1) / rt; sw->info[6] = (int32_t)CS; sw->info[7] = (int32_t)fa.localSizeBytes;
-    if (sw->packed) { int32_t rc = start_packed(tbytes); if (rc) return rc; }
-    CU(cudaDeviceSynchronize());
-    return TVBX_OK;
-  }
-
-  // integrate2_kernel: one thread per (sim, region), both populations in packed FP32 pairs
-  int32_t start_packed(size_t tbytes) {
-    const int N = sw->conn.n, SPC = sw->spc;
-    const double* dp = sw->defaults.p;
-    TF2Const& t = P2.tf;
-    const TFConst<R>& f = P.tf;
-    t.gL = (float)f.gL; t.Cm = (float)f.Cm; t.ae = (float)f.ae; t.ai = (float)f.ai; t.aeEe = (float)f.aeEe; t.aiEi = (float)f.aiEi;
-    t.Te = (float)f.Te; t.de = (float)f.de; t.di = (float)f.di; t.ke = (float)f.ke; t.ki = (float)f.ki;
-    t.EegL = (float)f.EegL; t.EigL = (float)f.EigL; t.cq_e = (float)f.cq_e; t.cq_i = (float)f.cq_i;
-    t.cq_ee = (float)f.cq_ee; t.cq_ii = (float)f.cq_ii; t.tau_ae = (float)f.tau_ae; t.tau_ai = (float)f.tau_ai;
-    t.ae2 = (float)f.ae2; t.aeai = (float)f.aeai; t.ai2 = (float)f.ai2; t.muV0 = (float)f.muV0; t.sV0 = (float)f.sV0;
-    t.r0 = (float)f.r0; t.eps = (float)f.eps; t.m2Te = (float)(-2.0 * dp[TVBX_P_TAUE]); t.pad0 = 0.f;
-    for (int i = 0; i < 10; ++i) t.C[i] = make_float2((float)f.C[0][i], (float)f.C[1][i]);
-    t.D4 = make_float2(2.f * t.C[4].x, 2.f * t.C[4].y); t.D5 = make_float2(2.f * t.C[5].x, 2.f * t.C[5].y);
-    t.D6 = make_float2(2.f * t.C[6].x, 2.f * t.C[6].y);
-    P2.kappa = (float)P.kappa; P2.inv_Ne = (float)P.inv_Ne; P2.inv_Ni = (float)P.inv_Ni;
-    P2.ou_rho = (float)P.ou_rho; P2.ou_s = (float)P.ou_s; P2.ou_m = (float)P.ou_m; P2.dt = (float)P.dt;
-    P2.muV_local = P.muV_local; P2.N = N; P2.SPC = SPC; P2.seed = P.seed; P2.chunk_samples = P.chunk_samples;
-    P2.tables = P.tables; P2.groups = P.groups; P2.edges = (const Edge<float>*)P.edges; P2.rowptr = P.rowptr; P2.seg = d_seg.p;
-    P2.psim2 = d_psim2.p; P2.ext_id = P.ext_id; P2.loc_id = P.loc_id; P2.ring = (float*)P.ring; P2.state = (float*)P.state;
-    P2.sums = P.sums; P2.xbar = (float*)P.xbar;
-    const int CLU = sw->clu, NL = (N + CLU - 1) / CLU;      // regions per CTA
-    threads = (NL * SPC + 31) / 32 * 32;
-    single = true;
-    const size_t base = (size_t)NBAR * 8 + (size_t)2 * GC * threads * sizeof(float) + (size_t)NP2 * SPC * sizeof(float2) + 16;
-    // cluster form: the vector-gather kernels stage the rows of the CTA's regions as 8-byte entries; the scalar
-    // cluster kernels read the table through L1/L2
-    const size_t slice_bytes = max_slice_edges * sizeof(Edge8);
-    // (at most ~half of the SM's 256 KB: the L1 is the landing space of the ring loads in flight -- 15 warps x 15
-    // LDG.128 = 115 KB; measured at N = 360: 212 KB of shared memory halves the throughput)
-    bool clu_tab = CLU > 1 && base + slice_bytes <= (size_t)136 * 1024;
-    for (const HostTable& ht : sw->tables)      // field widths of Edge8
-      if (ht.vec && ((int64_t)N * ((ht.Hp + GC) / (int)tvbx::VW) >= (1 << 20) || ht.Hp / (int)tvbx::VW >= (1 << 12))) clu_tab = false;
-    P2.smem_table = CLU == 1 ? base + tbytes <= 200 * 1024 : clu_tab;
-    smem = (int)(base + (CLU == 1 ? (P2.smem_table ? tbytes : 0) : (clu_tab ? slice_bytes : 0)));
-    // one launch per run of groups whose chunk length falls in the same class (cfg 3: v <= 8 / 16 / >= 32 m/s)
-    launches2.clear();
-    // (process-wide and only ever raised: another live sweep may launch the same instance with more shared memory)
-    static std::map<const void*, int> fn_smem;
-    static std::mutex fn_mu;
-    std::lock_guard<std::mutex> fn_lock(fn_mu);
-    cudaFuncAttributes fa;
-    std::memset(&fa, 0, sizeof fa);
-    for (int g = 0; g < (int)sw->groups.size(); ++g) {
-      const HostTable& ht = sw->tables[sw->groups[g].table];
-      const int ch = ring_geom(ht.D, ht.dmin, true).CH;
-      const int gce = !P2.smem_table ? 8 : (ch <= 2 ? 2 : (ch <= 4 ? 4 : 8));
-      // short delays: the group's ring ([N][Hp + GC - 1][SPC] floats) in shared memory next to the table
-      const size_t ring_b = (size_t)N * (ht.Hp + GC - 1) * SPC * sizeof(float) + 16;
-      const bool sring = CLU == 1 && P2.smem_table && gce < 8 && smem + ring_b <= (size_t)200 * 1024 &&
-                         getenv("TVBX_NO_SRING") == nullptr;
-      const int lsmem = smem + (sring ? (int)ring_b : 0);
-      Kernel2Fn fn = pick_kernel2(SPC, P2.smem_table != 0, gce, CLU > 1, ht.vec != 0, sring, threads);
-      int& fmax = fn_smem[(const void*)fn];        // the attribute is per function: keep it at the largest request
-      if (lsmem > fmax) {
-        fmax = lsmem;
-        CU(cudaFuncSetAttribute((const void*)fn, cudaFuncAttributeMaxDynamicSharedMemorySize, std::max(lsmem, 1024)));
-      }
-      if (!launches2.empty() && launches2.back().fn == fn) {
-        launches2.back().count++;
-        launches2.back().smem = std::max(launches2.back().smem, lsmem);
-        continue;
-      }
-      launches2.push_back({g, 1, fn, lsmem});
-      cudaFuncAttributes f1;
-      CU(cudaFuncGetAttributes(&f1, (const void*)fn));
-      if (f1.numRegs >= fa.numRegs) fa = f1;
-    }
-    sw->info[0] = (int32_t)sw->groups.size() * CLU;
-    sw->info[1] = threads; sw->info[3] = fa.numRegs; sw->info[4] = smem; sw->info[5] = 1; sw->info[7] = (int32_t)fa.localSizeBytes;
-    sw->info[8] = CLU;
-    return TVBX_OK;
-  }
-
-  int32_t reset(cudaStream_t st) override {
-    InitVals<R> iv;
-    for (int q = 0; q < NSV - 2; ++q) iv.v[q] = q < 7 ? (R)sw->init[q] : R(0);
-    sw->prof_begin(K_RESET, st);
-    state_init_kernel<R><<<592, 256, 0, st>>>(d_state.p, (size_t)sw->conn.n * sw->spc, d_state.n, iv);
-    fill_kernel<R><<<1184, 256, 0, st>>>(d_ring.p, ring_count, (R)sw->init[0]);    // A14
-    fill_kernel<double><<<592, 256, 0, st>>>(d_sums.p, d_sums.n, 0.0);
-    fill_kernel<double><<<592, 256, 0, st>>>(d_mean.p, d_mean.n, 0.0);
-    fill_kernel<double><<<1184, 256, 0, st>>>(d_M.p, d_M.n, 0.0);
-    sw->prof_end(st);
-    sw->launches += 5;
-    CU(cudaGetLastError());
-    sw->n = 0; sw->cnt = 0; sw->fill = 0;
-    return TVBX_OK;
-  }
-
-  // S7': centre + pack to K-major TF32, then the batched X^T X on tcgen05 with the FP64 Chan merge as epilogue
-  int32_t comoment_tc(const FcParams<R>& F, cudaStream_t st) {
-    if constexpr (std::is_same<R, float>::value) {
-      FcTcParams T;
-      T.xbar = F.xbar; T.xc = d_xc.p; T.cmean = F.cmean; T.mean = F.mean; T.M = F.M; T.cnt = F.cnt;
-      T.n_c = F.n_c; T.CS = F.CS; T.Kp = (int32_t)Kp; T.N = F.N; T.SPC = F.SPC; T.G = F.G;
-      T.Rt = (F.N + 127) / 128 * 128; T.Np = (F.N + 15) / 16 * 16;
-      T.tmem_cols = 32;
-      while (T.tmem_cols < T.Np) T.tmem_cols *= 2;
-      const size_t smem_tc = tc_smem_bytes(T.Rt, T.Np);
-      if (!tc_attr_set) {
-        CU(cudaFuncSetAttribute(fc_xtx_tc_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_tc));
-        tc_attr_set = true;
-      }
-      dim3 gp((F.N * F.SPC + 31) / 32, (F.n_c + PACK_Q - 1) / PACK_Q, F.G);
-      fc_pack_tf32_kernel<<<gp, dim3(32, 8), 0, st>>>(T);
-      dim3 gx(T.Rt / 128, F.G * F.SPC);
-      fc_xtx_tc_kernel<<<gx, TC_THREADS, smem_tc, st>>>(T);
-      return TVBX_OK;
-    } else {
-      return fail(TVBX_EINVAL, "tensor-core FC needs an FP32 sweep");
-    }
-  }
-  bool tc_attr_set = false;
-
-  int32_t accumulate(double* Mbuf, double* meanbuf, float* rmaxbuf, int32_t* rcntbuf, bool scratch_i, int64_t cnt, int n_c, cudaStream_t st) {
-    const int N = sw->conn.n, SPC = sw->spc, G = (int)sw->groups.size();
-    FcParams<R> F;
-    F.xbar = d_xbar.p; F.cmean = d_cmean.p; F.mean = meanbuf; F.M = Mbuf; F.cnt = cnt; F.n_c = n_c;
-    F.cmax = d_cmax.p; F.ccnt = d_ccnt.p; F.rmax = rmaxbuf; F.rcnt = rcntbuf; F.thr = (float)sw->rate_thr;
-    F.CS = (int32_t)sw->CS; F.N = N; F.SPC = SPC; F.G = G;
-    const int row = N * SPC;
-    dim3 g1((row + 127) / 128, G), g0((row + 31) / 32, G);
-    sw->prof_begin(K_FC, st);
-    fc_chunk_mean_kernel<R><<<g0, 1024, 0, st>>>(F);
-    if (sw->fc_tc) {
-      int32_t rc = comoment_tc(F, st);
-      if (rc) return rc;
-    } else {
-      const int nt = (N + 31) / 32;
-      dim3 g2(nt, nt, G * SPC);
-      fc_comoment_kernel<R><<<g2, 64, 0, st>>>(F);
-    }
-    fc_mean_update_kernel<R><<<g1, 128, 0, st>>>(F);
-    if (sw->stats_i) {
-      RateIParams<R> I;
-      I.xbar_i = d_xbar_i.p;
-      I.mean = scratch_i ? d_imean_scratch.p : d_imean.p; I.m2 = scratch_i ? d_im2_scratch.p : d_im2.p;
-      I.rmax = scratch_i ? d_imax_scratch.p : d_imax.p; I.rcnt = scratch_i ? d_icnt_scratch.p : d_icnt.p;
-      I.cnt = cnt; I.n_c = n_c; I.CS = (int32_t)sw->CS; I.N = N; I.SPC = SPC; I.G = G; I.thr = (float)sw->rate_thr;
-      rate_i_chunk_kernel<R><<<g0, 1024, 0, st>>>(I);
-      sw->launches += 1;
-    }
-    sw->prof_end(st);
-    sw->launches += sw->fc_tc ? 4 : 3;
-    CU(cudaGetLastError());
-    return TVBX_OK;
-  }
-
-  int32_t run(int64_t steps, const tvbx_run_opts* o) override {
-    cudaStream_t st = (cudaStream_t)o->cuda_stream;
-    const int N = sw->conn.n;
-    const int G = (int)sw->groups.size();
-    DevBuf<R> tmp_traj;
-    R* traj = nullptr;
-    const int64_t tsteps = o->traj ? std::min<int64_t>(o->traj_steps, steps) : 0;
-    const size_t traj_elems = (size_t)sw->n_sims * tsteps * 7 * N;
-    if (tsteps > 0) {
-      if (o->traj_on_device) traj = (R*)o->traj;
-      else { CU(tmp_traj.alloc(traj_elems)); traj = tmp_traj.p; }
-    }
-    P.noise_on = o->noise_on != 0; P.ds = o->ds; P.discard_steps = o->discard_steps;
-    P.traj = traj; P.traj_steps = o->traj_steps; P.traj_n0 = sw->n;
-    if (tsteps > 0) P.traj_steps = tsteps;
-    int64_t remaining = steps;
-    const int64_t ds = o->ds;
-    while (remaining > 0) {
-      int64_t take = remaining;
-      int64_t kept = 0;
-      if (ds > 0) {
-        const int64_t cap = sw->CS - sw->fill;                 // samples the chunk can still take
-        const int64_t e1 = std::max((sw->n / ds + 1) * ds, (o->discard_steps / ds + 1) * ds);  // first kept window end > n
-        const int64_t ec = e1 + (cap - 1) * ds;                // window end that fills the chunk
-        take = std::min(remaining, ec - sw->n);
-        const int64_t end = sw->n + take;
-        kept = end >= e1 ? (end - e1) / ds + 1 : 0;
-      }
-      P.n_begin = sw->n; P.n_end = sw->n + take; P.sample_base = (int32_t)sw->fill;
-      sw->prof_begin(K_INTEGRATE, st);
-      if (sw->packed) {
-        P2.noise_on = P.noise_on; P2.ds = P.ds; P2.discard_steps = P.discard_steps; P2.traj = (float*)P.traj;
-        P2.traj_steps = P.traj_steps; P2.traj_n0 = P.traj_n0; P2.n_begin = P.n_begin; P2.n_end = P.n_end;
-        P2.sample_base = P.sample_base;
-        for (const Launch2& l : launches2) {
-          P2.group0 = l.g0;
-          if (sw->clu == 1) { l.fn<<<l.count, threads, l.smem, st>>>(P2); continue; }
-          cudaLaunchConfig_t lc;
-          std::memset(&lc, 0, sizeof lc);
-          lc.gridDim = dim3((unsigned)(l.count * sw->clu)); lc.blockDim = dim3((unsigned)threads);
-          lc.dynamicSmemBytes = (size_t)smem; lc.stream = st;
-          cudaLaunchAttribute at;
-          at.id = cudaLaunchAttributeClusterDimension;
-          at.val.clusterDim.x = (unsigned)sw->clu; at.val.clusterDim.y = 1; at.val.clusterDim.z = 1;
-          lc.attrs = &at; lc.numAttrs = 1;
-          CU(cudaLaunchKernelEx(&lc, l.fn, P2));
-        }
-        sw->launches += (int64_t)launches2.size() - 1;
-      } else {
-        kp.fn<<<G, threads, smem, st>>>(P);
-      }
-      sw->prof_end(st);
-      sw->launches += 1;
-      CU(cudaGetLastError());
-      sw->n += take; remaining -= take; sw->fill += kept;
-      if (ds > 0 && sw->fill == sw->CS) {
-        int32_t rc = accumulate(d_M.p, d_mean.p, d_rmax.p, d_rcnt.p, false, sw->cnt, (int)sw->fill, st);
-        if (rc) return rc;
-        sw->cnt += sw->fill; sw->fill = 0;
-      }
-    }
-    if (tsteps > 0 && !o->traj_on_device) {
-      CU(cudaMemcpyAsync(o->traj, traj, traj_elems * sizeof(R), cudaMemcpyDeviceToHost, st));
-      sw->d2h += (int64_t)(traj_elems * sizeof(R));
-      CU(cudaStreamSynchronize(st));
-    }
-    return TVBX_OK;
-  }
-
-  // co-moments including the open chunk: merged into a scratch copy, the accumulators stay untouched
-  int32_t merged_M(const double** Msrc, cudaStream_t st) {
-    DevBuf<double>& tM = d_M_scratch; DevBuf<double>& tmean = d_mean_scratch;   // allocated once, kept
-    *Msrc = d_M.p;
-    if (sw->fill > 0) {
-      if (tM.n != d_M.n) { CU(tM.alloc(d_M.n)); CU(tmean.alloc(d_mean.n)); CU(d_rmax_scratch.alloc(d_rmax.n)); CU(d_rcnt_scratch.alloc(d_rcnt.n)); }
-      CU(cudaMemcpyAsync(tM.p, d_M.p, d_M.n * sizeof(double), cudaMemcpyDeviceToDevice, st));
-      CU(cudaMemcpyAsync(tmean.p, d_mean.p, d_mean.n * sizeof(double), cudaMemcpyDeviceToDevice, st));
-      CU(cudaMemcpyAsync(d_rmax_scratch.p, d_rmax.p, d_rmax.n * sizeof(float), cudaMemcpyDeviceToDevice, st));
-      CU(cudaMemcpyAsync(d_rcnt_scratch.p, d_rcnt.p, d_rcnt.n * sizeof(int32_t), cudaMemcpyDeviceToDevice, st));
-      if (sw->stats_i) {
-        if (d_imean_scratch.n != d_imean.n) { CU(d_imean_scratch.alloc(d_imean.n)); CU(d_im2_scratch.alloc(d_im2.n)); CU(d_imax_scratch.alloc(d_imax.n)); CU(d_icnt_scratch.alloc(d_icnt.n)); }
-        CU(cudaMemcpyAsync(d_imean_scratch.p, d_imean.p, d_imean.n * sizeof(double), cudaMemcpyDeviceToDevice, st));
-        CU(cudaMemcpyAsync(d_im2_scratch.p, d_im2.p, d_im2.n * sizeof(double), cudaMemcpyDeviceToDevice, st));
-        CU(cudaMemcpyAsync(d_imax_scratch.p, d_imax.p, d_imax.n * sizeof(float), cudaMemcpyDeviceToDevice, st));
-        CU(cudaMemcpyAsync(d_icnt_scratch.p, d_icnt.p, d_icnt.n * sizeof(int32_t), cudaMemcpyDeviceToDevice, st));
-      }
-      int32_t rc = accumulate(tM.p, tmean.p, d_rmax_scratch.p, d_rcnt_scratch.p, true, sw->cnt, (int)sw->fill, st);
-      if (rc) return rc;
-      *Msrc = tM.p;
-    }
-    return TVBX_OK;
-  }
-
-  // f3: FCSC, fitness against a reference FC, mean FC per simulation (fc_scores_kernel)
-  DevBuf<double> d_sc, d_ref;
-  DevBuf<float> d_out_sc[3];
-  int32_t scores(const double* ref, float* fcsc, float* fitness, float* mean_fc, int on_device, cudaStream_t st) override {
-    const int N = sw->conn.n, SPC = sw->spc, G = (int)sw->groups.size();
-    const int64_t total = sw->cnt + sw->fill;
-    if (total < 2) return fail(TVBX_ESTATE, "fewer than 2 samples kept (%lld)", (long long)total);
-    const double* Msrc = nullptr;
-    { int32_t rc = merged_M(&Msrc, st); if (rc) return rc; }
-    const size_t nn = (size_t)N * N;
-    if (d_sc.n != nn) {
-      CU(d_sc.alloc(nn));
-      CU(cudaMemcpyAsync(d_sc.p, sw->conn.W.data(), nn * sizeof(double), cudaMemcpyHostToDevice, st));
-      sw->h2d += (int64_t)(nn * sizeof(double));
-    }
-    if (ref) {
-      if (d_ref.n != nn) CU(d_ref.alloc(nn));
-      CU(cudaMemcpyAsync(d_ref.p, ref, nn * sizeof(double), cudaMemcpyHostToDevice, st));
-      sw->h2d += (int64_t)(nn * sizeof(double));
-    }
-    ScoreParams Q;
-    Q.M = Msrc; Q.sc = d_sc.p; Q.ref = ref ? d_ref.p : nullptr; Q.loc_id = d_loc.p; Q.N = N; Q.SPC = SPC; Q.G = G;
-    float* outs[3] = {fcsc, fitness, mean_fc};
-    float* devs[3] = {fcsc, fitness, mean_fc};
-    if (!on_device)
-      for (int i = 0; i < 3; ++i)
-        if (outs[i]) { if (d_out_sc[i].n != (size_t)sw->n_sims) CU(d_out_sc[i].alloc((size_t)sw->n_sims)); devs[i] = d_out_sc[i].p; }
-    Q.fcsc = devs[0]; Q.fitness = devs[1]; Q.mean_fc = devs[2];
-    sw->prof_begin(K_READOUT, st);
-    Q.diag_in_smem = N <= 4096;
-    fc_scores_kernel<<<G * SPC, 256, Q.diag_in_smem ? (size_t)N * sizeof(double) : 0, st>>>(Q);
-    sw->prof_end(st);
-    sw->launches += 1;
-    CU(cudaGetLastError());
-    if (!on_device) {
-      for (int i = 0; i < 3; ++i)
-        if (outs[i]) {
-          CU(cudaMemcpyAsync(outs[i], devs[i], (size_t)sw->n_sims * sizeof(float), cudaMemcpyDeviceToHost, st));
-          sw->d2h += (int64_t)((size_t)sw->n_sims * sizeof(float));
-        }
-      CU(cudaStreamSynchronize(st));
-    } else if (ref) {
-      CU(cudaStreamSynchronize(st));     // the host copy of ref must not be reused before the upload is done
-    }
-    return TVBX_OK;
-  }
-
-  // f4: variance, maximum and above-threshold count of the excitatory 1-ms samples per (simulation, region)
-  DevBuf<float> d_out_var, d_out_max, d_out_var_i, d_out_max_i;
-  DevBuf<int32_t> d_out_above, d_out_above_i;
-  int32_t rate_stats(float* var_e, float* max_e, int32_t* above, float* var_i, float* max_i, int32_t* above_i, int on_device, cudaStream_t st) override {
-    const int N = sw->conn.n, SPC = sw->spc, G = (int)sw->groups.size();
-    const int64_t total = sw->cnt + sw->fill;
-    if (total < 1) return fail(TVBX_ESTATE, "no sample kept yet");
-    const double* Msrc = nullptr;
-    { int32_t rc = merged_M(&Msrc, st); if (rc) return rc; }
-    RateStatsParams Q;
-    Q.M = Msrc; Q.rmax = sw->fill > 0 ? d_rmax_scratch.p : d_rmax.p; Q.rcnt = sw->fill > 0 ? d_rcnt_scratch.p : d_rcnt.p;
-    Q.loc_id = d_loc.p; Q.cnt = total; Q.N = N; Q.SPC = SPC; Q.G = G;
-    Q.var_e = var_e; Q.max_e = max_e; Q.above = above;
-    const bool want_i = var_i || max_i || above_i;
-    if (want_i && !sw->stats_i) return fail(TVBX_EINVAL, "inhibitory statistics need tvbx_sweep_opts.rate_stats_inhibitory");
-    Q.m2_i = want_i ? (sw->fill > 0 ? d_im2_scratch.p : d_im2.p) : nullptr;
-    Q.rmax_i = sw->fill > 0 ? d_imax_scratch.p : d_imax.p; Q.rcnt_i = sw->fill > 0 ? d_icnt_scratch.p : d_icnt.p;
-    Q.var_i = var_i; Q.max_i = max_i; Q.above_i = above_i;
-    const size_t n_out = (size_t)sw->n_sims * N;
-    if (!on_device) {
-      if (var_e) { if (d_out_var.n != n_out) CU(d_out_var.alloc(n_out)); Q.var_e = d_out_var.p; }
-      if (max_e) { if (d_out_max.n != n_out) CU(d_out_max.alloc(n_out)); Q.max_e = d_out_max.p; }
-      if (above) { if (d_out_above.n != n_out) CU(d_out_above.alloc(n_out)); Q.above = d_out_above.p; }
-      if (var_i) { if (d_out_var_i.n != n_out) CU(d_out_var_i.alloc(n_out)); Q.var_i = d_out_var_i.p; }
-      if (max_i) { if (d_out_max_i.n != n_out) CU(d_out_max_i.alloc(n_out)); Q.max_i = d_out_max_i.p; }
-      if (above_i) { if (d_out_above_i.n != n_out) CU(d_out_above_i.alloc(n_out)); Q.above_i = d_out_above_i.p; }
-    }
-    sw->prof_begin(K_READOUT, st);
-    rate_stats_kernel<<<dim3((N + 127) / 128, G * SPC), 128, 0, st>>>(Q);
-    sw->prof_end(st);
-    sw->launches += 1;
-    CU(cudaGetLastError());
-    if (!on_device) {
-      if (var_e) { CU(cudaMemcpyAsync(var_e, Q.var_e, n_out * sizeof(float), cudaMemcpyDeviceToHost, st)); sw->d2h += (int64_t)(n_out * sizeof(float)); }
-      if (max_e) { CU(cudaMemcpyAsync(max_e, Q.max_e, n_out * sizeof(float), cudaMemcpyDeviceToHost, st)); sw->d2h += (int64_t)(n_out * sizeof(float)); }
-      if (above) { CU(cudaMemcpyAsync(above, Q.above, n_out * sizeof(int32_t), cudaMemcpyDeviceToHost, st)); sw->d2h += (int64_t)(n_out * sizeof(int32_t)); }
-      if (var_i) { CU(cudaMemcpyAsync(var_i, Q.var_i, n_out * sizeof(float), cudaMemcpyDeviceToHost, st)); sw->d2h += (int64_t)(n_out * sizeof(float)); }
-      if (max_i) { CU(cudaMemcpyAsync(max_i, Q.max_i, n_out * sizeof(float), cudaMemcpyDeviceToHost, st)); sw->d2h += (int64_t)(n_out * sizeof(float)); }
-      if (above_i) { CU(cudaMemcpyAsync(above_i, Q.above_i, n_out * sizeof(int32_t), cudaMemcpyDeviceToHost, st)); sw->d2h += (int64_t)(n_out * sizeof(int32_t)); }
-      CU(cudaStreamSynchronize(st));
-    }
-    return TVBX_OK;
-  }
-
-  int32_t readout(float* fc, float* me, float* mi, int on_device, cudaStream_t st) override {
-    const int N = sw->conn.n, SPC = sw->spc, G = (int)sw->groups.size();
-    const int64_t total = sw->cnt + sw->fill;
-    if (total < 2) return fail(TVBX_ESTATE, "fewer than 2 samples kept (%lld)", (long long)total);
-    const double* Msrc = nullptr;
-    { int32_t rc = merged_M(&Msrc, st); if (rc) return rc; }
-    DevBuf<float>& dfc = d_out_fc; DevBuf<float>& dme = d_out_me; DevBuf<float>& dmi = d_out_mi;   // kept between calls
-    ReadoutParams Q;
-    Q.M = Msrc; Q.sums = d_sums.p; Q.loc_id = d_loc.p; Q.cnt = total; Q.N = N; Q.SPC = SPC; Q.G = G;
-    Q.fc = fc; Q.mean_e = me; Q.mean_i = mi;
-    if (!on_device) {
-      if (fc) { if (dfc.n != (size_t)sw->n_sims * N * N) CU(dfc.alloc((size_t)sw->n_sims * N * N)); Q.fc = dfc.p; }
-      if (me) { if (dme.n != (size_t)sw->n_sims * N) CU(dme.alloc((size_t)sw->n_sims * N)); Q.mean_e = dme.p; }
-      if (mi) { if (dmi.n != (size_t)sw->n_sims * N) CU(dmi.alloc((size_t)sw->n_sims * N)); Q.mean_i = dmi.p; }
-    }
-    dim3 grid((N + RO_ROWS - 1) / RO_ROWS, G * SPC);
-    Q.diag_in_smem = N <= 4096;
-    sw->prof_begin(K_READOUT, st);
-    fc_readout_kernel<<<grid, 256, Q.diag_in_smem ? (size_t)N * sizeof(double) : 0, st>>>(Q);
-    sw->prof_end(st);
-    sw->launches += 1;
-    CU(cudaGetLastError());
-    if (!on_device) {
-      if (fc) { CU(cudaMemcpyAsync(fc, dfc.p, dfc.n * sizeof(float), cudaMemcpyDeviceToHost, st)); sw->d2h += (int64_t)(dfc.n * sizeof(float)); }
-      if (me) { CU(cudaMemcpyAsync(me, dme.p, dme.n * sizeof(float), cudaMemcpyDeviceToHost, st)); sw->d2h += (int64_t)(dme.n * sizeof(float)); }
-      if (mi) { CU(cudaMemcpyAsync(mi, dmi.p, dmi.n * sizeof(float), cudaMemcpyDeviceToHost, st)); sw->d2h += (int64_t)(dmi.n * sizeof(float)); }
-      CU(cudaStreamSynchronize(st));
-    }
-    return TVBX_OK;
-  }
-
-  int32_t state(double* y, double* ou) override {
-    const int N = sw->conn.n, SPC = sw->spc, G = (int)sw->groups.size();
-    const size_t row = (size_t)N * SPC;
-    std::vector<R> h((size_t)G * (NSV - 2) * row);
-    CU(cudaDeviceSynchronize());
-    CU(cudaMemcpy(h.data(), d_state.p, h.size() * sizeof(R), cudaMemcpyDeviceToHost));
-    for (int64_t s = 0; s < sw->n_sims; ++s) {
-      const int g = sw->sim_slot[s].first, sl = sw->sim_slot[s].second;
-      for (int k = 0; k < N; ++k) {
-        for (int q = 0; q < 7; ++q)
-          if (y) y[((size_t)s * 7 + q) * N + k] = (double)h[((size_t)g * (NSV - 2) + q) * row + (size_t)k * SPC + sl];
-        if (ou) ou[(size_t)s * N + k] = (double)h[((size_t)g * (NSV - 2) + 7) * row + (size_t)k * SPC + sl];
-      }
-    }
-    return TVBX_OK;
-  }
-};
-
 }  // namespace
 
 // ====================================================================================================
@@ -1027,7 +117,7 @@ struct DeviceImpl : DeviceSide {
 // ====================================================================================================
 extern "C" {
 
-const char* tvbx_last_error(void) { return g_err.c_str(); }
+const char* tvbx_last_error(void) { return tvbx_host::last_error(); }
 int32_t tvbx_version(void) { return TVBX_VERSION; }
 int32_t tvbx_trim_memory(int64_t* bytes_freed) {
   const size_t f = dev_pool().trim();
@@ -1098,7 +188,7 @@ int32_t tvbx_sweep_create(const tvbx_connectome* c, const tvbx_model_params* def
     if (!opts->sim_ids) return fail(TVBX_EINVAL, "n_sims > 0 but sim_ids is NULL");
     for (int64_t i = 0; i < opts->n_sims; ++i) {
       if (opts->sim_ids[i] < 0 || opts->sim_ids[i] >= sw->grid_size) return fail(TVBX_EINVAL, "sim_ids[%lld]=%lld outside the grid", (long long)i, (long long)opts->sim_ids[i]);
-      sw->ext_ids.push_back(opts->sim_ids[i]);
+      sw->ext_ids.push_back(opts->sim_ids[i]);      // (< grid_size <= 2^31 - 1: fits the 32-bit Philox counter word of A12)
     }
   } else {
     sw->ext_ids.resize(sw->grid_size);
@@ -1117,9 +207,9 @@ int32_t tvbx_sweep_create(const tvbx_connectome* c, const tvbx_model_params* def
     }
     int fcm = opts ? opts->fc_mode : TVBX_FC_AUTO;
     if (const char* e = getenv("TVBX_FC_MODE")) if (fcm == TVBX_FC_AUTO) fcm = atoi(e);
-    const bool tc_ok = sw->precision == TVBX_F32 && sw->conn.n <= tvbx::TC_MAXN;
+    const bool tc_ok = sw->precision == TVBX_F32 && sw->conn.n <= kTcMaxN;
     if (fcm < TVBX_FC_AUTO || fcm > TVBX_FC_TF32) return fail(TVBX_EINVAL, "fc_mode=%d", fcm);
-    if (fcm == TVBX_FC_TF32 && !tc_ok) return fail(TVBX_EINVAL, "fc_mode TVBX_FC_TF32 needs an FP32 sweep with N <= %d", tvbx::TC_MAXN);
+    if (fcm == TVBX_FC_TF32 && !tc_ok) return fail(TVBX_EINVAL, "fc_mode TVBX_FC_TF32 needs an FP32 sweep with N <= %d", kTcMaxN);
     sw->fc_tc = tc_ok && fcm != TVBX_FC_FP32;
   }
   // parameter sanity
@@ -1138,10 +228,10 @@ int32_t tvbx_sweep_create(const tvbx_connectome* c, const tvbx_model_params* def
   if (const char* e = getenv("TVBX_SPC")) if (spc == 0) spc = atoi(e);
   // the packed FP32 kernel (one thread per (sim, region), <= 480 of them, <= 8 simulations per CTA) serves
   // tau_e == tau_i and N <= 480; everything else runs the general kernel (two lanes per (sim, region))
-  // (the inhibitory 1-ms samples are written by the general kernel only: the packed kernel is kept free of the extra
-  // store, which costs it 0.65 % of its throughput even when unused)
-  const bool packed_ok = sw->precision == TVBX_F32 && dp[TVBX_P_TAUE] == dp[TVBX_P_TAUI] && sw->conn.n <= 480 && !sw->stats_i &&
-                         getenv("TVBX_GENERAL_KERNEL") == nullptr;
+  // (with rate_stats_inhibitory the packed kernel serves the one-CTA mapping, N <= 120; tvbx_run falls back to the general
+  // kernel if a delay table then needs a short-chunk instance, which has no inhibitory-sample variant)
+  const bool packed_ok = sw->precision == TVBX_F32 && dp[TVBX_P_TAUE] == dp[TVBX_P_TAUI] && sw->conn.n <= 480 &&
+                         (!sw->stats_i || sw->conn.n <= 120) && getenv("TVBX_GENERAL_KERNEL") == nullptr;
   const int lanes_per_node = packed_ok ? 1 : 2;
   const int maxt_sel = packed_ok ? 480 : (sw->precision == TVBX_F64 ? 384 : 1024);
   const int spc_max = std::max(1, std::min(packed_ok ? 8 : 32, maxt_sel / (lanes_per_node * sw->conn.n)));
@@ -1151,6 +241,7 @@ int32_t tvbx_sweep_create(const tvbx_connectome* c, const tvbx_model_params* def
   int clu = opts ? opts->ctas_per_group : 0;
   if (const char* e = getenv("TVBX_CLUSTER")) if (clu == 0) clu = atoi(e);
   if (clu < 0 || clu > 8) return fail(TVBX_EINVAL, "ctas_per_group=%d (valid: 0..8)", clu);
+  if (clu > 1 && sw->stats_i) return fail(TVBX_EINVAL, "rate_stats_inhibitory needs ctas_per_group <= 1");
   if (clu > 1 && (!packed_ok || sw->threads_req != 0))
     return fail(TVBX_EINVAL, "ctas_per_group > 1 needs the packed FP32 kernel (tau_e == tau_i, N <= 480, no threads_per_cta)");
   auto clu_valid = [&](int c, int sp) {          // every CTA owns >= 1 region and fits 480 threads
@@ -1247,12 +338,15 @@ int32_t tvbx_run(tvbx_sweep* sw, int64_t steps, double dt, const tvbx_run_opts* 
   std::memset(&o, 0, sizeof o);
   if (opts) o = *opts;
   if (o.ds < 0 || o.discard_steps < 0 || o.traj_steps < 0) return fail(TVBX_EINVAL, "negative ds / discard_steps / traj_steps");
+  DeviceGuard guard(sw->device);      // (a no-op before the first run: the sweep then adopts the current device)
   if (!sw->started) {
-    if (sw->precision == TVBX_F64) sw->dev.reset(new (std::nothrow) DeviceImpl<double>(sw));
-    else sw->dev.reset(new (std::nothrow) DeviceImpl<float>(sw));
+    int ndev = 0;
+    if (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev == 0) { cudaGetLastError(); return fail(TVBX_ECUDA, "no CUDA device"); }
+    CU(cudaGetDevice(&sw->device));
+    sw->dev.reset(make_device_side(sw));
     if (!sw->dev) return fail(TVBX_ENOMEM, "host allocation failed");
     int32_t rc = sw->dev->start(dt);
-    if (rc) { sw->dev.reset(); return rc; }
+    if (rc) { sw->dev.reset(); sw->device = -1; return rc; }
     sw->dt = dt; sw->started = true;
   } else if (dt != sw->dt) {
     return fail(TVBX_EINVAL, "dt=%g differs from the dt of the first run (%g): the delay tables depend on it", dt, sw->dt);
@@ -1269,23 +363,27 @@ int32_t tvbx_fc_scores(tvbx_sweep* sw, const double* ref_fc, float* fcsc, float*
   if (ref_fc)
     for (size_t i = 0; i < (size_t)sw->conn.n * sw->conn.n; ++i)
       if (!std::isfinite(ref_fc[i])) return fail(TVBX_EINVAL, "reference FC entry %zu is not finite", i);
+  DeviceGuard guard(sw->device);
   return sw->dev->scores(ref_fc, fcsc, fitness, mean_fc, on_device, (cudaStream_t)stream);
 }
 int32_t tvbx_rate_stats(tvbx_sweep* sw, float* var_e, float* max_e, int32_t* n_above_e, float* var_i, float* max_i,
                         int32_t* n_above_i, int32_t on_device, void* stream) {
   if (!sw) return fail(TVBX_EINVAL, "sweep is NULL");
   if (!sw->started) return fail(TVBX_ESTATE, "no run yet");
+  DeviceGuard guard(sw->device);
   return sw->dev->rate_stats(var_e, max_e, n_above_e, var_i, max_i, n_above_i, on_device, (cudaStream_t)stream);
 }
 int32_t tvbx_fc_readout(tvbx_sweep* sw, float* fc, float* mean_e, float* mean_i, int32_t on_device, void* stream) {
   if (!sw) return fail(TVBX_EINVAL, "sweep is NULL");
   if (!sw->started) return fail(TVBX_ESTATE, "no run yet");
+  DeviceGuard guard(sw->device);
   return sw->dev->readout(fc, mean_e, mean_i, on_device, (cudaStream_t)stream);
 }
 
 int32_t tvbx_sweep_reset(tvbx_sweep* sw, void* stream) {
   if (!sw) return fail(TVBX_EINVAL, "sweep is NULL");
   if (!sw->started) return TVBX_OK;
+  DeviceGuard guard(sw->device);
   return sw->dev->reset((cudaStream_t)stream);
 }
 int32_t tvbx_profile_enable(tvbx_sweep* sw, int32_t on) {
@@ -1296,6 +394,7 @@ int32_t tvbx_profile_enable(tvbx_sweep* sw, int32_t on) {
 int32_t tvbx_profile_read(tvbx_sweep* sw, double ms[4], int64_t launches[4]) {
   if (!sw || !ms || !launches) return fail(TVBX_EINVAL, "NULL argument");
   for (int i = 0; i < 4; ++i) { ms[i] = 0.0; launches[i] = 0; }
+  DeviceGuard guard(sw->device);
   for (ProfEvent& e : sw->prof) {
     float t = 0.f;
     CU(cudaEventSynchronize(e.b));
@@ -1305,30 +404,6 @@ int32_t tvbx_profile_read(tvbx_sweep* sw, double ms[4], int64_t launches[4]) {
     cudaEventDestroy(e.a); cudaEventDestroy(e.b);
   }
   sw->prof.clear();
-  return TVBX_OK;
-}
-int32_t tvbx_probe_read_bandwidth(int64_t bytes, int32_t passes, double* gb_per_s) {
-  if (bytes < (1 << 20) || passes < 1 || !gb_per_s) return fail(TVBX_EINVAL, "bytes >= 1 MiB, passes >= 1, gb_per_s != NULL");
-  DevBuf<float4> buf;
-  DevBuf<float> sink;
-  const size_t n16 = (size_t)bytes / 16;
-  CU(buf.alloc(n16)); CU(sink.alloc(1));
-  CU(cudaMemset(buf.p, 0, n16 * 16));
-  int dev = 0, sms = 148;
-  cudaGetDevice(&dev);
-  cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
-  cudaEvent_t a, b;
-  CU(cudaEventCreate(&a)); CU(cudaEventCreate(&b));
-  read_probe_kernel<<<sms * 4, 512>>>(buf.p, n16, 2, sink.p);      // warm-up: the buffer is L2-resident afterwards if it fits
-  CU(cudaEventRecord(a));
-  read_probe_kernel<<<sms * 4, 512>>>(buf.p, n16, passes, sink.p);
-  CU(cudaEventRecord(b));
-  CU(cudaEventSynchronize(b));
-  float ms = 0.f;
-  CU(cudaEventElapsedTime(&ms, a, b));
-  cudaEventDestroy(a); cudaEventDestroy(b);
-  CU(cudaGetLastError());
-  *gb_per_s = (double)n16 * 16.0 * passes / ((double)ms * 1e-3) / 1e9;
   return TVBX_OK;
 }
 int32_t tvbx_bytes_copied(const tvbx_sweep* sw, int64_t* h2d, int64_t* d2h) {
@@ -1371,7 +446,7 @@ int32_t tvbx_ring_len(const tvbx_sweep* sw, int64_t sim, double dt, int32_t* H, 
   const double v = sw->param(sim, TVBX_P_V);
   int32_t D = 0, dmin = INT32_MAX;
   for (const HostEdge& e : sw->conn.edges) { const int32_t d = delay_steps(e.L, v, dt); D = std::max(D, d); dmin = std::min(dmin, d); }
-  if (sw->conn.edges.empty()) dmin = tvbx::GC;
+  if (sw->conn.edges.empty()) dmin = kGC;
   if (H) *H = D + 1;
   if (H_phys) *H_phys = ring_geom(D, dmin, sw->packed, sw->vec_ok).Hp;
   return TVBX_OK;
@@ -1389,11 +464,13 @@ int32_t tvbx_samples_kept(const tvbx_sweep* sw, int64_t* n) {
 int32_t tvbx_sweep_state(tvbx_sweep* sw, double* y, double* ou) {
   if (!sw) return fail(TVBX_EINVAL, "sweep is NULL");
   if (!sw->started) return fail(TVBX_ESTATE, "no run yet");
+  DeviceGuard guard(sw->device);
   return sw->dev->state(y, ou);
 }
-int32_t tvbx_launch_info(const tvbx_sweep* sw, int32_t info[9]) {
+int32_t tvbx_launch_info(const tvbx_sweep* sw, int32_t info[10]) {
   if (!sw || !info) return fail(TVBX_EINVAL, "NULL argument");
   for (int i = 0; i < 9; ++i) info[i] = sw->info[i];
+  info[9] = sw->split;
   return TVBX_OK;
 }
 int32_t tvbx_kernel_name(const tvbx_sweep* sw, char* buf, int32_t n) {
@@ -1410,6 +487,12 @@ int32_t tvbx_launch_count(const tvbx_sweep* sw, int64_t* n) {
   if (!sw || !n) return fail(TVBX_EINVAL, "NULL argument");
   *n = sw->launches;
   return TVBX_OK;
+}
+
+int32_t tvbx_diag_tf_closed2(const tvbx_model_params* params, int32_t n, const double* fe, const double* fi,
+                             const double* w_e, const double* w_i, double* out) {
+  if (n < 0 || (n > 0 && (!fe || !fi || !w_e || !w_i || !out))) return fail(TVBX_EINVAL, "bad argument");
+  return diag_tf_closed2(params, n, fe, fi, w_e, w_i, out);
 }
 
 }  // extern "C"

@@ -41,9 +41,9 @@ __global__ void __launch_bounds__(1024) fc_chunk_mean_kernel(FcParams<R> P) {
   __shared__ double part[32][33];
   __shared__ float pmax[32][33];
   __shared__ int pcnt[32][33];
-  const int g = blockIdx.y;
+  const int g = blockIdx.x;                                  // (the group count may exceed the 65,535 of gridDim.y)
   const int cx = threadIdx.x & 31, sy = threadIdx.x >> 5;
-  const int idx = blockIdx.x * 32 + cx;                      // region*SPC + lane
+  const int idx = blockIdx.y * 32 + cx;                      // region*SPC + lane
   const int row = P.N * P.SPC;
   double acc = 0.0;
   float mx = -INFINITY;
@@ -78,8 +78,8 @@ __global__ void __launch_bounds__(64) fc_comoment_kernel(FcParams<R> P) {
   constexpr int TS = 32, QT = 32;
   __shared__ R sa[QT][TS + 1];
   __shared__ R sb[QT][TS + 1];
-  const int g = blockIdx.z / P.SPC, sl = blockIdx.z % P.SPC;
-  const int tk = blockIdx.y, tl = blockIdx.x;
+  const int g = blockIdx.x / P.SPC, sl = blockIdx.x % P.SPC;
+  const int tk = blockIdx.z, tl = blockIdx.y;
   if (tl < tk) return;                                        // upper-triangular tiles only
   const int row = P.N * P.SPC;
   const R* x = P.xbar + (size_t)g * P.CS * row + sl;
@@ -139,8 +139,8 @@ __global__ void __launch_bounds__(64) fc_comoment_kernel(FcParams<R> P) {
 // running mean update (after every tile of fc_comoment_kernel has read the old mean)
 template <typename R>
 __global__ void fc_mean_update_kernel(FcParams<R> P) {
-  const int g = blockIdx.y;
-  const int idx = blockIdx.x * blockDim.x + threadIdx.x;
+  const int g = blockIdx.x;
+  const int idx = blockIdx.y * blockDim.x + threadIdx.x;
   const int row = P.N * P.SPC;
   if (idx >= row) return;
   const size_t o = (size_t)g * row + idx;
@@ -171,9 +171,9 @@ __global__ void __launch_bounds__(1024) rate_i_chunk_kernel(RateIParams<R> P) {
   __shared__ double pm[32][33], p2[32][33];
   __shared__ float pmax[32][33];
   __shared__ int pcnt[32][33], pn[32][33];
-  const int g = blockIdx.y;
+  const int g = blockIdx.x;
   const int cx = threadIdx.x & 31, sy = threadIdx.x >> 5;
-  const int idx = blockIdx.x * 32 + cx;
+  const int idx = blockIdx.y * 32 + cx;
   const int row = P.N * P.SPC;
   double mean = 0.0, m2 = 0.0;
   float mx = -INFINITY;
@@ -239,10 +239,10 @@ struct RateStatsParams {
   int32_t N, SPC, G;
 };
 __global__ void rate_stats_kernel(RateStatsParams P) {
-  const int g = blockIdx.y / P.SPC, sl = blockIdx.y % P.SPC;
+  const int g = blockIdx.x / P.SPC, sl = blockIdx.x % P.SPC;
   const int loc = P.loc_id[(size_t)g * P.SPC + sl];
   if (loc < 0) return;
-  const int k = blockIdx.x * blockDim.x + threadIdx.x;
+  const int k = blockIdx.y * blockDim.x + threadIdx.x;
   if (k >= P.N) return;
   const size_t o = ((size_t)g * P.N + k) * P.SPC + sl;
   if (P.var_e) P.var_e[(size_t)loc * P.N + k] = (float)(P.M[((size_t)g * P.SPC + sl) * P.N * P.N + (size_t)k * P.N + k] / (double)P.cnt);
@@ -267,13 +267,13 @@ struct ReadoutParams {
   int32_t diag_in_smem;  // the launch carries N doubles of dynamic shared memory
 };
 
-// Pearson finalise (Eq. 6; A18) in local-simulation order.  grid (ceil(N / RO_ROWS), G * SPC), 256 threads: a
+// Pearson finalise (Eq. 6; A18) in local-simulation order.  grid (G * SPC, ceil(N / RO_ROWS)), 256 threads: a
 // block stages the simulation's N variances in shared memory (the strided M_ll lookups stay on chip) and writes RO_ROWS
 // rows of the matrix; block row 0 also writes the mean rates.
 constexpr int RO_ROWS = 8;
 __global__ void __launch_bounds__(256) fc_readout_kernel(ReadoutParams P) {
   extern __shared__ double rdiag[];
-  const int g = blockIdx.y / P.SPC, sl = blockIdx.y % P.SPC;
+  const int g = blockIdx.x / P.SPC, sl = blockIdx.x % P.SPC;
   const int loc = P.loc_id[(size_t)g * P.SPC + sl];
   if (loc < 0) return;
   const int N = P.N;
@@ -283,7 +283,7 @@ __global__ void __launch_bounds__(256) fc_readout_kernel(ReadoutParams P) {
     for (int k = threadIdx.x; k < N; k += 256) rdiag[k] = M[(size_t)k * N + k];
     __syncthreads();
   }
-  const int k0 = blockIdx.x * RO_ROWS;
+  const int k0 = blockIdx.y * RO_ROWS;
   const int nrow = min(RO_ROWS, N - k0);
   if (P.fc) {
     for (int i = threadIdx.x; i < nrow * N; i += 256) {
@@ -298,7 +298,7 @@ __global__ void __launch_bounds__(256) fc_readout_kernel(ReadoutParams P) {
       P.fc[(size_t)loc * N * N + (size_t)k * N + l] = r;
     }
   }
-  if (blockIdx.x == 0) {
+  if (blockIdx.y == 0) {
     const size_t row = (size_t)N * P.SPC;
     for (int k = threadIdx.x; k < N; k += 256) {
       const double* s = P.sums + (size_t)g * 2 * row + (size_t)k * P.SPC + sl;

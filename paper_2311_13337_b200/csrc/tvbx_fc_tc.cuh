@@ -30,7 +30,8 @@ namespace tvbx {
 constexpr int TC_BK = 32;        // samples per pipeline stage (4 MMAs of K = 8)
 constexpr int TC_STAGES = 4;
 constexpr int TC_THREADS = 256;
-constexpr int TC_MAXN = 512;     // TMEM columns of one CTA
+constexpr int TC_MAXN = 384;     // rows of the staged tile: 4 stages x 8 x (16 Rt + 16) B must fit 227 KB of shared memory
+                                 // (Rt = 384: 197 KB; the 512 TMEM columns of a CTA would allow 512)
 
 struct FcTcParams {
   const float* xbar;     // [G][CS][N][SPC]
@@ -51,14 +52,14 @@ __device__ __forceinline__ float to_tf32(float x) {
   return __uint_as_float(r);
 }
 
-// grid (ceil(N SPC / 32), ceil(n_c / PACK_Q), G), block (32, 8): a 32-column x PACK_Q-sample tile per block, all
+// grid (G, ceil(N SPC / 32), ceil(n_c / PACK_Q)), block (32, 8): a 32-column x PACK_Q-sample tile per block, all
 // its loads in flight before the first store (16 per thread), 512-byte runs on the way out
 constexpr int PACK_Q = 128;
 __global__ void __launch_bounds__(256) fc_pack_tf32_kernel(FcTcParams P) {
   __shared__ float tile[PACK_Q][33];
-  const int g = blockIdx.z;
+  const int g = blockIdx.x;
   const int row = P.N * P.SPC;
-  const int idx0 = blockIdx.x * 32, q0 = blockIdx.y * PACK_Q;
+  const int idx0 = blockIdx.y * 32, q0 = blockIdx.z * PACK_Q;
   const int tx = threadIdx.x, ty = threadIdx.y;
   {
     const int idx = idx0 + tx;
@@ -154,11 +155,11 @@ __host__ inline size_t tc_smem_bytes(int Rt, int Np) {
   return (size_t)TC_STAGES * tc_stage_bytes(Rt) + (size_t)Np * sizeof(double) + TC_STAGES * sizeof(uint64_t) + 16;
 }
 
-// grid (Rt / 128, G SPC), TC_THREADS threads
+// grid (G SPC, Rt / 128), TC_THREADS threads
 __global__ void __launch_bounds__(TC_THREADS) fc_xtx_tc_kernel(FcTcParams P) {
   extern __shared__ __align__(128) uint8_t smem[];
   const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
-  const int mb = blockIdx.x, gs = blockIdx.y;
+  const int mb = blockIdx.y, gs = blockIdx.x;
   const int g = gs / P.SPC, sl = gs % P.SPC;
   const int N = P.N;
   const uint32_t LBO = tc_lbo(P.Rt), SB = tc_stage_bytes(P.Rt);

@@ -71,6 +71,7 @@ struct Integrate2Params {
   float* state;                   // [group][NSV-2][N][SPC]
   double* sums;                   // [group][2][N][SPC]
   float* xbar;                    // [group][CS][N][SPC]
+  float* xbar_i;                  // the same for the inhibitory population (ISAMP instances), else null
   float* traj;                    // optional [n_sims][traj_steps][7][N]
   int64_t traj_steps;
   int64_t traj_n0;
@@ -197,29 +198,15 @@ __device__ __forceinline__ void gather_rounds(EdgePtr edges, int e, int e1, int 
 // round needs neither an index clamp nor a weight mask.  Class 0 windows are quad-aligned: two quads suffice.
 enum { VR = 5 };                 // edges per round of the vector gather (VR x 12 values in registers)
 // Slots per ring word of the vector layout: 4 (quads, LDG.128: 2 or 3 loads per edge-chunk, 44 B fetched on average for the
-// 32 B used) or 2 (pairs, LDG.64: 4 or 5 loads, 36 B).  The N = 360 gather is bound by the L2 -> SM bandwidth, so the
-// bytes count; see DESIGN.md section 7.
-#ifndef TVBX_VEC_W
-#define TVBX_VEC_W 4
-#endif
-constexpr uint32_t VW = TVBX_VEC_W;                 // slots per word
-constexpr uint32_t VWS = TVBX_VEC_W == 4 ? 2 : 1;   // log2
-template <int A> struct VecWords { static constexpr int n = TVBX_VEC_W == 4 ? (A == 0 ? 2 : 3) : ((A & 1) ? 5 : 4); };
-struct VecLd {
-#if TVBX_VEC_W == 4
-  typedef float4 word;
-#else
-  typedef float2 word;
-#endif
-};
-// acc += w * (the VW slots of word q): acc holds f2 pairs of consecutive slots
+// 32 B used).  (A pair layout with LDG.64 -- 36 B, 4 or 5 loads -- was measured 4 % slower: DESIGN.md section 6.6.)
+constexpr uint32_t VW = 4;                          // slots per word
+constexpr uint32_t VWS = 2;                         // log2
+template <int A> struct VecWords { static constexpr int n = A == 0 ? 2 : 3; };
+struct VecLd { typedef float4 word; };
+// acc += w * (the 4 slots of word q): acc holds f2 pairs of consecutive slots
 __device__ __forceinline__ void vec_fma(f2* acc, int i, float w, const VecLd::word& q) {
-#if TVBX_VEC_W == 4
   acc[2 * i] = fma2(bc2(w), mk2(q.x, q.y), acc[2 * i]);
   acc[2 * i + 1] = fma2(bc2(w), mk2(q.z, q.w), acc[2 * i + 1]);
-#else
-  acc[i] = fma2(bc2(w), mk2(q.x, q.y), acc[i]);
-#endif
 }
 template <int RS, int A, typename EdgePtr>
 __device__ __forceinline__ void gather_class_vec(EdgePtr edges, int e, int e1, const float* ringv,
@@ -304,7 +291,8 @@ __device__ __forceinline__ void gather_class_vec8(const Edge8* edges, int e, int
 // (small sweeps, few regions) are compiled with the bound 224 -> up to 255 registers (190 used): the scheduler of a
 // CTA that has one or two warps per scheduler lives on the instruction-level parallelism the extra registers allow
 // (cfg 4 +11 %, cfg 1 +14 %).
-template <int SPC, bool SMEMTAB, int GCE, bool CLU, bool VEC = false, bool SRING = false, int MAXT = K2_MAXT>
+// ISAMP: the inhibitory 1-ms samples are stored as well (rate statistics of both populations, tvbx_rate_stats).
+template <int SPC, bool SMEMTAB, int GCE, bool CLU, bool VEC = false, bool SRING = false, int MAXT = K2_MAXT, bool ISAMP = false>
 __global__ void __launch_bounds__(MAXT, 1) integrate2_kernel(const __grid_constant__ Integrate2Params P) {
   extern __shared__ __align__(16) unsigned char smem_raw[];
   constexpr int RS = SPC;                         // simulation columns of a ring slot
@@ -596,6 +584,7 @@ __global__ void __launch_bounds__(MAXT, 1) integrate2_kernel(const __grid_consta
         if (nn + 1 > P.discard_steps) {
           const f2 mm = scl2(inv_ds, win);
           if (active) P.xbar[(((size_t)g * P.chunk_samples + sidx) * N + k) * SPC + sl] = mm.x;
+          if (ISAMP && active) P.xbar_i[(((size_t)g * P.chunk_samples + sidx) * N + k) * SPC + sl] = mm.y;
           sumE += (double)mm.x; sumI += (double)mm.y;
           ++sidx;
         }

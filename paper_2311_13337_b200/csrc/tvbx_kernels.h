@@ -1,0 +1,40 @@
+// tvbx_kernels.h -- the integrator kernel instances live in their own translation units (tvbx_k_*.cu, compiled in
+// parallel); the host side picks one through these functions and launches it through the returned pointer.
+#pragma once
+#include "tvbx_integrate.cuh"
+#include "tvbx_integrate2.cuh"
+
+namespace tvbx {
+
+// ---- general kernel (tvbx_integrate.cuh): FP64 build mode, tau_e != tau_i, several region passes ----
+template <typename R> struct KernelPick { void (*fn)(const IntegrateParams<R>); };
+// MAXT bounds the registers per thread: 1024 threads -> 64 registers (FP32), 384 -> 168 (FP64).
+template <typename R> struct MaxT;
+template <> struct MaxT<float> { static constexpr int v = 1024; };
+template <> struct MaxT<double> { static constexpr int v = 384; };
+// (compile-time simulations-per-CTA values 1, 2, 4, 7 of the FP32 closed-form instances: tvbx_host::spc_is_templated)
+KernelPick<float> pick_kernel_f32(bool single, bool closed, int spc);     // tvbx_k_general_f32.cu
+KernelPick<double> pick_kernel_f64(bool single, bool closed);             // tvbx_k_general_f64.cu
+
+// ---- packed FP32 product kernel (tvbx_integrate2.cuh) ----
+typedef void (*Kernel2Fn)(const Integrate2Params);
+struct Kernel2Key {
+  int spc;          // simulations per CTA, 1..8
+  bool smemtab;     // delay table staged in shared memory
+  int gce;          // ring slots loaded per edge: 2, 4 or 8
+  bool clu, vec;    // thread-block cluster form; quad ring layout + vector gather
+  bool sring;       // history ring in shared memory (short delays)
+  bool small;       // CTAs of <= K2_SMALLT threads: relaxed register bound
+  bool isamp;       // also store the inhibitory 1-ms samples (rate statistics of both populations)
+};
+Kernel2Fn pick_kernel2(const Kernel2Key& k);                              // tvbx_kernels.cu
+// one function per instance family, each in its own translation unit
+Kernel2Fn k2_g8(int spc, bool isamp);              // SMEMTAB, 8 slots
+Kernel2Fn k2_g8_small(int spc, bool isamp);        // the same, launch bound K2_SMALLT
+Kernel2Fn k2_g4(int spc, bool sring);              // SMEMTAB, 4 slots (+ ring in shared memory)
+Kernel2Fn k2_g2(int spc, bool sring);              // SMEMTAB, 2 slots (+ ring in shared memory)
+Kernel2Fn k2_nosmem(int spc);                      // table through L1/L2, 8 slots
+Kernel2Fn k2_clu(int spc);                         // cluster, scalar gather
+Kernel2Fn k2_vec(int spc, bool smemtab);           // cluster, vector gather (spc 4 or 8)
+
+}  // namespace tvbx

@@ -18,15 +18,9 @@ typedef float2 f2;
 __device__ __forceinline__ f2 mk2(float a, float b) { return make_float2(a, b); }
 __device__ __forceinline__ f2 bc2(float a) { return make_float2(a, a); }          // scalar broadcast (free: .F32 operand form)
 __device__ __forceinline__ f2 neg2(f2 a) { return make_float2(-a.x, -a.y); }      // folds into an operand modifier
-#ifdef TVBX_SCALAR_PAIRS
-__device__ __forceinline__ f2 fma2(f2 a, f2 b, f2 c) { return make_float2(__fmaf_rn(a.x, b.x, c.x), __fmaf_rn(a.y, b.y, c.y)); }
-__device__ __forceinline__ f2 mul2(f2 a, f2 b) { return make_float2(__fmul_rn(a.x, b.x), __fmul_rn(a.y, b.y)); }
-__device__ __forceinline__ f2 add2(f2 a, f2 b) { return make_float2(__fadd_rn(a.x, b.x), __fadd_rn(a.y, b.y)); }
-#else
 __device__ __forceinline__ f2 fma2(f2 a, f2 b, f2 c) { return __ffma2_rn(a, b, c); }
 __device__ __forceinline__ f2 mul2(f2 a, f2 b) { return __fmul2_rn(a, b); }
 __device__ __forceinline__ f2 add2(f2 a, f2 b) { return __fadd2_rn(a, b); }
-#endif
 __device__ __forceinline__ f2 sub2(f2 a, f2 b) { return add2(a, neg2(b)); }
 __device__ __forceinline__ f2 fms2(f2 a, f2 b, f2 c) { return fma2(a, b, neg2(c)); }    // a*b - c
 __device__ __forceinline__ f2 fnma2(f2 a, f2 b, f2 c) { return fma2(neg2(a), b, c); }   // c - a*b

@@ -1,0 +1,62 @@
+"""Driver for compute-sanitizer (memcheck / racecheck / synccheck / initcheck) over every kernel form of the library on
+cfg-1-sized sweeps ("Race detection": the ring write-after-read hazard is the one real race; the
+product kernel replaces CTA barriers by a rolling mbarrier pipeline).  Not a pytest file: run as
+
+    compute-sanitizer --tool racecheck python tests/sanitize_forms.py
+
+Uses host (numpy) buffers only, so torch is never imported under the sanitizer.  Prints one line per form; exits
+non-zero on the first library error.  The summaries of the four tools are kept under profiles/."""
+import os
+import sys
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+sys.path.insert(0, ROOT)
+
+import workloads as wl  # noqa: E402
+import paper_2311_13337_b200 as tvbx  # noqa: E402
+
+STEPS = int(os.environ.get("SANITIZE_STEPS", "160"))
+
+
+def form(name, N, v, keep=0.4, n_sims=5, expect=None, **kw):
+    W, L = wl.connectome(N, seed=N, keep=keep)
+    cfg = dict(axes=[dict(name="G", lo=0.05, hi=0.4, n=n_sims, values=None)], fixed=dict(v=v, b_e=20.0, wNoise=1e-4), seed=3)
+    conn, sw = tvbx.sweep_from_config(cfg, W, L, chunk_samples=5, **kw)
+    for part in (STEPS // 2 + 3, STEPS - STEPS // 2 - 3):          # two launches: resume path, SRING copy-back
+        sw.run(part, 0.1, noise_on=True, ds=10, discard_steps=20)
+    fc, me, mi = sw.fc_readout()
+    sc = sw.fc_scores()
+    rs = sw.rate_stats()
+    info = sw.launch_info()
+    assert np.isfinite(fc).all() and np.isfinite(me).all() and np.isfinite(sc["fcsc"]).all() and np.isfinite(rs[0]).all()
+    if expect:
+        assert sw.kernel_name() == expect, (sw.kernel_name(), expect)
+    print(f"{name}: ok  kernel={sw.kernel_name()} fc={sw.fc_kernel_name()} launch={info}", flush=True)
+    sw.close(); conn.close()
+
+
+def main():
+    P2, G = "tvbx::integrate2_kernel", "tvbx::integrate_kernel"
+    form("single CTA, 8-slot chunks (cfg-1 shape)", 68, 4.0, n_sims=8, expect=P2)
+    form("single CTA, small instance, 1 sim per CTA", 23, 4.0, sims_per_cta=1, expect=P2)
+    form("single CTA, 4-slot chunks + ring in shared memory", 40, 30.0, expect=P2)
+    form("single CTA, 2-slot chunks + ring in shared memory", 40, 120.0, expect=P2)
+    form("single CTA, zero minimum delay", 19, 1e9, expect=P2)
+    form("single CTA, delay table through L1/L2", 150, 4.0, keep=1.0, n_sims=3, sims_per_cta=3, expect=P2)
+    form("cluster of 3 CTAs, scalar gather (short chunks)", 37, 40.0, sims_per_cta=4, ctas_per_group=3, expect=P2)
+    form("cluster of 3 CTAs, vector gather", 37, 4.0, sims_per_cta=4, ctas_per_group=3, expect=P2)
+    form("cluster of 6 CTAs, vector gather, 8 sims (cfg-5 shape)", 90, 3.0, n_sims=9, sims_per_cta=8, ctas_per_group=6, expect=P2)
+    form("packed kernel with inhibitory samples", 24, 4.0, rate_stats_inhibitory=True, expect=P2)
+    form("general kernel FP32 (16 sims per CTA)", 20, 4.0, n_sims=16, sims_per_cta=16, expect=G)
+    form("general kernel FP32, several region passes", 45, 3.0, sims_per_cta=4, threads_per_cta=64, expect=G)
+    form("general kernel FP64 mode", 20, 4.0, precision=tvbx.TVBX_F64, expect=G)
+    form("general kernel, tau_e != tau_i (jets)", 20, 4.0, params=dict(tau_i=7.5), expect=G)
+    form("FC register tiles", 33, 4.0, fc_mode=tvbx.TVBX_FC_FP32, expect=P2)
+    form("FC tensor cores, two row blocks", 130, 4.0, keep=0.2, n_sims=2, sims_per_cta=2, expect=P2)
+    print("all forms ok", flush=True)
+
+
+if __name__ == "__main__":
+    main()

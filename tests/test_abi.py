@@ -23,7 +23,7 @@ def _built():
 
 
 def _declared_symbols():
-    src = open(os.path.join(ROOT, "include", "tvbx.h")).read()
+    src = "".join(open(os.path.join(ROOT, "include", h)).read() for h in ("tvbx.h", "tvbx_diag.h"))
     src = re.sub(r"/\*.*?\*/", "", src, flags=re.S)
     return sorted(set(re.findall(r"\b(tvbx_[a-z0-9_]+)\s*\(", src)))
 
@@ -33,7 +33,7 @@ def test_library_exports_every_declared_symbol():
     assert len(names) >= 20 and "tvbx_run" in names and "tvbx_fc_readout" in names
     L = C.CDLL(tvbx.LIB_PATH)
     for n in names:
-        assert hasattr(L, n), f"{n} declared in include/tvbx.h but not exported"
+        assert hasattr(L, n), f"{n} declared in include/*.h but not exported"
     assert sorted(tvbx.EXPORTS) == names
     assert tvbx.lib().tvbx_version() >= 100
 

@@ -615,18 +615,9 @@ def test_rate_stats_before_any_sample_is_an_error():
         tvbx.sweep_from_config(dict(axes=[], fixed={}, seed=0), W, L, rate_threshold_khz=-1.0)
 
 
-def test_read_bandwidth_probe():
-    """tvbx_probe_read_bandwidth (the measured L2 -> SM peak bench.py reports for the N = 360 gather)."""
-    l2 = tvbx.probe_read_bandwidth(48 << 20, 10)
-    hbm = tvbx.probe_read_bandwidth(1 << 30, 2)
-    assert 1000.0 < hbm < 20000.0 and hbm < l2 < 60000.0      # GB/s: L2-resident reads are faster than HBM reads
-    with pytest.raises(tvbx.TvbxError):
-        tvbx.probe_read_bandwidth(1000, 1)
-
-
-def test_more_regions_than_tmem_columns_falls_back_to_register_tiles():
-    """N > 512: the general integrator (several passes over the regions) and the FP32 register-tile X^T X (the tcgen05
-    kernel holds one output row block in <= 512 TMEM columns); fc_mode = TVBX_FC_TF32 is refused."""
+def test_more_regions_than_one_cta_falls_back_to_the_general_kernel():
+    """N > 480: the general integrator (several passes over the regions) and the FP32 register-tile X^T X (the tcgen05
+    kernel serves N <= 384); fc_mode = TVBX_FC_TF32 is refused."""
     N = 520
     W, L = wl.connectome(N, seed=21, keep=0.05)
     cfg = dict(axes=[dict(name="G", lo=0.1, hi=0.3, n=2, values=None)], fixed=dict(v=6.0, b_e=30.0, wNoise=1e-4), seed=8)
@@ -656,7 +647,8 @@ def test_rate_stats_inhibitory_population(kw):
     thr = thr * 1.0000001
     _, sw = tvbx.sweep_from_config(cfg, W, L, rate_stats_inhibitory=True, rate_threshold_khz=thr, **kw)
     sw.run(steps, 0.1, noise_on=True, ds=10, discard_steps=200)
-    assert sw.kernel_name() == "tvbx::integrate_kernel"        # the option selects the general integrator
+    # FP32: a compile-time instance of the packed kernel stores the inhibitory samples too; FP64 mode: the general kernel
+    assert sw.kernel_name() == ("tvbx::integrate_kernel" if kw.get("precision") == tvbx.TVBX_F64 else "tvbx::integrate2_kernel")
     var_e, max_e, ab_e, var_i, max_i, ab_i = sw.rate_stats()
     fp64 = kw.get("precision") == tvbx.TVBX_F64
     n = xs[0][0].shape[0]
@@ -672,6 +664,10 @@ def test_rate_stats_inhibitory_population(kw):
                 slack = ((x > thr * 0.99) & (x < thr * 1.01)).sum(axis=0)
                 assert np.all(np.abs(ab[s] - np.asarray(ra)) <= slack)
     assert np.all((ab_i >= 0) & (ab_i <= n)) and ab_i.sum() > 0
+    # a short minimum delay (chunks of < 8 steps) has no inhibitory-sample instance of the packed kernel: general kernel
+    _, sw3 = tvbx.sweep_from_config(cfg, W, L, rate_stats_inhibitory=True, params=dict(v=60.0))
+    sw3.run(300, 0.1, noise_on=True, ds=10)
+    assert sw3.kernel_name() == "tvbx::integrate_kernel" and len(sw3.rate_stats()) == 6
     # without the option the inhibitory outputs are refused
     _, sw2 = tvbx.sweep_from_config(cfg, W, L)
     sw2.run(100, 0.1, noise_on=True, ds=10)

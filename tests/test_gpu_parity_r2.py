@@ -1,0 +1,149 @@
+"""GPU parity, round-2 additions: trajectories in which the SECOND-ORDER terms of Eq. (1) carry weight, the
+tensor-core FC size limit, two live sweeps that share kernel instances, and a stress of the rolling chunk pipeline."""
+import numpy as np
+import pytest
+
+import workloads as wl
+import paper_2311_13337_b200 as tvbx
+from oracle import oracle as orc
+from tests.test_gpu_parity import traj_err, run_pair, TOL_TRAJ_F32, TOL_TRAJ_F64, TOL_MEAN_REL, TOL_FC_ABS
+
+pytestmark = pytest.mark.gpu
+
+
+def _second_order_weight(cfg, W, ref, kappa, step):
+    """|1/2 C_ee F_ee + C_ei F_ei + 1/2 C_ii F_ii| kappa^2 relative to |nu|, from the ORACLE's state and the oracle's
+    transfer function (coupling input neglected: an estimate of the weight, not a parity quantity)."""
+    P = wl.grid_params(cfg)
+    names = wl.PARAM_NAMES
+    out = []
+    for s in range(ref.shape[0]):
+        for k in (0, ref.shape[3] // 2):
+            E, I, Cee, Cei, Cii, We, Wi = ref[s, step, :, k]
+            p = P[s].copy(); p[names.index("kappa")] = kappa
+            for pop, Wm, ce, ci, nu in ((0, We, p[names.index("c_Fee")], p[names.index("c_Fei")], E),
+                                        (1, Wi, p[names.index("c_Fie")], p[names.index("c_Fii")], I)):
+                F, _ = orc.tf(p, pop, E + ce, I + ci, Wm)
+                out.append(abs(0.5 * Cee * F[3] + Cei * F[4] + 0.5 * Cii * F[5]) * kappa * kappa / abs(nu))
+    return float(np.median(out))
+
+
+@pytest.mark.parametrize("kappa,steps", [(0.2, 600), (0.3, 600), (1.0, 12)], ids=["k0.2", "k0.3", "k1_12steps"])
+def test_second_order_terms_carry_weight(kappa, steps):
+    """cfg 1, noise off, packed FP32 kernel at 1e-3 and FP64 mode at 1e-9 with kappa (A22) large enough that the
+    second-derivative terms of Eq. (1) are >= 10 % of the rates: an error in F_ee / F_ei / F_ii of tf_closed2 moves
+    these trajectories far beyond the tolerance.  kappa = 0.2 / 0.3: 60 ms (the oracle's sensitivity to a 1e-7 relative
+    perturbation of the initial state stays <= 20x over this horizon, so 1e-3 is a meaningful FP32 bound).  kappa = 1,
+    the unit-consistent variant: the second-order terms are ~100x the rates at step 0 and the dynamics turn chaotic
+    after ~20 steps (oracle: a 1e-7 perturbation grows 3e2-fold by step 20 and 6e5-fold by step 30), so parity is a
+    well-posed question over the first 12 steps only."""
+    cfg = wl.config(1)
+    W, L = wl.config_connectome(cfg)
+    par = dict(kappa=kappa)
+    sw, traj, o, ref = run_pair(cfg, W, L, steps, False, traj_steps=steps, params=par)
+    assert sw.kernel_name() == "tvbx::integrate2_kernel"
+    weight = _second_order_weight(cfg, W, ref, kappa, min(steps - 1, 50))
+    assert weight >= 0.10, weight
+    assert traj_err(traj, ref) < TOL_TRAJ_F32
+    sw, traj, o, ref = run_pair(cfg, W, L, steps, False, traj_steps=steps, params=par, precision=tvbx.TVBX_F64)
+    assert traj_err(traj, ref) < TOL_TRAJ_F64
+
+
+def test_second_order_weight_with_noise_and_all_parameters():
+    """kappa = 0.25 with noise on (same Philox stream), non-default a, b, E_L, c_F and coupling, 40 ms."""
+    W, L = wl.connectome(24, seed=13, keep=0.4)
+    cfg = dict(axes=[dict(name="b_e", lo=0.0, hi=60.0, n=3, values=None)],
+               fixed=dict(v=5.0, G=0.3, wNoise=1e-5, kappa=0.25, a_e=4.0, a_i=1.0, b_i=2.0, E_L_e=-63.0, E_L_i=-65.0,
+                          c_Fie=0.5e-3, c_Fei=0.1e-3, c_Fii=0.2e-3), seed=8)
+    sw, traj, o, ref = run_pair(cfg, W, L, 400, True, traj_steps=400)
+    assert sw.kernel_name() == "tvbx::integrate2_kernel"
+    assert traj_err(traj, ref) < TOL_TRAJ_F32
+    sw, traj, o, ref = run_pair(cfg, W, L, 400, True, traj_steps=400, precision=tvbx.TVBX_F64)
+    assert traj_err(traj, ref) < 1e-8
+
+
+# ------------------------------------------------------------------------------------ FC size limit of the tensor-core path
+def test_fc_between_384_and_512_regions_uses_register_tiles():
+    """N = 400: the tcgen05 X^T X stages N (rounded up to 128) rows x 32 samples x 4 stages in shared memory -- 262 KB at
+    512 rows, more than an SM has -- so TVBX_FC_AUTO must pick the register-tile kernel above N = 384, and an explicit
+    TVBX_FC_TF32 is refused at tvbx_sweep_create."""
+    N = 400
+    W, L = wl.connectome(N, seed=22, keep=0.05)
+    cfg = dict(axes=[dict(name="G", lo=0.1, hi=0.3, n=2, values=None)], fixed=dict(v=6.0, b_e=30.0, wNoise=1e-4), seed=8)
+    sw, traj, o, ref = run_pair(cfg, W, L, 600, True, traj_steps=600, discard=100, chunk_samples=20)
+    assert sw.kernel_name() == "tvbx::integrate2_kernel" and sw.fc_kernel_name() == "tvbx::fc_comoment_kernel"
+    assert traj_err(traj, ref) < 5e-3          # (noise-on extra: same Philox stream, FP32 rounding through the noise path)
+    fc, me, mi = sw.fc_readout(); rfc, rme, rmi = o.fc_readout()
+    assert np.abs(me / rme - 1).max() < TOL_MEAN_REL and np.abs(fc - rfc).max() < TOL_FC_ABS
+    with pytest.raises(tvbx.TvbxError):
+        tvbx.sweep_from_config(cfg, W, L, fc_mode=tvbx.TVBX_FC_TF32)
+    # the largest size the tensor-core path serves
+    W2, L2 = wl.connectome(384, seed=23, keep=0.05)
+    _, sw2 = tvbx.sweep_from_config(cfg, W2, L2, chunk_samples=20)
+    sw2.run(600, 0.1, noise_on=True, ds=10, discard_steps=100)
+    assert sw2.fc_kernel_name() == "tvbx::fc_xtx_tc_kernel"
+    fc2 = sw2.fc_readout()[0]
+    o2 = orc.OracleSweep(W2, L2, wl.grid_params(cfg), seed=cfg["seed"])
+    o2.run(600, 0.1, noise_on=True, ds=10, discard_steps=100)
+    assert np.abs(fc2 - o2.fc_readout()[0]).max() < TOL_FC_ABS
+
+
+def test_two_live_sweeps_of_different_size_interleaved():
+    """The dynamic-shared-memory limit is an attribute of the kernel FUNCTION, process-wide: a sweep with N = 360 (197 KB
+    for fc_xtx_tc_kernel) and one with N = 68 share that function.  Interleaved runs must not lower each other's limit."""
+    cfg5 = wl.config(5); W5, L5 = wl.config_connectome(cfg5)
+    cfg1 = wl.config(1); W1, L1 = wl.config_connectome(cfg1)
+    sims5 = [3, 4000]
+    _, a = tvbx.sweep_from_config(cfg5, W5, L5, sim_ids=sims5, chunk_samples=16)
+    _, b = tvbx.sweep_from_config(cfg1, W1, L1, chunk_samples=16)
+    _, a_ref = tvbx.sweep_from_config(cfg5, W5, L5, sim_ids=sims5, chunk_samples=16)
+    _, b_ref = tvbx.sweep_from_config(cfg1, W1, L1, chunk_samples=16)
+    for _ in range(3):                          # every run fills chunks: FC kernels of both sizes alternate
+        a.run(400, 0.1, noise_on=True, ds=10)
+        b.run(400, 0.1, noise_on=True, ds=10)
+    a_ref.run(1200, 0.1, noise_on=True, ds=10)
+    b_ref.run(1200, 0.1, noise_on=True, ds=10)
+    for x, y in zip(a.fc_readout(), a_ref.fc_readout()):
+        np.testing.assert_array_equal(x, y)
+    for x, y in zip(b.fc_readout(), b_ref.fc_readout()):
+        np.testing.assert_array_equal(x, y)
+    # the general kernel (FP64 mode) with two sizes as well
+    W2, L2 = wl.connectome(90, seed=3, keep=0.3)
+    cfgs = dict(axes=[dict(name="G", lo=0.0, hi=0.3, n=2, values=None)], fixed=dict(v=4.0, wNoise=1e-4), seed=2)
+    _, c = tvbx.sweep_from_config(cfgs, W2, L2, precision=tvbx.TVBX_F64)
+    _, d = tvbx.sweep_from_config(cfgs, W1[:20, :20].copy(), L1[:20, :20].copy(), precision=tvbx.TVBX_F64)
+    c.run(100, 0.1, noise_on=True, ds=10); d.run(100, 0.1, noise_on=True, ds=10); c.run(100, 0.1, noise_on=True, ds=10)
+    assert c.steps_done() == 200 and d.steps_done() == 100
+
+
+# ------------------------------------------------------------------------------------ rolling chunk pipeline under stress
+@pytest.mark.parametrize("lmin,lmax,v", [(32.0, 60.0, 10.0), (1.0, 9.0, 5.0), (3.0, 40.0, 10.0)], ids=["lag4_ch8", "ch1_lag3", "ch2"])
+def test_chunk_pipeline_results_do_not_depend_on_the_mapping(lmin, lmax, v):
+    """integrate2_kernel has no CTA barrier: warps hand chunks over through a ring of mbarriers and may run up to LAG
+    chunks apart.  If a warp ever read a ring slot before its writer had stored it (or after it was overwritten), the
+    result would depend on warp timing.  Same simulations, odd N = 37, noise on, 6,000 steps (750 ... 6,000 chunks), under
+    mappings with very different warp counts and timing -- 1, 3 and 8 simulations per CTA, one CTA or a 4-CTA cluster
+    (scalar gather: per-node arithmetic identical) -- must agree BIT FOR BIT, twice in a row, and match the oracle.
+    lag4_ch8: minimum delay 32 steps -> chunks of 8, run-ahead limit LAG = 4; ch1_lag3: minimum delay 2 -> one-step
+    chunks, LAG = 3 (ring in shared memory); ch2: chunks of 2."""
+    N = 37
+    W, _ = wl.connectome(N, seed=5, keep=0.35)
+    rng = np.random.default_rng(11)
+    Lu = rng.uniform(lmin, lmax, (N, N)); L = np.triu(Lu, 1) + np.triu(Lu, 1).T
+    cfg = dict(axes=[dict(name="G", lo=0.05, hi=0.4, n=8, values=None)], fixed=dict(v=v, b_e=20.0, wNoise=1e-4), seed=9)
+    steps = 6000
+    outs = []
+    for kw in (dict(sims_per_cta=1), dict(sims_per_cta=3), dict(sims_per_cta=8), dict(sims_per_cta=3),
+               dict(sims_per_cta=2, ctas_per_group=4)):
+        _, sw = tvbx.sweep_from_config(cfg, W, L, chunk_samples=64, **kw)
+        sw.run(steps, 0.1, noise_on=True, ds=10, discard_steps=1000)
+        assert sw.kernel_name() == "tvbx::integrate2_kernel"
+        y, ou = sw.state()
+        outs.append((y, ou, sw.fc_readout()[1]))
+    for y, ou, me in outs[1:]:
+        np.testing.assert_array_equal(y, outs[0][0]); np.testing.assert_array_equal(ou, outs[0][1])
+        np.testing.assert_array_equal(me, outs[0][2])
+    o = orc.OracleSweep(W, L, wl.grid_params(cfg), seed=cfg["seed"])
+    o.run(steps, 0.1, noise_on=True, ds=10, discard_steps=1000)
+    rfc, rme, rmi = o.fc_readout()
+    assert np.abs(outs[0][2] / rme - 1).max() < TOL_MEAN_REL
