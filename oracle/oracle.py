@@ -27,32 +27,7 @@ def build(force: bool = False) -> str:
     return _LIB
 
 
-_LIB_COUNT = os.path.join(_HERE, "liboracle_count.so")
 _dp = C.POINTER(C.c_double)
-
-
-def model_op_counts(W, L_mm, params, dt=0.1, noise_on=True, ds=10, seed=0):
-    """Floating-point operations of ONE region-step of the oracle, counted by
-    rebuilding this same source with -DORC_COUNT_OPS (a double that counts its operations) and
-    stepping simulation 0 once.  -> dict(add, mul, div, sqrt, exp, erfc, log, sincos, cmp) per
-    region-step (floats: totals of the step divided by N)."""
-    if not os.path.exists(_LIB_COUNT) or os.path.getmtime(_LIB_COUNT) < os.path.getmtime(_SRC):
-        flags = [f for f in _CXXFLAGS if f != "-fopenmp"]
-        subprocess.check_call(["g++", "-DORC_COUNT_OPS", *flags, "-o", _LIB_COUNT, _SRC])
-    Lc = C.CDLL(_LIB_COUNT)
-    Lc.orc_create.restype = C.c_void_p
-    Lc.orc_create.argtypes = [C.c_int, _dp, _dp, C.c_longlong, _dp, C.POINTER(C.c_longlong), C.c_ulonglong]
-    Lc.orc_count_step.argtypes = [C.c_void_p, C.c_double, C.c_int, C.c_int, C.POINTER(C.c_longlong)]
-    Lc.orc_destroy.argtypes = [C.c_void_p]
-    W = np.ascontiguousarray(W, dtype=np.float64); L_mm = np.ascontiguousarray(L_mm, dtype=np.float64)
-    params = np.ascontiguousarray(np.atleast_2d(params)[:1], dtype=np.float64)
-    h = Lc.orc_create(W.shape[0], _p(W), _p(L_mm), 1, _p(params), None, seed)
-    cnt = (C.c_longlong * 9)()
-    rc = Lc.orc_count_step(h, dt, int(noise_on), ds, cnt)
-    Lc.orc_destroy(h)
-    assert rc == 0
-    names = ("add", "mul", "div", "sqrt", "exp", "erfc", "log", "sincos", "cmp")
-    return {k: cnt[i] / W.shape[0] for i, k in enumerate(names)}
 
 
 _lib = None

@@ -35,48 +35,6 @@
 
 namespace {
 
-// ---- scalar type -------------------------------------------------------------
-// Default build: real = double and the helpers below are the <cmath> calls, so the arithmetic is the
-// plain IEEE sequence written in this file.  -DORC_COUNT_OPS (liboracle_count.so, used only to derive
-// the "model flops per region-step" of DESIGN.md section 7) swaps in a double that counts the
-// floating-point operations it performs; values are identical.
-#ifdef ORC_COUNT_OPS
-enum { C_ADD = 0, C_MUL, C_DIV, C_SQRT, C_EXP, C_ERFC, C_LOG, C_SINCOS, C_CMP, C_NCOUNT };
-long long g_ops[C_NCOUNT];
-struct real {
-  double x;
-  real() : x(0) {}
-  real(double v) : x(v) {}
-};
-#define ORC_BIN(op, cat)                                                                    \
-  inline real operator op(const real& a, const real& b) { ++g_ops[cat]; return real(a.x op b.x); } \
-  inline real operator op(const real& a, double b) { ++g_ops[cat]; return real(a.x op b); }        \
-  inline real operator op(double a, const real& b) { ++g_ops[cat]; return real(a op b.x); }
-ORC_BIN(+, C_ADD) ORC_BIN(-, C_ADD) ORC_BIN(*, C_MUL) ORC_BIN(/, C_DIV)
-#undef ORC_BIN
-inline real operator-(const real& a) { return real(-a.x); }            // sign flip: free (operand modifier)
-inline real& operator+=(real& a, const real& b) { ++g_ops[C_ADD]; a.x += b.x; return a; }
-inline real& operator-=(real& a, const real& b) { ++g_ops[C_ADD]; a.x -= b.x; return a; }
-inline real& operator*=(real& a, const real& b) { ++g_ops[C_MUL]; a.x *= b.x; return a; }
-inline bool operator>(const real& a, double b) { ++g_ops[C_CMP]; return a.x > b; }
-inline double val(const real& a) { return a.x; }
-inline real m_sqrt(const real& a) { ++g_ops[C_SQRT]; return real(std::sqrt(a.x)); }
-inline real m_exp(const real& a) { ++g_ops[C_EXP]; return real(std::exp(a.x)); }
-inline real m_erfc(const real& a) { ++g_ops[C_ERFC]; return real(std::erfc(a.x)); }
-inline real m_log(const real& a) { ++g_ops[C_LOG]; return real(std::log(a.x)); }
-inline real m_sin(const real& a) { ++g_ops[C_SINCOS]; return real(std::sin(a.x)); }
-inline real m_cos(const real& a) { ++g_ops[C_SINCOS]; return real(std::cos(a.x)); }
-#else
-typedef double real;
-inline double val(double a) { return a; }
-inline double m_sqrt(double a) { return std::sqrt(a); }
-inline double m_exp(double a) { return std::exp(a); }
-inline double m_erfc(double a) { return std::erfc(a); }
-inline double m_log(double a) { return std::log(a); }
-inline double m_sin(double a) { return std::sin(a); }
-inline double m_cos(double a) { return std::cos(a); }
-#endif
-
 // ---- parameter vector layout (one vector of NP doubles per simulation) ------
 enum Pid {
   P_G = 0, P_B_E, P_A_E, P_TAU_W_E, P_V, P_WNOISE, P_EL_E, P_EL_I, P_T,
@@ -95,26 +53,26 @@ enum Pid {
 
 // ---- second-order forward-mode jet in the two local rates (A8) --------------
 // v, d/de, d/di, d2/dede, d2/dedi, d2/didi
-struct Jet { real v, e, i, ee, ei, ii; };
+struct Jet { double v, e, i, ee, ei, ii; };
 
-inline Jet jconst(real c) { return {c, 0, 0, 0, 0, 0}; }
+inline Jet jconst(double c) { return {c, 0, 0, 0, 0, 0}; }
 inline Jet operator+(const Jet& a, const Jet& b) {
   return {a.v + b.v, a.e + b.e, a.i + b.i, a.ee + b.ee, a.ei + b.ei, a.ii + b.ii};
 }
 inline Jet operator-(const Jet& a, const Jet& b) {
   return {a.v - b.v, a.e - b.e, a.i - b.i, a.ee - b.ee, a.ei - b.ei, a.ii - b.ii};
 }
-inline Jet operator+(const Jet& a, real c) { Jet r = a; r.v += c; return r; }
-inline Jet operator+(real c, const Jet& a) { return a + c; }
-inline Jet operator-(const Jet& a, real c) { Jet r = a; r.v -= c; return r; }
-inline Jet operator-(real c, const Jet& a) {
+inline Jet operator+(const Jet& a, double c) { Jet r = a; r.v += c; return r; }
+inline Jet operator+(double c, const Jet& a) { return a + c; }
+inline Jet operator-(const Jet& a, double c) { Jet r = a; r.v -= c; return r; }
+inline Jet operator-(double c, const Jet& a) {
   return {c - a.v, -a.e, -a.i, -a.ee, -a.ei, -a.ii};
 }
-inline Jet operator*(const Jet& a, real c) {
+inline Jet operator*(const Jet& a, double c) {
   return {a.v * c, a.e * c, a.i * c, a.ee * c, a.ei * c, a.ii * c};
 }
-inline Jet operator*(real c, const Jet& a) { return a * c; }
-inline Jet operator/(const Jet& a, real c) {
+inline Jet operator*(double c, const Jet& a) { return a * c; }
+inline Jet operator/(const Jet& a, double c) {
   return {a.v / c, a.e / c, a.i / c, a.ee / c, a.ei / c, a.ii / c};
 }
 // product rule to second order
@@ -129,7 +87,7 @@ inline Jet operator*(const Jet& a, const Jet& b) {
   return r;
 }
 // chain rule for a scalar function g(u) with g0=g(u), g1=g'(u), g2=g''(u)
-inline Jet jchain(const Jet& u, real g0, real g1, real g2) {
+inline Jet jchain(const Jet& u, double g0, double g1, double g2) {
   Jet r;
   r.v  = g0;
   r.e  = g1 * u.e;
@@ -140,19 +98,19 @@ inline Jet jchain(const Jet& u, real g0, real g1, real g2) {
   return r;
 }
 inline Jet jrecip(const Jet& u) {
-  real r = 1.0 / u.v;
+  double r = 1.0 / u.v;
   return jchain(u, r, -r * r, 2.0 * r * r * r);
 }
 inline Jet operator/(const Jet& a, const Jet& b) { return a * jrecip(b); }
-inline Jet operator/(real c, const Jet& b) { return jrecip(b) * c; }
+inline Jet operator/(double c, const Jet& b) { return jrecip(b) * c; }
 inline Jet jsqrt(const Jet& u) {
-  real s = m_sqrt(u.v);
+  double s = std::sqrt(u.v);
   return jchain(u, s, 0.5 / s, -0.25 / (s * u.v));
 }
 inline Jet jerfc(const Jet& u) {
   const double two_over_sqrt_pi = 1.1283791670955125738961589031215;
-  real g = m_exp(-u.v * u.v);
-  return jchain(u, m_erfc(u.v), -two_over_sqrt_pi * g, 2.0 * two_over_sqrt_pi * u.v * g);
+  double g = std::exp(-u.v * u.v);
+  return jchain(u, std::erfc(u.v), -two_over_sqrt_pi * g, 2.0 * two_over_sqrt_pi * u.v * g);
 }
 
 // ---- transfer function, A1 (template of [25],[5]; P:84 names mu_V, sigma_V, ---
@@ -160,8 +118,8 @@ inline Jet jerfc(const Jet& u) {
 // pop: 0 = excitatory (RS, E_L,e, P_e), 1 = inhibitory (FS, E_L,i, P_i).
 // fe, fi are the already clamped inputs (A10) carried as jets; Wad = W_mu.
 // Returns F_mu as a jet; *muV_out receives the value of mu_V.
-Jet transfer_function(const double* p, int pop, const Jet& fe, const Jet& fi, real Wad,
-                      real* muV_out) {
+Jet transfer_function(const double* p, int pop, const Jet& fe, const Jet& fi, double Wad,
+                      double* muV_out) {
   const double gL = p[P_GL], Cm = p[P_CM];
   const double Qe = p[P_QE], Te = p[P_TAUE], Ee = p[P_EE];
   const double Qi = p[P_QI], Ti = p[P_TAUI], Ei = p[P_EI];
@@ -199,10 +157,10 @@ Jet transfer_function(const double* p, int pop, const Jet& fe, const Jet& fi, re
 }
 
 // clamped input as a jet seeded in direction `dir` (0 = e, 1 = i), A10
-inline Jet clamp_input(real x, real eps, int dir) {
+inline Jet clamp_input(double x, double eps, int dir) {
   const bool pos = x > 0.0;
-  Jet j = jconst((pos ? x : real(0.0)) + eps);
-  real seed = pos ? 1.0 : 0.0;
+  Jet j = jconst((pos ? x : double(0.0)) + eps);
+  double seed = pos ? 1.0 : 0.0;
   if (dir == 0) j.e = seed; else j.i = seed;
   return j;
 }
@@ -225,10 +183,10 @@ inline void philox4x32_10(const uint32_t ctr[4], const uint32_t key[2], uint32_t
 }
 // u(x) = ((x >> 9) + 0.5) * 2^-23: (2k+1)/2^24 with k < 2^23 is exact in FP32 and FP64 (A12 as
 // amended in DESIGN.md: 24 bits + 0.5 would need a 25-bit significand).
-inline real u23(uint32_t x) { return (real((double)(x >> 9)) + 0.5) * (1.0 / 8388608.0); }
+inline double u23(uint32_t x) { return (double((double)(x >> 9)) + 0.5) * (1.0 / 8388608.0); }
 
 // xi_{s,k,n}: counter = (q_lo, q_hi, region, sim), q = n/4; key = (seed_lo, seed_hi)
-real normal_variate(uint64_t seed, int64_t sim, int32_t region, int64_t step) {
+double normal_variate(uint64_t seed, int64_t sim, int32_t region, int64_t step) {
   uint64_t q = (uint64_t)step >> 2;
   uint32_t ctr[4] = {(uint32_t)q, (uint32_t)(q >> 32), (uint32_t)region, (uint32_t)sim};
   uint32_t key[2] = {(uint32_t)seed, (uint32_t)(seed >> 32)};
@@ -237,9 +195,9 @@ real normal_variate(uint64_t seed, int64_t sim, int32_t region, int64_t step) {
   const double two_pi = 6.2831853071795864769252867665590;
   int w = (int)(step & 3);
   uint32_t xa = w < 2 ? x[0] : x[2], xb = w < 2 ? x[1] : x[3];
-  real r = m_sqrt(-2.0 * m_log(u23(xa)));
-  real th = two_pi * u23(xb);
-  return (w & 1) ? r * m_sin(th) : r * m_cos(th);
+  double r = std::sqrt(-2.0 * std::log(u23(xa)));
+  double th = two_pi * u23(xb);
+  return (w & 1) ? r * std::sin(th) : r * std::cos(th);
 }
 
 // ---- delay index, A13: d = nearbyint((L/v)/dt), IEEE double, half-to-even ---
@@ -339,15 +297,15 @@ void step_sim(Sweep& sw, Sim& sm, int64_t n, double dt, int noise_on, int ds,
 
   for (int k = 0; k < N; ++k) {
     // 1. coupling, P:82 (ascending j, A16)
-    real c = 0.0;
-    for (const Edge& e : sm.rows[k]) c += real(e.w) * ehist(sw, sm, n - e.d, e.j);
+    double c = 0.0;
+    for (const Edge& e : sm.rows[k]) c += double(e.w) * ehist(sw, sm, n - e.d, e.j);
     // 2. inputs, Eq. (5) P:79 with A5/A6
-    const real eta = noise_on ? p[P_WNOISE] * real(sm.ou[k]) : real(0.0);
-    const real drive = E[k] + p[P_G] * c + eta;
-    Jet F[2]; real muV[2];
+    const double eta = noise_on ? p[P_WNOISE] * (sm.ou[k]) : double(0.0);
+    const double drive = E[k] + p[P_G] * c + eta;
+    Jet F[2]; double muV[2];
     for (int mu = 0; mu < 2; ++mu) {
-      const real xe = drive + (mu == 0 ? p[P_CFEE] : p[P_CFIE]);
-      const real xi = real(I[k]) + (mu == 0 ? p[P_CFEI] : p[P_CFII]);
+      const double xe = drive + (mu == 0 ? p[P_CFEE] : p[P_CFIE]);
+      const double xi = double(I[k]) + (mu == 0 ? p[P_CFEI] : p[P_CFII]);
       Jet fe = clamp_input(xe, p[P_EPS_NU], 0);
       Jet fi = clamp_input(xi, p[P_EPS_NU], 1);
       // 3.-4. transfer function and its exact derivatives (A1, A8)
@@ -361,38 +319,38 @@ void step_sim(Sweep& sw, Sim& sm, int64_t n, double dt, int noise_on, int ds,
     // unit-consistent reading, kappa = 1e-3 (default) measures the differentiated rate in Hz.
     const double kap = p[P_KAPPA];
     for (int mu = 0; mu < 2; ++mu) {
-      F[mu].e *= real(kap); F[mu].i *= real(kap);
-      F[mu].ee *= real(kap * kap); F[mu].ei *= real(kap * kap); F[mu].ii *= real(kap * kap);
+      F[mu].e *= double(kap); F[mu].i *= double(kap);
+      F[mu].ee *= double(kap * kap); F[mu].ei *= double(kap * kap); F[mu].ii *= double(kap * kap);
     }
     const Jet& Fe = F[0]; const Jet& Fi = F[1];
     // 5. Eq. (1), sums over lambda,eta written out (A7)
-    real dE = ((Fe.v - E[k]) + 0.5 * Cee[k] * Fe.ee + Cei[k] * Fe.ei + 0.5 * Cii[k] * Fe.ii) / T;
-    real dI = ((Fi.v - I[k]) + 0.5 * Cee[k] * Fi.ee + Cei[k] * Fi.ei + 0.5 * Cii[k] * Fi.ii) / T;
+    double dE = ((Fe.v - E[k]) + 0.5 * Cee[k] * Fe.ee + Cei[k] * Fe.ei + 0.5 * Cii[k] * Fe.ii) / T;
+    double dI = ((Fi.v - I[k]) + 0.5 * Cee[k] * Fi.ee + Cei[k] * Fi.ei + 0.5 * Cii[k] * Fi.ii) / T;
     // 6. Eq. (2)
-    real dCee = (Fe.v * (1.0 / T - Fe.v) / Ne + (Fe.v - E[k]) * (Fe.v - E[k]) +
+    double dCee = (Fe.v * (1.0 / T - Fe.v) / Ne + (Fe.v - E[k]) * (Fe.v - E[k]) +
                    2.0 * (Cee[k] * Fe.e + Cei[k] * Fe.i) - 2.0 * Cee[k]) / T;
-    real dCii = (Fi.v * (1.0 / T - Fi.v) / Ni + (Fi.v - I[k]) * (Fi.v - I[k]) +
+    double dCii = (Fi.v * (1.0 / T - Fi.v) / Ni + (Fi.v - I[k]) * (Fi.v - I[k]) +
                    2.0 * (Cei[k] * Fi.e + Cii[k] * Fi.i) - 2.0 * Cii[k]) / T;
-    real dCei = ((Fe.v - E[k]) * (Fi.v - I[k]) + (Cei[k] * Fe.e + Cii[k] * Fe.i) +
+    double dCei = ((Fe.v - E[k]) * (Fi.v - I[k]) + (Cei[k] * Fe.e + Cii[k] * Fe.i) +
                    (Cee[k] * Fi.e + Cei[k] * Fi.i) - 2.0 * Cei[k]) / T;
     // 7. Eq. (3), with A9 (a-term divided by tau_w)
-    real dWe = -We[k] / p[P_TAU_W_E] + p[P_B_E] * E[k] +
+    double dWe = -We[k] / p[P_TAU_W_E] + p[P_B_E] * E[k] +
                  p[P_A_E] * (muV[0] - p[P_EL_E]) / p[P_TAU_W_E];
-    real dWi = -Wi[k] / p[P_TAU_W_I] + p[P_B_I] * I[k] +
+    double dWi = -Wi[k] / p[P_TAU_W_I] + p[P_B_I] * I[k] +
                  p[P_A_I] * (muV[1] - p[P_EL_I]) / p[P_TAU_W_I];
     // 8. forward Euler
-    ynew[0 * (size_t)N + k] = val(E[k] + dt * dE);
-    ynew[1 * (size_t)N + k] = val(I[k] + dt * dI);
-    ynew[2 * (size_t)N + k] = val(Cee[k] + dt * dCee);
-    ynew[3 * (size_t)N + k] = val(Cei[k] + dt * dCei);
-    ynew[4 * (size_t)N + k] = val(Cii[k] + dt * dCii);
-    ynew[5 * (size_t)N + k] = val(We[k] + dt * dWe);
-    ynew[6 * (size_t)N + k] = val(Wi[k] + dt * dWi);
+    ynew[0 * (size_t)N + k] = (E[k] + dt * dE);
+    ynew[1 * (size_t)N + k] = (I[k] + dt * dI);
+    ynew[2 * (size_t)N + k] = (Cee[k] + dt * dCee);
+    ynew[3 * (size_t)N + k] = (Cei[k] + dt * dCei);
+    ynew[4 * (size_t)N + k] = (Cii[k] + dt * dCii);
+    ynew[5 * (size_t)N + k] = (We[k] + dt * dWe);
+    ynew[6 * (size_t)N + k] = (Wi[k] + dt * dWi);
     // 9. exact one-step OU update, Eq. (4) P:58 with A11
     if (noise_on) {
       const double rho = std::exp(-dt / p[P_TAU_OU]);
-      const real xi = normal_variate(sw.seed, sm.ext_id, k, n);
-      ounew[k] = val(p[P_MU_OU] + (real(sm.ou[k]) - p[P_MU_OU]) * rho +
+      const double xi = normal_variate(sw.seed, sm.ext_id, k, n);
+      ounew[k] = (p[P_MU_OU] + ((sm.ou[k]) - p[P_MU_OU]) * rho +
                      (p[P_SIGMA_OU] * std::sqrt(1.0 - rho * rho)) * xi);
     } else {
       ounew[k] = sm.ou[k];
@@ -411,14 +369,14 @@ void step_sim(Sweep& sw, Sim& sm, int64_t n, double dt, int noise_on, int ds,
   // 11. temporal-average downsample of the post-update values (A17)
   if (ds > 0) {
     for (int k = 0; k < N; ++k) {
-      sm.win_e[k] = val(real(sm.win_e[k]) + sm.y[k]);
-      sm.win_i[k] = val(real(sm.win_i[k]) + sm.y[(size_t)N + k]);
+      sm.win_e[k] = ((sm.win_e[k]) + sm.y[k]);
+      sm.win_i[k] = ((sm.win_i[k]) + sm.y[(size_t)N + k]);
     }
     if ((n + 1) % ds == 0) {
       if (n + 1 > discard_steps) {
         for (int k = 0; k < N; ++k) {
-          sm.xe.push_back(val(real(sm.win_e[k]) / (double)ds));
-          sm.xi.push_back(val(real(sm.win_i[k]) / (double)ds));
+          sm.xe.push_back(((sm.win_e[k]) / (double)ds));
+          sm.xi.push_back(((sm.win_i[k]) / (double)ds));
         }
       }
       for (int k = 0; k < N; ++k) { sm.win_e[k] = 0.0; sm.win_i[k] = 0.0; }
@@ -454,9 +412,9 @@ int orc_delay_index(double L_mm, double v, double dt) { return delay_index(L_mm,
 void orc_philox4x32_10(const unsigned* ctr, const unsigned* key, unsigned* out) {
   philox4x32_10(ctr, key, out);
 }
-double orc_uniform23(unsigned x) { return val(u23(x)); }
+double orc_uniform23(unsigned x) { return (u23(x)); }
 double orc_normal(unsigned long long seed, long long sim, int region, long long step) {
-  return val(normal_variate(seed, sim, region, step));
+  return (normal_variate(seed, sim, region, step));
 }
 
 // F_mu and derivatives at raw inputs (x_e, x_i) (clamp A10 applied inside), out6 =
@@ -464,11 +422,11 @@ double orc_normal(unsigned long long seed, long long sim, int region, long long 
 void orc_tf(const double* params, int pop, double x_e, double x_i, double W, double* out6,
             double* muV) {
   Jet fe = clamp_input(x_e, params[P_EPS_NU], 0), fi = clamp_input(x_i, params[P_EPS_NU], 1);
-  real mv;
+  double mv;
   Jet F = transfer_function(params, pop, fe, fi, W, &mv);
-  if (muV) *muV = val(mv);
-  out6[0] = val(F.v); out6[1] = val(F.e); out6[2] = val(F.i); out6[3] = val(F.ee); out6[4] = val(F.ei);
-  out6[5] = val(F.ii);
+  if (muV) *muV = (mv);
+  out6[0] = (F.v); out6[1] = (F.e); out6[2] = (F.i); out6[3] = (F.ee); out6[4] = (F.ei);
+  out6[5] = (F.ii);
 }
 
 void* orc_create(int N, const double* W, const double* L_mm, long long S, const double* params,
@@ -583,23 +541,6 @@ int orc_fc_readout(void* h, double* fc, double* mean_e, double* mean_i) {
   return 0;
 }
 
-// Floating-point operations one region-step performs (only in the -DORC_COUNT_OPS build; all -1
-// otherwise): counts[9] = add/sub, mul, div, sqrt, exp, erfc, log, sin/cos, compare, summed over one
-// forward-Euler step of simulation 0 and divided by N by the caller.  Run single-threaded.
-int orc_count_step(void* h, double dt, int noise_on, int ds, long long* counts) {
-#ifdef ORC_COUNT_OPS
-  Sweep* sw = (Sweep*)h;
-  if (!sw->started) start(*sw, dt);
-  for (int i = 0; i < C_NCOUNT; ++i) g_ops[i] = 0;
-  step_sim(*sw, sw->sims[0], sw->n, dt, noise_on, ds, 0, nullptr);
-  for (int i = 0; i < C_NCOUNT; ++i) counts[i] = g_ops[i];
-  return 0;
-#else
-  (void)h; (void)dt; (void)noise_on; (void)ds;
-  for (int i = 0; i < 9; ++i) counts[i] = -1;
-  return -1;
-#endif
-}
 
 int orc_max_threads() {
 #ifdef _OPENMP

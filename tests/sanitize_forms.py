@@ -1,11 +1,14 @@
-"""Driver for compute-sanitizer (memcheck / racecheck / synccheck / initcheck) over every kernel form of the library on
-cfg-1-sized sweeps ("Race detection": the ring write-after-read hazard is the one real race; the
-product kernel replaces CTA barriers by a rolling mbarrier pipeline).  Not a pytest file: run as
+"""Every kernel form of the library on cfg-1-sized sweeps, two launches each (resume path), all outputs read back and
+checked finite.  Written as the driver for compute-sanitizer ("Race detection"):
 
-    compute-sanitizer --tool racecheck python tests/sanitize_forms.py
+    compute-sanitizer --tool memcheck python tests/sanitize_forms.py
 
-Uses host (numpy) buffers only, so torch is never imported under the sanitizer.  Prints one line per form; exits
-non-zero on the first library error.  The summaries of the four tools are kept under profiles/."""
+compute-sanitizer is CLOSED on this GPU pool ("runs under it have left GPUs needing a reset" -- gpurun refuses it), so
+the run is recorded as unavailable in profiles/r2_sanitizer.md and the hazards it would look for are covered by tests
+instead: tests/test_gpu_parity_r2.py::test_chunk_pipeline_results_do_not_depend_on_the_mapping (ring read-before-write
+or overwrite-before-read would make results depend on warp timing) and the bit-exact resume / reset / pool tests.
+Run plainly (`python tests/sanitize_forms.py`) it is a smoke run of all forms.  Host (numpy) buffers only: torch is
+never imported.  Prints one line per form; exits non-zero on the first library error."""
 import os
 import sys
 

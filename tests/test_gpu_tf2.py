@@ -7,10 +7,12 @@ configs actually visit.
 Why this test exists: in Eq. (1) the second derivatives enter as (1/2) C d2F kappa^2, 1e-7 of nu at the default
 kappa = 1e-3 -- no FP32 trajectory tolerance can see an error there.  Here each component is checked on its own.
 
-Tolerances (FP32 path, SFU rcp/sqrt/ex2 approximations, erfc fit 4.7e-7):
-  value, mu_V : 2e-5 relative
-  first       : 1e-4 relative
-  second      : 1e-3 relative
+Tolerances (FP32 path, SFU rcp/sqrt/ex2 approximations of <= 2 ulp, erfc fit 4.7e-7; on the tail of erfc a relative
+error d of its argument z becomes 2 z^2 d in F -- x 50 at z = 5 --, so the value cannot be held to FP32 epsilon):
+  mu_V        : 2e-5 relative
+  value       : 1e-4 relative     (measured on the B200: 4.9e-5)
+  first       : 2e-4 relative     (measured: 1.1e-4)
+  second      : 1e-3 relative     (measured: 1.2e-4)
 "relative" = |got - ref| / max(|ref|, floor_q) with floor_q = 1e-3 x the largest |ref| of that component over the same
 (population, W) slice: derivatives cross zero inside the grid, and an FP32 result cannot be relatively accurate at a zero
 crossing of a sum of O(max) terms."""
@@ -27,7 +29,7 @@ pytestmark = pytest.mark.gpu
 
 GRID_F = [1e-6, 2e-4, 1e-3, 5e-3, 2e-2, 8e-2, 0.2]       # tests/test_oracle_tf.py
 GRID_W = [0.0, 50.0, 200.0]
-TOL = np.array([2e-5, 1e-4, 1e-4, 1e-3, 1e-3, 1e-3])
+TOL = np.array([1e-4, 2e-4, 2e-4, 1e-3, 1e-3, 1e-3])
 NAMES = ("F", "F_e", "F_i", "F_ee", "F_ei", "F_ii")
 
 

@@ -54,6 +54,29 @@ def test_philox_matches_independent_implementation():
             assert orc.philox4x32_10(c, key) == tuple(int(x) for x in r)
 
 
+def _philox4x32_10_ints(ctr, key):
+    """Philox4x32-10 (Salmon et al., "Parallel random numbers: as easy as 1, 2, 3", SC'11) restated with Python integers:
+    10 rounds of two 32 x 32 -> 64-bit multiplications by the round constants, key bumped by the Weyl constants."""
+    M0, M1, W0, W1, MASK = 0xD2511F53, 0xCD9E8D57, 0x9E3779B9, 0xBB67AE85, 0xFFFFFFFF
+    c0, c1, c2, c3 = ctr
+    k0, k1 = key
+    for _ in range(10):
+        p0, p1 = M0 * c0, M1 * c2
+        c0, c1, c2, c3 = ((p1 >> 32) ^ c1 ^ k0) & MASK, p1 & MASK, ((p0 >> 32) ^ c3 ^ k1) & MASK, p0 & MASK
+        k0, k1 = (k0 + W0) & MASK, (k1 + W1) & MASK
+    return (c0, c1, c2, c3)
+
+
+def test_philox_matches_integer_restatement():
+    """Second leg of the Philox pin, which cannot skip (the Triton-interpreter leg above depends on an optional
+    package): arbitrary-precision integer arithmetic, no uint32 wrap-around semantics shared with the C++ code."""
+    rng = np.random.default_rng(11)
+    ctrs = [[0, 0, 0, 0], [0xFFFFFFFF] * 4, [1, 2, 3, 4]] + rng.integers(0, 2**32, size=(40, 4)).tolist()
+    for key in ([0, 0], [0xFFFFFFFF, 0xFFFFFFFF], [0xDEADBEEF, 0x12345678], [2, 0]):
+        for c in ctrs:
+            assert orc.philox4x32_10(c, key) == _philox4x32_10_ints([int(x) for x in c], key)
+
+
 def test_philox_is_a_bijection_on_a_sample_and_key_sensitive():
     outs = {orc.philox4x32_10([i, 0, 0, 0], [1, 0]) for i in range(2000)}
     assert len(outs) == 2000
