@@ -103,13 +103,17 @@ class Probes:
 
     KINDS = ("ffma2_3reg", "ffma2_bcast", "fmul2", "fadd2", "ffma", "mufu_rcp")
 
-    def __init__(self):
-        import ctypes as C
+    @staticmethod
+    def build():
         src, so = os.path.join(ROOT, "bench_probes.cu"), os.path.join(ROOT, "bench_probes.so")
         if not os.path.exists(so) or os.path.getmtime(so) < os.path.getmtime(src):
             subprocess.check_call(["nvcc", "-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-shared",
                                    "-Xcompiler", "-fPIC", "-o", so, src])
-        self.C, self.L = C, C.CDLL(so)
+        return so
+
+    def __init__(self):
+        import ctypes as C
+        self.C, self.L = C, C.CDLL(self.build())
         self.L.probe_read_bandwidth.argtypes = [C.c_longlong, C.c_int, C.POINTER(C.c_double)]
         self.L.probe_alu.argtypes = [C.c_int, C.c_int, C.POINTER(C.c_double)]
 

@@ -112,6 +112,9 @@ typedef struct tvbx_sweep_opts {
                              warp shuffles, so a sweep too small to fill the GPU with nodes runs twice the warps on a
                              shorter per-step dependency chain.  Packed FP32 kernel, one CTA per group only */
   int32_t reserved0;
+  double updown_threshold_khz; /* > 0: also keep the up / down-state episode statistics of the kept 1-ms excitatory samples
+                                  (tvbx_state_durations; Tab. 2 P:131 `mean_UD_duration`): a sample is UP iff it exceeds
+                                  this rate.  0 = off (the paper prints no threshold: DESIGN.md A25) */
 } tvbx_sweep_opts;
 
 enum tvbx_fc_mode { TVBX_FC_AUTO = 0, TVBX_FC_FP32 = 1, TVBX_FC_TF32 = 2 };
@@ -195,6 +198,22 @@ int32_t tvbx_fc_scores(tvbx_sweep* sw, const double* ref_fc, float* fcsc, float*
  * without rate_stats_inhibitory. */
 int32_t tvbx_rate_stats(tvbx_sweep* sw, float* var_e, float* max_e, int32_t* n_above_e, float* var_i, float* max_i,
                         int32_t* n_above_i, int32_t on_device, void* stream);
+
+/* Up / down-state durations per (simulation, region) (Tab. 2 P:131 `mean_UD_duration` "Mean duration of UP and
+ * DOWN states"; A25), over the kept 1-ms excitatory samples: a sample is UP iff it exceeds
+ * tvbx_sweep_opts.updown_threshold_khz; an episode is a maximal run of equal states; episodes cut by the start of the
+ * record or still open now are not counted.  n_up / n_down = number of episodes, mean_*_ms = their mean duration in ms
+ * (0 where there is none).  Outputs n_sims x N, host or device (on_device), any may be NULL; the open chunk is included,
+ * the accumulators stay untouched.  TVBX_ESTATE if the sweep was created without a threshold or before the first run. */
+int32_t tvbx_state_durations(tvbx_sweep* sw, int32_t* n_up, float* mean_up_ms, int32_t* n_down, float* mean_down_ms,
+                             int32_t on_device, void* stream);
+
+/* The k best simulations by an FC score (the grid search "output[s] the best ten fittest simulations";
+ * scores as in tvbx_fc_scores, Eq. (6)): which = 0 fcsc, 1 fitness (needs ref_fc), 2 mean_fc.  sim_ids[i] = external
+ * (grid) index of the i-th best simulation of this sweep object, scores[i] its score, best first, equal scores in ascending
+ * local order (A23); both HOST arrays of k entries; *n_out = min(k, n_sims).  1 <= k <= 1024. */
+int32_t tvbx_top_k(tvbx_sweep* sw, int32_t which, const double* ref_fc, int32_t k, int64_t* sim_ids, float* scores,
+                   int32_t* n_out, void* stream);
 
 /* Back to step 0 without re-allocating: state, OU, history ring, window sums and FC accumulators are
  * re-initialised on the device (enqueued on cuda_stream), the step and sample counters are zeroed.

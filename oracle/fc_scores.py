@@ -54,3 +54,20 @@ def fc_scores(fc, sc, ref=None):
     if ref is not None:
         out["fitness"] = [pearson_upper(f, ref) for f in fc]
     return out
+
+
+def top_k(scores, k):
+    """The k fittest simulations (the grid search "output[s] the best ten fittest simulations"): indices of
+    the k largest scores, best first; equal scores in ascending index (reading A23b: the paper does not say how ties are
+    broken).  Selection by repeated maximum, written out.  -> (indices, values)"""
+    s = [float(x) for x in scores]
+    taken = [False] * len(s)
+    idx, val = [], []
+    for _ in range(min(k, len(s))):
+        best = -1
+        for i in range(len(s)):
+            if not taken[i] and (best < 0 or s[i] > s[best]):
+                best = i
+        taken[best] = True
+        idx.append(best); val.append(s[best])
+    return idx, val

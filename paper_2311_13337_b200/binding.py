@@ -53,7 +53,7 @@ class SweepOpts(C.Structure):
                 ("sim_ids", C.POINTER(C.c_int64)), ("chunk_samples", C.c_int64),
                 ("threads_per_cta", C.c_int32), ("ctas_per_group", C.c_int32),
                 ("fc_mode", C.c_int32), ("rate_stats_inhibitory", C.c_int32), ("rate_threshold_khz", C.c_double),
-                ("lanes_per_node", C.c_int32), ("reserved0", C.c_int32)]
+                ("lanes_per_node", C.c_int32), ("reserved0", C.c_int32), ("updown_threshold_khz", C.c_double)]
 
 
 class RunOpts(C.Structure):
@@ -64,7 +64,8 @@ class RunOpts(C.Structure):
 
 EXPORTS = [
     "tvbx_default_params", "tvbx_create_connectome", "tvbx_destroy_connectome", "tvbx_sweep_create",
-    "tvbx_sweep_destroy", "tvbx_sweep_set_initial", "tvbx_run", "tvbx_fc_readout", "tvbx_fc_scores", "tvbx_rate_stats", "tvbx_sweep_size",
+    "tvbx_sweep_destroy", "tvbx_sweep_set_initial", "tvbx_run", "tvbx_fc_readout", "tvbx_fc_scores", "tvbx_rate_stats",
+    "tvbx_state_durations", "tvbx_top_k", "tvbx_sweep_size",
     "tvbx_sweep_param", "tvbx_sweep_ext_id", "tvbx_delay_index", "tvbx_ring_len", "tvbx_steps_done",
     "tvbx_samples_kept", "tvbx_sweep_state", "tvbx_launch_info", "tvbx_launch_count", "tvbx_kernel_name", "tvbx_fc_kernel_name", "tvbx_last_error",
     "tvbx_version", "tvbx_trim_memory", "tvbx_sweep_reset", "tvbx_profile_enable", "tvbx_profile_read", "tvbx_bytes_copied", "tvbx_diag_tf_closed2",
@@ -132,6 +133,8 @@ def lib():
             "tvbx_fc_readout": [vp, vp, vp, vp, i32, vp],
             "tvbx_fc_scores": [vp, vp, vp, vp, vp, i32, vp],
             "tvbx_rate_stats": [vp, vp, vp, vp, vp, vp, vp, i32, vp],
+            "tvbx_state_durations": [vp, vp, vp, vp, vp, i32, vp],
+            "tvbx_top_k": [vp, i32, vp, i32, C.POINTER(i64), fp, C.POINTER(i32), vp],
             "tvbx_sweep_size": [vp, C.POINTER(i64), C.POINTER(i64), C.POINTER(i32)],
             "tvbx_sweep_param": [vp, i64, i32, dp],
             "tvbx_sweep_ext_id": [vp, i64, C.POINTER(i64)],
@@ -204,7 +207,7 @@ class Sweep:
 
     def __init__(self, conn: Connectome, axes, seed=0, params=None, precision=TVBX_F32, sims_per_cta=0,
                  sim_ids=None, chunk_samples=0, threads_per_cta=0, init=None, ctas_per_group=0, fc_mode=0, rate_threshold_khz=0.0,
-                 rate_stats_inhibitory=False, lanes_per_node=0):
+                 rate_stats_inhibitory=False, lanes_per_node=0, updown_threshold_khz=0.0):
         L = lib()
         self.conn = conn
         m = ModelParams()
@@ -235,6 +238,7 @@ class Sweep:
         o = SweepOpts()
         o.precision = precision; o.sims_per_cta = sims_per_cta; o.chunk_samples = chunk_samples
         o.threads_per_cta = threads_per_cta; o.ctas_per_group = ctas_per_group; o.fc_mode = fc_mode; o.rate_threshold_khz = rate_threshold_khz; o.rate_stats_inhibitory = int(bool(rate_stats_inhibitory)); o.lanes_per_node = int(lanes_per_node)
+        o.updown_threshold_khz = float(updown_threshold_khz)
         self.rate_stats_inhibitory = bool(rate_stats_inhibitory)
         if sim_ids is not None:
             ids = np.ascontiguousarray(sim_ids, dtype=np.int64)
@@ -399,6 +403,27 @@ class Sweep:
         ptr += [None] * (6 - len(ptr))
         _chk(lib().tvbx_rate_stats(self._h, *ptr, 1 if device else 0, _stream_ptr(stream)))
         return tuple(out)
+
+    def state_durations(self, device=False, stream=None):
+        """tvbx_state_durations -> (n_up int32, mean_up_ms float32, n_down int32, mean_down_ms float32), each [S][N]."""
+        S, N = self.n_sims, self.n_regions
+        if device:
+            import torch
+            out = [torch.empty((S, N), device="cuda", dtype=d) for d in (torch.int32, torch.float32, torch.int32, torch.float32)]
+            ptr = [t.data_ptr() for t in out]
+        else:
+            out = [np.empty((S, N), d) for d in (np.int32, np.float32, np.int32, np.float32)]
+            ptr = [a.ctypes.data for a in out]
+        _chk(lib().tvbx_state_durations(self._h, *ptr, 1 if device else 0, _stream_ptr(stream)))
+        return tuple(out)
+
+    def top_k(self, k, which="fcsc", ref_fc=None, stream=None):
+        """tvbx_top_k -> (external sim ids int64 [n], scores float32 [n]), best first; which in fcsc / fitness / mean_fc."""
+        ref = None if ref_fc is None else np.ascontiguousarray(ref_fc, dtype=np.float64)
+        ids = np.zeros(k, np.int64); sc = np.zeros(k, np.float32); n = C.c_int32()
+        _chk(lib().tvbx_top_k(self._h, {"fcsc": 0, "fitness": 1, "mean_fc": 2}[which], None if ref is None else ref.ctypes.data, int(k),
+                              ids.ctypes.data_as(C.POINTER(C.c_int64)), sc.ctypes.data_as(C.POINTER(C.c_float)), C.byref(n), _stream_ptr(stream)))
+        return ids[:n.value], sc[:n.value]
 
     def kernel_name(self):
         buf = C.create_string_buffer(64)

@@ -201,6 +201,10 @@ int32_t tvbx_sweep_create(const tvbx_connectome* c, const tvbx_model_params* def
   sw->chunk_req = opts ? opts->chunk_samples : 0;
   {
     sw->stats_i = opts && opts->rate_stats_inhibitory != 0;
+    if (opts && opts->updown_threshold_khz != 0.0) {
+      if (!(opts->updown_threshold_khz > 0.0) || !std::isfinite(opts->updown_threshold_khz)) return fail(TVBX_EINVAL, "updown_threshold_khz=%g", opts->updown_threshold_khz);
+      sw->ud_thr = opts->updown_threshold_khz;
+    }
     if (opts && opts->rate_threshold_khz != 0.0) {
       if (!(opts->rate_threshold_khz > 0.0)) return fail(TVBX_EINVAL, "rate_threshold_khz=%g", opts->rate_threshold_khz);
       sw->rate_thr = opts->rate_threshold_khz;
@@ -372,6 +376,26 @@ int32_t tvbx_rate_stats(tvbx_sweep* sw, float* var_e, float* max_e, int32_t* n_a
   if (!sw->started) return fail(TVBX_ESTATE, "no run yet");
   DeviceGuard guard(sw->device);
   return sw->dev->rate_stats(var_e, max_e, n_above_e, var_i, max_i, n_above_i, on_device, (cudaStream_t)stream);
+}
+int32_t tvbx_state_durations(tvbx_sweep* sw, int32_t* n_up, float* mean_up_ms, int32_t* n_down, float* mean_down_ms,
+                             int32_t on_device, void* stream) {
+  if (!sw) return fail(TVBX_EINVAL, "sweep is NULL");
+  if (!(sw->ud_thr > 0.0)) return fail(TVBX_ESTATE, "the sweep was created without tvbx_sweep_opts.updown_threshold_khz");
+  if (!sw->started) return fail(TVBX_ESTATE, "no run yet");
+  DeviceGuard guard(sw->device);
+  return sw->dev->state_durations(n_up, mean_up_ms, n_down, mean_down_ms, on_device, (cudaStream_t)stream);
+}
+int32_t tvbx_top_k(tvbx_sweep* sw, int32_t which, const double* ref_fc, int32_t k, int64_t* sim_ids, float* scores,
+                   int32_t* n_out, void* stream) {
+  if (!sw || !sim_ids || !scores) return fail(TVBX_EINVAL, "NULL argument");
+  if (which < 0 || which > 2 || k < 1 || k > 1024) return fail(TVBX_EINVAL, "which in 0..2, k in 1..1024");
+  if (which == 1 && !ref_fc) return fail(TVBX_EINVAL, "fitness needs a reference FC");
+  if (!sw->started) return fail(TVBX_ESTATE, "no run yet");
+  if (ref_fc)
+    for (size_t i = 0; i < (size_t)sw->conn.n * sw->conn.n; ++i)
+      if (!std::isfinite(ref_fc[i])) return fail(TVBX_EINVAL, "reference FC entry %zu is not finite", i);
+  DeviceGuard guard(sw->device);
+  return sw->dev->top_k(which, ref_fc, k, sim_ids, scores, n_out, (cudaStream_t)stream);
 }
 int32_t tvbx_fc_readout(tvbx_sweep* sw, float* fc, float* mean_e, float* mean_i, int32_t on_device, void* stream) {
   if (!sw) return fail(TVBX_EINVAL, "sweep is NULL");

@@ -54,6 +54,7 @@ struct DeviceImpl : DeviceSide {
   DevBuf<float> d_imax, d_imax_scratch;
   DevBuf<int32_t> d_icnt, d_icnt_scratch;
   DevBuf<float> d_out_fc, d_out_me, d_out_mi;
+  DevBuf<int32_t> d_ud, d_ud_scratch;                // f4: up / down-state episode state per column (UD_NSTATE planes)
   IntegrateParams<R> P;
   KernelPick<R> kp{nullptr};
   // packed FP32 product kernel (sw->packed)
@@ -61,6 +62,7 @@ struct DeviceImpl : DeviceSide {
   std::vector<Launch2> launches2;
   DevBuf<float2> d_psim2;
   int threads = 0, smem = 0;
+  int run_ds = 1;      // temporal-average window of the runs so far (sample spacing of the 1-ms series = run_ds * dt)
   bool single = true;
   size_t ring_count = 0, max_slice_edges = 0;
 
@@ -229,6 +231,7 @@ struct DeviceImpl : DeviceSide {
       CU(cudaMemset(d_xbar_i.p, 0, d_xbar_i.n * sizeof(R)));
       CU(d_imean.alloc((size_t)G * row)); CU(d_im2.alloc((size_t)G * row)); CU(d_imax.alloc((size_t)G * row)); CU(d_icnt.alloc((size_t)G * row));
     }
+    if (sw->ud_thr > 0.0) CU(d_ud.alloc((size_t)UD_NSTATE * G * row));
     if (sw->fc_tc) CU(d_xc.alloc((size_t)G * Kp * row));
     CU(d_cmean.alloc((size_t)G * row)); CU(d_mean.alloc((size_t)G * row));
     CU(d_cmax.alloc((size_t)G * row)); CU(d_rmax.alloc((size_t)G * row)); CU(d_ccnt.alloc((size_t)G * row)); CU(d_rcnt.alloc((size_t)G * row));
@@ -296,8 +299,8 @@ struct DeviceImpl : DeviceSide {
     single = true;
     const size_t base = (size_t)NBAR * 8 + (size_t)2 * GC * threads * sizeof(float) + (size_t)NP2 * SPC * sizeof(float2) + 16;
     // cluster form: the vector-gather kernels stage the rows of the CTA's regions as 8-byte entries; the scalar
-    // cluster kernels read the table through L1/L2
-    const size_t slice_bytes = max_slice_edges * sizeof(Edge8);
+    // cluster kernels read the table through L1/L2, except the small-CTA instance (16-byte entries in shared memory)
+    const size_t slice_bytes = max_slice_edges * (sw->vec_ok ? sizeof(Edge8) : sizeof(Edge<float>));
     // (at most ~half of the SM's 256 KB: the L1 is the landing space of the ring loads in flight -- 15 warps x 15
     // LDG.128 = 115 KB; measured at N = 360: 212 KB of shared memory halves the throughput)
     bool clu_tab = CLU > 1 && base + slice_bytes <= (size_t)136 * 1024;
@@ -315,12 +318,13 @@ struct DeviceImpl : DeviceSide {
       const int gce = !P2.smem_table ? 8 : (ch <= 2 ? 2 : (ch <= 4 ? 4 : 8));
       // short delays: the group's ring ([N][Hp + GC - 1][SPC] floats) in shared memory next to the table
       const size_t ring_b = (size_t)N * (ht.Hp + GC - 1) * SPC * sizeof(float) + 16;
-      const bool sring = CLU == 1 && P2.smem_table && gce < 8 && smem + ring_b <= (size_t)200 * 1024 &&
-                         getenv("TVBX_NO_SRING") == nullptr;
+      // (and, for CTAs small enough for the relaxed register bound, whenever it fits: cfg 1)
+      const bool sring = CLU == 1 && P2.smem_table && (gce < 8 || (threads <= K2_SMALLT && !sw->stats_i)) &&
+                         smem + ring_b <= (size_t)200 * 1024 && getenv("TVBX_NO_SRING") == nullptr;
       const int lsmem = smem + (sring ? (int)ring_b : 0);
       Kernel2Key key;
       key.spc = SPC; key.smemtab = P2.smem_table != 0; key.gce = gce; key.clu = CLU > 1; key.vec = ht.vec != 0; key.sring = sring;
-      key.small = !key.clu && !key.vec && !sring && key.smemtab && gce == 8 && threads <= K2_SMALLT;
+      key.small = !key.vec && !sring && key.smemtab && gce == 8 && threads <= K2_SMALLT;
       key.isamp = sw->stats_i;
       Kernel2Fn fn = pick_kernel2(key);
       CU(raise_dynamic_smem((const void*)fn, lsmem));      // (per function, process-wide, raise-only)
@@ -349,6 +353,12 @@ struct DeviceImpl : DeviceSide {
     fill_kernel<double><<<592, 256, 0, st>>>(d_sums.p, d_sums.n, 0.0);
     fill_kernel<double><<<592, 256, 0, st>>>(d_mean.p, d_mean.n, 0.0);
     fill_kernel<double><<<1184, 256, 0, st>>>(d_M.p, d_M.n, 0.0);
+    if (sw->ud_thr > 0.0) {      // no state yet (-1) in plane 0, zeros elsewhere
+      const size_t plane = d_ud.n / UD_NSTATE;
+      fill_kernel<int32_t><<<592, 256, 0, st>>>(d_ud.p, plane, -1);
+      fill_kernel<int32_t><<<592, 256, 0, st>>>(d_ud.p + plane, d_ud.n - plane, 0);
+      sw->launches += 2;
+    }
     sw->prof_end(st);
     sw->launches += 5;
     CU(cudaGetLastError());
@@ -396,6 +406,10 @@ struct DeviceImpl : DeviceSide {
       fc_comoment_kernel<R><<<g2, 64, 0, st>>>(F);
     }
     fc_mean_update_kernel<R><<<g1, 128, 0, st>>>(F);
+    if (sw->ud_thr > 0.0 && !scratch_i) {      // (readout merges the open chunk into its own scratch copy: state_durations)
+      int32_t rc = updown_chunk(d_ud.p, n_c, st);
+      if (rc) return rc;
+    }
     if (sw->stats_i) {
       RateIParams<R> I;
       I.xbar_i = d_xbar_i.p;
@@ -424,6 +438,7 @@ struct DeviceImpl : DeviceSide {
       else { CU(tmp_traj.alloc(traj_elems)); traj = tmp_traj.p; }
     }
     P.noise_on = o->noise_on != 0; P.ds = o->ds; P.discard_steps = o->discard_steps;
+    if (o->ds > 0) run_ds = o->ds;
     P.traj = traj; P.traj_steps = o->traj_steps; P.traj_n0 = sw->n;
     if (tsteps > 0) P.traj_steps = tsteps;
     int64_t remaining = steps;
@@ -623,6 +638,85 @@ struct DeviceImpl : DeviceSide {
       if (mi) { CU(cudaMemcpyAsync(mi, dmi.p, dmi.n * sizeof(float), cudaMemcpyDeviceToHost, st)); sw->d2h += (int64_t)(dmi.n * sizeof(float)); }
       CU(cudaStreamSynchronize(st));
     }
+    return TVBX_OK;
+  }
+
+  int32_t updown_chunk(int32_t* stbuf, int n_c, cudaStream_t st) {
+    const int N = sw->conn.n, SPC = sw->spc, G = (int)sw->groups.size();
+    UpDownParams<R> U;
+    U.xbar = d_xbar.p; U.st = stbuf; U.n_c = n_c; U.CS = (int32_t)sw->CS; U.N = N; U.SPC = SPC; U.G = G; U.thr = (float)sw->ud_thr;
+    updown_chunk_kernel<R><<<dim3(G, (N * SPC + 127) / 128), 128, 0, st>>>(U);
+    sw->launches += 1;
+    CU(cudaGetLastError());
+    return TVBX_OK;
+  }
+
+  // f4: up / down-state episode counts and mean durations per (simulation, region)
+  DevBuf<int32_t> d_out_nup, d_out_ndn;
+  DevBuf<float> d_out_mup, d_out_mdn;
+  int32_t state_durations(int32_t* n_up, float* mean_up_ms, int32_t* n_down, float* mean_down_ms, int on_device, cudaStream_t st) override {
+    const int N = sw->conn.n, SPC = sw->spc, G = (int)sw->groups.size();
+    if (sw->cnt + sw->fill < 1) return fail(TVBX_ESTATE, "no sample kept yet");
+    const int32_t* src = d_ud.p;
+    if (sw->fill > 0) {      // the open chunk goes into a scratch copy of the state
+      if (d_ud_scratch.n != d_ud.n) CU(d_ud_scratch.alloc(d_ud.n));
+      CU(cudaMemcpyAsync(d_ud_scratch.p, d_ud.p, d_ud.n * sizeof(int32_t), cudaMemcpyDeviceToDevice, st));
+      sw->prof_begin(K_FC, st);
+      int32_t rc = updown_chunk(d_ud_scratch.p, (int)sw->fill, st);
+      sw->prof_end(st);
+      if (rc) return rc;
+      src = d_ud_scratch.p;
+    }
+    UpDownReadParams Q;
+    Q.st = src; Q.loc_id = d_loc.p; Q.n_up = n_up; Q.mean_up_ms = mean_up_ms; Q.n_down = n_down; Q.mean_down_ms = mean_down_ms;
+    Q.sample_ms = (float)((double)run_ds * sw->dt); Q.N = N; Q.SPC = SPC; Q.G = G;
+    const size_t n_out = (size_t)sw->n_sims * N;
+    if (!on_device) {
+      if (n_up) { if (d_out_nup.n != n_out) CU(d_out_nup.alloc(n_out)); Q.n_up = d_out_nup.p; }
+      if (n_down) { if (d_out_ndn.n != n_out) CU(d_out_ndn.alloc(n_out)); Q.n_down = d_out_ndn.p; }
+      if (mean_up_ms) { if (d_out_mup.n != n_out) CU(d_out_mup.alloc(n_out)); Q.mean_up_ms = d_out_mup.p; }
+      if (mean_down_ms) { if (d_out_mdn.n != n_out) CU(d_out_mdn.alloc(n_out)); Q.mean_down_ms = d_out_mdn.p; }
+    }
+    sw->prof_begin(K_READOUT, st);
+    updown_read_kernel<<<dim3(G * SPC, (N + 127) / 128), 128, 0, st>>>(Q);
+    sw->prof_end(st);
+    sw->launches += 1;
+    CU(cudaGetLastError());
+    if (!on_device) {
+      if (n_up) { CU(cudaMemcpyAsync(n_up, Q.n_up, n_out * sizeof(int32_t), cudaMemcpyDeviceToHost, st)); sw->d2h += (int64_t)(n_out * 4); }
+      if (n_down) { CU(cudaMemcpyAsync(n_down, Q.n_down, n_out * sizeof(int32_t), cudaMemcpyDeviceToHost, st)); sw->d2h += (int64_t)(n_out * 4); }
+      if (mean_up_ms) { CU(cudaMemcpyAsync(mean_up_ms, Q.mean_up_ms, n_out * sizeof(float), cudaMemcpyDeviceToHost, st)); sw->d2h += (int64_t)(n_out * 4); }
+      if (mean_down_ms) { CU(cudaMemcpyAsync(mean_down_ms, Q.mean_down_ms, n_out * sizeof(float), cudaMemcpyDeviceToHost, st)); sw->d2h += (int64_t)(n_out * 4); }
+      CU(cudaStreamSynchronize(st));
+    }
+    return TVBX_OK;
+  }
+
+  // f3: the k best simulations by one of the FC scores
+  DevBuf<float> d_topk_score[3], d_topk_val;
+  DevBuf<int32_t> d_topk_idx;
+  DevBuf<unsigned char> d_topk_taken;
+  int32_t top_k(int which, const double* ref, int k, int64_t* sim_ids, float* scores_out, int32_t* n_out, cudaStream_t st) override {
+    const size_t S = (size_t)sw->n_sims;
+    for (int i = 0; i < 3; ++i) if (d_topk_score[i].n != S) CU(d_topk_score[i].alloc(S));
+    int32_t rc = scores(ref, d_topk_score[0].p, ref ? d_topk_score[1].p : nullptr, d_topk_score[2].p, 1, st);
+    if (rc) return rc;
+    if (d_topk_taken.n != S) CU(d_topk_taken.alloc(S));
+    if (d_topk_idx.n != 1024) { CU(d_topk_idx.alloc(1024)); CU(d_topk_val.alloc(1024)); }
+    CU(cudaMemsetAsync(d_topk_taken.p, 0, S, st));
+    sw->prof_begin(K_READOUT, st);
+    topk_kernel<<<1, 1024, 0, st>>>(d_topk_score[which].p, d_topk_taken.p, (int)S, k, d_topk_idx.p, d_topk_val.p);
+    sw->prof_end(st);
+    sw->launches += 1;
+    CU(cudaGetLastError());
+    const int n = (int)std::min<size_t>((size_t)k, S);
+    std::vector<int32_t> idx(n);
+    CU(cudaMemcpyAsync(idx.data(), d_topk_idx.p, (size_t)n * sizeof(int32_t), cudaMemcpyDeviceToHost, st));
+    CU(cudaMemcpyAsync(scores_out, d_topk_val.p, (size_t)n * sizeof(float), cudaMemcpyDeviceToHost, st));
+    CU(cudaStreamSynchronize(st));
+    sw->d2h += (int64_t)n * 8;
+    for (int i = 0; i < n; ++i) sim_ids[i] = sw->ext_ids[idx[i]];
+    if (n_out) *n_out = n;
     return TVBX_OK;
   }
 

@@ -375,4 +375,94 @@ __global__ void __launch_bounds__(256) fc_scores_kernel(ScoreParams P) {
   }
 }
 
+
+// ---- up / down-state durations (f4; Tab. 2 P:131 `mean_UD_duration`; A25) ----
+// Per (group, region, lane) column the kept excitatory 1-ms samples are binarised (UP iff x > thr) and scanned in
+// time order; an episode = a maximal run of equal states, counted when it ENDS and only if it did not start at the
+// first kept sample (episodes cut by either end of the record have no known duration; the run still open at
+// readout is simply never counted).  State per column, 6 ints: [0] prev state (-1 none yet, 0 down, 1 up),
+// [1] length of the current run, [2] 1 while the current run is the record's first, [3] UP episodes,
+// [4] samples in UP episodes, [5] DOWN episodes, [6] samples in DOWN episodes.
+enum { UD_NSTATE = 7 };
+template <typename R>
+struct UpDownParams {
+  const R* xbar;        // [G][CS][N][SPC]
+  int32_t* st;          // [UD_NSTATE][G][N][SPC]
+  int32_t n_c, CS, N, SPC, G;
+  float thr;            // kHz
+};
+// one thread per column, the chunk's samples in order (coalesced across columns)
+template <typename R>
+__global__ void __launch_bounds__(128) updown_chunk_kernel(UpDownParams<R> P) {
+  const int g = blockIdx.x;
+  const int idx = blockIdx.y * blockDim.x + threadIdx.x;
+  const int row = P.N * P.SPC;
+  if (idx >= row) return;
+  const size_t plane = (size_t)P.G * row, o = (size_t)g * row + idx;
+  int prev = P.st[o], run = P.st[plane + o], first = P.st[2 * plane + o];
+  int cnt[2] = {P.st[5 * plane + o], P.st[3 * plane + o]}, tot[2] = {P.st[6 * plane + o], P.st[4 * plane + o]};
+  const R* x = P.xbar + (size_t)g * P.CS * row + idx;
+  for (int q = 0; q < P.n_c; ++q) {
+    const int s = (float)x[(size_t)q * row] > P.thr ? 1 : 0;
+    if (prev < 0) { prev = s; run = 1; first = 1; }
+    else if (s == prev) ++run;
+    else {
+      if (!first) { cnt[prev] += 1; tot[prev] += run; }
+      prev = s; run = 1; first = 0;
+    }
+  }
+  P.st[o] = prev; P.st[plane + o] = run; P.st[2 * plane + o] = first;
+  P.st[3 * plane + o] = cnt[1]; P.st[4 * plane + o] = tot[1]; P.st[5 * plane + o] = cnt[0]; P.st[6 * plane + o] = tot[0];
+}
+struct UpDownReadParams {
+  const int32_t* st;     // [UD_NSTATE][G][N][SPC]
+  const int32_t* loc_id; // [G][SPC]
+  int32_t* n_up;         // [n_sims][N] or null
+  float* mean_up_ms;
+  int32_t* n_down;
+  float* mean_down_ms;
+  float sample_ms;       // ds * dt
+  int32_t N, SPC, G;
+};
+__global__ void updown_read_kernel(UpDownReadParams P) {
+  const int g = blockIdx.x / P.SPC, sl = blockIdx.x % P.SPC;
+  const int loc = P.loc_id[(size_t)g * P.SPC + sl];
+  if (loc < 0) return;
+  const int k = blockIdx.y * blockDim.x + threadIdx.x;
+  if (k >= P.N) return;
+  const size_t plane = (size_t)P.G * P.N * P.SPC, o = ((size_t)g * P.N + k) * P.SPC + sl;
+  const int cu = P.st[3 * plane + o], tu = P.st[4 * plane + o], cd = P.st[5 * plane + o], td = P.st[6 * plane + o];
+  const size_t w = (size_t)loc * P.N + k;
+  if (P.n_up) P.n_up[w] = cu;
+  if (P.n_down) P.n_down[w] = cd;
+  if (P.mean_up_ms) P.mean_up_ms[w] = cu > 0 ? (float)((double)tu * (double)P.sample_ms / (double)cu) : 0.0f;
+  if (P.mean_down_ms) P.mean_down_ms[w] = cd > 0 ? (float)((double)td * (double)P.sample_ms / (double)cd) : 0.0f;
+}
+
+// ---- top-k of a per-simulation score (f3; "output the best ten fittest simulations"; A23b) ----
+// One CTA of 1024 threads: k rounds of a block-wide arg-max over the S scores (local simulation order), equal scores
+// to the lower index; a taken entry is marked in `taken` (S bytes, zeroed by the caller).  k and S are small.
+__global__ void __launch_bounds__(1024) topk_kernel(const float* __restrict__ score, unsigned char* __restrict__ taken, int S, int k,
+                                                    int32_t* __restrict__ out_idx, float* __restrict__ out_val) {
+  __shared__ float sv[1024];
+  __shared__ int si[1024];
+  for (int r = 0; r < k && r < S; ++r) {
+    float bv = -INFINITY; int bi = -1;
+    for (int i = threadIdx.x; i < S; i += 1024)
+      if (!taken[i] && (bi < 0 || score[i] > bv)) { bv = score[i]; bi = i; }      // ascending i: the first maximum wins
+    sv[threadIdx.x] = bv; si[threadIdx.x] = bi;
+    __syncthreads();
+    for (int w = 512; w > 0; w >>= 1) {
+      if (threadIdx.x < w) {
+        const float ov = sv[threadIdx.x + w]; const int oi = si[threadIdx.x + w];
+        const int mi = si[threadIdx.x];
+        if (oi >= 0 && (mi < 0 || ov > sv[threadIdx.x] || (ov == sv[threadIdx.x] && oi < mi))) { sv[threadIdx.x] = ov; si[threadIdx.x] = oi; }
+      }
+      __syncthreads();
+    }
+    if (threadIdx.x == 0) { out_idx[r] = si[0]; out_val[r] = sv[0]; taken[si[0]] = 1; }
+    __syncthreads();
+  }
+}
+
 }  // namespace tvbx

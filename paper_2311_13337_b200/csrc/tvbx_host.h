@@ -145,6 +145,8 @@ struct DeviceSide {
   virtual int32_t readout(float* fc, float* me, float* mi, int on_device, cudaStream_t st) = 0;
   virtual int32_t scores(const double* ref, float* fcsc, float* fitness, float* mean_fc, int on_device, cudaStream_t st) = 0;
   virtual int32_t rate_stats(float* var_e, float* max_e, int32_t* above, float* var_i, float* max_i, int32_t* above_i, int on_device, cudaStream_t st) = 0;
+  virtual int32_t state_durations(int32_t* n_up, float* mean_up_ms, int32_t* n_down, float* mean_down_ms, int on_device, cudaStream_t st) = 0;
+  virtual int32_t top_k(int which, const double* ref, int k, int64_t* sim_ids, float* scores, int32_t* n_out, cudaStream_t st) = 0;
   virtual int32_t state(double* y, double* ou) = 0;
   virtual int32_t reset(cudaStream_t st) = 0;
 };
@@ -174,6 +176,7 @@ struct tvbx_sweep {
   bool fc_tc = false;     // FC co-moment on the tensor cores (tvbx_fc_tc.cuh)
   double rate_thr = 0.1;  // kHz: samples above it are counted (f4; 100 Hz)
   bool stats_i = false;   // keep the inhibitory 1-ms samples of the chunk too and their running statistics
+  double ud_thr = 0.0;    // kHz: up / down-state threshold (f4, A25); 0 = the episode statistics are off
   double init[7] = {0.001, 0.001, 0, 0, 0, 0, 0};
   // grouping
   std::vector<tvbx_host::HostTable> tables;

@@ -40,7 +40,10 @@ enum { P2_GW = 0, P2_IT, P2_B, P2_AT, P2_ITW, P2_ATEL, P2_GLEL, P2_CFE, P2_CFI }
 enum { NBAR = 8, LAGMAX = 4 };   // mbarrier ring; chunks a warp may run ahead
 enum { K2_MAXT = 480 };          // threads per CTA: 65536 / 480 -> 128 registers per thread (rounded down from 136)
 enum { K2_SMALLT = 224 };        // small CTAs: launch bound 224 -> 255 registers per thread
-enum { PVN = 24 };               // ring values of the next chunk a thread keeps in flight across one compute step:
+#ifndef TVBX_PVN_SMALL
+#define TVBX_PVN_SMALL 24
+#endif
+enum { PVN = 24, PVN_SMALL = TVBX_PVN_SMALL };               // ring values of the next chunk a thread keeps in flight across one compute step:
                                  // PVN / GCE edges x the first GCE = 8, 4 or 2 slots (GCE >= the chunk length).  Rows up to
                                  // (PVN / GCE) * CH edges are fully pipelined; longer rows finish in rounds of 8 edges
 
@@ -354,6 +357,15 @@ __global__ void __launch_bounds__(MAXT, 1) integrate2_kernel(const __grid_consta
     }
     if (CLU) cluster_sync_all(); else __syncthreads();      // (remote arrivals need the peers' barriers initialised)
   }
+  // Scalar ring loads of the cluster forms go through L1 like those of a single CTA: a warp reads the ring only after
+  // its acquire.cluster wait on the chunk barrier, which invalidates the SM's L1 (CCTL.IVALL), so a line fetched
+  // afterwards cannot hold stale values of the slots that wait released; the 8 loads of an edge's window then hit the
+  // one or two lines the first of them brought in.  (TVBX_CLU_RING_CG=1 restores L2-only loads.)
+#ifndef TVBX_CLU_RING_CG
+#define TVBX_CLU_RING_CG 0
+#endif
+  constexpr bool RING_CG = CLU && TVBX_CLU_RING_CG != 0;
+  constexpr int PV = MAXT <= K2_SMALLT ? PVN_SMALL : PVN;      // ring values in flight across one compute step
   const bool noise = P.noise_on != 0;
   const bool active = tid < NODES;
   const int node = active ? tid : NODES - 1;
@@ -387,8 +399,8 @@ __global__ void __launch_bounds__(MAXT, 1) integrate2_kernel(const __grid_consta
 
   // S1, not pipelined: coupling sums of the chunk that starts at ring slot cur0 into this thread's column
   auto gather_from = [&](int e, int cur0, f2 acc[GC / 2]) {
-    if (SMEMTAB) gather_rounds<RS, GCE, CLU>(s_edges, e, pe1, e_last, ringg, cur0, Hp, acc);
-    else gather_rounds<RS, GCE, CLU>(g_edges, e, pe1, e_last, ringg, cur0, Hp, acc);
+    if (SMEMTAB) gather_rounds<RS, GCE, RING_CG>(s_edges, e, pe1, e_last, ringg, cur0, Hp, acc);
+    else gather_rounds<RS, GCE, RING_CG>(g_edges, e, pe1, e_last, ringg, cur0, Hp, acc);
   };
   // VEC: the row's alignment classes; one class after the other, all edges of the row, for the chunk at slot cur0
   int4 segk = make_int4(0, 0, 0, 0);
@@ -480,6 +492,13 @@ __global__ void __launch_bounds__(MAXT, 1) integrate2_kernel(const __grid_consta
     if (GCE == 8 && noise) normals_now(n, (int)min((int64_t)(VEC ? CH - (int)(n % CH) : CH), P.n_end - n));
   }
 
+  // per-simulation parameters: small CTAs (relaxed register bound) keep the 9 pairs in registers, the others read them
+  // from shared memory where they are used
+  constexpr bool PREG = MAXT <= K2_SMALLT;
+  f2 ps_reg[NP2];
+#pragma unroll
+  for (int q = 0; q < NP2; ++q) ps_reg[q] = PREG ? s_ps[q * SPC] : mk2(0.0f, 0.0f);
+  auto par = [&](int q) -> f2 { return PREG ? ps_reg[q] : s_ps[q * SPC]; };
   auto wait_chunk = [&](uint32_t w) {              // all warps of the group have written chunk w
     if (CLU) mbar_wait_cluster(bar_done + (w & (NBAR - 1)), (w / NBAR) & 1u);
     else mbar_wait(bar_done + (w & (NBAR - 1)), (w / NBAR) & 1u);
@@ -500,28 +519,33 @@ __global__ void __launch_bounds__(MAXT, 1) integrate2_kernel(const __grid_consta
     f2 pacc[GC / 2];                              // coupling sums of chunk m + 1 in the making
 #pragma unroll
     for (int j = 0; j < GC / 2; ++j) pacc[j] = mk2(0.0f, 0.0f);
-    const bool traj_on = P.traj != nullptr && loc >= 0 && active && n - P.traj_n0 < P.traj_steps;
+    // step bookkeeping relative to the chunk start, in 32 bits (the 64-bit global step index n stays outside the step loop)
+    const int64_t t_rel = n - P.traj_n0;                                             // trajectory row of the chunk's first step
+    const bool traj_on = P.traj != nullptr && loc >= 0 && active && t_rel < P.traj_steps;
+    const int traj_left = traj_on ? (int)min(P.traj_steps - t_rel, (int64_t)GC) : 0;     // steps of this chunk that are recorded
+    float* const traj0 = traj_on ? P.traj + (((size_t)loc * P.traj_steps + (size_t)t_rel) * 7) * N + k : nullptr;
+    const int keep_from = (int)max((int64_t)-1, min(P.discard_steps - n, (int64_t)GC));  // windows ending at step i are kept iff i >= keep_from
+    const uint32_t n_lo = (uint32_t)n;
 #pragma unroll 2      // two steps per trip: the address arithmetic and parameter loads of step i + 1 overlap the
                       // arithmetic of step i and the rematerialised per-thread constants are shared (cfg 2 +2.8 %; 4 is slower)
     for (int i = 0; i < ch; ++i) {
-      const int64_t nn = n + i;
       const float cpl = s_cpl[i * T];
       // ---- S1 for the next chunk: issue the loads of the next PVN / GCE edges now, add them below ----
-      float pv[PVN];
+      float pv[PV];
       if (VEC) {}
-      else if (SMEMTAB) gather_issue<RS, PVN / GCE, GCE, CLU>(s_edges, pe0 + (PVN / GCE) * i, e_last, ringg, cur1, Hp, pv);   // (a table has >= 1 entry)
-      else gather_issue<RS, PVN / GCE, GCE, CLU>(g_edges, pe0 + (PVN / GCE) * i, e_last, ringg, cur1, Hp, pv);
+      else if (SMEMTAB) gather_issue<RS, PV / GCE, GCE, RING_CG>(s_edges, pe0 + (PV / GCE) * i, e_last, ringg, cur1, Hp, pv);   // (a table has >= 1 entry)
+      else gather_issue<RS, PV / GCE, GCE, RING_CG>(g_edges, pe0 + (PV / GCE) * i, e_last, ringg, cur1, Hp, pv);
       // ---- S2 inputs (Eq. 5; A5, A6, A10) ----
-      const f2 gw = s_ps[P2_GW * SPC];
+      const f2 gw = par(P2_GW);
       float drive = __fmaf_rn(gw.x, cpl, nu.x);
       if (noise) drive = __fmaf_rn(gw.y, ou, drive);
-      const f2 xe = add2(bc2(drive), s_ps[P2_CFE * SPC]);
-      const f2 xi_ = add2(bc2(nu.y), s_ps[P2_CFI * SPC]);
+      const f2 xe = add2(bc2(drive), par(P2_CFE));
+      const f2 xi_ = add2(bc2(nu.y), par(P2_CFI));
       const f2 se = mk2(xe.x > 0.0f ? P.kappa : 0.0f, xe.y > 0.0f ? P.kappa : 0.0f);      // A22 and the clamp of A10
       const f2 si = mk2(xi_.x > 0.0f ? P.kappa : 0.0f, xi_.y > 0.0f ? P.kappa : 0.0f);
       const f2 fe = add2(mk2(fmaxf(xe.x, 0.0f), fmaxf(xe.y, 0.0f)), bc2(P.tf.eps));
       const f2 fi = add2(mk2(fmaxf(xi_.x, 0.0f), fmaxf(xi_.y, 0.0f)), bc2(P.tf.eps));
-      const f2 c0 = sub2(s_ps[P2_GLEL * SPC], W);
+      const f2 c0 = sub2(par(P2_GLEL), W);
       f2 muV;
       const Jet2 F = tf_closed2(P.tf, fe, fi, c0, &muV);
       if (P.muV_local) {                          // A9b alternative: mu_V of the local rates only
@@ -531,7 +555,7 @@ __global__ void __launch_bounds__(MAXT, 1) integrate2_kernel(const __grid_consta
         muV = mk2((base + c0.x) / den, (base + c0.y) / den);
       }
       // ---- S3 Eqs. (1)-(3), forward Euler (A7, A9) ----
-      const f2 IT = bc2(s_ps[P2_IT * SPC].x);
+      const f2 IT = bc2(par(P2_IT).x);
       const f2 Fe = mul2(F.e, se), Fi = mul2(F.i, si);
       const f2 dF = sub2(F.v, nu);
       f2 a2nd = fma2(bc2(0.5f * Cs.x), mul2(F.ee, mul2(se, se)), dF);
@@ -544,7 +568,7 @@ __global__ void __launch_bounds__(MAXT, 1) integrate2_kernel(const __grid_consta
       const f2 Co = mk2(Cei, Cs.x), Cp = mk2(Cs.y, Cei);            // the other row
       const f2 h2 = fma2(Co, Fe, mul2(Cp, Fi));
       const float dCei = __fmaf_rn(dF.x, dF.y, (h2.x + h2.y) - 2.0f * Cei) * IT.x;
-      const f2 dW = fma2(s_ps[P2_AT * SPC], muV, fms2(s_ps[P2_B * SPC], nu, fma2(W, s_ps[P2_ITW * SPC], s_ps[P2_ATEL * SPC])));
+      const f2 dW = fma2(par(P2_AT), muV, fms2(par(P2_B), nu, fma2(W, par(P2_ITW), par(P2_ATEL))));
       nu = fma2(bc2(dt), dnu, nu);
       Cs = fma2(bc2(dt), dCs, Cs);
       Cei = __fmaf_rn(dt, dCei, Cei);
@@ -553,38 +577,38 @@ __global__ void __launch_bounds__(MAXT, 1) integrate2_kernel(const __grid_consta
       if (GCE == 8) {
         if (noise) ou = __fmaf_rn(P.ou_rho, ou, __fmaf_rn(P.ou_s, s_xi[i * T], P.ou_m));
       } else if (noise) {
-        if (((uint32_t)nn & 3u) == 0) {           // a new quad of normals
+        if (((n_lo + (uint32_t)i) & 3u) == 0) {   // a new quad of normals
           float xi[4];
-          normals4<float>(P.seed, ext, (uint32_t)k, (uint64_t)nn >> 2, xi);
+          normals4<float>(P.seed, ext, (uint32_t)k, (uint64_t)(n + i) >> 2, xi);
 #pragma unroll
           for (int q = 0; q < 4; ++q) s_quad[q * T] = xi[q];
         }
-        ou = __fmaf_rn(P.ou_rho, ou, __fmaf_rn(P.ou_s, s_quad[((uint32_t)nn & 3u) * T], P.ou_m));
+        ou = __fmaf_rn(P.ou_rho, ou, __fmaf_rn(P.ou_s, s_quad[((n_lo + (uint32_t)i) & 3u) * T], P.ou_m));
       }
       // ---- S1 for the next chunk: the loads issued above have had the whole step to arrive ----
       if (VEC) {}
-      else if (SMEMTAB) gather_add<PVN / GCE, GCE>(s_edges, pe0 + (PVN / GCE) * i, pe1, pipe, pv, pacc);
-      else gather_add<PVN / GCE, GCE>(g_edges, pe0 + (PVN / GCE) * i, pe1, pipe, pv, pacc);
+      else if (SMEMTAB) gather_add<PV / GCE, GCE>(s_edges, pe0 + (PV / GCE) * i, pe1, pipe, pv, pacc);
+      else gather_add<PV / GCE, GCE>(g_edges, pe0 + (PV / GCE) * i, pe1, pipe, pv, pacc);
       // ---- S5 ring write: E at time nn+1 (mirror the first GC-1 slots behind the period) ----
       c = c + 1 == Hp ? 0 : c + 1;
-      if (active) {
+      {     // (lanes past the last node replay it: they store the same value to the same address, no predicate needed)
         const uint32_t o = VEC ? myrow + ((uint32_t)c & ~(VW - 1u)) * (uint32_t)RS + ((uint32_t)c & (VW - 1u)) : myrow + (uint32_t)c * (uint32_t)RS;
         ringg[o] = nu.x;
         if (c < (VEC ? GC : GC - 1)) ringg[o + (uint32_t)Hp * (uint32_t)RS] = nu.x;
       }
       // ---- trajectory (tests / cfg 1) ----
-      if (traj_on && nn - P.traj_n0 < P.traj_steps) {
-        float* t = P.traj + (((size_t)loc * P.traj_steps + (size_t)(nn - P.traj_n0)) * 7) * N + k;
+      if (i < traj_left) {
+        float* t = traj0 + (size_t)i * 7 * N;
         t[0] = nu.x; t[N] = nu.y; t[2 * N] = Cs.x; t[3 * N] = Cei; t[4 * N] = Cs.y; t[5 * N] = W.x; t[6 * N] = W.y;
       }
       // ---- S6 temporal average (A17) ----
       win = add2(win, nu);
       if (--win_left == 0) {
         win_left = P.ds;
-        if (nn + 1 > P.discard_steps) {
+        if (i >= keep_from) {
           const f2 mm = scl2(inv_ds, win);
-          if (active) P.xbar[(((size_t)g * P.chunk_samples + sidx) * N + k) * SPC + sl] = mm.x;
-          if (ISAMP && active) P.xbar_i[(((size_t)g * P.chunk_samples + sidx) * N + k) * SPC + sl] = mm.y;
+          P.xbar[(((size_t)g * P.chunk_samples + sidx) * N + k) * SPC + sl] = mm.x;
+          if (ISAMP) P.xbar_i[(((size_t)g * P.chunk_samples + sidx) * N + k) * SPC + sl] = mm.y;
           sumE += (double)mm.x; sumI += (double)mm.y;
           ++sidx;
         }
@@ -595,7 +619,7 @@ __global__ void __launch_bounds__(MAXT, 1) integrate2_kernel(const __grid_consta
       gather_vec(cur1);
       if (noise) normals_now(n + ch, (int)min((int64_t)CH, P.n_end - (n + ch)));
     } else if (pipe) {      // the row's remaining edges (long rows, short chunks), then chunk m + 1 replaces chunk m
-      gather_from(pe0 + (PVN / GCE) * ch, cur1, pacc);   // (the registers of the transfer function are free here)
+      gather_from(pe0 + (PV / GCE) * ch, cur1, pacc);   // (the registers of the transfer function are free here)
       if (GCE == 8 && noise) normals_now(n + ch, (int)min((int64_t)CH, P.n_end - (n + ch)));
 #pragma unroll
       for (int j = 0; j < GC / 2; ++j) { s_cpl[(2 * j) * T] = pacc[j].x; s_cpl[(2 * j + 1) * T] = pacc[j].y; }

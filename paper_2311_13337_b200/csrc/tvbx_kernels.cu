@@ -2,9 +2,9 @@
 #include "tvbx_kernels.h"
 namespace tvbx {
 Kernel2Fn pick_kernel2(const Kernel2Key& k) {
-  if (k.sring) return k.gce == 2 ? k2_g2(k.spc, true) : k2_g4(k.spc, true);
+  if (k.sring) return k.gce == 2 ? k2_g2(k.spc, true) : (k.gce == 4 ? k2_g4(k.spc, true) : k2_g8_small_sring(k.spc));
   if (k.clu && k.vec) return k2_vec(k.spc, k.smemtab);
-  if (k.clu) return k2_clu(k.spc);
+  if (k.clu) return (k.small && k.smemtab && k.gce == 8) ? k2_clu_small(k.spc) : k2_clu(k.spc);
   if (!k.smemtab) return k2_nosmem(k.spc);
   if (k.gce == 2) return k2_g2(k.spc, false);
   if (k.gce == 4) return k2_g4(k.spc, false);

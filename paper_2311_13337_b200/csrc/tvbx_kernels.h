@@ -31,10 +31,12 @@ Kernel2Fn pick_kernel2(const Kernel2Key& k);                              // tvb
 // one function per instance family, each in its own translation unit
 Kernel2Fn k2_g8(int spc, bool isamp);              // SMEMTAB, 8 slots
 Kernel2Fn k2_g8_small(int spc, bool isamp);        // the same, launch bound K2_SMALLT
+Kernel2Fn k2_g8_small_sring(int spc);              // the same with the ring in shared memory
 Kernel2Fn k2_g4(int spc, bool sring);              // SMEMTAB, 4 slots (+ ring in shared memory)
 Kernel2Fn k2_g2(int spc, bool sring);              // SMEMTAB, 2 slots (+ ring in shared memory)
 Kernel2Fn k2_nosmem(int spc);                      // table through L1/L2, 8 slots
 Kernel2Fn k2_clu(int spc);                         // cluster, scalar gather
+Kernel2Fn k2_clu_small(int spc);                   // cluster, scalar gather, the CTA's rows of the table in shared memory, launch bound K2_SMALLT
 Kernel2Fn k2_vec(int spc, bool smemtab);           // cluster, vector gather (spc 4 or 8)
 
 }  // namespace tvbx

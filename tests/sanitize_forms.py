@@ -26,14 +26,16 @@ STEPS = int(os.environ.get("SANITIZE_STEPS", "160"))
 def form(name, N, v, keep=0.4, n_sims=5, expect=None, **kw):
     W, L = wl.connectome(N, seed=N, keep=keep)
     cfg = dict(axes=[dict(name="G", lo=0.05, hi=0.4, n=n_sims, values=None)], fixed=dict(v=v, b_e=20.0, wNoise=1e-4), seed=3)
-    conn, sw = tvbx.sweep_from_config(cfg, W, L, chunk_samples=5, **kw)
+    conn, sw = tvbx.sweep_from_config(cfg, W, L, chunk_samples=5, updown_threshold_khz=5e-4, **kw)
     for part in (STEPS // 2 + 3, STEPS - STEPS // 2 - 3):          # two launches: resume path, SRING copy-back
         sw.run(part, 0.1, noise_on=True, ds=10, discard_steps=20)
     fc, me, mi = sw.fc_readout()
     sc = sw.fc_scores()
     rs = sw.rate_stats()
+    ud = sw.state_durations()
+    ids, best = sw.top_k(3, which="mean_fc")
     info = sw.launch_info()
-    assert np.isfinite(fc).all() and np.isfinite(me).all() and np.isfinite(sc["fcsc"]).all() and np.isfinite(rs[0]).all()
+    assert np.isfinite(fc).all() and np.isfinite(me).all() and np.isfinite(sc["fcsc"]).all() and np.isfinite(rs[0]).all() and np.isfinite(ud[1]).all() and len(ids) == min(3, n_sims)
     if expect:
         assert sw.kernel_name() == expect, (sw.kernel_name(), expect)
     print(f"{name}: ok  kernel={sw.kernel_name()} fc={sw.fc_kernel_name()} launch={info}", flush=True)
@@ -56,6 +58,7 @@ def main():
     form("general kernel FP32, several region passes", 45, 3.0, sims_per_cta=4, threads_per_cta=64, expect=G)
     form("general kernel FP64 mode", 20, 4.0, precision=tvbx.TVBX_F64, expect=G)
     form("general kernel, tau_e != tau_i (jets)", 20, 4.0, params=dict(tau_i=7.5), expect=G)
+    form("ring in shared memory for the whole launch (small CTA, 8-slot chunks)", 30, 8.0, n_sims=2, sims_per_cta=1, expect=P2)
     form("FC register tiles", 33, 4.0, fc_mode=tvbx.TVBX_FC_FP32, expect=P2)
     form("FC tensor cores, two row blocks", 130, 4.0, keep=0.2, n_sims=2, sims_per_cta=2, expect=P2)
     print("all forms ok", flush=True)

@@ -70,3 +70,15 @@ def test_fc_scores_shapes_and_permutation_equivariance():
     out_p = fs.fc_scores(fc[:, p][:, :, p], sc[p][:, p], ref[p][:, p])
     for k in out:
         np.testing.assert_allclose(out_p[k], out[k], atol=1e-13)
+
+
+def test_top_k_against_numpy_sort_and_ties():
+    from oracle import fc_scores as ofs
+    rng = np.random.default_rng(5)
+    s = np.round(rng.normal(size=300), 1)                     # rounded: many exact ties
+    for k in (1, 10, 300, 400):
+        idx, val = ofs.top_k(s, k)
+        order = np.lexsort((np.arange(s.size), -s))[:k]       # by score descending, then index ascending
+        assert idx == order.tolist() and val == s[order].tolist()
+    assert ofs.top_k([0.5, 0.5, 0.7, 0.5], 3) == ([2, 0, 1], [0.7, 0.5, 0.5])
+    assert ofs.top_k([], 3) == ([], [])
