@@ -106,13 +106,24 @@ struct DeviceImpl : DeviceSide {
       if (c.edges.empty()) dmin = GC;
       const RingGeom rg = ring_geom(D, dmin, sw->packed, sw->vec_ok);
       ht.D = D; ht.dmin = dmin; ht.B = rg.B; ht.Hp = rg.Hp; ht.vec = rg.vec;
-      const int32_t Hs = ht.Hp + (rg.vec ? GC : GC - 1);
+      // one-step chunks (minimum delay <= 2 steps; cfg 3: v = 64, 128 m/s): the packed kernel keeps the group's ring in
+      // shared memory with EVERY slot mirrored (row length 2 Hp), so a read at slot cur + (Hp - d) never wraps, and
+      // gathers the row once per step from there (tvbx_integrate2.cuh, GCE == 1) -- if ring + table fit next to the rest
+      bool short1 = false;
+      if (sw->packed && sw->clu == 1 && rg.CH == 1 && !sw->stats_i && getenv("TVBX_NO_SRING") == nullptr) {
+        const size_t thr2 = (size_t)(N * SPC + 31) / 32 * 32;
+        const size_t need = (size_t)NBAR * 8 + 2 * GC * thr2 * sizeof(float) + (size_t)NP2 * SPC * sizeof(float2) + 64 +
+                            (c.edges.size() + 4 * (size_t)N + 1) * sizeof(Edge<float>) + (size_t)(N + 1) * 4 + (size_t)N * 2 * rg.Hp * RS * sizeof(float);
+        short1 = need <= (size_t)200 * 1024;
+      }
+      ht.short1 = short1;
+      const int32_t Hs = short1 ? 2 * ht.Hp : ht.Hp + (rg.vec ? GC : GC - 1);
       if ((double)N * Hs * RS >= 4294967295.0) return fail(TVBX_EINVAL, "ring of one CTA exceeds 32-bit element offsets");
       tds[t].Hp = ht.Hp; tds[t].Hs = Hs; tds[t].B = ht.B; tds[t].n_edges = (int32_t)c.edges.size();
       tds[t].CH = rg.CH; tds[t].LAG = rg.LAG;
       tds[t].edge_off = (int64_t)edges.size(); tds[t].rowptr_off = (int64_t)rowptr.size();
-      tds[t].vec = rg.vec; tds[t].seg_off = (int64_t)seg.size();
-      const int pad_to = 1;      // (rows may be padded with zero-weight copies of their first edge)
+      tds[t].vec = rg.vec; tds[t].seg_off = (int64_t)seg.size(); tds[t].pad0 = short1 ? 1 : 0;
+      const int pad_to = short1 ? 4 : 1;      // rows padded with zero-weight copies of their first edge: whole rounds of 4 edges
       for (int k = 0; k < N; ++k) {
         rowptr.push_back((int32_t)(edges.size() - (size_t)tds[t].edge_off));
         const int r0 = c.rowptr[k], r1 = c.rowptr[k + 1];
@@ -176,7 +187,7 @@ struct DeviceImpl : DeviceSide {
     for (int g = 0; g < G; ++g) {
       const HostGroup& hg = sw->groups[g];
       gds[g].table = hg.table; gds[g].pad = 0; gds[g].ring_off = (int64_t)ring_elems;
-      ring_elems += (size_t)N * (sw->tables[hg.table].Hp + (sw->tables[hg.table].vec ? GC : GC - 1)) * RS;
+      ring_elems += (size_t)N * tds[hg.table].Hs * RS;
       ring_elems = (ring_elems + 31) / 32 * 32;      // every group's ring starts on a 128-byte line
       for (int sl = 0; sl < SPC; ++sl) {
         const int64_t s = hg.lanes[sl];
@@ -192,7 +203,7 @@ struct DeviceImpl : DeviceSide {
         for (int q = 0; q < NPS; ++q) psim[((size_t)g * NPS + q) * SPC + sl] = (R)vals[q];
         if (sw->packed) {     // the same scalars as (excitatory, inhibitory) pairs
           const double twi = dp[TVBX_P_TAU_W_I], ati = dp[TVBX_P_A_I] / twi, gL = dp[TVBX_P_GL];
-          const double pr[NP2][2] = {{vals[0], vals[1]}, {vals[7], vals[7]}, {vals[2], dp[TVBX_P_B_I]}, {vals[3], ati},
+          const double pr[NP2][2] = {{vals[0], vals[1]}, {vals[7], vals[7] * dt}, {vals[2], dp[TVBX_P_B_I]}, {vals[3], ati},
                                      {vals[4], 1.0 / twi}, {vals[3] * vals[5], ati * vals[6]}, {gL * vals[5], gL * vals[6]},
                                      {vals[8], vals[10]}, {vals[9], vals[11]}};
           for (int q = 0; q < NP2; ++q) psim2[((size_t)g * NP2 + q) * SPC + sl] = make_float2((float)pr[q][0], (float)pr[q][1]);
@@ -269,7 +280,9 @@ struct DeviceImpl : DeviceSide {
     threads = 2 * SPC * rt;
     if constexpr (std::is_same<R, float>::value) kp = pick_kernel_f32(single, tf.same_tau != 0, SPC);
     else kp = pick_kernel_f64(single, tf.same_tau != 0);
-    const size_t tbytes = (size_t)tds[0].n_edges * sizeof(Edge<R>) + (size_t)(N + 1) * 4;
+    int32_t max_edges = 0;
+    for (const TableDesc& td : tds) max_edges = std::max(max_edges, td.n_edges);      // (tables differ by their row padding)
+    const size_t tbytes = (size_t)max_edges * sizeof(Edge<R>) + (size_t)(N + 1) * 4;
     const size_t base = ((size_t)(GC + 10) * (threads / 2) + (size_t)L_NPAR * threads + 20) * sizeof(R) + 16;
     P.smem_table = base + tbytes <= 200 * 1024;
     smem = (int)(base + (P.smem_table ? tbytes : 0));
@@ -315,11 +328,11 @@ struct DeviceImpl : DeviceSide {
     for (int g = 0; g < (int)sw->groups.size(); ++g) {
       const HostTable& ht = sw->tables[sw->groups[g].table];
       const int ch = ring_geom(ht.D, ht.dmin, true).CH;
-      const int gce = !P2.smem_table ? 8 : (ch <= 2 ? 2 : (ch <= 4 ? 4 : 8));
+      const int gce = !P2.smem_table ? 8 : (ht.short1 ? 1 : (ch <= 2 ? 2 : (ch <= 4 ? 4 : 8)));
       // short delays: the group's ring ([N][Hp + GC - 1][SPC] floats) in shared memory next to the table
-      const size_t ring_b = (size_t)N * (ht.Hp + GC - 1) * SPC * sizeof(float) + 16;
+      const size_t ring_b = (size_t)N * (ht.short1 ? 2 * ht.Hp : ht.Hp + GC - 1) * SPC * sizeof(float) + 16;
       // (and, for CTAs small enough for the relaxed register bound, whenever it fits: cfg 1)
-      const bool sring = CLU == 1 && P2.smem_table && (gce < 8 || (threads <= K2_SMALLT && !sw->stats_i)) &&
+      const bool sring = ht.short1 || CLU == 1 && P2.smem_table && (gce < 8 || (threads <= K2_SMALLT && !sw->stats_i)) &&
                          smem + ring_b <= (size_t)200 * 1024 && getenv("TVBX_NO_SRING") == nullptr;
       const int lsmem = smem + (sring ? (int)ring_b : 0);
       Kernel2Key key;

@@ -68,6 +68,7 @@ struct Axis { int32_t id; std::vector<double> vals; };
 struct HostTable {      // one per distinct speed
   double v = 0;
   int32_t D = 0, dmin = 0, B = 1, Hp = 2, vec = 0;
+  bool short1 = false;           // one-step chunks with the fully mirrored ring in shared memory (packed kernel, GCE == 1)
   std::vector<int32_t> delays;   // per kept edge, CSR order
   std::vector<int64_t> sims;     // local sim indices
 };

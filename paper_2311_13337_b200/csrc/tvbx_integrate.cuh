@@ -90,7 +90,7 @@ struct TableDesc {      // one per distinct speed v
   int64_t rowptr_off;   // first entry of this table's row pointer (N+1 ints)
   int64_t seg_off;      // VEC tables (integrate2_kernel, quad ring layout): first entry of the [N][4] class ends
   int32_t vec;          // 1: quad ring layout, rows sorted by window alignment class
-  int32_t pad0;
+  int32_t pad0;         // 1: every ring slot is mirrored (row length Hs = 2 Hp): one-step chunks of integrate2_kernel (GCE == 1)
 };
 struct GroupDesc {      // one per CTA
   int32_t table;

@@ -36,14 +36,11 @@
 namespace tvbx {
 
 enum { NP2 = 9 };       // packed per-simulation parameters, see P2_*
-enum { P2_GW = 0, P2_IT, P2_B, P2_AT, P2_ITW, P2_ATEL, P2_GLEL, P2_CFE, P2_CFI };
+enum { P2_GW = 0, P2_IT, P2_B, P2_AT, P2_ITW, P2_ATEL, P2_GLEL, P2_CFE, P2_CFI };   // P2_IT = (1/T, dt/T)
 enum { NBAR = 8, LAGMAX = 4 };   // mbarrier ring; chunks a warp may run ahead
 enum { K2_MAXT = 480 };          // threads per CTA: 65536 / 480 -> 128 registers per thread (rounded down from 136)
 enum { K2_SMALLT = 224 };        // small CTAs: launch bound 224 -> 255 registers per thread
-#ifndef TVBX_PVN_SMALL
-#define TVBX_PVN_SMALL 24
-#endif
-enum { PVN = 24, PVN_SMALL = TVBX_PVN_SMALL };               // ring values of the next chunk a thread keeps in flight across one compute step:
+enum { PVN = 24 };               // ring values of the next chunk a thread keeps in flight across one compute step:
                                  // PVN / GCE edges x the first GCE = 8, 4 or 2 slots (GCE >= the chunk length).  Rows up to
                                  // (PVN / GCE) * CH edges are fully pipelined; longer rows finish in rounds of 8 edges
 
@@ -279,7 +276,8 @@ __device__ __forceinline__ void gather_class_vec8(const Edge8* edges, int e, int
 }
 
 // SPC: simulations per CTA (1..8); SMEMTAB: the delay table of the group's speed is staged in shared memory;
-// GCE: ring slots loaded per edge = 2, 4 or 8 >= the chunk length CH of the launched groups (P.group0 ...).
+// GCE: ring slots loaded per edge = 2, 4 or 8 >= the chunk length CH of the launched groups (P.group0 ...); 1 = the one-step
+// form (with SRING; see gather_short).
 // CLU: the group is integrated by a thread-block cluster; CTA r of the cluster owns the regions [r*NL, (r+1)*NL), NL =
 // ceil(N / cluster size) (N = 360: 6 CTAs x 60 regions x 8 simulations -- lanes that share a region then read whole
 // 32-byte sectors of the ring, which a single CTA of <= 480 threads cannot offer at N = 360).
@@ -325,13 +323,13 @@ __global__ void __launch_bounds__(MAXT, 1) integrate2_kernel(const __grid_consta
   const int n_stage = CLU ? g_rowptr[min(k0 + NL, N)] - rp0 + 1 : td.n_edges;
   Edge<float>* const s_edges = reinterpret_cast<Edge<float>*>(tab);
   Edge8* const s_edges8 = reinterpret_cast<Edge8*>(tab);           // (VEC: 8-byte entries instead)
+  float2* const s_edges1 = reinterpret_cast<float2*>(tab);         // (GCE == 1: 8-byte entries (w, offset) instead)
   int32_t* const s_rowptr = reinterpret_cast<int32_t*>(s_edges + n_stage);
   const Edge<float>* const g_edges = P.edges + td.edge_off + rp0;
   float* s_ring = nullptr;                                          // SRING: [N][Hs][SPC] behind the row pointers
-  if (SRING) {
-    uintptr_t a = reinterpret_cast<uintptr_t>(s_rowptr + N + 1);
-    a = (a + 15) & ~(uintptr_t)15;
-    s_ring = reinterpret_cast<float*>(a);
+  if (SRING) {      // (offset arithmetic on smem_raw itself, so the compiler keeps the shared address space: LDS / STS)
+    const size_t off = (size_t)(reinterpret_cast<unsigned char*>(s_rowptr + N + 1) - smem_raw);
+    s_ring = reinterpret_cast<float*>(smem_raw + ((off + 15) & ~(size_t)15));
   }
   {
     if (tid < NBAR) mbar_init(bar_done + tid, (uint32_t)(T >> 5) * nrank);
@@ -345,6 +343,11 @@ __global__ void __launch_bounds__(MAXT, 1) integrate2_kernel(const __grid_consta
           e8.w = ed.w; e8.qb = (ed.pad / qdiv) | ((ed.back >> VWS) << 20);
           s_edges8[i] = e8;
         }
+      } else if (GCE == 1) {      // one-step form: (w, element offset of slot Hp - d of the source row) in 8 bytes
+        for (int i = tid; i < n_stage; i += T) {
+          const Edge<float> ed = g_edges[i];
+          s_edges1[i] = make_float2(ed.w, __uint_as_float(ed.pad));
+        }
       } else {
         for (int i = tid; i < n_stage; i += T) s_edges[i] = g_edges[i];
       }
@@ -357,15 +360,12 @@ __global__ void __launch_bounds__(MAXT, 1) integrate2_kernel(const __grid_consta
     }
     if (CLU) cluster_sync_all(); else __syncthreads();      // (remote arrivals need the peers' barriers initialised)
   }
-  // Scalar ring loads of the cluster forms go through L1 like those of a single CTA: a warp reads the ring only after
-  // its acquire.cluster wait on the chunk barrier, which invalidates the SM's L1 (CCTL.IVALL), so a line fetched
-  // afterwards cannot hold stale values of the slots that wait released; the 8 loads of an edge's window then hit the
-  // one or two lines the first of them brought in.  (TVBX_CLU_RING_CG=1 restores L2-only loads.)
-#ifndef TVBX_CLU_RING_CG
-#define TVBX_CLU_RING_CG 0
-#endif
-  constexpr bool RING_CG = CLU && TVBX_CLU_RING_CG != 0;
-  constexpr int PV = MAXT <= K2_SMALLT ? PVN_SMALL : PVN;      // ring values in flight across one compute step
+  // Scalar ring loads of the cluster forms go through L1 like those of a single CTA (RING_CG = false): a warp reads the
+  // ring only after its acquire.cluster wait on the chunk barrier, which invalidates the SM's L1 (CCTL.IVALL), so a line
+  // fetched afterwards cannot hold stale values of the slots that wait released; the 8 loads of an edge's window then
+  // hit the one or two lines the first of them brought in (cfg 4 as 4-CTA clusters: 1.52e10 with L2-only loads, 1.61e10 so).
+  constexpr bool RING_CG = false;
+  constexpr int PV = PVN;                         // ring values in flight across one compute step
   const bool noise = P.noise_on != 0;
   const bool active = tid < NODES;
   const int node = active ? tid : NODES - 1;
@@ -455,8 +455,25 @@ __global__ void __launch_bounds__(MAXT, 1) integrate2_kernel(const __grid_consta
 #pragma unroll
     for (int j = 0; j < GC; ++j) s_cpl[j * T] = cpl[j];
   };
+  // GCE == 1 (one-step chunks; the host mirrors EVERY slot of these rings, Hs = 2 Hp, and pads every row to whole rounds
+  // of 4 edges with zero weights): the coupling sum of the step whose time index sits in ring slot cur0, straight from
+  // the ring in shared memory -- per edge one table entry, one add (slot cur0 + Hp - d never wraps), one load, one FMA,
+  // the row's edges in ascending order in one chain (the association of every other form of the gather).
+  auto gather_short = [&](int cur0) {
+    const float* const base = ringg + (uint32_t)cur0 * (uint32_t)RS;
+    float a = 0.0f;
+    for (int e = pe0; e < pe1; e += 4) {      // (rows start at multiples of 4 entries: two 16-byte loads bring four edges)
+      const float4 p01 = *reinterpret_cast<const float4*>(s_edges1 + e), p23 = *reinterpret_cast<const float4*>(s_edges1 + e + 2);
+      const float v0 = base[__float_as_uint(p01.y)], v1 = base[__float_as_uint(p01.w)];
+      const float v2 = base[__float_as_uint(p23.y)], v3 = base[__float_as_uint(p23.w)];
+      a = __fmaf_rn(p23.z, v3, __fmaf_rn(p23.x, v2, __fmaf_rn(p01.z, v1, __fmaf_rn(p01.x, v0, a))));
+    }
+    s_cpl[0] = a;
+  };
   auto gather_now = [&](int cur0) {
-    if (VEC) {
+    if (GCE == 1) {
+      gather_short(cur0);
+    } else if (VEC) {
       gather_head_vec(cur0);
     } else {
       f2 acc[GC / 2];
@@ -486,7 +503,7 @@ __global__ void __launch_bounds__(MAXT, 1) integrate2_kernel(const __grid_consta
     for (int q = 0; q < 4; ++q) s_quad[q * T] = xi[q];
   }
   // the gather of chunk m + 1 can overlap the compute of chunk m only if it does not need chunk m itself
-  const bool LA = LAG >= 2;
+  const bool LA = GCE != 1 && LAG >= 2;           // (one-step form: the row is gathered at the start of its own step; CH = 1 => LAG = d_min + 1)
   if (LA && n < P.n_end) {                        // chunk 0 of the launch has no predecessor to hide behind
     gather_now(c);
     if (GCE == 8 && noise) normals_now(n, (int)min((int64_t)(VEC ? CH - (int)(n % CH) : CH), P.n_end - n));
@@ -532,7 +549,7 @@ __global__ void __launch_bounds__(MAXT, 1) integrate2_kernel(const __grid_consta
       const float cpl = s_cpl[i * T];
       // ---- S1 for the next chunk: issue the loads of the next PVN / GCE edges now, add them below ----
       float pv[PV];
-      if (VEC) {}
+      if (VEC || GCE == 1) {}
       else if (SMEMTAB) gather_issue<RS, PV / GCE, GCE, RING_CG>(s_edges, pe0 + (PV / GCE) * i, e_last, ringg, cur1, Hp, pv);   // (a table has >= 1 entry)
       else gather_issue<RS, PV / GCE, GCE, RING_CG>(g_edges, pe0 + (PV / GCE) * i, e_last, ringg, cur1, Hp, pv);
       // ---- S2 inputs (Eq. 5; A5, A6, A10) ----
@@ -555,23 +572,23 @@ __global__ void __launch_bounds__(MAXT, 1) integrate2_kernel(const __grid_consta
         muV = mk2((base + c0.x) / den, (base + c0.y) / den);
       }
       // ---- S3 Eqs. (1)-(3), forward Euler (A7, A9) ----
-      const f2 IT = bc2(par(P2_IT).x);
+      const f2 itp = par(P2_IT);                  // (1/T, dt/T)
+      const f2 IT = bc2(itp.x), DT = bc2(itp.y);
       const f2 Fe = mul2(F.e, se), Fi = mul2(F.i, si);
       const f2 dF = sub2(F.v, nu);
       f2 a2nd = fma2(bc2(0.5f * Cs.x), mul2(F.ee, mul2(se, se)), dF);
       a2nd = fma2(bc2(Cei), mul2(F.ei, mul2(se, si)), a2nd);
       a2nd = fma2(bc2(0.5f * Cs.y), mul2(F.ii, mul2(si, si)), a2nd);
-      const f2 dnu = mul2(a2nd, IT);
       const f2 Ca = mk2(Cs.x, Cei), Cb = mk2(Cei, Cs.y);            // row mu of the covariance matrix
       const f2 gC = fma2(Ca, Fe, fms2(Cb, Fi, Cs));                 // (C dF/dnu)_mu,mu - C_mu,mu
-      const f2 dCs = mul2(fma2(mul2(F.v, sub2(IT, F.v)), invN, fma2(dF, dF, add2(gC, gC))), IT);
+      const f2 dCs = fma2(mul2(F.v, sub2(IT, F.v)), invN, fma2(dF, dF, add2(gC, gC)));     // T dC/dt
       const f2 Co = mk2(Cei, Cs.x), Cp = mk2(Cs.y, Cei);            // the other row
       const f2 h2 = fma2(Co, Fe, mul2(Cp, Fi));
-      const float dCei = __fmaf_rn(dF.x, dF.y, (h2.x + h2.y) - 2.0f * Cei) * IT.x;
+      const float dCei = __fmaf_rn(dF.x, dF.y, (h2.x + h2.y) - 2.0f * Cei);                 // T dC_ei/dt
       const f2 dW = fma2(par(P2_AT), muV, fms2(par(P2_B), nu, fma2(W, par(P2_ITW), par(P2_ATEL))));
-      nu = fma2(bc2(dt), dnu, nu);
-      Cs = fma2(bc2(dt), dCs, Cs);
-      Cei = __fmaf_rn(dt, dCei, Cei);
+      nu = fma2(DT, a2nd, nu);                    // y <- y + (dt / T) (T dy/dt)
+      Cs = fma2(DT, dCs, Cs);
+      Cei = __fmaf_rn(itp.y, dCei, Cei);
       W = fma2(bc2(dt), dW, W);
       // ---- S4 OU (Eq. 4, A11) ----
       if (GCE == 8) {
@@ -586,7 +603,7 @@ __global__ void __launch_bounds__(MAXT, 1) integrate2_kernel(const __grid_consta
         ou = __fmaf_rn(P.ou_rho, ou, __fmaf_rn(P.ou_s, s_quad[((n_lo + (uint32_t)i) & 3u) * T], P.ou_m));
       }
       // ---- S1 for the next chunk: the loads issued above have had the whole step to arrive ----
-      if (VEC) {}
+      if (VEC || GCE == 1) {}
       else if (SMEMTAB) gather_add<PV / GCE, GCE>(s_edges, pe0 + (PV / GCE) * i, pe1, pipe, pv, pacc);
       else gather_add<PV / GCE, GCE>(g_edges, pe0 + (PV / GCE) * i, pe1, pipe, pv, pacc);
       // ---- S5 ring write: E at time nn+1 (mirror the first GC-1 slots behind the period) ----
@@ -594,7 +611,7 @@ __global__ void __launch_bounds__(MAXT, 1) integrate2_kernel(const __grid_consta
       {     // (lanes past the last node replay it: they store the same value to the same address, no predicate needed)
         const uint32_t o = VEC ? myrow + ((uint32_t)c & ~(VW - 1u)) * (uint32_t)RS + ((uint32_t)c & (VW - 1u)) : myrow + (uint32_t)c * (uint32_t)RS;
         ringg[o] = nu.x;
-        if (c < (VEC ? GC : GC - 1)) ringg[o + (uint32_t)Hp * (uint32_t)RS] = nu.x;
+        if (GCE == 1 || c < (VEC ? GC : GC - 1)) ringg[o + (uint32_t)Hp * (uint32_t)RS] = nu.x;
       }
       // ---- trajectory (tests / cfg 1) ----
       if (i < traj_left) {

@@ -21,7 +21,7 @@ typedef void (*Kernel2Fn)(const Integrate2Params);
 struct Kernel2Key {
   int spc;          // simulations per CTA, 1..8
   bool smemtab;     // delay table staged in shared memory
-  int gce;          // ring slots loaded per edge: 2, 4 or 8
+  int gce;          // ring slots loaded per edge: 2, 4 or 8; 1 = the one-step form
   bool clu, vec;    // thread-block cluster form; quad ring layout + vector gather
   bool sring;       // history ring in shared memory (short delays)
   bool small;       // CTAs of <= K2_SMALLT threads: relaxed register bound
@@ -34,6 +34,7 @@ Kernel2Fn k2_g8_small(int spc, bool isamp);        // the same, launch bound K2_
 Kernel2Fn k2_g8_small_sring(int spc);              // the same with the ring in shared memory
 Kernel2Fn k2_g4(int spc, bool sring);              // SMEMTAB, 4 slots (+ ring in shared memory)
 Kernel2Fn k2_g2(int spc, bool sring);              // SMEMTAB, 2 slots (+ ring in shared memory)
+Kernel2Fn k2_g1(int spc);                          // one-step chunks: fully mirrored ring in shared memory, row gathered per step
 Kernel2Fn k2_nosmem(int spc);                      // table through L1/L2, 8 slots
 Kernel2Fn k2_clu(int spc);                         // cluster, scalar gather
 Kernel2Fn k2_clu_small(int spc);                   // cluster, scalar gather, the CTA's rows of the table in shared memory, launch bound K2_SMALLT

@@ -49,8 +49,11 @@ struct Jet2 { f2 v, e, i, ee, ei, ii; };
 // t = 1/(1 + 0.4|z|), degree-8 fit from csrc/gen_erfcx_coeffs.py, relative error <= 4.7e-7)
 __device__ __forceinline__ f2 half_erfc2(f2 z, f2* ex) {
   const f2 zz = mul2(z, z);
-  const f2 e = mk2(sfu_ex2(-1.4426950408889634f * zz.x), sfu_ex2(-1.4426950408889634f * zz.y));
-  const f2 t = mk2(sfu_rcp(__fmaf_rn(0.4f, fabsf(z.x), 1.0f)), sfu_rcp(__fmaf_rn(0.4f, fabsf(z.y), 1.0f)));
+  const f2 ez = scl2(-1.4426950408889634f, zz);
+  const f2 e = mk2(sfu_ex2(ez.x), sfu_ex2(ez.y));
+  const f2 az = mk2(fabsf(z.x), fabsf(z.y));
+  const f2 td = fma2(bc2(0.4f), az, bc2(1.0f));
+  const f2 t = mk2(sfu_rcp(td.x), sfu_rcp(td.y));
   f2 p = bc2(5.018728834e-02f);
   p = fma2(p, t, bc2(-1.826153469e-01f));
   p = fma2(p, t, bc2(1.686438582e-01f));
@@ -62,7 +65,10 @@ __device__ __forceinline__ f2 half_erfc2(f2 z, f2* ex) {
   p = fma2(p, t, bc2(2.256758607e-01f));
   const f2 h = mul2(mul2(scl2(0.5f, e), t), p);
   *ex = e;
-  return mk2(z.x >= 0.0f ? h.x : 1.0f - h.x, z.y >= 0.0f ? h.y : 1.0f - h.y);
+  // erfc(-a)/2 = 1 - erfc(a)/2: result = off + sgn h with sgn = +-1 carrying the sign bit of z and off = (1 - sgn)/2
+  const f2 sgn = mk2(__uint_as_float(0x3f800000u | (__float_as_uint(z.x) & 0x80000000u)),
+                     __uint_as_float(0x3f800000u | (__float_as_uint(z.y) & 0x80000000u)));
+  return fma2(sgn, h, fma2(bc2(-0.5f), sgn, bc2(0.5f)));
 }
 
 // F_mu(f_e, f_i, W_mu) for mu = e (.x) and mu = i (.y).  c0 = g_L E_L,mu - W_mu.  *muV_out = mu_V.
@@ -93,12 +99,12 @@ __device__ __forceinline__ Jet2 tf_closed2(const TF2Const& c, f2 fe, f2 fi, f2 c
   const f2 sig = sqrt2(mul2(mul2(scl2(0.5f, mul2(r, r)), mul2(r, Q)), iB));
   const f2 s_e = mul2(sig, Le), s_i = mul2(sig, Li);
   const f2 s_ee = mul2(sig, fma2(Le, Le, Lee)), s_ei = mul2(sig, fma2(Le, Li, Lei)), s_ii = mul2(sig, fma2(Li, Li, Lii));
-  // mu_V: mu_e = ae (E_e - mu_V) r, mu_i = ai (E_i - mu_V) r; second derivatives from (mu_V A)_xy = 0
+  // mu_V: mu_e = ae (E_e - mu_V) r, mu_i = ai (E_i - mu_V) r, and r = 1/A: r_e = -a1 r, r_i = -a2 r.
+  // Their second derivatives are multiples of the first ones -- (mu_V A)_xy = 0 gives m_ee = -2 a1 m_e,
+  // m_ei = -(a1 m_i + a2 m_e), m_ii = -2 a2 m_i, and r_ee = -2 a1 r_e, r_ei = -(a1 r_i + a2 r_e), r_ii = -2 a2 r_i --
+  // so they are never formed: they enter u_xy below through t_x = (g_m - 1) m_x + g_t r_x.
   const f2 m_e = mul2(a1, mul2(pe, r)), m_i = mul2(a2, mul2(pi, r));
-  const f2 m_ee = mul2(scl2(-2.0f, a1), m_e), m_ei = neg2(fma2(a1, m_i, mul2(a2, m_e))), m_ii = mul2(scl2(-2.0f, a2), m_i);
-  // r = 1/A
   const f2 r_e = neg2(mul2(a1, r)), r_i = neg2(mul2(a2, r));
-  const f2 r_ee = mul2(scl2(-2.0f, a1), r_e), r_ei = mul2(scl2(-2.0f, a1), r_i), r_ii = mul2(scl2(-2.0f, a2), r_i);
   // Table-1 polynomial in the centred variables (x, y, w) = (mu_V - muV0, sigma_V - sV0, r - r0)
   const f2 x = sub2(muV, bc2(c.muV0)), y = sub2(sig, bc2(c.sV0)), w = sub2(r, bc2(c.r0));
   // gradient first; the value then follows from Euler's identity for a quadratic form:
@@ -114,26 +120,33 @@ __device__ __forceinline__ Jet2 tf_closed2(const TF2Const& c, f2 fe, f2 fi, f2 c
   // u = V_thr - mu_V
   const f2 u = sub2(V, muV);
   const f2 gm1 = sub2(gm, bc2(1.0f));             // d(V_thr - mu_V)/d mu_V
-  const f2 u_e = fma2(gm1, m_e, fma2(gs, s_e, mul2(gt, r_e)));
-  const f2 u_i = fma2(gm1, m_i, fma2(gs, s_i, mul2(gt, r_i)));
-  const f2 u_ee = fma2(gm1, m_ee, fma2(gs, s_ee, fma2(gt, r_ee, fma2(hm_e, m_e, fma2(hs_e, s_e, mul2(ht_e, r_e))))));
-  const f2 u_ei = fma2(gm1, m_ei, fma2(gs, s_ei, fma2(gt, r_ei, fma2(hm_e, m_i, fma2(hs_e, s_i, mul2(ht_e, r_i))))));
-  const f2 u_ii = fma2(gm1, m_ii, fma2(gs, s_ii, fma2(gt, r_ii, fma2(hm_i, m_i, fma2(hs_i, s_i, mul2(ht_i, r_i))))));
-  // z = u / (sqrt2 sigma): with Wz = 1/(sqrt2 sigma), Wz_x = -Wz L_x, Wz_xy = Wz (L_x L_y - L_xy)
+  // u_x = t_x + g_s s_x;  u_xy = g_m1 m_xy + g_t r_xy + g_s s_xy + (grad_x)^T H (grad_y)
+  //      with g_m1 m_xy + g_t r_xy = -2 a1 t_e (ee), -(a1 t_i + a2 t_e) (ei), -2 a2 t_i (ii)
+  const f2 t_e = fma2(gm1, m_e, mul2(gt, r_e)), t_i = fma2(gm1, m_i, mul2(gt, r_i));
+  const f2 u_e = fma2(gs, s_e, t_e), u_i = fma2(gs, s_i, t_i);
+  const f2 q_ee = fma2(hm_e, m_e, fma2(hs_e, s_e, mul2(ht_e, r_e)));
+  const f2 q_ei = fma2(hm_e, m_i, fma2(hs_e, s_i, mul2(ht_e, r_i)));
+  const f2 q_ii = fma2(hm_i, m_i, fma2(hs_i, s_i, mul2(ht_i, r_i)));
+  const f2 u_ee = fma2(scl2(-2.0f, a1), t_e, fma2(gs, s_ee, q_ee));
+  const f2 u_ei = fnma2(a1, t_i, fnma2(a2, t_e, fma2(gs, s_ei, q_ei)));
+  const f2 u_ii = fma2(scl2(-2.0f, a2), t_i, fma2(gs, s_ii, q_ii));
+  // z = u Wz with Wz = 1/(sqrt2 sigma), Wz_x = -Wz L_x, Wz_xy = Wz (L_x L_y - L_xy):  z_x = Wz zh_x, z_xy = Wz zh_xy with
+  // zh_x = u_x - u L_x,  zh_xy = u (L_x L_y - L_xy) - u_x L_y - u_y L_x + u_xy   (Wz is applied once, in G1 below)
   const f2 Wz = scl2(0.70710678118654752440f, rcp2(sig));
   const f2 z = mul2(u, Wz);
-  const f2 z_e = mul2(Wz, fnma2(u, Le, u_e)), z_i = mul2(Wz, fnma2(u, Li, u_i));
-  const f2 z_ee = mul2(Wz, fma2(u, fms2(Le, Le, Lee), fma2(scl2(-2.0f, u_e), Le, u_ee)));
-  const f2 z_ei = mul2(Wz, fma2(u, fms2(Le, Li, Lei), fnma2(u_e, Li, fnma2(u_i, Le, u_ei))));
-  const f2 z_ii = mul2(Wz, fma2(u, fms2(Li, Li, Lii), fma2(scl2(-2.0f, u_i), Li, u_ii)));
+  const f2 zh_e = fnma2(u, Le, u_e), zh_i = fnma2(u, Li, u_i);
+  const f2 zh_ee = fma2(u, fms2(Le, Le, Lee), fma2(scl2(-2.0f, u_e), Le, u_ee));
+  const f2 zh_ei = fma2(u, fms2(Le, Li, Lei), fnma2(u_e, Li, fnma2(u_i, Le, u_ei)));
+  const f2 zh_ii = fma2(u, fms2(Li, Li, Lii), fma2(scl2(-2.0f, u_i), Li, u_ii));
   // E = erfc(z)/2:  E' = -exp(-z^2)/sqrt(pi),  E'' = -2 z E'
+  // E_x = E' z_x = G1 zh_x,  E_xy = E'' z_x z_y + E' z_xy = G1 (K zh_x zh_y + zh_xy)  with G1 = E' Wz, K = -2 z Wz
   f2 ex;
   const f2 E0 = half_erfc2(z, &ex);
-  const f2 g0 = scl2(-0.56418958354775628695f, ex);
-  const f2 zz = scl2(-2.0f, z);
-  const f2 E_e = mul2(g0, z_e), E_i = mul2(g0, z_i);
-  const f2 zze = mul2(zz, z_e);
-  const f2 E_ee = mul2(g0, fma2(zze, z_e, z_ee)), E_ei = mul2(g0, fma2(zze, z_i, z_ei)), E_ii = mul2(g0, fma2(mul2(zz, z_i), z_i, z_ii));
+  const f2 G1 = mul2(scl2(-0.56418958354775628695f, ex), Wz);
+  const f2 K = mul2(scl2(-2.0f, z), Wz);
+  const f2 kze = mul2(K, zh_e), kzi = mul2(K, zh_i);
+  const f2 E_e = mul2(G1, zh_e), E_i = mul2(G1, zh_i);
+  const f2 E_ee = mul2(G1, fma2(kze, zh_e, zh_ee)), E_ei = mul2(G1, fma2(kze, zh_i, zh_ei)), E_ii = mul2(G1, fma2(kzi, zh_i, zh_ii));
   // 1/(2 tau_V) = A/(2B):  Rv = A/B, dRv/dA = C_m/B^2, d2Rv/dA2 = -2 tau C_m / B^3
   const f2 Rv = mul2(A, iB);
   const f2 RA = mul2(scl2(c.Cm, iB), iB);

@@ -143,6 +143,18 @@ def test_chunk_pipeline_results_do_not_depend_on_the_mapping(lmin, lmax, v):
     for y, ou, me in outs[1:]:
         np.testing.assert_array_equal(y, outs[0][0]); np.testing.assert_array_equal(ou, outs[0][1])
         np.testing.assert_array_equal(me, outs[0][2])
+    # and under different co-scheduling: two sweeps running concurrently on two streams perturb each other's warp timing
+    import torch
+    s1, s2 = torch.cuda.Stream(), torch.cuda.Stream()
+    _, a = tvbx.sweep_from_config(cfg, W, L, chunk_samples=64, sims_per_cta=3)
+    _, b = tvbx.sweep_from_config(cfg, W, L, chunk_samples=64, sims_per_cta=1)
+    for part in (2500, 3500):
+        a.run(part, 0.1, noise_on=True, ds=10, discard_steps=1000, stream=s1)
+        b.run(part, 0.1, noise_on=True, ds=10, discard_steps=1000, stream=s2)
+    torch.cuda.synchronize()
+    for sw in (a, b):
+        y, ou = sw.state()
+        np.testing.assert_array_equal(y, outs[0][0]); np.testing.assert_array_equal(ou, outs[0][1])
     o = orc.OracleSweep(W, L, wl.grid_params(cfg), seed=cfg["seed"])
     o.run(steps, 0.1, noise_on=True, ds=10, discard_steps=1000)
     rfc, rme, rmi = o.fc_readout()
