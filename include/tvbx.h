@@ -26,7 +26,7 @@
 extern "C" {
 #endif
 
-#define TVBX_VERSION 200 /* 0.2.0: diagnostics moved to tvbx_diag.h; lanes_per_node, tvbx_top_k */
+#define TVBX_VERSION 200 /* 0.2.0: diagnostics moved to tvbx_diag.h; latency_form, tvbx_top_k */
 
 enum tvbx_status {
   TVBX_OK = 0,
@@ -105,12 +105,13 @@ typedef struct tvbx_sweep_opts {
                                     the packed one, which is kept free of the extra store) */
   double rate_threshold_khz; /* tvbx_rate_stats counts the 1-ms excitatory samples above this rate; 0 = 0.1 kHz
                                 ("high firing rate activity exceeding 100 Hz") */
-  int32_t lanes_per_node; /* 0 = choose; 1 = one thread per (simulation, region) node (throughput mapping); 2 = the
-                             low-latency mapping for small sweeps / long runs ("a lesser thread
-                             count per GPU to hide latency"): a lane PAIR per node splits the row's delayed gather and
-                             the second-derivative part of the transfer-function jet and exchanges the partial sums with
-                             warp shuffles, so a sweep too small to fill the GPU with nodes runs twice the warps on a
-                             shorter per-step dependency chain.  Packed FP32 kernel, one CTA per group only */
+  int32_t latency_form;   /* 0 = choose; 1 = off; 2 = on (TVBX_EINVAL where it does not apply).  The LOW-LATENCY form of the packed
+                             kernel for small sweeps / long runs ("a lesser thread count per GPU to
+                             hide latency"): when the sweep offers about one warp of nodes per warp scheduler, throughput is the
+                             latency of one warp's step; a producer warp per consumer warp then takes the delayed gather, the
+                             Philox draws and their bookkeeping off that chain and runs on the schedulers' idle issue slots
+                             (csrc/tvbx_integrate2_ws.cuh).  Same arithmetic and Philox stream: results are bit-identical.
+                             Applies to one-CTA groups of <= 160 nodes with 8-step chunks (minimum delay >= 15 steps) */
   int32_t reserved0;
   double updown_threshold_khz; /* > 0: also keep the up / down-state episode statistics of the kept 1-ms excitatory samples
                                   (tvbx_state_durations; Tab. 2 P:131 `mean_UD_duration`): a sample is UP iff it exceeds

@@ -25,7 +25,7 @@ int32_t tvbx_profile_read(tvbx_sweep* sw, double ms[4], int64_t launches[4]);
 int32_t tvbx_bytes_copied(const tvbx_sweep* sw, int64_t* h2d, int64_t* d2h);
 /* launch geometry chosen for the integrator: CTAs, threads per CTA, sims per CTA, registers per thread, dynamic
  * shared memory bytes, region passes per time block, samples per FC chunk, local-memory bytes per thread,
- * CTAs per group (thread-block cluster size), lanes per (simulation, region) node */
+ * CTAs per group (thread-block cluster size), 2 if the low-latency warp-pair form runs (else 1) */
 int32_t tvbx_launch_info(const tvbx_sweep* sw, int32_t info[10]);
 /* name of the integrator kernel this sweep runs: "tvbx::integrate2_kernel" = the packed FP32 product kernel
  * (tau_e == tau_i, regions-per-CTA * sims_per_cta <= 480, sims_per_cta <= 8), "tvbx::integrate_kernel" = the general

@@ -53,7 +53,7 @@ class SweepOpts(C.Structure):
                 ("sim_ids", C.POINTER(C.c_int64)), ("chunk_samples", C.c_int64),
                 ("threads_per_cta", C.c_int32), ("ctas_per_group", C.c_int32),
                 ("fc_mode", C.c_int32), ("rate_stats_inhibitory", C.c_int32), ("rate_threshold_khz", C.c_double),
-                ("lanes_per_node", C.c_int32), ("reserved0", C.c_int32), ("updown_threshold_khz", C.c_double)]
+                ("latency_form", C.c_int32), ("reserved0", C.c_int32), ("updown_threshold_khz", C.c_double)]
 
 
 class RunOpts(C.Structure):
@@ -207,7 +207,7 @@ class Sweep:
 
     def __init__(self, conn: Connectome, axes, seed=0, params=None, precision=TVBX_F32, sims_per_cta=0,
                  sim_ids=None, chunk_samples=0, threads_per_cta=0, init=None, ctas_per_group=0, fc_mode=0, rate_threshold_khz=0.0,
-                 rate_stats_inhibitory=False, lanes_per_node=0, updown_threshold_khz=0.0):
+                 rate_stats_inhibitory=False, latency_form=0, updown_threshold_khz=0.0):
         L = lib()
         self.conn = conn
         m = ModelParams()
@@ -237,7 +237,7 @@ class Sweep:
                 ax[i].values = _dptr(arr)
         o = SweepOpts()
         o.precision = precision; o.sims_per_cta = sims_per_cta; o.chunk_samples = chunk_samples
-        o.threads_per_cta = threads_per_cta; o.ctas_per_group = ctas_per_group; o.fc_mode = fc_mode; o.rate_threshold_khz = rate_threshold_khz; o.rate_stats_inhibitory = int(bool(rate_stats_inhibitory)); o.lanes_per_node = int(lanes_per_node)
+        o.threads_per_cta = threads_per_cta; o.ctas_per_group = ctas_per_group; o.fc_mode = fc_mode; o.rate_threshold_khz = rate_threshold_khz; o.rate_stats_inhibitory = int(bool(rate_stats_inhibitory)); o.latency_form = int(latency_form)
         o.updown_threshold_khz = float(updown_threshold_khz)
         self.rate_stats_inhibitory = bool(rate_stats_inhibitory)
         if sim_ids is not None:
@@ -345,7 +345,7 @@ class Sweep:
     def launch_info(self):
         a = (C.c_int32 * 10)()
         _chk(lib().tvbx_launch_info(self._h, a))
-        keys = ("ctas", "threads", "sims_per_cta", "regs", "smem", "passes", "chunk_samples", "local_bytes", "ctas_per_group", "lanes_per_node")
+        keys = ("ctas", "threads", "sims_per_cta", "regs", "smem", "passes", "chunk_samples", "local_bytes", "ctas_per_group", "latency_form")
         return dict(zip(keys, a[:]))
 
     def reset(self, stream=None):

@@ -198,6 +198,8 @@ int32_t tvbx_sweep_create(const tvbx_connectome* c, const tvbx_model_params* def
   sw->precision = opts ? opts->precision : TVBX_F32;
   if (sw->precision != TVBX_F32 && sw->precision != TVBX_F64) return fail(TVBX_EINVAL, "precision=%d", sw->precision);
   sw->threads_req = opts ? opts->threads_per_cta : 0;
+  sw->ws_req = opts ? opts->latency_form : 0;
+  if (sw->ws_req < 0 || sw->ws_req > 2) return fail(TVBX_EINVAL, "latency_form=%d (valid: 0, 1, 2)", sw->ws_req);
   sw->chunk_req = opts ? opts->chunk_samples : 0;
   {
     sw->stats_i = opts && opts->rate_stats_inhibitory != 0;
@@ -236,7 +238,7 @@ int32_t tvbx_sweep_create(const tvbx_connectome* c, const tvbx_model_params* def
   // kernel if a delay table then needs a short-chunk instance, which has no inhibitory-sample variant)
   const bool packed_ok = sw->precision == TVBX_F32 && dp[TVBX_P_TAUE] == dp[TVBX_P_TAUI] && sw->conn.n <= 480 &&
                          (!sw->stats_i || sw->conn.n <= 120) && getenv("TVBX_GENERAL_KERNEL") == nullptr;
-  const int lanes_per_node = packed_ok ? 1 : 2;
+  const int lanes_per_node = packed_ok ? 1 : 2;      // threads per (sim, region) node: the general kernel uses a lane pair
   const int maxt_sel = packed_ok ? 480 : (sw->precision == TVBX_F64 ? 384 : 1024);
   const int spc_max = std::max(1, std::min(packed_ok ? 8 : 32, maxt_sel / (lanes_per_node * sw->conn.n)));
   // CTAs per group (thread-block cluster): the packed kernel can split the regions of a group over up to 8 CTAs.

@@ -321,6 +321,25 @@ struct DeviceImpl : DeviceSide {
       if (ht.vec && ((int64_t)N * ((ht.Hp + GC) / (int)tvbx::VW) >= (1 << 20) || ht.Hp / (int)tvbx::VW >= (1 << 12))) clu_tab = false;
     P2.smem_table = CLU == 1 ? base + tbytes <= 200 * 1024 : clu_tab;
     smem = (int)(base + (CLU == 1 ? (P2.smem_table ? tbytes : 0) : (clu_tab ? slice_bytes : 0)));
+    // Low-latency form (tvbx_integrate2_ws.cuh): producer / consumer warp pairs.  It pays when the sweep leaves the warp
+    // schedulers mostly idle -- all its CTAs resident at once with at most ~2 warps of nodes per scheduler -- and applies to
+    // one-CTA groups of <= 160 nodes whose tables all run 8-step chunks from a shared-memory table.
+    bool ws = false;
+    {
+      int n_sm = 148;
+      cudaDeviceGetAttribute(&n_sm, cudaDevAttrMultiProcessorCount, sw->device);
+      bool ok = CLU == 1 && !sw->stats_i && 2 * threads <= k2_ws_max_threads() && P2.smem_table != 0;
+      for (const HostTable& ht : sw->tables) ok = ok && ring_geom(ht.D, ht.dmin, true).CH == GC && !ht.short1;
+      const bool small_sweep = (int)sw->groups.size() <= 2 * n_sm;
+      if (sw->ws_req == 2 && !ok)
+        return fail(TVBX_EINVAL, "latency_form = 2 needs one-CTA groups of <= %d nodes, 8-step chunks (minimum delay >= 15 steps), no inhibitory samples",
+                    k2_ws_max_threads() / 2);
+      ws = ok && (sw->ws_req == 2 || (sw->ws_req == 0 && small_sweep && getenv("TVBX_NO_WS") == nullptr));
+    }
+    const size_t ws_base = (size_t)NBAR * 8 + (size_t)(threads / 32) * 4 * 8 + (size_t)4 * GC * threads * sizeof(float) +
+                           (size_t)NP2 * SPC * sizeof(float2) + 16;
+    if (ws) smem = (int)(ws_base + tbytes);
+    sw->split = ws ? 2 : 1;
     // one launch per run of groups whose chunk length falls in the same class (cfg 3: v <= 8 / 16 / >= 32 m/s)
     launches2.clear();
     cudaFuncAttributes fa;
@@ -338,7 +357,7 @@ struct DeviceImpl : DeviceSide {
       Kernel2Key key;
       key.spc = SPC; key.smemtab = P2.smem_table != 0; key.gce = gce; key.clu = CLU > 1; key.vec = ht.vec != 0; key.sring = sring;
       key.small = !key.vec && !sring && key.smemtab && gce == 8 && threads <= K2_SMALLT;
-      key.isamp = sw->stats_i;
+      key.isamp = sw->stats_i; key.ws = ws;
       Kernel2Fn fn = pick_kernel2(key);
       CU(raise_dynamic_smem((const void*)fn, lsmem));      // (per function, process-wide, raise-only)
       if (!launches2.empty() && launches2.back().fn == fn) {
@@ -352,7 +371,7 @@ struct DeviceImpl : DeviceSide {
       if (f1.numRegs >= fa.numRegs) fa = f1;
     }
     sw->info[0] = (int32_t)sw->groups.size() * CLU;
-    sw->info[1] = threads; sw->info[3] = fa.numRegs; sw->info[4] = smem; sw->info[5] = 1; sw->info[7] = (int32_t)fa.localSizeBytes;
+    sw->info[1] = ws ? 2 * threads : threads; sw->info[3] = fa.numRegs; sw->info[4] = smem; sw->info[5] = 1; sw->info[7] = (int32_t)fa.localSizeBytes;
     sw->info[8] = CLU;
     return TVBX_OK;
   }
@@ -475,11 +494,11 @@ struct DeviceImpl : DeviceSide {
         P2.sample_base = P.sample_base;
         for (const Launch2& l : launches2) {
           P2.group0 = l.g0;
-          if (sw->clu == 1) { l.fn<<<l.count, threads, l.smem, st>>>(P2); continue; }
+          if (sw->clu == 1) { l.fn<<<l.count, sw->split == 2 ? 2 * threads : threads, l.smem, st>>>(P2); continue; }
           cudaLaunchConfig_t lc;
           std::memset(&lc, 0, sizeof lc);
           lc.gridDim = dim3((unsigned)(l.count * sw->clu)); lc.blockDim = dim3((unsigned)threads);
-          lc.dynamicSmemBytes = (size_t)smem; lc.stream = st;
+          lc.dynamicSmemBytes = (size_t)l.smem; lc.stream = st;
           cudaLaunchAttribute at;
           at.id = cudaLaunchAttributeClusterDimension;
           at.val.clusterDim.x = (unsigned)sw->clu; at.val.clusterDim.y = 1; at.val.clusterDim.z = 1;

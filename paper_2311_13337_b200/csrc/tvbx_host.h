@@ -172,7 +172,8 @@ struct tvbx_sweep {
   int32_t clu = 1;        // CTAs (one thread-block cluster) per group: the regions are split over them
   bool vec_ok = false;    // cluster form with 4 or 8 simulations per group: vector gather where the chunk length allows
   bool packed = false;    // FP32 closed-form product kernel (integrate2_kernel)
-  int32_t split = 1;      // lanes per (simulation, region) node of the packed kernel: 2 = the low-latency mapping (f1)
+  int32_t ws_req = 0;     // tvbx_sweep_opts.latency_form: 0 choose, 1 off, 2 on
+  int32_t split = 1;      // 2 while the low-latency warp-pair form of the packed kernel runs (f1), else 1
   int64_t chunk_req = 0;
   bool fc_tc = false;     // FC co-moment on the tensor cores (tvbx_fc_tc.cuh)
   double rate_thr = 0.1;  // kHz: samples above it are counted (f4; 100 Hz)

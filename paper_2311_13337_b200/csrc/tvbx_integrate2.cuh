@@ -275,6 +275,53 @@ __device__ __forceinline__ void gather_class_vec8(const Edge8* edges, int e, int
   for (int j = 0; j < GC; ++j) { const int i = A0 + j; cpl[j] += (i & 1) ? acc[i >> 1].y : acc[i >> 1].x; }
 }
 
+// S2 + S3 of one (simulation, region) node: the inputs of Eq. (5) (A5, A6, A10), both transfer functions with first
+// and second derivatives (tf_closed2), Eqs. (1)-(3) (A7, A9, A22) and the forward-Euler update of
+// nu = (E, I), Cs = (C_ee, C_ii), C_ei, W = (W_e, W_i).  cpl = the delayed coupling sum of this step, ou = the OU state
+// (not advanced here); par(q) = the node's packed per-simulation parameter q (P2_*).  Shared by every form of the kernel.
+template <typename ParF>
+__device__ __forceinline__ void node_step2(const Integrate2Params& P, ParF par, float cpl, bool noise, float dt, f2 invN,
+                                           f2& nu, f2& Cs, f2& W, float& Cei, float ou) {
+  // ---- S2 inputs (Eq. 5; A5, A6, A10) ----
+  const f2 gw = par(P2_GW);
+  float drive = __fmaf_rn(gw.x, cpl, nu.x);
+  if (noise) drive = __fmaf_rn(gw.y, ou, drive);
+  const f2 xe = add2(bc2(drive), par(P2_CFE));
+  const f2 xi_ = add2(bc2(nu.y), par(P2_CFI));
+  const f2 se = mk2(xe.x > 0.0f ? P.kappa : 0.0f, xe.y > 0.0f ? P.kappa : 0.0f);      // A22 and the clamp of A10
+  const f2 si = mk2(xi_.x > 0.0f ? P.kappa : 0.0f, xi_.y > 0.0f ? P.kappa : 0.0f);
+  const f2 fe = add2(mk2(fmaxf(xe.x, 0.0f), fmaxf(xe.y, 0.0f)), bc2(P.tf.eps));
+  const f2 fi = add2(mk2(fmaxf(xi_.x, 0.0f), fmaxf(xi_.y, 0.0f)), bc2(P.tf.eps));
+  const f2 c0 = sub2(par(P2_GLEL), W);
+  f2 muV;
+  const Jet2 F = tf_closed2(P.tf, fe, fi, c0, &muV);
+  if (P.muV_local) {                          // A9b alternative: mu_V of the local rates only
+    const float le = fmaxf(nu.x, 0.0f) + P.tf.eps, li = fmaxf(nu.y, 0.0f) + P.tf.eps;
+    const float den = __fmaf_rn(P.tf.ae, le, __fmaf_rn(P.tf.ai, li, P.tf.gL));
+    const float base = __fmaf_rn(P.tf.aeEe, le, P.tf.aiEi * li);
+    muV = mk2((base + c0.x) / den, (base + c0.y) / den);
+  }
+  // ---- S3 Eqs. (1)-(3), forward Euler (A7, A9) ----
+  const f2 itp = par(P2_IT);                  // (1/T, dt/T)
+  const f2 IT = bc2(itp.x), DT = bc2(itp.y);
+  const f2 Fe = mul2(F.e, se), Fi = mul2(F.i, si);
+  const f2 dF = sub2(F.v, nu);
+  f2 a2nd = fma2(bc2(0.5f * Cs.x), mul2(F.ee, mul2(se, se)), dF);
+  a2nd = fma2(bc2(Cei), mul2(F.ei, mul2(se, si)), a2nd);
+  a2nd = fma2(bc2(0.5f * Cs.y), mul2(F.ii, mul2(si, si)), a2nd);
+  const f2 Ca = mk2(Cs.x, Cei), Cb = mk2(Cei, Cs.y);            // row mu of the covariance matrix
+  const f2 gC = fma2(Ca, Fe, fms2(Cb, Fi, Cs));                 // (C dF/dnu)_mu,mu - C_mu,mu
+  const f2 dCs = fma2(mul2(F.v, sub2(IT, F.v)), invN, fma2(dF, dF, add2(gC, gC)));     // T dC/dt
+  const f2 Co = mk2(Cei, Cs.x), Cp = mk2(Cs.y, Cei);            // the other row
+  const f2 h2 = fma2(Co, Fe, mul2(Cp, Fi));
+  const float dCei = __fmaf_rn(dF.x, dF.y, (h2.x + h2.y) - 2.0f * Cei);                 // T dC_ei/dt
+  const f2 dW = fma2(par(P2_AT), muV, fms2(par(P2_B), nu, fma2(W, par(P2_ITW), par(P2_ATEL))));
+  nu = fma2(DT, a2nd, nu);                    // y <- y + (dt / T) (T dy/dt)
+  Cs = fma2(DT, dCs, Cs);
+  Cei = __fmaf_rn(itp.y, dCei, Cei);
+  W = fma2(bc2(dt), dW, W);
+}
+
 // SPC: simulations per CTA (1..8); SMEMTAB: the delay table of the group's speed is staged in shared memory;
 // GCE: ring slots loaded per edge = 2, 4 or 8 >= the chunk length CH of the launched groups (P.group0 ...); 1 = the one-step
 // form (with SRING; see gather_short).
@@ -552,44 +599,8 @@ __global__ void __launch_bounds__(MAXT, 1) integrate2_kernel(const __grid_consta
       if (VEC || GCE == 1) {}
       else if (SMEMTAB) gather_issue<RS, PV / GCE, GCE, RING_CG>(s_edges, pe0 + (PV / GCE) * i, e_last, ringg, cur1, Hp, pv);   // (a table has >= 1 entry)
       else gather_issue<RS, PV / GCE, GCE, RING_CG>(g_edges, pe0 + (PV / GCE) * i, e_last, ringg, cur1, Hp, pv);
-      // ---- S2 inputs (Eq. 5; A5, A6, A10) ----
-      const f2 gw = par(P2_GW);
-      float drive = __fmaf_rn(gw.x, cpl, nu.x);
-      if (noise) drive = __fmaf_rn(gw.y, ou, drive);
-      const f2 xe = add2(bc2(drive), par(P2_CFE));
-      const f2 xi_ = add2(bc2(nu.y), par(P2_CFI));
-      const f2 se = mk2(xe.x > 0.0f ? P.kappa : 0.0f, xe.y > 0.0f ? P.kappa : 0.0f);      // A22 and the clamp of A10
-      const f2 si = mk2(xi_.x > 0.0f ? P.kappa : 0.0f, xi_.y > 0.0f ? P.kappa : 0.0f);
-      const f2 fe = add2(mk2(fmaxf(xe.x, 0.0f), fmaxf(xe.y, 0.0f)), bc2(P.tf.eps));
-      const f2 fi = add2(mk2(fmaxf(xi_.x, 0.0f), fmaxf(xi_.y, 0.0f)), bc2(P.tf.eps));
-      const f2 c0 = sub2(par(P2_GLEL), W);
-      f2 muV;
-      const Jet2 F = tf_closed2(P.tf, fe, fi, c0, &muV);
-      if (P.muV_local) {                          // A9b alternative: mu_V of the local rates only
-        const float le = fmaxf(nu.x, 0.0f) + P.tf.eps, li = fmaxf(nu.y, 0.0f) + P.tf.eps;
-        const float den = __fmaf_rn(P.tf.ae, le, __fmaf_rn(P.tf.ai, li, P.tf.gL));
-        const float base = __fmaf_rn(P.tf.aeEe, le, P.tf.aiEi * li);
-        muV = mk2((base + c0.x) / den, (base + c0.y) / den);
-      }
-      // ---- S3 Eqs. (1)-(3), forward Euler (A7, A9) ----
-      const f2 itp = par(P2_IT);                  // (1/T, dt/T)
-      const f2 IT = bc2(itp.x), DT = bc2(itp.y);
-      const f2 Fe = mul2(F.e, se), Fi = mul2(F.i, si);
-      const f2 dF = sub2(F.v, nu);
-      f2 a2nd = fma2(bc2(0.5f * Cs.x), mul2(F.ee, mul2(se, se)), dF);
-      a2nd = fma2(bc2(Cei), mul2(F.ei, mul2(se, si)), a2nd);
-      a2nd = fma2(bc2(0.5f * Cs.y), mul2(F.ii, mul2(si, si)), a2nd);
-      const f2 Ca = mk2(Cs.x, Cei), Cb = mk2(Cei, Cs.y);            // row mu of the covariance matrix
-      const f2 gC = fma2(Ca, Fe, fms2(Cb, Fi, Cs));                 // (C dF/dnu)_mu,mu - C_mu,mu
-      const f2 dCs = fma2(mul2(F.v, sub2(IT, F.v)), invN, fma2(dF, dF, add2(gC, gC)));     // T dC/dt
-      const f2 Co = mk2(Cei, Cs.x), Cp = mk2(Cs.y, Cei);            // the other row
-      const f2 h2 = fma2(Co, Fe, mul2(Cp, Fi));
-      const float dCei = __fmaf_rn(dF.x, dF.y, (h2.x + h2.y) - 2.0f * Cei);                 // T dC_ei/dt
-      const f2 dW = fma2(par(P2_AT), muV, fms2(par(P2_B), nu, fma2(W, par(P2_ITW), par(P2_ATEL))));
-      nu = fma2(DT, a2nd, nu);                    // y <- y + (dt / T) (T dy/dt)
-      Cs = fma2(DT, dCs, Cs);
-      Cei = __fmaf_rn(itp.y, dCei, Cei);
-      W = fma2(bc2(dt), dW, W);
+      // ---- S2 + S3: inputs, both transfer functions with derivatives, Eqs. (1)-(3), forward Euler ----
+      node_step2(P, par, cpl, noise, dt, invN, nu, Cs, W, Cei, ou);
       // ---- S4 OU (Eq. 4, A11) ----
       if (GCE == 8) {
         if (noise) ou = __fmaf_rn(P.ou_rho, ou, __fmaf_rn(P.ou_s, s_xi[i * T], P.ou_m));

@@ -1,0 +1,201 @@
+// tvbx_integrate2_ws.cuh -- the LOW-LATENCY form of the packed FP32 integrator for small sweeps and long runs
+// (BASELINE.json cfg 4: 256 simulations x 3,000,000 steps, cfg 1: 8 simulations; PAPER.md
+// with few work-items per GPU there are too few threads to hide latency).
+//
+// A sweep of a few hundred simulations offers about ONE warp per warp scheduler (cfg 4: 544 warps of nodes on the 592
+// schedulers of a B200), so its throughput is the latency of one warp's Euler step: ~520 dependent-ish instructions, of
+// which only ~300 are the model (both transfer functions with their jets, Eqs. (1)-(3)); the rest is the delayed gather for
+// the next chunk (table reads, address arithmetic, 24 ring loads and their FMAs per step), the Philox / Box-Muller draws
+// and bookkeeping -- and the schedulers sit at a third of their issue slots.  This form splits the two roles over a warp
+// PAIR on the idle slots (warp specialisation):
+//   consumer warp  = the nodes' state in registers; per step: inputs, transfer functions, Euler, OU, ring write, sample
+//   producer warp  = the same 32 nodes (lane for lane); per chunk of <= 8 steps: waits until the ring holds what the chunk
+//                    needs, gathers the whole row for its steps, draws the chunk's normals, and leaves both in the pair's
+//                    double-buffered shared-memory columns
+// Hand-over per pair through two full / empty mbarriers per buffer; the ring dependency across warps through the same
+// rolling chunk barriers as integrate2_kernel (a consumer arrives when it has written a chunk, a producer waits for chunk
+// m - LAG of all consumers before it gathers chunk m).  Arithmetic, association of the coupling sum (the row's edges in
+// ascending order into each slot) and the Philox stream are those of integrate2_kernel: results are bit-identical.
+// One CTA per group, delay table in shared memory, chunks of 8 steps (minimum delay >= 15 steps); SRING: the group's ring
+// in shared memory for the launch (cfg 1).
+#pragma once
+#include "tvbx_integrate2.cuh"
+
+namespace tvbx {
+
+enum { K2_WST = 320 };           // threads per CTA of this form (consumers + producers): 65536 / 320 -> 204 registers per thread
+
+template <int SPC, bool SRING>
+__global__ void __launch_bounds__(K2_WST, 1) integrate2_ws_kernel(const __grid_constant__ Integrate2Params P) {
+  extern __shared__ __align__(16) unsigned char smem_raw[];
+  constexpr int RS = SPC;
+  const int g = (int)blockIdx.x + P.group0;
+  const int N = P.N;
+  const int T = blockDim.x, TC = T >> 1;                   // consumer threads = producer threads (whole warps)
+  const bool prod = (int)threadIdx.x >= TC;
+  const int tid = prod ? (int)threadIdx.x - TC : (int)threadIdx.x;     // node slot: the same for the two warps of a pair
+  const int NW = TC >> 5, wp = tid >> 5;                   // warp pairs, this thread's pair
+  const int NODES = N * SPC;
+  const GroupDesc gd = P.groups[g];
+  const TableDesc td = P.tables[gd.table];
+  const int Hp = td.Hp, Hs = td.Hs, CH = td.CH, LAG = td.LAG;
+  // shared memory: NBAR chunk barriers | [NW][2] full, [NW][2] empty | 2 x [GC][TC] coupling sums | 2 x [GC][TC] normals |
+  // [NP2][SPC] parameters | edge table, row pointers | (SRING) ring
+  uint64_t* const bar_done = reinterpret_cast<uint64_t*>(smem_raw);
+  uint64_t* const bar_full = bar_done + NBAR + (size_t)wp * 2;
+  uint64_t* const bar_empty = bar_done + NBAR + (size_t)NW * 2 + (size_t)wp * 2;
+  float* const s_cpl = reinterpret_cast<float*>(bar_done + NBAR + (size_t)NW * 4) + tid;       // + b * GC * TC + i * TC
+  float* const s_xi = s_cpl + (size_t)2 * GC * TC;
+  float2* s_ps = reinterpret_cast<float2*>(reinterpret_cast<float*>(bar_done + NBAR + (size_t)NW * 4) + (size_t)4 * GC * TC);
+  unsigned char* tab = reinterpret_cast<unsigned char*>(s_ps + NP2 * SPC);
+  tab += (16 - (reinterpret_cast<uintptr_t>(tab) & 15)) & 15;
+  Edge<float>* const s_edges = reinterpret_cast<Edge<float>*>(tab);
+  int32_t* const s_rowptr = reinterpret_cast<int32_t*>(s_edges + td.n_edges);
+  const Edge<float>* const g_edges = P.edges + td.edge_off;
+  const int32_t* const g_rowptr = P.rowptr + td.rowptr_off;
+  float* s_ring = nullptr;
+  if (SRING) {
+    const size_t off = (size_t)(reinterpret_cast<unsigned char*>(s_rowptr + N + 1) - smem_raw);
+    s_ring = reinterpret_cast<float*>(smem_raw + ((off + 15) & ~(size_t)15));
+  }
+  {
+    const int t = (int)threadIdx.x;
+    if (t < NBAR) mbar_init(bar_done + t, (uint32_t)NW);
+    if (t < NW * 4) mbar_init(bar_done + NBAR + t, 1u);
+    for (int i = t; i < NP2 * SPC; i += T) s_ps[i] = P.psim2[(size_t)g * NP2 * SPC + i];
+    for (int i = t; i < td.n_edges; i += T) s_edges[i] = g_edges[i];
+    for (int i = t; i <= N; i += T) s_rowptr[i] = g_rowptr[i];
+    if (SRING) {
+      const float* gr = P.ring + gd.ring_off;
+      const int nr = N * Hs * RS;
+      for (int i = t; i < nr; i += T) s_ring[i] = gr[i];
+    }
+    __syncthreads();
+  }
+  const bool noise = P.noise_on != 0;
+  const bool active = tid < NODES;
+  const int node = active ? tid : NODES - 1;      // lanes past the last node replay it (same values to the same addresses)
+  const int k = node / SPC, sl = node - k * SPC;
+  s_ps += sl;
+  float* const ringg = (SRING ? s_ring : P.ring + gd.ring_off) + sl;
+  const int e_last = td.n_edges - 1;
+  const int pe0 = s_rowptr[k], pe1 = s_rowptr[k + 1];
+  const uint32_t ext = (uint32_t)P.ext_id[(size_t)g * SPC + sl];
+  const int64_t n0 = P.n_begin;
+  const int c0 = (int)(n0 % Hp);
+
+  if (prod) {
+    // ================= producer: coupling sums and normals of chunk m into buffer m & 1 =================
+    int64_t n = n0;
+    int c = c0;
+    for (uint32_t m = 0; n < P.n_end; ++m) {
+      const int ch = (int)min((int64_t)CH, P.n_end - n);
+      const uint32_t b = m & 1u;
+      if (m >= 2) mbar_wait(bar_empty + b, ((m >> 1) - 1u) & 1u);                  // the consumer has finished chunk m - 2
+      if (m >= (uint32_t)LAG) { const uint32_t w = m - (uint32_t)LAG; mbar_wait(bar_done + (w & (NBAR - 1)), (w / NBAR) & 1u); }
+      f2 acc[GC / 2];
+#pragma unroll
+      for (int j = 0; j < GC / 2; ++j) acc[j] = mk2(0.0f, 0.0f);
+      gather_rounds<RS, GC, false>(s_edges, pe0, pe1, e_last, ringg, c, Hp, acc);   // the row's edges in ascending order
+      float* const cpl = s_cpl + (size_t)b * GC * TC;
+#pragma unroll
+      for (int j = 0; j < GC / 2; ++j) { cpl[(2 * j) * TC] = acc[j].x; cpl[(2 * j + 1) * TC] = acc[j].y; }
+      if (noise) {                                // A12: one Philox call per (sim, region) per 4 steps
+        float* const xo = s_xi + (size_t)b * GC * TC;
+        float xi[4] = {0.f, 0.f, 0.f, 0.f};
+        for (int i = 0; i < ch; ++i) {
+          const uint64_t nn = (uint64_t)(n + i);
+          if (i == 0 || (nn & 3) == 0) normals4<float>(P.seed, ext, (uint32_t)k, nn >> 2, xi);
+          const uint32_t q = (uint32_t)nn & 3u;
+          xo[i * TC] = q == 0 ? xi[0] : (q == 1 ? xi[1] : (q == 2 ? xi[2] : xi[3]));
+        }
+      }
+      __syncwarp();
+      if ((tid & 31) == 0) mbar_arrive(bar_full + b);
+      n += ch;
+      c += ch; if (c >= Hp) c -= Hp;
+    }
+  } else {
+    // ================= consumer: the nodes' state in registers, one Euler step after the other =================
+    f2 ps_reg[NP2];
+#pragma unroll
+    for (int q = 0; q < NP2; ++q) ps_reg[q] = s_ps[q * SPC];
+    auto par = [&](int q) -> f2 { return ps_reg[q]; };
+    const uint32_t myrow = (uint32_t)(k * Hs) * (uint32_t)RS;
+    const int loc = P.loc_id[(size_t)g * SPC + sl];
+    const float dt = P.dt;
+    const float inv_ds = P.ds > 0 ? 1.0f / (float)P.ds : 0.0f;
+    const f2 invN = mk2(P.inv_Ne, P.inv_Ni);
+    const size_t stride = (size_t)N * SPC;
+    float* const sp = P.state + (size_t)g * (NSV - 2) * stride + (size_t)k * SPC + sl;
+    double* const sump = P.sums + (size_t)g * 2 * stride + (size_t)k * SPC + sl;
+    f2 nu = mk2(sp[0], sp[stride]), Cs = mk2(sp[2 * stride], sp[4 * stride]), W = mk2(sp[5 * stride], sp[6 * stride]);
+    f2 win = mk2(sp[8 * stride], sp[9 * stride]);
+    float Cei = sp[3 * stride], ou = sp[7 * stride];
+    double sumE = sump[0], sumI = sump[stride];
+    int64_t n = n0;
+    int c = c0;
+    int win_left = P.ds > 0 ? P.ds - (int)(n % P.ds) : 0x7fffffff;
+    int sidx = P.sample_base;
+    for (uint32_t m = 0; n < P.n_end; ++m) {
+      const int ch = (int)min((int64_t)CH, P.n_end - n);
+      const uint32_t b = m & 1u;
+      const int64_t t_rel = n - P.traj_n0;
+      const bool traj_on = P.traj != nullptr && loc >= 0 && active && t_rel < P.traj_steps;
+      const int traj_left = traj_on ? (int)min(P.traj_steps - t_rel, (int64_t)GC) : 0;
+      float* const traj0 = traj_on ? P.traj + (((size_t)loc * P.traj_steps + (size_t)t_rel) * 7) * N + k : nullptr;
+      const int keep_from = (int)max((int64_t)-1, min(P.discard_steps - n, (int64_t)GC));
+      mbar_wait(bar_full + b, (m >> 1) & 1u);                                      // the pair's producer has filled buffer b
+      const float* const cplb = s_cpl + (size_t)b * GC * TC;
+      const float* const xib = s_xi + (size_t)b * GC * TC;
+#pragma unroll 2
+      for (int i = 0; i < ch; ++i) {
+        const float cpl = cplb[i * TC];
+        node_step2(P, par, cpl, noise, dt, invN, nu, Cs, W, Cei, ou);
+        if (noise) ou = __fmaf_rn(P.ou_rho, ou, __fmaf_rn(P.ou_s, xib[i * TC], P.ou_m));      // S4 (Eq. 4, A11)
+        // S5 ring write: E at the next time index (the first GC - 1 slots are mirrored behind the period)
+        c = c + 1 == Hp ? 0 : c + 1;
+        {
+          const uint32_t o = myrow + (uint32_t)c * (uint32_t)RS;
+          ringg[o] = nu.x;
+          if (c < GC - 1) ringg[o + (uint32_t)Hp * (uint32_t)RS] = nu.x;
+        }
+        if (i < traj_left) {
+          float* t = traj0 + (size_t)i * 7 * N;
+          t[0] = nu.x; t[N] = nu.y; t[2 * N] = Cs.x; t[3 * N] = Cei; t[4 * N] = Cs.y; t[5 * N] = W.x; t[6 * N] = W.y;
+        }
+        // S6 temporal average (A17)
+        win = add2(win, nu);
+        if (--win_left == 0) {
+          win_left = P.ds;
+          if (i >= keep_from) {
+            const f2 mm = scl2(inv_ds, win);
+            P.xbar[(((size_t)g * P.chunk_samples + sidx) * N + k) * SPC + sl] = mm.x;
+            sumE += (double)mm.x; sumI += (double)mm.y;
+            ++sidx;
+          }
+          win = mk2(0.0f, 0.0f);
+        }
+      }
+      __syncwarp();
+      if ((tid & 31) == 0) {
+        mbar_arrive(bar_done + (m & (NBAR - 1)));      // chunk m is in the ring
+        mbar_arrive(bar_empty + b);                    // buffer b may be refilled
+      }
+      n += ch;
+    }
+    if (active) {
+      sp[0] = nu.x; sp[stride] = nu.y; sp[2 * stride] = Cs.x; sp[3 * stride] = Cei; sp[4 * stride] = Cs.y;
+      sp[5 * stride] = W.x; sp[6 * stride] = W.y; sp[7 * stride] = ou; sp[8 * stride] = win.x; sp[9 * stride] = win.y;
+      sump[0] = sumE; sump[stride] = sumI;
+    }
+  }
+  if (SRING) {                                    // the ring goes back to global memory for the next launch
+    __syncthreads();
+    float* gr = P.ring + gd.ring_off;
+    const int nr = N * Hs * RS;
+    for (int i = (int)threadIdx.x; i < nr; i += T) gr[i] = s_ring[i];
+  }
+}
+
+}  // namespace tvbx

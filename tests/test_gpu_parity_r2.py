@@ -159,3 +159,48 @@ def test_chunk_pipeline_results_do_not_depend_on_the_mapping(lmin, lmax, v):
     o.run(steps, 0.1, noise_on=True, ds=10, discard_steps=1000)
     rfc, rme, rmi = o.fc_readout()
     assert np.abs(outs[0][2] / rme - 1).max() < TOL_MEAN_REL
+
+
+# ------------------------------------------------------------------------------------ f1: the low-latency warp-pair form
+@pytest.mark.parametrize("N,n_sims,spc,v", [(68, 8, 1, 4.0), (68, 6, 2, 4.0), (23, 5, 5, 3.0), (37, 7, 3, 5.0)],
+                         ids=["cfg1_shape", "cfg4_shape", "n23_spc5", "n37_spc3"])
+def test_latency_form_is_bitwise_the_throughput_form(N, n_sims, spc, v):
+    """tvbx_sweep_opts.latency_form: producer / consumer warp pairs (csrc/tvbx_integrate2_ws.cuh) take the delayed gather
+    and the Philox draws off the consumer's dependency chain.  Same arithmetic, same association of the coupling sum, same
+    Philox stream: trajectories, OU state, FC and means must equal those of the one-warp form BIT FOR BIT, across several
+    launches (resume), with the ring in global or in shared memory; and both match the oracle."""
+    W, L = (wl.config_connectome(wl.config(1)) if N == 68 else wl.connectome(N, seed=N, keep=0.4))
+    cfg = dict(axes=[dict(name="G", lo=0.0, hi=0.4, n=n_sims, values=None)], fixed=dict(v=v, b_e=30.0, wNoise=1e-4), seed=12)
+    outs = {}
+    for form in (1, 2):
+        _, sw = tvbx.sweep_from_config(cfg, W, L, sims_per_cta=spc, latency_form=form, chunk_samples=40)
+        tr = [sw.run(part, 0.1, noise_on=True, ds=10, discard_steps=100, traj_steps=part) for part in (403, 1, 996)]
+        assert sw.launch_info()["latency_form"] == form and sw.kernel_name() == "tvbx::integrate2_kernel"
+        outs[form] = (np.concatenate(tr, axis=1), sw.state(), sw.fc_readout())
+    np.testing.assert_array_equal(outs[1][0], outs[2][0])
+    for a, b in zip(outs[1][1] + outs[1][2], outs[2][1] + outs[2][2]):
+        np.testing.assert_array_equal(a, b)
+    o = orc.OracleSweep(W, L, wl.grid_params(cfg), seed=cfg["seed"])
+    ref = o.run(1400, 0.1, noise_on=True, ds=10, discard_steps=100, traj_steps=1400)
+    assert traj_err(outs[2][0], ref) < 5e-3            # (noise-on extra: same Philox stream)
+    rfc, rme, rmi = o.fc_readout()
+    assert np.abs(outs[2][2][1] / rme - 1).max() < TOL_MEAN_REL and np.abs(outs[2][2][0] - rfc).max() < TOL_FC_ABS
+
+
+def test_latency_form_is_chosen_for_small_sweeps_and_refused_where_it_does_not_apply():
+    cfg = wl.config(4)
+    W, L = wl.config_connectome(cfg)
+    _, sw = tvbx.sweep_from_config(cfg, W, L)
+    sw.run(10, 0.1, noise_on=True, ds=10)
+    assert sw.launch_info()["latency_form"] == 2        # 256 sims: all CTAs resident, about one warp per scheduler
+    cfg2 = wl.config(2)
+    _, sw2 = tvbx.sweep_from_config(cfg2, W, L)
+    sw2.run(10, 0.1, noise_on=True, ds=10)
+    assert sw2.launch_info()["latency_form"] == 1       # 1,024 sims fill the GPU: throughput form
+    _, sw3 = tvbx.sweep_from_config(cfg2, W, L, latency_form=2)
+    with pytest.raises(tvbx.TvbxError):
+        sw3.run(10, 0.1, noise_on=True, ds=10)          # 476 nodes per CTA: does not apply
+    cfgv = dict(axes=[dict(name="G", lo=0.0, hi=0.4, n=4, values=None)], fixed=dict(v=60.0), seed=1)
+    _, sw4 = tvbx.sweep_from_config(cfgv, W, L, latency_form=2)
+    with pytest.raises(tvbx.TvbxError):
+        sw4.run(10, 0.1, noise_on=True, ds=10)          # minimum delay of 2 steps: one-step chunks
