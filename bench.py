@@ -77,7 +77,7 @@ def read_profile(cfg_id):
         vals = {}
         for line in txt.splitlines():
             parts = line.split()
-            if len(parts) >= 2 and re.match(r"^[a-z_]+__", parts[0]):
+            if len(parts) >= 2 and re.match(r"^[a-z0-9_]+__", parts[0]):
                 try:
                     vals[parts[0]] = (float(parts[1].replace(",", "")), parts[2] if len(parts) > 2 else "")
                 except ValueError:
@@ -263,10 +263,16 @@ def cpu_baseline(cfg_id):
 
 
 # ------------------------------------------------------------------------------------------------
-def measure_config(tvbx, torch, dist, cfg_id, steps, warmup, e2e_steps, sim_steps, rank, world, local, stream, pk, probes, clocks=None):
+def measure_config(tvbx, torch, dist, cfg_id, steps, warmup, e2e_steps, sim_steps, rank, world, local, stream, pk, probes, clocks=None,
+                   sim_slice=None):
     """One config: device-resident arm (value), end-to-end arm through the C ABI from host buffers (e2e), roofline.
     Returns a dict (rank 0 uses it)."""
     cfg, W, L, S = workload(cfg_id)
+    sim_ids = None
+    if sim_slice:                                # profiling runs only: every STEP-th simulation from START (cfg 3: one speed class)
+        start, stride = (int(x) for x in sim_slice.split(":"))
+        sim_ids = list(range(start, S, stride))
+        S = len(sim_ids)
     N, steps_sim = cfg["n"], (sim_steps or cfg["steps"])
     if steps_sim != cfg["steps"]:                # profiling runs only: keep the discard proportionate
         cfg["discard_steps"] = min(cfg["discard_steps"], (steps_sim // 5) // cfg["ds"] * cfg["ds"])
@@ -284,7 +290,7 @@ def measure_config(tvbx, torch, dist, cfg_id, steps, warmup, e2e_steps, sim_step
         return float(t.item())
 
     # ---- device-resident arm --------------------------------------------------------------------
-    conn, sw = tvbx.sweep_from_config(cfg, W, L, seed=seed)
+    conn, sw = tvbx.sweep_from_config(cfg, W, L, seed=seed, sim_ids=sim_ids)
     fc = torch.empty((S, N, N), device="cuda", dtype=torch.float32)
     me = torch.empty((S, N), device="cuda", dtype=torch.float32)
     mi = torch.empty((S, N), device="cuda", dtype=torch.float32)
@@ -359,7 +365,7 @@ def measure_config(tvbx, torch, dist, cfg_id, steps, warmup, e2e_steps, sim_step
     def e2e_step():
         nonlocal h2d, d2h
         ta = time.perf_counter()
-        c2, s2 = tvbx.sweep_from_config(cfg, W, L, seed=seed)
+        c2, s2 = tvbx.sweep_from_config(cfg, W, L, seed=seed, sim_ids=sim_ids)
         tb = time.perf_counter()
         s2.run(steps_sim, cfg["dt"], noise_on=True, ds=cfg["ds"], discard_steps=cfg["discard_steps"], stream=stream)
         tc = time.perf_counter()
@@ -453,10 +459,10 @@ def run_tvbx(args):
                   "hbm_read_gbs": P.read_bandwidth(4 << 30, 3)}
     clocks = ClockSampler(local) if rank == 0 else None
     head = measure_config(tvbx, torch, dist, args.config, args.steps, args.warmup, args.steps, args.sim_steps, rank, world, local,
-                          stream, pk, probes, clocks)
+                          stream, pk, probes, clocks, args.sim_slice)
     # the other BASELINE.json configs, each its own record (fewer repeats: the 1.5-3 s configs would not fit a default run)
     per_config = {}
-    if world == 1 and not args.headline_only and not args.sim_steps:
+    if world == 1 and not args.headline_only and not args.sim_steps and not args.sim_slice:
         plan = {1: (5, 3), 2: (3, 3), 3: (2, 3), 4: (1, 3), 5: (1, 3)}      # cfg -> (timed steps, warm-up steps)
         for cid, (k, w) in plan.items():
             if cid == args.config:
@@ -486,6 +492,7 @@ def main():
     ap.add_argument("--impl", default="tvbx", choices=["tvbx", "reference"])
     ap.add_argument("--config", type=int, default=2, help="BASELINE.json config number (1-5); the metric is quoted on 2")
     ap.add_argument("--sim-steps", type=int, default=0, help="override the Euler steps per simulation (profiling only)")
+    ap.add_argument("--sim-slice", default="", help="START:STEP -- only every STEP-th simulation from START (profiling only; cfg 3: one speed class = i:8)")
     ap.add_argument("--ref-steps", type=int, default=4000, help="Euler steps per oracle sample (--impl reference)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-probes", action="store_true", help="skip the ALU / L2 micro-benchmarks (bench_probes.cu)")

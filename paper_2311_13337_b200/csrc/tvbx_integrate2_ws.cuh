@@ -32,9 +32,15 @@ __global__ void __launch_bounds__(K2_WST, 1) integrate2_ws_kernel(const __grid_c
   const int g = (int)blockIdx.x + P.group0;
   const int N = P.N;
   const int T = blockDim.x, TC = T >> 1;                   // consumer threads = producer threads (whole warps)
-  const bool prod = (int)threadIdx.x >= TC;
-  const int tid = prod ? (int)threadIdx.x - TC : (int)threadIdx.x;     // node slot: the same for the two warps of a pair
-  const int NW = TC >> 5, wp = tid >> 5;                   // warp pairs, this thread's pair
+  const int NW = TC >> 5;                                  // warp pairs
+  // Which warp plays which role.  Warp w issues on scheduler w mod 4; a consumer carries ~3x the instructions of a producer.
+  // Consumers take warps 0 .. 3, one per scheduler; with a fifth pair (cfg 4: 136 nodes) its consumer is warp 6, so that the
+  // scheduler hosting two consumers hosts no producer (loads 530 / 530 / 660 / 430 issue slots per step instead of 760 / ...).
+  const int w = (int)threadIdx.x >> 5;
+  bool prod; int wp;
+  if (NW == 5) { prod = !(w < 4 || w == 6); wp = prod ? (w < 6 ? w - 4 : w - 5) : (w < 4 ? w : 4); }
+  else { prod = w >= NW; wp = prod ? w - NW : w; }
+  const int tid = wp * 32 + ((int)threadIdx.x & 31);       // node slot: the same for the two warps of a pair
   const int NODES = N * SPC;
   const GroupDesc gd = P.groups[g];
   const TableDesc td = P.tables[gd.table];

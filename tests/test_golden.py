@@ -119,3 +119,20 @@ def test_cuda_path_against_the_frozen_oracle_outputs():
         y, _ = sw.state()
         for q, nm in enumerate(names[:2]):
             assert float(y[0][q][0]) == pytest.approx(gold[f"node b_e={b_e:g} step=20000 {nm}"], rel=1e-3)
+
+
+def test_connectome_hashes():
+    """The seeded generator reproduces the recorded inputs bit for bit (tests/golden/connectome_sha256.txt)."""
+    import hashlib
+    want = {}
+    for line in open(os.path.join(os.path.dirname(__file__), "golden", "connectome_sha256.txt")):
+        if line.strip() and not line.startswith("#"):
+            parts = line.split()
+            want[parts[0]] = parts[-1]
+    for key, cid in (("cfg1-4", 1), ("cfg5", 5)):
+        W, L = wl.config_connectome(wl.config(cid))
+        assert W.dtype == np.float64 and W.flags.c_contiguous
+        assert hashlib.sha256(W.tobytes() + L.tobytes()).hexdigest() == want[key]
+    for cid in (2, 3, 4):                       # the same 68-region connectome
+        W, L = wl.config_connectome(wl.config(cid))
+        assert hashlib.sha256(W.tobytes() + L.tobytes()).hexdigest() == want["cfg1-4"]
