@@ -506,7 +506,7 @@ __global__ void __launch_bounds__(MAXT, 1) integrate2_kernel(const __grid_consta
   // of 4 edges with zero weights): the coupling sum of the step whose time index sits in ring slot cur0, straight from
   // the ring in shared memory -- per edge one table entry, one add (slot cur0 + Hp - d never wraps), one load, one FMA,
   // the row's edges in ascending order in one chain (the association of every other form of the gather).
-  auto gather_short = [&](int cur0) {
+  auto gather_short = [&](int cur0) -> float {
     const float* const base = ringg + (uint32_t)cur0 * (uint32_t)RS;
     float a = 0.0f;
     for (int e = pe0; e < pe1; e += 4) {      // (rows start at multiples of 4 entries: two 16-byte loads bring four edges)
@@ -515,11 +515,11 @@ __global__ void __launch_bounds__(MAXT, 1) integrate2_kernel(const __grid_consta
       const float v2 = base[__float_as_uint(p23.y)], v3 = base[__float_as_uint(p23.w)];
       a = __fmaf_rn(p23.z, v3, __fmaf_rn(p23.x, v2, __fmaf_rn(p01.z, v1, __fmaf_rn(p01.x, v0, a))));
     }
-    s_cpl[0] = a;
+    return a;
   };
   auto gather_now = [&](int cur0) {
     if (GCE == 1) {
-      gather_short(cur0);
+      s_cpl[0] = gather_short(cur0);      // (not used: the one-step form gathers inside its step loop)
     } else if (VEC) {
       gather_head_vec(cur0);
     } else {
@@ -567,12 +567,15 @@ __global__ void __launch_bounds__(MAXT, 1) integrate2_kernel(const __grid_consta
     if (CLU) mbar_wait_cluster(bar_done + (w & (NBAR - 1)), (w / NBAR) & 1u);
     else mbar_wait(bar_done + (w & (NBAR - 1)), (w / NBAR) & 1u);
   };
-  for (uint32_t m = 0; n < P.n_end; ++m) {
+  // One-step form (GCE == 1): the bookkeeping block below is still up to GC steps long, but every step is its own
+  // chunk of the rolling pipeline -- it waits for step m - LAG of all warps, gathers its row from the ring in shared
+  // memory, computes, writes the ring and arrives -- inside the step loop; m counts steps.
+  for (uint32_t m = 0; n < P.n_end; ) {
     // (VEC: a short first chunk brings the chunk starts to multiples of CH = GC, where every window alignment is fixed)
-    const int ch = (int)min((int64_t)(VEC ? CH - (int)(n % CH) : CH), P.n_end - n);
+    const int ch = (int)min((int64_t)(GCE == 1 ? GC : (VEC ? CH - (int)(n % CH) : CH)), P.n_end - n);
     const bool has_next = n + ch < P.n_end;
     const int cur1 = c + ch >= Hp ? c + ch - Hp : c + ch;          // ring slot of the next chunk's first step
-    if (!LA) {                                    // zero minimum delay: gather right before the chunk
+    if (!LA && GCE != 1) {                        // zero minimum delay: gather right before the chunk
       if (m >= (uint32_t)LAG) { const uint32_t w = m - (uint32_t)LAG; wait_chunk(w); }
       gather_now(c);
       if (GCE == 8 && noise) normals_now(n, ch);
@@ -593,7 +596,8 @@ __global__ void __launch_bounds__(MAXT, 1) integrate2_kernel(const __grid_consta
 #pragma unroll 2      // two steps per trip: the address arithmetic and parameter loads of step i + 1 overlap the
                       // arithmetic of step i and the rematerialised per-thread constants are shared (cfg 2 +2.8 %; 4 is slower)
     for (int i = 0; i < ch; ++i) {
-      const float cpl = s_cpl[i * T];
+      if (GCE == 1 && m + (uint32_t)i >= (uint32_t)LAG) wait_chunk(m + (uint32_t)i - (uint32_t)LAG);
+      const float cpl = GCE == 1 ? gather_short(c) : s_cpl[i * T];
       // ---- S1 for the next chunk: issue the loads of the next PVN / GCE edges now, add them below ----
       float pv[PV];
       if (VEC || GCE == 1) {}
@@ -642,6 +646,10 @@ __global__ void __launch_bounds__(MAXT, 1) integrate2_kernel(const __grid_consta
         }
         win = mk2(0.0f, 0.0f);
       }
+      if (GCE == 1) {       // one-step form: this step is a chunk of its own -- publish it
+        __syncwarp();
+        if ((tid & 31) == 0) mbar_arrive(bar_done + ((m + (uint32_t)i) & (NBAR - 1)));
+      }
     }
     if (pipe && VEC) {      // the whole row for chunk m + 1 with vector loads
       gather_vec(cur1);
@@ -653,12 +661,15 @@ __global__ void __launch_bounds__(MAXT, 1) integrate2_kernel(const __grid_consta
       for (int j = 0; j < GC / 2; ++j) { s_cpl[(2 * j) * T] = pacc[j].x; s_cpl[(2 * j + 1) * T] = pacc[j].y; }
     }
     // chunk m is written: publish it
-    __syncwarp();
-    if ((tid & 31) == 0) {
-      if (CLU) mbar_arrive_cluster(bar_done + (m & (NBAR - 1)), nrank);
-      else mbar_arrive(bar_done + (m & (NBAR - 1)));
+    if (GCE != 1) {
+      __syncwarp();
+      if ((tid & 31) == 0) {
+        if (CLU) mbar_arrive_cluster(bar_done + (m & (NBAR - 1)), nrank);
+        else mbar_arrive(bar_done + (m & (NBAR - 1)));
+      }
     }
     n += ch;
+    m += GCE == 1 ? (uint32_t)ch : 1u;
   }
   if (CLU) cluster_sync_all();                    // no CTA leaves while a peer may still arrive on its barriers
   if (SRING) {                                    // the ring goes back to global memory for the next launch
