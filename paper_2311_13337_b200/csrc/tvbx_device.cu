@@ -127,28 +127,39 @@ struct DeviceImpl : DeviceSide {
       for (int k = 0; k < N; ++k) {
         rowptr.push_back((int32_t)(edges.size() - (size_t)tds[t].edge_off));
         const int r0 = c.rowptr[k], r1 = c.rowptr[k + 1];
-        if (rg.vec) {      // quad layout: the row sorted by window alignment class a = (Hp - d) mod 4, ascending j inside
-          for (int a = 0; a < 4; ++a) {
+        if (rg.vec) {
+          // quad layout: the row as 7 segments by the alignment a = (Hp - d) mod 4 of an edge's 8-slot window, ascending j
+          // inside -- class 0 | classes 1, 2, 3 with the window shifted forward to the next quad boundary (two aligned quads
+          // instead of three; needs d >= 8 LAG - 1 + shift, tvbx_integrate2.cuh SHIFTED WINDOWS) | classes 1, 2, 3 "near"
+          // (closer than that: unshifted).  Every segment is padded to whole rounds of VR entries.
+          for (int sgm = 0; sgm < 7; ++sgm) {
+            const int a = sgm == 0 ? 0 : (sgm <= 3 ? sgm : sgm - 3);
+            const uint32_t sh = sgm >= 1 && sgm <= 3 ? (uint32_t)(4 - a) : 0u;
             int n_class = 0;
             for (int e = r0; e < r1; ++e) {
               const uint32_t back = (uint32_t)(ht.Hp - ht.delays[e]);
               if ((int)(back & 3u) != a) continue;
+              if (a != 0) {
+                const bool near_edge = ht.delays[e] < 8 * rg.LAG - 1 + (4 - a);
+                if (near_edge != (sgm > 3)) continue;
+              }
               Edge<R> ed;
               std::memset(&ed, 0, sizeof ed);
               ed.w = (R)c.edges[e].w;
               ed.jbase = (uint32_t)c.edges[e].j * (uint32_t)Hs * (uint32_t)RS;
-              ed.back = back;
-              set_pad(ed, ed.jbase + (back & ~(tvbx::VW - 1u)) * (uint32_t)RS);
+              ed.back = back + sh;
+              set_pad(ed, ed.jbase + (ed.back & ~(tvbx::VW - 1u)) * (uint32_t)RS);
               edges.push_back(ed);
               ++n_class;
             }
-            for (; n_class % VR != 0; ++n_class) {      // whole rounds: zero-weight copies of the class's last edge
+            for (; n_class % VR != 0; ++n_class) {      // whole rounds: zero-weight copies of the segment's last edge
               Edge<R> ed = edges.back();
               ed.w = R(0);
               edges.push_back(ed);
             }
             seg.push_back((int32_t)(edges.size() - (size_t)tds[t].edge_off));
           }
+          seg.push_back(0);      // (8 ints per row: two 16-byte loads)
           continue;
         }
         for (int e = r0; e < r1 || (e - r0) % pad_to != 0; ++e) {
@@ -231,7 +242,7 @@ struct DeviceImpl : DeviceSide {
     sw->CS = CS;
     int64_t* hb = &sw->h2d;
     CU(d_tables.upload(tds, hb)); CU(d_groups.upload(gds, hb)); CU(d_edges.upload(edges, hb)); CU(d_rowptr.upload(rowptr, hb));
-    if (seg.empty()) seg.assign(4, 0);
+    if (seg.empty()) seg.assign(8, 0);
     CU(d_seg.upload(seg, hb));
     CU(d_ext.upload(ext, hb)); CU(d_loc.upload(loc, hb)); CU(d_psim.upload(psim, hb));
     if (sw->packed) CU(d_psim2.upload(psim2, hb));
@@ -310,7 +321,8 @@ struct DeviceImpl : DeviceSide {
     const int CLU = sw->clu, NL = (N + CLU - 1) / CLU;      // regions per CTA
     threads = (NL * SPC + 31) / 32 * 32;
     single = true;
-    const size_t base = (size_t)NBAR * 8 + (size_t)2 * GC * threads * sizeof(float) + (size_t)NP2 * SPC * sizeof(float2) + 16;
+    // (vector-gather kernels keep two 8-step blocks of coupling sums per thread)
+    const size_t base = (size_t)NBAR * 8 + (size_t)(sw->vec_ok ? 3 : 2) * GC * threads * sizeof(float) + (size_t)NP2 * SPC * sizeof(float2) + 16;
     // cluster form: the vector-gather kernels stage the rows of the CTA's regions as 8-byte entries; the scalar
     // cluster kernels read the table through L1/L2, except the small-CTA instance (16-byte entries in shared memory)
     const size_t slice_bytes = max_slice_edges * (sw->vec_ok ? sizeof(Edge8) : sizeof(Edge<float>));

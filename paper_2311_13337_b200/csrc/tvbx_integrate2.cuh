@@ -63,7 +63,7 @@ struct Integrate2Params {
   const GroupDesc* groups;
   const Edge<float>* edges;
   const int32_t* rowptr;
-  const int32_t* seg;             // VEC tables: [N][4] end of the row's edges of alignment class 0..3 (TableDesc::seg_off)
+  const int32_t* seg;             // VEC tables: [N][8] ends of the 7 segments of a row (class 0, classes 1-3 shifted, classes 1-3 near; TableDesc::seg_off)
   const float2* psim2;            // [group][NP2][SPC]
   const int32_t* ext_id;          // [group][SPC]  external sim index (Philox counter)
   const int32_t* loc_id;          // [group][SPC]  local sim index (row of traj), -1 = padding lane
@@ -186,94 +186,75 @@ __device__ __forceinline__ void gather_rounds(EdgePtr edges, int e, int e1, int 
 
 // ---- vector form of the gather (VEC: cluster kernels whose chunk length is GC = 8) ---------------------------
 // Ring layout ring[group][region][slot / 4][sim][slot % 4] (Hp a multiple of 4, 8 mirror slots): the four
-// consecutive time slots of a quad sit in one 16-byte word per simulation, so a thread fetches its 8-slot window
-// with three aligned LDG.128 (12 slots) and the 8 lanes that share a region fetch whole 128-byte lines -- one L2
-// request per line instead of one per sector (the scalar cluster form is bound by the L1->XBAR request rate:
-// l1tex__m_l1tex2xbar_req_cycles_active 65 %).  Chunks start at multiples of GC, so the alignment of an edge's
-// window inside its first quad, a = (Hp - d) mod 4, never changes: the host sorts every row by a, the products
-// of a class are accumulated UNSHIFTED over the 12 fetched slots and folded once per class,
-// cpl[j] += acc[a + j] -- no per-edge select.  Per slot the association is: classes 0..3 in order, inside a class
-// the row's edges in ascending j (gather_head_vec reproduces it for the unaligned first chunk of a launch).
-// The host pads every class of a row to a multiple of VR entries with zero-weight copies of its last edge, so a
-// round needs neither an index clamp nor a weight mask.  Class 0 windows are quad-aligned: two quads suffice.
-enum { VR = 5 };                 // edges per round of the vector gather (VR x 12 values in registers)
-// Slots per ring word of the vector layout: 4 (quads, LDG.128: 2 or 3 loads per edge-chunk, 44 B fetched on average for the
-// 32 B used).  (A pair layout with LDG.64 -- 36 B, 4 or 5 loads -- was measured 4 % slower: DESIGN.md section 6.6.)
-constexpr uint32_t VW = 4;                          // slots per word
+// consecutive time slots of a quad sit in one 16-byte word per simulation, so the 8 lanes that share a region fetch
+// whole 128-byte lines with one LDG.128 each -- one L2 request per line instead of one per sector (the scalar cluster
+// form is bound by the L1->XBAR request rate).  Chunks start at multiples of GC, so the alignment of an edge's 8-slot
+// window inside its first quad, A = (Hp - d) mod 4, never changes, and the host sorts every row by it.
+//
+// SHIFTED WINDOWS.  An unaligned window (A != 0) spans three quads -- 48 bytes fetched for 32 used, and the gather
+// of N = 360 is bound by exactly those bytes (L2 -> SM path saturated).  So an edge of class A
+// fetches the TWO ALIGNED quads that start sh = (4 - A) mod 4 slots later: they hold its values for steps sh .. 7 of
+// the chunk being gathered and for steps 0 .. sh - 1 of the chunk after it.  Every thread therefore keeps TWO rows
+// of coupling sums in shared memory (16 slots, the 8-step block's parity selects the row): the gather for block b + 1
+// completes block b + 1's slots (whose first sh_max = 3 slots hold partial sums from the previous gather) and leaves
+// partial sums in the first three slots of block b + 2.  Reading sh slots further ahead needs the delay to be at
+// least 8 LAG - 1 + sh steps; the few edges closer than that ("near": cfg 5 has 0.1 % of them) keep the
+// unshifted three-quad window.  A row is stored as 7 segments: class 0 | classes 1, 2, 3 shifted | classes 1, 2, 3
+// near, each padded to whole rounds of VR entries with zero-weight copies of its last edge (no clamps, no masks).
+// Per slot j of a block the association is: the shifted classes with sh > j in class order (previous gather), then
+// class 0 and the shifted classes with sh <= j in class order, then the near classes; inside a class the row's edges
+// in ascending order.  gather_head_vec reproduces it with scalar loads for the first chunk of a launch.
+enum { VR = 4 };                 // edges per round of the vector gather (segments are padded to multiples of it)
+constexpr uint32_t VW = 4;                          // slots per ring word (a pair layout with LDG.64 was measured 4 % slower)
 constexpr uint32_t VWS = 2;                         // log2
-template <int A> struct VecWords { static constexpr int n = A == 0 ? 2 : 3; };
 struct VecLd { typedef float4 word; };
 // acc += w * (the 4 slots of word q): acc holds f2 pairs of consecutive slots
 __device__ __forceinline__ void vec_fma(f2* acc, int i, float w, const VecLd::word& q) {
   acc[2 * i] = fma2(bc2(w), mk2(q.x, q.y), acc[2 * i]);
   acc[2 * i + 1] = fma2(bc2(w), mk2(q.z, q.w), acc[2 * i + 1]);
 }
-template <int RS, int A, typename EdgePtr>
-__device__ __forceinline__ void gather_class_vec(EdgePtr edges, int e, int e1, const float* ringv,
-                                                 uint32_t curRS, uint32_t thr, uint32_t wrapRS, float cpl[GC]) {
-  constexpr int NQ = VecWords<A>::n;                      // words fetched per edge
-  constexpr int NA = NQ * (int)VW / 2;                    // f2 accumulators (pairs of consecutive slots)
-  constexpr int A0 = A & ((int)VW - 1);                   // offset of the window inside its first word
-  f2 acc[NA];
-#pragma unroll
-  for (int i = 0; i < NA; ++i) acc[i] = mk2(0.0f, 0.0f);
-  const uint32_t curW = curRS - wrapRS;
-  for (; e < e1; e += VR) {
-    VecLd::word q[VR][NQ];
-    float w[VR];
-#pragma unroll
-    for (int b = 0; b < VR; ++b) {
-      const Edge<float> ed = edges[e + b];
-      const uint32_t off = ed.pad + (ed.back >= thr ? curW : curRS);
-      const VecLd::word* src = reinterpret_cast<const VecLd::word*>(ringv + off);
-#pragma unroll
-      for (int i = 0; i < NQ; ++i) q[b][i] = __ldcg(src + i * RS);
-      w[b] = ed.w;
-    }
-#pragma unroll
-    for (int b = 0; b < VR; ++b) {
-#pragma unroll
-      for (int i = 0; i < NQ; ++i) vec_fma(acc, i, w[b], q[b][i]);
-    }
-  }
-#pragma unroll
-  for (int j = 0; j < GC; ++j) { const int i = A0 + j; cpl[j] += (i & 1) ? acc[i >> 1].y : acc[i >> 1].x; }
-}
-
-// The same with the 8-byte entries the vector kernels stage in shared memory (Edge8: w and, in one word, the
-// word index Q = j * Hs/VW + (Hp - d)/VW in the low 20 bits and (Hp - d)/VW in the high 12): half the shared
-// memory of the 16-byte entries, which leaves the L1 the room it needs as landing space for the loads in flight.
+// 8-byte table entry of the vector kernels: w and, in one word, the word index Q = j * Hs/VW + back/VW in the low 20 bits
+// and back/VW in the high 12 (back = Hp - d, plus the shift of a shifted class): half the shared memory of the 16-byte
+// entries, which leaves the L1 the room it needs as landing space for the loads in flight.
 struct __align__(8) Edge8 { float w; uint32_t qb; };
-template <int RS, int A>
-__device__ __forceinline__ void gather_class_vec8(const Edge8* edges, int e, int e1, const VecLd::word* ringw,
-                                                  uint32_t cur4, uint32_t thr4, uint32_t curW4, float cpl[GC]) {
-  constexpr int NQ = VecWords<A>::n;
-  constexpr int NA = NQ * (int)VW / 2;
-  constexpr int A0 = A & ((int)VW - 1);
-  f2 acc[NA];
+__device__ __forceinline__ Edge8 edge8_of(const Edge<float>& ed, uint32_t qdiv) {
+  Edge8 e8;
+  e8.w = ed.w; e8.qb = (ed.pad / qdiv) | ((ed.back >> VWS) << 20);
+  return e8;
+}
+// One segment of a row: edges [e, e1) (whole rounds of VR), NQ aligned quads per edge from the entry's word index on;
+// the products are accumulated unshifted over the NQ * 4 fetched slots in acc (NQ * 2 pairs).  get(e) -> Edge8.
+template <int RS, int NQ, int NE, typename Get>
+__device__ __forceinline__ void gather_round_vec(Get get, int e, const VecLd::word* ringw, uint32_t cur4, uint32_t thr4, uint32_t curW4, f2* acc) {
+  VecLd::word q[NE][NQ];
+  float w[NE];
 #pragma unroll
-  for (int i = 0; i < NA; ++i) acc[i] = mk2(0.0f, 0.0f);
-  for (; e < e1; e += VR) {
-    VecLd::word q[VR][NQ];
-    float w[VR];
+  for (int b = 0; b < NE; ++b) {
+    const Edge8 ed = get(e + b);
+    const uint32_t idx = (ed.qb & 0xFFFFFu) + ((ed.qb >> 20) >= thr4 ? curW4 : cur4);
+    const VecLd::word* src = ringw + (size_t)idx * RS;
 #pragma unroll
-    for (int b = 0; b < VR; ++b) {
-      const Edge8 ed = edges[e + b];
-      const uint32_t idx = (ed.qb & 0xFFFFFu) + ((ed.qb >> 20) >= thr4 ? curW4 : cur4);
-      const VecLd::word* src = ringw + (size_t)idx * RS;
-#pragma unroll
-      for (int i = 0; i < NQ; ++i) q[b][i] = __ldcg(src + i * RS);
-      w[b] = ed.w;
-    }
-#pragma unroll
-    for (int b = 0; b < VR; ++b) {
-#pragma unroll
-      for (int i = 0; i < NQ; ++i) vec_fma(acc, i, w[b], q[b][i]);
-    }
+    for (int i = 0; i < NQ; ++i) q[b][i] = __ldcg(src + i * RS);
+    w[b] = ed.w;
   }
 #pragma unroll
-  for (int j = 0; j < GC; ++j) { const int i = A0 + j; cpl[j] += (i & 1) ? acc[i >> 1].y : acc[i >> 1].x; }
+  for (int b = 0; b < NE; ++b) {
+#pragma unroll
+    for (int i = 0; i < NQ; ++i) vec_fma(acc, i, w[b], q[b][i]);
+  }
 }
+// (two-quad segments run rounds of 2 VR edges while they last -- 16 LDG.128 in flight per thread: with 10 the gather fell
+// from 10.4 to 6.4 TB/s on the L2 -> SM path -- then one round of VR)
+template <int RS, int NQ, typename Get>
+__device__ __forceinline__ void gather_seg_vec(Get get, int e, int e1, const VecLd::word* ringw, uint32_t cur4, uint32_t thr4,
+                                               uint32_t curW4, f2* acc) {
+#pragma unroll
+  for (int i = 0; i < NQ * 2; ++i) acc[i] = mk2(0.0f, 0.0f);
+  if (NQ == 2)
+    for (; e + 2 * VR <= e1; e += 2 * VR) gather_round_vec<RS, NQ, 2 * VR>(get, e, ringw, cur4, thr4, curW4, acc);
+  for (; e < e1; e += VR) gather_round_vec<RS, NQ, VR>(get, e, ringw, cur4, thr4, curW4, acc);
+}
+__device__ __forceinline__ float acc_slot(const f2* acc, int t) { return (t & 1) ? acc[t >> 1].y : acc[t >> 1].x; }
 
 // S2 + S3 of one (simulation, region) node: the inputs of Eq. (5) (A5, A6, A10), both transfer functions with first
 // and second derivatives (tf_closed2), Eqs. (1)-(3) (A7, A9, A22) and the forward-Euler update of
@@ -354,13 +335,14 @@ __global__ void __launch_bounds__(MAXT, 1) integrate2_kernel(const __grid_consta
   const GroupDesc gd = P.groups[g];
   const TableDesc td = P.tables[gd.table];
   const int Hp = td.Hp, Hs = td.Hs, CH = td.CH, LAG = td.LAG;
-  // shared memory: NBAR mbarriers | [GC][T] coupling sums | [GC][T] normals (private column per thread) |
+  // shared memory: NBAR mbarriers | [GC][T] coupling sums (VEC: [2 GC][T]) | [GC][T] normals (private column per thread) |
   // [NP2][SPC] packed per-sim parameters | edge table + row pointers (SMEMTAB)
   uint64_t* bar_done = reinterpret_cast<uint64_t*>(smem_raw);
   float* const s_cpl = reinterpret_cast<float*>(smem_raw + NBAR * 8) + tid;
-  float* const s_xi = s_cpl + (size_t)GC * T;     // GCE == 8: the normals of the chunk's steps; GCE < 8: rows 0..3 = the current Philox quad
+  constexpr int CPLROWS = VEC ? 2 * GC : GC;      // (VEC: two 8-step blocks of coupling sums, see SHIFTED WINDOWS)
+  float* const s_xi = s_cpl + (size_t)CPLROWS * T;  // GCE == 8: the normals of the chunk's steps; GCE < 8: rows 0..3 = the current Philox quad
   float* const s_quad = s_xi;
-  float2* s_ps = reinterpret_cast<float2*>(reinterpret_cast<float*>(smem_raw + NBAR * 8) + (size_t)2 * GC * T);
+  float2* s_ps = reinterpret_cast<float2*>(reinterpret_cast<float*>(smem_raw + NBAR * 8) + (size_t)(CPLROWS + GC) * T);
   unsigned char* tab = reinterpret_cast<unsigned char*>(s_ps + NP2 * SPC);
   tab += (16 - (reinterpret_cast<uintptr_t>(tab) & 15)) & 15;
   // the CTA's part of the delay table: all of it, or (CLU) the rows of its regions; edge indices below are relative
@@ -449,58 +431,85 @@ __global__ void __launch_bounds__(MAXT, 1) integrate2_kernel(const __grid_consta
     if (SMEMTAB) gather_rounds<RS, GCE, RING_CG>(s_edges, e, pe1, e_last, ringg, cur0, Hp, acc);
     else gather_rounds<RS, GCE, RING_CG>(g_edges, e, pe1, e_last, ringg, cur0, Hp, acc);
   };
-  // VEC: the row's alignment classes; one class after the other, all edges of the row, for the chunk at slot cur0
-  int4 segk = make_int4(0, 0, 0, 0);
+  // VEC: the row's seven segments (class 0 | classes 1-3 shifted | classes 1-3 near), ends relative to the staged part
+  int seg[7] = {0, 0, 0, 0, 0, 0, 0};
   if (VEC) {
-    segk = *reinterpret_cast<const int4*>(P.seg + td.seg_off + 4 * k);
-    segk.x -= rp0; segk.y -= rp0; segk.z -= rp0; segk.w -= rp0;
+    const int4 sa = *reinterpret_cast<const int4*>(P.seg + td.seg_off + 8 * k), sb = *reinterpret_cast<const int4*>(P.seg + td.seg_off + 8 * k + 4);
+    seg[0] = sa.x - rp0; seg[1] = sa.y - rp0; seg[2] = sa.z - rp0; seg[3] = sa.w - rp0;
+    seg[4] = sb.x - rp0; seg[5] = sb.y - rp0; seg[6] = sb.z - rp0;
   }
-  auto gather_vec = [&](int cur0) {                // cur0 a multiple of 4
-    float cpl[GC];
+  // the two rows of coupling sums of a VEC thread: block parity pb (0 / 1) -> row pb, 8 slots each, column stride T
+  auto cpl_slot = [&](int pb, int j) -> float* { return s_cpl + (size_t)(pb * GC + j) * T; };
+  // VEC: the gather for the 8-step block that starts at ring slot cur0 (a multiple of 4) and has parity pb1; completes
+  // that block's sums and leaves the partial sums of the first three slots of the block after it (see SHIFTED WINDOWS)
+  auto gather_vec = [&](int cur0, int pb1) {
+    float cA[GC], cB[3] = {0.0f, 0.0f, 0.0f};
 #pragma unroll
-    for (int j = 0; j < GC; ++j) cpl[j] = 0.0f;
-    const uint32_t thr = (uint32_t)(Hp - cur0), curRS = (uint32_t)cur0 * (uint32_t)RS, wrapRS = (uint32_t)Hp * (uint32_t)RS;
-    if (SMEMTAB) {
-      const VecLd::word* const ring4 = reinterpret_cast<const VecLd::word*>(ringg);
-      const uint32_t cur4 = (uint32_t)cur0 >> VWS, thr4 = thr >> VWS, curW4 = cur4 - ((uint32_t)Hp >> VWS);
-      gather_class_vec8<RS, 0>(s_edges8, pe0, segk.x, ring4, cur4, thr4, curW4, cpl);
-      gather_class_vec8<RS, 1>(s_edges8, segk.x, segk.y, ring4, cur4, thr4, curW4, cpl);
-      gather_class_vec8<RS, 2>(s_edges8, segk.y, segk.z, ring4, cur4, thr4, curW4, cpl);
-      gather_class_vec8<RS, 3>(s_edges8, segk.z, segk.w, ring4, cur4, thr4, curW4, cpl);
-    } else {
-      gather_class_vec<RS, 0>(g_edges, pe0, segk.x, ringg, curRS, thr, wrapRS, cpl);
-      gather_class_vec<RS, 1>(g_edges, segk.x, segk.y, ringg, curRS, thr, wrapRS, cpl);
-      gather_class_vec<RS, 2>(g_edges, segk.y, segk.z, ringg, curRS, thr, wrapRS, cpl);
-      gather_class_vec<RS, 3>(g_edges, segk.z, segk.w, ringg, curRS, thr, wrapRS, cpl);
+    for (int j = 0; j < GC; ++j) cA[j] = j < 3 ? *cpl_slot(pb1, j) : 0.0f;
+    const VecLd::word* const ring4 = reinterpret_cast<const VecLd::word*>(ringg);
+    const uint32_t thr4 = (uint32_t)(Hp - cur0) >> VWS, cur4 = (uint32_t)cur0 >> VWS, curW4 = cur4 - ((uint32_t)Hp >> VWS);
+    const uint32_t qdiv = VW * (uint32_t)RS;
+    auto get = [&](int e) -> Edge8 { return SMEMTAB ? s_edges8[e] : edge8_of(g_edges[e], qdiv); };
+    f2 acc[6];
+    gather_seg_vec<RS, 2>(get, pe0, seg[0], ring4, cur4, thr4, curW4, acc);          // class 0: aligned
+#pragma unroll
+    for (int t = 0; t < 8; ++t) cA[t] += acc_slot(acc, t);
+    gather_seg_vec<RS, 2>(get, seg[0], seg[1], ring4, cur4, thr4, curW4, acc);       // class 1, shifted by 3
+#pragma unroll
+    for (int t = 0; t < 8; ++t) { if (t + 3 < 8) cA[t + 3] += acc_slot(acc, t); else cB[t - 5] += acc_slot(acc, t); }
+    gather_seg_vec<RS, 2>(get, seg[1], seg[2], ring4, cur4, thr4, curW4, acc);       // class 2, shifted by 2
+#pragma unroll
+    for (int t = 0; t < 8; ++t) { if (t + 2 < 8) cA[t + 2] += acc_slot(acc, t); else cB[t - 6] += acc_slot(acc, t); }
+    gather_seg_vec<RS, 2>(get, seg[2], seg[3], ring4, cur4, thr4, curW4, acc);       // class 3, shifted by 1
+#pragma unroll
+    for (int t = 0; t < 8; ++t) { if (t + 1 < 8) cA[t + 1] += acc_slot(acc, t); else cB[t - 7] += acc_slot(acc, t); }
+    if (seg[6] > seg[3]) {                                                             // near edges: unshifted, three quads
+      gather_seg_vec<RS, 3>(get, seg[3], seg[4], ring4, cur4, thr4, curW4, acc);
+#pragma unroll
+      for (int j = 0; j < GC; ++j) cA[j] += acc_slot(acc, 1 + j);
+      gather_seg_vec<RS, 3>(get, seg[4], seg[5], ring4, cur4, thr4, curW4, acc);
+#pragma unroll
+      for (int j = 0; j < GC; ++j) cA[j] += acc_slot(acc, 2 + j);
+      gather_seg_vec<RS, 3>(get, seg[5], seg[6], ring4, cur4, thr4, curW4, acc);
+#pragma unroll
+      for (int j = 0; j < GC; ++j) cA[j] += acc_slot(acc, 3 + j);
     }
 #pragma unroll
-    for (int j = 0; j < GC; ++j) s_cpl[j * T] = cpl[j];
+    for (int j = 0; j < GC; ++j) *cpl_slot(pb1, j) = cA[j];
+#pragma unroll
+    for (int j = 0; j < 3; ++j) *cpl_slot(pb1 ^ 1, j) = cB[j];
   };
-  auto gather_head_vec = [&](int cur0) {           // any alignment (first chunk of a launch): scalar loads, same association
-    float cpl[GC];
-#pragma unroll
-    for (int j = 0; j < GC; ++j) cpl[j] = 0.0f;
-    const int ends[4] = {segk.x, segk.y, segk.z, segk.w};
-    int e = pe0;
-    for (int a = 0; a < 4; ++a) {
-      float acc8[GC];
-#pragma unroll
-      for (int j = 0; j < GC; ++j) acc8[j] = 0.0f;
-      for (; e < ends[a]; ++e) {
+  // VEC, first chunk of a launch (starts at step n0 anywhere inside its 8-step block): the same sums with scalar loads
+  // in the same association -- the block's slots from position n0 mod 8 on, and the partial sums of the next block
+  auto gather_head_vec = [&](int cur0, int64_t n0) {
+    const int o = (int)(n0 & 7), pb = (int)((n0 >> 3) & 1);
+    int cb = cur0 - o; if (cb < 0) cb += Hp;                 // ring slot of the block's first step
+    int cb2 = cb + GC; if (cb2 >= Hp) cb2 -= Hp;             // ... of the next block's
+    // one segment's sum for block position j: edges in order, one FMA chain from zero; sh = the shift the table entry carries
+    auto seg_sum = [&](int e0, int e1, int sh, int cbs, int j) -> float {
+      float a = 0.0f;
+      for (int e = e0; e < e1; ++e) {
         const Edge<float> ed = g_edges[e];
-        uint32_t s0 = (uint32_t)cur0 + ed.back;
-        if (s0 >= (uint32_t)Hp) s0 -= (uint32_t)Hp;
-#pragma unroll
-        for (int j = 0; j < GC; ++j) {
-          const uint32_t sj = s0 + (uint32_t)j;
-          acc8[j] = __fmaf_rn(ed.w, __ldcg(ringg + ed.jbase + (sj & ~(VW - 1u)) * (uint32_t)RS + (sj & (VW - 1u))), acc8[j]);
-        }
+        uint32_t sj = (uint32_t)cbs + (ed.back - (uint32_t)sh) + (uint32_t)j;
+        while (sj >= (uint32_t)Hp) sj -= (uint32_t)Hp;
+        a = __fmaf_rn(ed.w, __ldcg(ringg + ed.jbase + (sj & ~(VW - 1u)) * (uint32_t)RS + (sj & (VW - 1u))), a);
       }
-#pragma unroll
-      for (int j = 0; j < GC; ++j) cpl[j] += acc8[j];
+      return a;
+    };
+    const int sb[5] = {pe0, seg[0], seg[1], seg[2], seg[3]};      // segment c = [sb[c], sb[c + 1]): class c, shift (4 - c) mod 4
+    for (int j = o; j < GC; ++j) {
+      float v = 0.0f;
+      for (int c = 1; c < 4; ++c) if (4 - c > j) v += seg_sum(sb[c], sb[c + 1], 4 - c, cb, j);        // previous gather's part
+      v += seg_sum(sb[0], sb[1], 0, cb, j);
+      for (int c = 1; c < 4; ++c) if (4 - c <= j) v += seg_sum(sb[c], sb[c + 1], 4 - c, cb, j);
+      for (int c = 0; c < 3; ++c) v += seg_sum(seg[3 + c], seg[4 + c], 0, cb, j);                      // near classes 1, 2, 3
+      *cpl_slot(pb, j) = v;
     }
-#pragma unroll
-    for (int j = 0; j < GC; ++j) s_cpl[j * T] = cpl[j];
+    for (int j = 0; j < 3; ++j) {
+      float v = 0.0f;
+      for (int c = 1; c < 4; ++c) if (4 - c > j) v += seg_sum(sb[c], sb[c + 1], 4 - c, cb2, j);
+      *cpl_slot(pb ^ 1, j) = v;
+    }
   };
   // GCE == 1 (one-step chunks; the host mirrors EVERY slot of these rings, Hs = 2 Hp, and pads every row to whole rounds
   // of 4 edges with zero weights): the coupling sum of the step whose time index sits in ring slot cur0, straight from
@@ -521,7 +530,7 @@ __global__ void __launch_bounds__(MAXT, 1) integrate2_kernel(const __grid_consta
     if (GCE == 1) {
       s_cpl[0] = gather_short(cur0);      // (not used: the one-step form gathers inside its step loop)
     } else if (VEC) {
-      gather_head_vec(cur0);
+      gather_head_vec(cur0, n);
     } else {
       f2 acc[GC / 2];
 #pragma unroll
@@ -593,11 +602,12 @@ __global__ void __launch_bounds__(MAXT, 1) integrate2_kernel(const __grid_consta
     float* const traj0 = traj_on ? P.traj + (((size_t)loc * P.traj_steps + (size_t)t_rel) * 7) * N + k : nullptr;
     const int keep_from = (int)max((int64_t)-1, min(P.discard_steps - n, (int64_t)GC));  // windows ending at step i are kept iff i >= keep_from
     const uint32_t n_lo = (uint32_t)n;
+    const int cpl_row0 = VEC ? (int)(((n >> 3) & 1) * GC + (n & 7)) : 0;      // VEC: the block's row, from the chunk's position in it
 #pragma unroll 2      // two steps per trip: the address arithmetic and parameter loads of step i + 1 overlap the
                       // arithmetic of step i and the rematerialised per-thread constants are shared (cfg 2 +2.8 %; 4 is slower)
     for (int i = 0; i < ch; ++i) {
       if (GCE == 1 && m + (uint32_t)i >= (uint32_t)LAG) wait_chunk(m + (uint32_t)i - (uint32_t)LAG);
-      const float cpl = GCE == 1 ? gather_short(c) : s_cpl[i * T];
+      const float cpl = GCE == 1 ? gather_short(c) : s_cpl[(cpl_row0 + i) * T];
       // ---- S1 for the next chunk: issue the loads of the next PVN / GCE edges now, add them below ----
       float pv[PV];
       if (VEC || GCE == 1) {}
@@ -652,7 +662,7 @@ __global__ void __launch_bounds__(MAXT, 1) integrate2_kernel(const __grid_consta
       }
     }
     if (pipe && VEC) {      // the whole row for chunk m + 1 with vector loads
-      gather_vec(cur1);
+      gather_vec(cur1, (int)(((n + ch) >> 3) & 1));
       if (noise) normals_now(n + ch, (int)min((int64_t)CH, P.n_end - (n + ch)));
     } else if (pipe) {      // the row's remaining edges (long rows, short chunks), then chunk m + 1 replaces chunk m
       gather_from(pe0 + (PV / GCE) * ch, cur1, pacc);   // (the registers of the transfer function are free here)
