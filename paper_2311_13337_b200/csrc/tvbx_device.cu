@@ -162,13 +162,22 @@ struct DeviceImpl : DeviceSide {
           seg.push_back(0);      // (8 ints per row: two 16-byte loads)
           continue;
         }
-        for (int e = r0; e < r1 || (e - r0) % pad_to != 0; ++e) {
-          const int es = e < r1 ? e : r0;
+        // packed kernel: every row has at least kRowMin entries, so the pipelined batches of a chunk (PVN / GCE edges per
+        // step) index the table without a clamp and add without a row-end test (tvbx_integrate2.cuh, PADDED)
+        // -- and an ODD number of 16-byte entries: rows of equal even length would put the rows that the lanes of a warp
+        // read at the same step into the same shared-memory banks (cfg 1, one region per lane: 32-way conflicts, -9 %).
+        const int min_len = sw->packed && !short1 ? kRowMin : 0;
+        for (int e = r0; e < r1 || (e - r0) % pad_to != 0 || e - r0 < min_len || (min_len > 0 && (e - r0) % 2 == 0); ++e) {
           Edge<R> ed;
           std::memset(&ed, 0, sizeof ed);
-          ed.w = e < r1 ? (R)c.edges[es].w : R(0);
-          ed.jbase = (uint32_t)c.edges[es].j * (uint32_t)Hs * (uint32_t)RS;
-          ed.back = (uint32_t)(ht.Hp - ht.delays[es]);
+          if (r1 > r0) {      // zero-weight copies of the row's first edge behind its last one
+            const int es = e < r1 ? e : r0;
+            ed.w = e < r1 ? (R)c.edges[es].w : R(0);
+            ed.jbase = (uint32_t)c.edges[es].j * (uint32_t)Hs * (uint32_t)RS;
+            ed.back = (uint32_t)(ht.Hp - ht.delays[es]);
+          } else {            // a region without afferents: region 0, one slot back
+            ed.back = 1u;
+          }
           set_pad(ed, ed.jbase + ed.back * (uint32_t)RS);
           edges.push_back(ed);
         }

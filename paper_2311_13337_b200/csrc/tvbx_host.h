@@ -34,6 +34,9 @@ const char* last_error();
 
 // steps per gather chunk of the integrators (= mirror slots + 1), chunks a warp may run ahead (tvbx_integrate*.cuh)
 constexpr int kGC = 8, kLagMax = 4;
+// rows of a packed-kernel delay table are padded with zero-weight entries to at least this many (= PVN of
+// tvbx_integrate2.cuh: the edges a thread gathers software-pipelined across the steps of one chunk)
+constexpr int kRowMin = 24;
 // largest N the tensor-core FC serves (tvbx_fc_tc.cuh TC_MAXN: the staged tile must fit 227 KB of shared memory)
 constexpr int kTcMaxN = 384;
 

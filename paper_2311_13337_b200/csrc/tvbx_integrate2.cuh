@@ -42,7 +42,8 @@ enum { K2_MAXT = 480 };          // threads per CTA: 65536 / 480 -> 128 register
 enum { K2_SMALLT = 224 };        // small CTAs: launch bound 224 -> 255 registers per thread
 enum { PVN = 24 };               // ring values of the next chunk a thread keeps in flight across one compute step:
                                  // PVN / GCE edges x the first GCE = 8, 4 or 2 slots (GCE >= the chunk length).  Rows up to
-                                 // (PVN / GCE) * CH edges are fully pipelined; longer rows finish in rounds of 8 edges
+                                 // (PVN / GCE) * CH edges are fully pipelined; longer rows finish in rounds of 8 edges.
+                                 // The host pads every row of a packed-kernel table to >= PVN entries (tvbx_host.h kRowMin).
 
 struct Integrate2Params {
   TF2Const tf;
@@ -148,15 +149,17 @@ __device__ __forceinline__ float ring_ld(const float* p) { return CG ? __ldcg(p)
 // uses) -- it then reads other valid ring entries (the table index is clamped to e_last, rows are GC-1 mirror
 // slots longer than the period) whose weight gather_add sets to zero.  The caller adds them with gather_add --
 // later, when it wants the latency hidden.
-template <int RS, int EBT, int GCE, bool CG, typename EdgePtr>
+// PADDED: the caller knows that the entries [e, e + EBT) exist (the pipelined batches of a chunk: the host pads every
+// row of a packed-kernel table to >= K2_ROWMIN = 3 GC entries with zero weights), so the index needs no clamp.
+template <int RS, int EBT, int GCE, bool CG, bool PADDED = false, typename EdgePtr>
 __device__ __forceinline__ void gather_issue(EdgePtr edges, int e, int e_last, const float* ringg, int cur, int Hp, float* v) {
   // slot of the first read = (cur + back) mod Hp with back = Hp - d in [0, Hp]: wraps iff back >= Hp - cur.
   // The table stores pad = jbase + back * RS, so the element offset is pad + cur * RS - (wrap ? Hp * RS : 0).
-  const uint32_t thr = (uint32_t)(Hp - cur), curRS = (uint32_t)cur * (uint32_t)RS, wrapRS = (uint32_t)Hp * (uint32_t)RS;
+  const uint32_t thr = (uint32_t)(Hp - cur), curRS = (uint32_t)cur * (uint32_t)RS, curRSw = curRS - (uint32_t)Hp * (uint32_t)RS;
 #pragma unroll
   for (int b = 0; b < EBT; ++b) {
-    const Edge<float> ed = edges[min(e + b, e_last)];
-    const uint32_t off = ed.pad + curRS - (ed.back >= thr ? wrapRS : 0u);
+    const Edge<float> ed = edges[PADDED ? e + b : min(e + b, e_last)];
+    const uint32_t off = ed.pad + (ed.back >= thr ? curRSw : curRS);      // (one select between two uniform values)
     const float* src = ringg + off;
 #pragma unroll
     for (int j = 0; j < GCE; ++j) v[b * GCE + j] = ring_ld<CG>(src + j * RS);
@@ -164,11 +167,12 @@ __device__ __forceinline__ void gather_issue(EdgePtr edges, int e, int e_last, c
 }
 // acc[j] += w * (E(slot 2j), E(slot 2j+1)), j < GCE/2: the row's edges are added in ascending order into each
 // slot, so a simulation's coupling sum does not depend on which other simulations share its CTA
-template <int EBT, int GCE, typename EdgePtr>
+// (PADDED: entries past the row's last edge carry zero weights themselves -- no test)
+template <int EBT, int GCE, bool PADDED = false, typename EdgePtr>
 __device__ __forceinline__ void gather_add(EdgePtr edges, int e, int e1, bool enable, const float* v, f2 acc[GC / 2]) {
 #pragma unroll
   for (int b = 0; b < EBT; ++b) {
-    const float w = (enable && e + b < e1) ? edges[e + b].w : 0.0f;
+    const float w = PADDED ? edges[e + b].w : ((enable && e + b < e1) ? edges[e + b].w : 0.0f);
 #pragma unroll
     for (int j = 0; j < GCE / 2; ++j) acc[j] = fma2(bc2(w), mk2(v[b * GCE + 2 * j], v[b * GCE + 2 * j + 1]), acc[j]);
   }
@@ -343,8 +347,9 @@ __global__ void __launch_bounds__(MAXT, 1) integrate2_kernel(const __grid_consta
   float* const s_xi = s_cpl + (size_t)CPLROWS * T;  // GCE == 8: the normals of the chunk's steps; GCE < 8: rows 0..3 = the current Philox quad
   float* const s_quad = s_xi;
   float2* s_ps = reinterpret_cast<float2*>(reinterpret_cast<float*>(smem_raw + NBAR * 8) + (size_t)(CPLROWS + GC) * T);
-  unsigned char* tab = reinterpret_cast<unsigned char*>(s_ps + NP2 * SPC);
-  tab += (16 - (reinterpret_cast<uintptr_t>(tab) & 15)) & 15;
+  // (16-byte aligned by construction: smem_raw is, 64 bytes of barriers, columns of 4 T bytes in multiples of 16 rows, and
+  // the parameter block rounded up -- a run-time alignment of the pointer costs a dozen uniform instructions per step)
+  unsigned char* const tab = smem_raw + NBAR * 8 + (size_t)(CPLROWS + GC) * T * sizeof(float) + ((NP2 * SPC * sizeof(float2) + 15) & ~(size_t)15);
   // the CTA's part of the delay table: all of it, or (CLU) the rows of its regions; edge indices below are relative
   // to rp0.  (Every table ends with one zero-weight entry that no row owns: a part is never empty.)
   const int32_t* const g_rowptr = P.rowptr + td.rowptr_off;
@@ -400,7 +405,17 @@ __global__ void __launch_bounds__(MAXT, 1) integrate2_kernel(const __grid_consta
   const int node = active ? tid : NODES - 1;
   const int kl = node / SPC, sl = node - kl * SPC, k = k0 + kl;
   s_ps += sl;
-  float* const ringg = (SRING ? s_ring : P.ring + gd.ring_off) + (VEC ? (int)VW * sl : sl);   // this group's ring, the thread's simulation column
+  // the shared-memory address of the lane's parameter column, made opaque so that it stays in ONE register: left to
+  // itself the compiler re-derives it every step from tid, N and SPC (7 instructions) to stay under the register bound
+  uint32_t ps_a = (uint32_t)__cvta_generic_to_shared(s_ps);
+  asm volatile("" : "+r"(ps_a));
+  float* ringg = (SRING ? s_ring : P.ring + gd.ring_off) + (VEC ? (int)VW * sl : sl);   // this group's ring, the thread's simulation column
+  // (global ring: the pointer is made opaque so that it lives in one register pair and an access is base + 4 * offset;
+  // otherwise the compiler keeps the 64-bit element offset and re-adds it to the uniform base at every access)
+  if (!SRING && !CLU) {
+    asm volatile("" : "+l"(ringg));
+    __builtin_assume(__isGlobal(ringg));          // (still LDG / STG, not generic LD / ST)
+  }
   const int e_last = n_stage - 1;
   const uint32_t myrow = (uint32_t)(k * Hs) * (uint32_t)RS;
   const int loc = P.loc_id[(size_t)g * SPC + sl];
@@ -545,6 +560,15 @@ __global__ void __launch_bounds__(MAXT, 1) integrate2_kernel(const __grid_consta
   // Short chunks (GCE < 8, small minimum delay): the quad lives in s_quad and is redrawn every 4th step.
   auto normals_now = [&](int64_t n0, int ch0) {
     float xi[4] = {0.f, 0.f, 0.f, 0.f};
+    if (ch0 == GC && (n0 & 3) == 0) {       // the usual case, a whole chunk on a quad boundary: two Philox calls, eight plain stores
+#pragma unroll
+      for (int h = 0; h < GC / 4; ++h) {
+        normals4<float>(P.seed, ext, (uint32_t)k, ((uint64_t)n0 >> 2) + (uint64_t)h, xi);
+#pragma unroll
+        for (int q = 0; q < 4; ++q) s_xi[(4 * h + q) * T] = xi[q];
+      }
+      return;
+    }
     for (int i = 0; i < ch0; ++i) {
       const uint64_t nn = (uint64_t)(n0 + i);
       if (i == 0 || (nn & 3) == 0) normals4<float>(P.seed, ext, (uint32_t)k, nn >> 2, xi);
@@ -571,7 +595,12 @@ __global__ void __launch_bounds__(MAXT, 1) integrate2_kernel(const __grid_consta
   f2 ps_reg[NP2];
 #pragma unroll
   for (int q = 0; q < NP2; ++q) ps_reg[q] = PREG ? s_ps[q * SPC] : mk2(0.0f, 0.0f);
-  auto par = [&](int q) -> f2 { return PREG ? ps_reg[q] : s_ps[q * SPC]; };
+  auto par = [&](int q) -> f2 {
+    if (PREG) return ps_reg[q];
+    f2 v;
+    asm("ld.shared.v2.f32 {%0, %1}, [%2];" : "=f"(v.x), "=f"(v.y) : "r"(ps_a + (uint32_t)(q * SPC * 8)));
+    return v;
+  };
   auto wait_chunk = [&](uint32_t w) {              // all warps of the group have written chunk w
     if (CLU) mbar_wait_cluster(bar_done + (w & (NBAR - 1)), (w / NBAR) & 1u);
     else mbar_wait(bar_done + (w & (NBAR - 1)), (w / NBAR) & 1u);
@@ -597,27 +626,32 @@ __global__ void __launch_bounds__(MAXT, 1) integrate2_kernel(const __grid_consta
     for (int j = 0; j < GC / 2; ++j) pacc[j] = mk2(0.0f, 0.0f);
     // step bookkeeping relative to the chunk start, in 32 bits (the 64-bit global step index n stays outside the step loop)
     const int64_t t_rel = n - P.traj_n0;                                             // trajectory row of the chunk's first step
-    const bool traj_on = P.traj != nullptr && loc >= 0 && active && t_rel < P.traj_steps;
+    const bool traj_any = P.traj != nullptr && t_rel < P.traj_steps;                 // (uniform: one branch around the per-lane test)
+    const bool traj_on = traj_any && loc >= 0 && active;
     const int traj_left = traj_on ? (int)min(P.traj_steps - t_rel, (int64_t)GC) : 0;     // steps of this chunk that are recorded
     float* const traj0 = traj_on ? P.traj + (((size_t)loc * P.traj_steps + (size_t)t_rel) * 7) * N + k : nullptr;
     const int keep_from = (int)max((int64_t)-1, min(P.discard_steps - n, (int64_t)GC));  // windows ending at step i are kept iff i >= keep_from
     const uint32_t n_lo = (uint32_t)n;
     const int cpl_row0 = VEC ? (int)(((n >> 3) & 1) * GC + (n & 7)) : 0;      // VEC: the block's row, from the chunk's position in it
+    const float* cpl_p = s_cpl + cpl_row0 * T;    // running pointers into the thread's private columns (one add per step
+    const float* xi_p = s_xi;                     // instead of the row index times the runtime column stride)
 #pragma unroll 2      // two steps per trip: the address arithmetic and parameter loads of step i + 1 overlap the
                       // arithmetic of step i and the rematerialised per-thread constants are shared (cfg 2 +2.8 %; 4 is slower)
     for (int i = 0; i < ch; ++i) {
       if (GCE == 1 && m + (uint32_t)i >= (uint32_t)LAG) wait_chunk(m + (uint32_t)i - (uint32_t)LAG);
-      const float cpl = GCE == 1 ? gather_short(c) : s_cpl[(cpl_row0 + i) * T];
+      const float cpl = GCE == 1 ? gather_short(c) : *cpl_p;
+      cpl_p += T;
       // ---- S1 for the next chunk: issue the loads of the next PVN / GCE edges now, add them below ----
       float pv[PV];
       if (VEC || GCE == 1) {}
-      else if (SMEMTAB) gather_issue<RS, PV / GCE, GCE, RING_CG>(s_edges, pe0 + (PV / GCE) * i, e_last, ringg, cur1, Hp, pv);   // (a table has >= 1 entry)
-      else gather_issue<RS, PV / GCE, GCE, RING_CG>(g_edges, pe0 + (PV / GCE) * i, e_last, ringg, cur1, Hp, pv);
+      else if (SMEMTAB) gather_issue<RS, PV / GCE, GCE, RING_CG, true>(s_edges, pe0 + (PV / GCE) * i, e_last, ringg, cur1, Hp, pv);   // (a table has >= 1 entry)
+      else gather_issue<RS, PV / GCE, GCE, RING_CG, true>(g_edges, pe0 + (PV / GCE) * i, e_last, ringg, cur1, Hp, pv);
       // ---- S2 + S3: inputs, both transfer functions with derivatives, Eqs. (1)-(3), forward Euler ----
       node_step2(P, par, cpl, noise, dt, invN, nu, Cs, W, Cei, ou);
       // ---- S4 OU (Eq. 4, A11) ----
       if (GCE == 8) {
-        if (noise) ou = __fmaf_rn(P.ou_rho, ou, __fmaf_rn(P.ou_s, s_xi[i * T], P.ou_m));
+        if (noise) ou = __fmaf_rn(P.ou_rho, ou, __fmaf_rn(P.ou_s, *xi_p, P.ou_m));
+        xi_p += T;
       } else if (noise) {
         if (((n_lo + (uint32_t)i) & 3u) == 0) {   // a new quad of normals
           float xi[4];
@@ -629,8 +663,8 @@ __global__ void __launch_bounds__(MAXT, 1) integrate2_kernel(const __grid_consta
       }
       // ---- S1 for the next chunk: the loads issued above have had the whole step to arrive ----
       if (VEC || GCE == 1) {}
-      else if (SMEMTAB) gather_add<PV / GCE, GCE>(s_edges, pe0 + (PV / GCE) * i, pe1, pipe, pv, pacc);
-      else gather_add<PV / GCE, GCE>(g_edges, pe0 + (PV / GCE) * i, pe1, pipe, pv, pacc);
+      else if (SMEMTAB) gather_add<PV / GCE, GCE, true>(s_edges, pe0 + (PV / GCE) * i, pe1, pipe, pv, pacc);
+      else gather_add<PV / GCE, GCE, true>(g_edges, pe0 + (PV / GCE) * i, pe1, pipe, pv, pacc);
       // ---- S5 ring write: E at time nn+1 (mirror the first GC-1 slots behind the period) ----
       c = c + 1 == Hp ? 0 : c + 1;
       {     // (lanes past the last node replay it: they store the same value to the same address, no predicate needed)
@@ -639,7 +673,7 @@ __global__ void __launch_bounds__(MAXT, 1) integrate2_kernel(const __grid_consta
         if (GCE == 1 || c < (VEC ? GC : GC - 1)) ringg[o + (uint32_t)Hp * (uint32_t)RS] = nu.x;
       }
       // ---- trajectory (tests / cfg 1) ----
-      if (i < traj_left) {
+      if (traj_any && i < traj_left) {
         float* t = traj0 + (size_t)i * 7 * N;
         t[0] = nu.x; t[N] = nu.y; t[2 * N] = Cs.x; t[3 * N] = Cei; t[4 * N] = Cs.y; t[5 * N] = W.x; t[6 * N] = W.y;
       }

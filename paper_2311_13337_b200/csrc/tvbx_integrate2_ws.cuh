@@ -85,7 +85,9 @@ __global__ void __launch_bounds__(K2_WST, 1) integrate2_ws_kernel(const __grid_c
   s_ps += sl;
   float* const ringg = (SRING ? s_ring : P.ring + gd.ring_off) + sl;
   const int e_last = td.n_edges - 1;
-  const int pe0 = s_rowptr[k], pe1 = s_rowptr[k + 1];
+  const int pe0 = s_rowptr[k];
+  int pe1 = s_rowptr[k + 1];
+  while (pe1 > pe0 && s_edges[pe1 - 1].w == 0.0f) --pe1;      // (the row's zero-weight padding, tvbx_host.h kRowMin, is for the pipelined form)
   const uint32_t ext = (uint32_t)P.ext_id[(size_t)g * SPC + sl];
   const int64_t n0 = P.n_begin;
   const int c0 = (int)(n0 % Hp);
