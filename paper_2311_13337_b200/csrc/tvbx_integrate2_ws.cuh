@@ -83,7 +83,11 @@ __global__ void __launch_bounds__(K2_WST, 1) integrate2_ws_kernel(const __grid_c
   const int node = active ? tid : NODES - 1;      // lanes past the last node replay it (same values to the same addresses)
   const int k = node / SPC, sl = node - k * SPC;
   s_ps += sl;
-  float* const ringg = (SRING ? s_ring : P.ring + gd.ring_off) + sl;
+  float* ringg = (SRING ? s_ring : P.ring + gd.ring_off) + sl;
+  if (!SRING) {      // (one register pair, an access is base + 4 * offset: see integrate2_kernel)
+    asm volatile("" : "+l"(ringg));
+    __builtin_assume(__isGlobal(ringg));
+  }
   const int e_last = td.n_edges - 1;
   const int pe0 = s_rowptr[k];
   int pe1 = s_rowptr[k + 1];
@@ -149,18 +153,21 @@ __global__ void __launch_bounds__(K2_WST, 1) integrate2_ws_kernel(const __grid_c
       const int ch = (int)min((int64_t)CH, P.n_end - n);
       const uint32_t b = m & 1u;
       const int64_t t_rel = n - P.traj_n0;
-      const bool traj_on = P.traj != nullptr && loc >= 0 && active && t_rel < P.traj_steps;
+      const bool traj_any = P.traj != nullptr && t_rel < P.traj_steps;             // (uniform: one branch around the per-lane test)
+      const bool traj_on = traj_any && loc >= 0 && active;
       const int traj_left = traj_on ? (int)min(P.traj_steps - t_rel, (int64_t)GC) : 0;
       float* const traj0 = traj_on ? P.traj + (((size_t)loc * P.traj_steps + (size_t)t_rel) * 7) * N + k : nullptr;
       const int keep_from = (int)max((int64_t)-1, min(P.discard_steps - n, (int64_t)GC));
       mbar_wait(bar_full + b, (m >> 1) & 1u);                                      // the pair's producer has filled buffer b
-      const float* const cplb = s_cpl + (size_t)b * GC * TC;
-      const float* const xib = s_xi + (size_t)b * GC * TC;
+      const float* cpl_p = s_cpl + (size_t)b * GC * TC;      // running pointers into the thread's private columns
+      const float* xi_p = s_xi + (size_t)b * GC * TC;
 #pragma unroll 2
       for (int i = 0; i < ch; ++i) {
-        const float cpl = cplb[i * TC];
+        const float cpl = *cpl_p;
+        cpl_p += TC;
         node_step2(P, par, cpl, noise, dt, invN, nu, Cs, W, Cei, ou);
-        if (noise) ou = __fmaf_rn(P.ou_rho, ou, __fmaf_rn(P.ou_s, xib[i * TC], P.ou_m));      // S4 (Eq. 4, A11)
+        if (noise) ou = __fmaf_rn(P.ou_rho, ou, __fmaf_rn(P.ou_s, *xi_p, P.ou_m));      // S4 (Eq. 4, A11)
+        xi_p += TC;
         // S5 ring write: E at the next time index (the first GC - 1 slots are mirrored behind the period)
         c = c + 1 == Hp ? 0 : c + 1;
         {
@@ -168,7 +175,7 @@ __global__ void __launch_bounds__(K2_WST, 1) integrate2_ws_kernel(const __grid_c
           ringg[o] = nu.x;
           if (c < GC - 1) ringg[o + (uint32_t)Hp * (uint32_t)RS] = nu.x;
         }
-        if (i < traj_left) {
+        if (traj_any && i < traj_left) {
           float* t = traj0 + (size_t)i * 7 * N;
           t[0] = nu.x; t[N] = nu.y; t[2 * N] = Cs.x; t[3 * N] = Cei; t[4 * N] = Cs.y; t[5 * N] = W.x; t[6 * N] = W.y;
         }
