@@ -111,7 +111,12 @@ typedef struct tvbx_sweep_opts {
                              latency of one warp's step; a producer warp per consumer warp then takes the delayed gather, the
                              Philox draws and their bookkeeping off that chain and runs on the schedulers' idle issue slots
                              (csrc/tvbx_integrate2_ws.cuh).  Same arithmetic and Philox stream: results are bit-identical.
-                             Applies to one-CTA groups of <= 160 nodes with 8-step chunks (minimum delay >= 15 steps) */
+                             Applies to one-CTA groups of <= 160 nodes with 8-step chunks (minimum delay >= 15 steps).
+                             3 = on, GROUPED: the regions of a group of simulations are split over ctas_per_group CTAs on
+                             different SMs (cooperative launch, chunk hand-over through counters in global memory), so that
+                             every warp scheduler hosts at most ONE consumer warp -- chosen by 0 when the one-CTA mapping would
+                             put two on one scheduler and the whole grid fits the GPU at once (cfg 4: 7 simulations per 4
+                             CTAs).  With 3, sims_per_cta / ctas_per_group = 0 are chosen by the library */
   int32_t reserved0;
   double updown_threshold_khz; /* > 0: also keep the up / down-state episode statistics of the kept 1-ms excitatory samples
                                   (tvbx_state_durations; Tab. 2 P:131 `mean_UD_duration`): a sample is UP iff it exceeds

@@ -199,7 +199,7 @@ int32_t tvbx_sweep_create(const tvbx_connectome* c, const tvbx_model_params* def
   if (sw->precision != TVBX_F32 && sw->precision != TVBX_F64) return fail(TVBX_EINVAL, "precision=%d", sw->precision);
   sw->threads_req = opts ? opts->threads_per_cta : 0;
   sw->ws_req = opts ? opts->latency_form : 0;
-  if (sw->ws_req < 0 || sw->ws_req > 2) return fail(TVBX_EINVAL, "latency_form=%d (valid: 0, 1, 2)", sw->ws_req);
+  if (sw->ws_req < 0 || sw->ws_req > 3) return fail(TVBX_EINVAL, "latency_form=%d (valid: 0 .. 3)", sw->ws_req);
   sw->chunk_req = opts ? opts->chunk_samples : 0;
   {
     sw->stats_i = opts && opts->rate_stats_inhibitory != 0;
@@ -269,6 +269,42 @@ int32_t tvbx_sweep_create(const tvbx_connectome* c, const tvbx_model_params* def
     }
     if (best_thr > 0) spc = want; else clu = 0;
   }
+  // Grouped low-latency form (tvbx_integrate2_ws.cuh, GRP): a consumer warp per scheduler is the unit of that form's speed,
+  // and a one-CTA mapping of a few hundred simulations puts two on one scheduler (cfg 4: 2 x 68 nodes = 5 warps per SM, or
+  // two CTAs of 3).  Splitting the regions of s simulations over c CTAs with <= 128 nodes each leaves one per scheduler if
+  // the c * groups CTAs fit the SMs at once.  Taken by latency_form = 0 when no one-CTA mapping achieves that, and by 3.
+  if (packed_ok && !sw->stats_i && sw->threads_req == 0 &&
+      (sw->ws_req == 3 || (sw->ws_req == 0 && clu == 0 && spc == 0 && getenv("TVBX_NO_WS") == nullptr && getenv("TVBX_NO_WSG") == nullptr))) {
+    const int n_sm = 148;
+    std::map<double, int64_t> per_v;
+    for (int64_t s = 0; s < sw->n_sims; ++s) per_v[sw->param(s, TVBX_P_V)]++;
+    auto n_groups = [&](int s) { int64_t g = 0; for (auto& kv : per_v) g += (kv.second + s - 1) / s; return g; };
+    int best_plain = INT32_MAX;       // consumer warps on the busiest scheduler, best one-CTA mapping
+    for (int s = 1; s <= 8 && sw->conn.n * s <= 160; ++s) {
+      const int64_t ctas = n_groups(s);
+      const int64_t per_sm = (ctas + n_sm - 1) / n_sm;
+      best_plain = (int)std::min<int64_t>(best_plain, (((int64_t)sw->conn.n * s + 31) / 32 * per_sm + 3) / 4);
+    }
+    if (sw->ws_req == 3 || best_plain >= 2) {
+      double best_fill = 0.0;
+      int bc = 0, bs = 0;
+      for (int c = 2; c <= 8; ++c) {
+        if (clu != 0 && c != clu) continue;
+        for (int s = 1; s <= 8; ++s) {
+          if (spc != 0 && s != spc) continue;
+          const int nl = (sw->conn.n + c - 1) / c;
+          if (!clu_valid(c, s) || nl * s > 128) continue;
+          const int64_t ctas = n_groups(s) * c;
+          if (ctas > n_sm) continue;
+          const double fill = (double)sw->n_sims * sw->conn.n / ((double)ctas * 128.0);
+          if (fill > best_fill * 1.0001) { best_fill = fill; bc = c; bs = s; }      // (ties: fewer CTAs per group)
+        }
+      }
+      if (bc > 0) { clu = bc; spc = bs; sw->wsg = true; }
+      else if (sw->ws_req == 3)
+        return fail(TVBX_EINVAL, "latency_form = 3: no split of the regions over 2 .. 8 CTAs with <= 128 nodes each fits %d SMs at once", n_sm);
+    }
+  }
   if (clu == 0) clu = 1;
   if (clu > 1) {
     if (spc == 0) { spc = 8; while (spc > 1 && !clu_valid(clu, spc)) --spc; }
@@ -297,7 +333,10 @@ int32_t tvbx_sweep_create(const tvbx_connectome* c, const tvbx_model_params* def
   if (spc < 1 || spc > 32) return fail(TVBX_EINVAL, "sims_per_cta=%d (valid: 1..32)", spc);
   sw->spc = spc;
   sw->packed = packed_ok && spc <= 8 && ((sw->conn.n + clu - 1) / clu) * spc <= 480 && (sw->threads_req == 0 || sw->threads_req >= sw->conn.n * spc);
-  sw->vec_ok = sw->packed && clu > 1 && (spc == 8 || spc == 4) && getenv("TVBX_NO_VEC") == nullptr;
+  sw->vec_ok = sw->packed && clu > 1 && !sw->wsg && (spc == 8 || spc == 4) && getenv("TVBX_NO_VEC") == nullptr;
+  if (!sw->packed) sw->wsg = false;
+  if (sw->ws_req == 3 && !sw->wsg)
+    return fail(TVBX_EINVAL, "latency_form = 3 needs the packed FP32 kernel (tau_e == tau_i), no threads_per_cta, no inhibitory samples");
   // group the simulations by speed (one delay table per distinct v), then into CTAs of spc lanes
   std::map<double, int32_t> vmap;
   sw->sim_table.resize(sw->n_sims);

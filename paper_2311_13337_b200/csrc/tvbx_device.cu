@@ -61,6 +61,7 @@ struct DeviceImpl : DeviceSide {
   Integrate2Params P2;
   std::vector<Launch2> launches2;
   DevBuf<float2> d_psim2;
+  DevBuf<uint32_t> d_grpcnt;                          // grouped low-latency form: chunk counters [group][NBAR]
   int threads = 0, smem = 0;
   int run_ds = 1;      // temporal-average window of the runs so far (sample spacing of the 1-ms series = run_ds * dt)
   bool single = true;
@@ -359,6 +360,38 @@ struct DeviceImpl : DeviceSide {
     }
     const size_t ws_base = (size_t)NBAR * 8 + (size_t)(threads / 32) * 4 * 8 + (size_t)4 * GC * threads * sizeof(float) +
                            (size_t)NP2 * SPC * sizeof(float2) + 16;
+    // Grouped low-latency form: the mapping was chosen at tvbx_sweep_create (CLU CTAs per group, <= 4 consumer warps per
+    // CTA); it runs if the tables qualify and the whole grid is resident at once, else the cluster form serves the mapping.
+    bool grouped = false;
+    if (sw->wsg && CLU > 1) {
+      int n_sm = 148, coop = 0;
+      cudaDeviceGetAttribute(&n_sm, cudaDevAttrMultiProcessorCount, sw->device);
+      cudaDeviceGetAttribute(&coop, cudaDevAttrCooperativeLaunch, sw->device);
+      bool ok = coop != 0 && !sw->stats_i && !sw->vec_ok && 2 * threads <= k2_ws_max_threads() && ws_base + tbytes <= (size_t)200 * 1024;
+      for (const HostTable& ht : sw->tables) ok = ok && ring_geom(ht.D, ht.dmin, true).CH == GC && !ht.short1 && !ht.vec;
+      if (ok) {
+        const void* fn = (const void*)k2_wsg(SPC);
+        CU(raise_dynamic_smem(fn, (int)(ws_base + tbytes)));
+        int occ = 0;
+        CU(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, fn, 2 * threads, ws_base + tbytes));
+        ok = (int64_t)sw->groups.size() * CLU <= (int64_t)occ * n_sm;
+      }
+      if (sw->ws_req == 3 && !ok)
+        return fail(TVBX_EINVAL, "latency_form = 3 needs <= %d nodes per CTA, 8-step chunks (minimum delay >= 15 steps), no inhibitory samples and a grid that is resident at once",
+                    k2_ws_max_threads() / 2);
+      grouped = ok && getenv("TVBX_NO_WSG") == nullptr;
+      if (grouped) {
+        ws = true;
+        P2.smem_table = 1;
+        P2.grp_ctas = CLU;
+        int arrivals = 0;
+        for (int r = 0; r * NL < N; ++r) arrivals += (std::min(NL, N - r * NL) * SPC + 31) / 32;
+        P2.grp_arrivals = arrivals;
+        CU(d_grpcnt.alloc(sw->groups.size() * NBAR));
+        P2.grp_cnt = d_grpcnt.p;
+      }
+    }
+    sw->grouped = grouped;
     if (ws) smem = (int)(ws_base + tbytes);
     sw->split = ws ? 2 : 1;
     // one launch per run of groups whose chunk length falls in the same class (cfg 3: v <= 8 / 16 / >= 32 m/s)
@@ -378,7 +411,8 @@ struct DeviceImpl : DeviceSide {
       Kernel2Key key;
       key.spc = SPC; key.smemtab = P2.smem_table != 0; key.gce = gce; key.clu = CLU > 1; key.vec = ht.vec != 0; key.sring = sring;
       key.small = !key.vec && !sring && key.smemtab && gce == 8 && threads <= K2_SMALLT;
-      key.isamp = sw->stats_i; key.ws = ws;
+      key.isamp = sw->stats_i; key.ws = ws; key.grp = grouped;
+      if (grouped) { key.clu = false; key.sring = false; key.small = false; }
       Kernel2Fn fn = pick_kernel2(key);
       CU(raise_dynamic_smem((const void*)fn, lsmem));      // (per function, process-wide, raise-only)
       if (!launches2.empty() && launches2.back().fn == fn) {
@@ -516,6 +550,12 @@ struct DeviceImpl : DeviceSide {
         for (const Launch2& l : launches2) {
           P2.group0 = l.g0;
           if (sw->clu == 1) { l.fn<<<l.count, sw->split == 2 ? 2 * threads : threads, l.smem, st>>>(P2); continue; }
+          if (sw->grouped) {     // grouped low-latency form: the CTAs of a group wait on one another -> all resident (cooperative launch)
+            CU(cudaMemsetAsync(d_grpcnt.p, 0, d_grpcnt.bytes, st));
+            void* args[1] = {(void*)&P2};
+            CU(cudaLaunchCooperativeKernel((const void*)l.fn, dim3((unsigned)(l.count * sw->clu)), dim3((unsigned)(2 * threads)), args, (size_t)l.smem, st));
+            continue;
+          }
           cudaLaunchConfig_t lc;
           std::memset(&lc, 0, sizeof lc);
           lc.gridDim = dim3((unsigned)(l.count * sw->clu)); lc.blockDim = dim3((unsigned)threads);

@@ -177,6 +177,8 @@ struct tvbx_sweep {
   bool packed = false;    // FP32 closed-form product kernel (integrate2_kernel)
   int32_t ws_req = 0;     // tvbx_sweep_opts.latency_form: 0 choose, 1 off, 2 on
   int32_t split = 1;      // 2 while the low-latency warp-pair form of the packed kernel runs (f1), else 1
+  bool wsg = false;       // mapping chosen for the GROUPED low-latency form: `clu` CTAs per group, cooperative launch (else the cluster form)
+  bool grouped = false;   // ... and it runs (decided at the first tvbx_run, when the delays are known)
   int64_t chunk_req = 0;
   bool fc_tc = false;     // FC co-moment on the tensor cores (tvbx_fc_tc.cuh)
   double rate_thr = 0.1;  // kHz: samples above it are counted (f4; 100 Hz)

@@ -78,6 +78,10 @@ struct Integrate2Params {
   int64_t traj_n0;
   int32_t smem_table;             // edge table + row pointers staged in shared memory (else read through L1/L2)
   int32_t group0;                 // first group of this launch (groups of one launch share GCE)
+  // grouped low-latency form (tvbx_integrate2_ws.cuh, GRP): CTAs per group, consumer warps per group (= arrivals per
+  // chunk), and the chunk counters [group][NBAR] in global memory (zeroed before every launch)
+  int32_t grp_ctas, grp_arrivals;
+  uint32_t* grp_cnt;
 };
 
 __device__ __forceinline__ uint32_t smem_u32(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }

@@ -25,12 +25,29 @@ namespace tvbx {
 
 enum { K2_WST = 320 };           // threads per CTA of this form (consumers + producers): 65536 / 320 -> 204 registers per thread
 
-template <int SPC, bool SRING>
+// release-add on / acquire-load of a chunk counter in global memory (GRP: the CTAs of a group sit on different SMs)
+__device__ __forceinline__ void grp_arrive(uint32_t* p) {
+  asm volatile("red.release.gpu.global.add.u32 [%0], 1;" ::"l"(p) : "memory");
+}
+__device__ __forceinline__ uint32_t grp_poll(const uint32_t* p) {
+  uint32_t v;
+  asm volatile("ld.acquire.gpu.global.u32 %0, [%1];" : "=r"(v) : "l"(p) : "memory");
+  return v;
+}
+
+template <int SPC, bool SRING, bool GRP = false>
 __global__ void __launch_bounds__(K2_WST, 1) integrate2_ws_kernel(const __grid_constant__ Integrate2Params P) {
+  static_assert(!(GRP && SRING), "a group's ring is shared by its CTAs: global memory");
   extern __shared__ __align__(16) unsigned char smem_raw[];
   constexpr int RS = SPC;
-  const int g = (int)blockIdx.x + P.group0;
+  // GRP: the regions of a group are split over P.grp_ctas CTAs (any SMs; cooperative launch: all resident); CTA r owns the
+  // regions [r NL, (r + 1) NL), NL = ceil(N / grp_ctas)
+  const int GR = GRP ? P.grp_ctas : 1;
+  const int crank = GRP ? (int)blockIdx.x % GR : 0;
+  const int g = (GRP ? (int)blockIdx.x / GR : (int)blockIdx.x) + P.group0;
   const int N = P.N;
+  const int NLr = GRP ? (N + GR - 1) / GR : N;
+  const int k0 = crank * NLr;
   const int T = blockDim.x, TC = T >> 1;                   // consumer threads = producer threads (whole warps)
   const int NW = TC >> 5;                                  // warp pairs
   // Which warp plays which role.  Warp w issues on scheduler w mod 4; a consumer carries ~3x the instructions of a producer.
@@ -41,7 +58,7 @@ __global__ void __launch_bounds__(K2_WST, 1) integrate2_ws_kernel(const __grid_c
   if (NW == 5) { prod = !(w < 4 || w == 6); wp = prod ? (w < 6 ? w - 4 : w - 5) : (w < 4 ? w : 4); }
   else { prod = w >= NW; wp = prod ? w - NW : w; }
   const int tid = wp * 32 + ((int)threadIdx.x & 31);       // node slot: the same for the two warps of a pair
-  const int NODES = N * SPC;
+  const int NODES = min(NLr, N - k0) * SPC;
   const GroupDesc gd = P.groups[g];
   const TableDesc td = P.tables[gd.table];
   const int Hp = td.Hp, Hs = td.Hs, CH = td.CH, LAG = td.LAG;
@@ -81,7 +98,7 @@ __global__ void __launch_bounds__(K2_WST, 1) integrate2_ws_kernel(const __grid_c
   const bool noise = P.noise_on != 0;
   const bool active = tid < NODES;
   const int node = active ? tid : NODES - 1;      // lanes past the last node replay it (same values to the same addresses)
-  const int k = node / SPC, sl = node - k * SPC;
+  const int kl = node / SPC, sl = node - kl * SPC, k = k0 + kl;
   s_ps += sl;
   float* ringg = (SRING ? s_ring : P.ring + gd.ring_off) + sl;
   if (!SRING) {      // (one register pair, an access is base + 4 * offset: see integrate2_kernel)
@@ -93,6 +110,7 @@ __global__ void __launch_bounds__(K2_WST, 1) integrate2_ws_kernel(const __grid_c
   int pe1 = s_rowptr[k + 1];
   while (pe1 > pe0 && s_edges[pe1 - 1].w == 0.0f) --pe1;      // (the row's zero-weight padding, tvbx_host.h kRowMin, is for the pipelined form)
   const uint32_t ext = (uint32_t)P.ext_id[(size_t)g * SPC + sl];
+  uint32_t* const grp_cnt = GRP ? P.grp_cnt + (size_t)g * NBAR : nullptr;
   const int64_t n0 = P.n_begin;
   const int c0 = (int)(n0 % Hp);
 
@@ -103,24 +121,55 @@ __global__ void __launch_bounds__(K2_WST, 1) integrate2_ws_kernel(const __grid_c
     for (uint32_t m = 0; n < P.n_end; ++m) {
       const int ch = (int)min((int64_t)CH, P.n_end - n);
       const uint32_t b = m & 1u;
-      if (m >= 2) mbar_wait(bar_empty + b, ((m >> 1) - 1u) & 1u);                  // the consumer has finished chunk m - 2
-      if (m >= (uint32_t)LAG) { const uint32_t w = m - (uint32_t)LAG; mbar_wait(bar_done + (w & (NBAR - 1)), (w / NBAR) & 1u); }
+      // Gather and draw FIRST, into registers, as soon as the ring holds what chunk m needs -- up to LAG chunks ahead of the
+      // consumer; only the hand-over waits for the buffer.  (Waiting for the buffer first left the producer one chunk-time
+      // for all of it, too little once the ring loads cross to another SM's writes through L2: GRP.)
+      if (m >= (uint32_t)LAG) {                   // every consumer of the group has written chunk m - LAG
+        const uint32_t w = m - (uint32_t)LAG;
+        if (GRP) {      // slot w mod NBAR has then collected grp_arrivals for each of the chunks w, w - NBAR, ... of this launch
+          const uint32_t* const cp = grp_cnt + (w & (NBAR - 1));
+          const uint32_t want = (uint32_t)P.grp_arrivals * (w / NBAR + 1u);
+          while (grp_poll(cp) < want) {}
+        } else {
+          mbar_wait(bar_done + (w & (NBAR - 1)), (w / NBAR) & 1u);
+        }
+      }
       f2 acc[GC / 2];
 #pragma unroll
       for (int j = 0; j < GC / 2; ++j) acc[j] = mk2(0.0f, 0.0f);
-      gather_rounds<RS, GC, false>(s_edges, pe0, pe1, e_last, ringg, c, Hp, acc);   // the row's edges in ascending order
+      gather_rounds<RS, GC, GRP>(s_edges, pe0, pe1, e_last, ringg, c, Hp, acc);     // the row's edges in ascending order (GRP: through L2)
+      float xv[GC];
+#pragma unroll
+      for (int i = 0; i < GC; ++i) xv[i] = 0.0f;
+      if (noise) {                                // A12: one Philox call per (sim, region) per 4 steps
+        float xi[4] = {0.f, 0.f, 0.f, 0.f};
+        if (ch == GC && (n & 3) == 0) {           // a whole chunk on a quad boundary: two calls
+#pragma unroll
+          for (int h = 0; h < GC / 4; ++h) {
+            normals4<float>(P.seed, ext, (uint32_t)k, ((uint64_t)n >> 2) + (uint64_t)h, xi);
+#pragma unroll
+            for (int q = 0; q < 4; ++q) xv[4 * h + q] = xi[q];
+          }
+        } else {
+#pragma unroll
+          for (int i = 0; i < GC; ++i) {
+            if (i < ch) {
+              const uint64_t nn = (uint64_t)(n + i);
+              if (i == 0 || (nn & 3) == 0) normals4<float>(P.seed, ext, (uint32_t)k, nn >> 2, xi);
+              const uint32_t q = (uint32_t)nn & 3u;
+              xv[i] = q == 0 ? xi[0] : (q == 1 ? xi[1] : (q == 2 ? xi[2] : xi[3]));
+            }
+          }
+        }
+      }
+      if (m >= 2) mbar_wait(bar_empty + b, ((m >> 1) - 1u) & 1u);                  // the consumer has finished chunk m - 2
       float* const cpl = s_cpl + (size_t)b * GC * TC;
 #pragma unroll
       for (int j = 0; j < GC / 2; ++j) { cpl[(2 * j) * TC] = acc[j].x; cpl[(2 * j + 1) * TC] = acc[j].y; }
-      if (noise) {                                // A12: one Philox call per (sim, region) per 4 steps
+      if (noise) {
         float* const xo = s_xi + (size_t)b * GC * TC;
-        float xi[4] = {0.f, 0.f, 0.f, 0.f};
-        for (int i = 0; i < ch; ++i) {
-          const uint64_t nn = (uint64_t)(n + i);
-          if (i == 0 || (nn & 3) == 0) normals4<float>(P.seed, ext, (uint32_t)k, nn >> 2, xi);
-          const uint32_t q = (uint32_t)nn & 3u;
-          xo[i * TC] = q == 0 ? xi[0] : (q == 1 ? xi[1] : (q == 2 ? xi[2] : xi[3]));
-        }
+#pragma unroll
+        for (int i = 0; i < GC; ++i) xo[i * TC] = xv[i];
       }
       __syncwarp();
       if ((tid & 31) == 0) mbar_arrive(bar_full + b);
@@ -194,7 +243,8 @@ __global__ void __launch_bounds__(K2_WST, 1) integrate2_ws_kernel(const __grid_c
       }
       __syncwarp();
       if ((tid & 31) == 0) {
-        mbar_arrive(bar_done + (m & (NBAR - 1)));      // chunk m is in the ring
+        if (GRP) grp_arrive(grp_cnt + (m & (NBAR - 1)));      // chunk m is in the ring (release: visible to the other SMs' producers)
+        else mbar_arrive(bar_done + (m & (NBAR - 1)));
         mbar_arrive(bar_empty + b);                    // buffer b may be refilled
       }
       n += ch;

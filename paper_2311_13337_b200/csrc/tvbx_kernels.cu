@@ -2,6 +2,7 @@
 #include "tvbx_kernels.h"
 namespace tvbx {
 Kernel2Fn pick_kernel2(const Kernel2Key& k) {
+  if (k.ws && k.grp) return k2_wsg(k.spc);
   if (k.ws) return k2_ws(k.spc, k.sring);
   if (k.sring && k.gce == 1) return k2_g1(k.spc);
   if (k.sring) return k.gce == 2 ? k2_g2(k.spc, true) : (k.gce == 4 ? k2_g4(k.spc, true) : k2_g8_small_sring(k.spc));

@@ -27,6 +27,7 @@ struct Kernel2Key {
   bool small;       // CTAs of <= K2_SMALLT threads: relaxed register bound
   bool isamp;       // also store the inhibitory 1-ms samples (rate statistics of both populations)
   bool ws;          // low-latency form: producer / consumer warp pairs (tvbx_integrate2_ws.cuh)
+  bool grp;         // ... with the regions of a group split over several CTAs (cooperative launch)
 };
 Kernel2Fn pick_kernel2(const Kernel2Key& k);                              // tvbx_kernels.cu
 // one function per instance family, each in its own translation unit
@@ -40,6 +41,7 @@ Kernel2Fn k2_nosmem(int spc);                      // table through L1/L2, 8 slo
 Kernel2Fn k2_clu(int spc);                         // cluster, scalar gather
 Kernel2Fn k2_clu_small(int spc);                   // cluster, scalar gather, the CTA's rows of the table in shared memory, launch bound K2_SMALLT
 Kernel2Fn k2_ws(int spc, bool sring);               // low-latency warp-pair form (tvbx_integrate2_ws.cuh)
+Kernel2Fn k2_wsg(int spc);                         // the same, grouped: a group's regions over several CTAs (tvbx_k_packed_wsg.cu)
 int k2_ws_max_threads();                            // its launch bound (consumer + producer threads)
 Kernel2Fn k2_vec(int spc, bool smemtab);           // cluster, vector gather (spc 4 or 8)
 

@@ -187,12 +187,39 @@ def test_latency_form_is_bitwise_the_throughput_form(N, n_sims, spc, v):
     assert np.abs(outs[2][2][1] / rme - 1).max() < TOL_MEAN_REL and np.abs(outs[2][2][0] - rfc).max() < TOL_FC_ABS
 
 
+@pytest.mark.parametrize("N,n_sims,spc,clu,v", [(68, 14, 7, 4, 4.0), (68, 9, 3, 2, 4.0), (37, 5, 3, 2, 5.0), (23, 11, 8, 3, 3.0)],
+                         ids=["cfg4_mapping", "n68_3x2", "n37_3x2", "n23_8x3"])
+def test_grouped_latency_form_is_bitwise_the_throughput_form(N, n_sims, spc, clu, v):
+    """latency_form = 3: the regions of a group of simulations split over several CTAs on different SMs (cooperative launch),
+    chunk hand-over through release / acquire counters in global memory, ring loads through L2.  Trajectories, state, FC and
+    means must equal those of the one-warp form BIT FOR BIT across several launches (the counters are re-armed per launch),
+    including a last group with padding lanes and a last CTA with fewer regions."""
+    W, L = (wl.config_connectome(wl.config(1)) if N == 68 else wl.connectome(N, seed=N, keep=0.4))
+    cfg = dict(axes=[dict(name="G", lo=0.0, hi=0.4, n=n_sims, values=None)], fixed=dict(v=v, b_e=30.0, wNoise=1e-4), seed=12)
+    outs = {}
+    for form in (1, 3):
+        kw = dict(sims_per_cta=spc, ctas_per_group=clu) if form == 3 else {}
+        _, sw = tvbx.sweep_from_config(cfg, W, L, latency_form=form, chunk_samples=40, **kw)
+        tr = [sw.run(part, 0.1, noise_on=True, ds=10, discard_steps=100, traj_steps=part) for part in (403, 1, 996)]
+        info = sw.launch_info()
+        if form == 3:
+            assert info["latency_form"] == 2 and info["ctas_per_group"] == clu and info["sims_per_cta"] == spc
+            assert info["ctas"] == clu * ((n_sims + spc - 1) // spc)
+        outs[form] = (np.concatenate(tr, axis=1), sw.state(), sw.fc_readout())
+    np.testing.assert_array_equal(outs[1][0], outs[3][0])
+    for a, b in zip(outs[1][1] + outs[1][2], outs[3][1] + outs[3][2]):
+        np.testing.assert_array_equal(a, b)
+
+
 def test_latency_form_is_chosen_for_small_sweeps_and_refused_where_it_does_not_apply():
     cfg = wl.config(4)
     W, L = wl.config_connectome(cfg)
     _, sw = tvbx.sweep_from_config(cfg, W, L)
     sw.run(10, 0.1, noise_on=True, ds=10)
-    assert sw.launch_info()["latency_form"] == 2        # 256 sims: all CTAs resident, about one warp per scheduler
+    info = sw.launch_info()
+    assert info["latency_form"] == 2                    # 256 sims: all CTAs resident, about one warp per scheduler
+    # ... grouped: 7 simulations per 4 CTAs = 148 CTAs of 4 consumer warps, one per scheduler (the one-CTA mappings put two on one)
+    assert (info["ctas_per_group"], info["sims_per_cta"], info["ctas"], info["threads"]) == (4, 7, 148, 256)
     cfg2 = wl.config(2)
     _, sw2 = tvbx.sweep_from_config(cfg2, W, L)
     sw2.run(10, 0.1, noise_on=True, ds=10)
