@@ -367,13 +367,15 @@ struct DeviceImpl : DeviceSide {
       int n_sm = 148, coop = 0;
       cudaDeviceGetAttribute(&n_sm, cudaDevAttrMultiProcessorCount, sw->device);
       cudaDeviceGetAttribute(&coop, cudaDevAttrCooperativeLaunch, sw->device);
-      bool ok = coop != 0 && !sw->stats_i && !sw->vec_ok && 2 * threads <= k2_ws_max_threads() && ws_base + tbytes <= (size_t)200 * 1024;
+      // (two helper warps behind the warp pairs and NBAR more barriers: tvbx_integrate2_ws.cuh, GRP)
+      const size_t wsg_smem = ws_base + (size_t)NBAR * 8 + tbytes;
+      bool ok = coop != 0 && !sw->stats_i && !sw->vec_ok && 2 * threads + 64 <= k2_ws_max_threads() && wsg_smem <= (size_t)200 * 1024;
       for (const HostTable& ht : sw->tables) ok = ok && ring_geom(ht.D, ht.dmin, true).CH == GC && !ht.short1 && !ht.vec;
       if (ok) {
         const void* fn = (const void*)k2_wsg(SPC);
-        CU(raise_dynamic_smem(fn, (int)(ws_base + tbytes)));
+        CU(raise_dynamic_smem(fn, (int)wsg_smem));
         int occ = 0;
-        CU(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, fn, 2 * threads, ws_base + tbytes));
+        CU(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, fn, 2 * threads + 64, wsg_smem));
         ok = (int64_t)sw->groups.size() * CLU <= (int64_t)occ * n_sm;
       }
       if (sw->ws_req == 3 && !ok)
@@ -384,15 +386,13 @@ struct DeviceImpl : DeviceSide {
         ws = true;
         P2.smem_table = 1;
         P2.grp_ctas = CLU;
-        int arrivals = 0;
-        for (int r = 0; r * NL < N; ++r) arrivals += (std::min(NL, N - r * NL) * SPC + 31) / 32;
-        P2.grp_arrivals = arrivals;
+        P2.grp_arrivals = CLU;      // one publication per CTA and chunk
         CU(d_grpcnt.alloc(sw->groups.size() * NBAR));
         P2.grp_cnt = d_grpcnt.p;
       }
     }
     sw->grouped = grouped;
-    if (ws) smem = (int)(ws_base + tbytes);
+    if (ws) smem = (int)(ws_base + (grouped ? (size_t)NBAR * 8 : 0) + tbytes);
     sw->split = ws ? 2 : 1;
     // one launch per run of groups whose chunk length falls in the same class (cfg 3: v <= 8 / 16 / >= 32 m/s)
     launches2.clear();
@@ -426,7 +426,7 @@ struct DeviceImpl : DeviceSide {
       if (f1.numRegs >= fa.numRegs) fa = f1;
     }
     sw->info[0] = (int32_t)sw->groups.size() * CLU;
-    sw->info[1] = ws ? 2 * threads : threads; sw->info[3] = fa.numRegs; sw->info[4] = smem; sw->info[5] = 1; sw->info[7] = (int32_t)fa.localSizeBytes;
+    sw->info[1] = ws ? 2 * threads + (grouped ? 64 : 0) : threads; sw->info[3] = fa.numRegs; sw->info[4] = smem; sw->info[5] = 1; sw->info[7] = (int32_t)fa.localSizeBytes;
     sw->info[8] = CLU;
     return TVBX_OK;
   }
@@ -553,7 +553,7 @@ struct DeviceImpl : DeviceSide {
           if (sw->grouped) {     // grouped low-latency form: the CTAs of a group wait on one another -> all resident (cooperative launch)
             CU(cudaMemsetAsync(d_grpcnt.p, 0, d_grpcnt.bytes, st));
             void* args[1] = {(void*)&P2};
-            CU(cudaLaunchCooperativeKernel((const void*)l.fn, dim3((unsigned)(l.count * sw->clu)), dim3((unsigned)(2 * threads)), args, (size_t)l.smem, st));
+            CU(cudaLaunchCooperativeKernel((const void*)l.fn, dim3((unsigned)(l.count * sw->clu)), dim3((unsigned)(2 * threads + 64)), args, (size_t)l.smem, st));
             continue;
           }
           cudaLaunchConfig_t lc;

@@ -29,6 +29,11 @@ enum { K2_WST = 320 };           // threads per CTA of this form (consumers + pr
 __device__ __forceinline__ void grp_arrive(uint32_t* p) {
   asm volatile("red.release.gpu.global.add.u32 [%0], 1;" ::"l"(p) : "memory");
 }
+__device__ __forceinline__ uint32_t grp_poll_relaxed(const uint32_t* p) {
+  uint32_t v;
+  asm volatile("ld.relaxed.gpu.global.u32 %0, [%1];" : "=r"(v) : "l"(p) : "memory");
+  return v;
+}
 __device__ __forceinline__ uint32_t grp_poll(const uint32_t* p) {
   uint32_t v;
   asm volatile("ld.acquire.gpu.global.u32 %0, [%1];" : "=r"(v) : "l"(p) : "memory");
@@ -48,7 +53,8 @@ __global__ void __launch_bounds__(K2_WST, 1) integrate2_ws_kernel(const __grid_c
   const int N = P.N;
   const int NLr = GRP ? (N + GR - 1) / GR : N;
   const int k0 = crank * NLr;
-  const int T = blockDim.x, TC = T >> 1;                   // consumer threads = producer threads (whole warps)
+  // GRP: two helper warps behind the pairs (publisher, relay -- see below); blockDim = 2 TC + 64
+  const int T = blockDim.x, TC = (GRP ? T - 64 : T) >> 1;  // consumer threads = producer threads (whole warps)
   const int NW = TC >> 5;                                  // warp pairs
   // Which warp plays which role.  Warp w issues on scheduler w mod 4; a consumer carries ~3x the instructions of a producer.
   // Consumers take warps 0 .. 3, one per scheduler; with a fifth pair (cfg 4: 136 nodes) its consumer is warp 6, so that the
@@ -57,6 +63,8 @@ __global__ void __launch_bounds__(K2_WST, 1) integrate2_ws_kernel(const __grid_c
   bool prod; int wp;
   if (NW == 5) { prod = !(w < 4 || w == 6); wp = prod ? (w < 6 ? w - 4 : w - 5) : (w < 4 ? w : 4); }
   else { prod = w >= NW; wp = prod ? w - NW : w; }
+  const int helper = GRP && w >= 2 * NW ? w - 2 * NW + 1 : 0;      // 1 = publisher, 2 = relay
+  if (helper) wp = 0;
   const int tid = wp * 32 + ((int)threadIdx.x & 31);       // node slot: the same for the two warps of a pair
   const int NODES = min(NLr, N - k0) * SPC;
   const GroupDesc gd = P.groups[g];
@@ -67,9 +75,11 @@ __global__ void __launch_bounds__(K2_WST, 1) integrate2_ws_kernel(const __grid_c
   uint64_t* const bar_done = reinterpret_cast<uint64_t*>(smem_raw);
   uint64_t* const bar_full = bar_done + NBAR + (size_t)wp * 2;
   uint64_t* const bar_empty = bar_done + NBAR + (size_t)NW * 2 + (size_t)wp * 2;
-  float* const s_cpl = reinterpret_cast<float*>(bar_done + NBAR + (size_t)NW * 4) + tid;       // + b * GC * TC + i * TC
+  uint64_t* const bar_grp = bar_done + NBAR + (size_t)NW * 4;      // GRP: NBAR barriers "chunk w is in the ring, group-wide"
+  uint64_t* const bar_end = bar_grp + (GRP ? NBAR : 0);
+  float* const s_cpl = reinterpret_cast<float*>(bar_end) + tid;       // + b * GC * TC + i * TC
   float* const s_xi = s_cpl + (size_t)2 * GC * TC;
-  float2* s_ps = reinterpret_cast<float2*>(reinterpret_cast<float*>(bar_done + NBAR + (size_t)NW * 4) + (size_t)4 * GC * TC);
+  float2* s_ps = reinterpret_cast<float2*>(reinterpret_cast<float*>(bar_end) + (size_t)4 * GC * TC);
   unsigned char* tab = reinterpret_cast<unsigned char*>(s_ps + NP2 * SPC);
   tab += (16 - (reinterpret_cast<uintptr_t>(tab) & 15)) & 15;
   Edge<float>* const s_edges = reinterpret_cast<Edge<float>*>(tab);
@@ -85,6 +95,7 @@ __global__ void __launch_bounds__(K2_WST, 1) integrate2_ws_kernel(const __grid_c
     const int t = (int)threadIdx.x;
     if (t < NBAR) mbar_init(bar_done + t, (uint32_t)NW);
     if (t < NW * 4) mbar_init(bar_done + NBAR + t, 1u);
+    if (GRP && t < NBAR) mbar_init(bar_grp + t, 1u);
     for (int i = t; i < NP2 * SPC; i += T) s_ps[i] = P.psim2[(size_t)g * NP2 * SPC + i];
     for (int i = t; i < td.n_edges; i += T) s_edges[i] = g_edges[i];
     for (int i = t; i <= N; i += T) s_rowptr[i] = g_rowptr[i];
@@ -114,7 +125,32 @@ __global__ void __launch_bounds__(K2_WST, 1) integrate2_ws_kernel(const __grid_c
   const int64_t n0 = P.n_begin;
   const int c0 = (int)(n0 % Hp);
 
-  if (prod) {
+  if (helper) {
+    // ================= GRP helpers: the chunk hand-over between the CTAs of the group, off the consumers' chain =================
+    // publisher: when every local consumer has written chunk m (bar_done), one gpu-scope release-add on the group's counter of
+    //            slot m mod NBAR.  (Done by the consumers themselves, the release waits for their stores to reach L2 -- about
+    //            a microsecond per chunk on the chain that bounds the form.)
+    // relay:     polls that counter (relaxed loads, no L1 invalidation per poll) until all grp_arrivals CTAs have published
+    //            chunk w of this launch, takes one acquire, and completes the local barrier bar_grp the producers wait on.
+    // Causality: consumer stores -> arrive (release.cta) -> publisher wait (acquire.cta) -> red.release.gpu -> relay
+    // ld.acquire.gpu -> arrive (release.cta) -> producer wait (acquire.cta) -> ring loads through L2.
+    int64_t n = n0;
+    for (uint32_t m = 0; n < P.n_end; ++m, n += CH) {
+      const uint32_t slot = m & (NBAR - 1);
+      if (helper == 1) {
+        mbar_wait(bar_done + slot, (m / NBAR) & 1u);
+        if ((threadIdx.x & 31) == 0) grp_arrive(grp_cnt + slot);
+      } else {
+        const uint32_t want = (uint32_t)P.grp_arrivals * (m / NBAR + 1u);
+        if ((threadIdx.x & 31) == 0) {
+          while (grp_poll_relaxed(grp_cnt + slot) < want) {}
+          (void)grp_poll(grp_cnt + slot);
+          mbar_arrive(bar_grp + slot);
+        }
+        __syncwarp();
+      }
+    }
+  } else if (prod) {
     // ================= producer: coupling sums and normals of chunk m into buffer m & 1 =================
     int64_t n = n0;
     int c = c0;
@@ -126,13 +162,7 @@ __global__ void __launch_bounds__(K2_WST, 1) integrate2_ws_kernel(const __grid_c
       // for all of it, too little once the ring loads cross to another SM's writes through L2: GRP.)
       if (m >= (uint32_t)LAG) {                   // every consumer of the group has written chunk m - LAG
         const uint32_t w = m - (uint32_t)LAG;
-        if (GRP) {      // slot w mod NBAR has then collected grp_arrivals for each of the chunks w, w - NBAR, ... of this launch
-          const uint32_t* const cp = grp_cnt + (w & (NBAR - 1));
-          const uint32_t want = (uint32_t)P.grp_arrivals * (w / NBAR + 1u);
-          while (grp_poll(cp) < want) {}
-        } else {
-          mbar_wait(bar_done + (w & (NBAR - 1)), (w / NBAR) & 1u);
-        }
+        mbar_wait((GRP ? bar_grp : bar_done) + (w & (NBAR - 1)), (w / NBAR) & 1u);      // (GRP: signalled by the relay warp)
       }
       f2 acc[GC / 2];
 #pragma unroll
@@ -243,8 +273,7 @@ __global__ void __launch_bounds__(K2_WST, 1) integrate2_ws_kernel(const __grid_c
       }
       __syncwarp();
       if ((tid & 31) == 0) {
-        if (GRP) grp_arrive(grp_cnt + (m & (NBAR - 1)));      // chunk m is in the ring (release: visible to the other SMs' producers)
-        else mbar_arrive(bar_done + (m & (NBAR - 1)));
+        mbar_arrive(bar_done + (m & (NBAR - 1)));      // chunk m is in the ring (GRP: the publisher warp tells the other SMs)
         mbar_arrive(bar_empty + b);                    // buffer b may be refilled
       }
       n += ch;

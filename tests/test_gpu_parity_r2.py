@@ -219,7 +219,7 @@ def test_latency_form_is_chosen_for_small_sweeps_and_refused_where_it_does_not_a
     info = sw.launch_info()
     assert info["latency_form"] == 2                    # 256 sims: all CTAs resident, about one warp per scheduler
     # ... grouped: 7 simulations per 4 CTAs = 148 CTAs of 4 consumer warps, one per scheduler (the one-CTA mappings put two on one)
-    assert (info["ctas_per_group"], info["sims_per_cta"], info["ctas"], info["threads"]) == (4, 7, 148, 256)
+    assert (info["ctas_per_group"], info["sims_per_cta"], info["ctas"], info["threads"]) == (4, 7, 148, 320)
     cfg2 = wl.config(2)
     _, sw2 = tvbx.sweep_from_config(cfg2, W, L)
     sw2.run(10, 0.1, noise_on=True, ds=10)
