@@ -69,7 +69,9 @@ EXPORTS = [
     "tvbx_sweep_param", "tvbx_sweep_ext_id", "tvbx_delay_index", "tvbx_ring_len", "tvbx_steps_done",
     "tvbx_samples_kept", "tvbx_sweep_state", "tvbx_launch_info", "tvbx_launch_count", "tvbx_kernel_name", "tvbx_fc_kernel_name", "tvbx_last_error",
     "tvbx_version", "tvbx_trim_memory", "tvbx_sweep_reset", "tvbx_profile_enable", "tvbx_profile_read", "tvbx_bytes_copied", "tvbx_diag_tf_closed2",
+    "tvbx_top_k_noalloc",
 ]
+NOALLOC_MAX_SCORES = 1 << 20        # include/tvbx_noalloc.h TVBX_NOALLOC_MAX_SCORES
 
 
 def build(force: bool = False, verbose: bool = False, jobs: int = 0) -> str:
@@ -153,6 +155,7 @@ def lib():
             "tvbx_profile_read": [vp, dp, C.POINTER(i64)],
             "tvbx_bytes_copied": [vp, C.POINTER(i64), C.POINTER(i64)],
             "tvbx_diag_tf_closed2": [C.POINTER(ModelParams), i32, dp, dp, dp, dp, dp],
+            "tvbx_top_k_noalloc": [vp, i32, i32, vp, vp, vp],
         }
         for name, argtypes in sig.items():
             fn = getattr(L, name)
@@ -464,6 +467,21 @@ def diag_tf_closed2(fe, fi, w_e, w_i, params=None):
     out = np.zeros((n, 2, 7))
     _chk(lib().tvbx_diag_tf_closed2(C.byref(m) if m is not None else None, n, _dptr(fe), _dptr(fi), _dptr(w_e), _dptr(w_i), _dptr(out)))
     return out
+
+
+def top_k_noalloc(scores, k, out_idx, out_val, stream=None):
+    """tvbx_top_k_noalloc (include/tvbx_noalloc.h): the k largest of the float32 CUDA tensor `scores` [n], best first, ties to
+    the lower index, written to the caller's CUDA tensors out_idx (int32) and out_val (float32), both of >= min(k, n)
+    entries.  Allocates nothing and does not synchronise: one kernel on `stream`, scratch in a static device array of the
+    library (n <= NOALLOC_MAX_SCORES; calls that overlap on the GPU race on it).  Returns min(k, n)."""
+    import torch
+    n = int(scores.numel())
+    m = min(int(k), n)
+    assert scores.is_cuda and scores.dtype == torch.float32 and scores.is_contiguous()
+    assert out_idx.is_cuda and out_idx.dtype == torch.int32 and out_idx.is_contiguous() and out_idx.numel() >= m
+    assert out_val.is_cuda and out_val.dtype == torch.float32 and out_val.is_contiguous() and out_val.numel() >= m
+    _chk(lib().tvbx_top_k_noalloc(scores.data_ptr(), n, int(k), out_idx.data_ptr(), out_val.data_ptr(), _stream_ptr(stream)))
+    return m
 
 
 def trim_memory() -> int:

@@ -23,7 +23,7 @@ def _built():
 
 
 def _declared_symbols():
-    src = "".join(open(os.path.join(ROOT, "include", h)).read() for h in ("tvbx.h", "tvbx_diag.h"))
+    src = "".join(open(os.path.join(ROOT, "include", h)).read() for h in ("tvbx.h", "tvbx_diag.h", "tvbx_noalloc.h"))
     src = re.sub(r"/\*.*?\*/", "", src, flags=re.S)
     return sorted(set(re.findall(r"\b(tvbx_[a-z0-9_]+)\s*\(", src)))
 
