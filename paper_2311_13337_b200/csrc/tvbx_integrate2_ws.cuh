@@ -23,6 +23,7 @@
 
 namespace tvbx {
 
+enum { RELAY_POLL_NS = 2400, LAZY_WAIT_NS = 400 };      // GRP relay warp: poll period; producer / publisher warps: sleep between barrier tries
 enum { K2_WST = 320 };           // threads per CTA of this form (consumers + producers): 65536 / 320 -> 204 registers per thread
 
 // release-add on / acquire-load of a chunk counter in global memory (GRP: the CTAs of a group sit on different SMs)
@@ -38,6 +39,22 @@ __device__ __forceinline__ uint32_t grp_poll(const uint32_t* p) {
   uint32_t v;
   asm volatile("ld.acquire.gpu.global.u32 %0, [%1];" : "=r"(v) : "l"(p) : "memory");
   return v;
+}
+
+// wait of a HELPER-side warp (producer, publisher): between two failed tries the warp sleeps, so that it does not take
+// issue slots from the consumer warp on its scheduler (the consumer's own waits stay plain spins)
+__device__ __forceinline__ void mbar_wait_lazy(uint64_t* bar, uint32_t parity) {
+  uint32_t done;
+  for (;;) {
+    asm volatile(
+        "{\n"
+        ".reg .pred p;\n"
+        "mbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\n"
+        "selp.u32 %0, 1, 0, p;\n"
+        "}\n" : "=r"(done) : "r"(smem_u32(bar)), "r"(parity) : "memory");
+    if (done) break;
+    __nanosleep(LAZY_WAIT_NS);
+  }
 }
 
 template <int SPC, bool SRING, bool GRP = false>
@@ -138,12 +155,18 @@ __global__ void __launch_bounds__(K2_WST, 1) integrate2_ws_kernel(const __grid_c
     for (uint32_t m = 0; n < P.n_end; ++m, n += CH) {
       const uint32_t slot = m & (NBAR - 1);
       if (helper == 1) {
-        mbar_wait(bar_done + slot, (m / NBAR) & 1u);
+        mbar_wait_lazy(bar_done + slot, (m / NBAR) & 1u);
         if ((threadIdx.x & 31) == 0) grp_arrive(grp_cnt + slot);
       } else {
         const uint32_t want = (uint32_t)P.grp_arrivals * (m / NBAR + 1u);
         if ((threadIdx.x & 31) == 0) {
-          while (grp_poll_relaxed(grp_cnt + slot) < want) {}
+          // A slow poll, on purpose.  Measured on cfg 4 (chunk time of a consumer 4.9 us): spinning 2.84e10; a poll every
+          // 0.2 / 0.8 / 1.6 / 2.4 / 3.2 / 6.4 us -> 2.86 / 2.96 / 3.03 / 3.05 / 3.05 / 2.51e10.  Polling fast and then holding
+          // the hand-over back by 1.5 or 3 us gives 3.00e10 as well, sleeping first and then polling fast 2.86e10: what pays is
+          // that the producers start their gather LATER inside the LAG - 1 >= 1 chunks of slack they have (their loads and
+          // Philox draws then overlap the second half of the consumers' chunk instead of its start), not the saved issue
+          // slots.  The period must stay below the chunk time (8 steps of one consumer warp, ~0.5 us each in this form).
+          while (grp_poll_relaxed(grp_cnt + slot) < want) __nanosleep(RELAY_POLL_NS);
           (void)grp_poll(grp_cnt + slot);
           mbar_arrive(bar_grp + slot);
         }
@@ -162,7 +185,7 @@ __global__ void __launch_bounds__(K2_WST, 1) integrate2_ws_kernel(const __grid_c
       // for all of it, too little once the ring loads cross to another SM's writes through L2: GRP.)
       if (m >= (uint32_t)LAG) {                   // every consumer of the group has written chunk m - LAG
         const uint32_t w = m - (uint32_t)LAG;
-        mbar_wait((GRP ? bar_grp : bar_done) + (w & (NBAR - 1)), (w / NBAR) & 1u);      // (GRP: signalled by the relay warp)
+        mbar_wait_lazy((GRP ? bar_grp : bar_done) + (w & (NBAR - 1)), (w / NBAR) & 1u);      // (GRP: signalled by the relay warp)
       }
       f2 acc[GC / 2];
 #pragma unroll
@@ -192,7 +215,7 @@ __global__ void __launch_bounds__(K2_WST, 1) integrate2_ws_kernel(const __grid_c
           }
         }
       }
-      if (m >= 2) mbar_wait(bar_empty + b, ((m >> 1) - 1u) & 1u);                  // the consumer has finished chunk m - 2
+      if (m >= 2) mbar_wait_lazy(bar_empty + b, ((m >> 1) - 1u) & 1u);                  // the consumer has finished chunk m - 2
       float* const cpl = s_cpl + (size_t)b * GC * TC;
 #pragma unroll
       for (int j = 0; j < GC / 2; ++j) { cpl[(2 * j) * TC] = acc[j].x; cpl[(2 * j + 1) * TC] = acc[j].y; }
