@@ -158,79 +158,17 @@ int32_t tvbx_create_connectome(int32_t n, const double* W, const double* L_mm, t
 }
 int32_t tvbx_destroy_connectome(tvbx_connectome* c) { delete c; return TVBX_OK; }
 
-int32_t tvbx_sweep_create(const tvbx_connectome* c, const tvbx_model_params* defaults, int32_t n_axes,
-                          const tvbx_axis* axes, uint64_t seed, const tvbx_sweep_opts* opts, tvbx_sweep** out) {
-  if (!out) return fail(TVBX_EINVAL, "out is NULL");
-  *out = nullptr;
-  if (!c) return fail(TVBX_EINVAL, "connectome is NULL");
-  if (n_axes < 0 || n_axes > 16 || (n_axes > 0 && !axes)) return fail(TVBX_EINVAL, "bad axes");
-  std::unique_ptr<tvbx_sweep> sw(new (std::nothrow) tvbx_sweep());
-  if (!sw) return fail(TVBX_ENOMEM, "host allocation failed");
-  sw->conn = *c;
-  if (defaults) sw->defaults = *defaults; else default_params(&sw->defaults);
-  sw->seed = seed;
-  for (int a = 0; a < n_axes; ++a) {
-    const tvbx_axis& ax = axes[a];
-    if (ax.param_id < 0 || ax.param_id >= TVBX_N_SWEEPABLE) return fail(TVBX_EINVAL, "axis %d: parameter id %d is not sweepable", a, ax.param_id);
-    if (ax.n < 1) return fail(TVBX_EINVAL, "axis %d: n=%d", a, ax.n);
-    for (int b = 0; b < a; ++b) if (axes[b].param_id == ax.param_id) return fail(TVBX_EINVAL, "parameter id %d on two axes", ax.param_id);
-    Axis h; h.id = ax.param_id;
-    for (int i = 0; i < ax.n; ++i) {
-      const double val = ax.values ? ax.values[i] : axis_value(ax.lo, ax.hi, ax.n, i);
-      if (!std::isfinite(val)) return fail(TVBX_EINVAL, "axis %d: value %d not finite", a, i);
-      h.vals.push_back(val);
-    }
-    if (sw->grid_size > (int64_t)2147483647 / ax.n) return fail(TVBX_EINVAL, "grid larger than 2^31-1 simulations");
-    sw->grid_size *= ax.n;
-    sw->axes.push_back(std::move(h));
-  }
-  if (opts && opts->n_sims > 0) {
-    if (!opts->sim_ids) return fail(TVBX_EINVAL, "n_sims > 0 but sim_ids is NULL");
-    for (int64_t i = 0; i < opts->n_sims; ++i) {
-      if (opts->sim_ids[i] < 0 || opts->sim_ids[i] >= sw->grid_size) return fail(TVBX_EINVAL, "sim_ids[%lld]=%lld outside the grid", (long long)i, (long long)opts->sim_ids[i]);
-      sw->ext_ids.push_back(opts->sim_ids[i]);      // (< grid_size <= 2^31 - 1: fits the 32-bit Philox counter word of A12)
-    }
-  } else {
-    sw->ext_ids.resize(sw->grid_size);
-    for (int64_t i = 0; i < sw->grid_size; ++i) sw->ext_ids[i] = i;
-  }
-  sw->n_sims = (int64_t)sw->ext_ids.size();
-  sw->precision = opts ? opts->precision : TVBX_F32;
-  if (sw->precision != TVBX_F32 && sw->precision != TVBX_F64) return fail(TVBX_EINVAL, "precision=%d", sw->precision);
-  sw->threads_req = opts ? opts->threads_per_cta : 0;
-  sw->ws_req = opts ? opts->latency_form : 0;
-  if (sw->ws_req < 0 || sw->ws_req > 3) return fail(TVBX_EINVAL, "latency_form=%d (valid: 0 .. 3)", sw->ws_req);
-  sw->chunk_req = opts ? opts->chunk_samples : 0;
-  {
-    sw->stats_i = opts && opts->rate_stats_inhibitory != 0;
-    if (opts && opts->updown_threshold_khz != 0.0) {
-      if (!(opts->updown_threshold_khz > 0.0) || !std::isfinite(opts->updown_threshold_khz)) return fail(TVBX_EINVAL, "updown_threshold_khz=%g", opts->updown_threshold_khz);
-      sw->ud_thr = opts->updown_threshold_khz;
-    }
-    if (opts && opts->rate_threshold_khz != 0.0) {
-      if (!(opts->rate_threshold_khz > 0.0)) return fail(TVBX_EINVAL, "rate_threshold_khz=%g", opts->rate_threshold_khz);
-      sw->rate_thr = opts->rate_threshold_khz;
-    }
-    int fcm = opts ? opts->fc_mode : TVBX_FC_AUTO;
-    if (const char* e = getenv("TVBX_FC_MODE")) if (fcm == TVBX_FC_AUTO) fcm = atoi(e);
-    const bool tc_ok = sw->precision == TVBX_F32 && sw->conn.n <= kTcMaxN;
-    if (fcm < TVBX_FC_AUTO || fcm > TVBX_FC_TF32) return fail(TVBX_EINVAL, "fc_mode=%d", fcm);
-    if (fcm == TVBX_FC_TF32 && !tc_ok) return fail(TVBX_EINVAL, "fc_mode TVBX_FC_TF32 needs an FP32 sweep with N <= %d", kTcMaxN);
-    sw->fc_tc = tc_ok && fcm != TVBX_FC_FP32;
-  }
-  // parameter sanity
-  for (int64_t s = 0; s < sw->n_sims; ++s) {
-    if (!(sw->param(s, TVBX_P_V) > 0.0)) return fail(TVBX_EINVAL, "speed v must be > 0 (sim %lld)", (long long)s);
-    if (!(sw->param(s, TVBX_P_T) > 0.0) || !(sw->param(s, TVBX_P_TAU_W_E) > 0.0)) return fail(TVBX_EINVAL, "T and tau_w_e must be > 0 (sim %lld)", (long long)s);
-  }
+// The mapping of the sweep onto CTAs: simulations per CTA, CTAs per group, which integrator serves it, and the groups
+// themselves.  Run by tvbx_sweep_create; run AGAIN by the first tvbx_run with allow_wsg = false if the grouped low-latency
+// mapping was chosen and dt then shows that a delay table cannot run it (chunks shorter than 8 steps): the delays are only
+// known once dt is.
+static int32_t choose_mapping(tvbx_sweep* sw, bool allow_wsg) {
   const double* dp = sw->defaults.p;
-  if (!(dp[TVBX_P_TAU_W_I] > 0) || !(dp[TVBX_P_TAU_OU] > 0) || !(dp[TVBX_P_GL] > 0) || !(dp[TVBX_P_CM] > 0) ||
-      !(dp[TVBX_P_DMUV0] != 0) || !(dp[TVBX_P_DSV0] != 0) || !(dp[TVBX_P_DTVN0] != 0) || !(dp[TVBX_P_EPS_NU] > 0) ||
-      !(dp[TVBX_P_GINH] > 0 && dp[TVBX_P_GINH] < 1) || !(dp[TVBX_P_NTOT] > 0) || !(dp[TVBX_P_PCONN] > 0))
-    return fail(TVBX_EINVAL, "uniform model parameters out of range");
+  sw->wsg = false; sw->clu = 1;
+  sw->tables.clear(); sw->groups.clear(); sw->sim_table.clear(); sw->sim_slot.clear();
   // sims per CTA: any 1 .. floor(max threads / 2N).  Pick the count that minimises the number of
   // simulations the busiest SM has to integrate (148 SMs, CTAs of a sweep all resident or in waves).
-  int spc = opts ? opts->sims_per_cta : 0;
+  int spc = sw->spc_req;
   if (const char* e = getenv("TVBX_SPC")) if (spc == 0) spc = atoi(e);
   // the packed FP32 kernel (one thread per (sim, region), <= 480 of them, <= 8 simulations per CTA) serves
   // tau_e == tau_i and N <= 480; everything else runs the general kernel (two lanes per (sim, region))
@@ -244,7 +182,7 @@ int32_t tvbx_sweep_create(const tvbx_connectome* c, const tvbx_model_params* def
   // CTAs per group (thread-block cluster): the packed kernel can split the regions of a group over up to 8 CTAs.
   // Chosen when one CTA of <= 480 threads would hold fewer than 4 simulations (N > 120; cfg 5: N = 360 ->
   // 6 CTAs x 60 regions x 8 simulations): lanes that share a region then read whole sectors of the ring.
-  int clu = opts ? opts->ctas_per_group : 0;
+  int clu = sw->clu_req;
   if (const char* e = getenv("TVBX_CLUSTER")) if (clu == 0) clu = atoi(e);
   if (clu < 0 || clu > 8) return fail(TVBX_EINVAL, "ctas_per_group=%d (valid: 0..8)", clu);
   if (clu > 1 && sw->stats_i) return fail(TVBX_EINVAL, "rate_stats_inhibitory needs ctas_per_group <= 1");
@@ -274,7 +212,7 @@ int32_t tvbx_sweep_create(const tvbx_connectome* c, const tvbx_model_params* def
   // two CTAs of 3).  Splitting the regions of s simulations over c CTAs with <= 128 nodes each leaves one per scheduler if
   // the c * groups CTAs fit the SMs at once.  Taken by latency_form = 0 when no one-CTA mapping achieves that, and by 3.
   if (packed_ok && !sw->stats_i && sw->threads_req == 0 &&
-      (sw->ws_req == 3 || (sw->ws_req == 0 && clu == 0 && spc == 0 && getenv("TVBX_NO_WS") == nullptr && getenv("TVBX_NO_WSG") == nullptr))) {
+      allow_wsg && (sw->ws_req == 3 || (sw->ws_req == 0 && clu == 0 && spc == 0 && getenv("TVBX_NO_WS") == nullptr && getenv("TVBX_NO_WSG") == nullptr))) {
     const int n_sm = 148;
     std::map<double, int64_t> per_v;
     for (int64_t s = 0; s < sw->n_sims; ++s) per_v[sw->param(s, TVBX_P_V)]++;
@@ -362,6 +300,85 @@ int32_t tvbx_sweep_create(const tvbx_connectome* c, const tvbx_model_params* def
       sw->groups.push_back(std::move(g));
     }
   }
+  return TVBX_OK;
+}
+
+int32_t tvbx_sweep_create(const tvbx_connectome* c, const tvbx_model_params* defaults, int32_t n_axes,
+                          const tvbx_axis* axes, uint64_t seed, const tvbx_sweep_opts* opts, tvbx_sweep** out) {
+  if (!out) return fail(TVBX_EINVAL, "out is NULL");
+  *out = nullptr;
+  if (!c) return fail(TVBX_EINVAL, "connectome is NULL");
+  if (n_axes < 0 || n_axes > 16 || (n_axes > 0 && !axes)) return fail(TVBX_EINVAL, "bad axes");
+  std::unique_ptr<tvbx_sweep> sw(new (std::nothrow) tvbx_sweep());
+  if (!sw) return fail(TVBX_ENOMEM, "host allocation failed");
+  sw->conn = *c;
+  if (defaults) sw->defaults = *defaults; else default_params(&sw->defaults);
+  sw->seed = seed;
+  for (int a = 0; a < n_axes; ++a) {
+    const tvbx_axis& ax = axes[a];
+    if (ax.param_id < 0 || ax.param_id >= TVBX_N_SWEEPABLE) return fail(TVBX_EINVAL, "axis %d: parameter id %d is not sweepable", a, ax.param_id);
+    if (ax.n < 1) return fail(TVBX_EINVAL, "axis %d: n=%d", a, ax.n);
+    for (int b = 0; b < a; ++b) if (axes[b].param_id == ax.param_id) return fail(TVBX_EINVAL, "parameter id %d on two axes", ax.param_id);
+    Axis h; h.id = ax.param_id;
+    for (int i = 0; i < ax.n; ++i) {
+      const double val = ax.values ? ax.values[i] : axis_value(ax.lo, ax.hi, ax.n, i);
+      if (!std::isfinite(val)) return fail(TVBX_EINVAL, "axis %d: value %d not finite", a, i);
+      h.vals.push_back(val);
+    }
+    if (sw->grid_size > (int64_t)2147483647 / ax.n) return fail(TVBX_EINVAL, "grid larger than 2^31-1 simulations");
+    sw->grid_size *= ax.n;
+    sw->axes.push_back(std::move(h));
+  }
+  if (opts && opts->n_sims > 0) {
+    if (!opts->sim_ids) return fail(TVBX_EINVAL, "n_sims > 0 but sim_ids is NULL");
+    for (int64_t i = 0; i < opts->n_sims; ++i) {
+      if (opts->sim_ids[i] < 0 || opts->sim_ids[i] >= sw->grid_size) return fail(TVBX_EINVAL, "sim_ids[%lld]=%lld outside the grid", (long long)i, (long long)opts->sim_ids[i]);
+      sw->ext_ids.push_back(opts->sim_ids[i]);      // (< grid_size <= 2^31 - 1: fits the 32-bit Philox counter word of A12)
+    }
+  } else {
+    sw->ext_ids.resize(sw->grid_size);
+    for (int64_t i = 0; i < sw->grid_size; ++i) sw->ext_ids[i] = i;
+  }
+  sw->n_sims = (int64_t)sw->ext_ids.size();
+  sw->precision = opts ? opts->precision : TVBX_F32;
+  if (sw->precision != TVBX_F32 && sw->precision != TVBX_F64) return fail(TVBX_EINVAL, "precision=%d", sw->precision);
+  sw->threads_req = opts ? opts->threads_per_cta : 0;
+  sw->ws_req = opts ? opts->latency_form : 0;
+  if (sw->ws_req < 0 || sw->ws_req > 3) return fail(TVBX_EINVAL, "latency_form=%d (valid: 0 .. 3)", sw->ws_req);
+  sw->chunk_req = opts ? opts->chunk_samples : 0;
+  {
+    sw->stats_i = opts && opts->rate_stats_inhibitory != 0;
+    if (opts && opts->updown_threshold_khz != 0.0) {
+      if (!(opts->updown_threshold_khz > 0.0) || !std::isfinite(opts->updown_threshold_khz)) return fail(TVBX_EINVAL, "updown_threshold_khz=%g", opts->updown_threshold_khz);
+      sw->ud_thr = opts->updown_threshold_khz;
+    }
+    if (opts && opts->rate_threshold_khz != 0.0) {
+      if (!(opts->rate_threshold_khz > 0.0)) return fail(TVBX_EINVAL, "rate_threshold_khz=%g", opts->rate_threshold_khz);
+      sw->rate_thr = opts->rate_threshold_khz;
+    }
+    int fcm = opts ? opts->fc_mode : TVBX_FC_AUTO;
+    if (const char* e = getenv("TVBX_FC_MODE")) if (fcm == TVBX_FC_AUTO) fcm = atoi(e);
+    const bool tc_ok = sw->precision == TVBX_F32 && sw->conn.n <= kTcMaxN;
+    if (fcm < TVBX_FC_AUTO || fcm > TVBX_FC_TF32) return fail(TVBX_EINVAL, "fc_mode=%d", fcm);
+    if (fcm == TVBX_FC_TF32 && !tc_ok) return fail(TVBX_EINVAL, "fc_mode TVBX_FC_TF32 needs an FP32 sweep with N <= %d", kTcMaxN);
+    sw->fc_tc = tc_ok && fcm != TVBX_FC_FP32;
+  }
+  // parameter sanity
+  for (int64_t s = 0; s < sw->n_sims; ++s) {
+    if (!(sw->param(s, TVBX_P_V) > 0.0)) return fail(TVBX_EINVAL, "speed v must be > 0 (sim %lld)", (long long)s);
+    if (!(sw->param(s, TVBX_P_T) > 0.0) || !(sw->param(s, TVBX_P_TAU_W_E) > 0.0)) return fail(TVBX_EINVAL, "T and tau_w_e must be > 0 (sim %lld)", (long long)s);
+  }
+  const double* dp = sw->defaults.p;
+  if (!(dp[TVBX_P_TAU_W_I] > 0) || !(dp[TVBX_P_TAU_OU] > 0) || !(dp[TVBX_P_GL] > 0) || !(dp[TVBX_P_CM] > 0) ||
+      !(dp[TVBX_P_DMUV0] != 0) || !(dp[TVBX_P_DSV0] != 0) || !(dp[TVBX_P_DTVN0] != 0) || !(dp[TVBX_P_EPS_NU] > 0) ||
+      !(dp[TVBX_P_GINH] > 0 && dp[TVBX_P_GINH] < 1) || !(dp[TVBX_P_NTOT] > 0) || !(dp[TVBX_P_PCONN] > 0))
+    return fail(TVBX_EINVAL, "uniform model parameters out of range");
+  sw->spc_req = opts ? opts->sims_per_cta : 0;
+  sw->clu_req = opts ? opts->ctas_per_group : 0;
+  {
+    int32_t rc = choose_mapping(sw.get(), true);
+    if (rc) return rc;
+  }
   *out = sw.release();
   return TVBX_OK;
 }
@@ -388,6 +405,23 @@ int32_t tvbx_run(tvbx_sweep* sw, int64_t steps, double dt, const tvbx_run_opts* 
     int ndev = 0;
     if (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev == 0) { cudaGetLastError(); return fail(TVBX_ECUDA, "no CUDA device"); }
     CU(cudaGetDevice(&sw->device));
+    if (sw->wsg) {      // the grouped low-latency mapping needs 8-step chunks in every delay table: known only now, with dt
+      bool ok = true;
+      for (const HostTable& ht : sw->tables) {
+        int32_t D = 0, dmin = INT32_MAX;
+        for (const HostEdge& e : sw->conn.edges) {
+          const int32_t d = delay_steps(e.L, ht.v, dt);
+          D = std::max(D, d); dmin = std::min(dmin, d);
+        }
+        if (sw->conn.edges.empty()) dmin = kGC;
+        ok = ok && ring_geom(D, dmin, true).CH == kGC;
+      }
+      if (!ok) {
+        if (sw->ws_req == 3) return fail(TVBX_EINVAL, "latency_form = 3 needs 8-step chunks (minimum delay >= 15 steps)");
+        int32_t rc = choose_mapping(sw, false);      // the mapping the sweep would have got without the grouped form
+        if (rc) return rc;
+      }
+    }
     sw->dev.reset(make_device_side(sw));
     if (!sw->dev) return fail(TVBX_ENOMEM, "host allocation failed");
     int32_t rc = sw->dev->start(dt);

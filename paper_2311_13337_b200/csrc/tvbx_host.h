@@ -172,6 +172,7 @@ struct tvbx_sweep {
   std::vector<int64_t> ext_ids;
   uint64_t seed = 0;
   int32_t precision = TVBX_F32, spc = 8, threads_req = 0;
+  int32_t spc_req = 0, clu_req = 0;   // tvbx_sweep_opts.sims_per_cta / ctas_per_group as requested (0 = choose)
   int32_t clu = 1;        // CTAs (one thread-block cluster) per group: the regions are split over them
   bool vec_ok = false;    // cluster form with 4 or 8 simulations per group: vector gather where the chunk length allows
   bool packed = false;    // FP32 closed-form product kernel (integrate2_kernel)

@@ -211,6 +211,48 @@ def test_grouped_latency_form_is_bitwise_the_throughput_form(N, n_sims, spc, clu
         np.testing.assert_array_equal(a, b)
 
 
+def test_grouped_latency_form_under_concurrent_launches_and_its_fallback():
+    """(a) Two sweeps in the grouped form (cooperative launches, each wants the whole GPU) enqueued on two streams at once:
+    the launches must serialise, not deadlock, and give the results of a run on its own.  (b) The grouped mapping is chosen
+    at tvbx_sweep_create, before dt is known; if the delays then turn out too short for 8-step chunks, the first tvbx_run
+    falls back to the mapping the sweep would have had without it -- bit-identical to latency_form = 1."""
+    import torch
+    cfg = wl.config(4)
+    W, L = wl.config_connectome(cfg)
+    kw = dict(noise_on=True, ds=10, discard_steps=200)
+
+    def one(stream=None):
+        _, sw = tvbx.sweep_from_config(cfg, W, L, chunk_samples=64)
+        return sw
+    ref = one(); ref.run(1500, 0.1, **kw)
+    assert ref.launch_info()["ctas_per_group"] == 4
+    want = ref.fc_readout() + ref.state()
+    a, b = one(), one()
+    s1, s2 = torch.cuda.Stream(), torch.cuda.Stream()
+    for part in (700, 800):
+        a.run(part, 0.1, stream=s1, **kw)
+        b.run(part, 0.1, stream=s2, **kw)
+    torch.cuda.synchronize()
+    for sw in (a, b):
+        for x, y in zip(sw.fc_readout() + sw.state(), want):
+            np.testing.assert_array_equal(x, y)
+    # (b) 40 simulations at v = 60 m/s: minimum delay 2 steps -> one-step chunks
+    cfgf = dict(axes=[dict(name="G", lo=0.0, hi=0.4, n=40, values=None)], fixed=dict(v=60.0, wNoise=1e-4), seed=3)
+    outs = []
+    for form in (0, 1):
+        _, sw = tvbx.sweep_from_config(cfgf, W, L, latency_form=form, chunk_samples=40)
+        sw.run(900, 0.1, **kw)
+        info = sw.launch_info()
+        assert info["ctas_per_group"] == 1 and info["latency_form"] == 1
+        outs.append((info["sims_per_cta"], sw.fc_readout() + sw.state()))
+    assert outs[0][0] == outs[1][0]
+    for x, y in zip(outs[0][1], outs[1][1]):
+        np.testing.assert_array_equal(x, y)
+    _, sw3 = tvbx.sweep_from_config(cfgf, W, L, latency_form=3)
+    with pytest.raises(tvbx.TvbxError):
+        sw3.run(10, 0.1, **kw)
+
+
 def test_latency_form_is_chosen_for_small_sweeps_and_refused_where_it_does_not_apply():
     cfg = wl.config(4)
     W, L = wl.config_connectome(cfg)
