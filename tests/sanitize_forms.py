@@ -59,6 +59,9 @@ def main():
     form("general kernel FP64 mode", 20, 4.0, precision=tvbx.TVBX_F64, expect=G)
     form("general kernel, tau_e != tau_i (jets)", 20, 4.0, params=dict(tau_i=7.5), expect=G)
     form("ring in shared memory for the whole launch (small CTA, 8-slot chunks)", 30, 8.0, n_sims=2, sims_per_cta=1, expect=P2)
+    form("low-latency warp pairs, one CTA per group", 40, 4.0, n_sims=4, sims_per_cta=2, latency_form=2, expect=P2)
+    form("one-step chunks, fully mirrored ring in shared memory", 40, 300.0, expect=P2)
+    form("grouped low-latency form: 3 CTAs per group, cooperative launch", 37, 4.0, n_sims=7, sims_per_cta=3, ctas_per_group=3, latency_form=3, expect=P2)
     form("FC register tiles", 33, 4.0, fc_mode=tvbx.TVBX_FC_FP32, expect=P2)
     form("FC tensor cores, two row blocks", 130, 4.0, keep=0.2, n_sims=2, sims_per_cta=2, expect=P2)
     print("all forms ok", flush=True)
