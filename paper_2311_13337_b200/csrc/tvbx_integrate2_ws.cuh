@@ -18,6 +18,14 @@
 // ascending order into each slot) and the Philox stream are those of integrate2_kernel: results are bit-identical.
 // One CTA per group, delay table in shared memory, chunks of 8 steps (minimum delay >= 15 steps); SRING: the group's ring
 // in shared memory for the launch (cfg 1).
+//
+// GRP (the grouped form, cfg 4): the unit of this form's speed is ONE consumer warp per warp
+// scheduler, and no one-CTA mapping of a few hundred simulations gives that (cfg 4: 2 x 68 nodes = 5 warps per SM).  So the
+// REGIONS of a group are split over P.grp_ctas CTAs (cfg 4: 7 simulations x 17 regions per CTA, 4 CTAs per group, 148 CTAs
+// of 4 pairs).  The CTAs of a group sit on different SMs and wait on one another: cooperative launch (all resident), ring in
+// global memory read through L2, chunk hand-over through counters in global memory.  Two helper warps per CTA keep that
+// hand-over off the pairs: the publisher (release-add when all local consumers have written a chunk) and the relay (polls
+// until every CTA of the group has, then completes the local barrier the producers wait on).  Still bit-identical.
 #pragma once
 #include "tvbx_integrate2.cuh"
 
