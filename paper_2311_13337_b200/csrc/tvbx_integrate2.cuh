@@ -639,8 +639,11 @@ __global__ void __launch_bounds__(MAXT, 1) integrate2_kernel(const __grid_consta
     const int cpl_row0 = VEC ? (int)(((n >> 3) & 1) * GC + (n & 7)) : 0;      // VEC: the block's row, from the chunk's position in it
     const float* cpl_p = s_cpl + cpl_row0 * T;    // running pointers into the thread's private columns (one add per step
     const float* xi_p = s_xi;                     // instead of the row index times the runtime column stride)
-#pragma unroll 2      // two steps per trip: the address arithmetic and parameter loads of step i + 1 overlap the
-                      // arithmetic of step i and the rematerialised per-thread constants are shared (cfg 2 +2.8 %; 4 is slower)
+    // Steps per trip of the loop: 2 let the address arithmetic and parameter loads of step i + 1 overlap the arithmetic of
+    // step i (round 1: cfg 2 +2.8 %; 4 is slower); after round 2's trimming of the loop 1 is ahead again on the one-CTA
+    // forms (cfg 2 +1.0 %, cfg 3 +0.5 %), 2 stays ahead with the vector gather (cfg 5 +0.5 %).
+    constexpr int STEP_UNROLL = VEC ? 2 : 1;
+#pragma unroll STEP_UNROLL
     for (int i = 0; i < ch; ++i) {
       if (GCE == 1 && m + (uint32_t)i >= (uint32_t)LAG) wait_chunk(m + (uint32_t)i - (uint32_t)LAG);
       const float cpl = GCE == 1 ? gather_short(c) : *cpl_p;
