@@ -31,7 +31,7 @@ size_t DevPool::capacity() {
 }
 static size_t trim_locked(DevPool& P) {
   size_t freed = P.cached;
-  for (auto& kv : P.free_) { DeviceGuard guard(kv.first.first); cudaFree(kv.second); }
+  for (auto& kv : P.free_) { DeviceGuard guard(kv.first.first); cudaFree(kv.second); P.mem_[kv.first.first].delta -= (long long)kv.first.second; }
   P.free_.clear(); P.cached = 0;
   return freed;
 }
@@ -46,11 +46,30 @@ cudaError_t DevPool::get(void** p, size_t bytes, int* device) {
   if (it != free_.end()) { *p = it->second; cached -= bytes; free_.erase(it); return cudaSuccess; }
   e = cudaMalloc(p, bytes);
   if (e != cudaSuccess && cached > 0) { cudaGetLastError(); trim_locked(*this); e = cudaMalloc(p, bytes); }
+  if (e == cudaSuccess) mem_[dev].delta += (long long)bytes;
+  else mem_[dev].t_ms = -1e300;      // (the figure was wrong: ask again next time)
   return e;
+}
+cudaError_t DevPool::mem_info(size_t* free_b, size_t* total_b) {
+  int dev = 0;
+  cudaError_t e = cudaGetDevice(&dev);
+  if (e != cudaSuccess) return e;
+  std::lock_guard<std::mutex> g(mu);
+  MemInfo& m = mem_[dev];
+  const double now = std::chrono::duration<double, std::milli>(std::chrono::steady_clock::now().time_since_epoch()).count();
+  if (now - m.t_ms > kMemInfoTtlMs) {
+    e = cudaMemGetInfo(&m.free_b, &m.total_b);
+    if (e != cudaSuccess) return e;
+    m.t_ms = now; m.delta = 0;
+  }
+  const long long f = (long long)m.free_b - m.delta;
+  *free_b = (size_t)std::max<long long>(f, 0);
+  *total_b = m.total_b;
+  return cudaSuccess;
 }
 void DevPool::put(void* p, size_t bytes, int device) {
   std::lock_guard<std::mutex> g(mu);
-  if (cached + bytes > capacity()) { DeviceGuard guard(device); cudaFree(p); return; }
+  if (cached + bytes > capacity()) { DeviceGuard guard(device); cudaFree(p); mem_[device].delta -= (long long)bytes; return; }
   free_.insert({{device, bytes}, p}); cached += bytes;
 }
 size_t DevPool::cached_bytes() { std::lock_guard<std::mutex> g(mu); return cached; }

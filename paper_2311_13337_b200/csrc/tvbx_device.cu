@@ -234,7 +234,7 @@ struct DeviceImpl : DeviceSide {
     // ---- memory budget ----
     const size_t row = (size_t)N * SPC;
     size_t free_b = 0, total_b = 0;
-    CU(cudaMemGetInfo(&free_b, &total_b));
+    CU(dev_pool().mem_info(&free_b, &total_b));      // (cached: cudaMemGetInfo itself can take tens of ms, tvbx_host.h)
     free_b += dev_pool().cached_bytes();           // pooled buffers are reusable (or trimmed on demand)
     int64_t CS = sw->chunk_req;
     if (CS <= 0) {

@@ -8,6 +8,7 @@
 #include <cuda_runtime.h>
 
 #include <algorithm>
+#include <chrono>
 #include <cmath>
 #include <cstdint>
 #include <cstdlib>
@@ -103,7 +104,16 @@ struct DevPool {
   cudaError_t get(void** p, size_t bytes, int* device);
   void put(void* p, size_t bytes, int device);     // the caller has made sure no kernel still uses p
   size_t cached_bytes();
+  // Free / total memory of the current device as the library knows it.  cudaMemGetInfo is a driver round trip that now
+  // and then takes tens of milliseconds (measured: up to 80 ms inside the first tvbx_run of a sweep, on an idle GPU), so
+  // it is asked at most once per kMemInfoTtlMs per device; in between the answer is corrected by the pool's own cudaMalloc /
+  // cudaFree.  Allocations by others inside that window are not seen: a sweep sized on a stale figure fails in cudaMalloc
+  // with TVBX_ENOMEM (which refreshes the figure) instead of in the budget check.
+  struct MemInfo { double t_ms = -1e300; size_t free_b = 0, total_b = 0; long long delta = 0; };
+  std::map<int, MemInfo> mem_;
+  cudaError_t mem_info(size_t* free_b, size_t* total_b);
 };
+constexpr double kMemInfoTtlMs = 1000.0;
 DevPool& dev_pool();
 
 template <typename T>
