@@ -446,9 +446,15 @@ __global__ void __launch_bounds__(MAXT, 1) integrate2_kernel(const __grid_consta
   int sidx = P.sample_base;
 
   // S1, not pipelined: coupling sums of the chunk that starts at ring slot cur0 into this thread's column
+  // (unpipelined rounds stop at the row's last REAL edge: the zero-weight entries the host pads every row with -- to >= PVN,
+  // an odd count -- serve the pipelined batches only; a row of <= 24 edges otherwise paid a round of 8 edges x GCE loads per
+  // chunk for its 25th, empty entry: 8 of the 32 LDG per step of cfg 2)
+  int pe1t = pe1;
+  if (!VEC && GCE != 1)
+    while (pe1t > pe0 && (SMEMTAB ? s_edges[pe1t - 1].w : g_edges[pe1t - 1].w) == 0.0f) --pe1t;
   auto gather_from = [&](int e, int cur0, f2 acc[GC / 2]) {
-    if (SMEMTAB) gather_rounds<RS, GCE, RING_CG>(s_edges, e, pe1, e_last, ringg, cur0, Hp, acc);
-    else gather_rounds<RS, GCE, RING_CG>(g_edges, e, pe1, e_last, ringg, cur0, Hp, acc);
+    if (SMEMTAB) gather_rounds<RS, GCE, RING_CG>(s_edges, e, pe1t, e_last, ringg, cur0, Hp, acc);
+    else gather_rounds<RS, GCE, RING_CG>(g_edges, e, pe1t, e_last, ringg, cur0, Hp, acc);
   };
   // VEC: the row's seven segments (class 0 | classes 1-3 shifted | classes 1-3 near), ends relative to the staged part
   int seg[7] = {0, 0, 0, 0, 0, 0, 0};
